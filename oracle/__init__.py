@@ -1,0 +1,179 @@
+"""ORACLE — TEST INFRASTRUCTURE ONLY (see wm_oracle.cpp header).
+
+ctypes binding of the scalar C++ CPU oracle.  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this package; the product
+package never does.  Inputs/outputs are numpy arrays in the layouts of the paper's state
+definition as fixed by the C-ABI (time-major [B][T][A], roadgraph [B][R]).
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "wm_oracle.cpp")
+_LIB = os.path.join(_HERE, "libwm_oracle.so")
+
+DYN_BICYCLE = 0
+DYN_DELTA_LOCAL = 1
+BAND = 1e-4  # ambiguity band in metres (BASELINE.json north_star)
+
+TRAJ_F = ("x", "y", "yaw", "vel_x", "vel_y", "length", "width")
+RG_F = ("x", "y", "dir_x", "dir_y")
+
+
+def build(force=False):
+    """Compile wm_oracle.cpp -> libwm_oracle.so (g++ -O2, OpenMP over scenarios)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["g++", "-O2", "-fopenmp", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC",
+           "-o", _LIB, _SRC]
+    subprocess.check_call(cmd)
+    return _LIB
+
+
+class _Traj(C.Structure):
+    _fields_ = [("B", C.c_int32), ("A", C.c_int32), ("T", C.c_int32)] + \
+               [(k, C.c_void_p) for k in TRAJ_F] + [("valid", C.c_void_p)]
+
+
+class _Rg(C.Structure):
+    _fields_ = [("B", C.c_int32), ("R", C.c_int32)] + [(k, C.c_void_p) for k in RG_F] + \
+               [("type", C.c_void_p), ("id", C.c_void_p), ("valid", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_count_segments.restype = C.c_int32
+        _lib.orc_num_threads.restype = C.c_int32
+    return _lib
+
+
+def num_threads():
+    return int(lib().orc_num_threads())
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _check(a, dtype, shape):
+    assert a.dtype == dtype and a.flags["C_CONTIGUOUS"] and tuple(a.shape) == tuple(shape), \
+        (a.dtype, a.shape, dtype, shape)
+
+
+def _traj(tr):
+    B, T, A = tr["x"].shape
+    for k in TRAJ_F:
+        _check(tr[k], np.float32, (B, T, A))
+    _check(tr["valid"], np.uint8, (B, T, A))
+    s = _Traj(B, A, T, *[_p(tr[k]) for k in TRAJ_F], _p(tr["valid"]))
+    return s, (B, T, A)
+
+
+def _rg(rg):
+    B, R = rg["x"].shape
+    for k in RG_F:
+        _check(rg[k], np.float32, (B, R))
+    _check(rg["type"], np.int32, (B, R)); _check(rg["id"], np.int32, (B, R))
+    _check(rg["valid"], np.uint8, (B, R))
+    return _Rg(B, R, *[_p(rg[k]) for k in RG_F], _p(rg["type"]), _p(rg["id"]), _p(rg["valid"])), (B, R)
+
+
+def copy_traj(tr):
+    return {k: np.ascontiguousarray(v).copy() for k, v in tr.items()}
+
+
+def empty_like_traj(tr):
+    return {k: np.zeros_like(v) for k, v in tr.items()}
+
+
+def reset(log, history=11):
+    sim = empty_like_traj(log)
+    ls, _ = _traj(log); ss, _ = _traj(sim)
+    lib().orc_reset(C.byref(ls), C.byref(ss), C.c_int32(history))
+    return sim
+
+
+def step(log, sim, t, dynamics, action, action_valid, dt=0.1, max_accel=6.0, max_curvature=0.3):
+    """In place: writes sim row t+1. action [B][C][A] float32, action_valid [B][A] uint8."""
+    ls, (B, T, A) = _traj(log); ss, _ = _traj(sim)
+    Cn = 2 if dynamics == DYN_BICYCLE else 3
+    _check(action, np.float32, (B, Cn, A)); _check(action_valid, np.uint8, (B, A))
+    lib().orc_step(C.byref(ls), C.byref(ss), C.c_int32(t), C.c_int32(dynamics), C.c_double(dt),
+                   C.c_double(max_accel), C.c_double(max_curvature), _p(action), C.c_int64(Cn * A),
+                   _p(action_valid), C.c_int64(A))
+    return sim
+
+
+def overlap(sim, t, want_gap=True, want_pair=True):
+    ss, (B, T, A) = _traj(sim)
+    gap = np.empty((B, A, A), np.float64) if want_gap else None
+    pair = np.empty((B, A, A), np.uint8) if want_pair else None
+    flag = np.empty((B, A), np.uint8)
+    lib().orc_overlap(C.byref(ss), C.c_int32(t), _p(gap), _p(pair), _p(flag))
+    return dict(gap=gap, pair=pair, flag=flag)
+
+
+def offroad(sim, t, rg, band=BAND, details=True):
+    ss, (B, T, A) = _traj(sim); rs, _ = _rg(rg)
+    sd = np.empty((B, A), np.float32); flag = np.empty((B, A), np.uint8)
+    csd = np.empty((B, 4, A), np.float32) if details else None
+    amb = np.empty((B, 4, A), np.uint8) if details else None
+    win = np.empty((B, 4, A), np.int32) if details else None
+    lib().orc_offroad(C.byref(ss), C.c_int32(t), C.byref(rs), C.c_double(band), _p(sd), _p(csd),
+                      _p(flag), _p(amb), _p(win))
+    return dict(signed_dist=sd, corner_dist=csd, flag=flag, ambig=amb, win_seg=win)
+
+
+def count_segments(rg, b):
+    rs, _ = _rg(rg)
+    return int(lib().orc_count_segments(C.byref(rs), C.c_int32(b)))
+
+
+def log_divergence(log, sim, t):
+    ls, (B, T, A) = _traj(log); ss, _ = _traj(sim)
+    d = np.empty((B, A), np.float32); v = np.empty((B, A), np.uint8)
+    lib().orc_log_divergence(C.byref(ls), C.byref(ss), C.c_int32(t), _p(d), _p(v))
+    return dict(dist=d, valid=v)
+
+
+def observe_history(sim, t, H=11):
+    ss, (B, T, A) = _traj(sim)
+    hist = np.empty((B, A, H, 7, A), np.float32); hv = np.empty((B, A, H, A), np.uint8)
+    lib().orc_observe_history(C.byref(ss), C.c_int32(t), C.c_int32(H), _p(hist), _p(hv))
+    return dict(hist=hist, hist_valid=hv)
+
+
+def observe_topk(sim, rg, t, k):
+    ss, (B, T, A) = _traj(sim); rs, _ = _rg(rg)
+    idx = np.empty((B, A, k), np.int32); feat = np.empty((B, A, 4, k), np.float32)
+    typ = np.empty((B, A, k), np.int32); kth = np.empty((B, A), np.float32)
+    lib().orc_observe_topk(C.byref(ss), C.byref(rs), C.c_int32(t), C.c_int32(k), _p(idx), _p(feat),
+                           _p(typ), _p(kth))
+    return dict(rg_index=idx, rg_feat=feat, rg_type=typ, kth_key=kth)
+
+
+def rollout(log, sim, rg, t0, n_steps, dynamics, actions, action_valid, dt=0.1, max_accel=6.0,
+            max_curvature=0.3, band=BAND):
+    """In place on sim rows t0+1..t0+n_steps. actions [B][n_steps][C][A]."""
+    ls, (B, T, A) = _traj(log); ss, _ = _traj(sim); rs, _ = _rg(rg)
+    Cn = 2 if dynamics == DYN_BICYCLE else 3
+    _check(actions, np.float32, (B, n_steps, Cn, A)); _check(action_valid, np.uint8, (B, n_steps, A))
+    out = dict(overlap=np.empty((B, n_steps, A), np.uint8), offroad=np.empty((B, n_steps, A), np.uint8),
+               offroad_dist=np.empty((B, n_steps, A), np.float32), log_div=np.empty((B, n_steps, A), np.float32),
+               any_overlap=np.empty((B, A), np.uint8), any_offroad=np.empty((B, A), np.uint8),
+               ade=np.empty((B, A), np.float32))
+    lib().orc_rollout(C.byref(ls), C.byref(ss), C.byref(rs), C.c_int32(t0), C.c_int32(n_steps),
+                      C.c_int32(dynamics), C.c_double(dt), C.c_double(max_accel), C.c_double(max_curvature),
+                      _p(actions), _p(action_valid), C.c_double(band), _p(out["overlap"]), _p(out["offroad"]),
+                      _p(out["offroad_dist"]), _p(out["log_div"]), _p(out["any_overlap"]),
+                      _p(out["any_offroad"]), _p(out["ade"]))
+    return out

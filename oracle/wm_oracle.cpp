@@ -1,0 +1,472 @@
+// =====================================================================================
+// ORACLE — TEST INFRASTRUCTURE ONLY.  Not part of the product path.
+//
+// A plain, slow, scalar CPU restatement of what the Waymax closed-loop step computes
+// (arXiv 2310.08710; citations are PAPER.md line numbers + section/equation, and the
+// DESIGN.md reading numbers D1..D27 where the paper is silent).  Arithmetic is double
+// precision; inputs and outputs are the float32 / uint8 / int32 arrays the CUDA library
+// sees, and state is rounded to float32 at each step boundary.  It shares no code, header,
+// table or helper with paper_2310_08710_b200/csrc; only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may call it.
+//
+// Parity pins (tests/test_oracle_*.py): every function below is pinned by closed forms,
+// hand cases, brute force or invariants; none is "parity unpinned".
+//
+// The only loops that are parallel are `#pragma omp parallel for` over scenarios b
+// (scenarios are independent); nothing else is blocked, fused or
+// reordered.
+// =====================================================================================
+#include <algorithm>
+#include <cfloat>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" {
+
+struct orc_traj {            // [B][T][A] each, time-major
+  int32_t B, A, T;
+  float *x, *y, *yaw, *vel_x, *vel_y, *length, *width;
+  uint8_t* valid;
+};
+struct orc_roadgraph {       // [B][R] each
+  int32_t B, R;
+  float *x, *y, *dir_x, *dir_y;
+  int32_t *type, *id;
+  uint8_t* valid;
+};
+
+enum { ORC_DYN_BICYCLE = 0, ORC_DYN_DELTA_LOCAL = 1 };
+enum { ORC_TYPE_ROAD_EDGE = 2 };
+
+static inline size_t row(const orc_traj* tr, int b, int t) {
+  return ((size_t)b * tr->T + t) * tr->A;
+}
+
+// -------------------------------------------------------------------------------------
+// O1/O2 + D8/D9: one transition, row t -> row t+1.
+//   InvertibleBicycle: PAPER.md L339-L350 (Appendix A.1, Eq. 2), literal: the position uses
+//     the velocity components, the acceleration term uses the yaw.
+//   DeltaLocal: PAPER.md L324-L333 (Eq. 1) after rotating the body-frame delta by yaw (D2).
+//   Action clipping to +-max_accel / +-max_curvature when the limit is > 0 (D7; limits
+//     6 m/s^2, 0.3 1/m from L104).
+//   use_dyn = action_valid && sim.valid[t]; otherwise row t+1 <- log row t+1 (D8, L164).
+//   Controlled: valid'=1, length/width carried over (D9). No yaw wrapping (D5), no speed
+//   clamp (D6).
+// action: [B][C][A] with batch stride `act_stride_b` floats (C=2: a,kappa; C=3: dx,dy,dyaw).
+// -------------------------------------------------------------------------------------
+void orc_step(const orc_traj* log, orc_traj* sim, int32_t t, int32_t dynamics, double dt,
+              double max_accel, double max_curvature, const float* action,
+              int64_t act_stride_b, const uint8_t* action_valid, int64_t av_stride_b) {
+  const int B = sim->B, A = sim->A;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b) {
+    const size_t r0 = row(sim, b, t), r1 = row(sim, b, t + 1), l1 = row(log, b, t + 1);
+    const float* act = action + (size_t)b * act_stride_b;
+    const uint8_t* av = action_valid + (size_t)b * av_stride_b;
+    for (int a = 0; a < A; ++a) {
+      const bool use_dyn = av[a] != 0 && sim->valid[r0 + a] != 0;
+      if (!use_dyn) {
+        sim->x[r1 + a] = log->x[l1 + a];
+        sim->y[r1 + a] = log->y[l1 + a];
+        sim->yaw[r1 + a] = log->yaw[l1 + a];
+        sim->vel_x[r1 + a] = log->vel_x[l1 + a];
+        sim->vel_y[r1 + a] = log->vel_y[l1 + a];
+        sim->length[r1 + a] = log->length[l1 + a];
+        sim->width[r1 + a] = log->width[l1 + a];
+        sim->valid[r1 + a] = log->valid[l1 + a];
+        continue;
+      }
+      const double x = sim->x[r0 + a], y = sim->y[r0 + a], th = sim->yaw[r0 + a];
+      const double vx = sim->vel_x[r0 + a], vy = sim->vel_y[r0 + a];
+      double xn, yn, thn, vxn, vyn;
+      if (dynamics == ORC_DYN_BICYCLE) {
+        double acc = act[0 * A + a], kappa = act[1 * A + a];
+        if (max_accel > 0) acc = std::min(std::max(acc, -max_accel), max_accel);
+        if (max_curvature > 0) kappa = std::min(std::max(kappa, -max_curvature), max_curvature);
+        const double v = std::sqrt(vx * vx + vy * vy);
+        xn = x + vx * dt + 0.5 * acc * std::cos(th) * dt * dt;       // Eq. 2
+        yn = y + vy * dt + 0.5 * acc * std::sin(th) * dt * dt;       // L341
+        thn = th + kappa * (v * dt + 0.5 * acc * dt * dt);           // L343
+        const double vn = v + acc * dt;                              // L345
+        vxn = vn * std::cos(thn);                                    // L347
+        vyn = vn * std::sin(thn);                                    // L349
+      } else {
+        const double dx = act[0 * A + a], dy = act[1 * A + a], dyaw = act[2 * A + a];
+        const double c = std::cos(th), s = std::sin(th);
+        xn = x + c * dx - s * dy;                                    // Eq. 1, world delta
+        yn = y + s * dx + c * dy;                                    // L326
+        thn = th + dyaw;                                             // L328
+        // Eq. 1: v' = (x'-x)/dt, evaluated on the float32 state that is stored.
+        const double xs = (double)(float)xn, ys = (double)(float)yn;
+        vxn = (xs - x) / dt;
+        vyn = (ys - y) / dt;
+      }
+      sim->x[r1 + a] = (float)xn;
+      sim->y[r1 + a] = (float)yn;
+      sim->yaw[r1 + a] = (float)thn;
+      sim->vel_x[r1 + a] = (float)vxn;
+      sim->vel_y[r1 + a] = (float)vyn;
+      sim->length[r1 + a] = sim->length[r0 + a];
+      sim->width[r1 + a] = sim->width[r0 + a];
+      sim->valid[r1 + a] = 1;
+    }
+  }
+}
+
+// a0 (L122, L78): sim[0..history-1] <- log[0..history-1]; later rows invalid and zero.
+void orc_reset(const orc_traj* log, orc_traj* sim, int32_t history) {
+  const int B = sim->B, A = sim->A, T = sim->T;
+  for (int b = 0; b < B; ++b)
+    for (int t = 0; t < T; ++t) {
+      const size_t r = row(sim, b, t);
+      for (int a = 0; a < A; ++a) {
+        const bool c = t < history;
+        sim->x[r + a] = c ? log->x[r + a] : 0.f;
+        sim->y[r + a] = c ? log->y[r + a] : 0.f;
+        sim->yaw[r + a] = c ? log->yaw[r + a] : 0.f;
+        sim->vel_x[r + a] = c ? log->vel_x[r + a] : 0.f;
+        sim->vel_y[r + a] = c ? log->vel_y[r + a] : 0.f;
+        sim->length[r + a] = c ? log->length[r + a] : 0.f;
+        sim->width[r + a] = c ? log->width[r + a] : 0.f;
+        sim->valid[r + a] = c ? log->valid[r + a] : 0;
+      }
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O3 overlap (collision metric): two oriented rectangles intersect with
+// positive area iff no edge-normal axis separates them.
+//   gap(i,j) = max over the 4 edge normals u of |u.(c_j-c_i)| - (r_i(u)+r_j(u)),
+//   r(u) = (L/2)|u.f| + (W/2)|u.s|;  overlap = valid_i && valid_j && i!=j && gap<0 (D12,D13)
+// Outputs: gap [B][A][A] double (may be NULL; +inf where not evaluated), pair [B][A][A]
+// uint8 (may be NULL), flag [B][A] uint8 (row OR).
+// -------------------------------------------------------------------------------------
+void orc_overlap(const orc_traj* sim, int32_t t, double* gap, uint8_t* pair, uint8_t* flag) {
+  const int B = sim->B, A = sim->A;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b) {
+    const size_t r = row(sim, b, t);
+    for (int i = 0; i < A; ++i) {
+      uint8_t any = 0;
+      for (int j = 0; j < A; ++j) {
+        double g = INFINITY;
+        uint8_t ov = 0;
+        if (i != j && sim->valid[r + i] && sim->valid[r + j]) {
+          const double ci[2] = {sim->x[r + i], sim->y[r + i]}, cj[2] = {sim->x[r + j], sim->y[r + j]};
+          const double thi = sim->yaw[r + i], thj = sim->yaw[r + j];
+          const double fi[2] = {std::cos(thi), std::sin(thi)}, si[2] = {-std::sin(thi), std::cos(thi)};
+          const double fj[2] = {std::cos(thj), std::sin(thj)}, sj[2] = {-std::sin(thj), std::cos(thj)};
+          const double hli = 0.5 * sim->length[r + i], hwi = 0.5 * sim->width[r + i];
+          const double hlj = 0.5 * sim->length[r + j], hwj = 0.5 * sim->width[r + j];
+          const double d[2] = {cj[0] - ci[0], cj[1] - ci[1]};
+          const double* axes[4] = {fi, si, fj, sj};
+          g = -INFINITY;
+          for (int k = 0; k < 4; ++k) {
+            const double* u = axes[k];
+            const double ri = hli * std::fabs(u[0] * fi[0] + u[1] * fi[1]) + hwi * std::fabs(u[0] * si[0] + u[1] * si[1]);
+            const double rj = hlj * std::fabs(u[0] * fj[0] + u[1] * fj[1]) + hwj * std::fabs(u[0] * sj[0] + u[1] * sj[1]);
+            const double sep = std::fabs(u[0] * d[0] + u[1] * d[1]) - (ri + rj);
+            g = std::max(g, sep);
+          }
+          ov = g < 0.0;
+        }
+        if (gap) gap[((size_t)b * A + i) * A + j] = g;
+        if (pair) pair[((size_t)b * A + i) * A + j] = ov;
+        any |= ov;
+      }
+      flag[(size_t)b * A + i] = any;
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------
+// O4 offroad (readings D14-D20).
+// Segments: consecutive array entries (i,i+1), both valid, both ROAD_EDGE, same id; a valid
+// road-edge point that starts no segment and ends none is a zero-length segment.  The sign
+// direction is the segment vector e, or the stored dir when e = 0 (D16).
+// Per corner q (corner order: 0 front-left, 1 front-right, 2 rear-right, 3 rear-left):
+//   t* = clamp(((q-p0).e)/(e.e),0,1); closest = p0 | p1 | p0+t*e; d = |q-closest|;
+//   winner = min d, exact ties -> lower index (D17); side = e x (q-p0);
+//   sd = side>0 ? -d : +d (left of the oriented edge = on-road = negative).
+// Agent value = max over corners; flag = valid && sd_max > 0 (D18, D19).  No segments:
+// sd = -FLT_MAX, flag 0 (D20).  Invalid agents: outputs 0 (D10).
+// Ambiguity (P15) per corner: d < band, lateral |side|/|e| < band, or a segment of the
+// opposite sign within band of the winning distance.
+// Outputs: sd [B][A], corner_sd [B][4][A] (may be NULL), flag [B][A], ambig [B][4][A] (NULL ok),
+// win_seg [B][4][A] int32 = first-point index of the winning segment (NULL ok).
+// -------------------------------------------------------------------------------------
+struct OrcSeg { double p0x, p0y, p1x, p1y, sx, sy; int32_t src; };
+
+static void build_segments(const orc_roadgraph* rg, int b, std::vector<OrcSeg>& segs) {
+  const int R = rg->R;
+  const size_t o = (size_t)b * R;
+  segs.clear();
+  auto edge = [&](int i) { return rg->valid[o + i] != 0 && rg->type[o + i] == ORC_TYPE_ROAD_EDGE; };
+  auto starts = [&](int i) { return i + 1 < R && edge(i) && edge(i + 1) && rg->id[o + i] == rg->id[o + i + 1]; };
+  for (int i = 0; i < R; ++i) {
+    const bool s = starts(i);
+    const bool iso = edge(i) && !s && !(i > 0 && starts(i - 1));
+    if (!s && !iso) continue;
+    OrcSeg g;
+    g.p0x = rg->x[o + i]; g.p0y = rg->y[o + i];
+    if (s) { g.p1x = rg->x[o + i + 1]; g.p1y = rg->y[o + i + 1]; } else { g.p1x = g.p0x; g.p1y = g.p0y; }
+    const double ex = g.p1x - g.p0x, ey = g.p1y - g.p0y;
+    if (ex * ex + ey * ey > 0.0) { g.sx = ex; g.sy = ey; } else { g.sx = rg->dir_x[o + i]; g.sy = rg->dir_y[o + i]; }
+    g.src = i;
+    segs.push_back(g);
+  }
+}
+
+int32_t orc_count_segments(const orc_roadgraph* rg, int32_t b) {
+  std::vector<OrcSeg> segs; build_segments(rg, b, segs); return (int32_t)segs.size();
+}
+
+void orc_offroad(const orc_traj* sim, int32_t t, const orc_roadgraph* rg, double band, float* sd_out,
+                 float* corner_sd, uint8_t* flag, uint8_t* ambig, int32_t* win_seg) {
+  const int B = sim->B, A = sim->A;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int b = 0; b < B; ++b) {
+    std::vector<OrcSeg> segs;
+    build_segments(rg, b, segs);
+    const size_t r = row(sim, b, t);
+    for (int a = 0; a < A; ++a) {
+      const size_t oa = (size_t)b * A + a;
+      if (!sim->valid[r + a]) {
+        sd_out[oa] = 0.f; flag[oa] = 0;
+        for (int k = 0; k < 4; ++k) {
+          const size_t oc = ((size_t)b * 4 + k) * A + a;
+          if (corner_sd) corner_sd[oc] = 0.f;
+          if (ambig) ambig[oc] = 0;
+          if (win_seg) win_seg[oc] = -1;
+        }
+        continue;
+      }
+      const double cx = sim->x[r + a], cy = sim->y[r + a], th = sim->yaw[r + a];
+      const double hl = 0.5 * sim->length[r + a], hw = 0.5 * sim->width[r + a];
+      const double fx = std::cos(th), fy = std::sin(th), sx = -std::sin(th), sy = std::cos(th);
+      const double sl[4] = {+1, +1, -1, -1}, sw[4] = {+1, -1, -1, +1};  // FL, FR, RR, RL
+      double sd_max = -DBL_MAX;
+      for (int k = 0; k < 4; ++k) {
+        const double qx = cx + sl[k] * hl * fx + sw[k] * hw * sx;
+        const double qy = cy + sl[k] * hl * fy + sw[k] * hw * sy;
+        double best = INFINITY, best_side = 0, best_snorm = 1; int best_i = -1;
+        double best_pos = INFINITY, best_neg = INFINITY;   // min d among side>0 / side<=0 segments
+        for (size_t i = 0; i < segs.size(); ++i) {
+          const OrcSeg& g = segs[i];
+          const double ex = g.p1x - g.p0x, ey = g.p1y - g.p0y, ee = ex * ex + ey * ey;
+          const double wx = qx - g.p0x, wy = qy - g.p0y;
+          double px = g.p0x, py = g.p0y;
+          if (ee > 0.0) {
+            double ts = (wx * ex + wy * ey) / ee;
+            ts = std::min(std::max(ts, 0.0), 1.0);
+            if (ts <= 0.0) { px = g.p0x; py = g.p0y; }
+            else if (ts >= 1.0) { px = g.p1x; py = g.p1y; }
+            else { px = g.p0x + ts * ex; py = g.p0y + ts * ey; }
+          }
+          const double d = std::sqrt((qx - px) * (qx - px) + (qy - py) * (qy - py));
+          const double side = g.sx * wy - g.sy * wx;
+          if (side > 0) best_pos = std::min(best_pos, d); else best_neg = std::min(best_neg, d);
+          if (d < best) { best = d; best_side = side; best_snorm = std::sqrt(g.sx * g.sx + g.sy * g.sy); best_i = g.src; }
+        }
+        double sd; uint8_t amb = 0;
+        if (best_i < 0) { sd = -(double)FLT_MAX; }
+        else {
+          sd = best_side > 0 ? -best : best;
+          const double opp = best_side > 0 ? best_neg : best_pos;
+          const double lateral = best_snorm > 0 ? std::fabs(best_side) / best_snorm : 0.0;
+          amb = (best < band) || (lateral < band) || (opp - best < band);
+        }
+        const size_t oc = ((size_t)b * 4 + k) * A + a;
+        if (corner_sd) corner_sd[oc] = (float)sd;
+        if (ambig) ambig[oc] = amb;
+        if (win_seg) win_seg[oc] = best_i;
+        sd_max = std::max(sd_max, sd);
+      }
+      sd_out[oa] = (float)sd_max;
+      flag[oa] = sd_max > 0.0;
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------
+// O5 log divergence (displacement error): L2 distance between simulated and
+// logged XY at the same timestep; valid iff both valid, else 0.
+// -------------------------------------------------------------------------------------
+void orc_log_divergence(const orc_traj* log, const orc_traj* sim, int32_t t, float* dist, uint8_t* valid) {
+  const int B = sim->B, A = sim->A;
+  for (int b = 0; b < B; ++b) {
+    const size_t r = row(sim, b, t), l = row(log, b, t);
+    for (int a = 0; a < A; ++a) {
+      const bool v = sim->valid[r + a] && log->valid[l + a];
+      double d = 0;
+      if (v) {
+        const double dx = (double)sim->x[r + a] - log->x[l + a], dy = (double)sim->y[r + a] - log->y[l + a];
+        d = std::sqrt(dx * dx + dy * dy);
+      }
+      dist[(size_t)b * A + a] = (float)d;
+      valid[(size_t)b * A + a] = v;
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------
+// O6 observation, history part (D22): for each ego e valid at t and every
+// agent a, steps t-H+1..t: p' = R(-yaw_e)(p - p_e), yaw' = wrap(yaw - yaw_e) to [-pi,pi),
+// v' = R(-yaw_e) v, length/width copied; valid' = valid[a,h] && valid[e,t]; invalid -> 0.
+// hist [B][E][H][7][A] (x,y,yaw,vx,vy,length,width), hist_valid [B][E][H][A].
+// -------------------------------------------------------------------------------------
+static double wrap_pi(double a) {
+  const double two_pi = 2.0 * M_PI;
+  double w = std::fmod(a + M_PI, two_pi);
+  if (w < 0) w += two_pi;
+  return w - M_PI;
+}
+
+void orc_observe_history(const orc_traj* sim, int32_t t, int32_t H, float* hist, uint8_t* hist_valid) {
+  const int B = sim->B, A = sim->A;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b) {
+    const size_t rt = row(sim, b, t);
+    for (int e = 0; e < A; ++e) {
+      const bool ev = sim->valid[rt + e] != 0;
+      const double ex = ev ? sim->x[rt + e] : 0, ey = ev ? sim->y[rt + e] : 0, eth = ev ? sim->yaw[rt + e] : 0;
+      const double c = std::cos(eth), s = std::sin(eth);
+      for (int h = 0; h < H; ++h) {
+        const size_t rh = row(sim, b, t - H + 1 + h);
+        for (int a = 0; a < A; ++a) {
+          const bool v = ev && sim->valid[rh + a] != 0;
+          double o[7] = {0, 0, 0, 0, 0, 0, 0};
+          if (v) {
+            const double dx = sim->x[rh + a] - ex, dy = sim->y[rh + a] - ey;
+            o[0] = c * dx + s * dy;
+            o[1] = -s * dx + c * dy;
+            o[2] = wrap_pi((double)sim->yaw[rh + a] - eth);
+            const double vx = sim->vel_x[rh + a], vy = sim->vel_y[rh + a];
+            o[3] = c * vx + s * vy;
+            o[4] = -s * vx + c * vy;
+            o[5] = sim->length[rh + a];
+            o[6] = sim->width[rh + a];
+          }
+          const size_t base = ((((size_t)b * A + e) * H + h) * 7) * A + a;
+          for (int f = 0; f < 7; ++f) hist[base + (size_t)f * A] = (float)o[f];
+          hist_valid[(((size_t)b * A + e) * H + h) * A + a] = v;
+        }
+      }
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------
+// O7 observation, roadgraph part ("sub-samples the roadgraph via distance";
+// D23-D25): for each ego valid at t, the k valid roadgraph points nearest the ego centre,
+// ties -> lower index, emitted in ascending index order, padded with -1.
+// The integer decision (which points) is taken in float32, the kernel's precision:
+//   key = fma(dy, dy, dx*dx) with dx = fl(px-ex), dy = fl(py-ey), round-to-nearest
+// (DESIGN.md R-topk).  Features are computed in double: p' = R(-yaw_e)(p-p_e),
+// dir' = R(-yaw_e) dir.  Also returns kth_key [B][E] = float32 key of the k-th selected point
+// (NaN if fewer than k valid points) for the band report.
+// rg_index [B][E][k], rg_feat [B][E][4][k] (x,y,dir_x,dir_y), rg_type [B][E][k].
+// -------------------------------------------------------------------------------------
+void orc_observe_topk(const orc_traj* sim, const orc_roadgraph* rg, int32_t t, int32_t k,
+                      int32_t* rg_index, float* rg_feat, int32_t* rg_type, float* kth_key) {
+  const int B = sim->B, A = sim->A, R = rg->R;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int b = 0; b < B; ++b) {
+    const size_t rt = row(sim, b, t), o = (size_t)b * R;
+    std::vector<std::pair<float, int32_t>> keys;
+    std::vector<int32_t> sel;
+    for (int e = 0; e < A; ++e) {
+      int32_t* oi = rg_index + ((size_t)b * A + e) * k;
+      float* of = rg_feat + ((size_t)b * A + e) * 4 * k;
+      int32_t* ot = rg_type + ((size_t)b * A + e) * k;
+      for (int j = 0; j < k; ++j) { oi[j] = -1; ot[j] = 0; of[j] = of[k + j] = of[2 * k + j] = of[3 * k + j] = 0.f; }
+      if (kth_key) kth_key[(size_t)b * A + e] = NAN;
+      if (!sim->valid[rt + e]) continue;
+      const float exf = sim->x[rt + e], eyf = sim->y[rt + e];
+      keys.clear();
+      for (int i = 0; i < R; ++i) {
+        if (!rg->valid[o + i]) continue;
+        const float dx = rg->x[o + i] - exf, dy = rg->y[o + i] - eyf;
+        const float key = std::fmaf(dy, dy, dx * dx);
+        keys.emplace_back(key, i);
+      }
+      std::sort(keys.begin(), keys.end());      // lexicographic (key, index)
+      const int n = std::min<int>(k, (int)keys.size());
+      sel.clear();
+      for (int j = 0; j < n; ++j) sel.push_back(keys[j].second);
+      std::sort(sel.begin(), sel.end());        // ascending index (D24)
+      if (kth_key && (int)keys.size() >= k && k > 0) kth_key[(size_t)b * A + e] = keys[k - 1].first;
+      const double ex = exf, ey = eyf, eth = sim->yaw[rt + e];
+      const double c = std::cos(eth), s = std::sin(eth);
+      for (int j = 0; j < n; ++j) {
+        const int i = sel[j];
+        const double dx = rg->x[o + i] - ex, dy = rg->y[o + i] - ey;
+        const double ux = rg->dir_x[o + i], uy = rg->dir_y[o + i];
+        oi[j] = i;
+        of[0 * k + j] = (float)(c * dx + s * dy);
+        of[1 * k + j] = (float)(-s * dx + c * dy);
+        of[2 * k + j] = (float)(c * ux + s * uy);
+        of[3 * k + j] = (float)(-s * ux + c * uy);
+        ot[j] = rg->type[o + i];
+      }
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------
+// O8 rollout (D11, D21): n_steps x (O1/O2 -> O3, O4, O5 on row t+1).
+// Per-step rows [B][n_steps][A]; aggregates [B][A]: any-overlap, any-offroad,
+// ADE = sum of valid distances / count (0 if count 0).  actions [B][n_steps][C][A],
+// action_valid [B][n_steps][A].  Any output pointer may be NULL.
+// -------------------------------------------------------------------------------------
+void orc_rollout(const orc_traj* log, orc_traj* sim, const orc_roadgraph* rg, int32_t t0, int32_t n_steps,
+                 int32_t dynamics, double dt, double max_accel, double max_curvature,
+                 const float* actions, const uint8_t* action_valid, double band,
+                 uint8_t* overlap, uint8_t* offroad, float* offroad_dist, float* log_div,
+                 uint8_t* any_overlap, uint8_t* any_offroad, float* ade) {
+  const int B = sim->B, A = sim->A;
+  const int C = dynamics == ORC_DYN_BICYCLE ? 2 : 3;
+  const size_t BA = (size_t)B * A;
+  std::vector<uint8_t> f_ov(BA), f_off(BA), v_ld(BA);
+  std::vector<float> sd(BA), ld(BA);
+  std::vector<double> sum(BA, 0.0);
+  std::vector<int32_t> cnt(BA, 0);
+  if (any_overlap) std::memset(any_overlap, 0, BA);
+  if (any_offroad) std::memset(any_offroad, 0, BA);
+  for (int s = 0; s < n_steps; ++s) {
+    const int t = t0 + s;
+    orc_step(log, sim, t, dynamics, dt, max_accel, max_curvature, actions + (size_t)s * C * A,
+             (int64_t)n_steps * C * A, action_valid + (size_t)s * A, (int64_t)n_steps * A);
+    orc_overlap(sim, t + 1, nullptr, nullptr, f_ov.data());
+    orc_offroad(sim, t + 1, rg, band, sd.data(), nullptr, f_off.data(), nullptr, nullptr);
+    orc_log_divergence(log, sim, t + 1, ld.data(), v_ld.data());
+    for (int b = 0; b < B; ++b)
+      for (int a = 0; a < A; ++a) {
+        const size_t i = (size_t)b * A + a, o = ((size_t)b * n_steps + s) * A + a;
+        if (overlap) overlap[o] = f_ov[i];
+        if (offroad) offroad[o] = f_off[i];
+        if (offroad_dist) offroad_dist[o] = sd[i];
+        if (log_div) log_div[o] = ld[i];
+        if (any_overlap) any_overlap[i] |= f_ov[i];
+        if (any_offroad) any_offroad[i] |= f_off[i];
+        if (v_ld[i]) { sum[i] += ld[i]; cnt[i] += 1; }
+      }
+  }
+  if (ade)
+    for (size_t i = 0; i < BA; ++i) ade[i] = cnt[i] ? (float)(sum[i] / cnt[i]) : 0.f;
+}
+
+int32_t orc_num_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"
