@@ -1,0 +1,197 @@
+/*
+ * wm.h — C-ABI of the B200-native Waymax closed-loop step (arXiv 2310.08710).
+ *
+ * One thing is exported: the data-parallel hot path of the simulator — the batched
+ * closed-loop environment step over B scenarios x A agents — as hand-written sm_100a CUDA
+ * kernels.  Citations are PAPER.md line numbers (+ section / equation); "Dnn" are the
+ * readings listed in DESIGN.md where the paper is silent or ambiguous.
+ *
+ * Conventions
+ *  - Every function returns int: WM_OK (0) or a negative wm_status.  Nothing throws, aborts
+ *    or prints.  After WM_ERR_CUDA, wm_last_cuda_error() returns the cudaError_t.
+ *  - Unless a function says HOST, every data pointer is a DEVICE pointer owned by the
+ *    caller; the library owns only what hangs off wm_handle (prepared road-edge segments,
+ *    prepared roadgraph points, scratch, the instantiated CUDA graph, staging buffers).
+ *  - Work is enqueued on the caller's stream (`void* stream` = cudaStream_t; NULL = the
+ *    legacy default stream) and NOT synchronised, unless a function says it synchronises.
+ *  - Functions are pure in the paper's sense (L120): outputs depend only on the arguments,
+ *    repeated calls are bit-identical.
+ *  - Arrays are struct-of-arrays, innermost dimension contiguous, 16-byte aligned:
+ *      trajectories  [B][T][A]  (time-major rows of A agents; paper state L82, L322)
+ *      roadgraph     [B][R]
+ *      actions       [B][C][A]  (one step) or [B][n_steps][C][A] (rollout)
+ *  - Invalid slots (valid == 0) may hold anything, NaN included; they are never read for
+ *    arithmetic that reaches an output (D10).  Outputs for invalid agents are 0 / flag 0 /
+ *    index -1.
+ *  - Limits: 1 <= A <= 1024, 1 <= B, T >= 1, R >= 1, topk <= R, history <= T.
+ */
+#ifndef WM_H_
+#define WM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  WM_OK = 0,
+  WM_ERR_ARG = -1,          /* null / misaligned pointer, bad shape, t out of range */
+  WM_ERR_CUDA = -2,         /* a CUDA call failed; see wm_last_cuda_error() */
+  WM_ERR_UNSUPPORTED = -3,  /* e.g. A > 1024, topk > R */
+  WM_ERR_STATE = -4         /* e.g. metrics_offroad before wm_prepare */
+} wm_status;
+
+enum { WM_DYN_INVERTIBLE_BICYCLE = 0, WM_DYN_DELTA_LOCAL = 1 };
+enum { WM_TYPE_LANE = 1, WM_TYPE_ROAD_EDGE = 2 };
+
+/* Dynamic state, PAPER.md L82 / L322: s = (x, y, yaw, v_x, v_y) + box dims + validity,
+ * per agent and timestep.  Each pointer addresses [B][T][A]. */
+typedef struct {
+  int32_t B, A, T;
+  float *x, *y, *yaw, *vel_x, *vel_y, *length, *width;
+  uint8_t* valid;
+} wm_traj;
+
+/* Static roadgraph, PAPER.md L82 / L100: oriented points; z ignored (D27). [B][R] each. */
+typedef struct {
+  int32_t B, R;
+  float *x, *y, *dir_x, *dir_y;
+  int32_t *type, *id;
+  uint8_t* valid;
+} wm_roadgraph;
+
+typedef struct {
+  int32_t dynamics;     /* WM_DYN_* */
+  float dt;             /* 0.1 s (D1) */
+  float max_accel;      /* 6.0 m/s^2, L104; <= 0 disables clipping (D7) */
+  float max_curvature;  /* 0.3 1/m,  L104; <= 0 disables clipping (D7) */
+  int32_t history;      /* 11 steps: the first second of the log (L78) */
+  int32_t topk;         /* 1000 nearest roadgraph points per ego (D23) */
+} wm_config;
+
+typedef struct wm_handle wm_handle; /* opaque */
+
+/* Per-step metric rows [B][n_steps][A] and aggregates [B][A] of a rollout. Any pointer may be
+ * NULL (that output is skipped). ade = sum of valid log divergences / count (D21). */
+typedef struct {
+  uint8_t *overlap, *offroad;
+  float *offroad_dist, *log_div;
+  uint8_t *any_overlap, *any_offroad;
+  float* ade;
+} wm_rollout_out;
+
+/* Create / destroy a handle. `cfg` is copied. HOST pointers. wm_destroy synchronises. */
+int wm_create(wm_handle** out, const wm_config* cfg);
+int wm_destroy(wm_handle* h);
+int wm_last_cuda_error(void);
+/* Human-readable build tag, e.g. "wm_b200 sm_100a". HOST. */
+const char* wm_version(void);
+
+/*
+ * Static precompute at reset time (the roadgraph does not change during an episode, L82):
+ *  - road-edge segments for the offroad metric (L100; D14-D17): consecutive entries
+ *    (i, i+1) with both valid, both WM_TYPE_ROAD_EDGE and equal id form a segment; an
+ *    isolated valid road-edge point is a zero-length segment signed by its stored dir;
+ *  - a packed copy of the roadgraph points for the top-k observation (L82).
+ * Keeps pointers to nothing in `rg` (everything needed is copied); `rg` must match the B of
+ * later calls.  SYNCHRONISES the stream (it sizes its buffers from a device-side count).
+ * `n_segments_max` (HOST, may be NULL) receives max_b S_e(b).
+ */
+int wm_prepare(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, void* stream);
+
+/* reset(scenario), L122 / L78: sim rows [0, history) <- log rows; later rows are cleared
+ * (valid = 0, fields 0).  *t (HOST, may be NULL) receives history - 1. */
+int wm_reset(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t* t, void* stream);
+
+/*
+ * step(state, action), L123: writes row t+1 of `sim` from row t.
+ *  - WM_DYN_INVERTIBLE_BICYCLE, Appendix A.1 Eq. 2 (L339-L350), action (a, kappa), C = 2;
+ *  - WM_DYN_DELTA_LOCAL, Eq. 1 (L324-L333) on the body-frame delta (dx, dy, dyaw) rotated by
+ *    yaw_t (D2), C = 3.
+ * An agent is moved by the dynamics iff action_valid && sim.valid[t]; every other slot of
+ * row t+1 is copied from log row t+1, all 8 fields (log playback, L164; D8).  Controlled
+ * agents keep length/width and get valid = 1 (D9).  Actions are clipped to
+ * +-max_accel / +-max_curvature (D7).  Yaw is not wrapped (D5), speed is not clamped (D6).
+ * action [B][C][A]; action_valid [B][A]. Requires 0 <= t < T-1.
+ */
+int wm_step(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t, const float* action,
+            const uint8_t* action_valid, void* stream);
+
+/*
+ * Collision metric, L102: for every pair of valid agents at row t, do the oriented
+ * rectangles (centre x,y; length along yaw, width across) intersect with positive area
+ * (D12: touching is not overlap; D13: no self pairs).
+ * pair_bits [B][A][ceil(A/32)] uint32, bit j%32 of word j/32 of row i = overlap(i, j); may be
+ * NULL.  agent_flag [B][A] = OR_j overlap(i, j).
+ */
+int wm_metrics_overlap(wm_handle* h, const wm_traj* sim, int32_t t, uint32_t* pair_bits,
+                       uint8_t* agent_flag, void* stream);
+
+/*
+ * Off-road metric, L100: signed distance of each of the 4 box corners of every valid agent
+ * at row t to the nearest road-edge segment (prepared by wm_prepare); negative on the left
+ * of the oriented edge (on-road), positive on the right (D15-D17, D19).
+ * signed_dist [B][A] = max over the 4 corners (D18); corner_dist [B][4][A] (corner order:
+ * 0 front-left, 1 front-right, 2 rear-right, 3 rear-left), may be NULL; agent_flag [B][A] =
+ * valid && signed_dist > 0.  A scenario without road-edge segments gives -FLT_MAX, flag 0
+ * (D20).  Returns WM_ERR_STATE before wm_prepare.
+ */
+int wm_metrics_offroad(wm_handle* h, const wm_traj* sim, int32_t t, float* signed_dist,
+                       float* corner_dist, uint8_t* agent_flag, void* stream);
+
+/* Displacement error, L106: dist [B][A] = ||(x,y)_sim - (x,y)_log||_2 at row t,
+ * valid [B][A] = both valid; dist = 0 where not valid. */
+int wm_log_divergence(wm_handle* h, const wm_traj* log, const wm_traj* sim, int32_t t,
+                      float* dist, uint8_t* valid, void* stream);
+
+/*
+ * Default observation, L82: for every ego e (every agent slot; egos invalid at t get zeros /
+ * -1) at row t:
+ *  - hist [B][A_ego][H][7][A], hist_valid [B][A_ego][H][A]: all agents' last H = history
+ *    steps (rows t-H+1 .. t) in the ego frame at t: p' = R(-yaw_e)(p - p_e),
+ *    yaw' = wrap(yaw - yaw_e) in [-pi, pi), v' = R(-yaw_e) v, length, width (D22);
+ *  - rg_index [B][A_ego][k], rg_feat [B][A_ego][4][k] (x', y', dir_x', dir_y'), rg_type
+ *    [B][A_ego][k]: the k = topk valid roadgraph points nearest the ego centre, ties to the
+ *    lower index, emitted in ascending index order, padded with -1 / 0 (D23-D25).  The
+ *    selection key is the float32 value fma(dy, dy, dx*dx), dx = px - ex, dy = py - ey.
+ * Either group of outputs may be skipped by passing NULL for all of its pointers.
+ * The top-k part needs wm_prepare (WM_ERR_STATE otherwise). Requires t >= history-1.
+ */
+int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t t, float* hist,
+               uint8_t* hist_valid, int32_t* rg_index, float* rg_feat, int32_t* rg_type,
+               void* stream);
+
+/*
+ * Rollout, L200: for s = 0 .. n_steps-1: wm_step at t0+s, then overlap, offroad and log
+ * divergence on row t0+s+1 (D11), written to row s of the per-step outputs; aggregates over
+ * the n_steps rows at the end.  The whole sequence is one CUDA graph, captured on the first
+ * call for a given argument set and replayed afterwards (re-captured when any pointer or
+ * shape changes); no host synchronisation inside.
+ * actions [B][n_steps][C][A]; action_valid [B][n_steps][A].
+ */
+int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t0, int32_t n_steps,
+               const float* actions, const uint8_t* action_valid, const wm_rollout_out* out,
+               void* stream);
+
+/*
+ * The same job from HOST memory (pinned recommended): uploads the scenario (log, roadgraph)
+ * and the actions, runs wm_prepare, wm_reset and wm_rollout from t0 = history-1, downloads the
+ * metric rows and aggregates into the HOST buffers of `out`, and, when sim_host is not NULL,
+ * the simulated trajectory.  Device staging buffers are owned by the handle and reused.
+ * SYNCHRONISES before returning.  All pointers inside the structs are HOST pointers.
+ */
+int wm_rollout_host(wm_handle* h, const wm_traj* log_host, const wm_roadgraph* rg_host,
+                    int32_t n_steps, const float* actions_host, const uint8_t* action_valid_host,
+                    const wm_rollout_out* out_host, wm_traj* sim_host, void* stream);
+
+/* Introspection for tests and the bench (HOST outputs; each synchronises the stream).
+ * wm_segment_counts: n_seg [B] int32 copied to HOST.  wm_kernel_launches: number of kernels
+ * this handle has launched (graph replays count their kernel nodes). */
+int wm_segment_counts(wm_handle* h, int32_t* n_seg_host, int32_t B, void* stream);
+int64_t wm_kernel_launches(const wm_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WM_H_ */

@@ -1,0 +1,41 @@
+"""In-tree build of the CUDA C-ABI library (libwm_b200.so) for sm_100a with nvcc.
+
+nvcc cross-compiles without a GPU; the built .so sits beside this file so that it travels
+to the GPU box with the repository snapshot.
+"""
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(_HERE, "csrc")
+LIB = os.path.join(_HERE, "libwm_b200.so")
+SOURCES = ["wm_api.cu", "wm_dynamics.cu", "wm_overlap.cu", "wm_offroad.cu", "wm_observe.cu"]
+HEADERS = [os.path.join(CSRC, "wm_internal.cuh"), os.path.join(_HERE, "..", "include", "wm.h")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+
+
+def _stale():
+    if not os.path.exists(LIB):
+        return True
+    m = os.path.getmtime(LIB)
+    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]
+    return any(os.path.getmtime(d) > m for d in deps)
+
+
+def build(force=False, verbose=False):
+    """Compile every kernel for sm_100a into one shared library. Returns its path."""
+    if not force and not _stale():
+        return LIB
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    if verbose or res.returncode != 0:
+        print(res.stdout)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed building libwm_b200.so")
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True, verbose=True))

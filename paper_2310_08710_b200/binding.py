@@ -1,0 +1,231 @@
+"""Thin Python binding of the C-ABI in include/wm.h (same names, argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libwm_b200.so; PyTorch is used to own
+device memory and streams.  There is no CPU or eager fallback: if the shared library is
+missing or a call fails, this module raises.
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import _build
+
+WM_OK, WM_ERR_ARG, WM_ERR_CUDA, WM_ERR_UNSUPPORTED, WM_ERR_STATE = 0, -1, -2, -3, -4
+WM_DYN_INVERTIBLE_BICYCLE, WM_DYN_DELTA_LOCAL = 0, 1
+WM_TYPE_LANE, WM_TYPE_ROAD_EDGE = 1, 2
+_ERR = {-1: "WM_ERR_ARG", -2: "WM_ERR_CUDA", -3: "WM_ERR_UNSUPPORTED", -4: "WM_ERR_STATE"}
+
+TRAJ_F = ("x", "y", "yaw", "vel_x", "vel_y", "length", "width")
+RG_F = ("x", "y", "dir_x", "dir_y")
+
+EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
+           "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
+           "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches")
+
+
+class wm_traj(C.Structure):
+    _fields_ = [("B", C.c_int32), ("A", C.c_int32), ("T", C.c_int32)] + \
+               [(k, C.c_void_p) for k in TRAJ_F] + [("valid", C.c_void_p)]
+
+
+class wm_roadgraph(C.Structure):
+    _fields_ = [("B", C.c_int32), ("R", C.c_int32)] + [(k, C.c_void_p) for k in RG_F] + \
+               [("type", C.c_void_p), ("id", C.c_void_p), ("valid", C.c_void_p)]
+
+
+class wm_config(C.Structure):
+    _fields_ = [("dynamics", C.c_int32), ("dt", C.c_float), ("max_accel", C.c_float),
+                ("max_curvature", C.c_float), ("history", C.c_int32), ("topk", C.c_int32)]
+
+
+class wm_rollout_out(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in ("overlap", "offroad", "offroad_dist", "log_div",
+                                           "any_overlap", "any_offroad", "ade")]
+
+
+_lib = None
+
+
+def lib_path():
+    return _build.LIB
+
+
+def load():
+    """dlopen libwm_b200.so (building it first if the sources are newer). Raises if absent."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        if not os.path.exists(path):
+            raise RuntimeError("libwm_b200.so is missing: the CUDA extension must be built (no fallback)")
+        _lib = C.CDLL(path)
+        _lib.wm_version.restype = C.c_char_p
+        _lib.wm_kernel_launches.restype = C.c_int64
+        _lib.wm_kernel_launches.argtypes = [C.c_void_p]
+        for name in EXPORTS:
+            getattr(_lib, name)
+    return _lib
+
+
+class WmError(RuntimeError):
+    pass
+
+
+def _check(rc, what):
+    if rc != WM_OK:
+        extra = ""
+        if rc == WM_ERR_CUDA:
+            extra = " (cudaError_t %d)" % load().wm_last_cuda_error()
+        raise WmError("%s failed: %s%s" % (what, _ERR.get(rc, rc), extra))
+
+
+def _ptr(t, dtype=None, device_type="cuda"):
+    if t is None:
+        return None
+    assert isinstance(t, torch.Tensor) and t.is_contiguous(), "contiguous torch tensor expected"
+    assert t.device.type == device_type, "tensor on %s expected, got %s" % (device_type, t.device)
+    if dtype is not None:
+        assert t.dtype == dtype, (t.dtype, dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def traj_struct(tr, device_type="cuda"):
+    """dict of [B][T][A] tensors -> wm_traj."""
+    B, T, A = tr["x"].shape
+    for k in TRAJ_F:
+        assert tuple(tr[k].shape) == (B, T, A)
+    return wm_traj(B, A, T, *[_ptr(tr[k], torch.float32, device_type) for k in TRAJ_F],
+                   _ptr(tr["valid"], torch.uint8, device_type))
+
+
+def roadgraph_struct(rg, device_type="cuda"):
+    B, R = rg["x"].shape
+    return wm_roadgraph(B, R, *[_ptr(rg[k], torch.float32, device_type) for k in RG_F],
+                        _ptr(rg["type"], torch.int32, device_type), _ptr(rg["id"], torch.int32, device_type),
+                        _ptr(rg["valid"], torch.uint8, device_type))
+
+
+def rollout_out_struct(out, device_type="cuda"):
+    dt = dict(overlap=torch.uint8, offroad=torch.uint8, offroad_dist=torch.float32, log_div=torch.float32,
+              any_overlap=torch.uint8, any_offroad=torch.uint8, ade=torch.float32)
+    return wm_rollout_out(*[_ptr(out.get(k), dt[k], device_type) for k in dt])
+
+
+# ---- the entry points, same names as the C-ABI ----
+def wm_version():
+    return load().wm_version().decode()
+
+
+def wm_create(dynamics=WM_DYN_INVERTIBLE_BICYCLE, dt=0.1, max_accel=6.0, max_curvature=0.3, history=11, topk=1000):
+    h = C.c_void_p()
+    cfg = wm_config(dynamics, dt, max_accel, max_curvature, history, topk)
+    _check(load().wm_create(C.byref(h), C.byref(cfg)), "wm_create")
+    return h
+
+
+def wm_destroy(h):
+    _check(load().wm_destroy(h), "wm_destroy")
+
+
+def wm_prepare(h, rg, stream=None):
+    n = C.c_int32(0)
+    s = roadgraph_struct(rg)
+    _check(load().wm_prepare(h, C.byref(s), C.byref(n), _stream(stream)), "wm_prepare")
+    return n.value
+
+
+def wm_reset(h, log, sim, stream=None):
+    t = C.c_int32(0)
+    ls, ss = traj_struct(log), traj_struct(sim)
+    _check(load().wm_reset(h, C.byref(ls), C.byref(ss), C.byref(t), _stream(stream)), "wm_reset")
+    return t.value
+
+
+def wm_step(h, log, sim, t, action, action_valid, stream=None):
+    ls, ss = traj_struct(log), traj_struct(sim)
+    _check(load().wm_step(h, C.byref(ls), C.byref(ss), C.c_int32(t), _ptr(action, torch.float32),
+                          _ptr(action_valid, torch.uint8), _stream(stream)), "wm_step")
+
+
+def wm_metrics_overlap(h, sim, t, pair_bits, agent_flag, stream=None):
+    ss = traj_struct(sim)
+    _check(load().wm_metrics_overlap(h, C.byref(ss), C.c_int32(t), _ptr(pair_bits, torch.int32),
+                                     _ptr(agent_flag, torch.uint8), _stream(stream)), "wm_metrics_overlap")
+
+
+def wm_metrics_offroad(h, sim, t, signed_dist, corner_dist, agent_flag, stream=None):
+    ss = traj_struct(sim)
+    _check(load().wm_metrics_offroad(h, C.byref(ss), C.c_int32(t), _ptr(signed_dist, torch.float32),
+                                     _ptr(corner_dist, torch.float32), _ptr(agent_flag, torch.uint8),
+                                     _stream(stream)), "wm_metrics_offroad")
+
+
+def wm_log_divergence(h, log, sim, t, dist, valid, stream=None):
+    ls, ss = traj_struct(log), traj_struct(sim)
+    _check(load().wm_log_divergence(h, C.byref(ls), C.byref(ss), C.c_int32(t), _ptr(dist, torch.float32),
+                                    _ptr(valid, torch.uint8), _stream(stream)), "wm_log_divergence")
+
+
+def wm_observe(h, sim, rg, t, hist=None, hist_valid=None, rg_index=None, rg_feat=None, rg_type=None, stream=None):
+    ss = traj_struct(sim)
+    rs = roadgraph_struct(rg) if rg is not None else None
+    _check(load().wm_observe(h, C.byref(ss), C.byref(rs) if rs is not None else None, C.c_int32(t),
+                             _ptr(hist, torch.float32), _ptr(hist_valid, torch.uint8), _ptr(rg_index, torch.int32),
+                             _ptr(rg_feat, torch.float32), _ptr(rg_type, torch.int32), _stream(stream)), "wm_observe")
+
+
+def wm_rollout(h, log, sim, t0, n_steps, actions, action_valid, out, stream=None):
+    ls, ss = traj_struct(log), traj_struct(sim)
+    os_ = rollout_out_struct(out)
+    _check(load().wm_rollout(h, C.byref(ls), C.byref(ss), C.c_int32(t0), C.c_int32(n_steps),
+                             _ptr(actions, torch.float32), _ptr(action_valid, torch.uint8), C.byref(os_),
+                             _stream(stream)), "wm_rollout")
+
+
+def wm_rollout_host(h, log_host, rg_host, n_steps, actions_host, action_valid_host, out_host, sim_host=None, stream=None):
+    ls, rs = traj_struct(log_host, "cpu"), roadgraph_struct(rg_host, "cpu")
+    os_ = rollout_out_struct(out_host, "cpu")
+    sh = traj_struct(sim_host, "cpu") if sim_host is not None else None
+    _check(load().wm_rollout_host(h, C.byref(ls), C.byref(rs), C.c_int32(n_steps),
+                                  _ptr(actions_host, torch.float32, "cpu"), _ptr(action_valid_host, torch.uint8, "cpu"),
+                                  C.byref(os_), C.byref(sh) if sh is not None else None, _stream(stream)),
+           "wm_rollout_host")
+
+
+def wm_segment_counts(h, B, stream=None):
+    buf = (C.c_int32 * B)()
+    _check(load().wm_segment_counts(h, buf, C.c_int32(B), _stream(stream)), "wm_segment_counts")
+    return list(buf)
+
+
+def wm_kernel_launches(h):
+    return int(load().wm_kernel_launches(h))
+
+
+# ---- small conveniences for tests / bench: torch allocation of the ABI's arrays ----
+def to_device(d, device="cuda"):
+    """numpy dict (wm_scenarios layout) -> dict of contiguous torch tensors on `device`."""
+    return {k: torch.from_numpy(v).contiguous().to(device) for k, v in d.items()}
+
+
+def empty_traj_like(tr):
+    return {k: torch.zeros_like(v) for k, v in tr.items()}
+
+
+def alloc_rollout_out(B, n_steps, A, device="cuda", pin=False):
+    kw = dict(device=device)
+    if pin and device == "cpu":
+        kw["pin_memory"] = True
+    return dict(overlap=torch.zeros((B, n_steps, A), dtype=torch.uint8, **kw),
+                offroad=torch.zeros((B, n_steps, A), dtype=torch.uint8, **kw),
+                offroad_dist=torch.zeros((B, n_steps, A), dtype=torch.float32, **kw),
+                log_div=torch.zeros((B, n_steps, A), dtype=torch.float32, **kw),
+                any_overlap=torch.zeros((B, A), dtype=torch.uint8, **kw),
+                any_offroad=torch.zeros((B, A), dtype=torch.uint8, **kw),
+                ade=torch.zeros((B, A), dtype=torch.float32, **kw))

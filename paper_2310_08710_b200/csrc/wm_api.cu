@@ -1,0 +1,326 @@
+// C-ABI entry points (include/wm.h): argument checks, handle state, rollout graph capture,
+// host-buffer staging.  Every step of the path runs in the kernels of the sibling files.
+#include <stdlib.h>
+#include <string.h>
+
+#include "wm_internal.cuh"
+
+thread_local int g_wm_last_cuda_error = 0;
+
+extern "C" int wm_last_cuda_error(void) { return g_wm_last_cuda_error; }
+extern "C" const char* wm_version(void) { return "wm_b200 0.1 (sm_100a; FFMA2 offroad scan, bulk-TMA tiles, CUDA-graph rollout)"; }
+
+static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
+static bool traj_ok(const wm_traj* t) {
+  if (!t || t->B < 1 || t->A < 1 || t->T < 1) return false;
+  const void* ptrs[8] = {t->x, t->y, t->yaw, t->vel_x, t->vel_y, t->length, t->width, t->valid};
+  for (int i = 0; i < 8; ++i) if (!ptrs[i] || !aligned16(ptrs[i])) return false;
+  return true;
+}
+static bool rg_ok(const wm_roadgraph* g) {
+  if (!g || g->B < 1 || g->R < 1) return false;
+  const void* ptrs[7] = {g->x, g->y, g->dir_x, g->dir_y, g->type, g->id, g->valid};
+  for (int i = 0; i < 7; ++i) if (!ptrs[i] || !aligned16(ptrs[i])) return false;
+  return true;
+}
+static bool same_shape(const wm_traj* a, const wm_traj* b) { return a->B == b->B && a->A == b->A && a->T == b->T; }
+
+extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
+  if (!out || !cfg) return WM_ERR_ARG;
+  if (cfg->dynamics != WM_DYN_INVERTIBLE_BICYCLE && cfg->dynamics != WM_DYN_DELTA_LOCAL) return WM_ERR_ARG;
+  if (!(cfg->dt > 0.f) || cfg->history < 1 || cfg->topk < 0) return WM_ERR_ARG;
+  wm_handle* h = (wm_handle*)calloc(1, sizeof(wm_handle));
+  if (!h) return WM_ERR_ARG;
+  h->cfg = *cfg;
+  cudaError_t e = cudaGetDevice(&h->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device);
+  int major = 0;
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, h->device);
+  if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
+  if (major != 10) { free(h); return WM_ERR_UNSUPPORTED; }    // sm_100a kernels only; no fallback
+  e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking);
+  if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
+  *out = h;
+  return WM_OK;
+}
+
+void wm_drop_graph(wm_handle* h) {
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  if (h->graph) cudaGraphDestroy(h->graph);
+  h->graph_exec = nullptr; h->graph = nullptr; h->graph_kernels = 0;
+  memset(h->graph_key, 0, sizeof(h->graph_key));
+}
+
+extern "C" int wm_destroy(wm_handle* h) {
+  if (!h) return WM_ERR_ARG;
+  cudaDeviceSynchronize();
+  wm_drop_graph(h);
+  wm_prepare_free(h);
+  cudaFree(h->scratch);
+  for (int i = 0; i < 16; ++i) cudaFree(h->stage[i]);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  free(h);
+  return WM_OK;
+}
+
+extern "C" int64_t wm_kernel_launches(const wm_handle* h) { return h ? h->launches : 0; }
+
+extern "C" int wm_prepare(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, void* stream) {
+  if (!h || !rg_ok(rg)) return WM_ERR_ARG;
+  return wm_prepare_impl(h, rg, n_segments_max, (cudaStream_t)stream);
+}
+
+extern "C" int wm_segment_counts(wm_handle* h, int32_t* n_seg_host, int32_t B, void* stream) {
+  if (!h || !n_seg_host) return WM_ERR_ARG;
+  if (!h->n_seg || B != h->prep_B) return WM_ERR_STATE;
+  WM_CUDA(cudaMemcpyAsync(n_seg_host, h->n_seg, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  WM_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_reset(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t* t, void* stream) {
+  if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim)) return WM_ERR_ARG;
+  if (h->cfg.history > sim->T) return WM_ERR_ARG;
+  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  WM_CUDA(wm_launch_reset(h, *log, *sim, h->cfg.history, (cudaStream_t)stream));
+  if (t) *t = h->cfg.history - 1;
+  return WM_OK;
+}
+
+extern "C" int wm_step(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t, const float* action,
+                       const uint8_t* action_valid, void* stream) {
+  if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !action || !action_valid) return WM_ERR_ARG;
+  if (t < 0 || t + 1 >= sim->T) return WM_ERR_ARG;
+  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  WM_CUDA(wm_launch_step(h, *log, *sim, t, action, (int64_t)C * sim->A, action_valid, sim->A, nullptr, nullptr, 0,
+                         (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_metrics_overlap(wm_handle* h, const wm_traj* sim, int32_t t, uint32_t* pair_bits,
+                                  uint8_t* agent_flag, void* stream) {
+  if (!h || !traj_ok(sim) || !agent_flag) return WM_ERR_ARG;
+  if (t < 0 || t >= sim->T) return WM_ERR_ARG;
+  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  WM_CUDA(wm_launch_overlap(h, *sim, t, pair_bits, agent_flag, sim->A, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_metrics_offroad(wm_handle* h, const wm_traj* sim, int32_t t, float* signed_dist,
+                                  float* corner_dist, uint8_t* agent_flag, void* stream) {
+  if (!h || !traj_ok(sim) || !signed_dist || !agent_flag) return WM_ERR_ARG;
+  if (t < 0 || t >= sim->T) return WM_ERR_ARG;
+  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
+  WM_CUDA(wm_launch_offroad(h, *sim, t, signed_dist, sim->A, corner_dist, agent_flag, sim->A, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_log_divergence(wm_handle* h, const wm_traj* log, const wm_traj* sim, int32_t t, float* dist,
+                                 uint8_t* valid, void* stream) {
+  if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !dist) return WM_ERR_ARG;
+  if (t < 0 || t >= sim->T) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_logdiv(h, *log, *sim, t, dist, valid, sim->A, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t t, float* hist,
+                          uint8_t* hist_valid, int32_t* rg_index, float* rg_feat, int32_t* rg_type, void* stream) {
+  if (!h || !traj_ok(sim)) return WM_ERR_ARG;
+  const bool want_hist = hist || hist_valid, want_topk = rg_index || rg_feat || rg_type;
+  if (want_hist && !(hist && hist_valid)) return WM_ERR_ARG;
+  if (want_topk && !(rg_index && rg_feat && rg_type && rg_ok(rg))) return WM_ERR_ARG;
+  if (t < h->cfg.history - 1 || t >= sim->T) return WM_ERR_ARG;
+  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (want_hist) WM_CUDA(wm_launch_observe_hist(h, *sim, t, hist, hist_valid, (cudaStream_t)stream));
+  if (want_topk) {
+    if (h->cfg.topk < 1 || h->cfg.topk > rg->R) return WM_ERR_UNSUPPORTED;
+    if (!h->pts || h->prep_B != sim->B || h->prep_R != rg->R || rg->B != sim->B) return WM_ERR_STATE;
+    WM_CUDA(wm_launch_observe_topk(h, *sim, *rg, t, rg_index, rg_feat, rg_type, (cudaStream_t)stream));
+  }
+  return WM_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// rollout: n_steps x {step (+log divergence) -> overlap -> offroad}, aggregates; one graph.
+// ---------------------------------------------------------------------------------------
+static int ensure_scratch(wm_handle* h, size_t bytes) {
+  if (h->scratch_bytes >= bytes) return WM_OK;
+  wm_drop_graph(h);
+  cudaFree(h->scratch); h->scratch = nullptr; h->scratch_bytes = 0;
+  WM_CUDA(cudaMalloc(&h->scratch, bytes));
+  h->scratch_bytes = bytes;
+  return WM_OK;
+}
+
+static int enqueue_rollout(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
+                           const float* actions, const uint8_t* action_valid, const wm_rollout_out& o,
+                           uint8_t* ld_valid_rows, cudaStream_t s) {
+  const int A = sim.A;
+  const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  const int64_t row_stride = (int64_t)n_steps * A;
+  for (int k = 0; k < n_steps; ++k) {
+    const int t = t0 + k;
+    WM_CUDA(wm_launch_step(h, log, sim, t, actions + (int64_t)k * C * A, (int64_t)n_steps * C * A,
+                           action_valid + (int64_t)k * A, row_stride, o.log_div + (int64_t)k * A,
+                           ld_valid_rows + (int64_t)k * A, row_stride, s));
+    WM_CUDA(wm_launch_overlap(h, sim, t + 1, nullptr, o.overlap + (int64_t)k * A, row_stride, s));
+    WM_CUDA(wm_launch_offroad(h, sim, t + 1, o.offroad_dist + (int64_t)k * A, row_stride, nullptr,
+                              o.offroad + (int64_t)k * A, row_stride, s));
+  }
+  WM_CUDA(wm_launch_aggregate(h, sim.B, A, n_steps, o, ld_valid_rows, s));
+  return WM_OK;
+}
+
+extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t0, int32_t n_steps,
+                          const float* actions, const uint8_t* action_valid, const wm_rollout_out* out, void* stream) {
+  if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !actions || !action_valid || !out) return WM_ERR_ARG;
+  if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
+  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
+  const int64_t rows = (int64_t)sim->B * n_steps * sim->A;
+  // rows the caller did not ask for still feed the aggregates: put them in scratch
+  size_t need = (size_t)rows;                                  // ld_valid rows (uint8)
+  need = (need + 255) / 256 * 256;
+  const size_t off_ov = need;    if (!out->overlap) need += (size_t)rows;
+  need = (need + 255) / 256 * 256;
+  const size_t off_of = need;    if (!out->offroad) need += (size_t)rows;
+  need = (need + 255) / 256 * 256;
+  const size_t off_sd = need;    if (!out->offroad_dist) need += (size_t)rows * 4;
+  need = (need + 255) / 256 * 256;
+  const size_t off_ld = need;    if (!out->log_div) need += (size_t)rows * 4;
+  int rc = ensure_scratch(h, need);
+  if (rc != WM_OK) return rc;
+  unsigned char* sc = (unsigned char*)h->scratch;
+  wm_rollout_out o = *out;
+  if (!o.overlap) o.overlap = sc + off_ov;
+  if (!o.offroad) o.offroad = sc + off_of;
+  if (!o.offroad_dist) o.offroad_dist = (float*)(sc + off_sd);
+  if (!o.log_div) o.log_div = (float*)(sc + off_ld);
+  uint8_t* ld_valid_rows = sc;
+
+  uint64_t key[24];
+  memset(key, 0, sizeof(key));
+  int n = 0;
+  const void* ptrs[] = {log->x, log->y, log->yaw, log->vel_x, log->vel_y, log->length, log->width, log->valid,
+                        sim->x, sim->y, sim->yaw, sim->vel_x, sim->vel_y, sim->length, sim->width, sim->valid,
+                        actions, action_valid, o.overlap, o.offroad, o.offroad_dist};
+  for (const void* p : ptrs) key[n++] = (uint64_t)(uintptr_t)p;
+  key[n++] = (uint64_t)(uintptr_t)o.log_div ^ ((uint64_t)(uintptr_t)o.any_overlap << 1) ^ ((uint64_t)(uintptr_t)o.any_offroad << 2) ^
+             ((uint64_t)(uintptr_t)o.ade << 3);
+  key[n++] = ((uint64_t)sim->B << 40) ^ ((uint64_t)sim->A << 20) ^ (uint64_t)sim->T;
+  key[n++] = ((uint64_t)(uint32_t)t0 << 32) ^ (uint64_t)(uint32_t)n_steps ^ ((uint64_t)h->cfg.dynamics << 62);
+
+  if (!h->graph_exec || memcmp(key, h->graph_key, sizeof(key)) != 0) {
+    wm_drop_graph(h);
+    const int64_t before = h->launches;
+    WM_CUDA(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    rc = enqueue_rollout(h, *log, *sim, t0, n_steps, actions, action_valid, o, ld_valid_rows, h->cap_stream);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
+    h->graph_kernels = h->launches - before;
+    h->launches = before;                    // capture launched nothing yet
+    if (rc != WM_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    WM_CUDA(e);
+    h->graph = g;
+    WM_CUDA(cudaGraphInstantiate(&h->graph_exec, h->graph, 0));
+    memcpy(h->graph_key, key, sizeof(key));
+  }
+  WM_CUDA(cudaGraphLaunch(h->graph_exec, (cudaStream_t)stream));
+  h->launches += h->graph_kernels;
+  return WM_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// the same job from host memory
+// ---------------------------------------------------------------------------------------
+static int stage_alloc(wm_handle* h, int slot, size_t bytes) {
+  if (h->stage_bytes[slot] >= bytes) return WM_OK;
+  wm_drop_graph(h);
+  cudaFree(h->stage[slot]); h->stage[slot] = nullptr; h->stage_bytes[slot] = 0;
+  WM_CUDA(cudaMalloc(&h->stage[slot], bytes));
+  h->stage_bytes[slot] = bytes;
+  return WM_OK;
+}
+
+static size_t al256(size_t n) { return (n + 255) / 256 * 256; }
+
+extern "C" int wm_rollout_host(wm_handle* h, const wm_traj* lh, const wm_roadgraph* gh, int32_t n_steps,
+                               const float* actions_host, const uint8_t* action_valid_host,
+                               const wm_rollout_out* oh, wm_traj* sim_host, void* stream) {
+  if (!h || !lh || !gh || !actions_host || !action_valid_host || !oh) return WM_ERR_ARG;
+  if (lh->B < 1 || lh->A < 1 || lh->T < 1 || gh->B != lh->B || gh->R < 1) return WM_ERR_ARG;
+  const int B = lh->B, A = lh->A, T = lh->T, R = gh->R;
+  const int t0 = h->cfg.history - 1;
+  if (n_steps < 1 || t0 + n_steps >= T) return WM_ERR_ARG;
+  if (A > 1024) return WM_ERR_UNSUPPORTED;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  const size_t nTA = (size_t)B * T * A, nR = (size_t)B * R, rows = (size_t)B * n_steps * A, nBA = (size_t)B * A;
+  // slot 0: log traj, 1: sim traj, 2: roadgraph, 3: actions + valid, 4: outputs
+  const size_t traj_bytes = 7 * al256(nTA * 4) + al256(nTA);
+  const size_t rg_bytes = 6 * al256(nR * 4) + al256(nR);
+  const size_t act_bytes = al256(rows * C * 4) + al256(rows);
+  const size_t out_bytes = 2 * al256(rows) + 2 * al256(rows * 4) + 2 * al256(nBA) + al256(nBA * 4);
+  int rc;
+  if ((rc = stage_alloc(h, 0, traj_bytes)) != WM_OK) return rc;
+  if ((rc = stage_alloc(h, 1, traj_bytes)) != WM_OK) return rc;
+  if ((rc = stage_alloc(h, 2, rg_bytes)) != WM_OK) return rc;
+  if ((rc = stage_alloc(h, 3, act_bytes)) != WM_OK) return rc;
+  if ((rc = stage_alloc(h, 4, out_bytes)) != WM_OK) return rc;
+  auto carve_traj = [&](void* base, wm_traj& t) {
+    unsigned char* p = (unsigned char*)base;
+    t.B = B; t.A = A; t.T = T;
+    float** f[7] = {&t.x, &t.y, &t.yaw, &t.vel_x, &t.vel_y, &t.length, &t.width};
+    for (int i = 0; i < 7; ++i) { *f[i] = (float*)p; p += al256(nTA * 4); }
+    t.valid = p;
+  };
+  wm_traj dl, ds;
+  carve_traj(h->stage[0], dl);
+  carve_traj(h->stage[1], ds);
+  wm_roadgraph dg;
+  {
+    unsigned char* p = (unsigned char*)h->stage[2];
+    dg.B = B; dg.R = R;
+    dg.x = (float*)p; p += al256(nR * 4); dg.y = (float*)p; p += al256(nR * 4);
+    dg.dir_x = (float*)p; p += al256(nR * 4); dg.dir_y = (float*)p; p += al256(nR * 4);
+    dg.type = (int32_t*)p; p += al256(nR * 4); dg.id = (int32_t*)p; p += al256(nR * 4);
+    dg.valid = p;
+  }
+  float* d_act = (float*)h->stage[3];
+  uint8_t* d_av = (uint8_t*)h->stage[3] + al256(rows * C * 4);
+  wm_rollout_out dout;
+  {
+    unsigned char* p = (unsigned char*)h->stage[4];
+    dout.overlap = p; p += al256(rows); dout.offroad = p; p += al256(rows);
+    dout.offroad_dist = (float*)p; p += al256(rows * 4); dout.log_div = (float*)p; p += al256(rows * 4);
+    dout.any_overlap = p; p += al256(nBA); dout.any_offroad = p; p += al256(nBA);
+    dout.ade = (float*)p;
+  }
+#define H2D(dst, src, n) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyHostToDevice, s))
+#define D2H(dst, src, n) do { if (dst) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyDeviceToHost, s)); } while (0)
+  H2D(dl.x, lh->x, nTA * 4); H2D(dl.y, lh->y, nTA * 4); H2D(dl.yaw, lh->yaw, nTA * 4);
+  H2D(dl.vel_x, lh->vel_x, nTA * 4); H2D(dl.vel_y, lh->vel_y, nTA * 4);
+  H2D(dl.length, lh->length, nTA * 4); H2D(dl.width, lh->width, nTA * 4); H2D(dl.valid, lh->valid, nTA);
+  H2D(dg.x, gh->x, nR * 4); H2D(dg.y, gh->y, nR * 4); H2D(dg.dir_x, gh->dir_x, nR * 4); H2D(dg.dir_y, gh->dir_y, nR * 4);
+  H2D(dg.type, gh->type, nR * 4); H2D(dg.id, gh->id, nR * 4); H2D(dg.valid, gh->valid, nR);
+  H2D(d_act, actions_host, rows * C * 4); H2D(d_av, action_valid_host, rows);
+  if ((rc = wm_prepare(h, &dg, nullptr, s)) != WM_OK) return rc;
+  if ((rc = wm_reset(h, &dl, &ds, nullptr, s)) != WM_OK) return rc;
+  if ((rc = wm_rollout(h, &dl, &ds, t0, n_steps, d_act, d_av, &dout, s)) != WM_OK) return rc;
+  D2H(oh->overlap, dout.overlap, rows); D2H(oh->offroad, dout.offroad, rows);
+  D2H(oh->offroad_dist, dout.offroad_dist, rows * 4); D2H(oh->log_div, dout.log_div, rows * 4);
+  D2H(oh->any_overlap, dout.any_overlap, nBA); D2H(oh->any_offroad, dout.any_offroad, nBA);
+  D2H(oh->ade, dout.ade, nBA * 4);
+  if (sim_host) {
+    D2H(sim_host->x, ds.x, nTA * 4); D2H(sim_host->y, ds.y, nTA * 4); D2H(sim_host->yaw, ds.yaw, nTA * 4);
+    D2H(sim_host->vel_x, ds.vel_x, nTA * 4); D2H(sim_host->vel_y, ds.vel_y, nTA * 4);
+    D2H(sim_host->length, ds.length, nTA * 4); D2H(sim_host->width, ds.width, nTA * 4); D2H(sim_host->valid, ds.valid, nTA);
+  }
+#undef H2D
+#undef D2H
+  WM_CUDA(cudaStreamSynchronize(s));
+  return WM_OK;
+}

@@ -1,0 +1,179 @@
+// reset (a0), dynamics step (a1, a2) with optional fused log divergence (a5), aggregates (a8).
+// One thread per (scenario, agent): these kernels move ~12 KB per scenario-step and are
+// HBM/latency bound; rows are time-major so a warp touches one contiguous 128 B line per field.
+#include "wm_internal.cuh"
+
+// ---------------------------------------------------------------------------------------
+// a0 reset(scenario), PAPER.md L122 / L78.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_reset(wm_traj log, wm_traj sim, int history) {
+  const int64_t n = (int64_t)sim.B * sim.T * sim.A;
+  const int64_t TA = (int64_t)sim.T * sim.A;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const int t = (int)((i % TA) / sim.A);
+    const bool c = t < history;
+    sim.x[i] = c ? log.x[i] : 0.f;
+    sim.y[i] = c ? log.y[i] : 0.f;
+    sim.yaw[i] = c ? log.yaw[i] : 0.f;
+    sim.vel_x[i] = c ? log.vel_x[i] : 0.f;
+    sim.vel_y[i] = c ? log.vel_y[i] : 0.f;
+    sim.length[i] = c ? log.length[i] : 0.f;
+    sim.width[i] = c ? log.width[i] : 0.f;
+    sim.valid[i] = c ? log.valid[i] : (uint8_t)0;
+  }
+}
+
+cudaError_t wm_launch_reset(wm_handle* h, const wm_traj& log, const wm_traj& sim, int history, cudaStream_t s) {
+  const int64_t n = (int64_t)sim.B * sim.T * sim.A;
+  int grid = (int)((n + 255) / 256);
+  const int cap = h->num_sms * 32;
+  if (grid > cap) grid = cap;
+  k_reset<<<grid, 256, 0, s>>>(log, sim, history);
+  h->launches++;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// a1 / a2 step(state, action); Eq. 2 (L339-L350) and Eq. 1 (L324-L333).
+// ---------------------------------------------------------------------------------------
+struct StepParams {
+  wm_row cur;       // sim row t
+  wm_row nxt_log;   // log row t+1
+  wm_row_mut nxt;   // sim row t+1
+  const float* action; int64_t act_stride_b;
+  const uint8_t* av;   int64_t av_stride_b;
+  float* ld_dist; uint8_t* ld_valid; int64_t ld_stride_b;
+  int B, A, dynamics;
+  float dt, max_accel, max_curvature;
+};
+
+__global__ void __launch_bounds__(256) k_step(StepParams p) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= (int64_t)p.B * p.A) return;
+  const int b = (int)(i / p.A), a = (int)(i % p.A);
+  const int64_t c = (int64_t)b * p.cur.stride_b + a;       // same offset in all three rows
+  const bool use_dyn = p.av[(int64_t)b * p.av_stride_b + a] != 0 && p.cur.valid[c] != 0;
+  const float lx = p.nxt_log.x[c], ly = p.nxt_log.y[c];
+  const uint8_t lvalid = p.nxt_log.valid[c];
+  float xn, yn, thn, vxn, vyn, ln, wn;
+  uint8_t vn;
+  if (use_dyn) {
+    const float x = p.cur.x[c], y = p.cur.y[c], th = p.cur.yaw[c];
+    const float vx = p.cur.vel_x[c], vy = p.cur.vel_y[c];
+    const float* act = p.action + (int64_t)b * p.act_stride_b + a;
+    float sn, cs;
+    sincosf(th, &sn, &cs);
+    const float dt = p.dt;
+    if (p.dynamics == WM_DYN_INVERTIBLE_BICYCLE) {
+      float acc = act[0], kappa = act[p.A];
+      if (p.max_accel > 0.f) acc = fminf(fmaxf(acc, -p.max_accel), p.max_accel);
+      if (p.max_curvature > 0.f) kappa = fminf(fmaxf(kappa, -p.max_curvature), p.max_curvature);
+      const float v = sqrtf(fmaf(vx, vx, vy * vy));
+      const float h = 0.5f * acc * dt * dt;            // a dt^2 / 2
+      xn = x + fmaf(vx, dt, h * cs);                   // Eq. 2
+      yn = y + fmaf(vy, dt, h * sn);                   // L341
+      thn = fmaf(kappa, fmaf(v, dt, h), th);           // L343
+      const float v1 = fmaf(acc, dt, v);               // L345
+      float s1, c1;
+      sincosf(thn, &s1, &c1);
+      vxn = v1 * c1;                                   // L347
+      vyn = v1 * s1;                                   // L349
+    } else {
+      const float dx = act[0], dy = act[p.A], dyaw = act[2 * (int64_t)p.A];
+      xn = x + (cs * dx - sn * dy);                    // Eq. 1 on the rotated delta (D2)
+      yn = y + (sn * dx + cs * dy);
+      thn = th + dyaw;
+      vxn = (xn - x) / dt;                             // Eq. 1: on the stored float32 x'
+      vyn = (yn - y) / dt;
+    }
+    ln = p.cur.length[c];
+    wn = p.cur.width[c];
+    vn = 1;                                            // D9
+  } else {                                             // log playback, L164 / D8
+    xn = lx; yn = ly; thn = p.nxt_log.yaw[c];
+    vxn = p.nxt_log.vel_x[c]; vyn = p.nxt_log.vel_y[c];
+    ln = p.nxt_log.length[c]; wn = p.nxt_log.width[c];
+    vn = lvalid;
+  }
+  p.nxt.x[c] = xn; p.nxt.y[c] = yn; p.nxt.yaw[c] = thn;
+  p.nxt.vel_x[c] = vxn; p.nxt.vel_y[c] = vyn;
+  p.nxt.length[c] = ln; p.nxt.width[c] = wn; p.nxt.valid[c] = vn;
+  if (p.ld_dist) {                                     // fused a5 on row t+1, L106
+    const bool v = vn != 0 && lvalid != 0;
+    float d = 0.f;
+    if (v) { const float ex = xn - lx, ey = yn - ly; d = sqrtf(fmaf(ex, ex, ey * ey)); }
+    p.ld_dist[(int64_t)b * p.ld_stride_b + a] = d;
+    if (p.ld_valid) p.ld_valid[(int64_t)b * p.ld_stride_b + a] = v;
+  }
+}
+
+cudaError_t wm_launch_step(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t,
+                           const float* action, int64_t act_stride_b, const uint8_t* av,
+                           int64_t av_stride_b, float* ld_dist, uint8_t* ld_valid,
+                           int64_t ld_stride_b, cudaStream_t s) {
+  StepParams p;
+  p.cur = wm_make_row(sim, t);
+  p.nxt_log = wm_make_row(log, t + 1);
+  p.nxt = wm_make_row_mut(sim, t + 1);
+  p.action = action; p.act_stride_b = act_stride_b;
+  p.av = av; p.av_stride_b = av_stride_b;
+  p.ld_dist = ld_dist; p.ld_valid = ld_valid; p.ld_stride_b = ld_stride_b;
+  p.B = sim.B; p.A = sim.A; p.dynamics = h->cfg.dynamics;
+  p.dt = h->cfg.dt; p.max_accel = h->cfg.max_accel; p.max_curvature = h->cfg.max_curvature;
+  const int64_t n = (int64_t)sim.B * sim.A;
+  k_step<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(p);
+  h->launches++;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// a5 log divergence.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_logdiv(wm_row lg, wm_row sm, int B, int A, float* dist, uint8_t* valid, int64_t stride_b) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= (int64_t)B * A) return;
+  const int b = (int)(i / A), a = (int)(i % A);
+  const int64_t cs = (int64_t)b * sm.stride_b + a, cl = (int64_t)b * lg.stride_b + a;
+  const bool v = sm.valid[cs] != 0 && lg.valid[cl] != 0;
+  float d = 0.f;
+  if (v) { const float ex = sm.x[cs] - lg.x[cl], ey = sm.y[cs] - lg.y[cl]; d = sqrtf(fmaf(ex, ex, ey * ey)); }
+  dist[(int64_t)b * stride_b + a] = d;
+  if (valid) valid[(int64_t)b * stride_b + a] = v;
+}
+
+cudaError_t wm_launch_logdiv(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t, float* dist,
+                             uint8_t* valid, int64_t stride_b, cudaStream_t s) {
+  const int64_t n = (int64_t)sim.B * sim.A;
+  k_logdiv<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(wm_make_row(log, t), wm_make_row(sim, t), sim.B, sim.A, dist, valid, stride_b);
+  h->launches++;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// a8 aggregates over the n_steps metric rows (D21): any-overlap, any-offroad, ADE.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_aggregate(int B, int A, int n_steps, wm_rollout_out out, const uint8_t* ld_valid) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= (int64_t)B * A) return;
+  const int b = (int)(i / A), a = (int)(i % A);
+  uint8_t ov = 0, off = 0;
+  double sum = 0.0;
+  int cnt = 0;
+  for (int s = 0; s < n_steps; ++s) {
+    const int64_t o = ((int64_t)b * n_steps + s) * A + a;
+    if (out.overlap) ov |= out.overlap[o];
+    if (out.offroad) off |= out.offroad[o];
+    if (out.log_div && ld_valid[o]) { sum += (double)out.log_div[o]; cnt++; }
+  }
+  if (out.any_overlap) out.any_overlap[i] = ov;
+  if (out.any_offroad) out.any_offroad[i] = off;
+  if (out.ade) out.ade[i] = cnt ? (float)(sum / cnt) : 0.f;
+}
+
+cudaError_t wm_launch_aggregate(wm_handle* h, int B, int A, int n_steps, const wm_rollout_out& out,
+                                const uint8_t* ld_valid_rows, cudaStream_t s) {
+  const int64_t n = (int64_t)B * A;
+  k_aggregate<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(B, A, n_steps, out, ld_valid_rows);
+  h->launches++;
+  return cudaGetLastError();
+}

@@ -1,0 +1,149 @@
+// Internal declarations of the wm_* library (sm_100a only). Not part of the public ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/wm.h"
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "this library is written for sm_100a (B200) only"
+#endif
+
+// ---------------------------------------------------------------------------------------
+// Layout constants of the prepared road-edge segments.
+// A tile holds 512 segments = 32 lanes x 16 consecutive segments ("run") per lane, stored so
+// that one LDS.128 per lane fetches the same component of two consecutive segments:
+//   float4 index inside a tile = (it*3 + c)*32 + lane,  it = (s%16)/2,  lane = (s%512)/16
+//   c = 0: {p0x[lo], p0x[hi], p0y[lo], p0y[hi]}   lo/hi = segments 2*it, 2*it+1 of the run
+//   c = 1: {ex[lo],  ex[hi],  ey[lo],  ey[hi]}    e = p1 - p0
+//   c = 2: {gx[lo],  gx[hi],  gy[lo],  gy[hi]}    g = e / (e.e)   (0 for zero-length)
+// ---------------------------------------------------------------------------------------
+constexpr int WM_TILE_SEGS = 512;
+constexpr int WM_RUN = 16;                 // consecutive segments owned by one lane
+constexpr int WM_TILE_F4 = 8 * 3 * 32;     // float4 per tile
+constexpr int WM_TILE_BYTES = WM_TILE_F4 * 16;   // 12288
+constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding segments
+
+// Prepared roadgraph points for top-k: float2 (x, y) per point, invalid -> (WM_FAR, WM_FAR),
+// padded to a multiple of WM_PT_TILE.
+constexpr int WM_PT_TILE = 2048;
+
+struct wm_handle {
+  wm_config cfg;
+  int device;
+  int num_sms;
+  int64_t launches;
+  // prepared static data (wm_prepare)
+  int32_t prep_B, prep_R;
+  int32_t seg_tiles;        // tiles per scenario in `edges`
+  int32_t seg_max;          // max_b n_seg[b]
+  int32_t* n_seg;           // [B]
+  float4* edges;            // [B][seg_tiles][WM_TILE_F4]
+  float2* sign_dir;         // [B][seg_tiles*512]  sign direction (e, or stored dir if e == 0)
+  int32_t* seg_src;         // [B][seg_tiles*512]  first-point index of each segment
+  int32_t pts_pad;          // padded R
+  float2* pts;              // [B][pts_pad]
+  // rollout graph cache
+  cudaStream_t cap_stream;
+  cudaGraph_t graph;
+  cudaGraphExec_t graph_exec;
+  int64_t graph_kernels;
+  uint64_t graph_key[24];
+  // scratch for rollouts / host staging
+  void* scratch; size_t scratch_bytes;
+  void* stage[16]; size_t stage_bytes[16];
+};
+
+extern thread_local int g_wm_last_cuda_error;
+
+#define WM_CUDA(call)                                   \
+  do {                                                  \
+    cudaError_t e__ = (call);                           \
+    if (e__ != cudaSuccess) {                           \
+      g_wm_last_cuda_error = (int)e__;                  \
+      return WM_ERR_CUDA;                               \
+    }                                                   \
+  } while (0)
+
+// A time row of a trajectory: pointers to row t of scenario 0, batch stride in elements.
+struct wm_row {
+  const float *x, *y, *yaw, *vel_x, *vel_y, *length, *width;
+  const uint8_t* valid;
+  int64_t stride_b;
+};
+struct wm_row_mut {
+  float *x, *y, *yaw, *vel_x, *vel_y, *length, *width;
+  uint8_t* valid;
+  int64_t stride_b;
+};
+static inline wm_row wm_make_row(const wm_traj& tr, int t) {
+  const int64_t o = (int64_t)t * tr.A;
+  return wm_row{tr.x + o, tr.y + o, tr.yaw + o, tr.vel_x + o, tr.vel_y + o, tr.length + o,
+                tr.width + o, tr.valid + o, (int64_t)tr.T * tr.A};
+}
+static inline wm_row_mut wm_make_row_mut(const wm_traj& tr, int t) {
+  const int64_t o = (int64_t)t * tr.A;
+  return wm_row_mut{tr.x + o, tr.y + o, tr.yaw + o, tr.vel_x + o, tr.vel_y + o, tr.length + o,
+                    tr.width + o, tr.valid + o, (int64_t)tr.T * tr.A};
+}
+
+// ---- launchers (each enqueues on `s`, returns the launch error, bumps h->launches) ----
+cudaError_t wm_launch_reset(wm_handle* h, const wm_traj& log, const wm_traj& sim, int history, cudaStream_t s);
+// dynamics row t -> t+1; optional fused log divergence of row t+1 (ld_dist may be NULL)
+cudaError_t wm_launch_step(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t,
+                           const float* action, int64_t act_stride_b, const uint8_t* av,
+                           int64_t av_stride_b, float* ld_dist, uint8_t* ld_valid,
+                           int64_t ld_stride_b, cudaStream_t s);
+cudaError_t wm_launch_logdiv(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t, float* dist,
+                             uint8_t* valid, int64_t stride_b, cudaStream_t s);
+cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t* pair_bits,
+                              uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
+cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
+                              float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
+cudaError_t wm_launch_aggregate(wm_handle* h, int B, int A, int n_steps, const wm_rollout_out& out,
+                                const uint8_t* ld_valid_rows, cudaStream_t s);
+int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);
+void wm_prepare_free(wm_handle* h);
+void wm_drop_graph(wm_handle* h);
+cudaError_t wm_launch_observe_hist(wm_handle* h, const wm_traj& sim, int t, float* hist, uint8_t* hist_valid, cudaStream_t s);
+cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_roadgraph& rg, int t,
+                                   int32_t* rg_index, float* rg_feat, int32_t* rg_type, cudaStream_t s);
+
+#ifdef __CUDACC__
+// ---------------------------------------------------------------------------------------
+// Device helpers: packed fp32x2 arithmetic (FFMA2/FADD2/FMUL2 on sm_100a), 3-input min,
+// mbarrier + 1-D bulk TMA (cp.async.bulk -> UBLKCP).
+// ---------------------------------------------------------------------------------------
+typedef unsigned long long wm_u64;
+__device__ __forceinline__ wm_u64 pk2(float lo, float hi) { wm_u64 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(wm_u64 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ wm_u64 fma2(wm_u64 a, wm_u64 b, wm_u64 c) { wm_u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ wm_u64 add2(wm_u64 a, wm_u64 b) { wm_u64 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ wm_u64 sub2(wm_u64 a, wm_u64 b) { wm_u64 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ wm_u64 mul2(wm_u64 a, wm_u64 b) { wm_u64 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ float min3f(float a, float b, float c) { float d; asm("min.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c)); return d; }
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// 1-D bulk copy global -> shared, completion counted in bytes on `bar`. bytes % 16 == 0.
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+#endif

@@ -1,0 +1,442 @@
+// a4 off-road metric, PAPER.md L100 (+ L176: "the Off-Road metric needs to find nearby
+// roadgraph points, which is a slow operation" — this kernel IS the cost of the step).
+//
+// wm_prepare: compacts road-edge segments once per scenario into 512-segment tiles laid out
+// for conflict-free LDS.128 and packed fp32x2 arithmetic (wm_internal.cuh).
+//
+// k_offroad: one CTA per scenario.  The scenario's segment tiles are streamed into shared
+// memory by 1-D bulk TMA (cp.async.bulk, mbarrier completion) into two buffers; lanes own
+// SEGMENTS (a run of 16 consecutive ones per tile), a warp owns a "unit" of 2 valid agents
+// = 8 box corners held in registers, and evaluates 2 segments x 8 corners per iteration
+// with FFMA2/FADD2/FMUL2 (two segments packed per instruction):
+//     w = (c - p0) + off_k;  t = sat(w.g);  r = w - t e;  d2 = r.r          (8.5 FP32 lane-ops)
+//     min tracked per (lane, corner) with one 3-input FMNMX per packed pair
+// The argmin is tracked at run granularity (tile, lane); at the end the winning run of each
+// corner (16 segments) is re-scanned to get the exact segment (lowest index on ties, D17), the
+// sign from the oriented edge (D16) and the signed distance.  Valid agents are compacted first,
+// so invalid slots cost nothing.  Bound: FP32 pipe (see DESIGN.md roofline).
+#include <float.h>
+
+#include "wm_internal.cuh"
+
+// ======================================================================================
+// wm_prepare kernels
+// ======================================================================================
+struct RgView {
+  const float *x, *y, *dir_x, *dir_y;
+  const int32_t *type, *id;
+  const uint8_t* valid;
+  int R;
+};
+
+__device__ __forceinline__ bool rg_is_edge(const RgView& g, int64_t o, int i) {
+  return g.valid[o + i] != 0 && g.type[o + i] == WM_TYPE_ROAD_EDGE;
+}
+__device__ __forceinline__ bool rg_starts(const RgView& g, int64_t o, int i) {
+  return i + 1 < g.R && rg_is_edge(g, o, i) && rg_is_edge(g, o, i + 1) && g.id[o + i] == g.id[o + i + 1];
+}
+// point i contributes a record: a segment (i, i+1), or an isolated zero-length segment (D16)
+__device__ __forceinline__ bool rg_record(const RgView& g, int64_t o, int i, bool* is_seg) {
+  if (i >= g.R) { *is_seg = false; return false; }
+  const bool s = rg_starts(g, o, i);
+  *is_seg = s;
+  if (s) return true;
+  return rg_is_edge(g, o, i) && !(i > 0 && rg_starts(g, o, i - 1));
+}
+
+__global__ void __launch_bounds__(256) k_count_segments(RgView g, int32_t* n_seg) {
+  __shared__ int s_cnt;
+  if (threadIdx.x == 0) s_cnt = 0;
+  __syncthreads();
+  const int64_t o = (int64_t)blockIdx.x * g.R;
+  int c = 0;
+  for (int i = threadIdx.x; i < g.R; i += blockDim.x) { bool sg; c += rg_record(g, o, i, &sg) ? 1 : 0; }
+  atomicAdd(&s_cnt, c);
+  __syncthreads();
+  if (threadIdx.x == 0) n_seg[blockIdx.x] = s_cnt;
+}
+
+__device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir, int32_t* seg_src, int s,
+                                              float p0x, float p0y, float ex, float ey, float gx, float gy,
+                                              float sx, float sy, int src) {
+  const int tau = s / WM_TILE_SEGS, r = s % WM_TILE_SEGS;
+  const int lane = r / WM_RUN, j = r % WM_RUN, it = j >> 1, half = j & 1;
+  float* t = tile_base + (int64_t)tau * (WM_TILE_F4 * 4);
+  float* q0 = t + ((it * 3 + 0) * 32 + lane) * 4;
+  float* q1 = t + ((it * 3 + 1) * 32 + lane) * 4;
+  float* q2 = t + ((it * 3 + 2) * 32 + lane) * 4;
+  q0[half] = p0x; q0[2 + half] = p0y;
+  q1[half] = ex;  q1[2 + half] = ey;
+  q2[half] = gx;  q2[2 + half] = gy;
+  sign_dir[s] = make_float2(sx, sy);
+  seg_src[s] = src;
+}
+
+__global__ void __launch_bounds__(1024) k_fill_segments(RgView g, int seg_tiles, float4* edges, float2* sign_dir, int32_t* seg_src) {
+  __shared__ int s_warp[32];
+  __shared__ int s_base;
+  const int b = blockIdx.x;
+  const int64_t o = (int64_t)b * g.R;
+  const int cap = seg_tiles * WM_TILE_SEGS;
+  float* tile_base = (float*)(edges + (int64_t)b * seg_tiles * WM_TILE_F4);
+  float2* sd = sign_dir + (int64_t)b * cap;
+  int32_t* src = seg_src + (int64_t)b * cap;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) s_base = 0;
+  __syncthreads();
+  for (int base = 0; base < g.R; base += blockDim.x) {
+    const int i = base + threadIdx.x;
+    bool is_seg;
+    const bool rec = rg_record(g, o, i, &is_seg);
+    const uint32_t bal = __ballot_sync(0xffffffffu, rec);
+    if (lane == 0) s_warp[warp] = __popc(bal);
+    __syncthreads();
+    int pre = s_base;
+    for (int w = 0; w < warp; ++w) pre += s_warp[w];
+    if (rec) {
+      const int s = pre + __popc(bal & ((1u << lane) - 1u));
+      const float p0x = g.x[o + i], p0y = g.y[o + i];
+      float ex = 0.f, ey = 0.f;
+      if (is_seg) { ex = g.x[o + i + 1] - p0x; ey = g.y[o + i + 1] - p0y; }
+      const float ee = fmaf(ex, ex, ey * ey);
+      float gx = 0.f, gy = 0.f, sx, sy;
+      if (ee > 0.f) { gx = ex / ee; gy = ey / ee; sx = ex; sy = ey; }
+      else { ex = 0.f; ey = 0.f; sx = g.dir_x[o + i]; sy = g.dir_y[o + i]; }
+      store_segment(tile_base, sd, src, s, p0x, p0y, ex, ey, gx, gy, sx, sy, i);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) { int tot = 0; for (int w = 0; w < 32; ++w) tot += s_warp[w]; s_base += tot; }
+    __syncthreads();
+  }
+  // padding records: far away, never win against a real segment
+  for (int s = s_base + threadIdx.x; s < cap; s += blockDim.x)
+    store_segment(tile_base, sd, src, s, WM_FAR, WM_FAR, 0.f, 0.f, 0.f, 0.f, 1.f, 0.f, -1);
+}
+
+// packed copy of the roadgraph points for the top-k observation
+__global__ void __launch_bounds__(256) k_pack_points(RgView g, int pts_pad, float2* pts) {
+  const int64_t o = (int64_t)blockIdx.y * g.R;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= pts_pad) return;
+  float2 v = make_float2(WM_FAR, WM_FAR);
+  if (i < g.R && g.valid[o + i] != 0) v = make_float2(g.x[o + i], g.y[o + i]);
+  pts[(int64_t)blockIdx.y * pts_pad + i] = v;
+}
+
+void wm_prepare_free(wm_handle* h) {
+  cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pts);
+  h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pts = nullptr;
+  h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0; h->pts_pad = 0;
+}
+
+int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s) {
+  const int B = rg->B, R = rg->R;
+  RgView g{rg->x, rg->y, rg->dir_x, rg->dir_y, rg->type, rg->id, rg->valid, R};
+  // Buffers are reused when the shapes fit, so device pointers (and a captured rollout graph)
+  // stay valid across scenarios of the same shape.
+  if (h->prep_B != B || h->prep_R != R) {
+    wm_drop_graph(h);
+    wm_prepare_free(h);
+    WM_CUDA(cudaMalloc(&h->n_seg, (size_t)B * sizeof(int32_t)));
+    h->pts_pad = (R + WM_PT_TILE - 1) / WM_PT_TILE * WM_PT_TILE;
+    WM_CUDA(cudaMalloc(&h->pts, (size_t)B * h->pts_pad * sizeof(float2)));
+    h->prep_B = B; h->prep_R = R;
+  }
+  k_count_segments<<<B, 256, 0, s>>>(g, h->n_seg);
+  h->launches++;
+  WM_CUDA(cudaGetLastError());
+  int32_t* host = (int32_t*)malloc((size_t)B * sizeof(int32_t));
+  if (!host) return WM_ERR_ARG;
+  cudaError_t e = cudaMemcpyAsync(host, h->n_seg, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  int mx = 0;
+  if (e == cudaSuccess) for (int b = 0; b < B; ++b) mx = host[b] > mx ? host[b] : mx;
+  free(host);
+  WM_CUDA(e);
+  h->seg_max = mx;
+  int tiles = (mx + WM_TILE_SEGS - 1) / WM_TILE_SEGS;
+  if (tiles < 1) tiles = 1;
+  if (tiles > h->seg_tiles || !h->edges) {       // grow only: seg_tiles is the row stride of `edges`
+    wm_drop_graph(h);
+    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src);
+    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr;
+    h->seg_tiles = tiles;
+    const size_t cap = (size_t)tiles * WM_TILE_SEGS;
+    WM_CUDA(cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES));
+    WM_CUDA(cudaMalloc(&h->sign_dir, (size_t)B * cap * sizeof(float2)));
+    WM_CUDA(cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t)));
+  }
+  k_fill_segments<<<B, 1024, 0, s>>>(g, h->seg_tiles, h->edges, h->sign_dir, h->seg_src);
+  h->launches++;
+  WM_CUDA(cudaGetLastError());
+  k_pack_points<<<dim3((h->pts_pad + 255) / 256, B), 256, 0, s>>>(g, h->pts_pad, h->pts);
+  h->launches++;
+  WM_CUDA(cudaGetLastError());
+  WM_CUDA(cudaStreamSynchronize(s));
+  if (n_segments_max) *n_segments_max = mx;
+  return WM_OK;
+}
+
+// ======================================================================================
+// k_offroad
+// ======================================================================================
+constexpr int OFF_THREADS = 512;
+constexpr int OFF_WARPS = OFF_THREADS / 32;
+constexpr int OFF_NA = 2;                  // agents per warp unit (8 corners in registers)
+
+struct OffroadParams {
+  wm_row row;
+  int A;
+  const float4* edges; const float2* sign_dir; const int32_t* n_seg;
+  int seg_tiles;          // tiles per scenario in `edges`
+  int tiles_per_buf;      // capacity of one shared-memory buffer, in tiles
+  float* sd; int64_t sd_stride_b;
+  float* corner;          // [B][4][A] or NULL
+  uint8_t* flag; int64_t flag_stride_b;
+};
+
+// shared-memory carve-up (dynamic): [bars 16 B][agent SoA 6*Ap floats][aidx Ap ints][keys 4*Ap u64][buffers]
+__host__ __device__ inline size_t off_fixed_bytes(int A) {
+  const size_t Ap = (size_t)((A + 31) / 32) * 32;
+  size_t n = 128 + Ap * 6 * 4 + Ap * 4 + Ap * 4 * 8;
+  return (n + 127) / 128 * 128;
+}
+
+// distance^2 of one corner to one segment, the arithmetic both the scan and the re-scan use
+__device__ __forceinline__ float seg_d2(float wx, float wy, float ex, float ey, float gx, float gy) {
+  const float t = __saturatef(fmaf(wy, gy, wx * gx));
+  const float rx = fmaf(-t, ex, wx), ry = fmaf(-t, ey, wy);
+  return fmaf(ry, ry, rx * rx);
+}
+
+__global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int A = p.A, Ap = ((A + 31) / 32) * 32;
+  uint64_t* bars = (uint64_t*)smem_raw;                       // [2] full barriers
+  int* s_misc = (int*)(smem_raw + 16);                        // [0] nvalid, [1..] scan scratch
+  float* s_ag = (float*)(smem_raw + 128);                     // [6][Ap] cx, cy, ax, ay, bx, by (compacted)
+  int* s_aidx = (int*)(s_ag + 6 * Ap);                        // [Ap] compact -> agent slot
+  wm_u64* s_key = (wm_u64*)(s_aidx + Ap);                     // [4*Ap] (d2 bits << 32) | run id
+  float4* s_buf = (float4*)(smem_raw + off_fixed_bytes(A));   // 2 x tiles_per_buf tiles
+
+  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nseg = p.n_seg[b];
+  const int nt = (nseg + WM_TILE_SEGS - 1) / WM_TILE_SEGS;    // tiles of this scenario
+  const int G = (nt + p.tiles_per_buf - 1) / p.tiles_per_buf; // tile groups
+  const int TB = G > 0 ? (nt + G - 1) / G : 0;                // balanced tiles per group
+  const float4* edges_b = p.edges + (int64_t)b * p.seg_tiles * WM_TILE_F4;
+
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  // ---- producer: start the first two groups (overlaps with the agent set-up below) ----
+  if (tid == 0) {
+    for (int g = 0; g < 2 && g < G; ++g) {
+      const int t0 = g * TB, n = min(TB, nt - t0);
+      mbar_expect_tx(&bars[g], (uint32_t)n * WM_TILE_BYTES);
+      for (int t = 0; t < n; ++t)
+        tma_load_1d(s_buf + ((int64_t)g * p.tiles_per_buf + t) * WM_TILE_F4, edges_b + (int64_t)(t0 + t) * WM_TILE_F4, WM_TILE_BYTES, &bars[g]);
+    }
+  }
+
+  // ---- agent set-up: order-preserving compaction of valid agents, corner offsets ----
+  const int64_t ro = (int64_t)b * p.row.stride_b;
+  if (tid == 0) s_misc[0] = 0;
+  __syncthreads();
+  for (int base = 0; base < Ap; base += OFF_THREADS) {
+    const int a = base + tid;
+    const bool v = a < A && p.row.valid[ro + a] != 0;
+    const uint32_t bal = __ballot_sync(0xffffffffu, v);
+    if (lane == 0) s_misc[1 + warp] = __popc(bal);
+    __syncthreads();
+    int pre = s_misc[0];
+    for (int w = 0; w < warp; ++w) pre += s_misc[1 + w];
+    if (v) {
+      const int ci = pre + __popc(bal & ((1u << lane) - 1u));
+      const float x = p.row.x[ro + a], y = p.row.y[ro + a];
+      float sn, cs;
+      sincosf(p.row.yaw[ro + a], &sn, &cs);
+      const float hl = 0.5f * p.row.length[ro + a], hw = 0.5f * p.row.width[ro + a];
+      const float hfx = hl * cs, hfy = hl * sn, hsx = -hw * sn, hsy = hw * cs;
+      s_ag[0 * Ap + ci] = x;          s_ag[1 * Ap + ci] = y;
+      s_ag[2 * Ap + ci] = hfx + hsx;  s_ag[3 * Ap + ci] = hfy + hsy;   // a: front-left offset
+      s_ag[4 * Ap + ci] = hfx - hsx;  s_ag[5 * Ap + ci] = hfy - hsy;   // b: front-right offset
+      s_aidx[ci] = a;
+    } else if (a < A) {                                                 // D10: zeros for invalid agents
+      p.sd[(int64_t)b * p.sd_stride_b + a] = 0.f;
+      p.flag[(int64_t)b * p.flag_stride_b + a] = 0;
+      if (p.corner) for (int k = 0; k < 4; ++k) p.corner[((int64_t)b * 4 + k) * A + a] = 0.f;
+    }
+    __syncthreads();
+    if (tid == 0) { int tot = 0; for (int w = 0; w < OFF_WARPS; ++w) tot += s_misc[1 + w]; s_misc[0] += tot; }
+    __syncthreads();
+  }
+  const int nvalid = s_misc[0];
+  for (int i = tid; i < 4 * nvalid; i += OFF_THREADS) s_key[i] = ~0ull;
+  __syncthreads();
+
+  // ---- scan ----
+  const int nunits = (nvalid + OFF_NA - 1) / OFF_NA;
+  for (int g = 0; g < G; ++g) {
+    const int t0 = g * TB, ntg = min(TB, nt - t0);
+    const int ncells = nunits * ntg;
+    const int c_begin = (int)(((long long)warp * ncells) / OFF_WARPS);
+    const int c_end = (int)(((long long)(warp + 1) * ncells) / OFF_WARPS);
+    // every warp waits, cells or not: no bulk copy may be in flight when the buffers are
+    // recycled or the CTA exits
+    mbar_wait(&bars[g & 1], (uint32_t)((g >> 1) & 1));
+    const float4* buf = s_buf + (int64_t)(g & 1) * p.tiles_per_buf * WM_TILE_F4;
+
+    int cur_u = -1;
+    float cx[OFF_NA], cy[OFF_NA], ax[OFF_NA], ay[OFF_NA], bx[OFF_NA], by[OFF_NA];
+    float best[OFF_NA * 4];
+    int brun[OFF_NA * 4];
+
+    auto flush = [&]() {
+      if (cur_u < 0) return;
+#pragma unroll
+      for (int k = 0; k < OFF_NA * 4; ++k) {
+        const int ci = cur_u * OFF_NA + (k >> 2);
+        const uint32_t bits = __float_as_uint(best[k]);
+        const uint32_t m = __reduce_min_sync(0xffffffffu, bits);
+        const uint32_t cand = bits == m ? (uint32_t)brun[k] * 32u + (uint32_t)lane : 0xffffffffu;
+        const uint32_t r = __reduce_min_sync(0xffffffffu, cand);
+        if (lane == 0 && ci < nvalid) atomicMin(&s_key[ci * 4 + (k & 3)], ((wm_u64)m << 32) | r);
+      }
+    };
+
+    for (int c = c_begin; c < c_end; ++c) {
+      const int u = c / ntg, tl = c - u * ntg;
+      if (u != cur_u) {
+        flush();
+        cur_u = u;
+#pragma unroll
+        for (int n = 0; n < OFF_NA; ++n) {
+          const int ci = min(u * OFF_NA + n, nvalid - 1);    // odd tail: duplicate (result dropped)
+          cx[n] = s_ag[0 * Ap + ci]; cy[n] = s_ag[1 * Ap + ci];
+          ax[n] = s_ag[2 * Ap + ci]; ay[n] = s_ag[3 * Ap + ci];
+          bx[n] = s_ag[4 * Ap + ci]; by[n] = s_ag[5 * Ap + ci];
+        }
+#pragma unroll
+        for (int k = 0; k < OFF_NA * 4; ++k) { best[k] = __int_as_float(0x7f800000); brun[k] = 0; }
+      }
+      const float4* tp = buf + (int64_t)tl * WM_TILE_F4 + lane;
+      float cm[OFF_NA * 4];
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        const float4 P = tp[(it * 3 + 0) * 32], E = tp[(it * 3 + 1) * 32], Gv = tp[(it * 3 + 2) * 32];
+        const wm_u64 Px = pk2(P.x, P.y), Py = pk2(P.z, P.w), Ex = pk2(E.x, E.y), Ey = pk2(E.z, E.w), Gx = pk2(Gv.x, Gv.y);
+#pragma unroll
+        for (int n = 0; n < OFF_NA; ++n) {
+          const wm_u64 wcx = sub2(pk2(cx[n], cx[n]), Px), wcy = sub2(pk2(cy[n], cy[n]), Py);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            wm_u64 wx, wy;
+            if (k == 0)      { wx = add2(wcx, pk2(ax[n], ax[n])); wy = add2(wcy, pk2(ay[n], ay[n])); }
+            else if (k == 1) { wx = add2(wcx, pk2(bx[n], bx[n])); wy = add2(wcy, pk2(by[n], by[n])); }
+            else if (k == 2) { wx = sub2(wcx, pk2(ax[n], ax[n])); wy = sub2(wcy, pk2(ay[n], ay[n])); }
+            else             { wx = sub2(wcx, pk2(bx[n], bx[n])); wy = sub2(wcy, pk2(by[n], by[n])); }
+            const wm_u64 tm = mul2(wx, Gx);
+            float tl0, tl1, wy0, wy1;
+            upk2(tm, tl0, tl1); upk2(wy, wy0, wy1);
+            const float t0s = __saturatef(fmaf(wy0, Gv.z, tl0)), t1s = __saturatef(fmaf(wy1, Gv.w, tl1));
+            const wm_u64 nt2 = pk2(-t0s, -t1s);
+            const wm_u64 rx = fma2(nt2, Ex, wx), ry = fma2(nt2, Ey, wy);
+            const wm_u64 d2 = fma2(ry, ry, mul2(rx, rx));
+            float d0, d1;
+            upk2(d2, d0, d1);
+            if (it == 0) cm[n * 4 + k] = fminf(d0, d1); else cm[n * 4 + k] = min3f(cm[n * 4 + k], d0, d1);
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < OFF_NA * 4; ++k) {
+        if (cm[k] < best[k]) brun[k] = t0 + tl;
+        best[k] = fminf(best[k], cm[k]);
+      }
+    }
+    flush();
+    if (g + 2 < G) {                       // recycle this buffer for group g+2
+      __syncthreads();
+      if (tid == 0) {
+        fence_proxy_async();
+        const int g2 = g + 2, t2 = g2 * TB, n2 = min(TB, nt - t2);
+        mbar_expect_tx(&bars[g & 1], (uint32_t)n2 * WM_TILE_BYTES);
+        for (int t = 0; t < n2; ++t)
+          tma_load_1d(s_buf + ((int64_t)(g & 1) * p.tiles_per_buf + t) * WM_TILE_F4, edges_b + (int64_t)(t2 + t) * WM_TILE_F4, WM_TILE_BYTES, &bars[g & 1]);
+      }
+    }
+  }
+  __syncthreads();
+
+  // ---- finalize: exact segment inside the winning run, sign, signed distance ----
+  float* s_csd = (float*)s_buf;            // [4*nvalid] corner signed distances (buffers are free now)
+  for (int i = tid; i < 4 * nvalid; i += OFF_THREADS) {
+    const int ci = i >> 2, k = i & 3;
+    float sd = -FLT_MAX;                                                   // D20
+    if (nseg > 0) {
+      const uint32_t run = (uint32_t)(s_key[i] & 0xffffffffull);
+      const int tau = (int)(run >> 5), ln = (int)(run & 31u);
+      const float offx = (k & 1) ? s_ag[4 * Ap + ci] : s_ag[2 * Ap + ci];
+      const float offy = (k & 1) ? s_ag[5 * Ap + ci] : s_ag[3 * Ap + ci];
+      const float sgn = (k & 2) ? -1.f : 1.f;
+      const float qx = s_ag[0 * Ap + ci], qy = s_ag[1 * Ap + ci];
+      const float4* tp = edges_b + (int64_t)tau * WM_TILE_F4 + ln;
+      float bd2 = __int_as_float(0x7f800000), bwx = 0.f, bwy = 0.f;
+      int bj = 0;
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        const float4 P = __ldg(&tp[(it * 3 + 0) * 32]), E = __ldg(&tp[(it * 3 + 1) * 32]), Gv = __ldg(&tp[(it * 3 + 2) * 32]);
+        const float w0x = fmaf(sgn, offx, qx - P.x), w0y = fmaf(sgn, offy, qy - P.z);
+        const float w1x = fmaf(sgn, offx, qx - P.y), w1y = fmaf(sgn, offy, qy - P.w);
+        const float d0 = seg_d2(w0x, w0y, E.x, E.z, Gv.x, Gv.z);
+        const float d1 = seg_d2(w1x, w1y, E.y, E.w, Gv.y, Gv.w);
+        if (d0 < bd2) { bd2 = d0; bwx = w0x; bwy = w0y; bj = 2 * it; }
+        if (d1 < bd2) { bd2 = d1; bwx = w1x; bwy = w1y; bj = 2 * it + 1; }
+      }
+      const int s = tau * WM_TILE_SEGS + ln * WM_RUN + bj;
+      const float2 sdir = __ldg(&p.sign_dir[(int64_t)b * p.seg_tiles * WM_TILE_SEGS + s]);
+      const float side = fmaf(sdir.x, bwy, -sdir.y * bwx);                 // e x (q - p0), D16
+      const float d = sqrtf(bd2);
+      sd = side > 0.f ? -d : d;                                            // left = on-road = negative
+    }
+    s_csd[i] = sd;
+    if (p.corner) p.corner[((int64_t)b * 4 + k) * A + s_aidx[ci]] = sd;
+  }
+  __syncthreads();
+  for (int ci = tid; ci < nvalid; ci += OFF_THREADS) {
+    const float m = fmaxf(fmaxf(s_csd[4 * ci], s_csd[4 * ci + 1]), fmaxf(s_csd[4 * ci + 2], s_csd[4 * ci + 3]));  // D18
+    const int a = s_aidx[ci];
+    p.sd[(int64_t)b * p.sd_stride_b + a] = m;
+    p.flag[(int64_t)b * p.flag_stride_b + a] = (uint8_t)(m > 0.f);         // D19
+  }
+}
+
+cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
+                              float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s) {
+  OffroadParams p;
+  p.row = wm_make_row(sim, t);
+  p.A = sim.A;
+  p.edges = h->edges; p.sign_dir = h->sign_dir; p.n_seg = h->n_seg; p.seg_tiles = h->seg_tiles;
+  p.sd = sd; p.sd_stride_b = sd_stride_b; p.corner = corner; p.flag = flag; p.flag_stride_b = flag_stride_b;
+  const size_t fixed = off_fixed_bytes(sim.A);
+  const size_t max_smem = 227 * 1024;
+  int tpb = (int)((max_smem - fixed) / (2 * (size_t)WM_TILE_BYTES));
+  const int need = (h->seg_tiles + 1) / 2;        // two buffers hold the whole scenario if they can
+  if (tpb > need) tpb = need;
+  if (tpb < 1) tpb = 1;
+  p.tiles_per_buf = tpb;
+  const size_t smem = fixed + 2 * (size_t)tpb * WM_TILE_BYTES;
+  static size_t configured = 0;
+  if (smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_offroad, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem);
+    if (e != cudaSuccess) return e;
+    configured = max_smem;
+  }
+  k_offroad<<<sim.B, OFF_THREADS, smem, s>>>(p);
+  h->launches++;
+  return cudaGetLastError();
+}

@@ -1,0 +1,256 @@
+"""-m gpu parity tests: the CUDA path (through the C-ABI) against the CPU oracle, element by
+element on the same seeded inputs."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import wm_scenarios as ws
+import paper_2310_08710_b200 as wm
+from gpu_util import (dev, host, row_of, assert_state_close, gpu_offroad, compare_offroad, gpu_overlap,
+                      compare_overlap, ang_diff, DIST_REL, DIST_ABS)
+
+pytestmark = pytest.mark.gpu
+
+DYN = {"bicycle": (wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE),
+       "delta_local": (wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL)}
+
+
+@pytest.fixture(scope="module")
+def cfg1():
+    return ws.make_config(1)
+
+
+def _setup(cfg, dynamics="bicycle", **kw):
+    h = wm.wm_create(dynamics=DYN[dynamics][0], **kw)
+    log_d, rg_d = dev(cfg["log"]), dev(cfg["roadgraph"])
+    nseg = wm.wm_prepare(h, rg_d)
+    sim_d = wm.empty_traj_like(log_d)
+    return h, log_d, rg_d, sim_d, nseg
+
+
+# ---------------------------------------------------------------- prepare / reset
+def test_prepare_segment_counts_match_oracle(cfg1):
+    for cfg in (cfg1, ws.make_config(5, B=3, n_steps=1), ws.make_config(4, B=2)):
+        h, log_d, rg_d, sim_d, nseg = _setup(cfg)
+        B = cfg["log"]["x"].shape[0]
+        counts = wm.wm_segment_counts(h, B)
+        exp = [oracle.count_segments(cfg["roadgraph"], b) for b in range(B)]
+        assert counts == exp and nseg == max(exp)
+        wm.wm_destroy(h)
+
+
+def test_reset_matches_oracle(cfg1):
+    h, log_d, rg_d, sim_d, _ = _setup(cfg1)
+    for k in sim_d:
+        sim_d[k].fill_(3)
+    t = wm.wm_reset(h, log_d, sim_d)
+    assert t == 10
+    ref = oracle.reset(cfg1["log"])
+    got = host(sim_d)
+    for k in ref:
+        assert np.array_equal(got[k], ref[k], equal_nan=True), k
+    wm.wm_destroy(h)
+
+
+# ---------------------------------------------------------------- dynamics
+@pytest.mark.parametrize("cfgid,dyn", [(1, "bicycle"), (2, "delta_local"), (5, "bicycle")])
+def test_single_step_matches_oracle(cfgid, dyn):
+    cfg = ws.make_config(cfgid, B=None if cfgid == 1 else 24, n_steps=2 if cfgid == 5 else None)
+    h, log_d, rg_d, sim_d, _ = _setup(cfg, dyn)
+    t = wm.wm_reset(h, log_d, sim_d)
+    act = np.ascontiguousarray(cfg["actions"][:, 0]); av = np.ascontiguousarray(cfg["action_valid"][:, 0])
+    av[:, ::5] = 0                                             # some agents on log playback (D8)
+    wm.wm_step(h, log_d, sim_d, t, torch.from_numpy(act).cuda(), torch.from_numpy(av).cuda())
+    torch.cuda.synchronize()
+    sim_o = oracle.reset(cfg["log"])
+    oracle.step(cfg["log"], sim_o, t, DYN[dyn][1], act, av)
+    got = host(sim_d)
+    assert_state_close(row_of(got, t + 1), row_of(sim_o, t + 1))
+    pb = (av == 0) | (cfg["log"]["valid"][:, t] == 0)          # playback slots are bit copies of the log
+    for k in got:
+        assert np.array_equal(got[k][:, t + 1][pb], cfg["log"][k][:, t + 1][pb], equal_nan=True)
+    assert np.array_equal(got["valid"][:, t + 2:], np.zeros_like(got["valid"][:, t + 2:]))
+    wm.wm_destroy(h)
+
+
+def test_step_action_clipping_and_disabled_clipping(cfg1):
+    act = np.ascontiguousarray(cfg1["actions"][:, 0]) * np.float32(40.0)      # far outside 6 / 0.3
+    av = np.ascontiguousarray(cfg1["action_valid"][:, 0])
+    for lim in ((6.0, 0.3), (0.0, 0.0)):
+        h, log_d, rg_d, sim_d, _ = _setup(cfg1, max_accel=lim[0], max_curvature=lim[1])
+        t = wm.wm_reset(h, log_d, sim_d)
+        wm.wm_step(h, log_d, sim_d, t, torch.from_numpy(act).cuda(), torch.from_numpy(av).cuda())
+        sim_o = oracle.reset(cfg1["log"])
+        oracle.step(cfg1["log"], sim_o, t, oracle.DYN_BICYCLE, act, av, max_accel=lim[0], max_curvature=lim[1])
+        assert_state_close(row_of(host(sim_d), t + 1), row_of(sim_o, t + 1), pos_tol=2e-4, vel_tol=5e-3)
+        wm.wm_destroy(h)
+
+
+# ---------------------------------------------------------------- metrics on a given row
+@pytest.mark.parametrize("cfgid,B", [(1, 4), (2, 12), (4, 6), (5, 12)])
+def test_overlap_matches_oracle(cfgid, B):
+    cfg = ws.make_config(cfgid, B=B) if cfgid != 5 else ws.make_config(5, B=B, n_steps=1)
+    h, log_d, rg_d, sim_d, _ = _setup(cfg)
+    t = cfg["t0"]
+    pair, fl = gpu_overlap(h, log_d, t)
+    orc = oracle.overlap(cfg["log"], t)
+    st = compare_overlap(pair, fl, orc, cfg["log"]["valid"][:, t])
+    print("overlap cfg%d: %s" % (cfgid, st))
+    if cfgid == 4:
+        assert st["overlap_frac"] > 0.002
+    wm.wm_destroy(h)
+
+
+@pytest.mark.parametrize("cfgid,B", [(1, 4), (2, 6), (4, 6), (5, 6)])
+def test_offroad_matches_oracle(cfgid, B):
+    cfg = ws.make_config(cfgid, B=B) if cfgid != 5 else ws.make_config(5, B=B, n_steps=1)
+    h, log_d, rg_d, sim_d, _ = _setup(cfg)
+    t = cfg["t0"]
+    sd, cd, fl = gpu_offroad(h, log_d, t)
+    orc = oracle.offroad(cfg["log"], t, cfg["roadgraph"])
+    st = compare_offroad(sd, cd, fl, orc, cfg["log"]["valid"][:, t])
+    print("offroad cfg%d: %s flagged=%d" % (cfgid, st, int(fl.sum())))
+    assert st["ambiguous"] < 0.2 * st["corners"]
+    assert 0 < fl.sum() < (cfg["log"]["valid"][:, t] == 1).sum()
+    wm.wm_destroy(h)
+
+
+def test_log_divergence_matches_oracle(cfg1):
+    h, log_d, rg_d, sim_d, _ = _setup(cfg1)
+    t = wm.wm_reset(h, log_d, sim_d)
+    act = torch.from_numpy(np.ascontiguousarray(cfg1["actions"][:, 0])).cuda()
+    av = torch.from_numpy(np.ascontiguousarray(cfg1["action_valid"][:, 0])).cuda()
+    wm.wm_step(h, log_d, sim_d, t, act, av)
+    B, T, A = cfg1["log"]["x"].shape
+    d = torch.zeros((B, A), device="cuda"); v = torch.zeros((B, A), dtype=torch.uint8, device="cuda")
+    wm.wm_log_divergence(h, log_d, sim_d, t + 1, d, v)
+    orc = oracle.log_divergence(cfg1["log"], host(sim_d), t + 1)
+    assert np.array_equal(v.cpu().numpy(), orc["valid"])
+    assert np.allclose(d.cpu().numpy(), orc["dist"], rtol=1e-5, atol=1e-6)
+    assert d.max().item() > 0
+    wm.wm_destroy(h)
+
+
+# ---------------------------------------------------------------- rollout (P16)
+def _rollout_parity(cfg, n_steps, check_every=1):
+    log, rg = cfg["log"], cfg["roadgraph"]
+    B, T, A = log["x"].shape
+    h, log_d, rg_d, sim_d, _ = _setup(cfg)
+    t0 = wm.wm_reset(h, log_d, sim_d)
+    acts = np.ascontiguousarray(cfg["actions"][:, :n_steps]); av = np.ascontiguousarray(cfg["action_valid"][:, :n_steps])
+    out_d = wm.alloc_rollout_out(B, n_steps, A)
+    wm.wm_rollout(h, log_d, sim_d, t0, n_steps, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out_d)
+    torch.cuda.synchronize()
+    got, out = host(sim_d), host(out_d)
+    # (i) free-running state: GPU vs oracle
+    sim_o = oracle.reset(log)
+    orc_out = oracle.rollout(log, sim_o, rg, t0, n_steps, oracle.DYN_BICYCLE, acts, av)
+    assert_state_close(row_of(got, t0 + 1), row_of(sim_o, t0 + 1))
+    assert_state_close(row_of(got, t0 + n_steps), row_of(sim_o, t0 + n_steps), pos_tol=1e-3, yaw_tol=1e-4, vel_tol=1e-2)
+    # (ii) metrics teacher-forced on the GPU's own rows
+    stats = dict(corners=0, ambiguous=0, pairs=0, pair_amb=0)
+    for s in range(0, n_steps, check_every):
+        t = t0 + s + 1
+        valid = got["valid"][:, t]
+        orc_off = oracle.offroad(got, t, rg)
+        vq = valid == 1
+        clean = vq & ~(orc_off["ambig"] == 1).any(axis=1)
+        assert np.array_equal(out["offroad"][:, s][clean], orc_off["flag"][clean]), "step %d" % s
+        err = np.abs(out["offroad_dist"][:, s][clean].astype(np.float64) - orc_off["signed_dist"][clean])
+        assert (err <= DIST_REL * np.abs(orc_off["signed_dist"][clean]) + DIST_ABS).all(), (s, err.max())
+        assert np.all(out["offroad"][:, s][~vq] == 0)
+        stats["corners"] += int(4 * vq.sum()); stats["ambiguous"] += int(((orc_off["ambig"] == 1) & vq[:, None, :]).sum())
+        orc_ov = oracle.overlap(got, t, want_pair=False)
+        cl = ~(np.abs(orc_ov["gap"]) < 1e-4).any(axis=2)
+        assert np.array_equal(out["overlap"][:, s][cl], orc_ov["flag"][cl]), "step %d" % s
+        stats["pairs"] += int(np.isfinite(orc_ov["gap"]).sum()); stats["pair_amb"] += int((np.abs(orc_ov["gap"]) < 1e-4).sum())
+        orc_ld = oracle.log_divergence(log, got, t)
+        assert np.allclose(out["log_div"][:, s], orc_ld["dist"], rtol=1e-5, atol=1e-6)
+    # aggregates (D21) from the GPU's own rows
+    assert np.array_equal(out["any_overlap"], out["overlap"].max(axis=1))
+    assert np.array_equal(out["any_offroad"], out["offroad"].max(axis=1))
+    ldv = (got["valid"][:, t0 + 1:t0 + 1 + n_steps] == 1) & (log["valid"][:, t0 + 1:t0 + 1 + n_steps] == 1)
+    cnt = ldv.sum(axis=1)
+    ade = np.where(cnt > 0, (out["log_div"].astype(np.float64) * ldv).sum(axis=1) / np.maximum(cnt, 1), 0)
+    assert np.allclose(out["ade"], ade, rtol=1e-5, atol=1e-6)
+    # free-running flags agree with the free-running oracle except near band / drifted cases
+    agree = (out["offroad"] == orc_out["offroad"]).mean()
+    assert agree > 0.995, agree
+    wm.wm_destroy(h)
+    return stats
+
+
+def test_rollout_config1_full():
+    st = _rollout_parity(ws.make_config(1), 80)
+    print("rollout cfg1:", st)
+
+
+def test_rollout_config5_sample():
+    st = _rollout_parity(ws.make_config(5, B=6, n_steps=80), 80, check_every=8)
+    print("rollout cfg5 sample:", st)
+
+
+def test_rollout_graph_replay_is_deterministic_and_matches_eager(cfg1):
+    log = cfg1["log"]
+    B, T, A = log["x"].shape
+    n = 20
+    h, log_d, rg_d, sim_d, _ = _setup(cfg1)
+    acts = torch.from_numpy(np.ascontiguousarray(cfg1["actions"][:, :n])).cuda()
+    av = torch.from_numpy(np.ascontiguousarray(cfg1["action_valid"][:, :n])).cuda()
+    outs = []
+    for rep in range(3):                              # 1st call captures, 2nd/3rd replay (P14)
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        out_d = wm.alloc_rollout_out(B, n, A) if rep == 0 else out_d
+        wm.wm_rollout(h, log_d, sim_d, t0, n, acts, av, out_d)
+        torch.cuda.synchronize()
+        outs.append((host(sim_d), host(out_d)))
+    for k in outs[0][0]:
+        assert np.array_equal(outs[0][0][k], outs[2][0][k], equal_nan=True)
+    for k in outs[0][1]:
+        assert np.array_equal(outs[0][1][k], outs[2][1][k])
+    # eager: the individual entry points, step by step
+    sim_e = wm.empty_traj_like(log_d)
+    t0 = wm.wm_reset(h, log_d, sim_e)
+    sd = torch.zeros((B, A), device="cuda"); fl = torch.zeros((B, A), dtype=torch.uint8, device="cuda")
+    ov = torch.zeros((B, A), dtype=torch.uint8, device="cuda")
+    ld = torch.zeros((B, A), device="cuda"); lv = torch.zeros((B, A), dtype=torch.uint8, device="cuda")
+    for s in range(n):
+        wm.wm_step(h, log_d, sim_e, t0 + s, acts[:, s].contiguous(), av[:, s].contiguous())
+        wm.wm_metrics_overlap(h, sim_e, t0 + s + 1, None, ov)
+        wm.wm_metrics_offroad(h, sim_e, t0 + s + 1, sd, None, fl)
+        wm.wm_log_divergence(h, log_d, sim_e, t0 + s + 1, ld, lv)
+        torch.cuda.synchronize()
+        assert np.array_equal(ov.cpu().numpy(), outs[0][1]["overlap"][:, s])
+        assert np.array_equal(fl.cpu().numpy(), outs[0][1]["offroad"][:, s])
+        assert np.array_equal(sd.cpu().numpy(), outs[0][1]["offroad_dist"][:, s])
+        assert np.array_equal(ld.cpu().numpy(), outs[0][1]["log_div"][:, s])
+    got_e = host(sim_e)
+    for k in got_e:
+        assert np.array_equal(got_e[k], outs[0][0][k], equal_nan=True)
+    assert wm.wm_kernel_launches(h) > 3 * (3 * n + 1)
+    wm.wm_destroy(h)
+
+
+def test_rollout_host_matches_device_rollout(cfg1):
+    log, rg = cfg1["log"], cfg1["roadgraph"]
+    B, T, A = log["x"].shape
+    n = 30
+    h, log_d, rg_d, sim_d, _ = _setup(cfg1)
+    t0 = wm.wm_reset(h, log_d, sim_d)
+    acts = np.ascontiguousarray(cfg1["actions"][:, :n]); av = np.ascontiguousarray(cfg1["action_valid"][:, :n])
+    out_d = wm.alloc_rollout_out(B, n, A)
+    wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out_d)
+    torch.cuda.synchronize()
+    h2 = wm.wm_create()
+    pin = lambda d: {k: torch.from_numpy(v).pin_memory() for k, v in d.items()}
+    out_h = wm.alloc_rollout_out(B, n, A, device="cpu", pin=True)
+    sim_h = {k: torch.zeros_like(v).pin_memory() for k, v in pin(log).items()}
+    for rep in range(2):
+        wm.wm_rollout_host(h2, pin(log), pin(rg), n, torch.from_numpy(acts).pin_memory(),
+                           torch.from_numpy(av).pin_memory(), out_h, sim_h)
+    for k, v in host(out_d).items():
+        assert np.array_equal(v, out_h[k].numpy()), k
+    for k, v in host(sim_d).items():
+        assert np.array_equal(v, sim_h[k].numpy(), equal_nan=True), k
+    wm.wm_destroy(h); wm.wm_destroy(h2)

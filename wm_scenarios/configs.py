@@ -312,9 +312,9 @@ def make_config4(seed=None, b_ids=None, B=None, poison_invalid=True):
     z = np.zeros((Bn, A, 1))
     _fill_traj(log, slice(0, Bn), x[..., None], y[..., None], yaw[..., None], z, z, length, width,
                valid, poison_invalid)
-    # lot boundary: rectangle [-3,51] x [-3,195], counter-clockwise (interior on the left),
+    # lot boundary: rectangle [-1,49] x [-1,193] (1 m margin, so border cars can poke out), counter-clockwise (interior on the left),
     # one open polyline of R points at perimeter/R spacing (last gap stays open).
-    x0, x1, y0, y1 = -3.0, 51.0, -3.0, 195.0
+    x0, x1, y0, y1 = -1.0, 49.0, -1.0, 193.0
     w, h = x1 - x0, y1 - y0
     per = 2 * (w + h)
     s = np.arange(R) * (per / R)
