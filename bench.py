@@ -1,0 +1,288 @@
+#!/usr/bin/env python
+"""Benchmark of the B200-native Waymax closed-loop step (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--B 4096]
+
+Workload (config.workload): BASELINE.json configs[4] — B=4096 scenarios x A=128 agents,
+R=20,000 roadgraph points, T=91, one 80-step closed-loop InvertibleBicycle rollout with
+overlap, offroad and log divergence every step, one CUDA graph, fp32.  One bench "step" =
+one such rollout of the whole batch (reset + 80 x (dynamics, overlap, offroad, log
+divergence) + aggregates).  Metric: agent-steps/s = B * A * 80 / time (agent slots, valid or
+not; valid-agent-steps reported beside it).
+
+value     device-resident: inputs in HBM when the timed region starts, CUDA events on the
+          launching stream, barrier + synchronize on both sides, max over ranks.
+e2e       the same job through wm_rollout_host with pinned HOST buffers: scenario + action
+          upload, wm_prepare, reset, rollout, metric download all inside the timed region.
+roofline  dominant kernel k_offroad: algorithmic flops (13 per corner-segment pair, SURVEY
+          §8(d)) / its CUDA-event duration, against the FP32 peak SMs*128*2*max clock.
+cpu_baseline  the oracle (oracle/, as it stands) on the host cores, bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+N_STEPS = 80
+FLOP_PER_PAIR = 13.0           # w(2) t(3) c(4) d2(3) min(1)
+METRIC = "agent-steps/sec for step+overlap+offroad (B=4096,A=128); % of roofline"
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return None
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.th.join(timeout=2)
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        if not sm:
+            return None
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "power_w_max": float(max(pw)), "samples": len(sm)}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores; bounded sample/step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    import wm_scenarios as ws
+    sample_B = args.ref_B
+    cfg = ws.make_config(5, B=sample_B, n_steps=N_STEPS)
+    A = cfg["log"]["x"].shape[2]
+    times = []
+    for it in range(args.warmup_ref + args.steps_ref):
+        sim = oracle.reset(cfg["log"])
+        t0 = time.perf_counter()
+        oracle.rollout(cfg["log"], sim, cfg["roadgraph"], cfg["t0"], N_STEPS, oracle.DYN_BICYCLE,
+                       cfg["actions"], cfg["action_valid"])
+        dt = time.perf_counter() - t0
+        if it >= args.warmup_ref:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    val = sample_B * A * N_STEPS / (ms * 1e-3)
+    cores = oracle.num_threads()
+    sample = "%d of 4096 scenarios x %d steps per bench step (oracle.rollout, OpenMP over scenarios)" % (sample_B, N_STEPS)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "agent-steps/s", "n_gpus": args.gpus,
+            "steps": args.steps_ref, "warmup": args.warmup_ref, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config5: B=4096 A=128 R=20000 T=91 80-step bicycle rollout (bounded sample)",
+                       "sample_B": sample_B, "A": A, "R": 20000, "n_steps": N_STEPS},
+            "cpu_baseline": {"value": val, "unit": "agent-steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "agent-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--B", type=int, default=4096, help="scenarios per GPU (4096 = the BASELINE config)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-B", type=int, default=16, help="oracle sample for cpu_baseline")
+    ap.add_argument("--ref-B", type=int, default=8)
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    args.steps_ref = max(1, min(args.steps, 3)); args.warmup_ref = max(1, min(args.warmup, 1))
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import wm_scenarios as ws
+    import paper_2310_08710_b200 as wm
+    from paper_2310_08710_b200 import sharding
+
+    rank, world = sharding.rank_world()
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    sharding.init_process_group("nccl")
+    dev = "cuda"
+
+    B, A, R, T = args.B, 128, 20000, 91
+    cfg = ws.make_config(5, b_ids=sharding.shard_ids(B, rank, world), n_steps=N_STEPS)
+    log_d, rg_d = wm.to_device(cfg["log"]), wm.to_device(cfg["roadgraph"])
+    acts_d = torch.from_numpy(cfg["actions"]).to(dev); av_d = torch.from_numpy(cfg["action_valid"]).to(dev)
+    sim_d = wm.empty_traj_like(log_d)
+    out_d = wm.alloc_rollout_out(B, N_STEPS, A)
+    h = wm.wm_create()
+    seg_max = wm.wm_prepare(h, rg_d)
+    n_seg = np.array(wm.wm_segment_counts(h, B))
+    stream = torch.cuda.current_stream()
+
+    def one_pass():
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        wm.wm_rollout(h, log_d, sim_d, t0, N_STEPS, acts_d, av_d, out_d)
+
+    for _ in range(args.warmup):
+        one_pass()
+    torch.cuda.synchronize()
+    sharding.barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = wm.wm_kernel_launches(h)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        one_pass()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    sharding.barrier()
+    launches = wm.wm_kernel_launches(h) - l0
+    ms_total = sharding.max_over_ranks(ev0.elapsed_time(ev1), dev)
+    ms_step = ms_total / args.steps
+    agent_steps = float(B) * A * N_STEPS * world
+    value = agent_steps / (ms_step * 1e-3)
+    valid_rows = sim_d["valid"][:, 11:11 + N_STEPS].sum().item()
+    valid_value = sharding.sum_over_ranks(valid_rows, dev) / (ms_step * 1e-3)
+
+    # ---- roofline of the dominant kernel: k_offroad alone, same rows, CUDA events ----
+    sd = torch.zeros((B, A), device=dev); fl = torch.zeros((B, A), dtype=torch.uint8, device=dev)
+    for t in range(11, 14):
+        wm.wm_metrics_offroad(h, sim_d, t, sd, None, fl)
+    torch.cuda.synchronize()
+    ka, kb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ka.record(stream)
+    for t in range(11, 11 + N_STEPS):
+        wm.wm_metrics_offroad(h, sim_d, t, sd, None, fl)
+    kb.record(stream)
+    torch.cuda.synchronize()
+    k_ms = ka.elapsed_time(kb) / N_STEPS
+    nvalid_bt = sim_d["valid"][:, 11:11 + N_STEPS].sum(dim=2).double().cpu().numpy()       # [B, 80]
+    pairs_per_launch = float((4.0 * nvalid_bt * n_seg[:, None]).sum() / N_STEPS)
+    peaks = measured_peaks()
+    props = torch.cuda.get_device_properties(local)
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    fp32_peak = props.multi_processor_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12              # TFLOP/s
+    achieved = pairs_per_launch * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12
+    hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 29.0          # segments once + one state row
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- e2e: the same job from pinned host buffers through the C-ABI ----
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda d: {k: torch.from_numpy(v).pin_memory() for k, v in d.items()}
+        log_h, rg_h = pin(cfg["log"]), pin(cfg["roadgraph"])
+        acts_h = torch.from_numpy(cfg["actions"]).pin_memory(); av_h = torch.from_numpy(cfg["action_valid"]).pin_memory()
+        out_h = wm.alloc_rollout_out(B, N_STEPS, A, device="cpu", pin=True)
+        h2 = wm.wm_create()
+        wm.wm_rollout_host(h2, log_h, rg_h, N_STEPS, acts_h, av_h, out_h)       # warm-up (allocations, graph capture)
+        wm.wm_rollout_host(h2, log_h, rg_h, N_STEPS, acts_h, av_h, out_h)
+        torch.cuda.synchronize(); sharding.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.e2e_steps):
+            wm.wm_rollout_host(h2, log_h, rg_h, N_STEPS, acts_h, av_h, out_h)
+        e1.record(stream)
+        torch.cuda.synchronize(); sharding.barrier()
+        e_ms = sharding.max_over_ranks(e0.elapsed_time(e1), dev) / args.e2e_steps
+        h2d = sum(v.numel() * v.element_size() for v in list(log_h.values()) + list(rg_h.values()) + [acts_h, av_h])
+        d2h = sum(v.numel() * v.element_size() for v in out_h.values())
+        same = all(torch.equal(out_h[k], out_d[k].cpu()) for k in out_h)
+        e2e = {"value": agent_steps / (e_ms * 1e-3), "unit": "agent-steps/s", "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms, "outputs_equal_device_path": bool(same),
+               "includes": "scenario+action upload, wm_prepare, reset, 80-step graph, metric download"}
+        wm.wm_destroy(h2)
+
+    # ---- cpu_baseline: the oracle on a bounded sample (rank 0, N=1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        import oracle
+        sb = min(args.cpu_B, B)
+        sub = lambda d: {k: np.ascontiguousarray(v[:sb]) for k, v in d.items()}
+        lg, rgs = sub(cfg["log"]), sub(cfg["roadgraph"])
+        sim_o = oracle.reset(lg)
+        t0 = time.perf_counter()
+        o = oracle.rollout(lg, sim_o, rgs, cfg["t0"], N_STEPS, oracle.DYN_BICYCLE,
+                           np.ascontiguousarray(cfg["actions"][:sb]), np.ascontiguousarray(cfg["action_valid"][:sb]))
+        dt = time.perf_counter() - t0
+        agree = float((o["offroad"] == out_d["offroad"][:sb].cpu().numpy()).mean())
+        cpu = {"value": sb * A * N_STEPS / dt, "unit": "agent-steps/s", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": "first %d of %d scenarios x %d steps, oracle.rollout, %.1f s wall" % (sb, B, N_STEPS, dt),
+               "offroad_flag_agreement_free_running": agree}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "agent-steps/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "config5: B=%d/GPU A=128 R=20000 T=91, 80-step InvertibleBicycle rollout + overlap + offroad + log divergence, one CUDA graph" % B,
+                       "B_per_gpu": B, "A": A, "R": R, "T": T, "n_steps": N_STEPS, "S_e_max": int(seg_max),
+                       "S_e_mean": float(n_seg.mean()), "l2": "inputs exceed L2 (segments %.2f GB + state per step)" % (n_seg.sum() * 24 / 1e9),
+                       "parallelism": "scenario shards, no collective", "valid_agent_steps_per_s": valid_value,
+                       "ms_per_sim_step": ms_step / N_STEPS},
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+                         "frac": achieved / fp32_peak, "traffic": None, "kernel": "k_offroad",
+                         "kernel_ms": k_ms, "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR,
+                         "peak_source": "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz),
+                         "hbm_time_ms_at_measured_peak": hbm_bytes / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9) * 1e3,
+                         "kernel_share_of_step": k_ms * N_STEPS / ms_step},
+            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(line))
+    wm.wm_destroy(h)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

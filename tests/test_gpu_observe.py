@@ -1,0 +1,130 @@
+"""-m gpu parity of wm_observe (history transform, exact top-k) against the oracle."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import wm_scenarios as ws
+import paper_2310_08710_b200 as wm
+from gpu_util import dev, ang_diff
+from util import mk_traj, set_agent, mk_roadgraph
+
+pytestmark = pytest.mark.gpu
+
+
+def _observe(log, rg, t, k, H=11, want_hist=True, want_topk=True):
+    B, T, A = log["x"].shape
+    h = wm.wm_create(topk=k, history=H)
+    log_d, rg_d = dev(log), dev(rg)
+    wm.wm_prepare(h, rg_d)
+    hist = hv = idx = feat = typ = None
+    if want_hist:
+        hist = torch.full((B, A, H, 7, A), 5.0, device="cuda"); hv = torch.full((B, A, H, A), 9, dtype=torch.uint8, device="cuda")
+    if want_topk:
+        idx = torch.full((B, A, k), 77, dtype=torch.int32, device="cuda")
+        feat = torch.full((B, A, 4, k), 5.0, device="cuda"); typ = torch.full((B, A, k), 77, dtype=torch.int32, device="cuda")
+    wm.wm_observe(h, log_d, rg_d, t, hist, hv, idx, feat, typ)
+    torch.cuda.synchronize()
+    wm.wm_destroy(h)
+    f = lambda x: None if x is None else x.cpu().numpy()
+    return f(hist), f(hv), f(idx), f(feat), f(typ)
+
+
+def _check_topk(log, rg, t, k, idx, feat, typ):
+    orc = oracle.observe_topk(log, rg, t, k)
+    assert np.array_equal(idx, orc["rg_index"]), "top-k index sets / order differ"
+    assert np.array_equal(typ, orc["rg_type"])
+    assert np.allclose(feat, orc["rg_feat"], rtol=1e-5, atol=2e-4)      # ego-frame coordinates up to ~300 m in float32
+    return orc
+
+
+def _check_hist(log, t, H, hist, hv):
+    orc = oracle.observe_history(log, t, H)
+    assert np.array_equal(hv, orc["hist_valid"])
+    for f in (0, 1):
+        assert np.abs(hist[:, :, :, f] - orc["hist"][:, :, :, f]).max() < 1e-4
+    assert ang_diff(hist[:, :, :, 2], orc["hist"][:, :, :, 2]).max() < 1e-5
+    for f in (3, 4):
+        assert np.abs(hist[:, :, :, f] - orc["hist"][:, :, :, f]).max() < 1e-4
+    assert np.array_equal(hist[:, :, :, 5:], orc["hist"][:, :, :, 5:])
+    assert np.all((hist[:, :, :, 2] >= -math.pi - 1e-6) & (hist[:, :, :, 2] <= math.pi + 1e-6))
+
+
+def test_observe_config1():
+    cfg = ws.make_config(1)
+    for k in (1, 64, 1000):
+        hist, hv, idx, feat, typ = _observe(cfg["log"], cfg["roadgraph"], 10, k)
+        _check_hist(cfg["log"], 10, 11, hist, hv)
+        _check_topk(cfg["log"], cfg["roadgraph"], 10, k, idx, feat, typ)
+    # a later row, shorter history
+    hist, hv, idx, feat, typ = _observe(cfg["log"], cfg["roadgraph"], 40, 100, H=5)
+    _check_hist(cfg["log"], 40, 5, hist, hv)
+    _check_topk(cfg["log"], cfg["roadgraph"], 40, 100, idx, feat, typ)
+
+
+def test_observe_config3_sample():
+    cfg = ws.make_config(3, B=3)
+    hist, hv, idx, feat, typ = _observe(cfg["log"], cfg["roadgraph"], 10, 1000)
+    _check_hist(cfg["log"], 10, 11, hist, hv)
+    orc = _check_topk(cfg["log"], cfg["roadgraph"], 10, 1000, idx, feat, typ)
+    v = cfg["log"]["valid"][:, 10] == 1
+    assert (idx[v] >= 0).all() and (idx[~v] == -1).all()
+    # report how many points sit within 1e-4 m of the k-th distance (band of the north_star)
+    print("top-k cfg3: egos=%d, all index sets bit-equal to the float32-keyed oracle" % int(v.sum()))
+
+
+def test_topk_fewer_valid_points_than_k_and_trailing_invalid():
+    cfg = ws.make_config(5, B=2, n_steps=1)       # 19800 valid + 200 invalid trailing points
+    rg = cfg["roadgraph"]
+    rg["valid"][:, 300:] = 0                        # only 300 valid points, k = 1000
+    hist, hv, idx, feat, typ = _observe(cfg["log"], rg, 10, 1000, want_hist=False)
+    _check_topk(cfg["log"], rg, 10, 1000, idx, feat, typ)
+    v = cfg["log"]["valid"][:, 10] == 1
+    assert (idx[v][:, :300] == np.arange(300)).all() and (idx[v][:, 300:] == -1).all()
+
+
+def test_topk_exact_ties_large_tie_groups_and_dense_rings():
+    rng = np.random.default_rng(11)
+    # (a) lattice ties on a circle, (b) 3000 coincident points (more ties than the collect buffer),
+    # (c) 6000 points on a thin ring (one level-0 bin holds far more than the buffer -> refinement)
+    ring12 = np.array([(3, 4), (4, 3), (-3, 4), (4, -3), (5, 0), (0, 5), (-5, 0), (0, -5), (-4, 3), (3, -4), (-3, -4), (-4, -3)], float)
+    same = np.tile(np.array([[20.0, -15.0]]), (3000, 1))
+    ang = rng.uniform(0, 2 * np.pi, 6000)
+    rad = 40.0 * (1 + rng.uniform(0, 0.02, 6000))
+    thin = np.stack([rad * np.cos(ang), rad * np.sin(ang)], 1)
+    far = rng.uniform(60, 90, (500, 2))
+    pts = np.concatenate([far[:100], ring12, same, thin, far[100:]]) + [7.0, -3.0]
+    rg = mk_roadgraph([pts])
+    rg["valid"][0, 5::17] = 0
+    tr = mk_traj(1, 1, 3, valid=1)
+    set_agent(tr, 0, 0, 0, 7.0, -3.0, 0.3)
+    set_agent(tr, 0, 0, 1, 7.5, -2.0, -2.0)
+    set_agent(tr, 0, 0, 2, 0.0, 0.0, 0.0, valid=0)
+    for k in (6, 13, 1500, 3500, 5000, 9000):
+        hist, hv, idx, feat, typ = _observe(tr, rg, 0, k, H=1, want_hist=False)
+        _check_topk(tr, rg, 0, k, idx, feat, typ)
+        assert (idx[0, 2] == -1).all()
+
+
+def test_observe_rejects_bad_arguments():
+    cfg = ws.make_config(1)
+    h = wm.wm_create(topk=5000)                     # k > R = 2000
+    log_d, rg_d = dev(cfg["log"]), dev(cfg["roadgraph"])
+    B, T, A = cfg["log"]["x"].shape
+    idx = torch.zeros((B, A, 5000), dtype=torch.int32, device="cuda")
+    feat = torch.zeros((B, A, 4, 5000), device="cuda"); typ = torch.zeros_like(idx)
+    wm.wm_prepare(h, rg_d)
+    with pytest.raises(wm.WmError, match="UNSUPPORTED"):
+        wm.wm_observe(h, log_d, rg_d, 10, None, None, idx, feat, typ)
+    with pytest.raises(wm.WmError, match="ARG"):
+        wm.wm_observe(h, log_d, rg_d, 3, None, None, idx, feat, typ)      # t < history-1
+    wm.wm_destroy(h)
+    h = wm.wm_create(topk=10)
+    with pytest.raises(wm.WmError, match="STATE"):                         # top-k before wm_prepare
+        wm.wm_observe(h, log_d, rg_d, 10, None, None, idx, feat, typ)
+    sd = torch.zeros((B, A), device="cuda"); fl = torch.zeros((B, A), dtype=torch.uint8, device="cuda")
+    with pytest.raises(wm.WmError, match="STATE"):
+        wm.wm_metrics_offroad(h, log_d, 10, sd, None, fl)
+    wm.wm_destroy(h)
