@@ -36,6 +36,16 @@ FLOP_PER_PAIR = 13.0           # w(2) t(3) c(4) d2(3) min(1)
 METRIC = "agent-steps/sec for step+overlap+offroad (B=4096,A=128); % of roofline"
 
 
+def profiled_traffic():
+    """dram__bytes_read+write per k_offroad launch from the latest committed ncu summary."""
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_k_offroad_traffic_bytes.txt")))
+    try:
+        return float(open(files[-1]).read().split()[0]) if files else None
+    except Exception:
+        return None
+
+
 def measured_peaks():
     try:
         return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -272,7 +282,7 @@ def main():
                        "parallelism": "scenario shards, no collective", "valid_agent_steps_per_s": valid_value,
                        "ms_per_sim_step": ms_step / N_STEPS},
             "roofline": {"bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                         "frac": achieved / fp32_peak, "traffic": None, "kernel": "k_offroad",
+                         "frac": achieved / fp32_peak, "traffic": profiled_traffic(), "kernel": "k_offroad",
                          "kernel_ms": k_ms, "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR,
                          "peak_source": "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz),
                          "hbm_time_ms_at_measured_peak": hbm_bytes / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9) * 1e3,
