@@ -14,7 +14,11 @@ value     device-resident: inputs in HBM when the timed region starts, CUDA even
           launching stream, barrier + synchronize on both sides, max over ranks.
 e2e       the same job through wm_rollout_host with pinned HOST buffers: scenario + action
           upload, wm_prepare, reset, rollout, metric download all inside the timed region.
-roofline  dominant kernel k_offroad: algorithmic flops (13 per corner-segment pair, SURVEY
+roofline  dominant kernel k_offroad_cull (exact search with group culling): after culling the
+          nearest roof is HBM (every segment tile is still streamed once per launch), so
+          achieved = algorithmic bytes / CUDA-event duration against the measured HBM peak; the
+          FP32 fractions on evaluated pairs and on the brute-force pair count are given beside it.
+roofline_bruteforce  the brute-force kernel k_offroad: 13 flop per corner-segment pair (SURVEY
           §8(d)) / its CUDA-event duration, against the FP32 peak SMs*128*2*max clock.
 cpu_baseline  the oracle (oracle/, as it stands) on the host cores, bounded sample.
 """
@@ -36,10 +40,10 @@ FLOP_PER_PAIR = 13.0           # w(2) t(3) c(4) d2(3) min(1)
 METRIC = "agent-steps/sec for step+overlap+offroad (B=4096,A=128); % of roofline"
 
 
-def profiled_traffic():
-    """dram__bytes_read+write per k_offroad launch from the latest committed ncu summary."""
+def profiled_traffic(kernel):
+    """dram__bytes_read+write per launch of `kernel` from the latest committed ncu summary."""
     import glob
-    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_k_offroad_traffic_bytes.txt")))
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_%s_traffic_bytes.txt" % kernel)))
     try:
         return float(open(files[-1]).read().split()[0]) if files else None
     except Exception:
@@ -206,26 +210,56 @@ def main():
     valid_rows = sim_d["valid"][:, 11:11 + N_STEPS].sum().item()
     valid_value = sharding.sum_over_ranks(valid_rows, dev) / (ms_step * 1e-3)
 
-    # ---- roofline of the dominant kernel: k_offroad alone, same rows, CUDA events ----
+    # ---- rooflines: the offroad kernel alone, same rows, CUDA events on the launching stream ----
     sd = torch.zeros((B, A), device=dev); fl = torch.zeros((B, A), dtype=torch.uint8, device=dev)
-    for t in range(11, 14):
-        wm.wm_metrics_offroad(h, sim_d, t, sd, None, fl)
-    torch.cuda.synchronize()
-    ka, kb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ka.record(stream)
-    for t in range(11, 11 + N_STEPS):
-        wm.wm_metrics_offroad(h, sim_d, t, sd, None, fl)
-    kb.record(stream)
-    torch.cuda.synchronize()
-    k_ms = ka.elapsed_time(kb) / N_STEPS
+
+    def time_offroad(handle):
+        for t in range(11, 14):
+            wm.wm_metrics_offroad(handle, sim_d, t, sd, None, fl)
+        torch.cuda.synchronize()
+        ka, kb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ka.record(stream)
+        for t in range(11, 11 + N_STEPS):
+            wm.wm_metrics_offroad(handle, sim_d, t, sd, None, fl)
+        kb.record(stream)
+        torch.cuda.synchronize()
+        return ka.elapsed_time(kb) / N_STEPS
+
+    wm.wm_offroad_stats(h)
+    k_ms = time_offroad(h)                                     # default mode: exact search with group culling
+    ev_pairs, bf_pairs = wm.wm_offroad_stats(h)
+    pairs_eval = ev_pairs / float(N_STEPS + 3)
     nvalid_bt = sim_d["valid"][:, 11:11 + N_STEPS].sum(dim=2).double().cpu().numpy()       # [B, 80]
-    pairs_per_launch = float((4.0 * nvalid_bt * n_seg[:, None]).sum() / N_STEPS)
+    pairs_per_launch = float((4.0 * nvalid_bt * n_seg[:, None]).sum() / N_STEPS)            # brute-force count
     peaks = measured_peaks()
     props = torch.cuda.get_device_properties(local)
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     fp32_peak = props.multi_processor_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12              # TFLOP/s
-    achieved = pairs_per_launch * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12
-    hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 29.0          # segments once + one state row
+    hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 29.0 + B * A * 5.0    # segments once + one state row + outputs
+    hb = wm.wm_create(offroad_mode=wm.WM_OFFROAD_BRUTE_FORCE)  # the FP32-roofline reference kernel
+    wm.wm_prepare(hb, rg_d)
+    kb_ms = time_offroad(hb)
+    wm.wm_destroy(hb)
+    bf_achieved = pairs_per_launch * FLOP_PER_PAIR / (kb_ms * 1e-3) / 1e12
+    peak_src = "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz)
+    roofline = {"bound": "hbm", "achieved": hbm_bytes / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": hbm_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "traffic": profiled_traffic("k_offroad_cull"),
+                "kernel": "k_offroad_cull", "kernel_ms": k_ms, "algorithmic_bytes_per_launch": hbm_bytes,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
+                "kernel_share_of_step": k_ms * N_STEPS / ms_step,
+                "pairs_bruteforce_per_launch": pairs_per_launch, "pairs_evaluated_per_launch": pairs_eval,
+                "evaluated_fraction": pairs_eval / pairs_per_launch,
+                "alu_frac_on_evaluated_pairs": pairs_eval * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12 / fp32_peak,
+                "alu_frac_bruteforce_equivalent": pairs_per_launch * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12 / fp32_peak,
+                "note": "exact culling (SURVEY 8(d)): the FP32 fraction is given on evaluated pairs and on the brute-force count"}
+    roofline_bf = {"bound": "alu", "achieved": bf_achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+                   "frac": bf_achieved / fp32_peak, "traffic": profiled_traffic("k_offroad_brute"),
+                   "kernel": "k_offroad (offroad_mode=WM_OFFROAD_BRUTE_FORCE)", "kernel_ms": kb_ms,
+                   "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR, "peak_source": peak_src}
+    rl_ms = max(pairs_per_launch * FLOP_PER_PAIR / (fp32_peak * 1e12), hbm_bytes / (hbm_peak * 1e9)) * 1e3
+    step_roofline = {"definition": "north_star: slower of algorithmic bytes/HBM peak and brute-force FP32 flops/FP32 peak, per simulated step",
+                     "roofline_ms": rl_ms, "achieved_ms": ms_step / N_STEPS, "frac": rl_ms / (ms_step / N_STEPS)}
     clocks = sampler.stop() if rank == 0 else None
 
     # ---- e2e: the same job from pinned host buffers through the C-ABI ----
@@ -281,12 +315,7 @@ def main():
                        "S_e_mean": float(n_seg.mean()), "l2": "inputs exceed L2 (segments %.2f GB + state per step)" % (n_seg.sum() * 24 / 1e9),
                        "parallelism": "scenario shards, no collective", "valid_agent_steps_per_s": valid_value,
                        "ms_per_sim_step": ms_step / N_STEPS},
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                         "frac": achieved / fp32_peak, "traffic": profiled_traffic(), "kernel": "k_offroad",
-                         "kernel_ms": k_ms, "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR,
-                         "peak_source": "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz),
-                         "hbm_time_ms_at_measured_peak": hbm_bytes / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9) * 1e3,
-                         "kernel_share_of_step": k_ms * N_STEPS / ms_step},
+            "roofline": roofline, "roofline_bruteforce": roofline_bf, "step_roofline": step_roofline,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line))

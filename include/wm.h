@@ -68,7 +68,14 @@ typedef struct {
   float max_curvature;  /* 0.3 1/m,  L104; <= 0 disables clipping (D7) */
   int32_t history;      /* 11 steps: the first second of the log (L78) */
   int32_t topk;         /* 1000 nearest roadgraph points per ego (D23) */
+  int32_t offroad_mode; /* WM_OFFROAD_*: how wm_metrics_offroad / wm_rollout search the segments */
 } wm_config;
+
+/* Both modes return the same values (the nearest segment is found exactly in both).
+ * CULLED (default): segments are stored in spatial order with one bounding circle per group of
+ *   64; a group is evaluated only if its lower bound can beat the current best of the agent.
+ * BRUTE_FORCE: every corner-segment pair is evaluated (the FP32-roofline reference kernel). */
+enum { WM_OFFROAD_CULLED = 0, WM_OFFROAD_BRUTE_FORCE = 1 };
 
 typedef struct wm_handle wm_handle; /* opaque */
 
@@ -190,6 +197,10 @@ int wm_rollout_host(wm_handle* h, const wm_traj* log_host, const wm_roadgraph* r
  * this handle has launched (graph replays count their kernel nodes). */
 int wm_segment_counts(wm_handle* h, int32_t* n_seg_host, int32_t B, void* stream);
 int64_t wm_kernel_launches(const wm_handle* h);
+/* wm_offroad_stats: out_host[0] = corner-segment pairs the culled offroad search evaluated since
+ * the last call, out_host[1] = pairs a brute-force search would have evaluated for the same
+ * launches (both 0 in brute-force mode). Resets the counters. */
+int wm_offroad_stats(wm_handle* h, int64_t* out_host, void* stream);
 
 #ifdef __cplusplus
 }

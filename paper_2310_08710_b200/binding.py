@@ -14,6 +14,7 @@ from . import _build
 WM_OK, WM_ERR_ARG, WM_ERR_CUDA, WM_ERR_UNSUPPORTED, WM_ERR_STATE = 0, -1, -2, -3, -4
 WM_DYN_INVERTIBLE_BICYCLE, WM_DYN_DELTA_LOCAL = 0, 1
 WM_TYPE_LANE, WM_TYPE_ROAD_EDGE = 1, 2
+WM_OFFROAD_CULLED, WM_OFFROAD_BRUTE_FORCE = 0, 1
 _ERR = {-1: "WM_ERR_ARG", -2: "WM_ERR_CUDA", -3: "WM_ERR_UNSUPPORTED", -4: "WM_ERR_STATE"}
 
 TRAJ_F = ("x", "y", "yaw", "vel_x", "vel_y", "length", "width")
@@ -21,7 +22,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches")
+           "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats")
 
 
 class wm_traj(C.Structure):
@@ -36,7 +37,8 @@ class wm_roadgraph(C.Structure):
 
 class wm_config(C.Structure):
     _fields_ = [("dynamics", C.c_int32), ("dt", C.c_float), ("max_accel", C.c_float),
-                ("max_curvature", C.c_float), ("history", C.c_int32), ("topk", C.c_int32)]
+                ("max_curvature", C.c_float), ("history", C.c_int32), ("topk", C.c_int32),
+                ("offroad_mode", C.c_int32)]
 
 
 class wm_rollout_out(C.Structure):
@@ -122,9 +124,10 @@ def wm_version():
     return load().wm_version().decode()
 
 
-def wm_create(dynamics=WM_DYN_INVERTIBLE_BICYCLE, dt=0.1, max_accel=6.0, max_curvature=0.3, history=11, topk=1000):
+def wm_create(dynamics=WM_DYN_INVERTIBLE_BICYCLE, dt=0.1, max_accel=6.0, max_curvature=0.3, history=11, topk=1000,
+              offroad_mode=WM_OFFROAD_CULLED):
     h = C.c_void_p()
-    cfg = wm_config(dynamics, dt, max_accel, max_curvature, history, topk)
+    cfg = wm_config(dynamics, dt, max_accel, max_curvature, history, topk, offroad_mode)
     _check(load().wm_create(C.byref(h), C.byref(cfg)), "wm_create")
     return h
 
@@ -206,6 +209,13 @@ def wm_segment_counts(h, B, stream=None):
 
 def wm_kernel_launches(h):
     return int(load().wm_kernel_launches(h))
+
+
+def wm_offroad_stats(h, stream=None):
+    """(pairs evaluated, brute-force pairs) of the culled offroad search since the last call."""
+    buf = (C.c_int64 * 2)()
+    _check(load().wm_offroad_stats(h, buf, _stream(stream)), "wm_offroad_stats")
+    return int(buf[0]), int(buf[1])
 
 
 # ---- small conveniences for tests / bench: torch allocation of the ABI's arrays ----

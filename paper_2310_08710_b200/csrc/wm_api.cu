@@ -30,6 +30,7 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (!out || !cfg) return WM_ERR_ARG;
   if (cfg->dynamics != WM_DYN_INVERTIBLE_BICYCLE && cfg->dynamics != WM_DYN_DELTA_LOCAL) return WM_ERR_ARG;
   if (!(cfg->dt > 0.f) || cfg->history < 1 || cfg->topk < 0) return WM_ERR_ARG;
+  if (cfg->offroad_mode != WM_OFFROAD_CULLED && cfg->offroad_mode != WM_OFFROAD_BRUTE_FORCE) return WM_ERR_ARG;
   wm_handle* h = (wm_handle*)calloc(1, sizeof(wm_handle));
   if (!h) return WM_ERR_ARG;
   h->cfg = *cfg;
@@ -40,8 +41,22 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
   if (major != 10) { free(h); return WM_ERR_UNSUPPORTED; }    // sm_100a kernels only; no fallback
   e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaMalloc(&h->cull_stats, 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMemset(h->cull_stats, 0, 2 * sizeof(unsigned long long));
   if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
   *out = h;
+  return WM_OK;
+}
+
+extern "C" int wm_offroad_stats(wm_handle* h, int64_t* out_host, void* stream) {
+  if (!h || !out_host) return WM_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  unsigned long long v[2];
+  WM_CUDA(cudaMemcpyAsync(v, h->cull_stats, sizeof(v), cudaMemcpyDeviceToHost, s));
+  WM_CUDA(cudaMemsetAsync(h->cull_stats, 0, sizeof(v), s));
+  WM_CUDA(cudaStreamSynchronize(s));
+  out_host[0] = (int64_t)v[0] * 64 * 4;      // corner-segment pairs evaluated (64 segments x 4 corners per group)
+  out_host[1] = (int64_t)v[1] * 64 * 4;      // pairs a brute-force search would have evaluated
   return WM_OK;
 }
 
@@ -58,6 +73,7 @@ extern "C" int wm_destroy(wm_handle* h) {
   wm_drop_graph(h);
   wm_prepare_free(h);
   cudaFree(h->scratch);
+  cudaFree(h->cull_stats);
   for (int i = 0; i < 16; ++i) cudaFree(h->stage[i]);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   free(h);

@@ -40,7 +40,8 @@ struct wm_handle {
   int32_t* n_seg;           // [B]
   float4* edges;            // [B][seg_tiles][WM_TILE_F4]
   float2* sign_dir;         // [B][seg_tiles*512]  sign direction (e, or stored dir if e == 0)
-  int32_t* seg_src;         // [B][seg_tiles*512]  first-point index of each segment
+  int32_t* seg_src;         // [B][seg_tiles*512]  first-point index of each stored segment (-1: padding)
+  float4* groups;           // [B][seg_tiles*8]    bounding circle {cx, cy, r, 0} of each 64-segment group
   int32_t pts_pad;          // padded R
   float2* pts;              // [B][pts_pad]
   // rollout graph cache
@@ -52,6 +53,7 @@ struct wm_handle {
   // scratch for rollouts / host staging
   void* scratch; size_t scratch_bytes;
   void* stage[16]; size_t stage_bytes[16];
+  unsigned long long* cull_stats;   // device [2]: groups evaluated, groups considered (culled mode)
 };
 
 extern thread_local int g_wm_last_cuda_error;
@@ -100,6 +102,8 @@ cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t*
                               uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
 cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
                               float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
+cudaError_t wm_launch_offroad_culled(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
+                                     float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
 cudaError_t wm_launch_aggregate(wm_handle* h, int B, int A, int n_steps, const wm_rollout_out& out,
                                 const uint8_t* ld_valid_rows, cudaStream_t s);
 int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);

@@ -16,6 +16,7 @@
 // sign from the oriented edge (D16) and the signed distance.  Valid agents are compacted first,
 // so invalid slots cost nothing.  Bound: FP32 pipe (see DESIGN.md roofline).
 #include <float.h>
+#include <stdlib.h>
 
 #include "wm_internal.cuh"
 
@@ -56,11 +57,98 @@ __global__ void __launch_bounds__(256) k_count_segments(RgView g, int32_t* n_seg
   if (threadIdx.x == 0) n_seg[blockIdx.x] = s_cnt;
 }
 
-__device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir, int32_t* seg_src, int s,
-                                              float p0x, float p0y, float ex, float ey, float gx, float gy,
-                                              float sx, float sy, int src) {
+// ---------------------------------------------------------------------------------------
+// Spatial order.  Segments are stored in the order (Morton code of the grid cell that holds
+// their first point, first-point index): inside a cell, polyline pieces stay contiguous, and
+// any 64 consecutive stored segments (a "group": one packed iteration of a warp) form a compact
+// cluster whose bounding box lets the culled kernel skip the whole group exactly.
+// k_sort_segments writes the permutation into seg_src.  `grid` cells per axis (<= 64) over the
+// scenario's own bounding box.
+// ---------------------------------------------------------------------------------------
+constexpr int SORT_CELLS = 64 * 64;                 // counters (4096 = 4 per thread)
+
+__device__ __forceinline__ uint32_t part1by1(uint32_t v) {   // spread the low 6 bits
+  v &= 0x3fu;
+  v = (v | (v << 4)) & 0x30fu;
+  v = (v | (v << 2)) & 0x333u;
+  v = (v | (v << 1)) & 0x555u;
+  return v;
+}
+
+__global__ void __launch_bounds__(1024) k_sort_segments(RgView g, int cap, int32_t* seg_src, int grid) {
+  __shared__ int s_cnt[SORT_CELLS];
+  __shared__ int s_start[SORT_CELLS];
+  __shared__ float s_red[4][32];
+  __shared__ int s_wsum[32];
+  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t o = (int64_t)b * g.R;
+  int32_t* out = seg_src + (int64_t)b * cap;
+  // bounding box of the records' first points
+  float x0 = 3.0e38f, y0 = 3.0e38f, x1 = -3.0e38f, y1 = -3.0e38f;
+  for (int i = tid; i < g.R; i += blockDim.x) {
+    bool sg;
+    if (rg_record(g, o, i, &sg)) {
+      const float x = g.x[o + i], y = g.y[o + i];
+      x0 = fminf(x0, x); y0 = fminf(y0, y); x1 = fmaxf(x1, x); y1 = fmaxf(y1, y);
+    }
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    x0 = fminf(x0, __shfl_xor_sync(0xffffffffu, x0, d)); y0 = fminf(y0, __shfl_xor_sync(0xffffffffu, y0, d));
+    x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, d)); y1 = fmaxf(y1, __shfl_xor_sync(0xffffffffu, y1, d));
+  }
+  if (lane == 0) { s_red[0][warp] = x0; s_red[1][warp] = y0; s_red[2][warp] = x1; s_red[3][warp] = y1; }
+  for (int c = tid; c < SORT_CELLS; c += blockDim.x) s_cnt[c] = 0;
+  __syncthreads();
+  x0 = s_red[0][0]; y0 = s_red[1][0]; x1 = s_red[2][0]; y1 = s_red[3][0];
+  for (int w = 1; w < 32; ++w) {
+    x0 = fminf(x0, s_red[0][w]); y0 = fminf(y0, s_red[1][w]); x1 = fmaxf(x1, s_red[2][w]); y1 = fmaxf(y1, s_red[3][w]);
+  }
+  const float sx = (float)grid / fmaxf(x1 - x0, 1e-3f), sy = (float)grid / fmaxf(y1 - y0, 1e-3f);
+  auto cell_of = [&](int i) -> int {
+    const int ix = min(grid - 1, max(0, (int)((g.x[o + i] - x0) * sx)));
+    const int iy = min(grid - 1, max(0, (int)((g.y[o + i] - y0) * sy)));
+    return (int)(part1by1((uint32_t)ix) | (part1by1((uint32_t)iy) << 1));
+  };
+  for (int i = tid; i < g.R; i += blockDim.x) { bool sg; if (rg_record(g, o, i, &sg)) atomicAdd(&s_cnt[cell_of(i)], 1); }
+  __syncthreads();
+  // exclusive scan of the 4096 counters: 4 per thread
+  int c4[4], sum = 0;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) { c4[q] = s_cnt[tid * 4 + q]; sum += c4[q]; }
+  int inc = sum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+  if (lane == 31) s_wsum[warp] = inc;
+  __syncthreads();
+  int base = 0;
+  for (int w = 0; w < warp; ++w) base += s_wsum[w];
+  int run = base + inc - sum;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) { s_start[tid * 4 + q] = run; run += c4[q]; }
+  __syncthreads();
+  for (int c = tid; c < SORT_CELLS; c += blockDim.x) s_cnt[c] = s_start[c];          // cursors
+  __syncthreads();
+  for (int i = tid; i < g.R; i += blockDim.x) { bool sg; if (rg_record(g, o, i, &sg)) out[atomicAdd(&s_cnt[cell_of(i)], 1)] = i; }
+  __syncthreads();
+  // deterministic order inside a cell: ascending point index (insertion sort, cells are small)
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const int c = tid * 4 + q, lo = s_start[c], hi = s_cnt[c];
+    for (int a = lo + 1; a < hi; ++a) {
+      const int v = out[a];
+      int k = a - 1;
+      while (k >= lo && out[k] > v) { out[k + 1] = out[k]; --k; }
+      out[k + 1] = v;
+    }
+  }
+}
+
+// position of stored segment s inside its tile: it = (s%512)/64, lane = (s%64)/2, half = s&1
+__device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir, int s, float p0x, float p0y,
+                                              float ex, float ey, float gx, float gy, float sx, float sy) {
   const int tau = s / WM_TILE_SEGS, r = s % WM_TILE_SEGS;
-  const int lane = r / WM_RUN, j = r % WM_RUN, it = j >> 1, half = j & 1;
+  const int it = r >> 6, lane = (r >> 1) & 31, half = r & 1;
   float* t = tile_base + (int64_t)tau * (WM_TILE_F4 * 4);
   float* q0 = t + ((it * 3 + 0) * 32 + lane) * 4;
   float* q1 = t + ((it * 3 + 1) * 32 + lane) * 4;
@@ -69,48 +157,58 @@ __device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir
   q1[half] = ex;  q1[2 + half] = ey;
   q2[half] = gx;  q2[2 + half] = gy;
   sign_dir[s] = make_float2(sx, sy);
-  seg_src[s] = src;
 }
 
-__global__ void __launch_bounds__(1024) k_fill_segments(RgView g, int seg_tiles, float4* edges, float2* sign_dir, int32_t* seg_src) {
-  __shared__ int s_warp[32];
-  __shared__ int s_base;
-  const int b = blockIdx.x;
+// One warp per group of 64 stored segments: writes the tile records and the group's bounding
+// circle {cx, cy, r, 0} (r inflated so that float32 rounding can never make the bound unsafe).
+__global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, const int32_t* n_seg, float4* edges,
+                                                       float2* sign_dir, int32_t* seg_src, float4* groups) {
+  const int b = blockIdx.y, lane = threadIdx.x & 31;
+  const int grp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int ngrp = seg_tiles * (WM_TILE_SEGS / 64);
+  if (grp >= ngrp) return;
   const int64_t o = (int64_t)b * g.R;
-  const int cap = seg_tiles * WM_TILE_SEGS;
+  const int cap = seg_tiles * WM_TILE_SEGS, n = n_seg[b];
   float* tile_base = (float*)(edges + (int64_t)b * seg_tiles * WM_TILE_F4);
   float2* sd = sign_dir + (int64_t)b * cap;
   int32_t* src = seg_src + (int64_t)b * cap;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (threadIdx.x == 0) s_base = 0;
-  __syncthreads();
-  for (int base = 0; base < g.R; base += blockDim.x) {
-    const int i = base + threadIdx.x;
-    bool is_seg;
-    const bool rec = rg_record(g, o, i, &is_seg);
-    const uint32_t bal = __ballot_sync(0xffffffffu, rec);
-    if (lane == 0) s_warp[warp] = __popc(bal);
-    __syncthreads();
-    int pre = s_base;
-    for (int w = 0; w < warp; ++w) pre += s_warp[w];
-    if (rec) {
-      const int s = pre + __popc(bal & ((1u << lane) - 1u));
+  float x0 = 3.0e38f, y0 = 3.0e38f, x1 = -3.0e38f, y1 = -3.0e38f;
+  float ax[2], ay[2], bx[2], by[2];
+  bool real[2];
+#pragma unroll
+  for (int hf = 0; hf < 2; ++hf) {
+    const int s = grp * 64 + lane * 2 + hf;
+    real[hf] = s < n;
+    if (real[hf]) {
+      const int i = src[s];
+      const bool is_seg = rg_starts(g, o, i);
       const float p0x = g.x[o + i], p0y = g.y[o + i];
       float ex = 0.f, ey = 0.f;
       if (is_seg) { ex = g.x[o + i + 1] - p0x; ey = g.y[o + i + 1] - p0y; }
       const float ee = fmaf(ex, ex, ey * ey);
       float gx = 0.f, gy = 0.f, sx, sy;
       if (ee > 0.f) { gx = ex / ee; gy = ey / ee; sx = ex; sy = ey; }
-      else { ex = 0.f; ey = 0.f; sx = g.dir_x[o + i]; sy = g.dir_y[o + i]; }
-      store_segment(tile_base, sd, src, s, p0x, p0y, ex, ey, gx, gy, sx, sy, i);
+      else { ex = 0.f; ey = 0.f; sx = g.dir_x[o + i]; sy = g.dir_y[o + i]; }     // D16 / D29
+      store_segment(tile_base, sd, s, p0x, p0y, ex, ey, gx, gy, sx, sy);
+      ax[hf] = p0x; ay[hf] = p0y; bx[hf] = p0x + ex; by[hf] = p0y + ey;
+      x0 = fminf(x0, fminf(ax[hf], bx[hf])); x1 = fmaxf(x1, fmaxf(ax[hf], bx[hf]));
+      y0 = fminf(y0, fminf(ay[hf], by[hf])); y1 = fmaxf(y1, fmaxf(ay[hf], by[hf]));
+    } else {                                      // padding: far away, never wins against a real segment
+      store_segment(tile_base, sd, s, WM_FAR, WM_FAR, 0.f, 0.f, 0.f, 0.f, 1.f, 0.f);
+      src[s] = -1;
     }
-    __syncthreads();
-    if (threadIdx.x == 0) { int tot = 0; for (int w = 0; w < 32; ++w) tot += s_warp[w]; s_base += tot; }
-    __syncthreads();
   }
-  // padding records: far away, never win against a real segment
-  for (int s = s_base + threadIdx.x; s < cap; s += blockDim.x)
-    store_segment(tile_base, sd, src, s, WM_FAR, WM_FAR, 0.f, 0.f, 0.f, 0.f, 1.f, 0.f, -1);
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    x0 = fminf(x0, __shfl_xor_sync(0xffffffffu, x0, d)); y0 = fminf(y0, __shfl_xor_sync(0xffffffffu, y0, d));
+    x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, d)); y1 = fmaxf(y1, __shfl_xor_sync(0xffffffffu, y1, d));
+  }
+  // axis-aligned bounding box {x0, y0, x1, y1} of the group's segments (exact: min/max of the
+  // float32 endpoints; p1 = p0 + e may round by an ulp, covered by the kernel's 1e-3 m slack)
+  if (lane == 0) {
+    const bool any = x1 >= x0;
+    groups[(int64_t)b * ngrp + grp] = any ? make_float4(x0, y0, x1, y1) : make_float4(WM_FAR, WM_FAR, WM_FAR, WM_FAR);
+  }
 }
 
 // packed copy of the roadgraph points for the top-k observation
@@ -124,8 +222,8 @@ __global__ void __launch_bounds__(256) k_pack_points(RgView g, int pts_pad, floa
 }
 
 void wm_prepare_free(wm_handle* h) {
-  cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pts);
-  h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pts = nullptr;
+  cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pts); cudaFree(h->groups);
+  h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pts = nullptr; h->groups = nullptr;
   h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0; h->pts_pad = 0;
 }
 
@@ -158,15 +256,24 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
   if (tiles < 1) tiles = 1;
   if (tiles > h->seg_tiles || !h->edges) {       // grow only: seg_tiles is the row stride of `edges`
     wm_drop_graph(h);
-    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src);
-    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr;
+    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->groups);
+    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->groups = nullptr;
     h->seg_tiles = tiles;
     const size_t cap = (size_t)tiles * WM_TILE_SEGS;
     WM_CUDA(cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES));
     WM_CUDA(cudaMalloc(&h->sign_dir, (size_t)B * cap * sizeof(float2)));
     WM_CUDA(cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t)));
+    WM_CUDA(cudaMalloc(&h->groups, (size_t)B * tiles * (WM_TILE_SEGS / 64) * sizeof(float4)));
   }
-  k_fill_segments<<<B, 1024, 0, s>>>(g, h->seg_tiles, h->edges, h->sign_dir, h->seg_src);
+  static int sort_grid = 0;
+  if (!sort_grid) { const char* e = getenv("WM_SORT_GRID"); sort_grid = e ? atoi(e) : 16; if (sort_grid < 1 || sort_grid > 64) sort_grid = 16; }
+  k_sort_segments<<<B, 1024, 0, s>>>(g, h->seg_tiles * WM_TILE_SEGS, h->seg_src, sort_grid);
+  h->launches++;
+  WM_CUDA(cudaGetLastError());
+  {
+    const int ngrp = h->seg_tiles * (WM_TILE_SEGS / 64);
+    k_fill_segments<<<dim3((ngrp + 7) / 8, B), 256, 0, s>>>(g, h->seg_tiles, h->n_seg, h->edges, h->sign_dir, h->seg_src, h->groups);
+  }
   h->launches++;
   WM_CUDA(cudaGetLastError());
   k_pack_points<<<dim3((h->pts_pad + 255) / 256, B), 256, 0, s>>>(g, h->pts_pad, h->pts);
@@ -180,14 +287,14 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
 // ======================================================================================
 // k_offroad
 // ======================================================================================
-constexpr int OFF_THREADS = 512;
-constexpr int OFF_WARPS = OFF_THREADS / 32;
+// CTA size is a template parameter: 512 threads x 1 CTA/SM or 256 threads x 2 CTAs/SM
+
 constexpr int OFF_NA = 2;                  // agents per warp unit (8 corners in registers)
 
 struct OffroadParams {
   wm_row row;
   int A;
-  const float4* edges; const float2* sign_dir; const int32_t* n_seg;
+  const float4* edges; const float2* sign_dir; const int32_t* n_seg; const int32_t* seg_src;
   int seg_tiles;          // tiles per scenario in `edges`
   int tiles_per_buf;      // capacity of one shared-memory buffer, in tiles
   float* sd; int64_t sd_stride_b;
@@ -209,7 +316,9 @@ __device__ __forceinline__ float seg_d2(float wx, float wy, float ex, float ey, 
   return fmaf(ry, ry, rx * rx);
 }
 
-__global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
+template <int OFF_THREADS, int OFF_MINB>
+__global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams p) {
+  constexpr int OFF_WARPS = OFF_THREADS / 32;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int A = p.A, Ap = ((A + 31) / 32) * 32;
   uint64_t* bars = (uint64_t*)smem_raw;                       // [2] full barriers
@@ -223,7 +332,7 @@ __global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
   const int nseg = p.n_seg[b];
   const int nt = (nseg + WM_TILE_SEGS - 1) / WM_TILE_SEGS;    // tiles of this scenario
   const int G = (nt + p.tiles_per_buf - 1) / p.tiles_per_buf; // tile groups
-  const int TB = G > 0 ? (nt + G - 1) / G : 0;                // balanced tiles per group
+  // group g covers tiles [g*nt/G, (g+1)*nt/G): balanced, each at most tiles_per_buf
   const float4* edges_b = p.edges + (int64_t)b * p.seg_tiles * WM_TILE_F4;
 
   if (tid == 0) {
@@ -235,7 +344,7 @@ __global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
   // ---- producer: start the first two groups (overlaps with the agent set-up below) ----
   if (tid == 0) {
     for (int g = 0; g < 2 && g < G; ++g) {
-      const int t0 = g * TB, n = min(TB, nt - t0);
+      const int t0 = (g * nt) / G, n = ((g + 1) * nt) / G - t0;
       mbar_expect_tx(&bars[g], (uint32_t)n * WM_TILE_BYTES);
       for (int t = 0; t < n; ++t)
         tma_load_1d(s_buf + ((int64_t)g * p.tiles_per_buf + t) * WM_TILE_F4, edges_b + (int64_t)(t0 + t) * WM_TILE_F4, WM_TILE_BYTES, &bars[g]);
@@ -281,7 +390,7 @@ __global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
   // ---- scan ----
   const int nunits = (nvalid + OFF_NA - 1) / OFF_NA;
   for (int g = 0; g < G; ++g) {
-    const int t0 = g * TB, ntg = min(TB, nt - t0);
+    const int t0 = (g * nt) / G, ntg = ((g + 1) * nt) / G - t0;
     const int ncells = nunits * ntg;
     const int c_begin = (int)(((long long)warp * ncells) / OFF_WARPS);
     const int c_end = (int)(((long long)(warp + 1) * ncells) / OFF_WARPS);
@@ -363,7 +472,7 @@ __global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
       __syncthreads();
       if (tid == 0) {
         fence_proxy_async();
-        const int g2 = g + 2, t2 = g2 * TB, n2 = min(TB, nt - t2);
+        const int g2 = g + 2, t2 = (g2 * nt) / G, n2 = ((g2 + 1) * nt) / G - t2;
         mbar_expect_tx(&bars[g & 1], (uint32_t)n2 * WM_TILE_BYTES);
         for (int t = 0; t < n2; ++t)
           tma_load_1d(s_buf + ((int64_t)(g & 1) * p.tiles_per_buf + t) * WM_TILE_F4, edges_b + (int64_t)(t2 + t) * WM_TILE_F4, WM_TILE_BYTES, &bars[g & 1]);
@@ -385,19 +494,23 @@ __global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
       const float sgn = (k & 2) ? -1.f : 1.f;
       const float qx = s_ag[0 * Ap + ci], qy = s_ag[1 * Ap + ci];
       const float4* tp = edges_b + (int64_t)tau * WM_TILE_F4 + ln;
+      // the lane's 16 stored segments of this tile sit at it*64 + lane*2 + {0,1}; exact ties
+      // inside the run go to the lower source point index (D17)
+      const int32_t* srcp = p.seg_src + (int64_t)b * p.seg_tiles * WM_TILE_SEGS + tau * WM_TILE_SEGS + ln * 2;
       float bd2 = __int_as_float(0x7f800000), bwx = 0.f, bwy = 0.f;
-      int bj = 0;
+      int bs = 0, bsrc = 0x7fffffff;
 #pragma unroll
       for (int it = 0; it < 8; ++it) {
         const float4 P = __ldg(&tp[(it * 3 + 0) * 32]), E = __ldg(&tp[(it * 3 + 1) * 32]), Gv = __ldg(&tp[(it * 3 + 2) * 32]);
+        const int2 sr = __ldg((const int2*)(srcp + it * 64));
         const float w0x = fmaf(sgn, offx, qx - P.x), w0y = fmaf(sgn, offy, qy - P.z);
         const float w1x = fmaf(sgn, offx, qx - P.y), w1y = fmaf(sgn, offy, qy - P.w);
         const float d0 = seg_d2(w0x, w0y, E.x, E.z, Gv.x, Gv.z);
         const float d1 = seg_d2(w1x, w1y, E.y, E.w, Gv.y, Gv.w);
-        if (d0 < bd2) { bd2 = d0; bwx = w0x; bwy = w0y; bj = 2 * it; }
-        if (d1 < bd2) { bd2 = d1; bwx = w1x; bwy = w1y; bj = 2 * it + 1; }
+        if (sr.x >= 0 && (d0 < bd2 || (d0 == bd2 && sr.x < bsrc))) { bd2 = d0; bwx = w0x; bwy = w0y; bs = it * 64; bsrc = sr.x; }
+        if (sr.y >= 0 && (d1 < bd2 || (d1 == bd2 && sr.y < bsrc))) { bd2 = d1; bwx = w1x; bwy = w1y; bs = it * 64 + 1; bsrc = sr.y; }
       }
-      const int s = tau * WM_TILE_SEGS + ln * WM_RUN + bj;
+      const int s = tau * WM_TILE_SEGS + ln * 2 + bs;
       const float2 sdir = __ldg(&p.sign_dir[(int64_t)b * p.seg_tiles * WM_TILE_SEGS + s]);
       const float side = fmaf(sdir.x, bwy, -sdir.y * bwx);                 // e x (q - p0), D16
       const float d = sqrtf(bd2);
@@ -417,26 +530,39 @@ __global__ void __launch_bounds__(OFF_THREADS, 1) k_offroad(OffroadParams p) {
 
 cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
                               float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s) {
+  if (h->cfg.offroad_mode != WM_OFFROAD_BRUTE_FORCE)
+    return wm_launch_offroad_culled(h, sim, t, sd, sd_stride_b, corner, flag, flag_stride_b, s);
   OffroadParams p;
   p.row = wm_make_row(sim, t);
   p.A = sim.A;
-  p.edges = h->edges; p.sign_dir = h->sign_dir; p.n_seg = h->n_seg; p.seg_tiles = h->seg_tiles;
+  p.edges = h->edges; p.sign_dir = h->sign_dir; p.n_seg = h->n_seg; p.seg_src = h->seg_src; p.seg_tiles = h->seg_tiles;
   p.sd = sd; p.sd_stride_b = sd_stride_b; p.corner = corner; p.flag = flag; p.flag_stride_b = flag_stride_b;
   const size_t fixed = off_fixed_bytes(sim.A);
-  const size_t max_smem = 227 * 1024;
+  // Two 256-thread CTAs per SM (each <= 113 KB of shared memory) so that one CTA's set-up,
+  // flushes and re-scan overlap the other's main loop; one 512-thread CTA per SM when the
+  // per-agent arrays leave too little room (large A).  WM_OFFROAD_CTA=512|256 forces a variant.
+  static int forced = -1;
+  if (forced < 0) { const char* e = getenv("WM_OFFROAD_CTA"); forced = e ? atoi(e) : 0; }
+  const size_t sm_total = 227 * 1024, per_cta2 = (sm_total - 2048) / 2;
+  bool two = fixed + 2 * 2 * (size_t)WM_TILE_BYTES <= per_cta2;
+  if (forced == 512) two = false;
+  if (forced == 256 && fixed + 2 * (size_t)WM_TILE_BYTES <= per_cta2) two = true;
+  const size_t max_smem = two ? per_cta2 : sm_total;
   int tpb = (int)((max_smem - fixed) / (2 * (size_t)WM_TILE_BYTES));
   const int need = (h->seg_tiles + 1) / 2;        // two buffers hold the whole scenario if they can
   if (tpb > need) tpb = need;
   if (tpb < 1) tpb = 1;
   p.tiles_per_buf = tpb;
   const size_t smem = fixed + 2 * (size_t)tpb * WM_TILE_BYTES;
-  static size_t configured = 0;
-  if (smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_offroad, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_offroad<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_total);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_offroad<256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)per_cta2);
     if (e != cudaSuccess) return e;
-    configured = max_smem;
+    configured = true;
   }
-  k_offroad<<<sim.B, OFF_THREADS, smem, s>>>(p);
+  if (two) k_offroad<256, 2><<<sim.B, 256, smem, s>>>(p);
+  else k_offroad<512, 1><<<sim.B, 512, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
 }

@@ -102,10 +102,12 @@ def test_overlap_matches_oracle(cfgid, B):
     wm.wm_destroy(h)
 
 
+@pytest.mark.parametrize("mode", ["culled", "brute"])
 @pytest.mark.parametrize("cfgid,B", [(1, 4), (2, 6), (4, 6), (5, 6)])
-def test_offroad_matches_oracle(cfgid, B):
+def test_offroad_matches_oracle(cfgid, B, mode):
     cfg = ws.make_config(cfgid, B=B) if cfgid != 5 else ws.make_config(5, B=B, n_steps=1)
-    h, log_d, rg_d, sim_d, _ = _setup(cfg)
+    h, log_d, rg_d, sim_d, _ = _setup(
+        cfg, offroad_mode=wm.WM_OFFROAD_CULLED if mode == "culled" else wm.WM_OFFROAD_BRUTE_FORCE)
     t = cfg["t0"]
     sd, cd, fl = gpu_offroad(h, log_d, t)
     orc = oracle.offroad(cfg["log"], t, cfg["roadgraph"])
@@ -114,6 +116,21 @@ def test_offroad_matches_oracle(cfgid, B):
     assert st["ambiguous"] < 0.2 * st["corners"]
     assert 0 < fl.sum() < (cfg["log"]["valid"][:, t] == 1).sum()
     wm.wm_destroy(h)
+
+
+def test_offroad_culled_equals_brute_force_bitwise():
+    """Culling only changes WHICH pairs are evaluated: the per-pair arithmetic is the same, so the
+    distances of both modes are bit-identical (signs too, outside exact float32 ties)."""
+    for cfgid, B in ((1, 4), (4, 4), (5, 16), (2, 8)):
+        cfg = ws.make_config(cfgid, B=B) if cfgid != 5 else ws.make_config(5, B=B, n_steps=1)
+        res = []
+        for mode in (wm.WM_OFFROAD_CULLED, wm.WM_OFFROAD_BRUTE_FORCE):
+            h, log_d, rg_d, sim_d, _ = _setup(cfg, offroad_mode=mode)
+            res.append(gpu_offroad(h, log_d, cfg["t0"]))
+            wm.wm_destroy(h)
+        assert np.array_equal(np.abs(res[0][1]), np.abs(res[1][1])), cfgid
+        assert (res[0][1] != res[1][1]).mean() < 1e-3
+        assert (res[0][2] != res[1][2]).mean() < 1e-3
 
 
 def test_log_divergence_matches_oracle(cfg1):
