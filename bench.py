@@ -140,6 +140,135 @@ def run_reference(args):
     return 0
 
 
+def run_supplementary(args):
+    """Supplementary lines for the other hot-path rows: config 3 observation (a6, a7), config 2
+    single DeltaLocal step + metrics (a2-a5), config 4 overlap-dense stress (a3, a4).  N=1 only."""
+    import torch
+    import oracle
+    import wm_scenarios as ws
+    import paper_2310_08710_b200 as wm
+    torch.cuda.set_device(0)
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(steps):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / steps
+
+    W, K = max(args.warmup, 3), args.steps
+    if args.workload == "observe":
+        cfg = ws.make_config(3)
+        log, rg = cfg["log"], cfg["roadgraph"]
+        B, T, A = log["x"].shape
+        k, H, t = 1000, 11, 10
+        h = wm.wm_create(topk=k)
+        log_d, rg_d = wm.to_device(log), wm.to_device(rg)
+        wm.wm_prepare(h, rg_d)
+        hist = torch.empty((B, A, H, 7, A), device="cuda"); hv = torch.empty((B, A, H, A), dtype=torch.uint8, device="cuda")
+        idx = torch.empty((B, A, k), dtype=torch.int32, device="cuda")
+        feat = torch.empty((B, A, 4, k), device="cuda"); typ = torch.empty((B, A, k), dtype=torch.int32, device="cuda")
+        l0 = wm.wm_kernel_launches(h)
+        ms = timed(lambda: wm.wm_observe(h, log_d, rg_d, t, hist, hv, idx, feat, typ), K, W)
+        launches = (wm.wm_kernel_launches(h) - l0) * K // (K + W)
+        ms_h = timed(lambda: wm.wm_observe(h, log_d, rg_d, t, hist, hv, None, None, None), K, W)
+        ms_k = timed(lambda: wm.wm_observe(h, log_d, rg_d, t, None, None, idx, feat, typ), K, W)
+        egos = int(log["valid"][:, t].sum())
+        out_bytes = sum(x.numel() * x.element_size() for x in (hist, hv, idx, feat, typ))
+        in_bytes = B * rg["x"].shape[1] * 8 + B * H * A * 29
+        # oracle sample: 2 scenarios
+        sb = 2
+        sub = lambda d: {q: np.ascontiguousarray(v[:sb]) for q, v in d.items()}
+        t0 = time.perf_counter()
+        ok = oracle.observe_topk(sub(log), sub(rg), t, k); oracle.observe_history(sub(log), t, H)
+        dt = time.perf_counter() - t0
+        same = bool(np.array_equal(idx[:sb].cpu().numpy(), ok["rg_index"]))
+        line = {"metric": "ego observations/s (history in ego frame + top-1000 roadgraph points), config 3", "value": B * A / (ms * 1e-3),
+                "unit": "ego-observations/s", "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "config3: B=256 A=128 R=30000 H=11 k=1000, every valid agent an ego", "valid_egos": egos,
+                           "l2": "outputs 2.2 GB exceed L2", "ms_history": ms_h, "ms_topk": ms_k},
+                "roofline": {"bound": "hbm", "achieved": (out_bytes + in_bytes) / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": (out_bytes + in_bytes) / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": None,
+                             "kernel": "k_observe_hist + k_observe_topk", "algorithmic_bytes": out_bytes + in_bytes,
+                             "history_frac": (hist.numel() * 4 + hv.numel() + B * H * A * 29) / (ms_h * 1e-3) / 1e9 / hbm_peak,
+                             "topk_frac": (out_bytes - hist.numel() * 4 - hv.numel() + B * rg["x"].shape[1] * 8) / (ms_k * 1e-3) / 1e9 / hbm_peak,
+                             "note": "top-k is ALU/shared-memory bound (3 passes over R per ego), see DESIGN.md"},
+                "cpu_baseline": {"value": sb * A / dt, "unit": "ego-observations/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                 "sample": "first %d of %d scenarios, %.1f s wall" % (sb, B, dt), "index_sets_equal": same},
+                "e2e": None, "gpu_launches": int(launches), "clocks": None}
+    else:
+        cid = 2 if args.workload == "step2" else 4
+        cfg = ws.make_config(cid)
+        log, rg = cfg["log"], cfg["roadgraph"]
+        B, T, A = log["x"].shape
+        h = wm.wm_create(dynamics=wm.WM_DYN_DELTA_LOCAL)
+        log_d, rg_d = wm.to_device(log), wm.to_device(rg)
+        seg_max = wm.wm_prepare(h, rg_d)
+        sim_d = wm.empty_traj_like(log_d)
+        t = wm.wm_reset(h, log_d, sim_d) if cid == 2 else 0
+        Wd = (A + 31) // 32
+        bits = torch.empty((B, A, Wd), dtype=torch.int32, device="cuda"); ofl = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+        sd = torch.empty((B, A), device="cuda"); fl = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+        ld = torch.empty((B, A), device="cuda"); lv = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+        if cid == 2:
+            act = torch.from_numpy(np.ascontiguousarray(cfg["actions"][:, 0])).cuda()
+            av = torch.from_numpy(np.ascontiguousarray(cfg["action_valid"][:, 0])).cuda()
+
+            def fn():
+                wm.wm_step(h, log_d, sim_d, t, act, av)
+                wm.wm_metrics_overlap(h, sim_d, t + 1, bits, ofl)
+                wm.wm_metrics_offroad(h, sim_d, t + 1, sd, None, fl)
+                wm.wm_log_divergence(h, log_d, sim_d, t + 1, ld, lv)
+        else:
+            src = log_d
+
+            def fn():
+                wm.wm_metrics_overlap(h, src, 0, bits, ofl)
+                wm.wm_metrics_offroad(h, src, 0, sd, None, fl)
+        l0 = wm.wm_kernel_launches(h)
+        ms = timed(fn, K, W)
+        launches = (wm.wm_kernel_launches(h) - l0) * K // (K + W)
+        row = sim_d if cid == 2 else log_d
+        ms_ov = timed(lambda: wm.wm_metrics_overlap(h, row, t + 1 if cid == 2 else 0, bits, ofl), K, W)
+        wm.wm_offroad_stats(h)
+        ms_off = timed(lambda: wm.wm_metrics_offroad(h, row, t + 1 if cid == 2 else 0, sd, None, fl), K, W)
+        ev, bf = wm.wm_offroad_stats(h)
+        n_seg = np.array(wm.wm_segment_counts(h, B))
+        hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 34.0
+        sb = min(8, B)
+        sub = lambda d: {q: np.ascontiguousarray(v[:sb]) for q, v in d.items()}
+        rowh = {q: v[:sb].cpu().numpy() for q, v in row.items()}
+        tt = t + 1 if cid == 2 else 0
+        t0 = time.perf_counter()
+        oo = oracle.offroad(rowh, tt, sub(rg), details=False); oracle.overlap(rowh, tt, want_gap=False, want_pair=False)
+        dt = time.perf_counter() - t0
+        line = {"metric": "agent-steps/s, config %d (%s)" % (cid, "DeltaLocal step + overlap + offroad + log divergence" if cid == 2 else "overlap + offroad, crowded lot"),
+                "value": B * A / (ms * 1e-3), "unit": "agent-steps/s", "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "config%d: B=%d A=%d R=%d" % (cid, B, A, rg["x"].shape[1]), "S_e_max": int(seg_max),
+                           "ms_overlap": ms_ov, "ms_offroad": ms_off, "l2": ("segment tiles %d MB per call exceed L2" if n_seg.sum() * 24 > 126e6 else "segment tiles %d MB fit in L2 (small config, not flushed)") % int(n_seg.sum() * 24 / 1e6)},
+                "roofline": {"bound": "hbm", "achieved": hbm_bytes / (ms_off * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": hbm_bytes / (ms_off * 1e-3) / 1e9 / hbm_peak, "traffic": None, "kernel": "k_offroad_cull",
+                             "kernel_ms": ms_off, "evaluated_fraction": ev / max(bf, 1),
+                             "note": "small batch: %d CTAs on 148 SMs, latency/launch bound" % B},
+                "cpu_baseline": {"value": sb * A / dt, "unit": "agent-steps/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                 "sample": "metrics of the first %d of %d scenarios, %.2f s wall" % (sb, B, dt),
+                                 "offroad_flags_equal": bool(np.array_equal(oo["flag"], fl[:sb].cpu().numpy()))},
+                "e2e": None, "gpu_launches": int(launches), "clocks": None}
+    print(json.dumps(line))
+    wm.wm_destroy(h)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -151,12 +280,17 @@ def main():
     ap.add_argument("--cpu-B", type=int, default=16, help="oracle sample for cpu_baseline")
     ap.add_argument("--ref-B", type=int, default=8)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4"],
+                    help="rollout = the BASELINE metric (config 5, default); the others time the remaining "
+                         "SURVEY 8(a) rows on configs 3, 2, 4 (supplementary lines, same JSON shape)")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     args.steps_ref = max(1, min(args.steps, 3)); args.warmup_ref = max(1, min(args.warmup, 1))
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload != "rollout":
+        return run_supplementary(args)
 
     import torch
     import wm_scenarios as ws
