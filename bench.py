@@ -239,9 +239,11 @@ def run_supplementary(args):
         launches = (wm.wm_kernel_launches(h) - l0) * K // (K + W)
         row = sim_d if cid == 2 else log_d
         ms_ov = timed(lambda: wm.wm_metrics_overlap(h, row, t + 1 if cid == 2 else 0, bits, ofl), K, W)
-        wm.wm_offroad_stats(h)
         ms_off = timed(lambda: wm.wm_metrics_offroad(h, row, t + 1 if cid == 2 else 0, sd, None, fl), K, W)
-        ev, bf = wm.wm_offroad_stats(h)
+        wm.wm_offroad_stats_enable(h, True); wm.wm_offroad_stats(h)
+        wm.wm_metrics_offroad(h, row, t + 1 if cid == 2 else 0, sd, None, fl)
+        ev, bf, n_slow, n_corner = wm.wm_offroad_stats(h)
+        wm.wm_offroad_stats_enable(h, False)
         n_seg = np.array(wm.wm_segment_counts(h, B))
         hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 34.0
         sb = min(8, B)
@@ -257,8 +259,9 @@ def run_supplementary(args):
                 "config": {"workload": "config%d: B=%d A=%d R=%d" % (cid, B, A, rg["x"].shape[1]), "S_e_max": int(seg_max),
                            "ms_overlap": ms_ov, "ms_offroad": ms_off, "l2": ("segment tiles %d MB per call exceed L2" if n_seg.sum() * 24 > 126e6 else "segment tiles %d MB fit in L2 (small config, not flushed)") % int(n_seg.sum() * 24 / 1e6)},
                 "roofline": {"bound": "hbm", "achieved": hbm_bytes / (ms_off * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                             "frac": hbm_bytes / (ms_off * 1e-3) / 1e9 / hbm_peak, "traffic": None, "kernel": "k_offroad_cull",
-                             "kernel_ms": ms_off, "evaluated_fraction": ev / max(bf, 1),
+                             "frac": hbm_bytes / (ms_off * 1e-3) / 1e9 / hbm_peak, "traffic": None, "kernel": "k_offroad_grid",
+                             "kernel_ms": ms_off, "evaluated_fraction": ev / max(bf, 1), "pairs_per_corner": ev / max(n_corner, 1),
+                             "slow_path_corner_fraction": n_slow / max(n_corner, 1),
                              "note": "small batch: %d CTAs on 148 SMs, latency/launch bound" % B},
                 "cpu_baseline": {"value": sb * A / dt, "unit": "agent-steps/s", "cores": oracle.num_threads(), "kind": "oracle",
                                  "sample": "metrics of the first %d of %d scenarios, %.2f s wall" % (sb, B, dt),
@@ -359,10 +362,13 @@ def main():
         torch.cuda.synchronize()
         return ka.elapsed_time(kb) / N_STEPS
 
-    wm.wm_offroad_stats(h)
-    k_ms = time_offroad(h)                                     # default mode: exact search with group culling
-    ev_pairs, bf_pairs = wm.wm_offroad_stats(h)
-    pairs_eval = ev_pairs / float(N_STEPS + 3)
+    k_ms = time_offroad(h)                                     # default mode: exact grid search
+    wm.wm_offroad_stats_enable(h, True); wm.wm_offroad_stats(h)
+    for t in range(11, 11 + N_STEPS):
+        wm.wm_metrics_offroad(h, sim_d, t, sd, None, fl)
+    ev_pairs, bf_pairs, n_slow, n_corner = wm.wm_offroad_stats(h)
+    wm.wm_offroad_stats_enable(h, False)
+    pairs_eval = ev_pairs / float(N_STEPS)
     nvalid_bt = sim_d["valid"][:, 11:11 + N_STEPS].sum(dim=2).double().cpu().numpy()       # [B, 80]
     pairs_per_launch = float((4.0 * nvalid_bt * n_seg[:, None]).sum() / N_STEPS)            # brute-force count
     peaks = measured_peaks()
@@ -378,12 +384,13 @@ def main():
     bf_achieved = pairs_per_launch * FLOP_PER_PAIR / (kb_ms * 1e-3) / 1e12
     peak_src = "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz)
     roofline = {"bound": "hbm", "achieved": hbm_bytes / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": hbm_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "traffic": profiled_traffic("k_offroad_cull"),
-                "kernel": "k_offroad_cull", "kernel_ms": k_ms, "algorithmic_bytes_per_launch": hbm_bytes,
+                "frac": hbm_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "traffic": profiled_traffic("k_offroad_grid"),
+                "kernel": "k_offroad_grid", "kernel_ms": k_ms, "algorithmic_bytes_per_launch": hbm_bytes,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
                 "kernel_share_of_step": k_ms * N_STEPS / ms_step,
                 "pairs_bruteforce_per_launch": pairs_per_launch, "pairs_evaluated_per_launch": pairs_eval,
-                "evaluated_fraction": pairs_eval / pairs_per_launch,
+                "evaluated_fraction": pairs_eval / pairs_per_launch, "pairs_per_corner": ev_pairs / max(n_corner, 1),
+                "slow_path_corner_fraction": n_slow / max(n_corner, 1),
                 "alu_frac_on_evaluated_pairs": pairs_eval * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12 / fp32_peak,
                 "alu_frac_bruteforce_equivalent": pairs_per_launch * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12 / fp32_peak,
                 "note": "exact culling (SURVEY 8(d)): the FP32 fraction is given on evaluated pairs and on the brute-force count"}

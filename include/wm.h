@@ -197,10 +197,14 @@ int wm_rollout_host(wm_handle* h, const wm_traj* log_host, const wm_roadgraph* r
  * this handle has launched (graph replays count their kernel nodes). */
 int wm_segment_counts(wm_handle* h, int32_t* n_seg_host, int32_t B, void* stream);
 int64_t wm_kernel_launches(const wm_handle* h);
-/* wm_offroad_stats: out_host[0] = corner-segment pairs the culled offroad search evaluated since
- * the last call, out_host[1] = pairs a brute-force search would have evaluated for the same
- * launches (both 0 in brute-force mode). Resets the counters. */
+/* wm_offroad_stats: counters of the exact grid search (WM_OFFROAD_CULLED) since the last call,
+ * out_host[4] int64 on the HOST: [0] corner-segment pairs evaluated, [1] pairs a brute-force
+ * search would have evaluated for the same launches, [2] corners that took the full chunk
+ * search (outside the grid or a crowded cell), [3] corners queried.  Resets the counters.
+ * Counting costs global atomics, so it is off until wm_offroad_stats_enable(h, 1); toggling it
+ * drops a cached rollout graph.  All 0 in brute-force mode. */
 int wm_offroad_stats(wm_handle* h, int64_t* out_host, void* stream);
+int wm_offroad_stats_enable(wm_handle* h, int32_t on);
 
 #ifdef __cplusplus
 }

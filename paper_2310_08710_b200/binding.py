@@ -22,7 +22,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats")
+           "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
 
 
 class wm_traj(C.Structure):
@@ -212,10 +212,15 @@ def wm_kernel_launches(h):
 
 
 def wm_offroad_stats(h, stream=None):
-    """(pairs evaluated, brute-force pairs) of the culled offroad search since the last call."""
-    buf = (C.c_int64 * 2)()
+    """(pairs evaluated, brute-force pairs, slow-path corners, corners) of the exact grid search
+    since the last call; counted only after wm_offroad_stats_enable(h, True)."""
+    buf = (C.c_int64 * 4)()
     _check(load().wm_offroad_stats(h, buf, _stream(stream)), "wm_offroad_stats")
-    return int(buf[0]), int(buf[1])
+    return tuple(int(v) for v in buf)
+
+
+def wm_offroad_stats_enable(h, on=True):
+    _check(load().wm_offroad_stats_enable(h, C.c_int32(1 if on else 0)), "wm_offroad_stats_enable")
 
 
 # ---- small conveniences for tests / bench: torch allocation of the ABI's arrays ----

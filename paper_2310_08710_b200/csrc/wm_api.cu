@@ -41,8 +41,8 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
   if (major != 10) { free(h); return WM_ERR_UNSUPPORTED; }    // sm_100a kernels only; no fallback
   e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking);
-  if (e == cudaSuccess) e = cudaMalloc(&h->cull_stats, 2 * sizeof(unsigned long long));
-  if (e == cudaSuccess) e = cudaMemset(h->cull_stats, 0, 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&h->cull_stats, 4 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMemset(h->cull_stats, 0, 4 * sizeof(unsigned long long));
   if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
   *out = h;
   return WM_OK;
@@ -51,12 +51,18 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
 extern "C" int wm_offroad_stats(wm_handle* h, int64_t* out_host, void* stream) {
   if (!h || !out_host) return WM_ERR_ARG;
   cudaStream_t s = (cudaStream_t)stream;
-  unsigned long long v[2];
+  unsigned long long v[4];
   WM_CUDA(cudaMemcpyAsync(v, h->cull_stats, sizeof(v), cudaMemcpyDeviceToHost, s));
   WM_CUDA(cudaMemsetAsync(h->cull_stats, 0, sizeof(v), s));
   WM_CUDA(cudaStreamSynchronize(s));
-  out_host[0] = (int64_t)v[0] * 64 * 4;      // corner-segment pairs evaluated (64 segments x 4 corners per group)
-  out_host[1] = (int64_t)v[1] * 64 * 4;      // pairs a brute-force search would have evaluated
+  for (int i = 0; i < 4; ++i) out_host[i] = (int64_t)v[i];
+  return WM_OK;
+}
+
+extern "C" int wm_offroad_stats_enable(wm_handle* h, int32_t on) {
+  if (!h) return WM_ERR_ARG;
+  if ((h->stats_on != 0) != (on != 0)) wm_drop_graph(h);     // the counter pointer is a kernel argument
+  h->stats_on = on != 0;
   return WM_OK;
 }
 

@@ -1,0 +1,249 @@
+// a4 off-road metric, exact grid search — the default mode (WM_OFFROAD_CULLED).
+// See wm_grid.cuh for the structure and the argument why no nearest segment can be missed.
+//
+//   k_grid_params  per scenario: bounding box of the segments -> grid origin, cell side, nx, ny
+//   k_build_cells  per cell: dmin(c), then the runs of records with dist(c, s) <= dmin + 2 rho
+//   k_offroad_grid one thread per box corner, 4 lanes per agent: header load, candidate walk,
+//                  sign of the winner; max over the corners by shuffles
+//
+// Bound of k_offroad_grid: instruction issue (about 18 instructions per evaluated pair, ~25
+// pairs per corner) and L1/L2 gather latency; HBM traffic is the touched 32-byte records only.
+#include <stdlib.h>
+
+#include "wm_grid.cuh"
+
+// ======================================================================================
+// grid construction (wm_prepare)
+// ======================================================================================
+constexpr float GRID_MARGIN = 16.f;       // metres of grid beyond the segments' bounding box
+constexpr int BUILD_MAXRUN = 12;          // runs per cell before the cell falls back to the full search
+constexpr int BUILD_MAXCAND = 256;        // candidates per cell before it falls back
+
+__global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const float4* chunks, int seg_cap, float h_min,
+                                                     WmGrid* gridp, int32_t* pool_cnt) {
+  __shared__ float s_red[4][4];
+  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n = n_seg[b], nch = (n + WM_CHUNK - 1) / WM_CHUNK;
+  const float4* ch = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
+  float x0 = 3.0e38f, y0 = 3.0e38f, x1 = -3.0e38f, y1 = -3.0e38f;
+  for (int c = tid; c < nch; c += blockDim.x) {
+    const float4 bb = ch[c];
+    x0 = fminf(x0, bb.x); y0 = fminf(y0, bb.y); x1 = fmaxf(x1, bb.z); y1 = fmaxf(y1, bb.w);
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    x0 = fminf(x0, __shfl_xor_sync(0xffffffffu, x0, d)); y0 = fminf(y0, __shfl_xor_sync(0xffffffffu, y0, d));
+    x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, d)); y1 = fmaxf(y1, __shfl_xor_sync(0xffffffffu, y1, d));
+  }
+  if (lane == 0) { s_red[0][warp] = x0; s_red[1][warp] = y0; s_red[2][warp] = x1; s_red[3][warp] = y1; }
+  __syncthreads();
+  if (tid == 0) {
+    for (int w = 1; w < 4; ++w) {
+      x0 = fminf(x0, s_red[0][w]); y0 = fminf(y0, s_red[1][w]); x1 = fmaxf(x1, s_red[2][w]); y1 = fmaxf(y1, s_red[3][w]);
+    }
+    WmGrid g;
+    g.nseg = n; g.pad = 0;
+    if (n <= 0) { g.x0 = 0.f; g.y0 = 0.f; g.h = h_min; g.inv_h = 1.f / h_min; g.nx = 0; g.ny = 0; }
+    else {
+      const float W = (x1 - x0) + 2.f * GRID_MARGIN, H = (y1 - y0) + 2.f * GRID_MARGIN;
+      const float h = fmaxf(h_min, fmaxf(W, H) * (1.0001f / WM_GRID_NG));
+      g.x0 = x0 - GRID_MARGIN; g.y0 = y0 - GRID_MARGIN; g.h = h; g.inv_h = 1.f / h;
+      g.nx = min(WM_GRID_NG, (int)ceilf(W / h)); g.ny = min(WM_GRID_NG, (int)ceilf(H / h));
+    }
+    gridp[b] = g;
+    pool_cnt[b] = 0;
+  }
+}
+
+// plain float32 distance^2 from a cell centre to a record (safety comes from the slack below)
+__device__ __forceinline__ float centre_d2(const float4 r0, const float4 r1, float cx, float cy) {
+  const float wx = cx - r0.x, wy = cy - r0.y;
+  const float t = __saturatef(fmaf(wy, r1.y, wx * r1.x));
+  const float rx = fmaf(-t, r0.z, wx), ry = fmaf(-t, r0.w, wy);
+  return fmaf(ry, ry, rx * rx);
+}
+
+// One warp per block of 8 x 4 cells, one lane per cell.  Chunks that cannot hold a candidate of
+// any cell of the block are dropped with one box-box test per chunk (lanes over chunks); the
+// survivors are walked twice with lanes over cells: dmin(c), then the candidate runs.
+__global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* chunks, int seg_cap,
+                                                     const WmGrid* gridp, uint4* cells, uint32_t* pool, int32_t* pool_cnt) {
+  __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
+  const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const WmGrid g = gridp[b];
+  const int nbx = (g.nx + 7) >> 3, nby = (g.ny + 3) >> 2;
+  const int wg = blockIdx.x * 8 + warp;
+  if (wg >= nbx * nby) return;                                  // warp-uniform
+  const int bx = wg % nbx, by = wg / nbx;
+  const int ix = bx * 8 + (lane & 7), iy = by * 4 + (lane >> 3);
+  const bool in = ix < g.nx && iy < g.ny;
+  const float4* rec = segrec + (int64_t)b * seg_cap * 2;
+  const float4* ch = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
+  const int n = g.nseg, nch = (n + WM_CHUNK - 1) / WM_CHUNK;
+  const float h = g.h;
+  const float cx = g.x0 + ((float)ix + 0.5f) * h, cy = g.y0 + ((float)iy + 0.5f) * h;
+  // cell box inflated by delta (float32 rounding of the query's cell index), half diagonal rho
+  const float delta = 1e-3f + 1e-4f * h;
+  const float rho = 1.41421362f * (0.5f * h + delta);
+  // block box
+  const float X0 = g.x0 + (float)(bx * 8) * h - delta, X1 = g.x0 + (float)(bx * 8 + 8) * h + delta;
+  const float Y0 = g.y0 + (float)(by * 4) * h - delta, Y1 = g.y0 + (float)(by * 4 + 4) * h + delta;
+  const float INF = __int_as_float(0x7f800000);
+
+  // upper bound for the whole block: every cell centre has a segment within maxdist(block, chunk box)
+  float ub2 = INF;
+  for (int c = lane; c < nch; c += 32) {
+    const float4 bb = __ldg(ch + c);
+    const float dx = fmaxf(fabsf(X1 - bb.x), fabsf(bb.z - X0)), dy = fmaxf(fabsf(Y1 - bb.y), fabsf(bb.w - Y0));
+    ub2 = fminf(ub2, fmaf(dx, dx, dy * dy));
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) ub2 = fminf(ub2, __shfl_xor_sync(0xffffffffu, ub2, d));
+  const float reach = sqrtf(ub2) * 1.001f + 2.f * rho + 2e-3f;   // no candidate of any cell lies farther from the block
+  const float reach2 = reach * reach;
+  auto survivors = [&](int r) -> uint32_t {
+    const int c = r * 32 + lane;
+    bool sv = false;
+    if (c < nch) {
+      const float4 bb = __ldg(ch + c);
+      const float dx = fmaxf(fmaxf(bb.x - X1, X0 - bb.z), 0.f), dy = fmaxf(fmaxf(bb.y - Y1, Y0 - bb.w), 0.f);
+      sv = fmaf(dx, dx, dy * dy) <= reach2;
+    }
+    return __ballot_sync(0xffffffffu, sv);
+  };
+  const int nround = (nch + 31) >> 5;
+
+  // pass 1: dmin(c)
+  float dmin2 = INF;
+  for (int r = 0; r < nround; ++r) {
+    uint32_t mask = survivors(r);
+    while (mask) {
+      const int c = r * 32 + __ffs(mask) - 1;
+      mask &= mask - 1;
+      const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
+#pragma unroll 4
+      for (int s = s0; s < s1; ++s) dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * s), __ldg(rec + 2 * s + 1), cx, cy));
+    }
+  }
+  // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack), as runs of consecutive records
+  const float dmin = sqrtf(dmin2);
+  const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
+  const float thr2 = thr * thr;
+  int nr = 0, ncand = 0, rs = 0, rl = 0;
+  for (int r = 0; r < nround; ++r) {
+    uint32_t mask = survivors(r);
+    while (mask) {
+      const int c = r * 32 + __ffs(mask) - 1;
+      mask &= mask - 1;
+      const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
+#pragma unroll 2
+      for (int s = s0; s < s1; ++s) {
+        const float d2 = centre_d2(__ldg(rec + 2 * s), __ldg(rec + 2 * s + 1), cx, cy);
+        if (in && d2 <= thr2) {
+          ++ncand;
+          if (rl > 0 && s == rs + rl && rl < 255) ++rl;
+          else {
+            if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; }
+            rs = s; rl = 1;
+          }
+        }
+      }
+    }
+  }
+  if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; }
+  if (!in) return;
+  uint4 hd = make_uint4(0xffffffffu, 0xffffffffu, 0u, 0u);     // fall back to the full search
+  if (nr <= 4 && ncand <= BUILD_MAXCAND) {
+    hd.x = nr > 0 ? s_runs[warp][0][lane] : 0u;                 // nr >= 1 whenever n > 0
+    hd.y = nr > 1 ? s_runs[warp][1][lane] : 0u;
+    hd.z = nr > 2 ? s_runs[warp][2][lane] : 0u;
+    hd.w = nr > 3 ? s_runs[warp][3][lane] : 0u;
+  } else if (nr <= BUILD_MAXRUN && ncand <= BUILD_MAXCAND) {
+    const int off = atomicAdd(&pool_cnt[b], nr);
+    if (off + nr <= WM_POOL_CAP) {
+      uint32_t* pr = pool + (int64_t)b * WM_POOL_CAP + off;
+      for (int i = 0; i < nr; ++i) pr[i] = s_runs[warp][i][lane];
+      hd.y = (uint32_t)off; hd.z = (uint32_t)nr;
+    }
+  }
+  cells[(int64_t)b * WM_GRID_CELLS + iy * g.nx + ix] = hd;
+}
+
+cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s) {
+  static float h_min = 0.f;
+  if (h_min <= 0.f) { const char* e = getenv("WM_GRID_CELL"); h_min = e ? (float)atof(e) : 2.0f; if (!(h_min >= 0.25f && h_min <= 64.f)) h_min = 2.0f; }
+  const int seg_cap = h->seg_tiles * WM_TILE_SEGS;
+  k_grid_params<<<B, 128, 0, s>>>(h->n_seg, h->chunks, seg_cap, h_min, h->gridp, h->pool_cnt);
+  h->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const int nwarps = (WM_GRID_NG / 8) * (WM_GRID_NG / 4);
+  k_build_cells<<<dim3(nwarps / 8, B), 256, 0, s>>>(h->segrec, h->chunks, seg_cap, h->gridp, h->cells, h->pool, h->pool_cnt);
+  h->launches++;
+  return cudaGetLastError();
+}
+
+// ======================================================================================
+// k_offroad_grid
+// ======================================================================================
+struct GridParams {
+  wm_row row;
+  int A;
+  const float4* segrec; const float4* chunks; const uint4* cells; const uint32_t* pool; const WmGrid* gridp;
+  int seg_cap;
+  float* sd; int64_t sd_stride_b;
+  float* corner;
+  uint8_t* flag; int64_t flag_stride_b;
+  unsigned long long* stats;
+};
+
+__global__ void __launch_bounds__(128) k_offroad_grid(GridParams p) {
+  const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
+  const int a = blockIdx.x * 32 + (tid >> 2), k = tid & 3;
+  const int A = p.A;
+  const int64_t ro = (int64_t)b * p.row.stride_b;
+  const bool v = a < A && p.row.valid[ro + a] != 0;
+  const WmGridView gv = wm_grid_view(p.segrec, p.chunks, p.cells, p.pool, p.gridp, p.seg_cap, WM_POOL_CAP, b);
+  int n_eval = 0;
+  bool slow = false;
+  float cx = 0.f, cy = 0.f, offx = 0.f, offy = 0.f;
+  if (v) {
+    cx = p.row.x[ro + a]; cy = p.row.y[ro + a];
+    float ax, ay, bx, by;
+    wm_box_offsets(p.row.yaw[ro + a], p.row.length[ro + a], p.row.width[ro + a], ax, ay, bx, by);
+    const float ox = (k & 1) ? bx : ax, oy = (k & 1) ? by : ay;
+    offx = (k & 2) ? -ox : ox; offy = (k & 2) ? -oy : oy;
+  }
+  const float sd = wm_grid_corner_sd(gv, v, cx, cy, offx, offy, n_eval, slow);     // 0 for invalid agents (D10)
+  if (a < A && p.corner) p.corner[((int64_t)b * 4 + k) * A + a] = sd;
+  float m = fmaxf(sd, __shfl_xor_sync(0xffffffffu, sd, 1));                  // D18: max over the 4 corners
+  m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+  if (k == 0 && a < A) {
+    p.sd[(int64_t)b * p.sd_stride_b + a] = v ? m : 0.f;
+    p.flag[(int64_t)b * p.flag_stride_b + a] = (uint8_t)(v && m > 0.f);      // D19
+  }
+  if (p.stats) {
+    const unsigned ne = __reduce_add_sync(0xffffffffu, (unsigned)n_eval);
+    const unsigned nv = __popc(__ballot_sync(0xffffffffu, v)), ns = __popc(__ballot_sync(0xffffffffu, slow));
+    if (lane == 0 && nv) {
+      atomicAdd(&p.stats[0], (unsigned long long)ne);
+      atomicAdd(&p.stats[1], (unsigned long long)nv * (unsigned long long)max(gv.g.nseg, 0));
+      if (ns) atomicAdd(&p.stats[2], (unsigned long long)ns);
+      atomicAdd(&p.stats[3], (unsigned long long)nv);
+    }
+  }
+}
+
+cudaError_t wm_launch_offroad_grid(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
+                                   float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s) {
+  GridParams p;
+  p.row = wm_make_row(sim, t);
+  p.A = sim.A;
+  p.segrec = h->segrec; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
+  p.seg_cap = h->seg_tiles * WM_TILE_SEGS;
+  p.sd = sd; p.sd_stride_b = sd_stride_b; p.corner = corner; p.flag = flag; p.flag_stride_b = flag_stride_b;
+  p.stats = h->stats_on ? h->cull_stats : nullptr;
+  k_offroad_grid<<<dim3((sim.A + 31) / 32, sim.B), 128, 0, s>>>(p);
+  h->launches++;
+  return cudaGetLastError();
+}

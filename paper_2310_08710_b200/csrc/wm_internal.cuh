@@ -24,6 +24,18 @@ constexpr int WM_TILE_F4 = 8 * 3 * 32;     // float4 per tile
 constexpr int WM_TILE_BYTES = WM_TILE_F4 * 16;   // 12288
 constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding segments
 
+// Exact grid search (wm_grid.cuh): road-edge segments in ascending source order as 32-byte
+// records, bounding boxes per chunk of WM_CHUNK records, and a grid of at most
+// WM_GRID_NG x WM_GRID_NG cells per scenario, each with a 16-byte header:
+//   {run, run, run, run}          up to 4 inline runs, run = (first record << 8) | count, 0 = none
+//   {~0, pool offset, n runs, 0}  more runs, in the scenario's pool
+//   {~0, ~0, 0, 0}                too many candidates: search all chunks
+constexpr int WM_CHUNK = 32;
+constexpr int WM_GRID_NG = 128;
+constexpr int WM_GRID_CELLS = WM_GRID_NG * WM_GRID_NG;
+constexpr int WM_POOL_CAP = 2 * WM_GRID_CELLS;   // overflow runs per scenario
+struct WmGrid { float x0, y0, inv_h, h; int nx, ny, nseg, pad; };
+
 // Prepared roadgraph points for top-k: float2 (x, y) per point, invalid -> (WM_FAR, WM_FAR),
 // padded to a multiple of WM_PT_TILE.
 constexpr int WM_PT_TILE = 2048;
@@ -41,7 +53,12 @@ struct wm_handle {
   float4* edges;            // [B][seg_tiles][WM_TILE_F4]
   float2* sign_dir;         // [B][seg_tiles*512]  sign direction (e, or stored dir if e == 0)
   int32_t* seg_src;         // [B][seg_tiles*512]  first-point index of each stored segment (-1: padding)
-  float4* groups;           // [B][seg_tiles*8]    bounding circle {cx, cy, r, 0} of each 64-segment group
+  float4* segrec;           // [B][seg_tiles*512][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}, ascending source order
+  float4* chunks;           // [B][seg_tiles*16]   bounding box of each chunk of 32 records
+  WmGrid* gridp;            // [B]
+  uint4* cells;             // [B][WM_GRID_CELLS]  cell headers
+  uint32_t* pool;           // [B][WM_POOL_CAP]    overflow runs
+  int32_t* pool_cnt;        // [B]
   int32_t pts_pad;          // padded R
   float2* pts;              // [B][pts_pad]
   // rollout graph cache
@@ -53,7 +70,8 @@ struct wm_handle {
   // scratch for rollouts / host staging
   void* scratch; size_t scratch_bytes;
   void* stage[16]; size_t stage_bytes[16];
-  unsigned long long* cull_stats;   // device [2]: groups evaluated, groups considered (culled mode)
+  unsigned long long* cull_stats;   // device [4]: pairs evaluated, brute-force pairs, slow-path corners, corners
+  int stats_on;                     // counters are collected only when enabled (wm_offroad_stats_enable)
 };
 
 extern thread_local int g_wm_last_cuda_error;
@@ -102,10 +120,11 @@ cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t*
                               uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
 cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
                               float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
-cudaError_t wm_launch_offroad_culled(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
+cudaError_t wm_launch_offroad_grid(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
                                      float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
 cudaError_t wm_launch_aggregate(wm_handle* h, int B, int A, int n_steps, const wm_rollout_out& out,
                                 const uint8_t* ld_valid_rows, cudaStream_t s);
+cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s);
 int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);
 void wm_prepare_free(wm_handle* h);
 void wm_drop_graph(wm_handle* h);
@@ -126,6 +145,18 @@ __device__ __forceinline__ wm_u64 add2(wm_u64 a, wm_u64 b) { wm_u64 d; asm("add.
 __device__ __forceinline__ wm_u64 sub2(wm_u64 a, wm_u64 b) { wm_u64 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ wm_u64 mul2(wm_u64 a, wm_u64 b) { wm_u64 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ float min3f(float a, float b, float c) { float d; asm("min.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c)); return d; }
+
+// corner offsets of a box: a = front-left, b = front-right; corners 0..3 = c+a, c+b, c-a, c-b
+// (D30).  Explicit round-to-nearest ops so that every kernel derives bit-identical offsets.
+__device__ __forceinline__ void wm_box_offsets(float yaw, float length, float width, float& ax, float& ay, float& bx,
+                                               float& by) {
+  float sn, cs;
+  sincosf(yaw, &sn, &cs);
+  const float hl = 0.5f * length, hw = 0.5f * width;
+  const float hfx = __fmul_rn(hl, cs), hfy = __fmul_rn(hl, sn), hsx = -__fmul_rn(hw, sn), hsy = __fmul_rn(hw, cs);
+  ax = __fadd_rn(hfx, hsx); ay = __fadd_rn(hfy, hsy);
+  bx = __fsub_rn(hfx, hsx); by = __fsub_rn(hfy, hsy);
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {

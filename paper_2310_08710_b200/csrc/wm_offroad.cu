@@ -58,89 +58,31 @@ __global__ void __launch_bounds__(256) k_count_segments(RgView g, int32_t* n_seg
 }
 
 // ---------------------------------------------------------------------------------------
-// Spatial order.  Segments are stored in the order (Morton code of the grid cell that holds
-// their first point, first-point index): inside a cell, polyline pieces stay contiguous, and
-// any 64 consecutive stored segments (a "group": one packed iteration of a warp) form a compact
-// cluster whose bounding box lets the culled kernel skip the whole group exactly.
-// k_sort_segments writes the permutation into seg_src.  `grid` cells per axis (<= 64) over the
-// scenario's own bounding box.
+// Segment order = ascending first-point index (order-preserving compaction), so that "lower
+// stored index" IS the tie rule D17 everywhere, and polyline pieces stay contiguous (the grid
+// cells of wm_grid.cu hold runs of consecutive records).  k_order_segments writes seg_src.
 // ---------------------------------------------------------------------------------------
-constexpr int SORT_CELLS = 64 * 64;                 // counters (4096 = 4 per thread)
-
-__device__ __forceinline__ uint32_t part1by1(uint32_t v) {   // spread the low 6 bits
-  v &= 0x3fu;
-  v = (v | (v << 4)) & 0x30fu;
-  v = (v | (v << 2)) & 0x333u;
-  v = (v | (v << 1)) & 0x555u;
-  return v;
-}
-
-__global__ void __launch_bounds__(1024) k_sort_segments(RgView g, int cap, int32_t* seg_src, int grid) {
-  __shared__ int s_cnt[SORT_CELLS];
-  __shared__ int s_start[SORT_CELLS];
-  __shared__ float s_red[4][32];
-  __shared__ int s_wsum[32];
+__global__ void __launch_bounds__(1024) k_order_segments(RgView g, int cap, int32_t* seg_src) {
+  __shared__ int s_w[32];
+  __shared__ int s_base;
   const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t o = (int64_t)b * g.R;
   int32_t* out = seg_src + (int64_t)b * cap;
-  // bounding box of the records' first points
-  float x0 = 3.0e38f, y0 = 3.0e38f, x1 = -3.0e38f, y1 = -3.0e38f;
-  for (int i = tid; i < g.R; i += blockDim.x) {
+  if (tid == 0) s_base = 0;
+  __syncthreads();
+  for (int base = 0; base < g.R; base += 1024) {
+    const int i = base + tid;
     bool sg;
-    if (rg_record(g, o, i, &sg)) {
-      const float x = g.x[o + i], y = g.y[o + i];
-      x0 = fminf(x0, x); y0 = fminf(y0, y); x1 = fmaxf(x1, x); y1 = fmaxf(y1, y);
-    }
-  }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) {
-    x0 = fminf(x0, __shfl_xor_sync(0xffffffffu, x0, d)); y0 = fminf(y0, __shfl_xor_sync(0xffffffffu, y0, d));
-    x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, d)); y1 = fmaxf(y1, __shfl_xor_sync(0xffffffffu, y1, d));
-  }
-  if (lane == 0) { s_red[0][warp] = x0; s_red[1][warp] = y0; s_red[2][warp] = x1; s_red[3][warp] = y1; }
-  for (int c = tid; c < SORT_CELLS; c += blockDim.x) s_cnt[c] = 0;
-  __syncthreads();
-  x0 = s_red[0][0]; y0 = s_red[1][0]; x1 = s_red[2][0]; y1 = s_red[3][0];
-  for (int w = 1; w < 32; ++w) {
-    x0 = fminf(x0, s_red[0][w]); y0 = fminf(y0, s_red[1][w]); x1 = fmaxf(x1, s_red[2][w]); y1 = fmaxf(y1, s_red[3][w]);
-  }
-  const float sx = (float)grid / fmaxf(x1 - x0, 1e-3f), sy = (float)grid / fmaxf(y1 - y0, 1e-3f);
-  auto cell_of = [&](int i) -> int {
-    const int ix = min(grid - 1, max(0, (int)((g.x[o + i] - x0) * sx)));
-    const int iy = min(grid - 1, max(0, (int)((g.y[o + i] - y0) * sy)));
-    return (int)(part1by1((uint32_t)ix) | (part1by1((uint32_t)iy) << 1));
-  };
-  for (int i = tid; i < g.R; i += blockDim.x) { bool sg; if (rg_record(g, o, i, &sg)) atomicAdd(&s_cnt[cell_of(i)], 1); }
-  __syncthreads();
-  // exclusive scan of the 4096 counters: 4 per thread
-  int c4[4], sum = 0;
-#pragma unroll
-  for (int q = 0; q < 4; ++q) { c4[q] = s_cnt[tid * 4 + q]; sum += c4[q]; }
-  int inc = sum;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-  if (lane == 31) s_wsum[warp] = inc;
-  __syncthreads();
-  int base = 0;
-  for (int w = 0; w < warp; ++w) base += s_wsum[w];
-  int run = base + inc - sum;
-#pragma unroll
-  for (int q = 0; q < 4; ++q) { s_start[tid * 4 + q] = run; run += c4[q]; }
-  __syncthreads();
-  for (int c = tid; c < SORT_CELLS; c += blockDim.x) s_cnt[c] = s_start[c];          // cursors
-  __syncthreads();
-  for (int i = tid; i < g.R; i += blockDim.x) { bool sg; if (rg_record(g, o, i, &sg)) out[atomicAdd(&s_cnt[cell_of(i)], 1)] = i; }
-  __syncthreads();
-  // deterministic order inside a cell: ascending point index (insertion sort, cells are small)
-#pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    const int c = tid * 4 + q, lo = s_start[c], hi = s_cnt[c];
-    for (int a = lo + 1; a < hi; ++a) {
-      const int v = out[a];
-      int k = a - 1;
-      while (k >= lo && out[k] > v) { out[k + 1] = out[k]; --k; }
-      out[k + 1] = v;
-    }
+    const bool rec = rg_record(g, o, i, &sg);
+    const uint32_t bal = __ballot_sync(0xffffffffu, rec);
+    if (lane == 0) s_w[warp] = __popc(bal);
+    __syncthreads();
+    int pre = s_base;
+    for (int w = 0; w < warp; ++w) pre += s_w[w];
+    if (rec) out[pre + __popc(bal & ((1u << lane) - 1u))] = i;
+    __syncthreads();
+    if (tid == 0) { int tot = 0; for (int w = 0; w < 32; ++w) tot += s_w[w]; s_base += tot; }
+    __syncthreads();
   }
 }
 
@@ -159,10 +101,10 @@ __device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir
   sign_dir[s] = make_float2(sx, sy);
 }
 
-// One warp per group of 64 stored segments: writes the tile records and the group's bounding
-// circle {cx, cy, r, 0} (r inflated so that float32 rounding can never make the bound unsafe).
+// One warp per group of 64 stored segments: writes the tile records (brute-force layout), the
+// 32-byte records of the grid search, and the bounding box of each chunk of 32 records.
 __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, const int32_t* n_seg, float4* edges,
-                                                       float2* sign_dir, int32_t* seg_src, float4* groups) {
+                                                       float2* sign_dir, int32_t* seg_src, float4* segrec, float4* chunks) {
   const int b = blockIdx.y, lane = threadIdx.x & 31;
   const int grp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int ngrp = seg_tiles * (WM_TILE_SEGS / 64);
@@ -190,24 +132,30 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
       if (ee > 0.f) { gx = ex / ee; gy = ey / ee; sx = ex; sy = ey; }
       else { ex = 0.f; ey = 0.f; sx = g.dir_x[o + i]; sy = g.dir_y[o + i]; }     // D16 / D29
       store_segment(tile_base, sd, s, p0x, p0y, ex, ey, gx, gy, sx, sy);
+      float4* rec = segrec + ((int64_t)b * cap + s) * 2;
+      rec[0] = make_float4(p0x, p0y, ex, ey);
+      rec[1] = make_float4(gx, gy, sx, sy);
       ax[hf] = p0x; ay[hf] = p0y; bx[hf] = p0x + ex; by[hf] = p0y + ey;
       x0 = fminf(x0, fminf(ax[hf], bx[hf])); x1 = fmaxf(x1, fmaxf(ax[hf], bx[hf]));
       y0 = fminf(y0, fminf(ay[hf], by[hf])); y1 = fmaxf(y1, fmaxf(ay[hf], by[hf]));
     } else {                                      // padding: far away, never wins against a real segment
       store_segment(tile_base, sd, s, WM_FAR, WM_FAR, 0.f, 0.f, 0.f, 0.f, 1.f, 0.f);
+      float4* rec = segrec + ((int64_t)b * cap + s) * 2;
+      rec[0] = make_float4(WM_FAR, WM_FAR, 0.f, 0.f);
+      rec[1] = make_float4(0.f, 0.f, 1.f, 0.f);
       src[s] = -1;
     }
   }
 #pragma unroll
-  for (int d = 16; d > 0; d >>= 1) {
+  for (int d = 8; d > 0; d >>= 1) {             // 16 lanes = one chunk of 32 records
     x0 = fminf(x0, __shfl_xor_sync(0xffffffffu, x0, d)); y0 = fminf(y0, __shfl_xor_sync(0xffffffffu, y0, d));
     x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, d)); y1 = fmaxf(y1, __shfl_xor_sync(0xffffffffu, y1, d));
   }
-  // axis-aligned bounding box {x0, y0, x1, y1} of the group's segments (exact: min/max of the
-  // float32 endpoints; p1 = p0 + e may round by an ulp, covered by the kernel's 1e-3 m slack)
-  if (lane == 0) {
+  // axis-aligned bounding box {x0, y0, x1, y1} of the chunk's segments (min/max of the float32
+  // endpoints; p1 = p0 + e may round by an ulp, covered by the slack of the cull tests)
+  if ((lane & 15) == 0) {
     const bool any = x1 >= x0;
-    groups[(int64_t)b * ngrp + grp] = any ? make_float4(x0, y0, x1, y1) : make_float4(WM_FAR, WM_FAR, WM_FAR, WM_FAR);
+    chunks[(int64_t)b * ngrp * 2 + grp * 2 + (lane >> 4)] = any ? make_float4(x0, y0, x1, y1) : make_float4(WM_FAR, WM_FAR, WM_FAR, WM_FAR);
   }
 }
 
@@ -222,8 +170,10 @@ __global__ void __launch_bounds__(256) k_pack_points(RgView g, int pts_pad, floa
 }
 
 void wm_prepare_free(wm_handle* h) {
-  cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pts); cudaFree(h->groups);
-  h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pts = nullptr; h->groups = nullptr;
+  cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pts);
+  cudaFree(h->segrec); cudaFree(h->chunks); cudaFree(h->gridp); cudaFree(h->cells); cudaFree(h->pool); cudaFree(h->pool_cnt);
+  h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pts = nullptr;
+  h->segrec = nullptr; h->chunks = nullptr; h->gridp = nullptr; h->cells = nullptr; h->pool = nullptr; h->pool_cnt = nullptr;
   h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0; h->pts_pad = 0;
 }
 
@@ -238,6 +188,10 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
     WM_CUDA(cudaMalloc(&h->n_seg, (size_t)B * sizeof(int32_t)));
     h->pts_pad = (R + WM_PT_TILE - 1) / WM_PT_TILE * WM_PT_TILE;
     WM_CUDA(cudaMalloc(&h->pts, (size_t)B * h->pts_pad * sizeof(float2)));
+    WM_CUDA(cudaMalloc(&h->gridp, (size_t)B * sizeof(WmGrid)));
+    WM_CUDA(cudaMalloc(&h->cells, (size_t)B * WM_GRID_CELLS * sizeof(uint4)));
+    WM_CUDA(cudaMalloc(&h->pool, (size_t)B * WM_POOL_CAP * sizeof(uint32_t)));
+    WM_CUDA(cudaMalloc(&h->pool_cnt, (size_t)B * sizeof(int32_t)));
     h->prep_B = B; h->prep_R = R;
   }
   k_count_segments<<<B, 256, 0, s>>>(g, h->n_seg);
@@ -256,26 +210,26 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
   if (tiles < 1) tiles = 1;
   if (tiles > h->seg_tiles || !h->edges) {       // grow only: seg_tiles is the row stride of `edges`
     wm_drop_graph(h);
-    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->groups);
-    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->groups = nullptr;
+    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->segrec); cudaFree(h->chunks);
+    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->segrec = nullptr; h->chunks = nullptr;
     h->seg_tiles = tiles;
     const size_t cap = (size_t)tiles * WM_TILE_SEGS;
     WM_CUDA(cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES));
     WM_CUDA(cudaMalloc(&h->sign_dir, (size_t)B * cap * sizeof(float2)));
     WM_CUDA(cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t)));
-    WM_CUDA(cudaMalloc(&h->groups, (size_t)B * tiles * (WM_TILE_SEGS / 64) * sizeof(float4)));
+    WM_CUDA(cudaMalloc(&h->segrec, (size_t)B * cap * 2 * sizeof(float4)));
+    WM_CUDA(cudaMalloc(&h->chunks, (size_t)B * (cap / WM_CHUNK) * sizeof(float4)));
   }
-  static int sort_grid = 0;
-  if (!sort_grid) { const char* e = getenv("WM_SORT_GRID"); sort_grid = e ? atoi(e) : 16; if (sort_grid < 1 || sort_grid > 64) sort_grid = 16; }
-  k_sort_segments<<<B, 1024, 0, s>>>(g, h->seg_tiles * WM_TILE_SEGS, h->seg_src, sort_grid);
+  k_order_segments<<<B, 1024, 0, s>>>(g, h->seg_tiles * WM_TILE_SEGS, h->seg_src);
   h->launches++;
   WM_CUDA(cudaGetLastError());
   {
     const int ngrp = h->seg_tiles * (WM_TILE_SEGS / 64);
-    k_fill_segments<<<dim3((ngrp + 7) / 8, B), 256, 0, s>>>(g, h->seg_tiles, h->n_seg, h->edges, h->sign_dir, h->seg_src, h->groups);
+    k_fill_segments<<<dim3((ngrp + 7) / 8, B), 256, 0, s>>>(g, h->seg_tiles, h->n_seg, h->edges, h->sign_dir, h->seg_src, h->segrec, h->chunks);
   }
   h->launches++;
   WM_CUDA(cudaGetLastError());
+  WM_CUDA(wm_launch_build_grid(h, B, s));
   k_pack_points<<<dim3((h->pts_pad + 255) / 256, B), 256, 0, s>>>(g, h->pts_pad, h->pts);
   h->launches++;
   WM_CUDA(cudaGetLastError());
@@ -366,13 +320,11 @@ __global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams
     if (v) {
       const int ci = pre + __popc(bal & ((1u << lane) - 1u));
       const float x = p.row.x[ro + a], y = p.row.y[ro + a];
-      float sn, cs;
-      sincosf(p.row.yaw[ro + a], &sn, &cs);
-      const float hl = 0.5f * p.row.length[ro + a], hw = 0.5f * p.row.width[ro + a];
-      const float hfx = hl * cs, hfy = hl * sn, hsx = -hw * sn, hsy = hw * cs;
-      s_ag[0 * Ap + ci] = x;          s_ag[1 * Ap + ci] = y;
-      s_ag[2 * Ap + ci] = hfx + hsx;  s_ag[3 * Ap + ci] = hfy + hsy;   // a: front-left offset
-      s_ag[4 * Ap + ci] = hfx - hsx;  s_ag[5 * Ap + ci] = hfy - hsy;   // b: front-right offset
+      float oax, oay, obx, oby;
+      wm_box_offsets(p.row.yaw[ro + a], p.row.length[ro + a], p.row.width[ro + a], oax, oay, obx, oby);
+      s_ag[0 * Ap + ci] = x;    s_ag[1 * Ap + ci] = y;
+      s_ag[2 * Ap + ci] = oax;  s_ag[3 * Ap + ci] = oay;   // a: front-left offset
+      s_ag[4 * Ap + ci] = obx;  s_ag[5 * Ap + ci] = oby;   // b: front-right offset
       s_aidx[ci] = a;
     } else if (a < A) {                                                 // D10: zeros for invalid agents
       p.sd[(int64_t)b * p.sd_stride_b + a] = 0.f;
@@ -531,7 +483,7 @@ __global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams
 cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
                               float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s) {
   if (h->cfg.offroad_mode != WM_OFFROAD_BRUTE_FORCE)
-    return wm_launch_offroad_culled(h, sim, t, sd, sd_stride_b, corner, flag, flag_stride_b, s);
+    return wm_launch_offroad_grid(h, sim, t, sd, sd_stride_b, corner, flag, flag_stride_b, s);
   OffroadParams p;
   p.row = wm_make_row(sim, t);
   p.A = sim.A;
