@@ -69,6 +69,7 @@ typedef struct {
   int32_t history;      /* 11 steps: the first second of the log (L78) */
   int32_t topk;         /* 1000 nearest roadgraph points per ego (D23) */
   int32_t offroad_mode; /* WM_OFFROAD_*: how wm_metrics_offroad / wm_rollout search the segments */
+  int32_t rollout_mode; /* WM_ROLLOUT_*: how wm_rollout runs the n_steps */
 } wm_config;
 
 /* Both modes return the same values (the nearest segment is found exactly in both).
@@ -76,6 +77,13 @@ typedef struct {
  *   64; a group is evaluated only if its lower bound can beat the current best of the agent.
  * BRUTE_FORCE: every corner-segment pair is evaluated (the FP32-roofline reference kernel). */
 enum { WM_OFFROAD_CULLED = 0, WM_OFFROAD_BRUTE_FORCE = 1 };
+
+/* Both modes return bit-identical rows (same device arithmetic), both as one CUDA graph (L200).
+ * FUSED (default): one kernel, one CTA per scenario, state resident in shared memory for all
+ *   n_steps; needs WM_OFFROAD_CULLED (with BRUTE_FORCE the stepwise graph is used).
+ * STEPWISE: n_steps x {k_step, k_overlap, k_offroad} + k_aggregate, the kernels of the single-step
+ *   entry points. */
+enum { WM_ROLLOUT_FUSED = 0, WM_ROLLOUT_STEPWISE = 1 };
 
 typedef struct wm_handle wm_handle; /* opaque */
 

@@ -15,6 +15,7 @@ WM_OK, WM_ERR_ARG, WM_ERR_CUDA, WM_ERR_UNSUPPORTED, WM_ERR_STATE = 0, -1, -2, -3
 WM_DYN_INVERTIBLE_BICYCLE, WM_DYN_DELTA_LOCAL = 0, 1
 WM_TYPE_LANE, WM_TYPE_ROAD_EDGE = 1, 2
 WM_OFFROAD_CULLED, WM_OFFROAD_BRUTE_FORCE = 0, 1
+WM_ROLLOUT_FUSED, WM_ROLLOUT_STEPWISE = 0, 1
 _ERR = {-1: "WM_ERR_ARG", -2: "WM_ERR_CUDA", -3: "WM_ERR_UNSUPPORTED", -4: "WM_ERR_STATE"}
 
 TRAJ_F = ("x", "y", "yaw", "vel_x", "vel_y", "length", "width")
@@ -38,7 +39,7 @@ class wm_roadgraph(C.Structure):
 class wm_config(C.Structure):
     _fields_ = [("dynamics", C.c_int32), ("dt", C.c_float), ("max_accel", C.c_float),
                 ("max_curvature", C.c_float), ("history", C.c_int32), ("topk", C.c_int32),
-                ("offroad_mode", C.c_int32)]
+                ("offroad_mode", C.c_int32), ("rollout_mode", C.c_int32)]
 
 
 class wm_rollout_out(C.Structure):
@@ -125,9 +126,9 @@ def wm_version():
 
 
 def wm_create(dynamics=WM_DYN_INVERTIBLE_BICYCLE, dt=0.1, max_accel=6.0, max_curvature=0.3, history=11, topk=1000,
-              offroad_mode=WM_OFFROAD_CULLED):
+              offroad_mode=WM_OFFROAD_CULLED, rollout_mode=WM_ROLLOUT_FUSED):
     h = C.c_void_p()
-    cfg = wm_config(dynamics, dt, max_accel, max_curvature, history, topk, offroad_mode)
+    cfg = wm_config(dynamics, dt, max_accel, max_curvature, history, topk, offroad_mode, rollout_mode)
     _check(load().wm_create(C.byref(h), C.byref(cfg)), "wm_create")
     return h
 

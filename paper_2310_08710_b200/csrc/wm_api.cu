@@ -31,6 +31,7 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (cfg->dynamics != WM_DYN_INVERTIBLE_BICYCLE && cfg->dynamics != WM_DYN_DELTA_LOCAL) return WM_ERR_ARG;
   if (!(cfg->dt > 0.f) || cfg->history < 1 || cfg->topk < 0) return WM_ERR_ARG;
   if (cfg->offroad_mode != WM_OFFROAD_CULLED && cfg->offroad_mode != WM_OFFROAD_BRUTE_FORCE) return WM_ERR_ARG;
+  if (cfg->rollout_mode != WM_ROLLOUT_FUSED && cfg->rollout_mode != WM_ROLLOUT_STEPWISE) return WM_ERR_ARG;
   wm_handle* h = (wm_handle*)calloc(1, sizeof(wm_handle));
   if (!h) return WM_ERR_ARG;
   h->cfg = *cfg;
@@ -202,8 +203,9 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
   if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
   if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
   if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
-  const int64_t rows = (int64_t)sim->B * n_steps * sim->A;
-  // rows the caller did not ask for still feed the aggregates: put them in scratch
+  const bool fused = h->cfg.rollout_mode == WM_ROLLOUT_FUSED && h->cfg.offroad_mode == WM_OFFROAD_CULLED;
+  const int64_t rows = fused ? 0 : (int64_t)sim->B * n_steps * sim->A;
+  // stepwise: rows the caller did not ask for still feed the aggregates: put them in scratch
   size_t need = (size_t)rows;                                  // ld_valid rows (uint8)
   need = (need + 255) / 256 * 256;
   const size_t off_ov = need;    if (!out->overlap) need += (size_t)rows;
@@ -217,10 +219,12 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
   if (rc != WM_OK) return rc;
   unsigned char* sc = (unsigned char*)h->scratch;
   wm_rollout_out o = *out;
+  if (!fused) {
   if (!o.overlap) o.overlap = sc + off_ov;
   if (!o.offroad) o.offroad = sc + off_of;
   if (!o.offroad_dist) o.offroad_dist = (float*)(sc + off_sd);
   if (!o.log_div) o.log_div = (float*)(sc + off_ld);
+  }
   uint8_t* ld_valid_rows = sc;
 
   uint64_t key[24];
@@ -234,12 +238,19 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
              ((uint64_t)(uintptr_t)o.ade << 3);
   key[n++] = ((uint64_t)sim->B << 40) ^ ((uint64_t)sim->A << 20) ^ (uint64_t)sim->T;
   key[n++] = ((uint64_t)(uint32_t)t0 << 32) ^ (uint64_t)(uint32_t)n_steps ^ ((uint64_t)h->cfg.dynamics << 62);
+  key[n++] = (uint64_t)(uintptr_t)h->segrec ^ ((uint64_t)(uintptr_t)h->cells << 1);
 
   if (!h->graph_exec || memcmp(key, h->graph_key, sizeof(key)) != 0) {
     wm_drop_graph(h);
     const int64_t before = h->launches;
     WM_CUDA(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-    rc = enqueue_rollout(h, *log, *sim, t0, n_steps, actions, action_valid, o, ld_valid_rows, h->cap_stream);
+    if (fused) {
+      cudaError_t le = wm_launch_rollout_fused(h, *log, *sim, t0, n_steps, actions, action_valid, o, h->cap_stream);
+      rc = WM_OK;
+      if (le != cudaSuccess) { g_wm_last_cuda_error = (int)le; rc = WM_ERR_CUDA; }
+    } else {
+      rc = enqueue_rollout(h, *log, *sim, t0, n_steps, actions, action_valid, o, ld_valid_rows, h->cap_stream);
+    }
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
     h->graph_kernels = h->launches - before;

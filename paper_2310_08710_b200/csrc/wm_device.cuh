@@ -1,0 +1,64 @@
+// Per-agent / per-pair device arithmetic shared by the stepwise kernels (wm_dynamics.cu,
+// wm_overlap.cu) and the fused rollout kernel (wm_rollout_fused.cu), so that both paths return
+// bit-identical results (P14).
+#pragma once
+#include "wm_internal.cuh"
+
+// a1 / a2: successor state of one controlled agent.  (sn, cs) = sincosf(th).  For the bicycle
+// model (s1, c1) = sincosf(th') is returned as well (Eq. 2 needs it for the velocity).
+// PAPER.md Eq. 2 (L339-L350), Eq. 1 (L324-L333) on the body-frame delta rotated by th (D2).
+struct WmDynCfg { int dynamics; float dt, max_accel, max_curvature; };
+
+__device__ __forceinline__ void wm_dyn_step(const WmDynCfg& k, float x, float y, float th, float vx, float vy, float sn,
+                                            float cs, float a0, float a1, float a2, float& xn, float& yn, float& thn,
+                                            float& vxn, float& vyn, float& s1, float& c1) {
+  const float dt = k.dt;
+  if (k.dynamics == WM_DYN_INVERTIBLE_BICYCLE) {
+    float acc = a0, kappa = a1;
+    if (k.max_accel > 0.f) acc = fminf(fmaxf(acc, -k.max_accel), k.max_accel);                    // D7
+    if (k.max_curvature > 0.f) kappa = fminf(fmaxf(kappa, -k.max_curvature), k.max_curvature);
+    const float v = sqrtf(fmaf(vx, vx, vy * vy));
+    const float h = 0.5f * acc * dt * dt;            // a dt^2 / 2
+    xn = x + fmaf(vx, dt, h * cs);                   // Eq. 2
+    yn = y + fmaf(vy, dt, h * sn);                   // L341
+    thn = fmaf(kappa, fmaf(v, dt, h), th);           // L343
+    const float v1 = fmaf(acc, dt, v);               // L345
+    sincosf(thn, &s1, &c1);
+    vxn = v1 * c1;                                   // L347
+    vyn = v1 * s1;                                   // L349
+  } else {
+    const float dx = a0, dy = a1, dyaw = a2;
+    xn = x + (cs * dx - sn * dy);                    // Eq. 1 on the rotated delta (D2)
+    yn = y + (sn * dx + cs * dy);
+    thn = th + dyaw;
+    vxn = (xn - x) / dt;                             // Eq. 1: on the stored float32 x' (D28)
+    vyn = (yn - y) / dt;
+    sincosf(thn, &s1, &c1);
+  }
+}
+
+// a5: displacement error, L106
+__device__ __forceinline__ float wm_logdiv(float x, float y, float lx, float ly) {
+  const float ex = x - lx, ey = y - ly;
+  return sqrtf(fmaf(ex, ex, ey * ey));
+}
+
+// a3: strict positive-area overlap (D12): gap < 0 on all four edge-normal axes.
+// (dx, dy) = c_j - c_i; (c, s) = cos/sin of each yaw; hl, hw half extents.
+__device__ __forceinline__ bool wm_sat_overlap(float dx, float dy, float ci, float si, float hli, float hwi,
+                                               float cj, float sj, float hlj, float hwj) {
+  const float c = fabsf(fmaf(ci, cj, si * sj));      // |f_i . f_j| = |s_i . s_j|
+  const float s = fabsf(fmaf(si, cj, -ci * sj));     // |f_i . s_j| = |s_i . f_j|
+  const float g0 = fabsf(fmaf(dx, ci, dy * si)) - (hli + fmaf(hlj, c, hwj * s));    // axis f_i
+  const float g1 = fabsf(fmaf(dy, ci, -dx * si)) - (hwi + fmaf(hlj, s, hwj * c));   // axis s_i
+  const float g2 = fabsf(fmaf(dx, cj, dy * sj)) - (hlj + fmaf(hli, c, hwi * s));    // axis f_j
+  const float g3 = fabsf(fmaf(dy, cj, -dx * sj)) - (hwj + fmaf(hli, s, hwi * c));   // axis s_j
+  return fmaxf(fmaxf(g0, g1), fmaxf(g2, g3)) < 0.f;
+}
+
+// Conservative pre-test of a3: two boxes can only overlap if their centres are closer than the
+// sum of their circumradii (rr = r_i + r_j).  The 1.001 factor and the absolute term keep the
+// float32 test on the safe side, so skipping the separating-axis test never changes a result.
+__device__ __forceinline__ bool wm_circles_touch(float dx, float dy, float rr) {
+  return fmaf(dx, dx, dy * dy) <= fmaf(rr * rr, 1.001f, 1e-6f);
+}

@@ -1,7 +1,7 @@
 // reset (a0), dynamics step (a1, a2) with optional fused log divergence (a5), aggregates (a8).
 // One thread per (scenario, agent): these kernels move ~12 KB per scenario-step and are
 // HBM/latency bound; rows are time-major so a warp touches one contiguous 128 B line per field.
-#include "wm_internal.cuh"
+#include "wm_device.cuh"
 
 // ---------------------------------------------------------------------------------------
 // a0 reset(scenario), PAPER.md L122 / L78.
@@ -61,31 +61,11 @@ __global__ void __launch_bounds__(256) k_step(StepParams p) {
     const float x = p.cur.x[c], y = p.cur.y[c], th = p.cur.yaw[c];
     const float vx = p.cur.vel_x[c], vy = p.cur.vel_y[c];
     const float* act = p.action + (int64_t)b * p.act_stride_b + a;
-    float sn, cs;
+    float sn, cs, s1, c1;
     sincosf(th, &sn, &cs);
-    const float dt = p.dt;
-    if (p.dynamics == WM_DYN_INVERTIBLE_BICYCLE) {
-      float acc = act[0], kappa = act[p.A];
-      if (p.max_accel > 0.f) acc = fminf(fmaxf(acc, -p.max_accel), p.max_accel);
-      if (p.max_curvature > 0.f) kappa = fminf(fmaxf(kappa, -p.max_curvature), p.max_curvature);
-      const float v = sqrtf(fmaf(vx, vx, vy * vy));
-      const float h = 0.5f * acc * dt * dt;            // a dt^2 / 2
-      xn = x + fmaf(vx, dt, h * cs);                   // Eq. 2
-      yn = y + fmaf(vy, dt, h * sn);                   // L341
-      thn = fmaf(kappa, fmaf(v, dt, h), th);           // L343
-      const float v1 = fmaf(acc, dt, v);               // L345
-      float s1, c1;
-      sincosf(thn, &s1, &c1);
-      vxn = v1 * c1;                                   // L347
-      vyn = v1 * s1;                                   // L349
-    } else {
-      const float dx = act[0], dy = act[p.A], dyaw = act[2 * (int64_t)p.A];
-      xn = x + (cs * dx - sn * dy);                    // Eq. 1 on the rotated delta (D2)
-      yn = y + (sn * dx + cs * dy);
-      thn = th + dyaw;
-      vxn = (xn - x) / dt;                             // Eq. 1: on the stored float32 x'
-      vyn = (yn - y) / dt;
-    }
+    const WmDynCfg dc{p.dynamics, p.dt, p.max_accel, p.max_curvature};
+    const float a2 = p.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 0.f : act[2 * (int64_t)p.A];
+    wm_dyn_step(dc, x, y, th, vx, vy, sn, cs, act[0], act[p.A], a2, xn, yn, thn, vxn, vyn, s1, c1);
     ln = p.cur.length[c];
     wn = p.cur.width[c];
     vn = 1;                                            // D9
@@ -101,7 +81,7 @@ __global__ void __launch_bounds__(256) k_step(StepParams p) {
   if (p.ld_dist) {                                     // fused a5 on row t+1, L106
     const bool v = vn != 0 && lvalid != 0;
     float d = 0.f;
-    if (v) { const float ex = xn - lx, ey = yn - ly; d = sqrtf(fmaf(ex, ex, ey * ey)); }
+    if (v) d = wm_logdiv(xn, yn, lx, ly);
     p.ld_dist[(int64_t)b * p.ld_stride_b + a] = d;
     if (p.ld_valid) p.ld_valid[(int64_t)b * p.ld_stride_b + a] = v;
   }
@@ -136,7 +116,7 @@ __global__ void __launch_bounds__(256) k_logdiv(wm_row lg, wm_row sm, int B, int
   const int64_t cs = (int64_t)b * sm.stride_b + a, cl = (int64_t)b * lg.stride_b + a;
   const bool v = sm.valid[cs] != 0 && lg.valid[cl] != 0;
   float d = 0.f;
-  if (v) { const float ex = sm.x[cs] - lg.x[cl], ey = sm.y[cs] - lg.y[cl]; d = sqrtf(fmaf(ex, ex, ey * ey)); }
+  if (v) d = wm_logdiv(sm.x[cs], sm.y[cs], lg.x[cl], lg.y[cl]);
   dist[(int64_t)b * stride_b + a] = d;
   if (valid) valid[(int64_t)b * stride_b + a] = v;
 }

@@ -63,11 +63,49 @@ __device__ __forceinline__ float centre_d2(const float4 r0, const float4 r1, flo
   return fmaf(ry, ry, rx * rx);
 }
 
+// rules P and N below; (cx, cy) cell centre, hh half side of the inflated cell
+__device__ __forceinline__ bool slab_drop(const float4* __restrict__ rec, const int32_t* __restrict__ src, int s, int n,
+                                          const float4 q0, const float4 q1, float cx, float cy, float hh) {
+  const float ex = q0.z, ey = q0.w;
+  if (ex == 0.f && ey == 0.f) return false;                       // isolated point: no slab
+  const float ae = fabsf(ex) + fabsf(ey);
+  const float eps = 2e-3f * ae;                                     // 2 mm along e: far above float32 rounding
+  const int is = __ldg(src + s);
+  const float wx = cx - q0.x, wy = cy - q0.y;
+  const float pc = fmaf(wx, ex, wy * ey);                           // (c - p0).e
+  if (s > 0 && __ldg(src + s - 1) + 1 == is) {                      // rule P (s-1 is a real segment then)
+    const float4 m1 = __ldg(rec + 2 * (s - 1) + 1);
+    if ((m1.x != 0.f || m1.y != 0.f) && pc + hh * ae < -eps) return true;
+  }
+  if (s + 1 < n && __ldg(src + s + 1) == is + 1) {                  // rule N
+    const float4 n0 = __ldg(rec + 2 * (s + 1));
+    const float fx = n0.z, fy = n0.w, af = fabsf(fx) + fabsf(fy);
+    if (af > 0.f) {
+      const float vx = cx - n0.x, vy = cy - n0.y;                   // c - p1, p1 = p0(s+1) as stored
+      const bool beyond = fmaf(vx, ex, vy * ey) - hh * ae > eps;
+      const bool inside_next = fmaf(vx, fx, vy * fy) - hh * af > 2e-3f * af;
+      if (beyond && inside_next) return true;
+    }
+  }
+  return false;
+}
+
 // One warp per block of 8 x 4 cells, one lane per cell.  Chunks that cannot hold a candidate of
 // any cell of the block are dropped with one box-box test per chunk (lanes over chunks); the
 // survivors are walked twice with lanes over cells: dmin(c), then the candidate runs.
-__global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* chunks, int seg_cap,
-                                                     const WmGrid* gridp, uint4* cells, uint32_t* pool, int32_t* pool_cnt) {
+//
+// A record that passes the distance test is still dropped when it can never be the REPORTED
+// nearest segment of any point of the cell (exact in real arithmetic, tested on the four corners
+// of the inflated cell because the conditions are linear in q):
+//   P  the whole cell projects before p0 of s, and s-1 ends in that same stored point: then
+//      d(q, s-1) <= |q - p0| = d(q, s) and the tie rule prefers the lower index (D17);
+//   N  the whole cell projects beyond p1 of s AND onto the interior side of s+1, which starts in
+//      that same stored point: then d(q, s+1) < |q - p1| = d(q, s).
+// Along a polyline this leaves the few segments whose perpendicular slab meets the cell (about
+// h/spacing + 2) instead of everything within dmin + 2 rho.
+__global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* chunks, const int32_t* seg_src,
+                                                     int seg_cap, const WmGrid* gridp, uint4* cells, uint32_t* pool,
+                                                     int32_t* pool_cnt) {
   __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
   const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const WmGrid g = gridp[b];
@@ -79,12 +117,14 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   const bool in = ix < g.nx && iy < g.ny;
   const float4* rec = segrec + (int64_t)b * seg_cap * 2;
   const float4* ch = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
+  const int32_t* src = seg_src + (int64_t)b * seg_cap;
   const int n = g.nseg, nch = (n + WM_CHUNK - 1) / WM_CHUNK;
   const float h = g.h;
   const float cx = g.x0 + ((float)ix + 0.5f) * h, cy = g.y0 + ((float)iy + 0.5f) * h;
   // cell box inflated by delta (float32 rounding of the query's cell index), half diagonal rho
   const float delta = 1e-3f + 1e-4f * h;
-  const float rho = 1.41421362f * (0.5f * h + delta);
+  const float hh = 0.5f * h + delta;
+  const float rho = 1.41421362f * hh;
   // block box
   const float X0 = g.x0 + (float)(bx * 8) * h - delta, X1 = g.x0 + (float)(bx * 8 + 8) * h + delta;
   const float Y0 = g.y0 + (float)(by * 4) * h - delta, Y1 = g.y0 + (float)(by * 4 + 4) * h + delta;
@@ -138,8 +178,9 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
       const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
 #pragma unroll 2
       for (int s = s0; s < s1; ++s) {
-        const float d2 = centre_d2(__ldg(rec + 2 * s), __ldg(rec + 2 * s + 1), cx, cy);
-        if (in && d2 <= thr2) {
+        const float4 q0 = __ldg(rec + 2 * s), q1 = __ldg(rec + 2 * s + 1);
+        const float d2 = centre_d2(q0, q1, cx, cy);
+        if (in && d2 <= thr2 && !slab_drop(rec, src, s, n, q0, q1, cx, cy, hh)) {
           ++ncand;
           if (rl > 0 && s == rs + rl && rl < 255) ++rl;
           else {
@@ -178,7 +219,7 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   const int nwarps = (WM_GRID_NG / 8) * (WM_GRID_NG / 4);
-  k_build_cells<<<dim3(nwarps / 8, B), 256, 0, s>>>(h->segrec, h->chunks, seg_cap, h->gridp, h->cells, h->pool, h->pool_cnt);
+  k_build_cells<<<dim3(nwarps / 8, B), 256, 0, s>>>(h->segrec, h->chunks, h->seg_src, seg_cap, h->gridp, h->cells, h->pool, h->pool_cnt);
   h->launches++;
   return cudaGetLastError();
 }

@@ -51,92 +51,204 @@ __device__ __forceinline__ float wm_rec_d2(const float4 r0, const float4 r1, flo
   return __fmaf_rn(ry, ry, __fmul_rn(rx, rx));
 }
 
-__device__ __forceinline__ void wm_grid_run(const float4* __restrict__ rec, uint32_t run, float cx, float cy,
-                                            float offx, float offy, float& best, int& bs, int& n_eval) {
-  int s = (int)(run >> 8);
-  const int e = s + (int)(run & 255u);
-  n_eval += e - s;
-#pragma unroll 4
-  for (; s < e; ++s) {
-    const float d2 = wm_rec_d2(__ldg(rec + 2 * s), __ldg(rec + 2 * s + 1), cx, cy, offx, offy);
-    if (d2 < best) { best = d2; bs = s; }      // ascending s + strict '<': exact ties -> lower index (D17)
+// Walk of a cell's candidate runs as ONE flat loop (a warp runs max-over-lanes of the total
+// count, not the sum of per-run maxima), 4 records per iteration with all 8 loads issued before
+// the arithmetic (the walk is latency bound otherwise).  Slots beyond the end of a run re-read
+// its first record: evaluating a candidate twice is harmless.  Up to 4 runs sit in registers,
+// refilled from the pool.
+__device__ __forceinline__ void wm_grid_walk(const float4* __restrict__ rec, uint32_t r0, uint32_t r1, uint32_t r2,
+                                             uint32_t r3, const uint32_t* __restrict__ pool, int n_pool, float cx,
+                                             float cy, float offx, float offy, float& best, int& bs, int& n_eval) {
+  int s = 0, left = 0;
+  for (;;) {
+    if (left <= 0) {
+      if (r0 == 0u) {
+        if (n_pool <= 0) break;
+        r0 = __ldg(pool);
+        r1 = n_pool > 1 ? __ldg(pool + 1) : 0u;
+        r2 = n_pool > 2 ? __ldg(pool + 2) : 0u;
+        r3 = n_pool > 3 ? __ldg(pool + 3) : 0u;
+        pool += 4; n_pool -= 4;
+      }
+      s = (int)(r0 >> 8); left = (int)(r0 & 255u);
+      n_eval += left;
+      r0 = r1; r1 = r2; r2 = r3; r3 = 0u;
+    }
+    const int s1 = left > 1 ? s + 1 : s, s2 = left > 2 ? s + 2 : s, s3 = left > 3 ? s + 3 : s;
+    const float4 a0 = __ldg(rec + 2 * s), b0 = __ldg(rec + 2 * s + 1), a1 = __ldg(rec + 2 * s1), b1 = __ldg(rec + 2 * s1 + 1);
+    const float4 a2 = __ldg(rec + 2 * s2), b2 = __ldg(rec + 2 * s2 + 1), a3 = __ldg(rec + 2 * s3), b3 = __ldg(rec + 2 * s3 + 1);
+    const float d0 = wm_rec_d2(a0, b0, cx, cy, offx, offy), d1 = wm_rec_d2(a1, b1, cx, cy, offx, offy);
+    const float d2 = wm_rec_d2(a2, b2, cx, cy, offx, offy), d3 = wm_rec_d2(a3, b3, cx, cy, offx, offy);
+    if (d0 < best) { best = d0; bs = s; }       // ascending index, strict '<': exact ties -> lower index (D17)
+    if (d1 < best) { best = d1; bs = s1; }
+    if (d2 < best) { best = d2; bs = s2; }
+    if (d3 < best) { best = d3; bs = s3; }
+    s += 4; left -= 4;
   }
 }
 
 // Exact search over all chunks with bounding-box culling, by a whole warp for ONE corner (points
-// outside the grid, crowded cells): lanes over chunks for the bounds, then lanes over the 32
-// records of each surviving chunk.  All 32 lanes call with the same arguments and get the same
-// result.  Chunks are visited in ascending order and a chunk replaces the incumbent only on
-// strict '<', inside a chunk the lowest lane wins: exact ties -> lower index (D17).
+// outside the grid, crowded cells).  Best-first: lanes over chunks find the chunk whose box is
+// nearest and evaluate it (lanes over its 32 records), which gives a tight bound at once; then
+// every other chunk whose box can still reach that bound is evaluated.  All 32 lanes call with the
+// same arguments and get the same result.  The incumbent is replaced on a smaller distance, or
+// on an equal distance and a lower record index: exact ties -> lower index (D17).
+__device__ __forceinline__ void wm_grid_eval_chunk(const WmGridView& v, int c, float cx, float cy, float offx, float offy,
+                                                   float& best, int& bs, int& n_eval) {
+  const int lane = threadIdx.x & 31;
+  const int s = c * WM_CHUNK + lane;
+  float d2 = __int_as_float(0x7f800000);
+  if (s < v.g.nseg) d2 = wm_rec_d2(__ldg(v.rec + 2 * s), __ldg(v.rec + 2 * s + 1), cx, cy, offx, offy);
+  n_eval += (lane == 0) ? min(WM_CHUNK, v.g.nseg - c * WM_CHUNK) : 0;
+  const uint32_t m = __reduce_min_sync(0xffffffffu, __float_as_uint(d2));       // d2 >= +0: bits order as floats
+  const int idx = c * WM_CHUNK + __ffs(__ballot_sync(0xffffffffu, __float_as_uint(d2) == m)) - 1;
+  if (m < __float_as_uint(best) || (m == __float_as_uint(best) && idx < bs)) { best = __uint_as_float(m); bs = idx; }
+}
+
+__device__ __forceinline__ float wm_chunk_lb2(const float4 bb, float qx, float qy) {
+  const float dx = fmaxf(fmaxf(bb.x - qx, qx - bb.z), 0.f), dy = fmaxf(fmaxf(bb.y - qy, qy - bb.w), 0.f);
+  return fmaf(dx, dx, dy * dy);
+}
+
 __device__ __forceinline__ void wm_grid_search_warp(const WmGridView& v, float cx, float cy, float offx, float offy,
                                                     float& best, int& bs, int& n_eval) {
   const int lane = threadIdx.x & 31;
-  const int nseg = v.g.nseg, nch = (nseg + WM_CHUNK - 1) / WM_CHUNK;
+  const int nch = (v.g.nseg + WM_CHUNK - 1) / WM_CHUNK;
   const float qx = cx + offx, qy = cy + offy;
   const float INF = __int_as_float(0x7f800000);
-  float U2 = INF;                                // some segment lies within the farthest corner of any chunk box
+  float lmin = INF;
+  int cmin = 0;
   for (int c = lane; c < nch; c += 32) {
-    const float4 bb = __ldg(v.chunks + c);
-    const float dx = fmaxf(fabsf(qx - bb.x), fabsf(qx - bb.z)), dy = fmaxf(fabsf(qy - bb.y), fabsf(qy - bb.w));
-    U2 = fminf(U2, fmaf(dx, dx, dy * dy));
+    const float lb2 = wm_chunk_lb2(__ldg(v.chunks + c), qx, qy);
+    if (lb2 < lmin) { lmin = lb2; cmin = c; }
   }
-  U2 = __uint_as_float(__reduce_min_sync(0xffffffffu, __float_as_uint(U2)));
-  best = INF; bs = 0;
+  const uint32_t mm = __reduce_min_sync(0xffffffffu, __float_as_uint(lmin));
+  const int c_first = __shfl_sync(0xffffffffu, cmin, __ffs(__ballot_sync(0xffffffffu, __float_as_uint(lmin) == mm)) - 1);
+  best = INF; bs = 0x7fffffff;
+  wm_grid_eval_chunk(v, c_first, cx, cy, offx, offy, best, bs, n_eval);
   for (int c0 = 0; c0 < nch; c0 += 32) {
     const int c = c0 + lane;
     float lb2 = INF;
-    if (c < nch) {
-      const float4 bb = __ldg(v.chunks + c);
-      const float dx = fmaxf(fmaxf(bb.x - qx, qx - bb.z), 0.f), dy = fmaxf(fmaxf(bb.y - qy, qy - bb.w), 0.f);
-      lb2 = fmaf(dx, dx, dy * dy);
-    }
-    uint32_t mask = __ballot_sync(0xffffffffu, lb2 <= fmaf(U2, WM_CULL_REL, WM_CULL_ABS));
+    if (c < nch && c != c_first) lb2 = wm_chunk_lb2(__ldg(v.chunks + c), qx, qy);
+    uint32_t mask = __ballot_sync(0xffffffffu, lb2 <= fmaf(best, WM_CULL_REL, WM_CULL_ABS));
     while (mask) {
       const int l = __ffs(mask) - 1;
       mask &= mask - 1;
       if (__shfl_sync(0xffffffffu, lb2, l) > fmaf(best, WM_CULL_REL, WM_CULL_ABS)) continue;   // warp-uniform
-      const int s = (c0 + l) * WM_CHUNK + lane;
-      float d2 = INF;
-      if (s < nseg) d2 = wm_rec_d2(__ldg(v.rec + 2 * s), __ldg(v.rec + 2 * s + 1), cx, cy, offx, offy);
-      n_eval += (lane == 0) ? min(WM_CHUNK, nseg - (c0 + l) * WM_CHUNK) : 0;
-      const uint32_t m = __reduce_min_sync(0xffffffffu, __float_as_uint(d2));   // d2 >= +0: bits order as floats
-      if (m < __float_as_uint(best)) {
-        best = __uint_as_float(m);
-        bs = (c0 + l) * WM_CHUNK + __ffs(__ballot_sync(0xffffffffu, __float_as_uint(d2) == m)) - 1;
-      }
+      wm_grid_eval_chunk(v, c0 + l, cx, cy, offx, offy, best, bs, n_eval);
     }
   }
 }
 
-// Signed distance of the box corner (c + off) to the nearest road-edge segment (D15-D17, D19,
-// D20).  Must be called by all 32 lanes of a warp (inactive lanes pass active = false): corners
-// that cannot use their cell's candidate list are searched one at a time by the whole warp.
-// n_eval counts evaluated pairs, fell_back is set for those corners.
-__device__ __forceinline__ float wm_grid_corner_sd(const WmGridView& v, bool active, float cx, float cy, float offx,
-                                                   float offy, int& n_eval, bool& fell_back) {
+// The same search for the four corners of ONE box at once (the fused rollout queues whole
+// agents): chunk boxes are bounded against the box centre and its circumradius R, records are
+// loaded once and evaluated for the four corners.  off[k] = corner k - centre.
+__device__ __forceinline__ void wm_grid_search_warp4(const WmGridView& v, float cx, float cy, const float (&offx)[4],
+                                                     const float (&offy)[4], float R, float (&best)[4], int (&bs)[4],
+                                                     int& n_eval) {
   const int lane = threadIdx.x & 31;
-  float best = __int_as_float(0x7f800000);
-  int bs = 0;
+  const int nseg = v.g.nseg, nch = (nseg + WM_CHUNK - 1) / WM_CHUNK;
+  const float INF = __int_as_float(0x7f800000);
+  auto eval4 = [&](int c) {
+    const int s = c * WM_CHUNK + lane;
+    float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
+    const bool in = s < nseg;
+    if (in) { r0 = __ldg(v.rec + 2 * s); r1 = __ldg(v.rec + 2 * s + 1); }
+    n_eval += (lane == 0) ? 4 * min(WM_CHUNK, nseg - c * WM_CHUNK) : 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const float d2 = in ? wm_rec_d2(r0, r1, cx, cy, offx[k], offy[k]) : INF;
+      const uint32_t m = __reduce_min_sync(0xffffffffu, __float_as_uint(d2));
+      if (m <= __float_as_uint(best[k])) {                       // warp-uniform
+        const int idx = c * WM_CHUNK + __ffs(__ballot_sync(0xffffffffu, __float_as_uint(d2) == m)) - 1;
+        if (m < __float_as_uint(best[k]) || idx < bs[k]) { best[k] = __uint_as_float(m); bs[k] = idx; }
+      }
+    }
+  };
+  float lmin = INF;
+  int cmin = 0;
+  for (int c = lane; c < nch; c += 32) {
+    const float lb2 = wm_chunk_lb2(__ldg(v.chunks + c), cx, cy);
+    if (lb2 < lmin) { lmin = lb2; cmin = c; }
+  }
+  const uint32_t mm = __reduce_min_sync(0xffffffffu, __float_as_uint(lmin));
+  const int c_first = __shfl_sync(0xffffffffu, cmin, __ffs(__ballot_sync(0xffffffffu, __float_as_uint(lmin) == mm)) - 1);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { best[k] = INF; bs[k] = 0x7fffffff; }
+  eval4(c_first);
+  // a chunk matters if its box comes within max_k dist_k of some corner: lb(centre) - R <= max_k sqrt(best_k)
+  auto reach2 = [&]() {
+    const float bm = fmaxf(fmaxf(best[0], best[1]), fmaxf(best[2], best[3]));
+    const float r = fmaf(sqrtf(bm), 1.0005f, R + 2e-3f);
+    return r * r;
+  };
+  float B2 = reach2();
+  for (int c0 = 0; c0 < nch; c0 += 32) {
+    const int c = c0 + lane;
+    float lb2 = INF;
+    if (c < nch && c != c_first) lb2 = wm_chunk_lb2(__ldg(v.chunks + c), cx, cy);
+    uint32_t mask = __ballot_sync(0xffffffffu, lb2 <= B2);
+    while (mask) {
+      const int l = __ffs(mask) - 1;
+      mask &= mask - 1;
+      if (__shfl_sync(0xffffffffu, lb2, l) > B2) continue;     // warp-uniform
+      eval4(c0 + l);
+      B2 = reach2();
+    }
+  }
+}
+
+// ---- query API (D15-D17, D19, D20) -------------------------------------------------------
+// wm_grid_fast:   per thread; walks the candidate list of the corner's cell.  Returns true when
+//                 the corner needs the warp search instead (outside the grid, crowded cell).
+// wm_grid_search_warp: above.
+// wm_grid_finish: per thread; sign from the oriented winning segment and the signed distance.
+// wm_grid_corner_sd: the three combined for a warp of corners (k_offroad_grid).
+__device__ __forceinline__ bool wm_grid_fast(const WmGridView& v, bool active, float cx, float cy, float offx, float offy,
+                                             float& best, int& bs, int& n_eval) {
+  best = __int_as_float(0x7f800000);
+  bs = 0;
   bool slow = false;
+  uint4 hd = make_uint4(0u, 0u, 0u, 0u);
+  const uint32_t* pool = v.pool;
+  int n_pool = 0;
   if (active && v.g.nseg > 0) {
     const float fx = (cx + offx - v.g.x0) * v.g.inv_h, fy = (cy + offy - v.g.y0) * v.g.inv_h;
     const int ix = (int)floorf(fx), iy = (int)floorf(fy);
     slow = !(fx >= 0.f && fy >= 0.f && ix < v.g.nx && iy < v.g.ny);
     if (!slow) {
-      const uint4 hd = __ldg(v.cells + iy * v.g.nx + ix);
-      if (hd.x != 0xffffffffu) {
-        wm_grid_run(v.rec, hd.x, cx, cy, offx, offy, best, bs, n_eval);
-        if (hd.y) wm_grid_run(v.rec, hd.y, cx, cy, offx, offy, best, bs, n_eval);
-        if (hd.z) wm_grid_run(v.rec, hd.z, cx, cy, offx, offy, best, bs, n_eval);
-        if (hd.w) wm_grid_run(v.rec, hd.w, cx, cy, offx, offy, best, bs, n_eval);
-      } else if (hd.y != 0xffffffffu) {
-        const uint32_t* pr = v.pool + hd.y;
-        for (uint32_t i = 0; i < hd.z; ++i) wm_grid_run(v.rec, __ldg(pr + i), cx, cy, offx, offy, best, bs, n_eval);
-      } else {
-        slow = true;
+      hd = __ldg(v.cells + iy * v.g.nx + ix);
+      if (hd.x == 0xffffffffu) {
+        slow = hd.y == 0xffffffffu;
+        if (!slow) { pool += hd.y; n_pool = (int)hd.z; }
+        hd = make_uint4(0u, 0u, 0u, 0u);
       }
     }
   }
+  wm_grid_walk(v.rec, hd.x, hd.y, hd.z, hd.w, pool, n_pool, cx, cy, offx, offy, best, bs, n_eval);   // no-op without runs
+  return slow;
+}
+
+__device__ __forceinline__ float wm_grid_finish(const WmGridView& v, float cx, float cy, float offx, float offy, float best,
+                                                int bs) {
+  if (v.g.nseg <= 0) return -FLT_MAX;                                      // D20
+  // e x (q - p0) > 0 is the left side of the oriented segment = on-road (D16)
+  const float4 r0 = __ldg(v.rec + 2 * bs), r1 = __ldg(v.rec + 2 * bs + 1);
+  const float wx = __fadd_rn(__fsub_rn(cx, r0.x), offx), wy = __fadd_rn(__fsub_rn(cy, r0.y), offy);
+  const float side = __fmaf_rn(r1.z, wy, -__fmul_rn(r1.w, wx));
+  const float d = sqrtf(best);
+  return side > 0.f ? -d : d;
+}
+
+// Must be called by all 32 lanes of a warp (inactive lanes pass active = false): corners that
+// cannot use their cell's candidate list are searched one at a time by the whole warp.
+// n_eval counts evaluated pairs, fell_back is set for those corners.
+__device__ __forceinline__ float wm_grid_corner_sd(const WmGridView& v, bool active, float cx, float cy, float offx,
+                                                   float offy, int& n_eval, bool& fell_back) {
+  const int lane = threadIdx.x & 31;
+  float best;
+  int bs;
+  const bool slow = wm_grid_fast(v, active, cx, cy, offx, offy, best, bs, n_eval);
   fell_back = slow;
   uint32_t todo = __ballot_sync(0xffffffffu, slow);
   while (todo) {
@@ -149,11 +261,5 @@ __device__ __forceinline__ float wm_grid_corner_sd(const WmGridView& v, bool act
     if (lane == l) { best = b2; bs = s2; n_eval += ne; }
   }
   if (!active) return 0.f;
-  if (v.g.nseg <= 0) return -FLT_MAX;                                      // D20
-  // sign from the oriented winning segment: e x (q - p0) > 0 is the left side = on-road (D16)
-  const float4 r0 = __ldg(v.rec + 2 * bs), r1 = __ldg(v.rec + 2 * bs + 1);
-  const float wx = __fadd_rn(__fsub_rn(cx, r0.x), offx), wy = __fadd_rn(__fsub_rn(cy, r0.y), offy);
-  const float side = __fmaf_rn(r1.z, wy, -__fmul_rn(r1.w, wx));
-  const float d = sqrtf(best);
-  return side > 0.f ? -d : d;
+  return wm_grid_finish(v, cx, cy, offx, offy, best, bs);
 }

@@ -125,6 +125,9 @@ cudaError_t wm_launch_offroad_grid(wm_handle* h, const wm_traj& sim, int t, floa
 cudaError_t wm_launch_aggregate(wm_handle* h, int B, int A, int n_steps, const wm_rollout_out& out,
                                 const uint8_t* ld_valid_rows, cudaStream_t s);
 cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s);
+cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
+                                    const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
+                                    cudaStream_t s);
 int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);
 void wm_prepare_free(wm_handle* h);
 void wm_drop_graph(wm_handle* h);
@@ -148,14 +151,18 @@ __device__ __forceinline__ float min3f(float a, float b, float c) { float d; asm
 
 // corner offsets of a box: a = front-left, b = front-right; corners 0..3 = c+a, c+b, c-a, c-b
 // (D30).  Explicit round-to-nearest ops so that every kernel derives bit-identical offsets.
-__device__ __forceinline__ void wm_box_offsets(float yaw, float length, float width, float& ax, float& ay, float& bx,
-                                               float& by) {
-  float sn, cs;
-  sincosf(yaw, &sn, &cs);
+__device__ __forceinline__ void wm_box_offsets_sc(float sn, float cs, float length, float width, float& ax, float& ay,
+                                                  float& bx, float& by) {
   const float hl = 0.5f * length, hw = 0.5f * width;
   const float hfx = __fmul_rn(hl, cs), hfy = __fmul_rn(hl, sn), hsx = -__fmul_rn(hw, sn), hsy = __fmul_rn(hw, cs);
   ax = __fadd_rn(hfx, hsx); ay = __fadd_rn(hfy, hsy);
   bx = __fsub_rn(hfx, hsx); by = __fsub_rn(hfy, hsy);
+}
+__device__ __forceinline__ void wm_box_offsets(float yaw, float length, float width, float& ax, float& ay, float& bx,
+                                               float& by) {
+  float sn, cs;
+  sincosf(yaw, &sn, &cs);
+  wm_box_offsets_sc(sn, cs, length, width, ax, ay, bx, by);
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -4,7 +4,7 @@
 // 32 agents i of block I (broadcast from shared memory).  One ballot gives word J of row i,
 // and each lane accumulates word I of its own row j, so a tile fills both triangles.
 // FP32-ALU bound (~40 flop per unordered pair), < 1 % of the step.
-#include "wm_internal.cuh"
+#include "wm_device.cuh"
 
 struct OverlapParams {
   wm_row row;
@@ -13,25 +13,14 @@ struct OverlapParams {
   uint8_t* flag; int64_t flag_stride_b;
 };
 
-// strict positive-area overlap (D12): gap < 0 on all four edge-normal axes
-__device__ __forceinline__ bool sat_overlap(float dx, float dy, float ci, float si, float hli, float hwi,
-                                            float cj, float sj, float hlj, float hwj) {
-  const float c = fabsf(fmaf(ci, cj, si * sj));      // |f_i . f_j| = |s_i . s_j|
-  const float s = fabsf(fmaf(si, cj, -ci * sj));     // |f_i . s_j| = |s_i . f_j|
-  const float g0 = fabsf(fmaf(dx, ci, dy * si)) - (hli + fmaf(hlj, c, hwj * s));    // axis f_i
-  const float g1 = fabsf(fmaf(dy, ci, -dx * si)) - (hwi + fmaf(hlj, s, hwj * c));   // axis s_i
-  const float g2 = fabsf(fmaf(dx, cj, dy * sj)) - (hlj + fmaf(hli, c, hwi * s));    // axis f_j
-  const float g3 = fabsf(fmaf(dy, cj, -dx * sj)) - (hwj + fmaf(hli, s, hwi * c));   // axis s_j
-  return fmaxf(fmaxf(g0, g1), fmaxf(g2, g3)) < 0.f;
-}
-
 __global__ void __launch_bounds__(256) k_overlap(OverlapParams p) {
   extern __shared__ float sm[];
   const int A = p.A, nb = p.W, Ap = nb * 32;
   float* sx = sm;            float* sy = sx + Ap;
   float* sc = sy + Ap;       float* ss = sc + Ap;
   float* shl = ss + Ap;      float* shw = shl + Ap;
-  uint32_t* svalid = (uint32_t*)(shw + Ap);   // [nb] ballot words
+  float* srad = shw + Ap;                     // circumradius
+  uint32_t* svalid = (uint32_t*)(srad + Ap);  // [nb] ballot words
   uint32_t* sany = svalid + nb;               // [Ap] any-overlap per agent
   const int b = blockIdx.x;
   const int64_t ro = (int64_t)b * p.row.stride_b;
@@ -44,6 +33,7 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapParams p) {
       hl = 0.5f * p.row.length[ro + a]; hw = 0.5f * p.row.width[ro + a];
     }
     sx[a] = x; sy[a] = y; sc[a] = c; ss[a] = s; shl[a] = hl; shw[a] = hw;
+    srad[a] = sqrtf(fmaf(hl, hl, hw * hw));
     sany[a] = 0;
     const uint32_t w = __ballot_sync(0xffffffffu, v);
     if ((a & 31) == 0) svalid[a >> 5] = w;
@@ -60,13 +50,15 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapParams p) {
     uint32_t colword = 0, rowword = 0;
     if (vi != 0 && vj != 0) {
       const int j = J * 32 + lane;
-      const float xj = sx[j], yj = sy[j], cj = sc[j], sj = ss[j], hlj = shl[j], hwj = shw[j];
+      const float xj = sx[j], yj = sy[j], cj = sc[j], sj = ss[j], hlj = shl[j], hwj = shw[j], rj = srad[j];
       const bool jv = (vj >> lane) & 1u;
       for (int ii = 0; ii < 32; ++ii) {
         if (!((vi >> ii) & 1u)) continue;          // warp-uniform skip of invalid i
         const int i = I * 32 + ii;
-        const bool ov = jv && i != j &&
-            sat_overlap(xj - sx[i], yj - sy[i], sc[i], ss[i], shl[i], shw[i], cj, sj, hlj, hwj);
+        const float dx = xj - sx[i], dy = yj - sy[i];
+        bool ov = jv && i != j && wm_circles_touch(dx, dy, rj + srad[i]);
+        if (!__any_sync(0xffffffffu, ov)) continue;                   // far apart: row word stays 0
+        ov = ov && wm_sat_overlap(dx, dy, sc[i], ss[i], shl[i], shw[i], cj, sj, hlj, hwj);
         const uint32_t w = __ballot_sync(0xffffffffu, ov);
         if (lane == ii) rowword = w;               // word J of row i
         colword |= (ov ? 1u : 0u) << ii;           // word I of row j
@@ -91,7 +83,7 @@ cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t*
   p.A = sim.A; p.W = (sim.A + 31) / 32;
   p.pair_bits = pair_bits; p.flag = flag; p.flag_stride_b = flag_stride_b;
   const int Ap = p.W * 32;
-  const size_t smem = (size_t)Ap * 7 * 4 + (size_t)p.W * 4;
+  const size_t smem = (size_t)Ap * 8 * 4 + (size_t)p.W * 4;
   k_overlap<<<sim.B, 256, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();

@@ -118,9 +118,11 @@ def test_offroad_matches_oracle(cfgid, B, mode):
     wm.wm_destroy(h)
 
 
-def test_offroad_culled_equals_brute_force_bitwise():
+def test_offroad_culled_equals_brute_force():
     """Culling only changes WHICH pairs are evaluated: the per-pair arithmetic is the same, so the
-    distances of both modes are bit-identical (signs too, outside exact float32 ties)."""
+    distances of both modes are bit-identical, except where the grid dropped one of two
+    neighbouring segments that tie at their shared vertex in real arithmetic (rules P/N of
+    wm_grid.cu) and float32 rounding separates them by an ulp."""
     for cfgid, B in ((1, 4), (4, 4), (5, 16), (2, 8)):
         cfg = ws.make_config(cfgid, B=B) if cfgid != 5 else ws.make_config(5, B=B, n_steps=1)
         res = []
@@ -128,8 +130,9 @@ def test_offroad_culled_equals_brute_force_bitwise():
             h, log_d, rg_d, sim_d, _ = _setup(cfg, offroad_mode=mode)
             res.append(gpu_offroad(h, log_d, cfg["t0"]))
             wm.wm_destroy(h)
-        assert np.array_equal(np.abs(res[0][1]), np.abs(res[1][1])), cfgid
-        assert (res[0][1] != res[1][1]).mean() < 1e-3
+        assert np.allclose(np.abs(res[0][1]), np.abs(res[1][1]), rtol=2e-6, atol=1e-6), cfgid
+        assert (np.abs(res[0][1]) != np.abs(res[1][1])).mean() < 1e-2
+        assert (res[0][1] != res[1][1]).mean() < 1e-2
         assert (res[0][2] != res[1][2]).mean() < 1e-3
 
 
@@ -208,11 +211,13 @@ def test_rollout_config5_sample():
     print("rollout cfg5 sample:", st)
 
 
-def test_rollout_graph_replay_is_deterministic_and_matches_eager(cfg1):
+@pytest.mark.parametrize("mode", ["fused", "stepwise"])
+def test_rollout_graph_replay_is_deterministic_and_matches_eager(cfg1, mode):
     log = cfg1["log"]
     B, T, A = log["x"].shape
     n = 20
-    h, log_d, rg_d, sim_d, _ = _setup(cfg1)
+    h, log_d, rg_d, sim_d, _ = _setup(cfg1, rollout_mode=wm.WM_ROLLOUT_FUSED if mode == "fused" else wm.WM_ROLLOUT_STEPWISE)
+    l_start = wm.wm_kernel_launches(h)
     acts = torch.from_numpy(np.ascontiguousarray(cfg1["actions"][:, :n])).cuda()
     av = torch.from_numpy(np.ascontiguousarray(cfg1["action_valid"][:, :n])).cuda()
     outs = []
@@ -245,8 +250,47 @@ def test_rollout_graph_replay_is_deterministic_and_matches_eager(cfg1):
     got_e = host(sim_e)
     for k in got_e:
         assert np.array_equal(got_e[k], outs[0][0][k], equal_nan=True)
-    assert wm.wm_kernel_launches(h) > 3 * (3 * n + 1)
+    per_rollout = 1 if mode == "fused" else 3 * n + 1            # kernel nodes of the graph (+ 1 reset each)
+    assert wm.wm_kernel_launches(h) - l_start == 3 * (per_rollout + 1) + 1 + 4 * n
     wm.wm_destroy(h)
+
+
+@pytest.mark.parametrize("cfgid,dyn,n", [(5, "bicycle", 80), (2, "delta_local", 1), (1, "bicycle", 80), (4, "bicycle", 3)])
+def test_rollout_fused_equals_stepwise_bitwise(cfgid, dyn, n):
+    """P14: the fused kernel and the stepwise graph run the same device arithmetic."""
+    cfg = ws.make_config(cfgid, B=5, n_steps=n) if cfgid in (2, 5) else ws.make_config(cfgid, B=3 if cfgid == 4 else None)
+    kw = {}
+    if cfgid == 4:                                    # A = 512 (two agent rounds per thread): the lot's single row, 5 times
+        cfg["log"] = {k: np.ascontiguousarray(np.repeat(v, 5, axis=1)) for k, v in cfg["log"].items()}
+        kw["history"] = 1
+    log = cfg["log"]
+    B, T, A = log["x"].shape
+    if cfgid == 4:                                    # the lot has no actions: half of the agents on log playback
+        rng = np.random.default_rng(4)
+        acts = rng.uniform(-1, 1, size=(B, n, 2, A)).astype(np.float32)
+        av = (rng.uniform(size=(B, n, A)) < 0.5).astype(np.uint8)
+    else:
+        acts = np.ascontiguousarray(cfg["actions"][:, :n]); av = np.ascontiguousarray(cfg["action_valid"][:, :n])
+    res = []
+    for mode in (wm.WM_ROLLOUT_FUSED, wm.WM_ROLLOUT_STEPWISE):
+        h, log_d, rg_d, sim_d, _ = _setup(cfg, dynamics=dyn, rollout_mode=mode, **kw)
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        out_d = wm.alloc_rollout_out(B, n, A)
+        wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out_d)
+        # outputs are optional: the same call with only the aggregates
+        out2 = {k: (v if k in ("any_overlap", "any_offroad", "ade") else None) for k, v in wm.alloc_rollout_out(B, n, A).items()}
+        sim2 = {k: v.clone() for k, v in sim_d.items()}
+        wm.wm_rollout(h, log_d, sim2, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out2)
+        torch.cuda.synchronize()
+        for k in ("any_overlap", "any_offroad", "ade"):
+            assert torch.equal(out2[k], out_d[k]), k
+        res.append((host(sim_d), host(out_d)))
+        wm.wm_destroy(h)
+    for k in res[0][0]:
+        assert np.array_equal(res[0][0][k], res[1][0][k], equal_nan=True), k
+    for k in res[0][1]:
+        assert np.array_equal(res[0][1][k], res[1][1][k]), k
+    assert res[0][1]["offroad"].sum() > 0
 
 
 def test_rollout_host_matches_device_rollout(cfg1):
