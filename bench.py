@@ -14,10 +14,11 @@ value     device-resident: inputs in HBM when the timed region starts, CUDA even
           launching stream, barrier + synchronize on both sides, max over ranks.
 e2e       the same job through wm_rollout_host with pinned HOST buffers: scenario + action
           upload, wm_prepare, reset, rollout, metric download all inside the timed region.
-roofline  dominant kernel k_offroad_cull (exact search with group culling): after culling the
-          nearest roof is HBM (every segment tile is still streamed once per launch), so
-          achieved = algorithmic bytes / CUDA-event duration against the measured HBM peak; the
-          FP32 fractions on evaluated pairs and on the brute-force pair count are given beside it.
+roofline  dominant kernel k_rollout_fused (the whole rollout is one launch of it).  The exact grid
+          search leaves ~0.2 % of the corner-segment pairs, so the slower roof of the kernel is its
+          compulsory HBM IO (actions + log row in, sim row + metric rows out, per agent-step):
+          achieved = those bytes / CUDA-event duration of the launch, against the measured HBM peak;
+          the FP32 fractions on evaluated pairs and on the brute-force pair count are beside it.
 roofline_bruteforce  the brute-force kernel k_offroad: 13 flop per corner-segment pair (SURVEY
           §8(d)) / its CUDA-event duration, against the FP32 peak SMs*128*2*max clock.
 cpu_baseline  the oracle (oracle/, as it stands) on the host cores, bounded sample.
@@ -362,7 +363,20 @@ def main():
         torch.cuda.synchronize()
         return ka.elapsed_time(kb) / N_STEPS
 
-    k_ms = time_offroad(h)                                     # default mode: exact grid search
+    # dominant kernel of the timed region: k_rollout_fused (one launch = the whole 80-step rollout)
+    def time_rollout():
+        wm.wm_rollout(h, log_d, sim_d, 10, N_STEPS, acts_d, av_d, out_d)
+        torch.cuda.synchronize()
+        ka, kb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ka.record(stream)
+        for _ in range(5):
+            wm.wm_rollout(h, log_d, sim_d, 10, N_STEPS, acts_d, av_d, out_d)
+        kb.record(stream)
+        torch.cuda.synchronize()
+        return ka.elapsed_time(kb) / 5
+
+    kf_ms = time_rollout()
+    k_ms = time_offroad(h)                                     # the single-step kernel of the same search
     wm.wm_offroad_stats_enable(h, True); wm.wm_offroad_stats(h)
     for t in range(11, 11 + N_STEPS):
         wm.wm_metrics_offroad(h, sim_d, t, sd, None, fl)
@@ -370,30 +384,41 @@ def main():
     wm.wm_offroad_stats_enable(h, False)
     pairs_eval = ev_pairs / float(N_STEPS)
     nvalid_bt = sim_d["valid"][:, 11:11 + N_STEPS].sum(dim=2).double().cpu().numpy()       # [B, 80]
-    pairs_per_launch = float((4.0 * nvalid_bt * n_seg[:, None]).sum() / N_STEPS)            # brute-force count
+    pairs_per_launch = float((4.0 * nvalid_bt * n_seg[:, None]).sum() / N_STEPS)            # brute-force count, per step
     peaks = measured_peaks()
     props = torch.cuda.get_device_properties(local)
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"
     fp32_peak = props.multi_processor_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12              # TFLOP/s
-    hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 29.0 + B * A * 5.0    # segments once + one state row + outputs
+    peak_src = "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz)
+    # compulsory bytes of one rollout launch: per agent-step the action (C*4) and its mask (1),
+    # log row t+1 in (29), sim row t+1 out (29), metric rows out (1+1+4+4); per agent row t0 in (29) and
+    # the aggregates out (1+1+4).  The search structures (cells, records) are not compulsory IO.
+    C_ACT = 2
+    fused_bytes = float(B) * N_STEPS * A * (C_ACT * 4 + 1 + 29 + 29 + 10) + float(B) * A * (29 + 6)
+    fused_flops = pairs_eval * N_STEPS * FLOP_PER_PAIR
+    roofline = {"bound": "hbm", "achieved": fused_bytes / (kf_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": fused_bytes / (kf_ms * 1e-3) / 1e9 / hbm_peak, "traffic": profiled_traffic("k_rollout_fused"),
+                "kernel": "k_rollout_fused", "kernel_ms": kf_ms, "algorithmic_bytes_per_launch": fused_bytes,
+                "peak_source": hbm_src, "kernel_share_of_step": kf_ms / ms_step,
+                "hbm_time_ms_at_peak": fused_bytes / (hbm_peak * 1e9) * 1e3,
+                "fp32_time_ms_at_peak_on_evaluated_pairs": fused_flops / (fp32_peak * 1e12) * 1e3,
+                "pairs_bruteforce_per_step": pairs_per_launch, "pairs_evaluated_per_step": pairs_eval,
+                "evaluated_fraction": pairs_eval / pairs_per_launch, "pairs_per_corner": ev_pairs / max(n_corner, 1),
+                "slow_path_corner_fraction": n_slow / max(n_corner, 1),
+                "alu_frac_on_evaluated_pairs": fused_flops / (kf_ms * 1e-3) / 1e12 / fp32_peak,
+                "alu_frac_bruteforce_equivalent": pairs_per_launch * N_STEPS * FLOP_PER_PAIR / (kf_ms * 1e-3) / 1e12 / fp32_peak,
+                "note": "exact culling (SURVEY 8(d)) leaves 0.2 % of the pairs, so the slower roof of the kernel is its "
+                        "compulsory HBM IO; the FP32 fractions on evaluated pairs and on the brute-force count are beside it"}
+    hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 29.0 + B * A * 5.0    # brute force: segments once + one state row + outputs
+    roofline_grid = {"bound": "hbm", "kernel": "k_offroad_grid (wm_metrics_offroad, one step)", "kernel_ms": k_ms,
+                     "algorithmic_bytes_per_launch": B * A * 34.0, "note": "single-step entry point of the same search"}
     hb = wm.wm_create(offroad_mode=wm.WM_OFFROAD_BRUTE_FORCE)  # the FP32-roofline reference kernel
     wm.wm_prepare(hb, rg_d)
     kb_ms = time_offroad(hb)
     wm.wm_destroy(hb)
     bf_achieved = pairs_per_launch * FLOP_PER_PAIR / (kb_ms * 1e-3) / 1e12
-    peak_src = "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz)
-    roofline = {"bound": "hbm", "achieved": hbm_bytes / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": hbm_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "traffic": profiled_traffic("k_offroad_grid"),
-                "kernel": "k_offroad_grid", "kernel_ms": k_ms, "algorithmic_bytes_per_launch": hbm_bytes,
-                "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
-                "kernel_share_of_step": k_ms * N_STEPS / ms_step,
-                "pairs_bruteforce_per_launch": pairs_per_launch, "pairs_evaluated_per_launch": pairs_eval,
-                "evaluated_fraction": pairs_eval / pairs_per_launch, "pairs_per_corner": ev_pairs / max(n_corner, 1),
-                "slow_path_corner_fraction": n_slow / max(n_corner, 1),
-                "alu_frac_on_evaluated_pairs": pairs_eval * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12 / fp32_peak,
-                "alu_frac_bruteforce_equivalent": pairs_per_launch * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12 / fp32_peak,
-                "note": "exact culling (SURVEY 8(d)): the FP32 fraction is given on evaluated pairs and on the brute-force count"}
     roofline_bf = {"bound": "alu", "achieved": bf_achieved, "peak": fp32_peak, "unit": "TFLOP/s",
                    "frac": bf_achieved / fp32_peak, "traffic": profiled_traffic("k_offroad_brute"),
                    "kernel": "k_offroad (offroad_mode=WM_OFFROAD_BRUTE_FORCE)", "kernel_ms": kb_ms,
@@ -456,7 +481,7 @@ def main():
                        "S_e_mean": float(n_seg.mean()), "l2": "inputs exceed L2 (segments %.2f GB + state per step)" % (n_seg.sum() * 24 / 1e9),
                        "parallelism": "scenario shards, no collective", "valid_agent_steps_per_s": valid_value,
                        "ms_per_sim_step": ms_step / N_STEPS},
-            "roofline": roofline, "roofline_bruteforce": roofline_bf, "step_roofline": step_roofline,
+            "roofline": roofline, "roofline_offroad_grid": roofline_grid, "roofline_bruteforce": roofline_bf, "step_roofline": step_roofline,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line))
