@@ -203,7 +203,8 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
   if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
   if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
   if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
-  const bool fused = h->cfg.rollout_mode == WM_ROLLOUT_FUSED && h->cfg.offroad_mode == WM_OFFROAD_CULLED;
+  const bool fused = h->cfg.rollout_mode == WM_ROLLOUT_FUSED && h->cfg.offroad_mode == WM_OFFROAD_CULLED &&
+                     n_steps < 60000;                  // its hash entries carry a 16-bit block number
   const int64_t rows = fused ? 0 : (int64_t)sim->B * n_steps * sim->A;
   // stepwise: rows the caller did not ask for still feed the aggregates: put them in scratch
   size_t need = (size_t)rows;                                  // ld_valid rows (uint8)

@@ -28,11 +28,12 @@ __device__ __forceinline__ void wm_dyn_step(const WmDynCfg& k, float x, float y,
     vyn = v1 * s1;                                   // L349
   } else {
     const float dx = a0, dy = a1, dyaw = a2;
-    xn = x + (cs * dx - sn * dy);                    // Eq. 1 on the rotated delta (D2)
-    yn = y + (sn * dx + cs * dy);
-    thn = th + dyaw;
-    vxn = (xn - x) / dt;                             // Eq. 1: on the stored float32 x' (D28)
-    vyn = (yn - y) / dt;
+    // explicit roundings: the compiler must not contract these differently in different kernels (P14)
+    xn = __fadd_rn(x, __fmaf_rn(cs, dx, -__fmul_rn(sn, dy)));     // Eq. 1 on the rotated delta (D2)
+    yn = __fadd_rn(y, __fmaf_rn(sn, dx, __fmul_rn(cs, dy)));
+    thn = __fadd_rn(th, dyaw);
+    vxn = __fdiv_rn(__fsub_rn(xn, x), dt);           // Eq. 1: on the stored float32 x' (D28)
+    vyn = __fdiv_rn(__fsub_rn(yn, y), dt);
     sincosf(thn, &s1, &c1);
   }
 }

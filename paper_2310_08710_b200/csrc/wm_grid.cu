@@ -15,12 +15,11 @@
 // ======================================================================================
 // grid construction (wm_prepare)
 // ======================================================================================
-constexpr float GRID_MARGIN = 16.f;       // metres of grid beyond the segments' bounding box
 constexpr int BUILD_MAXRUN = 12;          // runs per cell before the cell falls back to the full search
 constexpr int BUILD_MAXCAND = 256;        // candidates per cell before it falls back
 
 __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const float4* chunks, int seg_cap, float h_min,
-                                                     WmGrid* gridp, int32_t* pool_cnt) {
+                                                     float margin, WmGrid* gridp, int32_t* pool_cnt) {
   __shared__ float s_red[4][4];
   const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n = n_seg[b], nch = (n + WM_CHUNK - 1) / WM_CHUNK;
@@ -45,9 +44,9 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
     g.nseg = n; g.pad = 0;
     if (n <= 0) { g.x0 = 0.f; g.y0 = 0.f; g.h = h_min; g.inv_h = 1.f / h_min; g.nx = 0; g.ny = 0; }
     else {
-      const float W = (x1 - x0) + 2.f * GRID_MARGIN, H = (y1 - y0) + 2.f * GRID_MARGIN;
+      const float W = (x1 - x0) + 2.f * margin, H = (y1 - y0) + 2.f * margin;
       const float h = fmaxf(h_min, fmaxf(W, H) * (1.0001f / WM_GRID_NG));
-      g.x0 = x0 - GRID_MARGIN; g.y0 = y0 - GRID_MARGIN; g.h = h; g.inv_h = 1.f / h;
+      g.x0 = x0 - margin; g.y0 = y0 - margin; g.h = h; g.inv_h = 1.f / h;
       g.nx = min(WM_GRID_NG, (int)ceilf(W / h)); g.ny = min(WM_GRID_NG, (int)ceilf(H / h));
     }
     gridp[b] = g;
@@ -211,10 +210,15 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
 }
 
 cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s) {
-  static float h_min = 0.f;
-  if (h_min <= 0.f) { const char* e = getenv("WM_GRID_CELL"); h_min = e ? (float)atof(e) : 2.0f; if (!(h_min >= 0.25f && h_min <= 64.f)) h_min = 2.0f; }
+  // cell side (lower bound) and metres of grid beyond the segments' bounding box; the cell side grows
+  // when (bounding box + 2 margin) does not fit WM_GRID_NG cells
+  static float h_min = 0.f, margin = 0.f;
+  if (h_min <= 0.f) {
+    const char* e = getenv("WM_GRID_CELL"); h_min = e ? (float)atof(e) : 2.0f; if (!(h_min >= 0.25f && h_min <= 64.f)) h_min = 2.0f;
+    e = getenv("WM_GRID_MARGIN"); margin = e ? (float)atof(e) : 120.f; if (!(margin >= 1.f && margin <= 4096.f)) margin = 120.f;
+  }
   const int seg_cap = h->seg_tiles * WM_TILE_SEGS;
-  k_grid_params<<<B, 128, 0, s>>>(h->n_seg, h->chunks, seg_cap, h_min, h->gridp, h->pool_cnt);
+  k_grid_params<<<B, 128, 0, s>>>(h->n_seg, h->chunks, seg_cap, h_min, margin, h->gridp, h->pool_cnt);
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;

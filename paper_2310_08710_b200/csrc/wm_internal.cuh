@@ -31,9 +31,9 @@ constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding seg
 //   {~0, pool offset, n runs, 0}  more runs, in the scenario's pool
 //   {~0, ~0, 0, 0}                too many candidates: search all chunks
 constexpr int WM_CHUNK = 32;
-constexpr int WM_GRID_NG = 128;
+constexpr int WM_GRID_NG = 256;
 constexpr int WM_GRID_CELLS = WM_GRID_NG * WM_GRID_NG;
-constexpr int WM_POOL_CAP = 2 * WM_GRID_CELLS;   // overflow runs per scenario
+constexpr int WM_POOL_CAP = WM_GRID_CELLS;       // overflow runs per scenario
 struct WmGrid { float x0, y0, inv_h, h; int nx, ny, nseg, pad; };
 
 // Prepared roadgraph points for top-k: float2 (x, y) per point, invalid -> (WM_FAR, WM_FAR),
@@ -151,12 +151,15 @@ __device__ __forceinline__ float min3f(float a, float b, float c) { float d; asm
 
 // corner offsets of a box: a = front-left, b = front-right; corners 0..3 = c+a, c+b, c-a, c-b
 // (D30).  Explicit round-to-nearest ops so that every kernel derives bit-identical offsets.
-__device__ __forceinline__ void wm_box_offsets_sc(float sn, float cs, float length, float width, float& ax, float& ay,
-                                                  float& bx, float& by) {
-  const float hl = 0.5f * length, hw = 0.5f * width;
+__device__ __forceinline__ void wm_box_offsets_h(float sn, float cs, float hl, float hw, float& ax, float& ay, float& bx,
+                                                 float& by) {
   const float hfx = __fmul_rn(hl, cs), hfy = __fmul_rn(hl, sn), hsx = -__fmul_rn(hw, sn), hsy = __fmul_rn(hw, cs);
   ax = __fadd_rn(hfx, hsx); ay = __fadd_rn(hfy, hsy);
   bx = __fsub_rn(hfx, hsx); by = __fsub_rn(hfy, hsy);
+}
+__device__ __forceinline__ void wm_box_offsets_sc(float sn, float cs, float length, float width, float& ax, float& ay,
+                                                  float& bx, float& by) {
+  wm_box_offsets_h(sn, cs, 0.5f * length, 0.5f * width, ax, ay, bx, by);
 }
 __device__ __forceinline__ void wm_box_offsets(float yaw, float length, float width, float& ax, float& ay, float& bx,
                                                float& by) {

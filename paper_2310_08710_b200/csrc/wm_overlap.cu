@@ -56,7 +56,10 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapParams p) {
         if (!((vi >> ii) & 1u)) continue;          // warp-uniform skip of invalid i
         const int i = I * 32 + ii;
         const float dx = xj - sx[i], dy = yj - sy[i];
-        bool ov = jv && i != j && wm_circles_touch(dx, dy, rj + srad[i]);
+        // off-diagonal tiles have i < j; a diagonal tile takes each unordered pair once, as (i < j):
+        // the lower index is always in the i role, so overlap(i, j) == overlap(j, i) bit for bit
+        // (the fused rollout kernel evaluates pairs in this order as well, P14)
+        bool ov = jv && i < j && wm_circles_touch(dx, dy, rj + srad[i]);
         if (!__any_sync(0xffffffffu, ov)) continue;                   // far apart: row word stays 0
         ov = ov && wm_sat_overlap(dx, dy, sc[i], ss[i], shl[i], shw[i], cj, sj, hlj, hwj);
         const uint32_t w = __ballot_sync(0xffffffffu, ov);
@@ -65,6 +68,7 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapParams p) {
       }
     }
     const int i_mine = I * 32 + lane, j_mine = J * 32 + lane;
+    if (I == J) { rowword |= colword; colword = 0; }         // the diagonal word holds both triangles
     if (p.pair_bits) {
       if (i_mine < A) p.pair_bits[((int64_t)b * A + i_mine) * nb + J] = rowword;
       if (I != J && j_mine < A) p.pair_bits[((int64_t)b * A + j_mine) * nb + I] = colword;

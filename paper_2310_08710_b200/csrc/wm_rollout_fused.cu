@@ -1,38 +1,49 @@
 // a8 closed-loop rollout ("Rollout ... faster than running Step 80 times"), fused:
 // ONE kernel runs all n_steps of a scenario — dynamics (a1/a2), log divergence (a5), pairwise
-// overlap (a3), offroad (a4) and the aggregates — with the scenario's state resident in shared
-// memory, one CTA per scenario.  Per step the CTA only streams what is compulsory: the action
-// row and log row t+1 in, sim row t+1 and the metric rows out (~10 KB); the candidate road-edge
-// records of the grid search (wm_grid.cuh) stay hot in L1/L2 across steps because an agent moves
-// at most a few metres per step.
+// overlap (a3), offroad (a4) and the aggregates — one CTA per scenario, the scenario's state
+// resident in shared memory.
 //
-//   phase A  one thread per agent : metric rows of the previous step (overlap flag, max over the
-//            4 corner distances), successor state (shared arithmetic with k_step:
-//            wm_device.cuh), sim row t+1 -> HBM, log divergence, sin/cos, half extents, corner
-//            offsets -> shared memory
-//   phase B1 one thread per corner: candidate walk of the corner's grid cell; corners that need
-//            the full search (off the grid, crowded cell) go to a shared-memory queue
-//            one warp per (tile, quarter) of the A x A matrix: separating-axis test, any-flags
-//   phase B2 the queued corners, one warp each, spread over all warps of the CTA
+// The successor state depends on the state and the action only, never on a metric.  So the steps
+// are taken in blocks of up to FUSED_S: the agent threads first run the dynamics of the whole
+// block (one serial chain per agent, next step's inputs prefetched), leaving what the metrics need
+// (centre, sin/cos, half extents) in per-step slots of shared memory; then the metric work of all
+// steps of the block is one pool of independent warp tasks, handed out through a shared counter:
 //
-// Bound: compulsory HBM bytes (~10 KB per scenario-step) against the per-step latency chain of a
-// CTA (2 barriers, the dependent loads of the grid walk); see DESIGN.md.
-// Results are bit-identical to the stepwise graph (WM_ROLLOUT_STEPWISE), which runs the same
-// device functions kernel by kernel.
+//   phase A  one thread per agent : S successor states (shared arithmetic with k_step:
+//            wm_device.cuh), sim rows -> HBM, log divergence, per-step slots, spatial hash insert
+//   phase B  warp tasks, any warp : (step, 8 agents) -> 32 box corners: candidate walk of the corner's
+//                                   grid cell (wm_grid.cuh); corners off the grid or in a crowded
+//                                   cell are searched by the whole warp, one agent at a time;
+//                                   (step, 32 agents) -> overlap flags: each lane walks the 3 x 3 hash
+//                                   cells around its agent, circle pre-test, separating-axis test
+//   phase C  one thread per agent : metric rows of the block -> HBM, any-flags
+//
+// Overlap broad phase: agents are hashed by the 8 m cell of their centre (linked lists in shared
+// memory, entries tagged with the block number so nothing is ever cleared).  Two boxes whose
+// circumradii are both <= 3.9 m can only overlap from adjacent cells; larger boxes go to a list
+// that every agent checks, and check every agent themselves.  A pair is always evaluated with the
+// lower agent index in the i role, like k_overlap, so flags equal the stepwise kernels' bit for bit.
+//
+// Bound: instruction issue and the latency of the candidate walk's dependent loads; compulsory HBM
+// traffic is ~77 B per agent-step.  Results are bit-identical to the stepwise graph
+// (WM_ROLLOUT_STEPWISE), which runs the same device functions kernel by kernel.
 #include "wm_device.cuh"
 #include "wm_grid.cuh"
 
 #ifndef FUSED_NT
-#define FUSED_NT 512
+#define FUSED_NT 256
 #endif
 #ifndef FUSED_MINB
-#define FUSED_MINB 2
+#define FUSED_MINB 4
 #endif
-constexpr int FUSED_SUB = 4;          // an overlap tile is split into 4 tasks of 8 rows
+constexpr int FUSED_S = 8;                 // steps per block (fewer when A is large: shared memory)
+constexpr float FUSED_HASH_H = 8.f;        // hash cell side, metres
+constexpr float FUSED_RMAX = 3.9f;         // circumradius limit of hashed agents (< FUSED_HASH_H / 2, with margin)
+constexpr uint32_t FUSED_EMPTY = 0xffffu;
 
 struct FusedParams {
   wm_traj log, sim;
-  int t0, n_steps, C;
+  int t0, n_steps, C, S;
   const float* actions;               // [B][n_steps][C][A]
   const uint8_t* av;                  // [B][n_steps][A]
   wm_rollout_out out;                 // any pointer may be NULL
@@ -42,53 +53,68 @@ struct FusedParams {
   unsigned long long* stats;
 };
 
-__host__ __device__ inline size_t fused_smem_bytes(int A) {
-  const size_t Ap = (size_t)((A + 31) / 32) * 32;
-  return Ap * (16 * 4 + 8 + 4 + 4 + 16 + 4 + 4 + 1 + 1 + 1 + 1) + (Ap / 32) * 4 + 64;
+// shared-memory carve-up: persistent per-agent state, then S per-step slots
+__host__ __device__ inline int fused_nbk(int Ap) { int n = 64; while (n < 2 * Ap) n <<= 1; return n; }
+__host__ __device__ inline size_t fused_persist_bytes(int Ap) { return (size_t)Ap * (8 + 9 * 4 + 4 + 4) + 64; }
+__host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)Ap * (7 * 4 + 2 + 2 + 2) + (size_t)fused_nbk(Ap) * 4; }
+static inline int fused_pick_S(int A) {
+  const int Ap = (A + 31) / 32 * 32;
+  const size_t budget = 54 * 1024;                        // 4 CTAs per SM when it fits
+  const size_t per = fused_persist_bytes(Ap), slot = fused_slot_bytes(Ap);
+  int S = per + slot >= budget ? 1 : (int)((budget - per) / slot);
+  return S < 1 ? 1 : (S > FUSED_S ? FUSED_S : S);
 }
 
-// metric rows of step k for agent a, from what phase B left in shared memory (D18, D19, D10)
-__device__ __forceinline__ void fused_flush_metrics(const FusedParams& p, int64_t rb, int k, int a, int A,
-                                                    const uint8_t* s_valid, const uint32_t* s_ov, const float* s_csd,
-                                                    uint8_t* s_anyov, uint8_t* s_anyoff) {
-  const int64_t o = rb + (int64_t)k * A + a;
-  const uint8_t fo = (uint8_t)(s_ov[a] != 0);
-  if (p.out.overlap) p.out.overlap[o] = fo;
-  s_anyov[a] |= fo;
-  const bool v = s_valid[a] != 0;
-  const float4 cd = *(const float4*)(s_csd + 4 * a);
-  const float m = fmaxf(fmaxf(cd.x, cd.y), fmaxf(cd.z, cd.w));                 // D18: max over the 4 corners
-  const uint8_t ff = (uint8_t)(v && m > 0.f);                                  // D19
-  if (p.out.offroad_dist) p.out.offroad_dist[o] = v ? m : 0.f;
-  if (p.out.offroad) p.out.offroad[o] = ff;
-  s_anyoff[a] |= ff;
+struct FusedIn { float a0, a1, a2, lx, ly; uint8_t av, lv; };
+
+__device__ __forceinline__ FusedIn fused_load_in(const FusedParams& p, int64_t sb, int64_t ab, int k, int a, int A) {
+  FusedIn r;
+  const int64_t o = sb + (int64_t)(p.t0 + k + 1) * A + a;
+  const int64_t ak = ab + k;
+  r.av = p.av[ak * A + a];
+  const float* act = p.actions + ak * p.C * A + a;
+  r.a0 = act[0]; r.a1 = act[A]; r.a2 = p.C > 2 ? act[2 * (int64_t)A] : 0.f;
+  r.lx = p.log.x[o]; r.ly = p.log.y[o]; r.lv = p.log.valid[o];
+  return r;
+}
+
+__device__ __forceinline__ int fused_cell(float v) {
+  return (int)floorf(fminf(fmaxf(v * (1.f / FUSED_HASH_H), -1.0e9f), 1.0e9f));
+}
+__device__ __forceinline__ uint32_t fused_bucket(int ix, int iy, uint32_t mask) {
+  return (((uint32_t)ix * 73856093u) ^ ((uint32_t)iy * 19349663u)) & mask;
 }
 
 __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int A = p.sim.A, nb = (A + 31) / 32, Ap = nb * 32;
+  const int A = p.sim.A, nb = (A + 31) / 32, Ap = nb * 32, S = p.S;
+  const int NBK = fused_nbk(Ap);
+  // ---- persistent per-agent state ----
   double* s_sum = (double*)smem_raw;                 // [Ap] sum of valid log divergences (D21)
   float* sx = (float*)(s_sum + Ap);
   float* sy = sx + Ap;    float* syaw = sy + Ap;   float* svx = syaw + Ap;  float* svy = svx + Ap;
-  float* slen = svy + Ap; float* swid = slen + Ap;
-  float* sc = swid + Ap;  float* ss = sc + Ap;     float* shl = ss + Ap;    float* shw = shl + Ap;
-  float* oax = shw + Ap;  float* oay = oax + Ap;   float* obx = oay + Ap;   float* oby = obx + Ap;
-  float* srad = oby + Ap;                            // [Ap] circumradius of the box
-  int* s_cnt = (int*)(srad + Ap);                    // [Ap] count of valid log divergences
-  uint32_t* s_ov = (uint32_t*)(s_cnt + Ap);          // [Ap] overlap flag of the current step
-  float* s_csd = (float*)(s_ov + Ap);                // [4 Ap] signed distance of every corner, current step
-  int* s_q = (int*)(s_csd + 4 * Ap);                 // [Ap] queue of agents that need the warp search
-  uint32_t* s_qm = (uint32_t*)(s_q + Ap);            // [Ap] which corners of the agent (4 bits; 0 = not queued)
-  uint32_t* s_vw = s_qm + Ap;                        // [nb] validity ballot words
-  uint8_t* s_valid = (uint8_t*)(s_vw + nb);          // [Ap]
+  float* slen = svy + Ap; float* swid = slen + Ap; float* sc = swid + Ap;   float* ss = sc + Ap;
+  int* s_cnt = (int*)(ss + Ap);                      // [Ap] count of valid log divergences
+  uint8_t* s_valid = (uint8_t*)(s_cnt + Ap);         // [Ap]
   uint8_t* s_anyov = s_valid + Ap;                   // [Ap]
   uint8_t* s_anyoff = s_anyov + Ap;                  // [Ap]
+  int* s_nover = (int*)(s_anyoff + 2 * Ap);          // [2][FUSED_S] oversize counts, by block parity
+  // ---- per-step slots ----
+  float* px = (float*)(smem_raw + fused_persist_bytes(Ap));      // [S][Ap] each
+  float* py = px + S * Ap;  float* pc = py + S * Ap;  float* ps = pc + S * Ap;
+  float* phl = ps + S * Ap; float* phw = phl + S * Ap;
+  float* psd = phw + S * Ap;                         // max signed corner distance (a4)
+  uint32_t* heads = (uint32_t*)(psd + S * Ap);       // [S][NBK] (block tag << 16) | agent
+  uint16_t* nxt = (uint16_t*)(heads + S * NBK);      // [S][Ap] next agent of the same bucket
+  uint16_t* over = nxt + S * Ap;                     // [S][Ap] agents too large for the hash
+  uint8_t* pvalid = (uint8_t*)(over + S * Ap);       // [S][Ap]
+  uint8_t* pov = pvalid + S * Ap;                    // [S][Ap] overlap flag (a3)
 
-  __shared__ int s_nq;
-  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  __shared__ int s_task;
+  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
   const int64_t TA = (int64_t)p.sim.T * A;
   const int64_t sb = (int64_t)b * TA;                // scenario offset in the trajectories
-  const int64_t rb = (int64_t)b * p.n_steps * A;     // scenario offset in the metric rows
+  const int64_t ab = (int64_t)b * p.n_steps;         // scenario offset in the action / metric rows, in rows
   const WmGridView gv = wm_grid_view(p.segrec, p.chunks, p.cells, p.pool, p.gridp, p.seg_cap, WM_POOL_CAP, b);
 
   // ---- prologue: row t0 of the simulated trajectory -> shared memory ----
@@ -103,121 +129,174 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     }
     sx[a] = x; sy[a] = y; syaw[a] = th; svx[a] = vx; svy[a] = vy; slen[a] = ln; swid[a] = wd;
     sc[a] = cs; ss[a] = sn; s_valid[a] = v;
-    s_sum[a] = 0.0; s_cnt[a] = 0; s_ov[a] = 0; s_anyov[a] = 0; s_anyoff[a] = 0; s_qm[a] = 0;
+    s_sum[a] = 0.0; s_cnt[a] = 0; s_anyov[a] = 0; s_anyoff[a] = 0;
   }
+  for (int i = tid; i < S * NBK; i += FUSED_NT) heads[i] = 0u;          // tag 0 = no block
+  if (tid < 2 * FUSED_S) s_nover[tid] = 0;
   __syncthreads();
 
   int n_eval = 0, n_slow = 0, n_corner = 0;
-  for (int k = 0; k < p.n_steps; ++k) {
-    const int t1 = p.t0 + k + 1;
-    // ================= phase A: one thread per agent =================
-    if (tid == 0) s_nq = 0;               // last read in phase B2 of the previous step, before its closing barrier
+  for (int k0 = 0, blk = 1; k0 < p.n_steps; k0 += S, ++blk) {
+    const int Sb = min(S, p.n_steps - k0);
+    const uint32_t tag = (uint32_t)(blk & 0xffff) << 16;
+    int* nover = s_nover + (blk & 1) * FUSED_S;
+    // ================= phase A: one thread per agent, Sb steps =================
+    if (tid == 0) s_task = 0;                                            // last read in phase B of the previous block
+    if (tid < FUSED_S) s_nover[((blk + 1) & 1) * FUSED_S + tid] = 0;     // next block's counters (last read two barriers ago)
     for (int a = tid; a < Ap; a += FUSED_NT) {
-      if (k > 0 && a < A) fused_flush_metrics(p, rb, k - 1, a, A, s_valid, s_ov, s_csd, s_anyov, s_anyoff);
-      s_ov[a] = 0;
-      bool vn = false;
-      float cs = 1.f, sn = 0.f, hl = 0.f, hw = 0.f, xn = 0.f, yn = 0.f;
-      if (a < A) {
-        const int64_t o = sb + (int64_t)t1 * A + a;
-        const int64_t ak = (int64_t)b * p.n_steps + k;
-        const bool use_dyn = p.av[ak * A + a] != 0 && s_valid[a] != 0;          // D8
-        const float lx = p.log.x[o], ly = p.log.y[o];
-        const uint8_t lvalid = p.log.valid[o];
-        float thn, vxn, vyn, ln, wd;
+      if (a >= A) {
+        for (int s = 0; s < Sb; ++s) { pvalid[s * Ap + a] = 0; pov[s * Ap + a] = 0; psd[s * Ap + a] = 0.f; }
+        continue;
+      }
+      float x = sx[a], y = sy[a], th = syaw[a], vx = svx[a], vy = svy[a], ln = slen[a], wd = swid[a], cs = sc[a], sn = ss[a];
+      bool v = s_valid[a] != 0;
+      double sum = s_sum[a];
+      int cnt = s_cnt[a];
+      FusedIn in = fused_load_in(p, sb, ab, k0, a, A);
+      for (int s = 0; s < Sb; ++s) {
+        const int k = k0 + s;
+        const FusedIn cur = in;
+        if (s + 1 < Sb) in = fused_load_in(p, sb, ab, k + 1, a, A);     // prefetch: nothing below depends on it
+        const int64_t o = sb + (int64_t)(p.t0 + k + 1) * A + a;
+        const bool use_dyn = cur.av != 0 && v;                          // D8
+        float xn, yn, thn, vxn, vyn, s1 = 0.f, c1 = 1.f;
         if (use_dyn) {
-          const float* act = p.actions + ak * p.C * A + a;
-          const float a2 = p.C > 2 ? act[2 * (int64_t)A] : 0.f;
-          wm_dyn_step(p.dyn, sx[a], sy[a], syaw[a], svx[a], svy[a], ss[a], sc[a], act[0], act[A], a2, xn, yn, thn,
-                      vxn, vyn, sn, cs);
-          ln = slen[a]; wd = swid[a];
-          vn = true;                                                            // D9
-        } else {                                                                // log playback, L164
-          xn = lx; yn = ly; thn = p.log.yaw[o]; vxn = p.log.vel_x[o]; vyn = p.log.vel_y[o];
+          wm_dyn_step(p.dyn, x, y, th, vx, vy, sn, cs, cur.a0, cur.a1, cur.a2, xn, yn, thn, vxn, vyn, s1, c1);
+          v = true;                                                     // D9: keeps its box
+        } else {                                                        // log playback, L164
+          xn = cur.lx; yn = cur.ly; thn = p.log.yaw[o]; vxn = p.log.vel_x[o]; vyn = p.log.vel_y[o];
           ln = p.log.length[o]; wd = p.log.width[o];
-          vn = lvalid != 0;
-          if (vn) sincosf(thn, &sn, &cs);
+          v = cur.lv != 0;
+          if (v) sincosf(thn, &s1, &c1);
         }
         p.sim.x[o] = xn; p.sim.y[o] = yn; p.sim.yaw[o] = thn; p.sim.vel_x[o] = vxn; p.sim.vel_y[o] = vyn;
-        p.sim.length[o] = ln; p.sim.width[o] = wd; p.sim.valid[o] = (uint8_t)vn;
-        const bool ldv = vn && lvalid != 0;                                     // a5, L106
-        const float d = ldv ? wm_logdiv(xn, yn, lx, ly) : 0.f;
-        if (p.out.log_div) p.out.log_div[rb + (int64_t)k * A + a] = d;
-        if (ldv) { s_sum[a] += (double)d; s_cnt[a] += 1; }
-        sx[a] = xn; sy[a] = yn; syaw[a] = thn; svx[a] = vxn; svy[a] = vyn; slen[a] = ln; swid[a] = wd;
-        if (vn) { hl = 0.5f * ln; hw = 0.5f * wd; } else { cs = 1.f; sn = 0.f; xn = 0.f; yn = 0.f; }
+        p.sim.length[o] = ln; p.sim.width[o] = wd; p.sim.valid[o] = (uint8_t)v;
+        const bool ldv = v && cur.lv != 0;                              // a5, L106
+        const float d = ldv ? wm_logdiv(xn, yn, cur.lx, cur.ly) : 0.f;
+        if (p.out.log_div) p.out.log_div[(ab + k) * A + a] = d;
+        if (ldv) { sum += (double)d; cnt += 1; }
+        x = xn; y = yn; th = thn; vx = vxn; vy = vyn; sn = s1; cs = c1;
+        // what the metrics of this step need; invalid slots: finite zeros (D10)
+        const int q = s * Ap + a;
+        const float hl = v ? 0.5f * ln : 0.f, hw = v ? 0.5f * wd : 0.f;
+        px[q] = v ? xn : 0.f; py[q] = v ? yn : 0.f; pc[q] = v ? c1 : 1.f; ps[q] = v ? s1 : 0.f;
+        phl[q] = hl; phw[q] = hw; pvalid[q] = (uint8_t)v;
+        if (v) {
+          if (sqrtf(fmaf(hl, hl, hw * hw)) <= FUSED_RMAX) {
+            const uint32_t bk = fused_bucket(fused_cell(xn), fused_cell(yn), (uint32_t)NBK - 1u);
+            const uint32_t old = atomicExch(&heads[s * NBK + bk], tag | (uint32_t)a);
+            nxt[q] = (uint16_t)((old & 0xffff0000u) == tag ? (old & 0xffffu) : FUSED_EMPTY);
+          } else {
+            over[s * Ap + atomicAdd(&nover[s], 1)] = (uint16_t)a;
+          }
+        }
       }
-      float ax = 0.f, ay = 0.f, bx = 0.f, by = 0.f;
-      if (vn) wm_box_offsets_sc(sn, cs, slen[a], swid[a], ax, ay, bx, by);
-      else { sx[a] = xn; sy[a] = yn; }                  // invalid slots: finite zeros for the overlap loads (D10)
-      sc[a] = cs; ss[a] = sn; shl[a] = hl; shw[a] = hw; srad[a] = sqrtf(fmaf(hl, hl, hw * hw));
-      oax[a] = ax; oay[a] = ay; obx[a] = bx; oby[a] = by;
-      s_valid[a] = vn;
-      const uint32_t w = __ballot_sync(0xffffffffu, vn);
-      if (lane == 0) s_vw[a >> 5] = w;
+      sx[a] = x; sy[a] = y; syaw[a] = th; svx[a] = vx; svy[a] = vy; slen[a] = ln; swid[a] = wd; sc[a] = cs; ss[a] = sn;
+      s_valid[a] = v; s_sum[a] = sum; s_cnt[a] = cnt;
     }
     __syncthreads();
-    // ================= phase B1: corners (a4), candidate walk =================
-    for (int c0 = 0; c0 < 4 * Ap; c0 += FUSED_NT) {
-      if (c0 + (tid & ~31) >= 4 * Ap) continue;                                 // warp-uniform (4 Ap % 128 == 0)
-      const int c = c0 + tid, a = c >> 2, kk = c & 3;
-      const bool v = s_valid[a] != 0;
-      const float ox = (kk & 1) ? obx[a] : oax[a], oy = (kk & 1) ? oby[a] : oay[a];
-      const float offx = (kk & 2) ? -ox : ox, offy = (kk & 2) ? -oy : oy;
-      float best; int bs;
-      const bool slow = wm_grid_fast(gv, v, sx[a], sy[a], offx, offy, best, bs, n_eval);
-      n_slow += slow; n_corner += v;
-      if (slow) { if (atomicOr(&s_qm[a], 1u << kk) == 0u) s_q[atomicAdd(&s_nq, 1)] = a; }
-      else s_csd[c] = v ? wm_grid_finish(gv, sx[a], sy[a], offx, offy, best, bs) : 0.f;
-    }
-    // ================= phase B: pairs (a3) =================
-    const int ntask = nb * (nb + 1) / 2 * FUSED_SUB;
-    for (int task = warp; task < ntask; task += FUSED_NT / 32) {
-      const int tile = task / FUSED_SUB, q = task % FUSED_SUB;
-      int I = 0, rem = tile;
-      while (rem >= nb - I) { rem -= nb - I; ++I; }
-      const int J = I + rem;
-      const uint32_t vi = s_vw[I] & (0xffu << (q * 8)), vj = s_vw[J];
-      if (vi == 0 || vj == 0) continue;
-      const int j = J * 32 + lane;
-      const float xj = sx[j], yj = sy[j], cj = sc[j], sj = ss[j], hlj = shl[j], hwj = shw[j], rj = srad[j];
-      const bool jv = (vj >> lane) & 1u;
-      bool any_j = false;
-      for (int ii = q * 8; ii < q * 8 + 8; ++ii) {
-        if (!((vi >> ii) & 1u)) continue;               // warp-uniform skip of invalid i
-        const int i = I * 32 + ii;
-        const float dx = xj - sx[i], dy = yj - sy[i];
-        bool ov = jv && i != j && wm_circles_touch(dx, dy, rj + srad[i]);
-        if (!__any_sync(0xffffffffu, ov)) continue;     // far apart
-        ov = ov && wm_sat_overlap(dx, dy, sc[i], ss[i], shl[i], shw[i], cj, sj, hlj, hwj);
-        any_j |= ov;
-        if (__any_sync(0xffffffffu, ov) && lane == 0) s_ov[i] = 1u;
+    // ================= phase B: warp tasks =================
+    const int n_ctask = Sb * nb * 4, n_task = n_ctask + Sb * nb;
+    for (;;) {
+      int task = 0;
+      if (lane == 0) task = atomicAdd(&s_task, 1);
+      task = __shfl_sync(0xffffffffu, task, 0);
+      if (task >= n_task) break;
+      if (task < n_ctask) {
+        // ---- 32 corners of 8 agents of step s (a4) ----
+        const int s = task / (nb * 4), c = (task - s * nb * 4) * 32 + lane, a = c >> 2, kk = c & 3;
+        const int q = s * Ap + a;
+        const bool v = pvalid[q] != 0;
+        const float cx = px[q], cy = py[q], hl = phl[q], hw = phw[q];
+        float ax, ay, bx, by;
+        wm_box_offsets_h(ps[q], pc[q], hl, hw, ax, ay, bx, by);
+        const float ox = (kk & 1) ? bx : ax, oy = (kk & 1) ? by : ay;
+        const float offx = (kk & 2) ? -ox : ox, offy = (kk & 2) ? -oy : oy;
+        float best; int bs;
+        const bool slow = wm_grid_fast(gv, v, cx, cy, offx, offy, best, bs, n_eval);
+        n_slow += slow; n_corner += v;
+        uint32_t todo = __ballot_sync(0xffffffffu, slow);
+        while (todo) {                                  // agents with corners off the grid / in a crowded cell
+          const int g4 = (__ffs(todo) - 1) & ~3;
+          const uint32_t gm = (todo >> g4) & 15u;
+          todo &= ~(15u << g4);
+          const float acx = __shfl_sync(0xffffffffu, cx, g4), acy = __shfl_sync(0xffffffffu, cy, g4);
+          const float fax = __shfl_sync(0xffffffffu, offx, g4), fay = __shfl_sync(0xffffffffu, offy, g4);
+          const float fbx = __shfl_sync(0xffffffffu, offx, g4 + 1), fby = __shfl_sync(0xffffffffu, offy, g4 + 1);
+          const float ahl = __shfl_sync(0xffffffffu, hl, g4), ahw = __shfl_sync(0xffffffffu, hw, g4);
+          const float o4x[4] = {fax, fbx, -fax, -fbx}, o4y[4] = {fay, fby, -fay, -fby};
+          float b4[4]; int i4[4], ne = 0;
+          wm_grid_search_warp4(gv, acx, acy, o4x, o4y, sqrtf(fmaf(ahl, ahl, ahw * ahw)), b4, i4, ne);
+          if ((lane & ~3) == g4 && ((gm >> kk) & 1u)) {
+            best = kk == 0 ? b4[0] : kk == 1 ? b4[1] : kk == 2 ? b4[2] : b4[3];
+            bs = kk == 0 ? i4[0] : kk == 1 ? i4[1] : kk == 2 ? i4[2] : i4[3];
+          }
+          if (lane == 0) n_eval += ne;
+        }
+        float m = v ? wm_grid_finish(gv, cx, cy, offx, offy, best, bs) : 0.f;
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));               // D18: max over the 4 corners
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+        if (kk == 0) psd[q] = v ? m : 0.f;
+      } else {
+        // ---- overlap flags of 32 agents of step s (a3) ----
+        const int t2 = task - n_ctask, s = t2 / nb, i = (t2 - s * nb) * 32 + lane;
+        const int q0 = s * Ap, qi = q0 + i;
+        bool ov = false;
+        if (pvalid[qi] != 0) {
+          const float xi = px[qi], yi = py[qi], ci = pc[qi], si = ps[qi], hli = phl[qi], hwi = phw[qi];
+          const float ri = sqrtf(fmaf(hli, hli, hwi * hwi));
+          auto test = [&](int j) {
+            if (j == i) return;
+            const int qj = q0 + j;
+            const float hlj = phl[qj], hwj = phw[qj];
+            const float rj = sqrtf(fmaf(hlj, hlj, hwj * hwj));
+            // the lower index takes the i role of k_overlap: (dx, dy) = c_hi - c_lo
+            const bool lo = i < j;
+            const float dx = lo ? px[qj] - xi : xi - px[qj], dy = lo ? py[qj] - yi : yi - py[qj];
+            if (!wm_circles_touch(dx, dy, lo ? rj + ri : ri + rj)) return;
+            ov |= lo ? wm_sat_overlap(dx, dy, ci, si, hli, hwi, pc[qj], ps[qj], hlj, hwj)
+                     : wm_sat_overlap(dx, dy, pc[qj], ps[qj], hlj, hwj, ci, si, hli, hwi);
+          };
+          if (ri <= FUSED_RMAX) {
+            const int ix = fused_cell(xi), iy = fused_cell(yi);
+            for (int dyc = -1; dyc <= 1; ++dyc)
+              for (int dxc = -1; dxc <= 1; ++dxc) {
+                const uint32_t hd = heads[s * NBK + fused_bucket(ix + dxc, iy + dyc, (uint32_t)NBK - 1u)];
+                uint32_t j = (hd & 0xffff0000u) == tag ? (hd & 0xffffu) : FUSED_EMPTY;
+                while (j != FUSED_EMPTY) { test((int)j); j = nxt[q0 + j]; }
+              }
+            const int no = nover[s];
+            for (int e = 0; e < no; ++e) test((int)over[q0 + e]);
+          } else {
+            for (int j = 0; j < A; ++j) if (pvalid[q0 + j] != 0) test(j);
+          }
+        }
+        pov[qi] = (uint8_t)ov;
       }
-      if (any_j) s_ov[j] = 1u;
     }
     __syncthreads();
-    // ================= phase B2: queued agents, one warp each =================
-    const int nq = s_nq;
-    for (int i = warp; i < nq; i += FUSED_NT / 32) {
-      const int a = s_q[i];
-      const uint32_t qm = s_qm[a];
-      const float offx[4] = {oax[a], obx[a], -oax[a], -obx[a]}, offy[4] = {oay[a], oby[a], -oay[a], -oby[a]};
-      float best[4]; int bs[4], ne = 0;
-      wm_grid_search_warp4(gv, sx[a], sy[a], offx, offy, srad[a], best, bs, ne);
-      if (lane < 4) {
-        const float ox = lane == 0 ? offx[0] : lane == 1 ? offx[1] : lane == 2 ? offx[2] : offx[3];
-        const float oy = lane == 0 ? offy[0] : lane == 1 ? offy[1] : lane == 2 ? offy[2] : offy[3];
-        const float bb = lane == 0 ? best[0] : lane == 1 ? best[1] : lane == 2 ? best[2] : best[3];
-        const int bi = lane == 0 ? bs[0] : lane == 1 ? bs[1] : lane == 2 ? bs[2] : bs[3];
-        if ((qm >> lane) & 1u) s_csd[4 * a + lane] = wm_grid_finish(gv, sx[a], sy[a], ox, oy, bb, bi);
+    // ================= phase C: metric rows of the block (D18, D19, D10) =================
+    for (int a = tid; a < A; a += FUSED_NT) {
+      uint8_t aov = s_anyov[a], aoff = s_anyoff[a];
+      for (int s = 0; s < Sb; ++s) {
+        const int q = s * Ap + a;
+        const int64_t o = (ab + k0 + s) * A + a;
+        const bool v = pvalid[q] != 0;
+        const float m = psd[q];
+        const uint8_t fo = pov[q], ff = (uint8_t)(v && m > 0.f);
+        if (p.out.overlap) p.out.overlap[o] = fo;
+        if (p.out.offroad_dist) p.out.offroad_dist[o] = m;
+        if (p.out.offroad) p.out.offroad[o] = ff;
+        aov |= fo; aoff |= ff;
       }
-      if (lane == 0) { s_qm[a] = 0; n_eval += ne; }
+      s_anyov[a] = aov; s_anyoff[a] = aoff;
     }
-    __syncthreads();
+    // no barrier: phase A of the next block is run by the same threads for the same agents, and the
+    // hash entries are tagged with the block number
   }
 
-  // ---- epilogue: last overlap row, aggregates (D21) ----
+  // ---- epilogue: aggregates (D21) ----
   for (int a = tid; a < A; a += FUSED_NT) {
-    fused_flush_metrics(p, rb, p.n_steps - 1, a, A, s_valid, s_ov, s_csd, s_anyov, s_anyoff);
     const int64_t o = (int64_t)b * A + a;
     if (p.out.any_overlap) p.out.any_overlap[o] = s_anyov[a];
     if (p.out.any_offroad) p.out.any_offroad[o] = s_anyoff[a];
@@ -241,15 +320,18 @@ cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_t
   FusedParams p;
   p.log = log; p.sim = sim; p.t0 = t0; p.n_steps = n_steps;
   p.C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  p.S = fused_pick_S(sim.A);
   p.actions = actions; p.av = action_valid; p.out = out;
   p.dyn = WmDynCfg{h->cfg.dynamics, h->cfg.dt, h->cfg.max_accel, h->cfg.max_curvature};
   p.segrec = h->segrec; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
   p.seg_cap = h->seg_tiles * WM_TILE_SEGS;
   p.stats = h->stats_on ? h->cull_stats : nullptr;
-  const size_t smem = fused_smem_bytes(sim.A);
+  const int Ap = (sim.A + 31) / 32 * 32;
+  const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(1024));
+    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)(fused_persist_bytes(1024) + fused_slot_bytes(1024)));
     if (e != cudaSuccess) return e;
     configured = true;
   }
