@@ -10,19 +10,24 @@
 // steps of the block is one pool of independent warp tasks, handed out through a shared counter:
 //
 //   phase A  one thread per agent : S successor states (shared arithmetic with k_step:
-//            wm_device.cuh), sim rows -> HBM, log divergence, per-step slots, spatial hash insert
-//   phase B  warp tasks, any warp : (step, 8 agents) -> 32 box corners: candidate walk of the corner's
-//                                   grid cell (wm_grid.cuh); corners off the grid or in a crowded
-//                                   cell are searched by the whole warp, one agent at a time;
-//                                   (step, 32 agents) -> overlap flags: each lane walks the 3 x 3 hash
-//                                   cells around its agent, circle pre-test, separating-axis test
+//            wm_device.cuh), sim rows -> HBM, log divergence, per-step slots; the agent's bounding
+//            box over the block goes into a spatial hash
+//   phase B  warp tasks, any warp : (agent, S steps) -> its 4 S box corners, one per lane: candidate
+//                                   walk of the corner's grid cell (wm_grid.cuh).  The lanes of a task
+//                                   follow one agent through consecutive steps, so they walk the
+//                                   same few cells: equal list lengths, the same cache lines.  Corners
+//                                   off the grid or in a crowded cell are searched by the whole warp;
+//                                   (32 agents) -> overlap flags of the block: each lane walks the
+//                                   3 x 3 hash cells around its agent; pairs whose block bounding
+//                                   boxes meet get the separating-axis test step by step
 //   phase C  one thread per agent : metric rows of the block -> HBM, any-flags
 //
-// Overlap broad phase: agents are hashed by the 8 m cell of their centre (linked lists in shared
-// memory, entries tagged with the block number so nothing is ever cleared).  Two boxes whose
-// circumradii are both <= 3.9 m can only overlap from adjacent cells; larger boxes go to a list
-// that every agent checks, and check every agent themselves.  A pair is always evaluated with the
-// lower agent index in the i role, like k_overlap, so flags equal the stepwise kernels' bit for bit.
+// Overlap broad phase, once per block: an agent is hashed by the 24 m cell of the centre of its
+// bounding box over the block (linked lists in shared memory, entries tagged with the block number
+// so nothing is ever cleared).  Two agents whose boxes (inflated by the circumradius) have half
+// extents <= 11.7 m can only overlap from adjacent cells; larger ones go to a list that every agent
+// checks, and check every agent themselves.  A pair is always evaluated with the lower agent index
+// in the i role, like k_overlap, so flags equal the stepwise kernels' bit for bit.
 //
 // Bound: instruction issue and the latency of the candidate walk's dependent loads; compulsory HBM
 // traffic is ~77 B per agent-step.  Results are bit-identical to the stepwise graph
@@ -36,9 +41,9 @@
 #ifndef FUSED_MINB
 #define FUSED_MINB 4
 #endif
-constexpr int FUSED_S = 8;                 // steps per block (fewer when A is large: shared memory)
-constexpr float FUSED_HASH_H = 8.f;        // hash cell side, metres
-constexpr float FUSED_RMAX = 3.9f;         // circumradius limit of hashed agents (< FUSED_HASH_H / 2, with margin)
+constexpr int FUSED_S = 8;                 // steps per block: 8, 4, 2 or 1 (fewer when A is large: shared memory)
+constexpr float FUSED_HASH_H = 24.f;       // hash cell side, metres
+constexpr float FUSED_EXT_MAX = 11.7f;     // half extent limit of hashed agents (< FUSED_HASH_H / 2, with margin)
 constexpr uint32_t FUSED_EMPTY = 0xffffu;
 
 struct FusedParams {
@@ -55,14 +60,18 @@ struct FusedParams {
 
 // shared-memory carve-up: persistent per-agent state, then S per-step slots
 __host__ __device__ inline int fused_nbk(int Ap) { int n = 64; while (n < 2 * Ap) n <<= 1; return n; }
-__host__ __device__ inline size_t fused_persist_bytes(int Ap) { return (size_t)Ap * (8 + 9 * 4 + 4 + 4) + 64; }
-__host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)Ap * (7 * 4 + 2 + 2 + 2) + (size_t)fused_nbk(Ap) * 4; }
+__host__ __device__ inline size_t fused_persist_bytes(int Ap) {
+  return (size_t)Ap * (8 + 9 * 4 + 4 + 4 + 16 + 4 + 2 + 2) + (size_t)fused_nbk(Ap) * 4 + 64;
+}
+__host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)Ap * (7 * 4 + 2); }
 static inline int fused_pick_S(int A) {
   const int Ap = (A + 31) / 32 * 32;
   const size_t budget = 54 * 1024;                        // 4 CTAs per SM when it fits
   const size_t per = fused_persist_bytes(Ap), slot = fused_slot_bytes(Ap);
-  int S = per + slot >= budget ? 1 : (int)((budget - per) / slot);
-  return S < 1 ? 1 : (S > FUSED_S ? FUSED_S : S);
+  const int fit = per + slot >= budget ? 1 : (int)((budget - per) / slot);
+  int S = FUSED_S;
+  while (S > 1 && S > fit) S >>= 1;
+  return S;
 }
 
 struct FusedIn { float a0, a1, a2, lx, ly; uint8_t av, lv; };
@@ -91,23 +100,26 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
   const int NBK = fused_nbk(Ap);
   // ---- persistent per-agent state ----
   double* s_sum = (double*)smem_raw;                 // [Ap] sum of valid log divergences (D21)
-  float* sx = (float*)(s_sum + Ap);
+  float4* s_bb = (float4*)(s_sum + Ap);              // [Ap] bounding box over the block, inflated: x0, y0, x1, y1
+  float* sx = (float*)(s_bb + Ap);
   float* sy = sx + Ap;    float* syaw = sy + Ap;   float* svx = syaw + Ap;  float* svy = svx + Ap;
   float* slen = svy + Ap; float* swid = slen + Ap; float* sc = swid + Ap;   float* ss = sc + Ap;
-  int* s_cnt = (int*)(ss + Ap);                      // [Ap] count of valid log divergences
-  uint8_t* s_valid = (uint8_t*)(s_cnt + Ap);         // [Ap]
+  float* s_br = ss + Ap;                             // [Ap] largest circumradius over the block, inflated
+  int* s_cnt = (int*)(s_br + Ap);                    // [Ap] count of valid log divergences
+  uint32_t* heads = (uint32_t*)(s_cnt + Ap);         // [NBK] (block tag << 16) | agent
+  int* s_nover = (int*)(heads + NBK);                // [2] oversize counts, by block parity (+ padding to 64 B)
+  uint16_t* nxt = (uint16_t*)(s_nover + 16);         // [Ap] next agent of the same bucket
+  uint16_t* over = nxt + Ap;                         // [Ap] agents too large for the hash
+  uint8_t* s_valid = (uint8_t*)(over + Ap);          // [Ap]
   uint8_t* s_anyov = s_valid + Ap;                   // [Ap]
   uint8_t* s_anyoff = s_anyov + Ap;                  // [Ap]
-  int* s_nover = (int*)(s_anyoff + 2 * Ap);          // [2][FUSED_S] oversize counts, by block parity
+  uint8_t* s_bvalid = s_anyoff + Ap;                 // [Ap] valid at some step of the block
   // ---- per-step slots ----
   float* px = (float*)(smem_raw + fused_persist_bytes(Ap));      // [S][Ap] each
   float* py = px + S * Ap;  float* pc = py + S * Ap;  float* ps = pc + S * Ap;
   float* phl = ps + S * Ap; float* phw = phl + S * Ap;
   float* psd = phw + S * Ap;                         // max signed corner distance (a4)
-  uint32_t* heads = (uint32_t*)(psd + S * Ap);       // [S][NBK] (block tag << 16) | agent
-  uint16_t* nxt = (uint16_t*)(heads + S * NBK);      // [S][Ap] next agent of the same bucket
-  uint16_t* over = nxt + S * Ap;                     // [S][Ap] agents too large for the hash
-  uint8_t* pvalid = (uint8_t*)(over + S * Ap);       // [S][Ap]
+  uint8_t* pvalid = (uint8_t*)(psd + S * Ap);        // [S][Ap]
   uint8_t* pov = pvalid + S * Ap;                    // [S][Ap] overlap flag (a3)
 
   __shared__ int s_task;
@@ -131,27 +143,30 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     sc[a] = cs; ss[a] = sn; s_valid[a] = v;
     s_sum[a] = 0.0; s_cnt[a] = 0; s_anyov[a] = 0; s_anyoff[a] = 0;
   }
-  for (int i = tid; i < S * NBK; i += FUSED_NT) heads[i] = 0u;          // tag 0 = no block
-  if (tid < 2 * FUSED_S) s_nover[tid] = 0;
+  for (int i = tid; i < NBK; i += FUSED_NT) heads[i] = 0u;              // tag 0 = no block
+  if (tid < 2) s_nover[tid] = 0;
   __syncthreads();
 
+  // lanes of a corner task: 4 corners x S steps x (8 / S) agents
+  const int kk = lane & 3, ls = (lane >> 2) & (S - 1), la = (lane >> 2) / S, apt = 8 / S;
   int n_eval = 0, n_slow = 0, n_corner = 0;
   for (int k0 = 0, blk = 1; k0 < p.n_steps; k0 += S, ++blk) {
     const int Sb = min(S, p.n_steps - k0);
     const uint32_t tag = (uint32_t)(blk & 0xffff) << 16;
-    int* nover = s_nover + (blk & 1) * FUSED_S;
+    int* nover = s_nover + (blk & 1);
     // ================= phase A: one thread per agent, Sb steps =================
-    if (tid == 0) s_task = 0;                                            // last read in phase B of the previous block
-    if (tid < FUSED_S) s_nover[((blk + 1) & 1) * FUSED_S + tid] = 0;     // next block's counters (last read two barriers ago)
+    if (tid == 0) { s_task = 0; s_nover[(blk + 1) & 1] = 0; }           // both last read before the previous barrier
     for (int a = tid; a < Ap; a += FUSED_NT) {
       if (a >= A) {
         for (int s = 0; s < Sb; ++s) { pvalid[s * Ap + a] = 0; pov[s * Ap + a] = 0; psd[s * Ap + a] = 0.f; }
+        s_bvalid[a] = 0;
         continue;
       }
       float x = sx[a], y = sy[a], th = syaw[a], vx = svx[a], vy = svy[a], ln = slen[a], wd = swid[a], cs = sc[a], sn = ss[a];
       bool v = s_valid[a] != 0;
       double sum = s_sum[a];
       int cnt = s_cnt[a];
+      float bx0 = 3.0e38f, by0 = 3.0e38f, bx1 = -3.0e38f, by1 = -3.0e38f, br = 0.f;
       FusedIn in = fused_load_in(p, sb, ab, k0, a, A);
       for (int s = 0; s < Sb; ++s) {
         const int k = k0 + s;
@@ -180,33 +195,45 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         const int q = s * Ap + a;
         const float hl = v ? 0.5f * ln : 0.f, hw = v ? 0.5f * wd : 0.f;
         px[q] = v ? xn : 0.f; py[q] = v ? yn : 0.f; pc[q] = v ? c1 : 1.f; ps[q] = v ? s1 : 0.f;
-        phl[q] = hl; phw[q] = hw; pvalid[q] = (uint8_t)v;
+        phl[q] = hl; phw[q] = hw; pvalid[q] = (uint8_t)v; pov[q] = 0;
         if (v) {
-          if (sqrtf(fmaf(hl, hl, hw * hw)) <= FUSED_RMAX) {
-            const uint32_t bk = fused_bucket(fused_cell(xn), fused_cell(yn), (uint32_t)NBK - 1u);
-            const uint32_t old = atomicExch(&heads[s * NBK + bk], tag | (uint32_t)a);
-            nxt[q] = (uint16_t)((old & 0xffff0000u) == tag ? (old & 0xffffu) : FUSED_EMPTY);
-          } else {
-            over[s * Ap + atomicAdd(&nover[s], 1)] = (uint16_t)a;
-          }
+          bx0 = fminf(bx0, xn); bx1 = fmaxf(bx1, xn); by0 = fminf(by0, yn); by1 = fmaxf(by1, yn);
+          br = fmaxf(br, sqrtf(fmaf(hl, hl, hw * hw)));
         }
       }
       sx[a] = x; sy[a] = y; syaw[a] = th; svx[a] = vx; svy[a] = vy; slen[a] = ln; swid[a] = wd; sc[a] = cs; ss[a] = sn;
       s_valid[a] = v; s_sum[a] = sum; s_cnt[a] = cnt;
+      // overlap broad phase of the block: the agent's boxes all lie inside [bx0 - br, bx1 + br] x [..]
+      const bool bv = bx0 <= bx1;
+      s_bvalid[a] = (uint8_t)bv;
+      if (bv) {
+        br = fmaf(br, 1.001f, 1e-3f);                                   // float32 rounding of the pair tests
+        s_bb[a] = make_float4(bx0 - br, by0 - br, bx1 + br, by1 + br);
+        s_br[a] = br;
+        const float ext = 0.5f * fmaxf(bx1 - bx0, by1 - by0) + br;
+        if (ext <= FUSED_EXT_MAX) {
+          const uint32_t bk = fused_bucket(fused_cell(0.5f * (bx0 + bx1)), fused_cell(0.5f * (by0 + by1)), (uint32_t)NBK - 1u);
+          const uint32_t old = atomicExch(&heads[bk], tag | (uint32_t)a);
+          nxt[a] = (uint16_t)((old & 0xffff0000u) == tag ? (old & 0xffffu) : FUSED_EMPTY);
+        } else {
+          over[atomicAdd(nover, 1)] = (uint16_t)a;
+        }
+      }
     }
     __syncthreads();
     // ================= phase B: warp tasks =================
-    const int n_ctask = Sb * nb * 4, n_task = n_ctask + Sb * nb;
+    const int n_ctask = Ap / apt, n_task = n_ctask + nb;
     for (;;) {
       int task = 0;
       if (lane == 0) task = atomicAdd(&s_task, 1);
       task = __shfl_sync(0xffffffffu, task, 0);
       if (task >= n_task) break;
       if (task < n_ctask) {
-        // ---- 32 corners of 8 agents of step s (a4) ----
-        const int s = task / (nb * 4), c = (task - s * nb * 4) * 32 + lane, a = c >> 2, kk = c & 3;
-        const int q = s * Ap + a;
-        const bool v = pvalid[q] != 0;
+        // ---- the 4 corners of one agent (8 / S agents) at every step of the block (a4) ----
+        const int a = task * apt + la;
+        const int q = ls * Ap + a;
+        const bool v = ls < Sb && pvalid[q] != 0;
+        if (!__any_sync(0xffffffffu, v)) continue;                      // psd of invalid slots is never read
         const float cx = px[q], cy = py[q], hl = phl[q], hw = phw[q];
         float ax, ay, bx, by;
         wm_box_offsets_h(ps[q], pc[q], hl, hw, ax, ay, bx, by);
@@ -216,7 +243,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         const bool slow = wm_grid_fast(gv, v, cx, cy, offx, offy, best, bs, n_eval);
         n_slow += slow; n_corner += v;
         uint32_t todo = __ballot_sync(0xffffffffu, slow);
-        while (todo) {                                  // agents with corners off the grid / in a crowded cell
+        while (todo) {                                  // boxes with corners off the grid / in a crowded cell
           const int g4 = (__ffs(todo) - 1) & ~3;
           const uint32_t gm = (todo >> g4) & 15u;
           todo &= ~(15u << g4);
@@ -236,42 +263,52 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         float m = v ? wm_grid_finish(gv, cx, cy, offx, offy, best, bs) : 0.f;
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));               // D18: max over the 4 corners
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-        if (kk == 0) psd[q] = v ? m : 0.f;
+        if (kk == 0 && v) psd[q] = m;
       } else {
-        // ---- overlap flags of 32 agents of step s (a3) ----
-        const int t2 = task - n_ctask, s = t2 / nb, i = (t2 - s * nb) * 32 + lane;
-        const int q0 = s * Ap, qi = q0 + i;
-        bool ov = false;
-        if (pvalid[qi] != 0) {
-          const float xi = px[qi], yi = py[qi], ci = pc[qi], si = ps[qi], hli = phl[qi], hwi = phw[qi];
-          const float ri = sqrtf(fmaf(hli, hli, hwi * hwi));
-          auto test = [&](int j) {
-            if (j == i) return;
-            const int qj = q0 + j;
-            const float hlj = phl[qj], hwj = phw[qj];
-            const float rj = sqrtf(fmaf(hlj, hlj, hwj * hwj));
-            // the lower index takes the i role of k_overlap: (dx, dy) = c_hi - c_lo
-            const bool lo = i < j;
-            const float dx = lo ? px[qj] - xi : xi - px[qj], dy = lo ? py[qj] - yi : yi - py[qj];
-            if (!wm_circles_touch(dx, dy, lo ? rj + ri : ri + rj)) return;
-            ov |= lo ? wm_sat_overlap(dx, dy, ci, si, hli, hwi, pc[qj], ps[qj], hlj, hwj)
-                     : wm_sat_overlap(dx, dy, pc[qj], ps[qj], hlj, hwj, ci, si, hli, hwi);
-          };
-          if (ri <= FUSED_RMAX) {
-            const int ix = fused_cell(xi), iy = fused_cell(yi);
-            for (int dyc = -1; dyc <= 1; ++dyc)
-              for (int dxc = -1; dxc <= 1; ++dxc) {
-                const uint32_t hd = heads[s * NBK + fused_bucket(ix + dxc, iy + dyc, (uint32_t)NBK - 1u)];
-                uint32_t j = (hd & 0xffff0000u) == tag ? (hd & 0xffffu) : FUSED_EMPTY;
-                while (j != FUSED_EMPTY) { test((int)j); j = nxt[q0 + j]; }
-              }
-            const int no = nover[s];
-            for (int e = 0; e < no; ++e) test((int)over[q0 + e]);
-          } else {
-            for (int j = 0; j < A; ++j) if (pvalid[q0 + j] != 0) test(j);
+        // ---- overlap flags of 32 agents at every step of the block (a3) ----
+        const int i = (task - n_ctask) * 32 + lane;
+        if (s_bvalid[i] != 0) {                         // per lane: no warp-level operation inside
+        const float4 bi = s_bb[i];
+        const float ri = s_br[i];
+        uint32_t ovm = 0;                               // bit s: overlap at step s
+        auto test = [&](int j) {
+          if (j == i) return;
+          const float4 bj = s_bb[j];
+          if (bi.x > bj.z || bj.x > bi.z || bi.y > bj.w || bj.y > bi.w) return;       // boxes of the block apart
+          const float rr = ri + s_br[j], rr2 = rr * rr;
+          const int lo = min(i, j), hi = max(i, j);     // the lower index takes the i role of k_overlap
+          for (int s = 0; s < Sb; ++s) {
+            const int ql = s * Ap + lo, qh = s * Ap + hi;
+            if (pvalid[ql] == 0 || pvalid[qh] == 0) continue;
+            const float dx = px[qh] - px[ql], dy = py[qh] - py[ql];
+            if (fmaf(dx, dx, dy * dy) > rr2) continue;  // rr >= r_lo + r_hi of the step, inflated
+            const float hll = phl[ql], hwl = phw[ql], hlh = phl[qh], hwh = phw[qh];
+            // the pair test of k_overlap, operand for operand
+            if (wm_circles_touch(dx, dy, sqrtf(fmaf(hlh, hlh, hwh * hwh)) + sqrtf(fmaf(hll, hll, hwl * hwl))) &&
+                wm_sat_overlap(dx, dy, pc[ql], ps[ql], hll, hwl, pc[qh], ps[qh], hlh, hwh)) ovm |= 1u << s;
           }
+        };
+        if (0.5f * fmaxf(bi.z - bi.x, bi.w - bi.y) <= FUSED_EXT_MAX) {
+          const int ix = fused_cell(0.5f * (bi.x + bi.z)), iy = fused_cell(0.5f * (bi.y + bi.w));
+          uint32_t j = FUSED_EMPTY;
+          for (int probe = 0; ;) {                      // one flat loop over the 9 cells and their lists
+            if (j == FUSED_EMPTY) {
+              if (probe == 9) break;
+              const uint32_t hd = heads[fused_bucket(ix + probe % 3 - 1, iy + probe / 3 - 1, (uint32_t)NBK - 1u)];
+              j = (hd & 0xffff0000u) == tag ? (hd & 0xffffu) : FUSED_EMPTY;
+              ++probe;
+              continue;
+            }
+            test((int)j);
+            j = nxt[j];
+          }
+          const int no = *nover;
+          for (int e = 0; e < no; ++e) test((int)over[e]);
+        } else {
+          for (int j = 0; j < A; ++j) if (s_bvalid[j] != 0) test(j);
         }
-        pov[qi] = (uint8_t)ov;
+        for (int s = 0; s < Sb; ++s) if ((ovm >> s) & 1u) pov[s * Ap + i] = 1;
+        }
       }
     }
     __syncthreads();
@@ -282,7 +319,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         const int q = s * Ap + a;
         const int64_t o = (ab + k0 + s) * A + a;
         const bool v = pvalid[q] != 0;
-        const float m = psd[q];
+        const float m = v ? psd[q] : 0.f;
         const uint8_t fo = pov[q], ff = (uint8_t)(v && m > 0.f);
         if (p.out.overlap) p.out.overlap[o] = fo;
         if (p.out.offroad_dist) p.out.offroad_dist[o] = m;
