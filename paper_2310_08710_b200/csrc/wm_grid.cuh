@@ -23,17 +23,19 @@ constexpr float WM_CULL_ABS = 1e-5f;     //   (float32 rounding of 200 m-scale c
 
 struct WmGridView {          // one scenario's prepared search structures
   const float4* rec;         // [nseg][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}
+  const float4* pair;        // [ceil(nseg/2)][3] records 2p (e) and 2p+1 (o): {p0x_e,p0x_o,p0y_e,p0y_o} {-ex_e,-ex_o,-ey_e,-ey_o} {gx_e,gx_o,gy_e,gy_o}
   const float4* chunks;      // [ceil(nseg/32)] bounding boxes {x0,y0,x1,y1}
   const uint4* cells;        // [ny*nx] headers
   const uint32_t* pool;      // overflow runs
   WmGrid g;
 };
 
-__device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const float4* chunks, const uint4* cells,
+__device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const float4* segpair, const float4* chunks, const uint4* cells,
                                                    const uint32_t* pool, const WmGrid* gridp, int seg_cap,
                                                    int pool_cap, int b) {
   WmGridView v;
   v.rec = segrec + (int64_t)b * seg_cap * 2;
+  v.pair = segpair + (int64_t)b * (seg_cap / 2) * 3;
   v.chunks = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
   v.cells = cells + (int64_t)b * WM_GRID_CELLS;
   v.pool = pool + (int64_t)b * pool_cap;
@@ -51,17 +53,35 @@ __device__ __forceinline__ float wm_rec_d2(const float4 r0, const float4 r1, flo
   return __fmaf_rn(ry, ry, __fmul_rn(rx, rx));
 }
 
+// The same squared distances for the two records of a pair record at once, with packed float32x2
+// arithmetic (FADD2 / FMUL2 / FFMA2): component for component the operations and roundings of
+// wm_rec_d2, so both give the same bits (fma(-t, e, w) == fma(t, -e, w); the pair stores -e).
+__device__ __forceinline__ void wm_pair_d2(const float4 P, const float4 NE, const float4 G, wm_u64 cx2, wm_u64 cy2,
+                                           wm_u64 ox2, wm_u64 oy2, float& d_e, float& d_o) {
+  const wm_u64 wx = add2(sub2(cx2, pk2(P.x, P.y)), ox2), wy = add2(sub2(cy2, pk2(P.z, P.w)), oy2);
+  const wm_u64 m = mul2(wx, pk2(G.x, G.y));
+  float wy_e, wy_o, m_e, m_o;
+  upk2(wy, wy_e, wy_o); upk2(m, m_e, m_o);
+  const wm_u64 t = pk2(__saturatef(__fmaf_rn(wy_e, G.z, m_e)), __saturatef(__fmaf_rn(wy_o, G.w, m_o)));
+  const wm_u64 rx = fma2(t, pk2(NE.x, NE.y), wx), ry = fma2(t, pk2(NE.z, NE.w), wy);
+  upk2(fma2(ry, ry, mul2(rx, rx)), d_e, d_o);
+}
+
 // Walk of a cell's candidate runs as ONE flat loop (a warp runs max-over-lanes of the total
-// count, not the sum of per-run maxima), 4 records per iteration with all 8 loads issued before
-// the arithmetic (the walk is latency bound otherwise).  Slots beyond the end of a run re-read
-// its first record: evaluating a candidate twice is harmless.  Up to 4 runs sit in registers,
-// refilled from the pool.
-__device__ __forceinline__ void wm_grid_walk(const float4* __restrict__ rec, uint32_t r0, uint32_t r1, uint32_t r2,
+// count, not the sum of per-run maxima), two pair records = 4 records per iteration with all 6
+// loads issued before the arithmetic (the walk is latency bound otherwise).  A run that starts or
+// ends inside a pair record evaluates the pair's other record too, and a slot beyond the end of a
+// run re-reads its last pair: evaluating a real segment that is not a candidate, or a candidate
+// twice, cannot change the result (it is no nearer than the winner, and on an exact tie the winner
+// has the lower index: D17; indices are visited in ascending order with strict '<').  Padding
+// records sit at 1e18.  Up to 4 runs sit in registers, refilled from the pool.
+__device__ __forceinline__ void wm_grid_walk(const float4* __restrict__ pr, uint32_t r0, uint32_t r1, uint32_t r2,
                                              uint32_t r3, const uint32_t* __restrict__ pool, int n_pool, float cx,
                                              float cy, float offx, float offy, float& best, int& bs, int& n_eval) {
-  int s = 0, left = 0;
+  const wm_u64 cx2 = pk2(cx, cx), cy2 = pk2(cy, cy), ox2 = pk2(offx, offx), oy2 = pk2(offy, offy);
+  int p = 0, pe = -1;
   for (;;) {
-    if (left <= 0) {
+    if (p > pe) {
       if (r0 == 0u) {
         if (n_pool <= 0) break;
         r0 = __ldg(pool);
@@ -70,20 +90,22 @@ __device__ __forceinline__ void wm_grid_walk(const float4* __restrict__ rec, uin
         r3 = n_pool > 3 ? __ldg(pool + 3) : 0u;
         pool += 4; n_pool -= 4;
       }
-      s = (int)(r0 >> 8); left = (int)(r0 & 255u);
-      n_eval += left;
+      const int first = (int)(r0 >> 8), cnt = (int)(r0 & 255u);
+      p = first >> 1; pe = (first + cnt - 1) >> 1;
+      n_eval += cnt;
       r0 = r1; r1 = r2; r2 = r3; r3 = 0u;
     }
-    const int s1 = left > 1 ? s + 1 : s, s2 = left > 2 ? s + 2 : s, s3 = left > 3 ? s + 3 : s;
-    const float4 a0 = __ldg(rec + 2 * s), b0 = __ldg(rec + 2 * s + 1), a1 = __ldg(rec + 2 * s1), b1 = __ldg(rec + 2 * s1 + 1);
-    const float4 a2 = __ldg(rec + 2 * s2), b2 = __ldg(rec + 2 * s2 + 1), a3 = __ldg(rec + 2 * s3), b3 = __ldg(rec + 2 * s3 + 1);
-    const float d0 = wm_rec_d2(a0, b0, cx, cy, offx, offy), d1 = wm_rec_d2(a1, b1, cx, cy, offx, offy);
-    const float d2 = wm_rec_d2(a2, b2, cx, cy, offx, offy), d3 = wm_rec_d2(a3, b3, cx, cy, offx, offy);
-    if (d0 < best) { best = d0; bs = s; }       // ascending index, strict '<': exact ties -> lower index (D17)
-    if (d1 < best) { best = d1; bs = s1; }
-    if (d2 < best) { best = d2; bs = s2; }
-    if (d3 < best) { best = d3; bs = s3; }
-    s += 4; left -= 4;
+    const int q = min(p + 1, pe);
+    const float4 a0 = __ldg(pr + 3 * p), a1 = __ldg(pr + 3 * p + 1), a2 = __ldg(pr + 3 * p + 2);
+    const float4 b0 = __ldg(pr + 3 * q), b1 = __ldg(pr + 3 * q + 1), b2 = __ldg(pr + 3 * q + 2);
+    float d0, d1, d2, d3;
+    wm_pair_d2(a0, a1, a2, cx2, cy2, ox2, oy2, d0, d1);
+    wm_pair_d2(b0, b1, b2, cx2, cy2, ox2, oy2, d2, d3);
+    if (d0 < best) { best = d0; bs = 2 * p; }       // ascending index, strict '<': exact ties -> lower index (D17)
+    if (d1 < best) { best = d1; bs = 2 * p + 1; }
+    if (d2 < best) { best = d2; bs = 2 * q; }
+    if (d3 < best) { best = d3; bs = 2 * q + 1; }
+    p += 2;
   }
 }
 
@@ -225,7 +247,7 @@ __device__ __forceinline__ bool wm_grid_fast(const WmGridView& v, bool active, f
       }
     }
   }
-  wm_grid_walk(v.rec, hd.x, hd.y, hd.z, hd.w, pool, n_pool, cx, cy, offx, offy, best, bs, n_eval);   // no-op without runs
+  wm_grid_walk(v.pair, hd.x, hd.y, hd.z, hd.w, pool, n_pool, cx, cy, offx, offy, best, bs, n_eval);   // no-op without runs
   return slow;
 }
 
