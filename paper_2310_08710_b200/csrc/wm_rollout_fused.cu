@@ -18,8 +18,9 @@
 //                                   same few cells: equal list lengths, the same cache lines.  Corners
 //                                   off the grid or in a crowded cell are searched by the whole warp;
 //                                   (32 agents) -> overlap flags of the block: each lane walks the
-//                                   3 x 3 hash cells around its agent; pairs whose block bounding
-//                                   boxes meet get the separating-axis test step by step
+//                                   3 x 3 hash cells around its agent and lists the pairs whose
+//                                   block bounding boxes meet; then one lane per (pair, step) runs
+//                                   the circle and separating-axis tests
 //   phase C  one thread per agent : metric rows of the block -> HBM, any-flags
 //
 // Overlap broad phase, once per block: an agent is hashed by the 24 m cell of the centre of its
@@ -45,6 +46,8 @@ constexpr int FUSED_S = 8;                 // steps per block: 8, 4, 2 or 1 (few
 constexpr float FUSED_HASH_H = 24.f;       // hash cell side, metres
 constexpr float FUSED_EXT_MAX = 11.7f;     // half extent limit of hashed agents (< FUSED_HASH_H / 2, with margin)
 constexpr uint32_t FUSED_EMPTY = 0xffffu;
+constexpr int FUSED_PAD = 4;                // slot rows are Ap + 4 long: the 8 steps of an agent fall into 8 different banks
+constexpr int FUSED_PL = 96;                // pair list entries per warp (overlap narrow phase)
 
 struct FusedParams {
   wm_traj log, sim;
@@ -61,9 +64,9 @@ struct FusedParams {
 // shared-memory carve-up: persistent per-agent state, then S per-step slots
 __host__ __device__ inline int fused_nbk(int Ap) { int n = 64; while (n < 2 * Ap) n <<= 1; return n; }
 __host__ __device__ inline size_t fused_persist_bytes(int Ap) {
-  return (size_t)Ap * (8 + 9 * 4 + 4 + 4 + 16 + 4 + 2 + 2) + (size_t)fused_nbk(Ap) * 4 + 64;
+  return (size_t)Ap * (8 + 9 * 4 + 4 + 4 + 16 + 4 + 2 + 2) + (size_t)fused_nbk(Ap) * 4 + 64 + (FUSED_NT / 32) * (FUSED_PL + 1) * 4;
 }
-__host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)Ap * (7 * 4 + 2); }
+__host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)(Ap + FUSED_PAD) * (7 * 4 + 2); }
 static inline int fused_pick_S(int A) {
   const int Ap = (A + 31) / 32 * 32;
   const size_t budget = 54 * 1024;                        // 4 CTAs per SM when it fits
@@ -96,7 +99,7 @@ __device__ __forceinline__ uint32_t fused_bucket(int ix, int iy, uint32_t mask) 
 
 __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int A = p.sim.A, nb = (A + 31) / 32, Ap = nb * 32, S = p.S;
+  const int A = p.sim.A, nb = (A + 31) / 32, Ap = nb * 32, Aps = Ap + FUSED_PAD, S = p.S;
   const int NBK = fused_nbk(Ap);
   // ---- persistent per-agent state ----
   double* s_sum = (double*)smem_raw;                 // [Ap] sum of valid log divergences (D21)
@@ -108,19 +111,20 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
   int* s_cnt = (int*)(s_br + Ap);                    // [Ap] count of valid log divergences
   uint32_t* heads = (uint32_t*)(s_cnt + Ap);         // [NBK] (block tag << 16) | agent
   int* s_nover = (int*)(heads + NBK);                // [2] oversize counts, by block parity (+ padding to 64 B)
-  uint16_t* nxt = (uint16_t*)(s_nover + 16);         // [Ap] next agent of the same bucket
+  uint32_t* s_pl = (uint32_t*)(s_nover + 16);        // [warps][FUSED_PL + 1] pairs whose block boxes meet: count, (lo << 16) | hi
+  uint16_t* nxt = (uint16_t*)(s_pl + (FUSED_NT / 32) * (FUSED_PL + 1));      // [Ap] next agent of the same bucket
   uint16_t* over = nxt + Ap;                         // [Ap] agents too large for the hash
   uint8_t* s_valid = (uint8_t*)(over + Ap);          // [Ap]
   uint8_t* s_anyov = s_valid + Ap;                   // [Ap]
   uint8_t* s_anyoff = s_anyov + Ap;                  // [Ap]
   uint8_t* s_bvalid = s_anyoff + Ap;                 // [Ap] valid at some step of the block
   // ---- per-step slots ----
-  float* px = (float*)(smem_raw + fused_persist_bytes(Ap));      // [S][Ap] each
-  float* py = px + S * Ap;  float* pc = py + S * Ap;  float* ps = pc + S * Ap;
-  float* phl = ps + S * Ap; float* phw = phl + S * Ap;
-  float* psd = phw + S * Ap;                         // max signed corner distance (a4)
-  uint8_t* pvalid = (uint8_t*)(psd + S * Ap);        // [S][Ap]
-  uint8_t* pov = pvalid + S * Ap;                    // [S][Ap] overlap flag (a3)
+  float* px = (float*)(smem_raw + fused_persist_bytes(Ap));      // [S][Aps] each
+  float* py = px + S * Aps;  float* pc = py + S * Aps;  float* ps = pc + S * Aps;
+  float* phl = ps + S * Aps; float* phw = phl + S * Aps;
+  float* psd = phw + S * Aps;                        // max signed corner distance (a4)
+  uint8_t* pvalid = (uint8_t*)(psd + S * Aps);       // [S][Aps]
+  uint8_t* pov = pvalid + S * Aps;                   // [S][Aps] overlap flag (a3)
 
   __shared__ int s_task;
   const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
@@ -158,7 +162,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     if (tid == 0) { s_task = 0; s_nover[(blk + 1) & 1] = 0; }           // both last read before the previous barrier
     for (int a = tid; a < Ap; a += FUSED_NT) {
       if (a >= A) {
-        for (int s = 0; s < Sb; ++s) { pvalid[s * Ap + a] = 0; pov[s * Ap + a] = 0; psd[s * Ap + a] = 0.f; }
+        for (int s = 0; s < Sb; ++s) { pvalid[s * Aps + a] = 0; pov[s * Aps + a] = 0; psd[s * Aps + a] = 0.f; }
         s_bvalid[a] = 0;
         continue;
       }
@@ -192,7 +196,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         if (ldv) { sum += (double)d; cnt += 1; }
         x = xn; y = yn; th = thn; vx = vxn; vy = vyn; sn = s1; cs = c1;
         // what the metrics of this step need; invalid slots: finite zeros (D10)
-        const int q = s * Ap + a;
+        const int q = s * Aps + a;
         const float hl = v ? 0.5f * ln : 0.f, hw = v ? 0.5f * wd : 0.f;
         px[q] = v ? xn : 0.f; py[q] = v ? yn : 0.f; pc[q] = v ? c1 : 1.f; ps[q] = v ? s1 : 0.f;
         phl[q] = hl; phw[q] = hw; pvalid[q] = (uint8_t)v; pov[q] = 0;
@@ -231,7 +235,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
       if (task >= nb) {
         // ---- the 4 corners of one agent (8 / S agents) at every step of the block (a4) ----
         const int a = (task - nb) * apt + la;
-        const int q = ls * Ap + a;
+        const int q = ls * Aps + a;
         const bool v = ls < Sb && pvalid[q] != 0;
         if (!__any_sync(0xffffffffu, v)) continue;                      // psd of invalid slots is never read
         const float cx = px[q], cy = py[q], hl = phl[q], hw = phw[q];
@@ -266,48 +270,56 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         if (kk == 0 && v) psd[q] = m;
       } else {
         // ---- overlap flags of 32 agents at every step of the block (a3) ----
+        // broad phase, one lane per agent i: the pairs (i, j > i) whose block boxes meet go to the
+        // warp's list; narrow phase, one lane per (pair, step): the pair test of k_overlap
         const int i = task * 32 + lane;
-        if (s_bvalid[i] != 0) {                         // per lane: no warp-level operation inside
-        const float4 bi = s_bb[i];
-        const float ri = s_br[i];
-        uint32_t ovm = 0;                               // bit s: overlap at step s
-        auto test = [&](int j) {
-          if (j == i) return;
-          const float4 bj = s_bb[j];
-          if (bi.x > bj.z || bj.x > bi.z || bi.y > bj.w || bj.y > bi.w) return;       // boxes of the block apart
-          const float rr = ri + s_br[j], rr2 = rr * rr;
-          const int lo = min(i, j), hi = max(i, j);     // the lower index takes the i role of k_overlap
-          for (int s = 0; s < Sb; ++s) {
-            const int ql = s * Ap + lo, qh = s * Ap + hi;
-            if (pvalid[ql] == 0 || pvalid[qh] == 0) continue;
-            const float dx = px[qh] - px[ql], dy = py[qh] - py[ql];
-            if (fmaf(dx, dx, dy * dy) > rr2) continue;  // rr >= r_lo + r_hi of the step, inflated
-            const float hll = phl[ql], hwl = phw[ql], hlh = phl[qh], hwh = phw[qh];
-            // the pair test of k_overlap, operand for operand
-            if (wm_circles_touch(dx, dy, sqrtf(fmaf(hlh, hlh, hwh * hwh)) + sqrtf(fmaf(hll, hll, hwl * hwl))) &&
-                wm_sat_overlap(dx, dy, pc[ql], ps[ql], hll, hwl, pc[qh], ps[qh], hlh, hwh)) ovm |= 1u << s;
-          }
+        uint32_t* pl = s_pl + (tid >> 5) * (FUSED_PL + 1);
+        auto narrow = [&](int lo, int hi, int s) {       // lo < hi: the lower index takes the i role of k_overlap
+          const int ql = s * Aps + lo, qh = s * Aps + hi;
+          if (pvalid[ql] == 0 || pvalid[qh] == 0) return;
+          const float dx = px[qh] - px[ql], dy = py[qh] - py[ql];
+          const float hll = phl[ql], hwl = phw[ql], hlh = phl[qh], hwh = phw[qh];
+          if (wm_circles_touch(dx, dy, sqrtf(fmaf(hlh, hlh, hwh * hwh)) + sqrtf(fmaf(hll, hll, hwl * hwl))) &&
+              wm_sat_overlap(dx, dy, pc[ql], ps[ql], hll, hwl, pc[qh], ps[qh], hlh, hwh)) { pov[ql] = 1; pov[qh] = 1; }
         };
-        if (0.5f * fmaxf(bi.z - bi.x, bi.w - bi.y) <= FUSED_EXT_MAX) {
-          const int ix = fused_cell(0.5f * (bi.x + bi.z)), iy = fused_cell(0.5f * (bi.y + bi.w));
-          uint32_t j = FUSED_EMPTY;
-          for (int probe = 0; ;) {                      // one flat loop over the 9 cells and their lists
-            if (j == FUSED_EMPTY) {
-              if (probe == 9) break;
-              const uint32_t hd = heads[fused_bucket(ix + probe % 3 - 1, iy + probe / 3 - 1, (uint32_t)NBK - 1u)];
-              j = (hd & 0xffff0000u) == tag ? (hd & 0xffffu) : FUSED_EMPTY;
-              ++probe;
-              continue;
+        if (lane == 0) pl[0] = 0;
+        __syncwarp();
+        if (s_bvalid[i] != 0) {                         // per lane: no warp-level operation inside
+          const float4 bi = s_bb[i];
+          auto test = [&](int j) {
+            if (j <= i) return;
+            const float4 bj = s_bb[j];
+            if (bi.x > bj.z || bj.x > bi.z || bi.y > bj.w || bj.y > bi.w) return;     // boxes of the block apart
+            const uint32_t slot = atomicAdd(&pl[0], 1u);
+            if (slot < (uint32_t)FUSED_PL) pl[1 + slot] = ((uint32_t)i << 16) | (uint32_t)j;
+            else for (int s = 0; s < Sb; ++s) narrow(i, j, s);                        // list full: in place
+          };
+          if (0.5f * fmaxf(bi.z - bi.x, bi.w - bi.y) <= FUSED_EXT_MAX) {
+            const int ix = fused_cell(0.5f * (bi.x + bi.z)), iy = fused_cell(0.5f * (bi.y + bi.w));
+            uint32_t j = FUSED_EMPTY;
+            for (int probe = 0; ;) {                    // one flat loop over the 9 cells and their lists
+              if (j == FUSED_EMPTY) {
+                if (probe == 9) break;
+                const uint32_t hd = heads[fused_bucket(ix + probe % 3 - 1, iy + probe / 3 - 1, (uint32_t)NBK - 1u)];
+                j = (hd & 0xffff0000u) == tag ? (hd & 0xffffu) : FUSED_EMPTY;
+                ++probe;
+                continue;
+              }
+              test((int)j);
+              j = nxt[j];
             }
-            test((int)j);
-            j = nxt[j];
+            const int no = *nover;
+            for (int e = 0; e < no; ++e) test((int)over[e]);
+          } else {
+            for (int j = i + 1; j < A; ++j) if (s_bvalid[j] != 0) test(j);
           }
-          const int no = *nover;
-          for (int e = 0; e < no; ++e) test((int)over[e]);
-        } else {
-          for (int j = 0; j < A; ++j) if (s_bvalid[j] != 0) test(j);
         }
-        for (int s = 0; s < Sb; ++s) if ((ovm >> s) & 1u) pov[s * Ap + i] = 1;
+        __syncwarp();
+        const int np = (int)min(pl[0], (uint32_t)FUSED_PL);
+        for (int it = lane; it < np * S; it += 32) {
+          const uint32_t pr = pl[1 + it / S];
+          const int s = it & (S - 1);
+          if (s < Sb) narrow((int)(pr >> 16), (int)(pr & 0xffffu), s);
         }
       }
     }
@@ -316,7 +328,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     for (int a = tid; a < A; a += FUSED_NT) {
       uint8_t aov = s_anyov[a], aoff = s_anyoff[a];
       for (int s = 0; s < Sb; ++s) {
-        const int q = s * Ap + a;
+        const int q = s * Aps + a;
         const int64_t o = (ab + k0 + s) * A + a;
         const bool v = pvalid[q] != 0;
         const float m = v ? psd[q] : 0.f;
