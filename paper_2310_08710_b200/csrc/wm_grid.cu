@@ -234,7 +234,7 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s) {
 struct GridParams {
   wm_row row;
   int A;
-  const float4* segrec; const float4* segpair; const float4* chunks; const uint4* cells; const uint32_t* pool; const WmGrid* gridp;
+  const float4* segrec; const float4* segpair; const float4* segfin; const float4* chunks; const uint4* cells; const uint32_t* pool; const WmGrid* gridp;
   int seg_cap;
   float* sd; int64_t sd_stride_b;
   float* corner;
@@ -248,7 +248,7 @@ __global__ void __launch_bounds__(128) k_offroad_grid(GridParams p) {
   const int A = p.A;
   const int64_t ro = (int64_t)b * p.row.stride_b;
   const bool v = a < A && p.row.valid[ro + a] != 0;
-  const WmGridView gv = wm_grid_view(p.segrec, p.segpair, p.chunks, p.cells, p.pool, p.gridp, p.seg_cap, WM_POOL_CAP, b);
+  const WmGridView gv = wm_grid_view(p.segrec, p.segpair, p.segfin, p.chunks, p.cells, p.pool, p.gridp, p.seg_cap, WM_POOL_CAP, b);
   int n_eval = 0;
   bool slow = false;
   float cx = 0.f, cy = 0.f, offx = 0.f, offy = 0.f;
@@ -284,7 +284,7 @@ cudaError_t wm_launch_offroad_grid(wm_handle* h, const wm_traj& sim, int t, floa
   GridParams p;
   p.row = wm_make_row(sim, t);
   p.A = sim.A;
-  p.segrec = h->segrec; p.segpair = h->segpair; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
+  p.segrec = h->segrec; p.segpair = h->segpair; p.segfin = h->segfin; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
   p.seg_cap = h->seg_tiles * WM_TILE_SEGS;
   p.sd = sd; p.sd_stride_b = sd_stride_b; p.corner = corner; p.flag = flag; p.flag_stride_b = flag_stride_b;
   p.stats = h->stats_on ? h->cull_stats : nullptr;

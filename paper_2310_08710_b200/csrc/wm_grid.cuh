@@ -23,6 +23,7 @@ constexpr float WM_CULL_ABS = 1e-5f;     //   (float32 rounding of 200 m-scale c
 
 struct WmGridView {          // one scenario's prepared search structures
   const float4* rec;         // [nseg][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}
+  const float4* fin;         // [nseg] {p0x, p0y, sx, sy}
   const float4* pair;        // [ceil(nseg/2)][3] records 2p (e) and 2p+1 (o): {p0x_e,p0x_o,p0y_e,p0y_o} {-ex_e,-ex_o,-ey_e,-ey_o} {gx_e,gx_o,gy_e,gy_o}
   const float4* chunks;      // [ceil(nseg/32)] bounding boxes {x0,y0,x1,y1}
   const uint4* cells;        // [ny*nx] headers
@@ -30,12 +31,13 @@ struct WmGridView {          // one scenario's prepared search structures
   WmGrid g;
 };
 
-__device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const float4* segpair, const float4* chunks, const uint4* cells,
+__device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const float4* segpair, const float4* segfin, const float4* chunks, const uint4* cells,
                                                    const uint32_t* pool, const WmGrid* gridp, int seg_cap,
                                                    int pool_cap, int b) {
   WmGridView v;
   v.rec = segrec + (int64_t)b * seg_cap * 2;
   v.pair = segpair + (int64_t)b * (seg_cap / 2) * 3;
+  v.fin = segfin + (int64_t)b * seg_cap;
   v.chunks = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
   v.cells = cells + (int64_t)b * WM_GRID_CELLS;
   v.pool = pool + (int64_t)b * pool_cap;
@@ -255,9 +257,9 @@ __device__ __forceinline__ float wm_grid_finish(const WmGridView& v, float cx, f
                                                 int bs) {
   if (v.g.nseg <= 0) return -FLT_MAX;                                      // D20
   // e x (q - p0) > 0 is the left side of the oriented segment = on-road (D16)
-  const float4 r0 = __ldg(v.rec + 2 * bs), r1 = __ldg(v.rec + 2 * bs + 1);
-  const float wx = __fadd_rn(__fsub_rn(cx, r0.x), offx), wy = __fadd_rn(__fsub_rn(cy, r0.y), offy);
-  const float side = __fmaf_rn(r1.z, wy, -__fmul_rn(r1.w, wx));
+  const float4 f = __ldg(v.fin + bs);
+  const float wx = __fadd_rn(__fsub_rn(cx, f.x), offx), wy = __fadd_rn(__fsub_rn(cy, f.y), offy);
+  const float side = __fmaf_rn(f.z, wy, -__fmul_rn(f.w, wx));
   const float d = sqrtf(best);
   return side > 0.f ? -d : d;
 }

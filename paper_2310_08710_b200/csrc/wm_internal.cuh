@@ -54,6 +54,7 @@ struct wm_handle {
   float2* sign_dir;         // [B][seg_tiles*512]  sign direction (e, or stored dir if e == 0)
   int32_t* seg_src;         // [B][seg_tiles*512]  first-point index of each stored segment (-1: padding)
   float4* segrec;           // [B][seg_tiles*512][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}, ascending source order
+  float4* segfin;           // [B][seg_tiles*512] {p0x, p0y, sx, sy}: what the sign of the winner needs
   float4* segpair;          // [B][seg_tiles*256][3] the same records two by two, component-wise (wm_grid.cuh)
   float4* chunks;           // [B][seg_tiles*16]   bounding box of each chunk of 32 records
   WmGrid* gridp;            // [B]

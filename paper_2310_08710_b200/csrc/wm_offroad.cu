@@ -104,7 +104,7 @@ __device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir
 // One warp per group of 64 stored segments: writes the tile records (brute-force layout), the
 // 32-byte records of the grid search and their pair form, and the bounding box of each chunk of 32.
 __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, const int32_t* n_seg, float4* edges,
-                                                       float2* sign_dir, int32_t* seg_src, float4* segrec, float4* segpair, float4* chunks) {
+                                                       float2* sign_dir, int32_t* seg_src, float4* segrec, float4* segpair, float4* segfin, float4* chunks) {
   const int b = blockIdx.y, lane = threadIdx.x & 31;
   const int grp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int ngrp = seg_tiles * (WM_TILE_SEGS / 64);
@@ -136,6 +136,7 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
       float4* rec = segrec + ((int64_t)b * cap + s) * 2;
       rec[0] = make_float4(p0x, p0y, ex, ey);
       rec[1] = make_float4(gx, gy, sx, sy);
+      segfin[(int64_t)b * cap + s] = make_float4(p0x, p0y, sx, sy);
       pp[hf][0] = p0x; pp[hf][1] = p0y; pp[hf][2] = -ex; pp[hf][3] = -ey; pp[hf][4] = gx; pp[hf][5] = gy;
       ax[hf] = p0x; ay[hf] = p0y; bx[hf] = p0x + ex; by[hf] = p0y + ey;
       x0 = fminf(x0, fminf(ax[hf], bx[hf])); x1 = fmaxf(x1, fmaxf(ax[hf], bx[hf]));
@@ -145,6 +146,7 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
       float4* rec = segrec + ((int64_t)b * cap + s) * 2;
       rec[0] = make_float4(WM_FAR, WM_FAR, 0.f, 0.f);
       rec[1] = make_float4(0.f, 0.f, 1.f, 0.f);
+      segfin[(int64_t)b * cap + s] = make_float4(WM_FAR, WM_FAR, 1.f, 0.f);
       src[s] = -1;
       pp[hf][0] = WM_FAR; pp[hf][1] = WM_FAR; pp[hf][2] = 0.f; pp[hf][3] = 0.f; pp[hf][4] = 0.f; pp[hf][5] = 0.f;
     }
@@ -180,9 +182,9 @@ __global__ void __launch_bounds__(256) k_pack_points(RgView g, int pts_pad, floa
 
 void wm_prepare_free(wm_handle* h) {
   cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pts);
-  cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->chunks); cudaFree(h->gridp); cudaFree(h->cells); cudaFree(h->pool); cudaFree(h->pool_cnt);
+  cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->segfin); cudaFree(h->chunks); cudaFree(h->gridp); cudaFree(h->cells); cudaFree(h->pool); cudaFree(h->pool_cnt);
   h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pts = nullptr;
-  h->segrec = nullptr; h->segpair = nullptr; h->chunks = nullptr; h->gridp = nullptr; h->cells = nullptr; h->pool = nullptr; h->pool_cnt = nullptr;
+  h->segrec = nullptr; h->segpair = nullptr; h->segfin = nullptr; h->chunks = nullptr; h->gridp = nullptr; h->cells = nullptr; h->pool = nullptr; h->pool_cnt = nullptr;
   h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0; h->pts_pad = 0;
 }
 
@@ -219,8 +221,8 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
   if (tiles < 1) tiles = 1;
   if (tiles > h->seg_tiles || !h->edges) {       // grow only: seg_tiles is the row stride of `edges`
     wm_drop_graph(h);
-    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->chunks);
-    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->segrec = nullptr; h->segpair = nullptr; h->chunks = nullptr;
+    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->segfin); cudaFree(h->chunks);
+    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->segrec = nullptr; h->segpair = nullptr; h->segfin = nullptr; h->chunks = nullptr;
     h->seg_tiles = tiles;
     const size_t cap = (size_t)tiles * WM_TILE_SEGS;
     WM_CUDA(cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES));
@@ -228,6 +230,7 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
     WM_CUDA(cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t)));
     WM_CUDA(cudaMalloc(&h->segrec, (size_t)B * cap * 2 * sizeof(float4)));
     WM_CUDA(cudaMalloc(&h->segpair, (size_t)B * (cap / 2) * 3 * sizeof(float4)));
+    WM_CUDA(cudaMalloc(&h->segfin, (size_t)B * cap * sizeof(float4)));
     WM_CUDA(cudaMalloc(&h->chunks, (size_t)B * (cap / WM_CHUNK) * sizeof(float4)));
   }
   k_order_segments<<<B, 1024, 0, s>>>(g, h->seg_tiles * WM_TILE_SEGS, h->seg_src);
@@ -235,7 +238,7 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
   WM_CUDA(cudaGetLastError());
   {
     const int ngrp = h->seg_tiles * (WM_TILE_SEGS / 64);
-    k_fill_segments<<<dim3((ngrp + 7) / 8, B), 256, 0, s>>>(g, h->seg_tiles, h->n_seg, h->edges, h->sign_dir, h->seg_src, h->segrec, h->segpair, h->chunks);
+    k_fill_segments<<<dim3((ngrp + 7) / 8, B), 256, 0, s>>>(g, h->seg_tiles, h->n_seg, h->edges, h->sign_dir, h->seg_src, h->segrec, h->segpair, h->segfin, h->chunks);
   }
   h->launches++;
   WM_CUDA(cudaGetLastError());

@@ -56,7 +56,7 @@ struct FusedParams {
   const uint8_t* av;                  // [B][n_steps][A]
   wm_rollout_out out;                 // any pointer may be NULL
   WmDynCfg dyn;
-  const float4* segrec; const float4* segpair; const float4* chunks; const uint4* cells; const uint32_t* pool; const WmGrid* gridp;
+  const float4* segrec; const float4* segpair; const float4* segfin; const float4* chunks; const uint4* cells; const uint32_t* pool; const WmGrid* gridp;
   int seg_cap;
   unsigned long long* stats;
 };
@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
   const int64_t TA = (int64_t)p.sim.T * A;
   const int64_t sb = (int64_t)b * TA;                // scenario offset in the trajectories
   const int64_t ab = (int64_t)b * p.n_steps;         // scenario offset in the action / metric rows, in rows
-  const WmGridView gv = wm_grid_view(p.segrec, p.segpair, p.chunks, p.cells, p.pool, p.gridp, p.seg_cap, WM_POOL_CAP, b);
+  const WmGridView gv = wm_grid_view(p.segrec, p.segpair, p.segfin, p.chunks, p.cells, p.pool, p.gridp, p.seg_cap, WM_POOL_CAP, b);
 
   // ---- prologue: row t0 of the simulated trajectory -> shared memory ----
   for (int a = tid; a < Ap; a += FUSED_NT) {
@@ -372,7 +372,7 @@ cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_t
   p.S = fused_pick_S(sim.A);
   p.actions = actions; p.av = action_valid; p.out = out;
   p.dyn = WmDynCfg{h->cfg.dynamics, h->cfg.dt, h->cfg.max_accel, h->cfg.max_curvature};
-  p.segrec = h->segrec; p.segpair = h->segpair; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
+  p.segrec = h->segrec; p.segpair = h->segpair; p.segfin = h->segfin; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
   p.seg_cap = h->seg_tiles * WM_TILE_SEGS;
   p.stats = h->stats_on ? h->cull_stats : nullptr;
   const int Ap = (sim.A + 31) / 32 * 32;
