@@ -129,16 +129,29 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   const float Y0 = g.y0 + (float)(by * 4) * h - delta, Y1 = g.y0 + (float)(by * 4 + 4) * h + delta;
   const float INF = __int_as_float(0x7f800000);
 
-  // upper bound for the whole block: every cell centre has a segment within maxdist(block, chunk box)
-  float ub2 = INF;
+  // bound for the whole block: the chunk whose box is nearest to the block centre is evaluated
+  // exactly (lanes over its records); every cell centre of the block then has a segment within
+  // d_centre + (half diagonal of the block's cell centres), and no candidate of any cell lies
+  // farther than that + 2 rho from its cell centre, hence from the block box.
+  const float bcx = 0.5f * (X0 + X1), bcy = 0.5f * (Y0 + Y1);
+  float lmin = INF;
+  int cmin = 0;
   for (int c = lane; c < nch; c += 32) {
-    const float4 bb = __ldg(ch + c);
-    const float dx = fmaxf(fabsf(X1 - bb.x), fabsf(bb.z - X0)), dy = fmaxf(fabsf(Y1 - bb.y), fabsf(bb.w - Y0));
-    ub2 = fminf(ub2, fmaf(dx, dx, dy * dy));
+    const float lb2 = wm_chunk_lb2(__ldg(ch + c), bcx, bcy);
+    if (lb2 < lmin) { lmin = lb2; cmin = c; }
   }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) ub2 = fminf(ub2, __shfl_xor_sync(0xffffffffu, ub2, d));
-  const float reach = sqrtf(ub2) * 1.001f + 2.f * rho + 2e-3f;   // no candidate of any cell lies farther from the block
+  {
+    const uint32_t mm = __reduce_min_sync(0xffffffffu, __float_as_uint(lmin));
+    cmin = __shfl_sync(0xffffffffu, cmin, __ffs(__ballot_sync(0xffffffffu, __float_as_uint(lmin) == mm)) - 1);
+  }
+  float dc2 = INF;
+  {
+    const int sidx = cmin * WM_CHUNK + lane;
+    if (sidx < n) dc2 = centre_d2(__ldg(rec + 2 * sidx), __ldg(rec + 2 * sidx + 1), bcx, bcy);
+    dc2 = __uint_as_float(__reduce_min_sync(0xffffffffu, __float_as_uint(dc2)));
+  }
+  const float hdiag = 0.5f * h * 7.6157732f;                        // sqrt(7^2 + 3^2) cells between the extreme centres
+  const float reach = (sqrtf(dc2) + hdiag) * 1.001f + 2.f * rho + 4e-3f;
   const float reach2 = reach * reach;
   auto survivors = [&](int r) -> uint32_t {
     const int c = r * 32 + lane;
@@ -152,28 +165,38 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   };
   const int nround = (nch + 31) >> 5;
 
-  // pass 1: dmin(c)
+  // pass 1: dmin(c).  The block's nearest chunk first (a tight start); a chunk is evaluated only if
+  // its box can still improve some cell of the block.
   float dmin2 = INF;
+  auto pass1_chunk = [&](int c) {
+    const float lb2 = wm_chunk_lb2(__ldg(ch + c), cx, cy);
+    if (!__any_sync(0xffffffffu, lb2 < dmin2)) return;
+    const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
+#pragma unroll 4
+    for (int s = s0; s < s1; ++s) dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * s), __ldg(rec + 2 * s + 1), cx, cy));
+  };
+  if (nch > 0) pass1_chunk(cmin);
   for (int r = 0; r < nround; ++r) {
     uint32_t mask = survivors(r);
     while (mask) {
       const int c = r * 32 + __ffs(mask) - 1;
       mask &= mask - 1;
-      const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
-#pragma unroll 4
-      for (int s = s0; s < s1; ++s) dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * s), __ldg(rec + 2 * s + 1), cx, cy));
+      if (c != cmin) pass1_chunk(c);
     }
   }
-  // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack), as runs of consecutive records
+  // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack), as runs of consecutive records; chunks whose
+  // box is beyond that for every cell of the block are skipped
   const float dmin = sqrtf(dmin2);
   const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
   const float thr2 = thr * thr;
+  const float thr2c = in ? thr2 * 1.0001f + 1e-5f : -1.f;           // chunk-level test, a little wider
   int nr = 0, ncand = 0, rs = 0, rl = 0;
   for (int r = 0; r < nround; ++r) {
     uint32_t mask = survivors(r);
     while (mask) {
       const int c = r * 32 + __ffs(mask) - 1;
       mask &= mask - 1;
+      if (!__any_sync(0xffffffffu, wm_chunk_lb2(__ldg(ch + c), cx, cy) <= thr2c)) continue;
       const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
 #pragma unroll 2
       for (int s = s0; s < s1; ++s) {
