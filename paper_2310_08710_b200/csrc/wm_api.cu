@@ -335,13 +335,19 @@ extern "C" int wm_rollout_host(wm_handle* h, const wm_traj* lh, const wm_roadgra
   }
 #define H2D(dst, src, n) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyHostToDevice, s))
 #define D2H(dst, src, n) do { if (dst) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyDeviceToHost, s)); } while (0)
+  // The roadgraph goes first, on the handle's own stream, and wm_prepare runs there while the
+  // trajectories and actions (6x the bytes) are still crossing PCIe on the caller's stream.
+  // wm_prepare synchronises its stream before it returns, so what follows on `s` sees its results.
+  cudaStream_t s2 = h->cap_stream;
+#define H2D2(dst, src, n) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyHostToDevice, s2))
+  H2D2(dg.x, gh->x, nR * 4); H2D2(dg.y, gh->y, nR * 4); H2D2(dg.dir_x, gh->dir_x, nR * 4); H2D2(dg.dir_y, gh->dir_y, nR * 4);
+  H2D2(dg.type, gh->type, nR * 4); H2D2(dg.id, gh->id, nR * 4); H2D2(dg.valid, gh->valid, nR);
+#undef H2D2
   H2D(dl.x, lh->x, nTA * 4); H2D(dl.y, lh->y, nTA * 4); H2D(dl.yaw, lh->yaw, nTA * 4);
   H2D(dl.vel_x, lh->vel_x, nTA * 4); H2D(dl.vel_y, lh->vel_y, nTA * 4);
   H2D(dl.length, lh->length, nTA * 4); H2D(dl.width, lh->width, nTA * 4); H2D(dl.valid, lh->valid, nTA);
-  H2D(dg.x, gh->x, nR * 4); H2D(dg.y, gh->y, nR * 4); H2D(dg.dir_x, gh->dir_x, nR * 4); H2D(dg.dir_y, gh->dir_y, nR * 4);
-  H2D(dg.type, gh->type, nR * 4); H2D(dg.id, gh->id, nR * 4); H2D(dg.valid, gh->valid, nR);
   H2D(d_act, actions_host, rows * C * 4); H2D(d_av, action_valid_host, rows);
-  if ((rc = wm_prepare(h, &dg, nullptr, s)) != WM_OK) return rc;
+  if ((rc = wm_prepare(h, &dg, nullptr, s2)) != WM_OK) return rc;
   if ((rc = wm_reset(h, &dl, &ds, nullptr, s)) != WM_OK) return rc;
   if ((rc = wm_rollout(h, &dl, &ds, t0, n_steps, d_act, d_av, &dout, s)) != WM_OK) return rc;
   D2H(oh->overlap, dout.overlap, rows); D2H(oh->offroad, dout.offroad, rows);

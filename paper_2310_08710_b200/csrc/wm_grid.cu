@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
       g.nx = min(WM_GRID_NG, (int)ceilf(W / h)); g.ny = min(WM_GRID_NG, (int)ceilf(H / h));
     }
     gridp[b] = g;
-    pool_cnt[b] = 0;
+    pool_cnt[b] = 1;                                             // offset 0 is reserved (a header's {run, 0} means one run)
   }
 }
 
@@ -103,7 +103,7 @@ __device__ __forceinline__ bool slab_drop(const float4* __restrict__ rec, const 
 // Along a polyline this leaves the few segments whose perpendicular slab meets the cell (about
 // h/spacing + 2) instead of everything within dmin + 2 rho.
 __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* chunks, const int32_t* seg_src,
-                                                     int seg_cap, const WmGrid* gridp, uint4* cells, uint32_t* pool,
+                                                     int seg_cap, const WmGrid* gridp, uint2* cells, uint32_t* pool,
                                                      int32_t* pool_cnt) {
   __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
   const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -215,21 +215,20 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   }
   if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; }
   if (!in) return;
-  uint4 hd = make_uint4(0xffffffffu, 0xffffffffu, 0u, 0u);     // fall back to the full search
-  if (nr <= 4 && ncand <= BUILD_MAXCAND) {
+  uint2 hd = make_uint2(0xffffffffu, 0u);                      // fall back to the full search
+  if (nr <= 2 && ncand <= BUILD_MAXCAND) {
     hd.x = nr > 0 ? s_runs[warp][0][lane] : 0u;                 // nr >= 1 whenever n > 0
     hd.y = nr > 1 ? s_runs[warp][1][lane] : 0u;
-    hd.z = nr > 2 ? s_runs[warp][2][lane] : 0u;
-    hd.w = nr > 3 ? s_runs[warp][3][lane] : 0u;
   } else if (nr <= BUILD_MAXRUN && ncand <= BUILD_MAXCAND) {
-    const int off = atomicAdd(&pool_cnt[b], nr);
+    const int off = atomicAdd(&pool_cnt[b], nr);                // 1 count word + (nr - 1) runs
     if (off + nr <= WM_POOL_CAP) {
       uint32_t* pr = pool + (int64_t)b * WM_POOL_CAP + off;
-      for (int i = 0; i < nr; ++i) pr[i] = s_runs[warp][i][lane];
-      hd.y = (uint32_t)off; hd.z = (uint32_t)nr;
+      pr[0] = (uint32_t)(nr - 1);
+      for (int i = 1; i < nr; ++i) pr[i] = s_runs[warp][i][lane];
+      hd.x = s_runs[warp][0][lane]; hd.y = (uint32_t)off << 8;
     }
   }
-  cells[(int64_t)b * WM_GRID_CELLS + iy * g.nx + ix] = hd;
+  cells[(int64_t)b * WM_GRID_CELLS + wm_cell_index(ix, iy, g.nx)] = hd;
 }
 
 cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s) {
@@ -257,7 +256,7 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s) {
 struct GridParams {
   wm_row row;
   int A;
-  const float4* segrec; const float4* segpair; const float4* segfin; const float4* chunks; const uint4* cells; const uint32_t* pool; const WmGrid* gridp;
+  const float4* segrec; const float4* segpair; const float4* segfin; const float4* chunks; const uint2* cells; const uint32_t* pool; const WmGrid* gridp;
   int seg_cap;
   float* sd; int64_t sd_stride_b;
   float* corner;

@@ -21,17 +21,22 @@
 constexpr float WM_CULL_REL = 1.0005f;   // slack of the chunk cull test: lb^2 > best^2*REL + ABS
 constexpr float WM_CULL_ABS = 1e-5f;     //   (float32 rounding of 200 m-scale coordinates)
 
+// position of cell (ix, iy) in the header array: tiles of 2 x 2 cells, tile-row-major
+__host__ __device__ __forceinline__ int wm_cell_index(int ix, int iy, int nx) {
+  return (((iy >> 1) * ((nx + 1) >> 1) + (ix >> 1)) << 2) | ((iy & 1) << 1) | (ix & 1);
+}
+
 struct WmGridView {          // one scenario's prepared search structures
   const float4* rec;         // [nseg][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}
   const float4* fin;         // [nseg] {p0x, p0y, sx, sy}
   const float4* pair;        // [ceil(nseg/2)][3] records 2p (e) and 2p+1 (o): {p0x_e,p0x_o,p0y_e,p0y_o} {-ex_e,-ex_o,-ey_e,-ey_o} {gx_e,gx_o,gy_e,gy_o}
   const float4* chunks;      // [ceil(nseg/32)] bounding boxes {x0,y0,x1,y1}
-  const uint4* cells;        // [ny*nx] headers
+  const uint2* cells;        // headers, 2 x 2 tiles (wm_cell_index)
   const uint32_t* pool;      // overflow runs
   WmGrid g;
 };
 
-__device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const float4* segpair, const float4* segfin, const float4* chunks, const uint4* cells,
+__device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const float4* segpair, const float4* segfin, const float4* chunks, const uint2* cells,
                                                    const uint32_t* pool, const WmGrid* gridp, int seg_cap,
                                                    int pool_cap, int b) {
   WmGridView v;
@@ -233,7 +238,7 @@ __device__ __forceinline__ bool wm_grid_fast(const WmGridView& v, bool active, f
   best = __int_as_float(0x7f800000);
   bs = 0;
   bool slow = false;
-  uint4 hd = make_uint4(0u, 0u, 0u, 0u);
+  uint32_t r0 = 0u, r1 = 0u;
   const uint32_t* pool = v.pool;
   int n_pool = 0;
   if (active && v.g.nseg > 0) {
@@ -241,15 +246,17 @@ __device__ __forceinline__ bool wm_grid_fast(const WmGridView& v, bool active, f
     const int ix = (int)floorf(fx), iy = (int)floorf(fy);
     slow = !(fx >= 0.f && fy >= 0.f && ix < v.g.nx && iy < v.g.ny);
     if (!slow) {
-      hd = __ldg(v.cells + iy * v.g.nx + ix);
-      if (hd.x == 0xffffffffu) {
-        slow = hd.y == 0xffffffffu;
-        if (!slow) { pool += hd.y; n_pool = (int)hd.z; }
-        hd = make_uint4(0u, 0u, 0u, 0u);
+      const uint2 hd = __ldg(v.cells + wm_cell_index(ix, iy, v.g.nx));
+      r0 = hd.x; r1 = hd.y;
+      if (r0 == 0xffffffffu) { slow = true; r0 = 0u; r1 = 0u; }
+      else if (r1 != 0u && (r1 & 255u) == 0u) {                   // further runs in the pool
+        pool += r1 >> 8;
+        n_pool = (int)__ldg(pool);
+        ++pool; r1 = 0u;
       }
     }
   }
-  wm_grid_walk(v.pair, hd.x, hd.y, hd.z, hd.w, pool, n_pool, cx, cy, offx, offy, best, bs, n_eval);   // no-op without runs
+  wm_grid_walk(v.pair, r0, r1, 0u, 0u, pool, n_pool, cx, cy, offx, offy, best, bs, n_eval);   // no-op without runs
   return slow;
 }
 

@@ -26,14 +26,17 @@ constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding seg
 
 // Exact grid search (wm_grid.cuh): road-edge segments in ascending source order as 32-byte
 // records, bounding boxes per chunk of WM_CHUNK records, and a grid of at most
-// WM_GRID_NG x WM_GRID_NG cells per scenario, each with a 16-byte header:
-//   {run, run, run, run}          up to 4 inline runs, run = (first record << 8) | count, 0 = none
-//   {~0, pool offset, n runs, 0}  more runs, in the scenario's pool
-//   {~0, ~0, 0, 0}                too many candidates: search all chunks
+// WM_GRID_NG x WM_GRID_NG cells per scenario.  A cell has an 8-byte header {a, b} of runs,
+// run = (first record << 8) | count:
+//   {run, 0}                one run             {run, run}     two runs
+//   {run, pool offset << 8} more: pool[offset] = n, then n further runs (offset >= 1)
+//   {~0, 0}                 too many candidates: search all chunks
+// Headers are stored in tiles of 2 x 2 cells (one 32-byte sector = 4 m x 4 m at the default
+// cell side), tile-row-major: the four corners of a box and its next steps share sectors.
 constexpr int WM_CHUNK = 32;
 constexpr int WM_GRID_NG = 256;
 constexpr int WM_GRID_CELLS = WM_GRID_NG * WM_GRID_NG;
-constexpr int WM_POOL_CAP = WM_GRID_CELLS;       // overflow runs per scenario
+constexpr int WM_POOL_CAP = 2 * WM_GRID_CELLS;   // words of overflow runs per scenario
 struct WmGrid { float x0, y0, inv_h, h; int nx, ny, nseg, pad; };
 
 // Prepared roadgraph points for top-k: float2 (x, y) per point, invalid -> (WM_FAR, WM_FAR),
@@ -58,7 +61,7 @@ struct wm_handle {
   float4* segpair;          // [B][seg_tiles*256][3] the same records two by two, component-wise (wm_grid.cuh)
   float4* chunks;           // [B][seg_tiles*16]   bounding box of each chunk of 32 records
   WmGrid* gridp;            // [B]
-  uint4* cells;             // [B][WM_GRID_CELLS]  cell headers
+  uint2* cells;             // [B][WM_GRID_CELLS]  cell headers, 2 x 2 tiles
   uint32_t* pool;           // [B][WM_POOL_CAP]    overflow runs
   int32_t* pool_cnt;        // [B]
   int32_t pts_pad;          // padded R

@@ -200,7 +200,7 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
     h->pts_pad = (R + WM_PT_TILE - 1) / WM_PT_TILE * WM_PT_TILE;
     WM_CUDA(cudaMalloc(&h->pts, (size_t)B * h->pts_pad * sizeof(float2)));
     WM_CUDA(cudaMalloc(&h->gridp, (size_t)B * sizeof(WmGrid)));
-    WM_CUDA(cudaMalloc(&h->cells, (size_t)B * WM_GRID_CELLS * sizeof(uint4)));
+    WM_CUDA(cudaMalloc(&h->cells, (size_t)B * WM_GRID_CELLS * sizeof(uint2)));
     WM_CUDA(cudaMalloc(&h->pool, (size_t)B * WM_POOL_CAP * sizeof(uint32_t)));
     WM_CUDA(cudaMalloc(&h->pool_cnt, (size_t)B * sizeof(int32_t)));
     h->prep_B = B; h->prep_R = R;

@@ -56,7 +56,7 @@ struct FusedParams {
   const uint8_t* av;                  // [B][n_steps][A]
   wm_rollout_out out;                 // any pointer may be NULL
   WmDynCfg dyn;
-  const float4* segrec; const float4* segpair; const float4* segfin; const float4* chunks; const uint4* cells; const uint32_t* pool; const WmGrid* gridp;
+  const float4* segrec; const float4* segpair; const float4* segfin; const float4* chunks; const uint2* cells; const uint32_t* pool; const WmGrid* gridp;
   int seg_cap;
   unsigned long long* stats;
 };
