@@ -220,12 +220,11 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
     hd.x = nr > 0 ? s_runs[warp][0][lane] : 0u;                 // nr >= 1 whenever n > 0
     hd.y = nr > 1 ? s_runs[warp][1][lane] : 0u;
   } else if (nr <= BUILD_MAXRUN && ncand <= BUILD_MAXCAND) {
-    const int off = atomicAdd(&pool_cnt[b], nr);                // 1 count word + (nr - 1) runs
-    if (off + nr <= WM_POOL_CAP) {
+    const int off = atomicAdd(&pool_cnt[b], nr - 1);            // the (nr - 1) runs after the first
+    if (off + nr - 1 <= WM_POOL_CAP) {
       uint32_t* pr = pool + (int64_t)b * WM_POOL_CAP + off;
-      pr[0] = (uint32_t)(nr - 1);
-      for (int i = 1; i < nr; ++i) pr[i] = s_runs[warp][i][lane];
-      hd.x = s_runs[warp][0][lane]; hd.y = (uint32_t)off << 8;
+      for (int i = 1; i < nr; ++i) pr[i - 1] = s_runs[warp][i][lane];
+      hd.x = s_runs[warp][0][lane]; hd.y = ((uint32_t)(nr - 1) << 28) | ((uint32_t)off << 8);
     }
   }
   cells[(int64_t)b * WM_GRID_CELLS + wm_cell_index(ix, iy, g.nx)] = hd;

@@ -233,40 +233,55 @@ __device__ __forceinline__ void wm_grid_search_warp4(const WmGridView& v, float 
 // wm_grid_search_warp: above.
 // wm_grid_finish: per thread; sign from the oriented winning segment and the signed distance.
 // wm_grid_corner_sd: the three combined for a warp of corners (k_offroad_grid).
-__device__ __forceinline__ bool wm_grid_fast(const WmGridView& v, bool active, float cx, float cy, float offx, float offy,
-                                             float& best, int& bs, int& n_eval) {
-  best = __int_as_float(0x7f800000);
-  bs = 0;
-  bool slow = false;
-  uint32_t r0 = 0u, r1 = 0u;
-  const uint32_t* pool = v.pool;
-  int n_pool = 0;
+// header of the corner's cell, as the walk wants it: {0, 0} nothing to walk (inactive lane, no
+// segments), {~0, 0} the corner needs the warp search (outside the grid, crowded cell)
+__device__ __forceinline__ uint2 wm_grid_header(const WmGridView& v, bool active, float cx, float cy, float offx, float offy) {
+  uint2 hd = make_uint2(0u, 0u);
   if (active && v.g.nseg > 0) {
     const float fx = (cx + offx - v.g.x0) * v.g.inv_h, fy = (cy + offy - v.g.y0) * v.g.inv_h;
     const int ix = (int)floorf(fx), iy = (int)floorf(fy);
-    slow = !(fx >= 0.f && fy >= 0.f && ix < v.g.nx && iy < v.g.ny);
-    if (!slow) {
-      const uint2 hd = __ldg(v.cells + wm_cell_index(ix, iy, v.g.nx));
-      r0 = hd.x; r1 = hd.y;
-      if (r0 == 0xffffffffu) { slow = true; r0 = 0u; r1 = 0u; }
-      else if (r1 != 0u && (r1 & 255u) == 0u) {                   // further runs in the pool
-        pool += r1 >> 8;
-        n_pool = (int)__ldg(pool);
-        ++pool; r1 = 0u;
-      }
-    }
+    if (fx >= 0.f && fy >= 0.f && ix < v.g.nx && iy < v.g.ny) hd = __ldg(v.cells + wm_cell_index(ix, iy, v.g.nx));
+    else hd = make_uint2(0xffffffffu, 0u);
+  }
+  return hd;
+}
+
+__device__ __forceinline__ bool wm_grid_fast_hd(const WmGridView& v, uint2 hd, float cx, float cy, float offx, float offy,
+                                                float& best, int& bs, int& n_eval) {
+  best = __int_as_float(0x7f800000);
+  bs = 0;
+  uint32_t r0 = hd.x, r1 = hd.y;
+  const uint32_t* pool = v.pool;
+  int n_pool = 0;
+  const bool slow = r0 == 0xffffffffu;
+  if (slow) { r0 = 0u; r1 = 0u; }
+  else if (r1 != 0u && (r1 & 255u) == 0u) {                       // further runs in the pool
+    pool += (r1 >> 8) & 0xfffffu;
+    n_pool = (int)(r1 >> 28);
+    r1 = 0u;
   }
   wm_grid_walk(v.pair, r0, r1, 0u, 0u, pool, n_pool, cx, cy, offx, offy, best, bs, n_eval);   // no-op without runs
   return slow;
 }
 
+__device__ __forceinline__ bool wm_grid_fast(const WmGridView& v, bool active, float cx, float cy, float offx, float offy,
+                                             float& best, int& bs, int& n_eval) {
+  return wm_grid_fast_hd(v, wm_grid_header(v, active, cx, cy, offx, offy), cx, cy, offx, offy, best, bs, n_eval);
+}
+
 __device__ __forceinline__ float wm_grid_finish(const WmGridView& v, float cx, float cy, float offx, float offy, float best,
                                                 int bs) {
   if (v.g.nseg <= 0) return -FLT_MAX;                                      // D20
-  // e x (q - p0) > 0 is the left side of the oriented segment = on-road (D16)
-  const float4 f = __ldg(v.fin + bs);
-  const float wx = __fadd_rn(__fsub_rn(cx, f.x), offx), wy = __fadd_rn(__fsub_rn(cy, f.y), offy);
-  const float side = __fmaf_rn(f.z, wy, -__fmul_rn(f.w, wx));
+  // e x (q - p0) > 0 is the left side of the oriented segment = on-road (D16).  p0 and e come from
+  // the winner's pair record, which the walk has just pulled into L1 (no third dependent miss);
+  // only a zero-length segment needs its stored direction from the finish record (D16 / D29).
+  const float4 P = __ldg(v.pair + 3 * (bs >> 1)), NE = __ldg(v.pair + 3 * (bs >> 1) + 1);
+  const bool odd = (bs & 1) != 0;
+  const float p0x = odd ? P.y : P.x, p0y = odd ? P.w : P.z;
+  float sx = -(odd ? NE.y : NE.x), sy = -(odd ? NE.w : NE.z);
+  if (sx == 0.f && sy == 0.f) { const float4 f = __ldg(v.fin + bs); sx = f.z; sy = f.w; }
+  const float wx = __fadd_rn(__fsub_rn(cx, p0x), offx), wy = __fadd_rn(__fsub_rn(cy, p0y), offy);
+  const float side = __fmaf_rn(sx, wy, -__fmul_rn(sy, wx));
   const float d = sqrtf(best);
   return side > 0.f ? -d : d;
 }

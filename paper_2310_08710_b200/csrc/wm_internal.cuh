@@ -29,7 +29,7 @@ constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding seg
 // WM_GRID_NG x WM_GRID_NG cells per scenario.  A cell has an 8-byte header {a, b} of runs,
 // run = (first record << 8) | count:
 //   {run, 0}                one run             {run, run}     two runs
-//   {run, pool offset << 8} more: pool[offset] = n, then n further runs (offset >= 1)
+//   {run, n << 28 | pool offset << 8} more: n further runs at pool[offset] (offset >= 1, n <= 11)
 //   {~0, 0}                 too many candidates: search all chunks
 // Headers are stored in tiles of 2 x 2 cells (one 32-byte sector = 4 m x 4 m at the default
 // cell side), tile-row-major: the four corners of a box and its next steps share sectors.

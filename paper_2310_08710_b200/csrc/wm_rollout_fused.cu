@@ -97,9 +97,12 @@ __device__ __forceinline__ uint32_t fused_bucket(int ix, int iy, uint32_t mask) 
   return (((uint32_t)ix * 73856093u) ^ ((uint32_t)iy * 19349663u)) & mask;
 }
 
+// AP_C / S_C > 0: padded agent count and steps per block known at compile time (the shared-memory
+// carve-up then folds into immediate offsets); 0: taken from the arguments.
+template <int AP_C, int S_C>
 __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int A = p.sim.A, nb = (A + 31) / 32, Ap = nb * 32, Aps = Ap + FUSED_PAD, S = p.S;
+  const int A = p.sim.A, nb = AP_C ? AP_C / 32 : (A + 31) / 32, Ap = nb * 32, Aps = Ap + FUSED_PAD, S = S_C ? S_C : p.S;
   const int NBK = fused_nbk(Ap);
   // ---- persistent per-agent state ----
   double* s_sum = (double*)smem_raw;                 // [Ap] sum of valid log divergences (D21)
@@ -227,24 +230,41 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     __syncthreads();
     // ================= phase B: warp tasks =================
     const int n_ctask = Ap / apt, n_task = n_ctask + nb;             // the nb overlap tasks first: they are the long ones
-    for (;;) {
-      int task = 0;
-      if (lane == 0) task = atomicAdd(&s_task, 1);
-      task = __shfl_sync(0xffffffffu, task, 0);
-      if (task >= n_task) break;
+    // a corner task's lane: agent slot q, validity, centre, half extents, corner offset
+    auto corner = [&](int task, int& q, bool& v, float& cx, float& cy, float& hl, float& hw, float& offx, float& offy) {
+      const int a = (task - nb) * apt + la;
+      q = ls * Aps + a;
+      v = ls < Sb && pvalid[q] != 0;
+      cx = px[q]; cy = py[q]; hl = phl[q]; hw = phw[q];
+      float ax, ay, bx, by;
+      wm_box_offsets_h(ps[q], pc[q], hl, hw, ax, ay, bx, by);
+      const float ox = (kk & 1) ? bx : ax, oy = (kk & 1) ? by : ay;
+      offx = (kk & 2) ? -ox : ox; offy = (kk & 2) ? -oy : oy;
+    };
+    // the cell header of a task's corner is requested one task ahead: its miss overlaps the walk
+    auto header = [&](int task) {
+      if (task < nb || task >= n_task) return make_uint2(0u, 0u);
+      int q; bool v; float cx, cy, hl, hw, offx, offy;
+      corner(task, q, v, cx, cy, hl, hw, offx, offy);
+      return wm_grid_header(gv, v, cx, cy, offx, offy);
+    };
+    auto grab = [&]() {
+      int t = 0;
+      if (lane == 0) t = atomicAdd(&s_task, 1);
+      return __shfl_sync(0xffffffffu, t, 0);
+    };
+    int task = grab();
+    uint2 hd = header(task);
+    while (task < n_task) {
+      const int task_next = grab();
+      const uint2 hd_next = header(task_next);
       if (task >= nb) {
         // ---- the 4 corners of one agent (8 / S agents) at every step of the block (a4) ----
-        const int a = (task - nb) * apt + la;
-        const int q = ls * Aps + a;
-        const bool v = ls < Sb && pvalid[q] != 0;
-        if (!__any_sync(0xffffffffu, v)) continue;                      // psd of invalid slots is never read
-        const float cx = px[q], cy = py[q], hl = phl[q], hw = phw[q];
-        float ax, ay, bx, by;
-        wm_box_offsets_h(ps[q], pc[q], hl, hw, ax, ay, bx, by);
-        const float ox = (kk & 1) ? bx : ax, oy = (kk & 1) ? by : ay;
-        const float offx = (kk & 2) ? -ox : ox, offy = (kk & 2) ? -oy : oy;
+        int q; bool v; float cx, cy, hl, hw, offx, offy;
+        corner(task, q, v, cx, cy, hl, hw, offx, offy);
+        if (__any_sync(0xffffffffu, v)) {                               // psd of invalid slots is never read
         float best; int bs;
-        const bool slow = wm_grid_fast(gv, v, cx, cy, offx, offy, best, bs, n_eval);
+        const bool slow = wm_grid_fast_hd(gv, hd, cx, cy, offx, offy, best, bs, n_eval);
         n_slow += slow; n_corner += v;
         uint32_t todo = __ballot_sync(0xffffffffu, slow);
         while (todo) {                                  // boxes with corners off the grid / in a crowded cell
@@ -268,6 +288,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));               // D18: max over the 4 corners
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
         if (kk == 0 && v) psd[q] = m;
+        }
       } else {
         // ---- overlap flags of 32 agents at every step of the block (a3) ----
         // broad phase, one lane per agent i: the pairs (i, j > i) whose block boxes meet go to the
@@ -322,6 +343,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
           if (s < Sb) narrow((int)(pr >> 16), (int)(pr & 0xffffu), s);
         }
       }
+      task = task_next; hd = hd_next;
     }
     __syncthreads();
     // ================= phase C: metric rows of the block (D18, D19, D10) =================
@@ -379,12 +401,14 @@ cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_t
   const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)(fused_persist_bytes(1024) + fused_slot_bytes(1024)));
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  k_rollout_fused<<<sim.B, FUSED_NT, smem, s>>>(p);
+  if (Ap == 128 && p.S == 8) k_rollout_fused<128, 8><<<sim.B, FUSED_NT, smem, s>>>(p);
+  else if (Ap == 32 && p.S == 8) k_rollout_fused<32, 8><<<sim.B, FUSED_NT, smem, s>>>(p);
+  else k_rollout_fused<0, 0><<<sim.B, FUSED_NT, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
 }
