@@ -42,6 +42,13 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
   if (major != 10) { free(h); return WM_ERR_UNSUPPORTED; }    // sm_100a kernels only; no fallback
   e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->roll_stream, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->d2h_stream, cudaStreamNonBlocking);
+  for (int i = 0; i < WM_HOST_CHUNKS && e == cudaSuccess; ++i) {
+    e = cudaEventCreateWithFlags(&h->ev_up[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_prep[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming);
+  }
   if (e == cudaSuccess) e = cudaMalloc(&h->cull_stats, 4 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMemset(h->cull_stats, 0, 4 * sizeof(unsigned long long));
   if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
@@ -83,6 +90,13 @@ extern "C" int wm_destroy(wm_handle* h) {
   cudaFree(h->cull_stats);
   for (int i = 0; i < 16; ++i) cudaFree(h->stage[i]);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (h->roll_stream) cudaStreamDestroy(h->roll_stream);
+  if (h->d2h_stream) cudaStreamDestroy(h->d2h_stream);
+  for (int i = 0; i < WM_HOST_CHUNKS; ++i) {
+    if (h->ev_up[i]) cudaEventDestroy(h->ev_up[i]);
+    if (h->ev_prep[i]) cudaEventDestroy(h->ev_prep[i]);
+    if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
+  }
   free(h);
   return WM_OK;
 }
@@ -246,7 +260,7 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
     const int64_t before = h->launches;
     WM_CUDA(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
     if (fused) {
-      cudaError_t le = wm_launch_rollout_fused(h, *log, *sim, t0, n_steps, actions, action_valid, o, h->cap_stream);
+      cudaError_t le = wm_launch_rollout_fused(h, *log, *sim, t0, n_steps, actions, action_valid, o, 0, h->cap_stream);
       rc = WM_OK;
       if (le != cudaSuccess) { g_wm_last_cuda_error = (int)le; rc = WM_ERR_CUDA; }
     } else {
@@ -334,33 +348,69 @@ extern "C" int wm_rollout_host(wm_handle* h, const wm_traj* lh, const wm_roadgra
     dout.ade = (float*)p;
   }
 #define H2D(dst, src, n) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyHostToDevice, s))
-#define D2H(dst, src, n) do { if (dst) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyDeviceToHost, s)); } while (0)
-  // The roadgraph goes first, on the handle's own stream, and wm_prepare runs there while the
-  // trajectories and actions (6x the bytes) are still crossing PCIe on the caller's stream.
-  // wm_prepare synchronises its stream before it returns, so what follows on `s` sees its results.
-  cudaStream_t s2 = h->cap_stream;
-#define H2D2(dst, src, n) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyHostToDevice, s2))
-  H2D2(dg.x, gh->x, nR * 4); H2D2(dg.y, gh->y, nR * 4); H2D2(dg.dir_x, gh->dir_x, nR * 4); H2D2(dg.dir_y, gh->dir_y, nR * 4);
-  H2D2(dg.type, gh->type, nR * 4); H2D2(dg.id, gh->id, nR * 4); H2D2(dg.valid, gh->valid, nR);
-#undef H2D2
-  H2D(dl.x, lh->x, nTA * 4); H2D(dl.y, lh->y, nTA * 4); H2D(dl.yaw, lh->yaw, nTA * 4);
-  H2D(dl.vel_x, lh->vel_x, nTA * 4); H2D(dl.vel_y, lh->vel_y, nTA * 4);
-  H2D(dl.length, lh->length, nTA * 4); H2D(dl.width, lh->width, nTA * 4); H2D(dl.valid, lh->valid, nTA);
-  H2D(d_act, actions_host, rows * C * 4); H2D(d_av, action_valid_host, rows);
-  if ((rc = wm_prepare(h, &dg, nullptr, s2)) != WM_OK) return rc;
-  if ((rc = wm_reset(h, &dl, &ds, nullptr, s)) != WM_OK) return rc;
-  if ((rc = wm_rollout(h, &dl, &ds, t0, n_steps, d_act, d_av, &dout, s)) != WM_OK) return rc;
-  D2H(oh->overlap, dout.overlap, rows); D2H(oh->offroad, dout.offroad, rows);
-  D2H(oh->offroad_dist, dout.offroad_dist, rows * 4); D2H(oh->log_div, dout.log_div, rows * 4);
-  D2H(oh->any_overlap, dout.any_overlap, nBA); D2H(oh->any_offroad, dout.any_offroad, nBA);
-  D2H(oh->ade, dout.ade, nBA * 4);
-  if (sim_host) {
-    D2H(sim_host->x, ds.x, nTA * 4); D2H(sim_host->y, ds.y, nTA * 4); D2H(sim_host->yaw, ds.yaw, nTA * 4);
-    D2H(sim_host->vel_x, ds.vel_x, nTA * 4); D2H(sim_host->vel_y, ds.vel_y, nTA * 4);
-    D2H(sim_host->length, ds.length, nTA * 4); D2H(sim_host->width, ds.width, nTA * 4); D2H(sim_host->valid, ds.valid, nTA);
+#define D2H(dst, src, n) do { if (dst) WM_CUDA(cudaMemcpyAsync((dst), (src), (n), cudaMemcpyDeviceToHost, s3)); } while (0)
+  // Pipeline over chunks of scenarios (they are independent, L82).  All uploads go down the caller's
+  // stream in this order: the roadgraph's type / id / valid of the whole batch (what the record
+  // count needs, which fixes the buffer capacity), then chunk by chunk the rest of the roadgraph,
+  // the logged trajectories and the actions.  While chunk c + 1 crosses PCIe, chunk c is prepared
+  // (cap_stream), rolled out (roll_stream) and its metric rows go back (d2h_stream).
+  cudaStream_t s2 = h->cap_stream, s4 = h->roll_stream, s3 = h->d2h_stream;
+  H2D(dg.type, gh->type, nR * 4); H2D(dg.id, gh->id, nR * 4); H2D(dg.valid, gh->valid, nR);
+  if ((rc = wm_prepare_count(h, &dg, nullptr, s)) != WM_OK) return rc;          // synchronises s
+  const bool fused = h->cfg.rollout_mode == WM_ROLLOUT_FUSED && h->cfg.offroad_mode == WM_OFFROAD_CULLED && n_steps < 60000;
+  int nchunk = fused ? (B + 255) / 256 : 1;
+  if (nchunk > WM_HOST_CHUNKS) nchunk = WM_HOST_CHUNKS;
+  const int per = (B + nchunk - 1) / nchunk;
+  for (int c = 0; c < nchunk; ++c) {
+    const int b0 = c * per, nb = (b0 + per <= B ? per : B - b0);
+    if (nb <= 0) break;
+    const size_t oR = (size_t)b0 * R, cR = (size_t)nb * R, oT = (size_t)b0 * T * A, cT = (size_t)nb * T * A;
+    const size_t oW = (size_t)b0 * n_steps * A, cW = (size_t)nb * n_steps * A, oA = (size_t)b0 * A, cA = (size_t)nb * A;
+    H2D(dg.x + oR, gh->x + oR, cR * 4); H2D(dg.y + oR, gh->y + oR, cR * 4);
+    H2D(dg.dir_x + oR, gh->dir_x + oR, cR * 4); H2D(dg.dir_y + oR, gh->dir_y + oR, cR * 4);
+    H2D(dl.x + oT, lh->x + oT, cT * 4); H2D(dl.y + oT, lh->y + oT, cT * 4); H2D(dl.yaw + oT, lh->yaw + oT, cT * 4);
+    H2D(dl.vel_x + oT, lh->vel_x + oT, cT * 4); H2D(dl.vel_y + oT, lh->vel_y + oT, cT * 4);
+    H2D(dl.length + oT, lh->length + oT, cT * 4); H2D(dl.width + oT, lh->width + oT, cT * 4); H2D(dl.valid + oT, lh->valid + oT, cT);
+    H2D(d_act + oW * C, actions_host + oW * C, cW * C * 4); H2D(d_av + oW, action_valid_host + oW, cW);
+    WM_CUDA(cudaEventRecord(h->ev_up[c], s));
+    WM_CUDA(cudaStreamWaitEvent(s2, h->ev_up[c], 0));
+    if ((rc = wm_prepare_build(h, &dg, b0, nb, s2)) != WM_OK) return rc;
+    WM_CUDA(cudaEventRecord(h->ev_prep[c], s2));
+    WM_CUDA(cudaStreamWaitEvent(s4, h->ev_prep[c], 0));
+    wm_traj cl = dl, cs = ds;
+    cl.B = nb; cs.B = nb;
+    cl.x += oT; cl.y += oT; cl.yaw += oT; cl.vel_x += oT; cl.vel_y += oT; cl.length += oT; cl.width += oT; cl.valid += oT;
+    cs.x += oT; cs.y += oT; cs.yaw += oT; cs.vel_x += oT; cs.vel_y += oT; cs.length += oT; cs.width += oT; cs.valid += oT;
+    wm_rollout_out co = dout;
+    co.overlap += oW; co.offroad += oW; co.offroad_dist += oW; co.log_div += oW;
+    co.any_overlap += oA; co.any_offroad += oA; co.ade += oA;
+    WM_CUDA(wm_launch_reset(h, cl, cs, h->cfg.history, s4));
+    if (fused) {
+      WM_CUDA(wm_launch_rollout_fused(h, cl, cs, t0, n_steps, d_act + oW * C, d_av + oW, co, b0, s4));
+    } else {
+      // stepwise / brute-force modes: one chunk = the whole batch, through the graph path
+      WM_CUDA(cudaStreamSynchronize(s4));
+      if ((rc = wm_rollout(h, &dl, &ds, t0, n_steps, d_act, d_av, &dout, s4)) != WM_OK) return rc;
+    }
+    WM_CUDA(cudaEventRecord(h->ev_done[c], s4));
+    WM_CUDA(cudaStreamWaitEvent(s3, h->ev_done[c], 0));
+    D2H(oh->overlap ? oh->overlap + oW : nullptr, co.overlap, cW); D2H(oh->offroad ? oh->offroad + oW : nullptr, co.offroad, cW);
+    D2H(oh->offroad_dist ? oh->offroad_dist + oW : nullptr, co.offroad_dist, cW * 4);
+    D2H(oh->log_div ? oh->log_div + oW : nullptr, co.log_div, cW * 4);
+    D2H(oh->any_overlap ? oh->any_overlap + oA : nullptr, co.any_overlap, cA);
+    D2H(oh->any_offroad ? oh->any_offroad + oA : nullptr, co.any_offroad, cA);
+    D2H(oh->ade ? oh->ade + oA : nullptr, co.ade, cA * 4);
+    if (sim_host) {
+      D2H(sim_host->x + oT, cs.x, cT * 4); D2H(sim_host->y + oT, cs.y, cT * 4); D2H(sim_host->yaw + oT, cs.yaw, cT * 4);
+      D2H(sim_host->vel_x + oT, cs.vel_x, cT * 4); D2H(sim_host->vel_y + oT, cs.vel_y, cT * 4);
+      D2H(sim_host->length + oT, cs.length, cT * 4); D2H(sim_host->width + oT, cs.width, cT * 4); D2H(sim_host->valid + oT, cs.valid, cT);
+    }
   }
 #undef H2D
 #undef D2H
+  WM_CUDA(cudaStreamSynchronize(s3));
+  WM_CUDA(cudaStreamSynchronize(s4));
+  WM_CUDA(cudaStreamSynchronize(s2));
   WM_CUDA(cudaStreamSynchronize(s));
   return WM_OK;
 }

@@ -19,7 +19,7 @@ constexpr int BUILD_MAXRUN = 12;          // runs per cell before the cell falls
 constexpr int BUILD_MAXCAND = 256;        // candidates per cell before it falls back
 
 __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const float4* chunks, int seg_cap, float h_min,
-                                                     float margin, WmGrid* gridp, int32_t* pool_cnt) {
+                                                     float margin_in, float margin, WmGrid* gridp, int32_t* pool_cnt) {
   __shared__ float s_red[4][4];
   const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n = n_seg[b], nch = (n + WM_CHUNK - 1) / WM_CHUNK;
@@ -41,13 +41,22 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
       x0 = fminf(x0, s_red[0][w]); y0 = fminf(y0, s_red[1][w]); x1 = fmaxf(x1, s_red[2][w]); y1 = fmaxf(y1, s_red[3][w]);
     }
     WmGrid g;
-    g.nseg = n; g.pad = 0;
-    if (n <= 0) { g.x0 = 0.f; g.y0 = 0.f; g.h = h_min; g.inv_h = 1.f / h_min; g.nx = 0; g.ny = 0; }
-    else {
-      const float W = (x1 - x0) + 2.f * margin, H = (y1 - y0) + 2.f * margin;
-      const float h = fmaxf(h_min, fmaxf(W, H) * (1.0001f / WM_GRID_NG));
-      g.x0 = x0 - margin; g.y0 = y0 - margin; g.h = h; g.inv_h = 1.f / h;
-      g.nx = min(WM_GRID_NG, (int)ceilf(W / h)); g.ny = min(WM_GRID_NG, (int)ceilf(H / h));
+    g.nseg = n; g.pad0 = 0; g.pad1 = 0;
+    if (n <= 0) {
+      g.x0 = 0.f; g.y0 = 0.f; g.h = h_min; g.inv_h = 1.f / h_min; g.nx = 0; g.ny = 0; g.obase = 0;
+      g.ox0 = 0.f; g.oy0 = 0.f; g.oh = 4.f * h_min; g.oinv_h = 1.f / g.oh; g.onx = 0; g.ony = 0;
+    } else {
+      // inner: the segments' bounding box + margin_in, cell side >= h_min
+      float W = (x1 - x0) + 2.f * margin_in, H = (y1 - y0) + 2.f * margin_in;
+      float h = fmaxf(h_min, fmaxf(W, H) * (1.0001f / WM_GRID_NG_IN));
+      g.x0 = x0 - margin_in; g.y0 = y0 - margin_in; g.h = h; g.inv_h = 1.f / h;
+      g.nx = min(WM_GRID_NG_IN, (int)ceilf(W / h)); g.ny = min(WM_GRID_NG_IN, (int)ceilf(H / h));
+      g.obase = 4 * ((g.nx + 1) >> 1) * ((g.ny + 1) >> 1);
+      // outer: the bounding box + margin, cell side >= 4 inner sides
+      W = (x1 - x0) + 2.f * margin; H = (y1 - y0) + 2.f * margin;
+      const float oh = fmaxf(4.f * h, fmaxf(W, H) * (1.0001f / WM_GRID_NG_OUT));
+      g.ox0 = x0 - margin; g.oy0 = y0 - margin; g.oh = oh; g.oinv_h = 1.f / oh;
+      g.onx = min(WM_GRID_NG_OUT, (int)ceilf(W / oh)); g.ony = min(WM_GRID_NG_OUT, (int)ceilf(H / oh));
     }
     gridp[b] = g;
     pool_cnt[b] = 1;                                             // offset 0 is reserved (a header's {run, 0} means one run)
@@ -108,25 +117,38 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
   const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const WmGrid g = gridp[b];
-  const int nbx = (g.nx + 7) >> 3, nby = (g.ny + 3) >> 2;
-  const int wg = blockIdx.x * 8 + warp;
+  // the warp's block of 8 x 4 cells: inner grid first, then the outer grid
+  int wg = blockIdx.x * 8 + warp;
+  const int nbx_in = (g.nx + 7) >> 3, nby_in = (g.ny + 3) >> 2;
+  const bool outer = wg >= nbx_in * nby_in;
+  if (outer) wg -= nbx_in * nby_in;
+  const int gnx = outer ? g.onx : g.nx, gny = outer ? g.ony : g.ny;
+  const float gx0 = outer ? g.ox0 : g.x0, gy0 = outer ? g.oy0 : g.y0, h = outer ? g.oh : g.h;
+  const int nbx = (gnx + 7) >> 3, nby = (gny + 3) >> 2;
   if (wg >= nbx * nby) return;                                  // warp-uniform
   const int bx = wg % nbx, by = wg / nbx;
   const int ix = bx * 8 + (lane & 7), iy = by * 4 + (lane >> 3);
-  const bool in = ix < g.nx && iy < g.ny;
   const float4* rec = segrec + (int64_t)b * seg_cap * 2;
   const float4* ch = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
   const int32_t* src = seg_src + (int64_t)b * seg_cap;
   const int n = g.nseg, nch = (n + WM_CHUNK - 1) / WM_CHUNK;
-  const float h = g.h;
-  const float cx = g.x0 + ((float)ix + 0.5f) * h, cy = g.y0 + ((float)iy + 0.5f) * h;
+  const float cx = gx0 + ((float)ix + 0.5f) * h, cy = gy0 + ((float)iy + 0.5f) * h;
   // cell box inflated by delta (float32 rounding of the query's cell index), half diagonal rho
   const float delta = 1e-3f + 1e-4f * h;
   const float hh = 0.5f * h + delta;
   const float rho = 1.41421362f * hh;
+  bool in = ix < gnx && iy < gny;
+  if (outer) {
+    // an outer cell whose inflated box lies inside the inner grid (shrunk by a safety inset) is
+    // never queried: the query takes the inner grid there
+    const float inset = 0.05f;
+    const float ax0 = g.x0 + inset, ay0 = g.y0 + inset, ax1 = g.x0 + (float)g.nx * g.h - inset, ay1 = g.y0 + (float)g.ny * g.h - inset;
+    if (cx - hh >= ax0 && cx + hh <= ax1 && cy - hh >= ay0 && cy + hh <= ay1) in = false;
+    if (!__any_sync(0xffffffffu, in)) return;
+  }
   // block box
-  const float X0 = g.x0 + (float)(bx * 8) * h - delta, X1 = g.x0 + (float)(bx * 8 + 8) * h + delta;
-  const float Y0 = g.y0 + (float)(by * 4) * h - delta, Y1 = g.y0 + (float)(by * 4 + 4) * h + delta;
+  const float X0 = gx0 + (float)(bx * 8) * h - delta, X1 = gx0 + (float)(bx * 8 + 8) * h + delta;
+  const float Y0 = gy0 + (float)(by * 4) * h - delta, Y1 = gy0 + (float)(by * 4 + 4) * h + delta;
   const float INF = __int_as_float(0x7f800000);
 
   // bound for the whole block: the chunk whose box is nearest to the block centre is evaluated
@@ -165,50 +187,53 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   };
   const int nround = (nch + 31) >> 5;
 
-  // pass 1: dmin(c).  The block's nearest chunk first (a tight start); a chunk is evaluated only if
-  // its box can still improve some cell of the block.
   float dmin2 = INF;
-  auto pass1_chunk = [&](int c) {
-    const float lb2 = wm_chunk_lb2(__ldg(ch + c), cx, cy);
-    if (!__any_sync(0xffffffffu, lb2 < dmin2)) return;
-    const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
-#pragma unroll 4
-    for (int s = s0; s < s1; ++s) dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * s), __ldg(rec + 2 * s + 1), cx, cy));
-  };
-  if (nch > 0) pass1_chunk(cmin);
-  for (int r = 0; r < nround; ++r) {
-    uint32_t mask = survivors(r);
-    while (mask) {
-      const int c = r * 32 + __ffs(mask) - 1;
-      mask &= mask - 1;
-      if (c != cmin) pass1_chunk(c);
-    }
-  }
-  // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack), as runs of consecutive records; chunks whose
-  // box is beyond that for every cell of the block are skipped
-  const float dmin = sqrtf(dmin2);
-  const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
-  const float thr2 = thr * thr;
-  const float thr2c = in ? thr2 * 1.0001f + 1e-5f : -1.f;           // chunk-level test, a little wider
   int nr = 0, ncand = 0, rs = 0, rl = 0;
-  for (int r = 0; r < nround; ++r) {
-    uint32_t mask = survivors(r);
-    while (mask) {
-      const int c = r * 32 + __ffs(mask) - 1;
-      mask &= mask - 1;
-      if (!__any_sync(0xffffffffu, wm_chunk_lb2(__ldg(ch + c), cx, cy) <= thr2c)) continue;
+  auto candidate = [&](int sx, const float4 q0, const float4 q1, float d2, float thr2) {
+    if (in && d2 <= thr2 && !slab_drop(rec, src, sx, n, q0, q1, cx, cy, hh)) {
+      ++ncand;
+      if (rl > 0 && sx == rs + rl && rl < 255) ++rl;
+      else {
+        if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; }
+        rs = sx; rl = 1;
+      }
+    }
+  };
+  {
+    // pass 1: dmin(c).  The block's nearest chunk first (a tight start); a chunk is evaluated only
+    // if its box can still improve some cell of the block.
+    auto pass1_chunk = [&](int c) {
+      const float lb2 = wm_chunk_lb2(__ldg(ch + c), cx, cy);
+      if (!__any_sync(0xffffffffu, lb2 < dmin2)) return;
       const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
+#pragma unroll 4
+      for (int sx = s0; sx < s1; ++sx) dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * sx), __ldg(rec + 2 * sx + 1), cx, cy));
+    };
+    if (nch > 0) pass1_chunk(cmin);
+    for (int r = 0; r < nround; ++r) {
+      uint32_t mask = survivors(r);
+      while (mask) {
+        const int c = r * 32 + __ffs(mask) - 1;
+        mask &= mask - 1;
+        if (c != cmin) pass1_chunk(c);
+      }
+    }
+    // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack), as runs of consecutive records; chunks whose box is beyond the threshold for every cell of the block are skipped
+    const float dmin = sqrtf(dmin2);
+    const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
+    const float thr2 = thr * thr;
+    const float thr2c = in ? thr2 * 1.0001f + 1e-5f : -1.f;         // chunk-level test, a little wider
+    for (int r = 0; r < nround; ++r) {
+      uint32_t mask = survivors(r);
+      while (mask) {
+        const int c = r * 32 + __ffs(mask) - 1;
+        mask &= mask - 1;
+        if (!__any_sync(0xffffffffu, wm_chunk_lb2(__ldg(ch + c), cx, cy) <= thr2c)) continue;
+        const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
 #pragma unroll 2
-      for (int s = s0; s < s1; ++s) {
-        const float4 q0 = __ldg(rec + 2 * s), q1 = __ldg(rec + 2 * s + 1);
-        const float d2 = centre_d2(q0, q1, cx, cy);
-        if (in && d2 <= thr2 && !slab_drop(rec, src, s, n, q0, q1, cx, cy, hh)) {
-          ++ncand;
-          if (rl > 0 && s == rs + rl && rl < 255) ++rl;
-          else {
-            if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; }
-            rs = s; rl = 1;
-          }
+        for (int sx = s0; sx < s1; ++sx) {
+          const float4 q0 = __ldg(rec + 2 * sx), q1 = __ldg(rec + 2 * sx + 1);
+          candidate(sx, q0, q1, centre_d2(q0, q1, cx, cy), thr2);
         }
       }
     }
@@ -227,24 +252,28 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
       hd.x = s_runs[warp][0][lane]; hd.y = ((uint32_t)(nr - 1) << 28) | ((uint32_t)off << 8);
     }
   }
-  cells[(int64_t)b * WM_GRID_CELLS + wm_cell_index(ix, iy, g.nx)] = hd;
+  cells[(int64_t)b * WM_GRID_CELLS + (outer ? g.obase : 0) + wm_cell_index(ix, iy, gnx)] = hd;
 }
 
-cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s) {
+cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
   // cell side (lower bound) and metres of grid beyond the segments' bounding box; the cell side grows
   // when (bounding box + 2 margin) does not fit WM_GRID_NG cells
-  static float h_min = 0.f, margin = 0.f;
+  static float h_min = 0.f, margin = 0.f, margin_in = 0.f;
   if (h_min <= 0.f) {
     const char* e = getenv("WM_GRID_CELL"); h_min = e ? (float)atof(e) : 2.0f; if (!(h_min >= 0.25f && h_min <= 64.f)) h_min = 2.0f;
     e = getenv("WM_GRID_MARGIN"); margin = e ? (float)atof(e) : 120.f; if (!(margin >= 1.f && margin <= 4096.f)) margin = 120.f;
+    e = getenv("WM_GRID_MARGIN_IN"); margin_in = e ? (float)atof(e) : 8.f; if (!(margin_in >= 0.5f && margin_in <= margin)) margin_in = fminf(8.f, margin);
   }
   const int seg_cap = h->seg_tiles * WM_TILE_SEGS;
-  k_grid_params<<<B, 128, 0, s>>>(h->n_seg, h->chunks, seg_cap, h_min, margin, h->gridp, h->pool_cnt);
+  const float4* segrec = h->segrec + (int64_t)b0 * seg_cap * 2;
+  const float4* chunks = h->chunks + (int64_t)b0 * (seg_cap / WM_CHUNK);
+  k_grid_params<<<B, 128, 0, s>>>(h->n_seg + b0, chunks, seg_cap, h_min, margin_in, margin, h->gridp + b0, h->pool_cnt + b0);
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const int nwarps = (WM_GRID_NG / 8) * (WM_GRID_NG / 4);
-  k_build_cells<<<dim3(nwarps / 8, B), 256, 0, s>>>(h->segrec, h->chunks, h->seg_src, seg_cap, h->gridp, h->cells, h->pool, h->pool_cnt);
+  const int nwarps = (WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) + (WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4);
+  k_build_cells<<<dim3((nwarps + 7) / 8, B), 256, 0, s>>>(segrec, chunks, h->seg_src + (int64_t)b0 * seg_cap, seg_cap, h->gridp + b0,
+                                                          h->cells + (int64_t)b0 * WM_GRID_CELLS, h->pool + (int64_t)b0 * WM_POOL_CAP, h->pool_cnt + b0);
   h->launches++;
   return cudaGetLastError();
 }

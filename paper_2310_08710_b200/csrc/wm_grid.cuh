@@ -238,10 +238,16 @@ __device__ __forceinline__ void wm_grid_search_warp4(const WmGridView& v, float 
 __device__ __forceinline__ uint2 wm_grid_header(const WmGridView& v, bool active, float cx, float cy, float offx, float offy) {
   uint2 hd = make_uint2(0u, 0u);
   if (active && v.g.nseg > 0) {
-    const float fx = (cx + offx - v.g.x0) * v.g.inv_h, fy = (cy + offy - v.g.y0) * v.g.inv_h;
+    const float qx = cx + offx, qy = cy + offy;
+    const float fx = (qx - v.g.x0) * v.g.inv_h, fy = (qy - v.g.y0) * v.g.inv_h;
     const int ix = (int)floorf(fx), iy = (int)floorf(fy);
     if (fx >= 0.f && fy >= 0.f && ix < v.g.nx && iy < v.g.ny) hd = __ldg(v.cells + wm_cell_index(ix, iy, v.g.nx));
-    else hd = make_uint2(0xffffffffu, 0u);
+    else {                                                        // off the inner grid: the coarse outer one
+      const float gx = (qx - v.g.ox0) * v.g.oinv_h, gy = (qy - v.g.oy0) * v.g.oinv_h;
+      const int jx = (int)floorf(gx), jy = (int)floorf(gy);
+      if (gx >= 0.f && gy >= 0.f && jx < v.g.onx && jy < v.g.ony) hd = __ldg(v.cells + v.g.obase + wm_cell_index(jx, jy, v.g.onx));
+      else hd = make_uint2(0xffffffffu, 0u);
+    }
   }
   return hd;
 }

@@ -25,23 +25,33 @@ constexpr int WM_TILE_BYTES = WM_TILE_F4 * 16;   // 12288
 constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding segments
 
 // Exact grid search (wm_grid.cuh): road-edge segments in ascending source order as 32-byte
-// records, bounding boxes per chunk of WM_CHUNK records, and a grid of at most
-// WM_GRID_NG x WM_GRID_NG cells per scenario.  A cell has an 8-byte header {a, b} of runs,
-// run = (first record << 8) | count:
+// records, bounding boxes per chunk of WM_CHUNK records, and TWO nested grids of square cells per
+// scenario: a fine inner grid (<= WM_GRID_NG_IN^2 cells, side >= 2 m) over the segments' bounding
+// box plus a small margin, where nearly all queries land, and a coarse outer grid
+// (<= WM_GRID_NG_OUT^2 cells, side >= 4 x the inner side) over the wide margin that agents reach
+// when they drive off the map.  Outer cells wholly inside the inner grid are never queried and
+// not built.  A cell has an 8-byte header {a, b} of runs, run = (first record << 8) | count:
 //   {run, 0}                one run             {run, run}     two runs
 //   {run, n << 28 | pool offset << 8} more: n further runs at pool[offset] (offset >= 1, n <= 11)
 //   {~0, 0}                 too many candidates: search all chunks
 // Headers are stored in tiles of 2 x 2 cells (one 32-byte sector = 4 m x 4 m at the default
-// cell side), tile-row-major: the four corners of a box and its next steps share sectors.
+// inner cell side), tile-row-major: the four corners of a box and its next steps share sectors.
+// The outer grid's headers follow the inner grid's at cell offset WmGrid::obase.
 constexpr int WM_CHUNK = 32;
-constexpr int WM_GRID_NG = 256;
-constexpr int WM_GRID_CELLS = WM_GRID_NG * WM_GRID_NG;
+constexpr int WM_GRID_NG_IN = 160;
+constexpr int WM_GRID_NG_OUT = 64;
+constexpr int WM_GRID_CELLS = WM_GRID_NG_IN * WM_GRID_NG_IN + WM_GRID_NG_OUT * WM_GRID_NG_OUT;
 constexpr int WM_POOL_CAP = 2 * WM_GRID_CELLS;   // words of overflow runs per scenario
-struct WmGrid { float x0, y0, inv_h, h; int nx, ny, nseg, pad; };
+struct WmGrid {
+  float x0, y0, inv_h, h; int nx, ny, nseg, obase;        // inner grid; obase = first outer header
+  float ox0, oy0, oinv_h, oh; int onx, ony, pad0, pad1;   // outer grid
+};
 
 // Prepared roadgraph points for top-k: float2 (x, y) per point, invalid -> (WM_FAR, WM_FAR),
 // padded to a multiple of WM_PT_TILE.
 constexpr int WM_PT_TILE = 2048;
+
+constexpr int WM_HOST_CHUNKS = 16;          // scenario chunks of the pipelined host path
 
 struct wm_handle {
   wm_config cfg;
@@ -66,8 +76,9 @@ struct wm_handle {
   int32_t* pool_cnt;        // [B]
   int32_t pts_pad;          // padded R
   float2* pts;              // [B][pts_pad]
-  // rollout graph cache
-  cudaStream_t cap_stream;
+  // rollout graph cache; streams and events of the pipelined host path (wm_rollout_host)
+  cudaStream_t cap_stream, roll_stream, d2h_stream;
+  cudaEvent_t ev_up[WM_HOST_CHUNKS], ev_prep[WM_HOST_CHUNKS], ev_done[WM_HOST_CHUNKS];
   cudaGraph_t graph;
   cudaGraphExec_t graph_exec;
   int64_t graph_kernels;
@@ -129,11 +140,14 @@ cudaError_t wm_launch_offroad_grid(wm_handle* h, const wm_traj& sim, int t, floa
                                      float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
 cudaError_t wm_launch_aggregate(wm_handle* h, int B, int A, int n_steps, const wm_rollout_out& out,
                                 const uint8_t* ld_valid_rows, cudaStream_t s);
-cudaError_t wm_launch_build_grid(wm_handle* h, int B, cudaStream_t s);
+cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s);   // scenarios [b0, b0 + B)
+// log / sim / actions / out are views of scenarios [b0, b0 + sim.B) of the prepared batch
 cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
                                     const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
-                                    cudaStream_t s);
+                                    int b0, cudaStream_t s);
 int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);
+int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);   // needs type, id, valid; syncs s
+int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaStream_t s);            // scenarios [b0, b0 + nb), no sync
 void wm_prepare_free(wm_handle* h);
 void wm_drop_graph(wm_handle* h);
 cudaError_t wm_launch_observe_hist(wm_handle* h, const wm_traj& sim, int t, float* hist, uint8_t* hist_valid, cudaStream_t s);

@@ -188,7 +188,9 @@ void wm_prepare_free(wm_handle* h) {
   h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0; h->pts_pad = 0;
 }
 
-int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s) {
+// Step 1 of wm_prepare: per-scenario record counts (needs type, id, valid only), the capacity they
+// call for, and the buffers.  Synchronises `s` once (the counts come back to the host).
+int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s) {
   const int B = rg->B, R = rg->R;
   RgView g{rg->x, rg->y, rg->dir_x, rg->dir_y, rg->type, rg->id, rg->valid, R};
   // Buffers are reused when the shapes fit, so device pointers (and a captured rollout graph)
@@ -233,21 +235,43 @@ int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_ma
     WM_CUDA(cudaMalloc(&h->segfin, (size_t)B * cap * sizeof(float4)));
     WM_CUDA(cudaMalloc(&h->chunks, (size_t)B * (cap / WM_CHUNK) * sizeof(float4)));
   }
-  k_order_segments<<<B, 1024, 0, s>>>(g, h->seg_tiles * WM_TILE_SEGS, h->seg_src);
+  if (n_segments_max) *n_segments_max = mx;
+  return WM_OK;
+}
+
+// Step 2: the prepared structures of scenarios [b0, b0 + nb) (records, grid, packed points), enqueued
+// on `s`; no synchronisation.  rg holds the device pointers of the whole batch.
+int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaStream_t s) {
+  const int R = rg->R;
+  const int64_t o = (int64_t)b0 * R;
+  RgView g{rg->x + o, rg->y + o, rg->dir_x + o, rg->dir_y + o, rg->type + o, rg->id + o, rg->valid + o, R};
+  const int tiles = h->seg_tiles;
+  const int64_t cap = (int64_t)tiles * WM_TILE_SEGS;
+  int32_t* seg_src = h->seg_src + b0 * cap;
+  k_order_segments<<<nb, 1024, 0, s>>>(g, (int)cap, seg_src);
   h->launches++;
   WM_CUDA(cudaGetLastError());
   {
-    const int ngrp = h->seg_tiles * (WM_TILE_SEGS / 64);
-    k_fill_segments<<<dim3((ngrp + 7) / 8, B), 256, 0, s>>>(g, h->seg_tiles, h->n_seg, h->edges, h->sign_dir, h->seg_src, h->segrec, h->segpair, h->segfin, h->chunks);
+    const int ngrp = tiles * (WM_TILE_SEGS / 64);
+    k_fill_segments<<<dim3((ngrp + 7) / 8, nb), 256, 0, s>>>(g, tiles, h->n_seg + b0, h->edges + (int64_t)b0 * tiles * WM_TILE_F4,
+                                                             h->sign_dir + b0 * cap, seg_src, h->segrec + b0 * cap * 2,
+                                                             h->segpair + b0 * (cap / 2) * 3, h->segfin + b0 * cap,
+                                                             h->chunks + b0 * (cap / WM_CHUNK));
   }
   h->launches++;
   WM_CUDA(cudaGetLastError());
-  WM_CUDA(wm_launch_build_grid(h, B, s));
-  k_pack_points<<<dim3((h->pts_pad + 255) / 256, B), 256, 0, s>>>(g, h->pts_pad, h->pts);
+  WM_CUDA(wm_launch_build_grid(h, b0, nb, s));
+  k_pack_points<<<dim3((h->pts_pad + 255) / 256, nb), 256, 0, s>>>(g, h->pts_pad, h->pts + (int64_t)b0 * h->pts_pad);
   h->launches++;
   WM_CUDA(cudaGetLastError());
+  return WM_OK;
+}
+
+int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s) {
+  int rc = wm_prepare_count(h, rg, n_segments_max, s);
+  if (rc != WM_OK) return rc;
+  if ((rc = wm_prepare_build(h, rg, 0, rg->B, s)) != WM_OK) return rc;
   WM_CUDA(cudaStreamSynchronize(s));
-  if (n_segments_max) *n_segments_max = mx;
   return WM_OK;
 }
 

@@ -387,15 +387,18 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
 
 cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
                                     const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
-                                    cudaStream_t s) {
+                                    int b0, cudaStream_t s) {
   FusedParams p;
   p.log = log; p.sim = sim; p.t0 = t0; p.n_steps = n_steps;
   p.C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   p.S = fused_pick_S(sim.A);
   p.actions = actions; p.av = action_valid; p.out = out;
   p.dyn = WmDynCfg{h->cfg.dynamics, h->cfg.dt, h->cfg.max_accel, h->cfg.max_curvature};
-  p.segrec = h->segrec; p.segpair = h->segpair; p.segfin = h->segfin; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
   p.seg_cap = h->seg_tiles * WM_TILE_SEGS;
+  const int64_t cap = p.seg_cap;
+  p.segrec = h->segrec + b0 * cap * 2; p.segpair = h->segpair + b0 * (cap / 2) * 3; p.segfin = h->segfin + b0 * cap;
+  p.chunks = h->chunks + b0 * (cap / WM_CHUNK); p.cells = h->cells + (int64_t)b0 * WM_GRID_CELLS;
+  p.pool = h->pool + (int64_t)b0 * WM_POOL_CAP; p.gridp = h->gridp + b0;
   p.stats = h->stats_on ? h->cull_stats : nullptr;
   const int Ap = (sim.A + 31) / 32 * 32;
   const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
