@@ -15,7 +15,7 @@
 // ======================================================================================
 // grid construction (wm_prepare)
 // ======================================================================================
-constexpr int BUILD_MAXRUN = 12;          // runs per cell before the cell falls back to the full search
+constexpr int BUILD_MAXRUN = 16;          // runs per cell before the cell falls back to the full search
 constexpr int BUILD_MAXCAND = 256;        // candidates per cell before it falls back
 
 __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const float4* chunks, int seg_cap, float h_min,
@@ -41,22 +41,28 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
       x0 = fminf(x0, s_red[0][w]); y0 = fminf(y0, s_red[1][w]); x1 = fmaxf(x1, s_red[2][w]); y1 = fmaxf(y1, s_red[3][w]);
     }
     WmGrid g;
-    g.nseg = n; g.pad0 = 0; g.pad1 = 0;
+    g.nseg = n; g.icx0 = 0; g.icy0 = 0;
     if (n <= 0) {
       g.x0 = 0.f; g.y0 = 0.f; g.h = h_min; g.inv_h = 1.f / h_min; g.nx = 0; g.ny = 0; g.obase = 0;
       g.ox0 = 0.f; g.oy0 = 0.f; g.oh = 4.f * h_min; g.oinv_h = 1.f / g.oh; g.onx = 0; g.ony = 0;
     } else {
-      // inner: the segments' bounding box + margin_in, cell side >= h_min
-      float W = (x1 - x0) + 2.f * margin_in, H = (y1 - y0) + 2.f * margin_in;
-      float h = fmaxf(h_min, fmaxf(W, H) * (1.0001f / WM_GRID_NG_IN));
-      g.x0 = x0 - margin_in; g.y0 = y0 - margin_in; g.h = h; g.inv_h = 1.f / h;
-      g.nx = min(WM_GRID_NG_IN, (int)ceilf(W / h)); g.ny = min(WM_GRID_NG_IN, (int)ceilf(H / h));
-      g.obase = 4 * ((g.nx + 1) >> 1) * ((g.ny + 1) >> 1);
-      // outer: the bounding box + margin, cell side >= 4 inner sides
-      W = (x1 - x0) + 2.f * margin; H = (y1 - y0) + 2.f * margin;
-      const float oh = fmaxf(4.f * h, fmaxf(W, H) * (1.0001f / WM_GRID_NG_OUT));
+      // outer: the bounding box + margin; its cell side is 4 inner sides, and at most
+      // WM_GRID_NG_IN / 4 of its cells per axis lie under the inner grid
+      const float W = (x1 - x0) + 2.f * margin, H = (y1 - y0) + 2.f * margin;
+      const float Wi = (x1 - x0) + 2.f * margin_in, Hi = (y1 - y0) + 2.f * margin_in;
+      const float oh = fmaxf(4.f * h_min, fmaxf(fmaxf(W, H) * (1.0001f / WM_GRID_NG_OUT),
+                                                fmaxf(Wi, Hi) * (1.0001f / (WM_GRID_NG_IN / 4 - 1))));
       g.ox0 = x0 - margin; g.oy0 = y0 - margin; g.oh = oh; g.oinv_h = 1.f / oh;
       g.onx = min(WM_GRID_NG_OUT, (int)ceilf(W / oh)); g.ony = min(WM_GRID_NG_OUT, (int)ceilf(H / oh));
+      // inner: the outer cells that meet the bounding box + margin_in, each split 4 x 4
+      const int cx0 = max(0, (int)floorf((x0 - margin_in - g.ox0) / oh)), cy0 = max(0, (int)floorf((y0 - margin_in - g.oy0) / oh));
+      int cx1 = min(g.onx, (int)ceilf((x1 + margin_in - g.ox0) / oh)), cy1 = min(g.ony, (int)ceilf((y1 + margin_in - g.oy0) / oh));
+      cx1 = min(cx1, cx0 + WM_GRID_NG_IN / 4); cy1 = min(cy1, cy0 + WM_GRID_NG_IN / 4);
+      g.icx0 = cx0; g.icy0 = cy0;
+      g.h = 0.25f * oh; g.inv_h = 1.f / g.h;
+      g.x0 = g.ox0 + (float)cx0 * oh; g.y0 = g.oy0 + (float)cy0 * oh;
+      g.nx = 4 * (cx1 - cx0); g.ny = 4 * (cy1 - cy0);
+      g.obase = 4 * ((g.nx + 1) >> 1) * ((g.ny + 1) >> 1);
     }
     gridp[b] = g;
     pool_cnt[b] = 1;                                             // offset 0 is reserved (a header's {run, 0} means one run)
@@ -111,19 +117,17 @@ __device__ __forceinline__ bool slab_drop(const float4* __restrict__ rec, const 
 //      that same stored point: then d(q, s+1) < |q - p1| = d(q, s).
 // Along a polyline this leaves the few segments whose perpendicular slab meets the cell (about
 // h/spacing + 2) instead of everything within dmin + 2 rho.
+template <bool FINE>
 __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* chunks, const int32_t* seg_src,
                                                      int seg_cap, const WmGrid* gridp, uint2* cells, uint32_t* pool,
                                                      int32_t* pool_cnt) {
   __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
   const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const WmGrid g = gridp[b];
-  // the warp's block of 8 x 4 cells: inner grid first, then the outer grid
-  int wg = blockIdx.x * 8 + warp;
-  const int nbx_in = (g.nx + 7) >> 3, nby_in = (g.ny + 3) >> 2;
-  const bool outer = wg >= nbx_in * nby_in;
-  if (outer) wg -= nbx_in * nby_in;
-  const int gnx = outer ? g.onx : g.nx, gny = outer ? g.ony : g.ny;
-  const float gx0 = outer ? g.ox0 : g.x0, gy0 = outer ? g.oy0 : g.y0, h = outer ? g.oh : g.h;
+  // the warp's block of 8 x 4 cells of the outer (FINE = false) or the inner grid
+  const int wg = blockIdx.x * 8 + warp;
+  const int gnx = FINE ? g.nx : g.onx, gny = FINE ? g.ny : g.ony;
+  const float gx0 = FINE ? g.x0 : g.ox0, gy0 = FINE ? g.y0 : g.oy0, h = FINE ? g.h : g.oh;
   const int nbx = (gnx + 7) >> 3, nby = (gny + 3) >> 2;
   if (wg >= nbx * nby) return;                                  // warp-uniform
   const int bx = wg % nbx, by = wg / nbx;
@@ -131,25 +135,65 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   const float4* rec = segrec + (int64_t)b * seg_cap * 2;
   const float4* ch = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
   const int32_t* src = seg_src + (int64_t)b * seg_cap;
+  uint2* cells_b = cells + (int64_t)b * WM_GRID_CELLS;
+  uint32_t* pool_b = pool + (int64_t)b * WM_POOL_CAP;
   const int n = g.nseg, nch = (n + WM_CHUNK - 1) / WM_CHUNK;
   const float cx = gx0 + ((float)ix + 0.5f) * h, cy = gy0 + ((float)iy + 0.5f) * h;
   // cell box inflated by delta (float32 rounding of the query's cell index), half diagonal rho
   const float delta = 1e-3f + 1e-4f * h;
   const float hh = 0.5f * h + delta;
   const float rho = 1.41421362f * hh;
-  bool in = ix < gnx && iy < gny;
-  if (outer) {
-    // an outer cell whose inflated box lies inside the inner grid (shrunk by a safety inset) is
-    // never queried: the query takes the inner grid there
-    const float inset = 0.05f;
-    const float ax0 = g.x0 + inset, ay0 = g.y0 + inset, ax1 = g.x0 + (float)g.nx * g.h - inset, ay1 = g.y0 + (float)g.ny * g.h - inset;
-    if (cx - hh >= ax0 && cx + hh <= ax1 && cy - hh >= ay0 && cy + hh <= ay1) in = false;
-    if (!__any_sync(0xffffffffu, in)) return;
+  const bool in = ix < gnx && iy < gny;
+  const float INF = __int_as_float(0x7f800000);
+
+  float dmin2 = INF;
+  int nr = 0, ncand = 0, rs = 0, rl = 0;
+  auto flush_run = [&]() { if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; } };
+  auto candidate = [&](int sx, const float4 q0, const float4 q1, float d2, float thr2) {
+    if (in && d2 <= thr2 && !slab_drop(rec, src, sx, n, q0, q1, cx, cy, hh)) {
+      ++ncand;
+      if (rl > 0 && sx == rs + rl && rl < 255) ++rl;
+      else { flush_run(); rs = sx; rl = 1; }
+    }
+  };
+  bool done = false;
+  if (FINE) {
+    // Inner cell: its inflated box lies inside its parent's (the outer cell above it, 4 x 4 inner
+    // cells), so every segment that is the reported nearest one of a point of this cell is in the
+    // parent's list, and so is the nearest segment of the cell centre: both passes walk the
+    // parent's runs (a few dozen records) instead of the surviving chunks.  A crowded parent
+    // (no list) sends the warp down the chunk-wise path.
+    uint2 ph = make_uint2(0u, 0u);
+    if (in) ph = cells_b[g.obase + wm_cell_index(g.icx0 + (ix >> 2), g.icy0 + (iy >> 2), g.onx)];
+    if (!__any_sync(0xffffffffu, ph.x == 0xffffffffu)) {
+      auto walk = [&](auto&& f) {
+        uint32_t r = ph.x, r1 = ph.y;
+        const uint32_t* pl = pool_b;
+        int np = 0;
+        if (r1 != 0u && (r1 & 255u) == 0u) { pl += (r1 >> 8) & 0xfffffu; np = (int)(r1 >> 28); r1 = 0u; }
+        while (r != 0u) {
+          const int s0 = (int)(r >> 8), s1 = s0 + (int)(r & 255u);
+          for (int sx = s0; sx < s1; ++sx) f(sx);
+          if (r1 != 0u) { r = r1; r1 = 0u; }
+          else if (np > 0) { r = *pl++; --np; }
+          else r = 0u;
+        }
+      };
+      walk([&](int sx) { dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * sx), __ldg(rec + 2 * sx + 1), cx, cy)); });
+      const float dmin = sqrtf(dmin2);
+      const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
+      const float thr2 = thr * thr;
+      walk([&](int sx) {
+        const float4 q0 = __ldg(rec + 2 * sx), q1 = __ldg(rec + 2 * sx + 1);
+        candidate(sx, q0, q1, centre_d2(q0, q1, cx, cy), thr2);
+      });
+      done = true;
+    }
   }
+  if (!done) {
   // block box
   const float X0 = gx0 + (float)(bx * 8) * h - delta, X1 = gx0 + (float)(bx * 8 + 8) * h + delta;
   const float Y0 = gy0 + (float)(by * 4) * h - delta, Y1 = gy0 + (float)(by * 4 + 4) * h + delta;
-  const float INF = __int_as_float(0x7f800000);
 
   // bound for the whole block: the chunk whose box is nearest to the block centre is evaluated
   // exactly (lanes over its records); every cell centre of the block then has a segment within
@@ -187,18 +231,6 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   };
   const int nround = (nch + 31) >> 5;
 
-  float dmin2 = INF;
-  int nr = 0, ncand = 0, rs = 0, rl = 0;
-  auto candidate = [&](int sx, const float4 q0, const float4 q1, float d2, float thr2) {
-    if (in && d2 <= thr2 && !slab_drop(rec, src, sx, n, q0, q1, cx, cy, hh)) {
-      ++ncand;
-      if (rl > 0 && sx == rs + rl && rl < 255) ++rl;
-      else {
-        if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; }
-        rs = sx; rl = 1;
-      }
-    }
-  };
   {
     // pass 1: dmin(c).  The block's nearest chunk first (a tight start); a chunk is evaluated only
     // if its box can still improve some cell of the block.
@@ -238,7 +270,8 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
       }
     }
   }
-  if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; }
+  }
+  flush_run();
   if (!in) return;
   uint2 hd = make_uint2(0xffffffffu, 0u);                      // fall back to the full search
   if (nr <= 2 && ncand <= BUILD_MAXCAND) {
@@ -247,12 +280,12 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   } else if (nr <= BUILD_MAXRUN && ncand <= BUILD_MAXCAND) {
     const int off = atomicAdd(&pool_cnt[b], nr - 1);            // the (nr - 1) runs after the first
     if (off + nr - 1 <= WM_POOL_CAP) {
-      uint32_t* pr = pool + (int64_t)b * WM_POOL_CAP + off;
+      uint32_t* pr = pool_b + off;
       for (int i = 1; i < nr; ++i) pr[i - 1] = s_runs[warp][i][lane];
       hd.x = s_runs[warp][0][lane]; hd.y = ((uint32_t)(nr - 1) << 28) | ((uint32_t)off << 8);
     }
   }
-  cells[(int64_t)b * WM_GRID_CELLS + (outer ? g.obase : 0) + wm_cell_index(ix, iy, gnx)] = hd;
+  cells_b[(FINE ? 0 : g.obase) + wm_cell_index(ix, iy, gnx)] = hd;
 }
 
 cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
@@ -271,9 +304,15 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const int nwarps = (WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) + (WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4);
-  k_build_cells<<<dim3((nwarps + 7) / 8, B), 256, 0, s>>>(segrec, chunks, h->seg_src + (int64_t)b0 * seg_cap, seg_cap, h->gridp + b0,
-                                                          h->cells + (int64_t)b0 * WM_GRID_CELLS, h->pool + (int64_t)b0 * WM_POOL_CAP, h->pool_cnt + b0);
+  const int32_t* src = h->seg_src + (int64_t)b0 * seg_cap;
+  uint2* cells = h->cells + (int64_t)b0 * WM_GRID_CELLS;
+  uint32_t* pool = h->pool + (int64_t)b0 * WM_POOL_CAP;
+  // the outer grid first: its cells are the parents the inner cells build from
+  k_build_cells<false><<<dim3((WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4) / 8, B), 256, 0, s>>>(segrec, chunks, src, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  h->launches++;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_build_cells<true><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / 8, B), 256, 0, s>>>(segrec, chunks, src, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   return cudaGetLastError();
 }

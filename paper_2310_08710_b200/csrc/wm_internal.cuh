@@ -29,10 +29,11 @@ constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding seg
 // scenario: a fine inner grid (<= WM_GRID_NG_IN^2 cells, side >= 2 m) over the segments' bounding
 // box plus a small margin, where nearly all queries land, and a coarse outer grid
 // (<= WM_GRID_NG_OUT^2 cells, side >= 4 x the inner side) over the wide margin that agents reach
-// when they drive off the map.  Outer cells wholly inside the inner grid are never queried and
-// not built.  A cell has an 8-byte header {a, b} of runs, run = (first record << 8) | count:
+// when they drive off the map.  The inner grid is aligned with the outer one: an outer cell under
+// it is the PARENT of 4 x 4 inner cells, and wm_prepare builds an inner cell's candidates from its
+// parent's list instead of from all segments (wm_grid.cu).  A cell has an 8-byte header {a, b} of runs, run = (first record << 8) | count:
 //   {run, 0}                one run             {run, run}     two runs
-//   {run, n << 28 | pool offset << 8} more: n further runs at pool[offset] (offset >= 1, n <= 11)
+//   {run, n << 28 | pool offset << 8} more: n further runs at pool[offset] (offset >= 1, n <= 15)
 //   {~0, 0}                 too many candidates: search all chunks
 // Headers are stored in tiles of 2 x 2 cells (one 32-byte sector = 4 m x 4 m at the default
 // inner cell side), tile-row-major: the four corners of a box and its next steps share sectors.
@@ -44,7 +45,7 @@ constexpr int WM_GRID_CELLS = WM_GRID_NG_IN * WM_GRID_NG_IN + WM_GRID_NG_OUT * W
 constexpr int WM_POOL_CAP = 2 * WM_GRID_CELLS;   // words of overflow runs per scenario
 struct WmGrid {
   float x0, y0, inv_h, h; int nx, ny, nseg, obase;        // inner grid; obase = first outer header
-  float ox0, oy0, oinv_h, oh; int onx, ony, pad0, pad1;   // outer grid
+  float ox0, oy0, oinv_h, oh; int onx, ony, icx0, icy0;   // outer grid; the inner grid starts at its cell (icx0, icy0)
 };
 
 // Prepared roadgraph points for top-k: float2 (x, y) per point, invalid -> (WM_FAR, WM_FAR),

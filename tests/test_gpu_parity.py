@@ -315,3 +315,30 @@ def test_rollout_host_matches_device_rollout(cfg1):
     for k, v in host(sim_d).items():
         assert np.array_equal(v, sim_h[k].numpy(), equal_nan=True), k
     wm.wm_destroy(h); wm.wm_destroy(h2)
+
+
+def test_rollout_host_pipelined_chunks_match_device_rollout():
+    """wm_rollout_host splits B > 256 scenarios into chunks (upload / prepare / rollout / download
+    pipelined); every chunk must reproduce the device-resident rollout bit for bit, ragged last chunk."""
+    n = 12
+    cfg = ws.make_config(1, b_ids=np.arange(700), n_steps=n)
+    log, rg = cfg["log"], cfg["roadgraph"]
+    B, T, A = log["x"].shape
+    h, log_d, rg_d, sim_d, _ = _setup(cfg)
+    t0 = wm.wm_reset(h, log_d, sim_d)
+    acts = np.ascontiguousarray(cfg["actions"][:, :n]); av = np.ascontiguousarray(cfg["action_valid"][:, :n])
+    out_d = wm.alloc_rollout_out(B, n, A)
+    wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out_d)
+    torch.cuda.synchronize()
+    h2 = wm.wm_create()
+    pin = lambda d: {k: torch.from_numpy(v).pin_memory() for k, v in d.items()}
+    out_h = wm.alloc_rollout_out(B, n, A, device="cpu", pin=True)
+    sim_h = {k: torch.zeros_like(v).pin_memory() for k, v in pin(log).items()}
+    wm.wm_rollout_host(h2, pin(log), pin(rg), n, torch.from_numpy(acts).pin_memory(),
+                       torch.from_numpy(av).pin_memory(), out_h, sim_h)
+    for k, v in host(out_d).items():
+        assert np.array_equal(v, out_h[k].numpy()), k
+    for k, v in host(sim_d).items():
+        assert np.array_equal(v, sim_h[k].numpy(), equal_nan=True), k
+    assert out_h["offroad"].numpy().sum() > 0
+    wm.wm_destroy(h); wm.wm_destroy(h2)
