@@ -13,9 +13,10 @@ not; valid-agent-steps reported beside it).
 value     device-resident: inputs in HBM when the timed region starts, CUDA events on the
           launching stream, barrier + synchronize on both sides, max over ranks.
 e2e       the same job through wm_rollout_host with pinned HOST buffers: scenario + action
-          upload, wm_prepare, reset, rollout, metric download all inside the timed region.
+          upload, wm_prepare, reset, rollout, metric download all inside the timed region
+          (pipelined over scenario chunks: its floor is the PCIe time of the 3.8 GB upload).
 roofline  dominant kernel k_rollout_fused (the whole rollout is one launch of it).  The exact grid
-          search leaves ~0.2 % of the corner-segment pairs, so the slower roof of the kernel is its
+          search leaves < 0.1 % of the corner-segment pairs, so the slower roof of the kernel is its
           compulsory HBM IO (actions + log row in, sim row + metric rows out, per agent-step):
           achieved = those bytes / CUDA-event duration of the launch, against the measured HBM peak;
           the FP32 fractions on evaluated pairs and on the brute-force pair count are beside it.
@@ -288,6 +289,7 @@ def main():
                     help="rollout = the BASELINE metric (config 5, default); the others time the remaining "
                          "SURVEY 8(a) rows on configs 3, 2, 4 (supplementary lines, same JSON shape)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (single-step grid kernel, brute-force kernel)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     args.steps_ref = max(1, min(args.steps, 3)); args.warmup_ref = max(1, min(args.warmup, 1))
@@ -376,10 +378,9 @@ def main():
         return ka.elapsed_time(kb) / 5
 
     kf_ms = time_rollout()
-    k_ms = time_offroad(h)                                     # the single-step kernel of the same search
+    # pair counters of the search, from one more rollout with the kernel's counters switched on
     wm.wm_offroad_stats_enable(h, True); wm.wm_offroad_stats(h)
-    for t in range(11, 11 + N_STEPS):
-        wm.wm_metrics_offroad(h, sim_d, t, sd, None, fl)
+    wm.wm_rollout(h, log_d, sim_d, 10, N_STEPS, acts_d, av_d, out_d)
     ev_pairs, bf_pairs, n_slow, n_corner = wm.wm_offroad_stats(h)
     wm.wm_offroad_stats_enable(h, False)
     pairs_eval = ev_pairs / float(N_STEPS)
@@ -409,23 +410,29 @@ def main():
                 "slow_path_corner_fraction": n_slow / max(n_corner, 1),
                 "alu_frac_on_evaluated_pairs": fused_flops / (kf_ms * 1e-3) / 1e12 / fp32_peak,
                 "alu_frac_bruteforce_equivalent": pairs_per_launch * N_STEPS * FLOP_PER_PAIR / (kf_ms * 1e-3) / 1e12 / fp32_peak,
-                "note": "exact culling (SURVEY 8(d)) leaves 0.2 % of the pairs, so the slower roof of the kernel is its "
-                        "compulsory HBM IO; the FP32 fractions on evaluated pairs and on the brute-force count are beside it"}
+                "note": "exact culling (SURVEY 8(d)) leaves under 0.1 % of the pairs, so the slower roof of the kernel is its "
+                        "compulsory HBM IO; the FP32 fractions on evaluated pairs and on the brute-force count are beside it. "
+                        "ncu: the kernel is bound by gather latency and instruction issue, not by HBM bandwidth (profiles/)"}
     hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 29.0 + B * A * 5.0    # brute force: segments once + one state row + outputs
-    roofline_grid = {"bound": "hbm", "kernel": "k_offroad_grid (wm_metrics_offroad, one step)", "kernel_ms": k_ms,
-                     "algorithmic_bytes_per_launch": B * A * 34.0, "note": "single-step entry point of the same search"}
-    hb = wm.wm_create(offroad_mode=wm.WM_OFFROAD_BRUTE_FORCE)  # the FP32-roofline reference kernel
-    wm.wm_prepare(hb, rg_d)
-    kb_ms = time_offroad(hb)
-    wm.wm_destroy(hb)
-    bf_achieved = pairs_per_launch * FLOP_PER_PAIR / (kb_ms * 1e-3) / 1e12
-    roofline_bf = {"bound": "alu", "achieved": bf_achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                   "frac": bf_achieved / fp32_peak, "traffic": profiled_traffic("k_offroad_brute"),
-                   "kernel": "k_offroad (offroad_mode=WM_OFFROAD_BRUTE_FORCE)", "kernel_ms": kb_ms,
-                   "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR, "peak_source": peak_src}
     rl_ms = max(pairs_per_launch * FLOP_PER_PAIR / (fp32_peak * 1e12), hbm_bytes / (hbm_peak * 1e9)) * 1e3
     step_roofline = {"definition": "north_star: slower of algorithmic bytes/HBM peak and brute-force FP32 flops/FP32 peak, per simulated step",
                      "roofline_ms": rl_ms, "achieved_ms": ms_step / N_STEPS, "frac": rl_ms / (ms_step / N_STEPS)}
+    roofline_grid = roofline_bf = None
+    if not args.no_extras:
+        # side measurements, outside the timed region: the single-step entry point of the same search,
+        # and the brute-force kernel (every corner against every segment) against the FP32 peak
+        k_ms = time_offroad(h)
+        roofline_grid = {"bound": "hbm", "kernel": "k_offroad_grid (wm_metrics_offroad, one step)", "kernel_ms": k_ms,
+                         "algorithmic_bytes_per_launch": B * A * 34.0, "note": "single-step entry point of the same search"}
+        hb = wm.wm_create(offroad_mode=wm.WM_OFFROAD_BRUTE_FORCE)
+        wm.wm_prepare(hb, rg_d)
+        kb_ms = time_offroad(hb)
+        wm.wm_destroy(hb)
+        bf_achieved = pairs_per_launch * FLOP_PER_PAIR / (kb_ms * 1e-3) / 1e12
+        roofline_bf = {"bound": "alu", "achieved": bf_achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+                       "frac": bf_achieved / fp32_peak, "traffic": profiled_traffic("k_offroad_brute"),
+                       "kernel": "k_offroad (offroad_mode=WM_OFFROAD_BRUTE_FORCE)", "kernel_ms": kb_ms,
+                       "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR, "peak_source": peak_src}
     clocks = sampler.stop() if rank == 0 else None
 
     # ---- e2e: the same job from pinned host buffers through the C-ABI ----
@@ -451,7 +458,7 @@ def main():
         same = all(torch.equal(out_h[k], out_d[k].cpu()) for k in out_h)
         e2e = {"value": agent_steps / (e_ms * 1e-3), "unit": "agent-steps/s", "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms, "outputs_equal_device_path": bool(same),
-               "includes": "scenario+action upload, wm_prepare, reset, 80-step graph, metric download"}
+               "includes": "scenario+action upload, wm_prepare, reset, 80-step rollout, metric download; pipelined over 16 scenario chunks"}
         wm.wm_destroy(h2)
 
     # ---- cpu_baseline: the oracle on a bounded sample (rank 0, N=1 only) ----

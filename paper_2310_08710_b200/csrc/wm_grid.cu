@@ -1,13 +1,17 @@
 // a4 off-road metric, exact grid search — the default mode (WM_OFFROAD_CULLED).
 // See wm_grid.cuh for the structure and the argument why no nearest segment can be missed.
 //
-//   k_grid_params  per scenario: bounding box of the segments -> grid origin, cell side, nx, ny
-//   k_build_cells  per cell: dmin(c), then the runs of records with dist(c, s) <= dmin + 2 rho
-//   k_offroad_grid one thread per box corner, 4 lanes per agent: header load, candidate walk,
-//                  sign of the winner; max over the corners by shuffles
+//   k_grid_params        per scenario: bounding box of the segments -> the outer grid (box + wide margin,
+//                        coarse cells) and, aligned with it, the inner grid (box + small margin, each
+//                        outer cell under it split into 4 x 4)
+//   k_build_cells<false> per outer cell: dmin(c), then the runs of records with dist(c, s) <= dmin + 2 rho,
+//                        from the chunks whose boxes can matter (one warp per 8 x 4 cells)
+//   k_build_cells<true>  per inner cell: the same two passes over its PARENT's list only
+//   k_offroad_grid       one thread per box corner, 4 lanes per agent: header load, candidate walk,
+//                        sign of the winner; max over the corners by shuffles
 //
-// Bound of k_offroad_grid: instruction issue (about 18 instructions per evaluated pair, ~25
-// pairs per corner) and L1/L2 gather latency; HBM traffic is the touched 32-byte records only.
+// Bound of k_offroad_grid: instruction issue (about 14 instructions per evaluated pair, ~7 pairs
+// per corner) and L1/L2 gather latency; HBM traffic is the touched 32-byte sectors only.
 #include <stdlib.h>
 
 #include "wm_grid.cuh"
@@ -104,9 +108,10 @@ __device__ __forceinline__ bool slab_drop(const float4* __restrict__ rec, const 
   return false;
 }
 
-// One warp per block of 8 x 4 cells, one lane per cell.  Chunks that cannot hold a candidate of
-// any cell of the block are dropped with one box-box test per chunk (lanes over chunks); the
-// survivors are walked twice with lanes over cells: dmin(c), then the candidate runs.
+// One warp per block of 8 x 4 cells, one lane per cell.  Outer cells (and inner cells under a
+// crowded parent): chunks that cannot hold a candidate of any cell of the block are dropped with one
+// box-box test per chunk (lanes over chunks); the survivors are walked twice with lanes over cells:
+// dmin(c), then the candidate runs.  Inner cells: both passes walk the parent's runs.
 //
 // A record that passes the distance test is still dropped when it can never be the REPORTED
 // nearest segment of any point of the cell (exact in real arithmetic, tested on the four corners
@@ -289,13 +294,13 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
 }
 
 cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
-  // cell side (lower bound) and metres of grid beyond the segments' bounding box; the cell side grows
-  // when (bounding box + 2 margin) does not fit WM_GRID_NG cells
+  // inner cell side (lower bound), metres of outer / inner grid beyond the segments' bounding box; the
+  // cell sides grow when the boxes do not fit WM_GRID_NG_OUT / WM_GRID_NG_IN cells
   static float h_min = 0.f, margin = 0.f, margin_in = 0.f;
   if (h_min <= 0.f) {
     const char* e = getenv("WM_GRID_CELL"); h_min = e ? (float)atof(e) : 2.0f; if (!(h_min >= 0.25f && h_min <= 64.f)) h_min = 2.0f;
     e = getenv("WM_GRID_MARGIN"); margin = e ? (float)atof(e) : 120.f; if (!(margin >= 1.f && margin <= 4096.f)) margin = 120.f;
-    e = getenv("WM_GRID_MARGIN_IN"); margin_in = e ? (float)atof(e) : 8.f; if (!(margin_in >= 0.5f && margin_in <= margin)) margin_in = fminf(8.f, margin);
+    e = getenv("WM_GRID_MARGIN_IN"); margin_in = e ? (float)atof(e) : 32.f; if (!(margin_in >= 0.5f && margin_in <= margin)) margin_in = fminf(32.f, margin);
   }
   const int seg_cap = h->seg_tiles * WM_TILE_SEGS;
   const float4* segrec = h->segrec + (int64_t)b0 * seg_cap * 2;

@@ -2,17 +2,19 @@
 // per-cell candidate runs — device side of the query, shared by k_offroad_grid (wm_grid.cu)
 // and the fused rollout kernel (wm_rollout_fused.cu).
 //
-// wm_prepare stores the road-edge segments of a scenario in ascending source order as 32-byte
-// records and lays a grid of square cells (side h) over their bounding box.  For a cell with
-// centre c and half diagonal rho, every segment that can be the nearest one of ANY point q of
-// the cell satisfies  dist(c, s) <= dmin(c) + 2 rho   (triangle inequality, twice), where
-// dmin(c) is the distance from c to its own nearest segment.  The cell keeps exactly those
-// segments, as runs of consecutive record indices (polyline pieces are contiguous, so a road
-// cell holds 1-3 runs).  A query is then: one 16-byte header load, a walk over ~20-40
-// candidate records, no bounding tests.  Cells with too many runs, and points outside the
-// grid, take a per-thread search over all 32-record chunks with bounding-box culling, which
-// is exact as well.  Per-pair arithmetic is the same as in the brute-force kernel
-// (wm_offroad.cu), so both modes return the same distances bit for bit.
+// wm_prepare stores the road-edge segments of a scenario in ascending source order (32-byte
+// records, and the same two by two as 48-byte pair records for packed arithmetic) and lays two
+// nested grids of square cells over them (wm_internal.cuh): a fine inner one over the segments'
+// bounding box, a coarse outer one over the wide margin around it.  For a cell with centre c and
+// half diagonal rho, every segment that can be the nearest one of ANY point q of the cell satisfies
+//     dist(c, s) <= dmin(c) + 2 rho        (triangle inequality, twice)
+// where dmin(c) is the distance from c to its own nearest segment.  The cell keeps those segments
+// (minus the ones a neighbour on the same polyline always beats, wm_grid.cu), as runs of
+// consecutive record indices: polyline pieces are contiguous, so a road cell holds 1-3 runs.  A
+// query is then: one 8-byte header load, a walk over ~7 candidate records, no bounding tests.
+// Cells with too many runs, and points outside both grids, take a warp search over all 32-record
+// chunks with bounding-box culling, which is exact as well.  Per-pair arithmetic is the same as in
+// the brute-force kernel (wm_offroad.cu), so both modes return the same distances bit for bit.
 #pragma once
 #include <float.h>
 
