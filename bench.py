@@ -282,8 +282,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--B", type=int, default=4096, help="scenarios per GPU (4096 = the BASELINE config)")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--cpu-B", type=int, default=16, help="oracle sample for cpu_baseline")
-    ap.add_argument("--ref-B", type=int, default=8)
+    ap.add_argument("--cpu-B", type=int, default=256, help="oracle sample for cpu_baseline (256 scenarios: ~15 s on 16 cores)")
+    ap.add_argument("--ref-B", type=int, default=64, help="oracle sample per step of --impl reference (~4 s on 16 cores)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4"],
                     help="rollout = the BASELINE metric (config 5, default); the others time the remaining "
