@@ -174,7 +174,7 @@ extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* 
   if (want_hist) WM_CUDA(wm_launch_observe_hist(h, *sim, t, hist, hist_valid, (cudaStream_t)stream));
   if (want_topk) {
     if (h->cfg.topk < 1 || h->cfg.topk > rg->R) return WM_ERR_UNSUPPORTED;
-    if (!h->pts || h->prep_B != sim->B || h->prep_R != rg->R || rg->B != sim->B) return WM_ERR_STATE;
+    if (!h->pt_xy || h->prep_B != sim->B || h->prep_R != rg->R || rg->B != sim->B) return WM_ERR_STATE;
     WM_CUDA(wm_launch_observe_topk(h, *sim, *rg, t, rg_index, rg_feat, rg_type, (cudaStream_t)stream));
   }
   return WM_OK;

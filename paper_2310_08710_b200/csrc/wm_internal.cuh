@@ -48,9 +48,13 @@ struct WmGrid {
   float ox0, oy0, oinv_h, oh; int onx, ony, icx0, icy0;   // outer grid; the inner grid starts at its cell (icx0, icy0)
 };
 
-// Prepared roadgraph points for top-k: float2 (x, y) per point, invalid -> (WM_FAR, WM_FAR),
-// padded to a multiple of WM_PT_TILE.
-constexpr int WM_PT_TILE = 2048;
+// Prepared roadgraph points for the top-k observation (wm_observe.cu): the valid points of a
+// scenario bucketed into a uniform grid of at most WM_PT_NG x WM_PT_NG cells (side >= 4 m) over
+// their bounding box, stored cell by cell in row-major cell order: (x, y), original index, and the
+// start of every cell.  A row of consecutive cells is one contiguous run of points.
+constexpr int WM_PT_NG = 64;
+constexpr int WM_PT_CELLS = WM_PT_NG * WM_PT_NG;
+struct WmPtGrid { float x0, y0, inv_h, h; int nx, ny, nvalid, pad; };
 
 constexpr int WM_HOST_CHUNKS = 16;          // scenario chunks of the pipelined host path
 
@@ -75,8 +79,10 @@ struct wm_handle {
   uint2* cells;             // [B][WM_GRID_CELLS]  cell headers, 2 x 2 tiles
   uint32_t* pool;           // [B][WM_POOL_CAP]    overflow runs
   int32_t* pool_cnt;        // [B]
-  int32_t pts_pad;          // padded R
-  float2* pts;              // [B][pts_pad]
+  float2* pt_xy;            // [B][R] valid points in cell order (wm_observe.cu)
+  int32_t* pt_idx;          // [B][R] their roadgraph indices
+  int32_t* pt_start;        // [B][WM_PT_CELLS + 1] first point of every cell; [ny * nx] = number of valid points
+  WmPtGrid* pt_grid;        // [B]
   // rollout graph cache; streams and events of the pipelined host path (wm_rollout_host)
   cudaStream_t cap_stream, roll_stream, d2h_stream;
   cudaEvent_t ev_up[WM_HOST_CHUNKS], ev_prep[WM_HOST_CHUNKS], ev_done[WM_HOST_CHUNKS];
@@ -152,6 +158,7 @@ int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaS
 void wm_prepare_free(wm_handle* h);
 void wm_drop_graph(wm_handle* h);
 cudaError_t wm_launch_observe_hist(wm_handle* h, const wm_traj& sim, int t, float* hist, uint8_t* hist_valid, cudaStream_t s);
+cudaError_t wm_launch_point_grid(wm_handle* h, const wm_roadgraph& rg, int b0, int nb, cudaStream_t s);   // scenarios [b0, b0 + nb)
 cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_roadgraph& rg, int t,
                                    int32_t* rg_index, float* rg_feat, int32_t* rg_type, cudaStream_t s);
 

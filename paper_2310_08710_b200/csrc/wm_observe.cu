@@ -5,16 +5,21 @@
 // group of egos) stages the H history rows in shared memory once and streams out rows of A
 // floats, fully coalesced.
 //
-// k_observe_topk: exact top-k by MSB radix select on the float32 key d2 = fma(dy,dy,dx*dx)
-// (bit pattern of a non-negative float is order preserving).  One warp per valid ego, 16 egos
-// per CTA share each roadgraph tile, which is streamed through shared memory by bulk TMA in
-// double-buffered tiles.  Passes over the R points:
-//   1. histogram of the key's top bits in lane-private shared-memory counters (no atomics)
+// k_observe_topk: exact top-k on the float32 key d2 = fma(dy,dy,dx*dx) (the bit pattern of a
+// non-negative float is order preserving; DESIGN.md R-topk).  wm_prepare buckets the valid points of
+// a scenario into a uniform grid (k_point_grid).  One 128-thread CTA per ego:
+//   0. the square of cells around the ego's cell that holds ~1.35 k points (cell counts only);
+//   1. histogram of the keys' top bits over the points of that square (shared-memory atomics)
 //      -> bin of the k-th key (repeated on the bin's sub-range only if the bin is too large);
-//   2. collect the (key, index) pairs of that bin (<= 1024) -> bitwise descent gives the exact
-//      k-th key T and the number of ties to take;
-//   3. emit, in ascending index order (ballot + popc compaction): key < T, or key == T and
-//      among the first `quota` such points (ties -> lower index), with ego-frame features.
+//   2. collect the (key, index) pairs of that bin (<= 512) -> bitwise descent gives the exact k-th
+//      key T and the number of ties to take;
+//   3. every point outside a square of m rings is farther than m h, so if sqrt(T) < m h the k
+//      nearest points of the square are the k nearest of the scenario; otherwise the square grows
+//      to hold the disc of radius sqrt(T) and 1-2 run again (T of a subset is never too small);
+//   4. mark key < T in a bitmap over the roadgraph indices, key == T in a second one; the first
+//      `quota` tie bits in index order join (ties -> lower index, D23);
+//   5. emit the set bits in ascending index order (block scan of popcounts) with ego-frame features.
+// It reads ~2.3 k of the scenario's 30 k points per ego instead of all of them three times.
 #include "wm_internal.cuh"
 
 // ======================================================================================
@@ -92,282 +97,339 @@ cudaError_t wm_launch_observe_hist(wm_handle* h, const wm_traj& sim, int t, floa
 // ======================================================================================
 // top-k roadgraph points
 // ======================================================================================
-constexpr int TK_WARPS = 16;                 // egos per CTA
-constexpr int TK_THREADS = TK_WARPS * 32;
-constexpr int TK_BINS = 128;
-constexpr int TK_CAPB = 1024;                // boundary (key, index) pairs per ego: 8 KB, aliases the histogram
-constexpr uint32_t TK_KEY_FAR = 0x7149F2CAu; // bits of 1e30f: keys at or above are padding / invalid points
-constexpr int TK_BASE = 119 << 2;            // level-0 bins start at d2 = 2^-8 (2 mantissa bits per bin)
+constexpr int PG_THREADS = 1024;
+
+// wm_prepare: bucket the valid points of one scenario (one CTA) into the point grid.
+__global__ void __launch_bounds__(PG_THREADS) k_point_grid(const float* x, const float* y, const uint8_t* valid, int R,
+                                                           float2* pt_xy, int32_t* pt_idx, int32_t* pt_start, WmPtGrid* pt_grid) {
+  __shared__ int s_cnt[WM_PT_CELLS];
+  __shared__ float s_red[4][32];
+  __shared__ int s_scan[32];
+  __shared__ WmPtGrid s_g;
+  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t o = (int64_t)b * R;
+  x += o; y += o; valid += o; pt_xy += o; pt_idx += o;
+  pt_start += (int64_t)b * (WM_PT_CELLS + 1);
+  // bounding box of the valid points
+  float x0 = 3.0e38f, y0 = 3.0e38f, x1 = -3.0e38f, y1 = -3.0e38f;
+  for (int i = tid; i < R; i += PG_THREADS)
+    if (valid[i] != 0) { const float px = x[i], py = y[i]; x0 = fminf(x0, px); x1 = fmaxf(x1, px); y0 = fminf(y0, py); y1 = fmaxf(y1, py); }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    x0 = fminf(x0, __shfl_xor_sync(0xffffffffu, x0, d)); y0 = fminf(y0, __shfl_xor_sync(0xffffffffu, y0, d));
+    x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, d)); y1 = fmaxf(y1, __shfl_xor_sync(0xffffffffu, y1, d));
+  }
+  if (lane == 0) { s_red[0][warp] = x0; s_red[1][warp] = y0; s_red[2][warp] = x1; s_red[3][warp] = y1; }
+  for (int c = tid; c < WM_PT_CELLS; c += PG_THREADS) s_cnt[c] = 0;
+  __syncthreads();
+  if (tid == 0) {
+    for (int w = 1; w < PG_THREADS / 32; ++w) {
+      x0 = fminf(x0, s_red[0][w]); y0 = fminf(y0, s_red[1][w]); x1 = fmaxf(x1, s_red[2][w]); y1 = fmaxf(y1, s_red[3][w]);
+    }
+    WmPtGrid g;
+    g.pad = 0; g.nvalid = 0;
+    if (!(x1 >= x0)) { g.x0 = 0.f; g.y0 = 0.f; g.h = 4.f; g.inv_h = 0.25f; g.nx = 0; g.ny = 0; }
+    else {
+      const float W = x1 - x0, H = y1 - y0;
+      const float h = fmaxf(4.f, fmaxf(W, H) * (1.0001f / WM_PT_NG));
+      g.x0 = x0; g.y0 = y0; g.h = h; g.inv_h = 1.f / h;
+      g.nx = min(WM_PT_NG, (int)floorf(W / h) + 1); g.ny = min(WM_PT_NG, (int)floorf(H / h) + 1);
+    }
+    s_g = g;
+  }
+  __syncthreads();
+  const WmPtGrid g = s_g;
+  const int ncell = g.nx * g.ny;
+  auto cell_of = [&](float px, float py) {
+    const int i = min(g.nx - 1, max(0, (int)floorf((px - g.x0) * g.inv_h)));
+    const int j = min(g.ny - 1, max(0, (int)floorf((py - g.y0) * g.inv_h)));
+    return j * g.nx + i;
+  };
+  for (int i = tid; i < R; i += PG_THREADS) if (valid[i] != 0) atomicAdd(&s_cnt[cell_of(x[i], y[i])], 1);
+  __syncthreads();
+  // exclusive scan of the cell counts: each thread owns WM_PT_CELLS / PG_THREADS consecutive cells
+  constexpr int PER = WM_PT_CELLS / PG_THREADS;
+  int loc[PER], sum = 0;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) { loc[q] = sum; sum += s_cnt[tid * PER + q]; }
+  int inc = sum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+  if (lane == 31) s_scan[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    int v = s_scan[lane], w = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, w, d); if (lane >= d) w += u; }
+    s_scan[lane] = w - v;
+  }
+  __syncthreads();
+  const int base = s_scan[warp] + inc - sum;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) {
+    const int c = tid * PER + q;
+    s_cnt[c] = base + loc[q];                       // now the running cursor of the cell
+    if (c <= ncell) pt_start[c] = base + loc[q];    // cells >= ncell are empty: [ncell] = number of valid points
+  }
+  if (tid == PG_THREADS - 1) {
+    if (ncell == WM_PT_CELLS) pt_start[WM_PT_CELLS] = base + sum;
+    WmPtGrid gg = g; gg.nvalid = base + sum;
+    pt_grid[b] = gg;
+  }
+  __syncthreads();
+  for (int i = tid; i < R; i += PG_THREADS)
+    if (valid[i] != 0) {
+      const float px = x[i], py = y[i];
+      const int pos = atomicAdd(&s_cnt[cell_of(px, py)], 1);
+      pt_xy[pos] = make_float2(px, py);
+      pt_idx[pos] = i;
+    }
+}
+
+cudaError_t wm_launch_point_grid(wm_handle* h, const wm_roadgraph& rg, int b0, int nb, cudaStream_t s) {
+  const int64_t o = (int64_t)b0 * rg.R;
+  k_point_grid<<<nb, PG_THREADS, 0, s>>>(rg.x + o, rg.y + o, rg.valid + o, rg.R, h->pt_xy + o, h->pt_idx + o,
+                                         h->pt_start + (int64_t)b0 * (WM_PT_CELLS + 1), h->pt_grid + b0);
+  h->launches++;
+  return cudaGetLastError();
+}
+
+constexpr int TK_THREADS = 128;              // one CTA per ego
+constexpr int TK_BINS = 256;
+constexpr int TK_CAP = 512;                  // boundary (key, index) pairs
+constexpr int TK_BASE = 119 << 3;            // level-0 bins start at d2 = 2^-8, 3 mantissa bits per bin
 
 struct TopkParams {
   wm_row row;
   int A, R, k;
-  const float2* pts; int pts_pad;
-  const float *dir_x, *dir_y; const int32_t* type;
+  const float2* pt_xy; const int32_t* pt_idx; const int32_t* pt_start; const WmPtGrid* pt_grid;
+  const float *x, *y, *dir_x, *dir_y; const int32_t* type;
   int32_t* rg_index; float* rg_feat; int32_t* rg_type;
 };
 
-enum { TK_HIST0 = 0, TK_HISTN = 1, TK_COLLECT = 2, TK_EMIT = 3 };
+__device__ __forceinline__ int tk_bin0(uint32_t key) { return min(max((int)(key >> 20) - TK_BASE, 0), TK_BINS - 1); }
+__device__ __forceinline__ uint32_t tk_bin0_lo(int bin) { return bin <= 0 ? 0u : (uint32_t)(bin + TK_BASE) << 20; }
+__device__ __forceinline__ uint32_t tk_bin0_hi(int bin) { return bin >= TK_BINS - 1 ? 0xffffffffu : (uint32_t)(bin + TK_BASE + 1) << 20; }
 
-struct TkWarp {          // per-warp (per-ego) selection state, in registers
-  float ex, ey, cs, sn;
-  uint32_t lo, hi;       // undecided key range [lo, hi)
-  int shift;             // linear sub-bin shift for TK_HISTN
-  int c_less;            // points with key < lo
-  int kk;                // min(k, number of real points)
-  int in_bin;            // points with key in [lo, hi)
-  uint32_t T; int quota; // exact threshold and ties to take
-  int n_out, n_tie, n_col;
-  int ego;               // agent slot of this warp's ego (-1: none)
-  bool active, refine;
+struct TkShared {
+  uint32_t hist[TK_BINS];
+  uint2 col[TK_CAP];
+  int scan[TK_THREADS / 32];
+  uint32_t lo, hi, T;            // undecided key range [lo, hi); exact threshold
+  int shift, c_less, in_bin, n_col, quota, m, count, again;
 };
 
-__device__ __forceinline__ int tk_bin0(uint32_t key) {
-  if (key >= TK_KEY_FAR) return TK_BINS - 1;
-  const int v = (int)(key >> 21) - TK_BASE;
-  return min(max(v, 0), TK_BINS - 2);
-}
-__device__ __forceinline__ uint32_t tk_bin0_lo(int bin) { return bin <= 0 ? 0u : (uint32_t)(bin + TK_BASE) << 21; }
-__device__ __forceinline__ uint32_t tk_bin0_hi(int bin) {
-  return bin >= TK_BINS - 2 ? (bin == TK_BINS - 2 ? TK_KEY_FAR : 0xffffffffu) : (uint32_t)(bin + TK_BASE + 1) << 21;
+// exclusive prefix sum of v over the CTA; total in `total`
+__device__ __forceinline__ int tk_block_scan(int v, int* s_scan, int& total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += u; }
+  __syncthreads();                              // s_scan may still be read from a previous call
+  if (lane == 31) s_scan[warp] = inc;
+  __syncthreads();
+  int base = 0; total = 0;
+#pragma unroll
+  for (int w = 0; w < TK_THREADS / 32; ++w) { const int t = s_scan[w]; if (w < warp) base += t; total += t; }
+  return base + inc - v;
 }
 
-// One streaming pass over the scenario's points.  All warps of the CTA walk the same tiles
-// (double-buffered bulk TMA); each applies MODE to its own ego.
-template <int MODE>
-__device__ __forceinline__ void tk_pass(const TopkParams& p, int b, TkWarp& w, uint64_t* bars, float2* s_tiles,
-                                        uint16_t* s_hist, uint2* s_col, uint32_t& tile_seq) {
+// warp 0, after a histogram pass: the bin that holds rank `need` (1-based) of the current range
+__device__ __forceinline__ void tk_locate(TkShared& S, int need, bool level0) {
   const int lane = threadIdx.x & 31;
-  const int ntile = p.pts_pad / WM_PT_TILE;
-  const float2* src = p.pts + (int64_t)b * p.pts_pad;
-  const uint32_t lt = (1u << lane) - 1u;
-  if (threadIdx.x == 0) {
-    fence_proxy_async();
-    for (int i = 0; i < 2 && i < ntile; ++i) {
-      const uint32_t q = tile_seq + i;
-      mbar_expect_tx(&bars[q & 1], WM_PT_TILE * 8);
-      tma_load_1d(s_tiles + (q & 1) * WM_PT_TILE, src + (int64_t)i * WM_PT_TILE, WM_PT_TILE * 8, &bars[q & 1]);
-    }
-  }
-  for (int ti = 0; ti < ntile; ++ti) {
-    const uint32_t q = tile_seq + ti;
-    mbar_wait(&bars[q & 1], (q >> 1) & 1);
-    const float2* tile = s_tiles + (q & 1) * WM_PT_TILE;
-    if (w.active && (MODE != TK_HISTN || w.refine)) {
-#pragma unroll 4
-      for (int j = 0; j < WM_PT_TILE / 32; ++j) {
-        const int li = j * 32 + lane;
-        const float2 pt = tile[li];
-        const float dx = __fsub_rn(pt.x, w.ex), dy = __fsub_rn(pt.y, w.ey);
-        const uint32_t key = __float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-        if (MODE == TK_HIST0) {
-          uint16_t* c = s_hist + tk_bin0(key) * 32 + lane;
-          *c = (uint16_t)(*c + 1);
-        } else if (MODE == TK_HISTN) {
-          if (key >= w.lo && key < w.hi) {
-            uint16_t* c = s_hist + (int)((key - w.lo) >> w.shift) * 32 + lane;
-            *c = (uint16_t)(*c + 1);
-          }
-        } else if (MODE == TK_COLLECT) {
-          const bool in = key >= w.lo && key < w.hi;
-          const uint32_t bal = __ballot_sync(0xffffffffu, in);
-          if (in) s_col[w.n_col + __popc(bal & lt)] = make_uint2(key, (uint32_t)(ti * WM_PT_TILE + li));
-          w.n_col += __popc(bal);
-        } else {
-          const bool tie = key == w.T;
-          const uint32_t tb = __ballot_sync(0xffffffffu, tie);
-          const bool take = key < w.T || (tie && w.n_tie + __popc(tb & lt) < w.quota);
-          const uint32_t kb = __ballot_sync(0xffffffffu, take);
-          if (take) {
-            const int pos = w.n_out + __popc(kb & lt);
-            const int idx = ti * WM_PT_TILE + li;
-            const int64_t g = (int64_t)b * p.R + idx;
-            const float ux = __ldg(&p.dir_x[g]), uy = __ldg(&p.dir_y[g]);
-            const int64_t o_idx = ((int64_t)b * p.A + w.ego) * p.k + pos;
-            p.rg_index[o_idx] = idx;
-            p.rg_type[o_idx] = __ldg(&p.type[g]);
-            float* f = p.rg_feat + ((int64_t)b * p.A + w.ego) * 4 * p.k + pos;
-            f[0] = fmaf(w.cs, dx, w.sn * dy);
-            f[p.k] = fmaf(w.cs, dy, -w.sn * dx);
-            f[2 * (int64_t)p.k] = fmaf(w.cs, ux, w.sn * uy);
-            f[3 * (int64_t)p.k] = fmaf(w.cs, uy, -w.sn * ux);
-          }
-          w.n_tie += __popc(tb);
-          w.n_out += __popc(kb);
-        }
-      }
-    }
-    __syncthreads();                          // everyone is done with this buffer
-    if (threadIdx.x == 0 && ti + 2 < ntile) {
-      fence_proxy_async();
-      mbar_expect_tx(&bars[q & 1], WM_PT_TILE * 8);
-      tma_load_1d(s_tiles + (q & 1) * WM_PT_TILE, src + (int64_t)(ti + 2) * WM_PT_TILE, WM_PT_TILE * 8, &bars[q & 1]);
-    }
-  }
-  tile_seq += ntile;
-}
-
-// after a histogram pass: fold the lane-private counters, locate the bin holding rank kk
-__device__ __forceinline__ void tk_locate(TkWarp& w, uint16_t* s_hist, bool level0) {
-  const int lane = threadIdx.x & 31;
-  // lane l owns bins 4l .. 4l+3
-  int tot[4];
+  constexpr int PER = TK_BINS / 32;
+  int tot[PER], mine = 0;
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    const uint16_t* r = s_hist + (lane * 4 + q) * 32;
-    int s = 0;
-    for (int i = 0; i < 32; ++i) s += r[(i + lane) & 31];     // rotate to spread banks
-    tot[q] = s;
-  }
-  __syncwarp();
-  if (level0) {                                // real points = everything but the far bin
-    const int far = __shfl_sync(0xffffffffu, tot[3], 31);
-    int all = tot[0] + tot[1] + tot[2] + tot[3];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) all += __shfl_xor_sync(0xffffffffu, all, o);
-    w.kk = min(w.kk, all - far);
-  }
-  const int mine = tot[0] + tot[1] + tot[2] + tot[3];
+  for (int q = 0; q < PER; ++q) { tot[q] = (int)S.hist[lane * PER + q]; mine += tot[q]; }
   int inc = mine;
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-  const int need = w.kk - w.c_less;            // 1-based rank inside the current range
+  for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += u; }
   const uint32_t has = __ballot_sync(0xffffffffu, inc >= need);
-  int bin = 0, below = 0, cnt = 0;
-  if (need >= 1 && has) {
-    const int L = __ffs(has) - 1;
-    int ex = inc - mine, bq = 0, cq = 0, found = 0;
+  const int L = has ? __ffs(has) - 1 : 31;
+  int ex = inc - mine, bq = PER - 1, cq = 0, found = 0;
 #pragma unroll
-    for (int q = 0; q < 4; ++q) if (!found) { if (ex + tot[q] >= need) { bq = q; cq = tot[q]; found = 1; } else ex += tot[q]; }
-    bin = __shfl_sync(0xffffffffu, lane * 4 + bq, L);
-    below = __shfl_sync(0xffffffffu, ex, L);
-    cnt = __shfl_sync(0xffffffffu, cq, L);
+  for (int q = 0; q < PER; ++q) if (!found) { if (ex + tot[q] >= need) { bq = q; cq = tot[q]; found = 1; } else ex += tot[q]; }
+  const int bin = __shfl_sync(0xffffffffu, lane * PER + bq, L);
+  const int below = __shfl_sync(0xffffffffu, ex, L);
+  const int cnt = __shfl_sync(0xffffffffu, cq, L);
+  if (lane == 0) {
+    if (level0) { S.lo = tk_bin0_lo(bin); S.hi = tk_bin0_hi(bin); }
+    else { const uint32_t base = S.lo; S.lo = base + ((uint32_t)bin << S.shift); S.hi = min(S.hi, base + ((uint32_t)(bin + 1) << S.shift)); }
+    S.c_less += below;
+    S.in_bin = cnt;
   }
-  if (w.kk <= 0) { w.in_bin = 0; w.hi = w.lo; return; }
-  if (level0) { w.lo = tk_bin0_lo(bin); w.hi = tk_bin0_hi(bin); }
-  else { const uint32_t base = w.lo; w.lo = base + ((uint32_t)bin << w.shift); w.hi = min(w.hi, base + ((uint32_t)(bin + 1) << w.shift)); }
-  w.c_less += below;
-  w.in_bin = cnt;
 }
 
-__global__ void __launch_bounds__(TK_THREADS, 1) k_observe_topk(TopkParams p) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  uint64_t* bars = (uint64_t*)smem_raw;                                  // [2]
-  int* s_ego = (int*)(smem_raw + 16);                                    // [TK_WARPS] ego slots of this CTA
-  float2* s_tiles = (float2*)(smem_raw + 128);                           // 2 x WM_PT_TILE
-  uint16_t* s_hist_all = (uint16_t*)(smem_raw + 128 + 2 * WM_PT_TILE * 8);  // TK_WARPS x 8 KB
-  const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  uint16_t* s_hist = s_hist_all + warp * (TK_BINS * 32);
-  uint2* s_col = (uint2*)s_hist;
-  const int A = p.A, k = p.k;
+__global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
+  extern __shared__ __align__(16) uint32_t s_bits[];     // [2][Wd]: key < T; key == T (ties)
+  __shared__ TkShared S;
+  const int b = blockIdx.y, ego = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int A = p.A, k = p.k, R = p.R, Wd = (R + 31) >> 5;
+  uint32_t* bm = s_bits;
+  uint32_t* tb = s_bits + Wd;
   const int64_t ro = (int64_t)b * p.row.stride_b;
-
-  // the valid egos [16*blockIdx.x, +16) of the compacted list; invalid ego slots are filled by
-  // the CTA that covers the same slot range
-  if (threadIdx.x < TK_WARPS) s_ego[threadIdx.x] = -1;
-  if (threadIdx.x == 0) { mbar_init(&bars[0], 1); mbar_init(&bars[1], 1); mbar_fence_init(); }
-  __syncthreads();
-  if (warp == 0) {
-    int run = 0;
-    const int first = blockIdx.x * TK_WARPS;
-    for (int base = 0; base < A; base += 32) {
-      const int a = base + lane;
-      const bool v = a < A && p.row.valid[ro + a] != 0;
-      const uint32_t bal = __ballot_sync(0xffffffffu, v);
-      const int ci = run + __popc(bal & ((1u << lane) - 1u));
-      if (v && ci >= first && ci < first + TK_WARPS) s_ego[ci - first] = a;
-      run += __popc(bal);
+  const int64_t oi = ((int64_t)b * A + ego) * k;          // rg_index / rg_type row
+  float* feat = p.rg_feat + ((int64_t)b * A + ego) * 4 * k;
+  auto pad_from = [&](int n0) {                           // D10 / D25
+    for (int j = n0 + tid; j < k; j += TK_THREADS) {
+      p.rg_index[oi + j] = -1; p.rg_type[oi + j] = 0;
+      feat[j] = 0.f; feat[k + j] = 0.f; feat[2 * (int64_t)k + j] = 0.f; feat[3 * (int64_t)k + j] = 0.f;
     }
+  };
+  const WmPtGrid g = p.pt_grid[b];
+  const int kk = min(k, g.nvalid);
+  if (p.row.valid[ro + ego] == 0 || kk <= 0) { pad_from(0); return; }
+  const float ex = p.row.x[ro + ego], ey = p.row.y[ro + ego];
+  float sn, cs;
+  sincosf(p.row.yaw[ro + ego], &sn, &cs);
+  const float2* pxy = p.pt_xy + (int64_t)b * R;
+  const int32_t* pidx = p.pt_idx + (int64_t)b * R;
+  const int32_t* start = p.pt_start + (int64_t)b * (WM_PT_CELLS + 1);
+  const int ci = min(g.nx - 1, max(0, (int)floorf((ex - g.x0) * g.inv_h)));
+  const int cj = min(g.ny - 1, max(0, (int)floorf((ey - g.y0) * g.inv_h)));
+  // float32 rounding of cell assignments (points and ego): far above an ulp of the coordinates
+  const float tol = 2e-3f + 1e-6f * (fabsf(g.x0) + fabsf(g.y0) + (float)(g.nx + g.ny) * g.h);
+
+  // points in the square of m rings around the ego's cell (rows are contiguous runs)
+  auto square_count = [&](int m) {                        // warp 0
+    const int i0 = max(ci - m, 0), i1 = min(ci + m, g.nx - 1), j0 = max(cj - m, 0), j1 = min(cj + m, g.ny - 1);
+    int c = 0;
+    for (int j = j0 + lane; j <= j1; j += 32) c += __ldg(start + j * g.nx + i1 + 1) - __ldg(start + j * g.nx + i0);
+    return __reduce_add_sync(0xffffffffu, c);
+  };
+  if (warp == 0) {                                        // 0. the first square: ~1.35 k points
+    const int want = min(g.nvalid, kk + (kk * 35) / 100);
+    int m = 0, c = 0;
+    for (;; ++m) { c = square_count(m); if (c >= want || m >= WM_PT_NG) break; }
+    if (lane == 0) { S.m = m; S.count = c; }
   }
-  // fill the outputs of invalid ego slots in this CTA's slot range (D10 / D25)
-  for (int a = blockIdx.x * TK_WARPS + warp; a < min(A, (int)(blockIdx.x + 1) * TK_WARPS); a += TK_WARPS) {
-    if (p.row.valid[ro + a] == 0) {
-      for (int j = lane; j < k; j += 32) {
-        const int64_t o = ((int64_t)b * A + a) * k + j;
-        p.rg_index[o] = -1; p.rg_type[o] = 0;
-        float* f = p.rg_feat + ((int64_t)b * A + a) * 4 * k + j;
-        f[0] = 0.f; f[k] = 0.f; f[2 * (int64_t)k] = 0.f; f[3 * (int64_t)k] = 0.f;
+  for (int i = tid; i < 2 * Wd; i += TK_THREADS) s_bits[i] = 0u;
+  __syncthreads();
+
+  // one pass over the points of the current square: f(key, sorted position)
+  auto for_square = [&](auto&& f) {
+    const int m = S.m;
+    const int i0 = max(ci - m, 0), i1 = min(ci + m, g.nx - 1), j0 = max(cj - m, 0), j1 = min(cj + m, g.ny - 1);
+    for (int j = j0; j <= j1; ++j) {
+      const int s0 = __ldg(start + j * g.nx + i0), s1 = __ldg(start + j * g.nx + i1 + 1);
+      for (int s = s0 + tid; s < s1; s += TK_THREADS) {
+        const float2 pt = __ldg(pxy + s);
+        const float dx = __fsub_rn(pt.x, ex), dy = __fsub_rn(pt.y, ey);
+        f(__float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx))), s);
       }
     }
-  }
-  __syncthreads();
-  if (s_ego[0] < 0) return;                     // no valid ego left for this CTA (uniform)
+  };
 
-  TkWarp w;
-  const int ego = s_ego[warp];
-  w.ego = ego;
-  w.active = ego >= 0;
-  w.ex = w.ey = 0.f; w.cs = 1.f; w.sn = 0.f;
-  if (w.active) { w.ex = p.row.x[ro + ego]; w.ey = p.row.y[ro + ego]; sincosf(p.row.yaw[ro + ego], &w.sn, &w.cs); }
-  w.lo = 0; w.hi = 0xffffffffu; w.shift = 0; w.c_less = 0; w.kk = k; w.in_bin = 0;
-  w.T = 0; w.quota = 0; w.n_out = 0; w.n_tie = 0; w.n_col = 0; w.refine = false;
-  uint32_t tile_seq = 0;
-
-  // ---- pass 1: level-0 histogram ----
-  for (int i = lane; i < TK_BINS * 32 / 2; i += 32) ((uint32_t*)s_hist)[i] = 0;
-  __syncwarp();
-  tk_pass<TK_HIST0>(p, b, w, bars, s_tiles, s_hist, s_col, tile_seq);
-  if (w.active) tk_locate(w, s_hist, true);
-  // ---- refine while the bin of the k-th key is too large for the collect buffer ----
   for (;;) {
-    w.refine = w.active && w.in_bin > TK_CAPB && (w.hi - w.lo) > 1u;
-    if (!__syncthreads_or(w.refine ? 1 : 0)) break;
-    if (w.refine) {
-      const uint32_t span = w.hi - w.lo;
-      w.shift = max(0, 32 - __clz(span - 1) - 7);        // (span-1) >> shift < 128
-      for (int i = lane; i < TK_BINS * 32 / 2; i += 32) ((uint32_t*)s_hist)[i] = 0;
-      __syncwarp();
+    // ---- 1. level-0 histogram, bin of the kk-th key ----
+    for (int i = tid; i < TK_BINS; i += TK_THREADS) S.hist[i] = 0u;
+    if (tid == 0) { S.lo = 0u; S.hi = 0xffffffffu; S.c_less = 0; S.n_col = 0; S.shift = 0; }
+    __syncthreads();
+    for_square([&](uint32_t key, int) { atomicAdd(&S.hist[tk_bin0(key)], 1u); });
+    __syncthreads();
+    if (warp == 0) tk_locate(S, kk, true);
+    __syncthreads();
+    // ---- refine while the bin is too large for the collect buffer ----
+    while (S.in_bin > TK_CAP && S.hi - S.lo > 1u) {
+      const uint32_t lo = S.lo, hi = S.hi;
+      const int shift = max(0, 32 - __clz(hi - lo - 1u) - 8);           // (span - 1) >> shift < 256
+      __syncthreads();
+      for (int i = tid; i < TK_BINS; i += TK_THREADS) S.hist[i] = 0u;
+      if (tid == 0) S.shift = shift;
+      __syncthreads();
+      for_square([&](uint32_t key, int) { if (key >= lo && key < hi) atomicAdd(&S.hist[(key - lo) >> shift], 1u); });
+      __syncthreads();
+      if (warp == 0) tk_locate(S, kk - S.c_less, false);
+      __syncthreads();
     }
-    tk_pass<TK_HISTN>(p, b, w, bars, s_tiles, s_hist, s_col, tile_seq);
-    if (w.refine) tk_locate(w, s_hist, false);
-  }
-  __syncwarp();
-  // ---- pass 2: collect the undecided bin, then exact threshold by bitwise descent ----
-  const bool single = w.active && w.in_bin > TK_CAPB;     // one key value with > CAPB ties
-  {
-    TkWarp wc = w;
-    if (single || !w.active || w.kk <= 0) wc.hi = wc.lo;  // nothing to collect
-    wc.n_col = 0;
-    tk_pass<TK_COLLECT>(p, b, wc, bars, s_tiles, s_hist, s_col, tile_seq);
-    w.n_col = wc.n_col;
-  }
-  __syncwarp();
-  if (w.active && w.kk > 0) {
-    int r = w.kk - w.c_less;                               // 1-based rank inside [lo, hi)
-    if (single) { w.T = w.lo; w.quota = r; }
-    else {
-      uint32_t pfx = 0, mask = 0;
-      const uint32_t diff = w.lo ^ (w.hi - 1u);
-      const int top = diff ? 31 - __clz(diff) : -1;        // bits above `top` are common to the range
-      if (top < 31) { mask = ~((top >= 0 ? (2u << top) : 1u) - 1u); pfx = w.lo & mask; }
-      for (int bit = top; bit >= 0; --bit) {
-        const uint32_t m2 = mask | (1u << bit);
-        int c0 = 0;
-        for (int i = lane; i < w.n_col; i += 32) c0 += ((s_col[i].x & m2) == pfx) ? 1 : 0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) c0 += __shfl_xor_sync(0xffffffffu, c0, o);
-        if (r > c0) { r -= c0; pfx |= 1u << bit; }
-        mask = m2;
+    // ---- 2. collect the bin, exact threshold by bitwise descent ----
+    const uint32_t lo = S.lo, hi = S.hi;
+    const bool single = S.in_bin > TK_CAP;                // one key value with more than TK_CAP ties
+    if (!single) for_square([&](uint32_t key, int s) {
+      if (key >= lo && key < hi) { const int q = atomicAdd(&S.n_col, 1); if (q < TK_CAP) S.col[q] = make_uint2(key, (uint32_t)s); }
+    });
+    __syncthreads();
+    if (warp == 0) {
+      int r = kk - S.c_less;                              // 1-based rank inside [lo, hi)
+      uint32_t T = lo;
+      if (!single) {
+        const int n_col = min(S.n_col, TK_CAP);
+        uint32_t pfx = 0, mask = 0;
+        const uint32_t diff = lo ^ (hi - 1u);
+        const int top = diff ? 31 - __clz(diff) : -1;     // bits above `top` are common to the range
+        if (top < 31) { mask = ~((top >= 0 ? (2u << top) : 1u) - 1u); pfx = lo & mask; }
+        for (int bit = top; bit >= 0; --bit) {
+          const uint32_t m2 = mask | (1u << bit);
+          int c0 = 0;
+          for (int i = lane; i < n_col; i += 32) c0 += ((S.col[i].x & m2) == pfx) ? 1 : 0;
+          c0 = __reduce_add_sync(0xffffffffu, c0);
+          if (r > c0) { r -= c0; pfx |= 1u << bit; }
+          mask = m2;
+        }
+        T = pfx;
       }
-      w.T = pfx; w.quota = r;                              // r = ties (key == T) to take, in index order
+      // ---- 3. is the square large enough? ----
+      const int m = S.m;
+      const bool all = S.count >= g.nvalid;
+      const float reach = (float)m * g.h - tol;
+      const float dT = sqrtf(__uint_as_float(T)) * 1.000001f;
+      int again = 0;
+      if (!all && !(dT < reach)) {
+        int m2 = max(m + 1, (int)ceilf((dT + tol) * g.inv_h) + 1);
+        m2 = min(m2, WM_PT_NG);
+        const int c = square_count(m2);
+        if (lane == 0) { S.m = m2; S.count = c; }
+        again = 1;
+      }
+      if (lane == 0) { S.T = T; S.quota = r; S.again = again; }   // r = ties (key == T) to take, in index order
     }
-  } else { w.T = 0; w.quota = 0; }
-  // ---- pass 3: emit in ascending index order ----
-  {
-    TkWarp we = w;
-    we.n_out = 0; we.n_tie = 0;
-    if (!w.active || w.kk <= 0) { we.T = 0; we.quota = 0; }
-    tk_pass<TK_EMIT>(p, b, we, bars, s_tiles, s_hist, s_col, tile_seq);
-    w.n_out = we.n_out;
+    __syncthreads();
+    if (!S.again) break;
+    __syncthreads();
   }
-  if (w.active) {                                           // D25 padding
-    for (int j = w.n_out + lane; j < k; j += 32) {
-      const int64_t o = ((int64_t)b * A + ego) * k + j;
-      p.rg_index[o] = -1; p.rg_type[o] = 0;
-      float* f = p.rg_feat + ((int64_t)b * A + ego) * 4 * k + j;
-      f[0] = 0.f; f[k] = 0.f; f[2 * (int64_t)k] = 0.f; f[3 * (int64_t)k] = 0.f;
+
+  // ---- 4. mark the selected points over the roadgraph indices ----
+  const uint32_t T = S.T;
+  for_square([&](uint32_t key, int s) {
+    if (key <= T) { const int idx = __ldg(pidx + s); atomicOr((key < T ? bm : tb) + (idx >> 5), 1u << (idx & 31)); }
+  });
+  __syncthreads();
+  const int wpt = (Wd + TK_THREADS - 1) / TK_THREADS, w0 = min(tid * wpt, Wd), w1 = min(w0 + wpt, Wd);
+  {                                                       // the first `quota` ties in index order
+    int c = 0, total;
+    for (int w = w0; w < w1; ++w) c += __popc(tb[w]);
+    int left = S.quota - tk_block_scan(c, S.scan, total);
+    for (int w = w0; w < w1; ++w) {
+      uint32_t t = tb[w];
+      const int n = __popc(t);
+      if (left < n) { for (int drop = n - max(left, 0); drop > 0; --drop) t &= ~(0x80000000u >> __clz(t)); }   // keep the lowest bits
+      left -= n;
+      bm[w] |= t;
     }
   }
+  // ---- 5. emit in ascending index order ----
+  int c = 0, n_out;
+  for (int w = w0; w < w1; ++w) c += __popc(bm[w]);
+  int pos = tk_block_scan(c, S.scan, n_out);
+  const float *gx = p.x + (int64_t)b * R, *gy = p.y + (int64_t)b * R, *gdx = p.dir_x + (int64_t)b * R, *gdy = p.dir_y + (int64_t)b * R;
+  const int32_t* gt = p.type + (int64_t)b * R;
+  for (int w = w0; w < w1; ++w) {
+    uint32_t bits = bm[w];
+    while (bits) {
+      const int idx = w * 32 + __ffs(bits) - 1;
+      bits &= bits - 1;
+      const float dx = __fsub_rn(__ldg(gx + idx), ex), dy = __fsub_rn(__ldg(gy + idx), ey);
+      const float ux = __ldg(gdx + idx), uy = __ldg(gdy + idx);
+      p.rg_index[oi + pos] = idx;
+      p.rg_type[oi + pos] = __ldg(gt + idx);
+      feat[pos] = fmaf(cs, dx, sn * dy);
+      feat[k + pos] = fmaf(cs, dy, -sn * dx);
+      feat[2 * (int64_t)k + pos] = fmaf(cs, ux, sn * uy);
+      feat[3 * (int64_t)k + pos] = fmaf(cs, uy, -sn * ux);
+      ++pos;
+    }
+  }
+  pad_from(n_out);
 }
 
 cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_roadgraph& rg, int t,
@@ -375,18 +437,18 @@ cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_ro
   TopkParams p;
   p.row = wm_make_row(sim, t);
   p.A = sim.A; p.R = rg.R; p.k = h->cfg.topk;
-  p.pts = h->pts; p.pts_pad = h->pts_pad;
-  p.dir_x = rg.dir_x; p.dir_y = rg.dir_y; p.type = rg.type;
+  p.pt_xy = h->pt_xy; p.pt_idx = h->pt_idx; p.pt_start = h->pt_start; p.pt_grid = h->pt_grid;
+  p.x = rg.x; p.y = rg.y; p.dir_x = rg.dir_x; p.dir_y = rg.dir_y; p.type = rg.type;
   p.rg_index = rg_index; p.rg_feat = rg_feat; p.rg_type = rg_type;
-  const size_t smem = 128 + 2 * (size_t)WM_PT_TILE * 8 + (size_t)TK_WARPS * TK_BINS * 32 * 2;
-  static bool configured = false;
-  if (!configured) {
+  const size_t smem = 2 * (size_t)((rg.R + 31) / 32) * sizeof(uint32_t);
+  if (smem > 200 * 1024) return cudaErrorInvalidValue;       // R > 819 200 points per scenario
+  static size_t configured = 0;
+  if (smem > 40 * 1024 && smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(k_observe_topk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = true;
+    configured = smem;
   }
-  dim3 grid((sim.A + TK_WARPS - 1) / TK_WARPS, sim.B);
-  k_observe_topk<<<grid, TK_THREADS, smem, s>>>(p);
+  k_observe_topk<<<dim3(sim.A, sim.B), TK_THREADS, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
 }

@@ -170,22 +170,12 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
   }
 }
 
-// packed copy of the roadgraph points for the top-k observation
-__global__ void __launch_bounds__(256) k_pack_points(RgView g, int pts_pad, float2* pts) {
-  const int64_t o = (int64_t)blockIdx.y * g.R;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= pts_pad) return;
-  float2 v = make_float2(WM_FAR, WM_FAR);
-  if (i < g.R && g.valid[o + i] != 0) v = make_float2(g.x[o + i], g.y[o + i]);
-  pts[(int64_t)blockIdx.y * pts_pad + i] = v;
-}
-
 void wm_prepare_free(wm_handle* h) {
-  cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pts);
+  cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pt_xy); cudaFree(h->pt_idx); cudaFree(h->pt_start); cudaFree(h->pt_grid);
   cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->segfin); cudaFree(h->chunks); cudaFree(h->gridp); cudaFree(h->cells); cudaFree(h->pool); cudaFree(h->pool_cnt);
-  h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pts = nullptr;
+  h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pt_xy = nullptr; h->pt_idx = nullptr; h->pt_start = nullptr; h->pt_grid = nullptr;
   h->segrec = nullptr; h->segpair = nullptr; h->segfin = nullptr; h->chunks = nullptr; h->gridp = nullptr; h->cells = nullptr; h->pool = nullptr; h->pool_cnt = nullptr;
-  h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0; h->pts_pad = 0;
+  h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0;
 }
 
 // Step 1 of wm_prepare: per-scenario record counts (needs type, id, valid only), the capacity they
@@ -199,8 +189,10 @@ int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_m
     wm_drop_graph(h);
     wm_prepare_free(h);
     WM_CUDA(cudaMalloc(&h->n_seg, (size_t)B * sizeof(int32_t)));
-    h->pts_pad = (R + WM_PT_TILE - 1) / WM_PT_TILE * WM_PT_TILE;
-    WM_CUDA(cudaMalloc(&h->pts, (size_t)B * h->pts_pad * sizeof(float2)));
+    WM_CUDA(cudaMalloc(&h->pt_xy, (size_t)B * R * sizeof(float2)));
+    WM_CUDA(cudaMalloc(&h->pt_idx, (size_t)B * R * sizeof(int32_t)));
+    WM_CUDA(cudaMalloc(&h->pt_start, (size_t)B * (WM_PT_CELLS + 1) * sizeof(int32_t)));
+    WM_CUDA(cudaMalloc(&h->pt_grid, (size_t)B * sizeof(WmPtGrid)));
     WM_CUDA(cudaMalloc(&h->gridp, (size_t)B * sizeof(WmGrid)));
     WM_CUDA(cudaMalloc(&h->cells, (size_t)B * WM_GRID_CELLS * sizeof(uint2)));
     WM_CUDA(cudaMalloc(&h->pool, (size_t)B * WM_POOL_CAP * sizeof(uint32_t)));
@@ -261,9 +253,7 @@ int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaS
   h->launches++;
   WM_CUDA(cudaGetLastError());
   WM_CUDA(wm_launch_build_grid(h, b0, nb, s));
-  k_pack_points<<<dim3((h->pts_pad + 255) / 256, nb), 256, 0, s>>>(g, h->pts_pad, h->pts + (int64_t)b0 * h->pts_pad);
-  h->launches++;
-  WM_CUDA(cudaGetLastError());
+  WM_CUDA(wm_launch_point_grid(h, *rg, b0, nb, s));
   return WM_OK;
 }
 
