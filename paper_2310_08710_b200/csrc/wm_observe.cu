@@ -261,12 +261,13 @@ __device__ __forceinline__ void tk_locate(TkShared& S, int need, bool level0) {
 }
 
 __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
-  extern __shared__ __align__(16) uint32_t s_bits[];     // [2][Wd]: key < T; key == T (ties)
+  extern __shared__ __align__(16) uint32_t s_bits[];     // [2][Wd]: key < T; key == T (ties); then [k] indices
   __shared__ TkShared S;
   const int b = blockIdx.y, ego = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int A = p.A, k = p.k, R = p.R, Wd = (R + 31) >> 5;
   uint32_t* bm = s_bits;
   uint32_t* tb = s_bits + Wd;
+  int* list = (int*)(s_bits + 2 * Wd);                    // [k] selected indices, ascending
   const int64_t ro = (int64_t)b * p.row.stride_b;
   const int64_t oi = ((int64_t)b * A + ego) * k;          // rg_index / rg_type row
   float* feat = p.rg_feat + ((int64_t)b * A + ego) * 4 * k;
@@ -299,8 +300,17 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
   };
   if (warp == 0) {                                        // 0. the first square: ~1.35 k points
     const int want = min(g.nvalid, kk + (kk * 35) / 100);
-    int m = 0, c = 0;
-    for (;; ++m) { c = square_count(m); if (c >= want || m >= WM_PT_NG) break; }
+    // lanes over m = 0..31 (independent loads), then one m at a time
+    int c = 0;
+    {
+      const int m = lane;
+      const int i0 = max(ci - m, 0), i1 = min(ci + m, g.nx - 1), j0 = max(cj - m, 0), j1 = min(cj + m, g.ny - 1);
+      for (int j = j0; j <= j1; ++j) c += __ldg(start + j * g.nx + i1 + 1) - __ldg(start + j * g.nx + i0);
+    }
+    const uint32_t ok = __ballot_sync(0xffffffffu, c >= want);
+    int m = ok ? __ffs(ok) - 1 : 32;
+    c = __shfl_sync(0xffffffffu, c, m & 31);
+    if (!ok) for (;; ++m) { c = square_count(m); if (c >= want || m >= WM_PT_NG) break; }
     if (lane == 0) { S.m = m; S.count = c; }
   }
   for (int i = tid; i < 2 * Wd; i += TK_THREADS) s_bits[i] = 0u;
@@ -342,32 +352,32 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
       if (warp == 0) tk_locate(S, kk - S.c_less, false);
       __syncthreads();
     }
-    // ---- 2. collect the bin, exact threshold by bitwise descent ----
-    const uint32_t lo = S.lo, hi = S.hi;
-    const bool single = S.in_bin > TK_CAP;                // one key value with more than TK_CAP ties
-    if (!single) for_square([&](uint32_t key, int s) {
-      if (key >= lo && key < hi) { const int q = atomicAdd(&S.n_col, 1); if (q < TK_CAP) S.col[q] = make_uint2(key, (uint32_t)s); }
-    });
-    __syncthreads();
-    if (warp == 0) {
-      int r = kk - S.c_less;                              // 1-based rank inside [lo, hi)
-      uint32_t T = lo;
-      if (!single) {
-        const int n_col = min(S.n_col, TK_CAP);
-        uint32_t pfx = 0, mask = 0;
-        const uint32_t diff = lo ^ (hi - 1u);
-        const int top = diff ? 31 - __clz(diff) : -1;     // bits above `top` are common to the range
-        if (top < 31) { mask = ~((top >= 0 ? (2u << top) : 1u) - 1u); pfx = lo & mask; }
-        for (int bit = top; bit >= 0; --bit) {
-          const uint32_t m2 = mask | (1u << bit);
-          int c0 = 0;
-          for (int i = lane; i < n_col; i += 32) c0 += ((S.col[i].x & m2) == pfx) ? 1 : 0;
-          c0 = __reduce_add_sync(0xffffffffu, c0);
-          if (r > c0) { r -= c0; pfx |= 1u << bit; }
-          mask = m2;
-        }
-        T = pfx;
+    // ---- 2. collect the bin, then narrow [lo, hi) to one key value on the collected pairs ----
+    {
+      const uint32_t lo = S.lo, hi = S.hi;
+      if (S.in_bin <= TK_CAP && hi - lo > 1u) for_square([&](uint32_t key, int s) {
+        if (key >= lo && key < hi) { const int q = atomicAdd(&S.n_col, 1); if (q < TK_CAP) S.col[q] = make_uint2(key, (uint32_t)s); }
+      });
+      __syncthreads();
+    }
+    while (S.hi - S.lo > 1u) {                            // in_bin <= TK_CAP here: all of the range is in col
+      const uint32_t lo = S.lo, hi = S.hi;
+      const int shift = max(0, 32 - __clz(hi - lo - 1u) - 8), n_col = min(S.n_col, TK_CAP);
+      __syncthreads();
+      for (int i = tid; i < TK_BINS; i += TK_THREADS) S.hist[i] = 0u;
+      if (tid == 0) S.shift = shift;
+      __syncthreads();
+      for (int i = tid; i < n_col; i += TK_THREADS) {
+        const uint32_t key = S.col[i].x;
+        if (key >= lo && key < hi) atomicAdd(&S.hist[(key - lo) >> shift], 1u);
       }
+      __syncthreads();
+      if (warp == 0) tk_locate(S, kk - S.c_less, false);
+      __syncthreads();
+    }
+    if (warp == 0) {
+      const uint32_t T = S.lo;                            // the kk-th key; ties to take, in index order:
+      const int r = kk - S.c_less;
       // ---- 3. is the square large enough? ----
       const int m = S.m;
       const bool all = S.count >= g.nvalid;
@@ -394,40 +404,53 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
     if (key <= T) { const int idx = __ldg(pidx + s); atomicOr((key < T ? bm : tb) + (idx >> 5), 1u << (idx & 31)); }
   });
   __syncthreads();
-  const int wpt = (Wd + TK_THREADS - 1) / TK_THREADS, w0 = min(tid * wpt, Wd), w1 = min(w0 + wpt, Wd);
+  // Words are dealt round-robin (word r * 128 + tid in round r): the selected points cluster in index
+  // ranges (polylines near the ego), and this spreads a cluster over all threads.
+  const int rounds = (Wd + TK_THREADS - 1) / TK_THREADS;
   {                                                       // the first `quota` ties in index order
     int c = 0, total;
-    for (int w = w0; w < w1; ++w) c += __popc(tb[w]);
-    int left = S.quota - tk_block_scan(c, S.scan, total);
-    for (int w = w0; w < w1; ++w) {
-      uint32_t t = tb[w];
-      const int n = __popc(t);
-      if (left < n) { for (int drop = n - max(left, 0); drop > 0; --drop) t &= ~(0x80000000u >> __clz(t)); }   // keep the lowest bits
-      left -= n;
-      bm[w] |= t;
+    for (int w = tid; w < Wd; w += TK_THREADS) c += __popc(tb[w]);
+    tk_block_scan(c, S.scan, total);
+    const int quota = S.quota;
+    if (total <= quota) { for (int w = tid; w < Wd; w += TK_THREADS) bm[w] |= tb[w]; }
+    else {
+      int base = 0;
+      for (int r = 0; r < rounds; ++r) {
+        const int w = r * TK_THREADS + tid;
+        uint32_t t = w < Wd ? tb[w] : 0u;
+        const int n = __popc(t);
+        int tot_r;
+        const int left = quota - (base + tk_block_scan(n, S.scan, tot_r));
+        if (left < n) { for (int drop = n - max(left, 0); drop > 0; --drop) t &= ~(0x80000000u >> __clz(t)); }   // keep the lowest bits
+        if (w < Wd) bm[w] |= t;
+        base += tot_r;
+      }
     }
   }
-  // ---- 5. emit in ascending index order ----
-  int c = 0, n_out;
-  for (int w = w0; w < w1; ++w) c += __popc(bm[w]);
-  int pos = tk_block_scan(c, S.scan, n_out);
+  // ---- 5. the set bits in ascending index order -> list, then features with coalesced stores ----
+  int n_out = 0;
+  for (int r = 0; r < rounds; ++r) {
+    const int w = r * TK_THREADS + tid;
+    uint32_t bits = w < Wd ? bm[w] : 0u;
+    int tot_r;
+    int pos = n_out + tk_block_scan(__popc(bits), S.scan, tot_r);
+    while (bits) { if (pos < k) list[pos] = w * 32 + __ffs(bits) - 1; ++pos; bits &= bits - 1; }
+    n_out += tot_r;
+  }
+  __syncthreads();
+  n_out = min(n_out, k);
   const float *gx = p.x + (int64_t)b * R, *gy = p.y + (int64_t)b * R, *gdx = p.dir_x + (int64_t)b * R, *gdy = p.dir_y + (int64_t)b * R;
   const int32_t* gt = p.type + (int64_t)b * R;
-  for (int w = w0; w < w1; ++w) {
-    uint32_t bits = bm[w];
-    while (bits) {
-      const int idx = w * 32 + __ffs(bits) - 1;
-      bits &= bits - 1;
-      const float dx = __fsub_rn(__ldg(gx + idx), ex), dy = __fsub_rn(__ldg(gy + idx), ey);
-      const float ux = __ldg(gdx + idx), uy = __ldg(gdy + idx);
-      p.rg_index[oi + pos] = idx;
-      p.rg_type[oi + pos] = __ldg(gt + idx);
-      feat[pos] = fmaf(cs, dx, sn * dy);
-      feat[k + pos] = fmaf(cs, dy, -sn * dx);
-      feat[2 * (int64_t)k + pos] = fmaf(cs, ux, sn * uy);
-      feat[3 * (int64_t)k + pos] = fmaf(cs, uy, -sn * ux);
-      ++pos;
-    }
+  for (int j = tid; j < n_out; j += TK_THREADS) {
+    const int idx = list[j];
+    const float dx = __fsub_rn(__ldg(gx + idx), ex), dy = __fsub_rn(__ldg(gy + idx), ey);
+    const float ux = __ldg(gdx + idx), uy = __ldg(gdy + idx);
+    p.rg_index[oi + j] = idx;
+    p.rg_type[oi + j] = __ldg(gt + idx);
+    feat[j] = fmaf(cs, dx, sn * dy);
+    feat[k + j] = fmaf(cs, dy, -sn * dx);
+    feat[2 * (int64_t)k + j] = fmaf(cs, ux, sn * uy);
+    feat[3 * (int64_t)k + j] = fmaf(cs, uy, -sn * ux);
   }
   pad_from(n_out);
 }
@@ -440,7 +463,7 @@ cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_ro
   p.pt_xy = h->pt_xy; p.pt_idx = h->pt_idx; p.pt_start = h->pt_start; p.pt_grid = h->pt_grid;
   p.x = rg.x; p.y = rg.y; p.dir_x = rg.dir_x; p.dir_y = rg.dir_y; p.type = rg.type;
   p.rg_index = rg_index; p.rg_feat = rg_feat; p.rg_type = rg_type;
-  const size_t smem = 2 * (size_t)((rg.R + 31) / 32) * sizeof(uint32_t);
+  const size_t smem = (2 * (size_t)((rg.R + 31) / 32) + (size_t)h->cfg.topk) * sizeof(uint32_t);
   if (smem > 200 * 1024) return cudaErrorInvalidValue;       // R > 819 200 points per scenario
   static size_t configured = 0;
   if (smem > 40 * 1024 && smem > configured) {
