@@ -185,7 +185,7 @@ def run_supplementary(args):
         ms_k = timed(lambda: wm.wm_observe(h, log_d, rg_d, t, None, None, idx, feat, typ), K, W)
         egos = int(log["valid"][:, t].sum())
         out_bytes = sum(x.numel() * x.element_size() for x in (hist, hv, idx, feat, typ))
-        in_bytes = B * rg["x"].shape[1] * 8 + B * H * A * 29
+        in_bytes = B * rg["x"].shape[1] * 8 + B * H * A * 29      # point coordinates once + the H rows
         # oracle sample: 2 scenarios
         sb = 2
         sub = lambda d: {q: np.ascontiguousarray(v[:sb]) for q, v in d.items()}
@@ -203,7 +203,7 @@ def run_supplementary(args):
                              "kernel": "k_observe_hist + k_observe_topk", "algorithmic_bytes": out_bytes + in_bytes,
                              "history_frac": (hist.numel() * 4 + hv.numel() + B * H * A * 29) / (ms_h * 1e-3) / 1e9 / hbm_peak,
                              "topk_frac": (out_bytes - hist.numel() * 4 - hv.numel() + B * rg["x"].shape[1] * 8) / (ms_k * 1e-3) / 1e9 / hbm_peak,
-                             "note": "top-k is ALU/shared-memory bound (3 passes over R per ego), see DESIGN.md"},
+                             "note": "top-k: one CTA per ego selects inside a square of point-grid cells; instruction-issue bound, see DESIGN.md"},
                 "cpu_baseline": {"value": sb * A / dt, "unit": "ego-observations/s", "cores": oracle.num_threads(), "kind": "oracle",
                                  "sample": "first %d of %d scenarios, %.1f s wall" % (sb, B, dt), "index_sets_equal": same},
                 "e2e": None, "gpu_launches": int(launches), "clocks": None}

@@ -8,7 +8,7 @@
 // k_observe_topk: exact top-k on the float32 key d2 = fma(dy,dy,dx*dx) (the bit pattern of a
 // non-negative float is order preserving; DESIGN.md R-topk).  wm_prepare buckets the valid points of
 // a scenario into a uniform grid (k_point_grid).  One 128-thread CTA per ego:
-//   0. the square of cells around the ego's cell that holds ~1.35 k points (cell counts only);
+//   0. the square of cells around the ego's cell that holds ~1.6 k points (cell counts only);
 //   1. histogram of the keys' top bits over the points of that square (shared-memory atomics)
 //      -> bin of the k-th key (repeated on the bin's sub-range only if the bin is too large);
 //   2. collect the (key, index) pairs of that bin (<= 512) -> bitwise descent gives the exact k-th
@@ -298,8 +298,8 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
     for (int j = j0 + lane; j <= j1; j += 32) c += __ldg(start + j * g.nx + i1 + 1) - __ldg(start + j * g.nx + i0);
     return __reduce_add_sync(0xffffffffu, c);
   };
-  if (warp == 0) {                                        // 0. the first square: ~1.35 k points
-    const int want = min(g.nvalid, kk + (kk * 35) / 100);
+  if (warp == 0) {                                        // 0. the first square: ~1.6 k points
+    const int want = min(g.nvalid, kk + (kk * 60) / 100);
     // lanes over m = 0..31 (independent loads), then one m at a time
     int c = 0;
     {
