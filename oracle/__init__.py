@@ -177,3 +177,25 @@ def rollout(log, sim, rg, t0, n_steps, dynamics, actions, action_valid, dt=0.1, 
                       _p(out["offroad_dist"]), _p(out["log_div"]), _p(out["any_overlap"]),
                       _p(out["any_offroad"]), _p(out["ade"]))
     return out
+
+
+def expert_actions(tr, t, n_steps, dynamics, dt=0.1):
+    """O9: inverse kinematics on rows t+s, t+s+1 (L335 / Eq. 3). action [B][n_steps][C][A]."""
+    ts, (B, T, A) = _traj(tr)
+    Cn = 2 if dynamics == DYN_BICYCLE else 3
+    act = np.empty((B, n_steps, Cn, A), np.float32); val = np.empty((B, n_steps, A), np.uint8)
+    den = np.empty((B, n_steps, A), np.float64)
+    lib().orc_expert_actions(C.byref(ts), C.c_int32(t), C.c_int32(n_steps), C.c_int32(dynamics), C.c_double(dt),
+                             _p(act), _p(val), _p(den))
+    return dict(action=act, valid=val, kden=den)
+
+
+def kinematic(tr, t, n_steps=1, dt=0.1, max_accel=6.0, max_curvature=0.3):
+    """O10: kinematic infeasibility of the transitions into rows t..t+n_steps-1 (L104)."""
+    ts, (B, T, A) = _traj(tr)
+    shp = (B, n_steps, A)
+    acc = np.empty(shp, np.float32); cur = np.empty(shp, np.float32); den = np.empty(shp, np.float64)
+    flag = np.empty(shp, np.uint8); val = np.empty(shp, np.uint8)
+    lib().orc_kinematic(C.byref(ts), C.c_int32(t), C.c_int32(n_steps), C.c_double(dt), C.c_double(max_accel),
+                        C.c_double(max_curvature), _p(acc), _p(cur), _p(den), _p(flag), _p(val))
+    return dict(accel=acc, curvature=cur, kden=den, flag=flag, valid=val)

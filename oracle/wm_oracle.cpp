@@ -3,7 +3,7 @@
 //
 // A plain, slow, scalar CPU restatement of what the Waymax closed-loop step computes
 // (arXiv 2310.08710; citations are PAPER.md line numbers + section/equation, and the
-// DESIGN.md reading numbers D1..D27 where the paper is silent).  Arithmetic is double
+// DESIGN.md reading numbers D1..D32 where the paper is silent).  Arithmetic is double
 // precision; inputs and outputs are the float32 / uint8 / int32 arrays the CUDA library
 // sees, and state is rounded to float32 at each step boundary.  It shares no code, header,
 // table or helper with paper_2310_08710_b200/csrc; only tests/, __graft_entry__.smoke()
@@ -459,6 +459,90 @@ void orc_rollout(const orc_traj* log, orc_traj* sim, const orc_roadgraph* rg, in
   }
   if (ade)
     for (size_t i = 0; i < BA; ++i) ade[i] = cnt[i] ? (float)(sum[i] / cnt[i]) : 0.f;
+}
+
+// -------------------------------------------------------------------------------------
+// O9 expert actor = inverse kinematics on two consecutive rows ("Expert";
+// L335 delta inverse; L352-L359 Eq. 3 bicycle inverse).  Steps s = 0..n_steps-1 use rows
+// t+s and t+s+1 of `tr`.  Output action [B][n_steps][C][A], valid [B][n_steps][A] = both rows
+// valid; invalid -> action 0.
+//   bicycle (Eq. 3):  a = (v' - v) / dt,  v = sqrt(vx^2 + vy^2)
+//                     kappa = wrap(atan2(vy', vx') - theta) / (v dt + a dt^2 / 2)
+//     D4: the heading is atan2(v_y', v_x') (the paper's "arctan v_x'/v_y'" is garbled);
+//     D32: the heading difference is wrapped into [-pi, pi) (yaw is not wrapped in step, D5);
+//     D31: kappa = 0 when the float32 speeds v and v' are both exactly 0 (denominator 0).
+//   delta (L335) in the body frame of row t+s (D2): (dx, dy) = R(-theta) (p' - p), dyaw = theta' - theta.
+// `kden` (may be NULL, bicycle only): the denominator of kappa, for the test tolerances.
+// -------------------------------------------------------------------------------------
+static double orc_wrap_pi(double a) {
+  const double two_pi = 6.283185307179586476925286766559;
+  a = std::fmod(a + 3.14159265358979323846, two_pi);
+  if (a < 0) a += two_pi;
+  return a - 3.14159265358979323846;
+}
+
+static void inverse_bicycle(const orc_traj* tr, size_t i0, size_t i1, double dt, double* a_out, double* k_out, double* den_out) {
+  const double vx = tr->vel_x[i0], vy = tr->vel_y[i0], vx1 = tr->vel_x[i1], vy1 = tr->vel_y[i1];
+  const double v = std::sqrt(vx * vx + vy * vy), v1 = std::sqrt(vx1 * vx1 + vy1 * vy1);
+  const double a = (v1 - v) / dt;                                   // Eq. 3
+  const double den = v * dt + 0.5 * a * dt * dt;                    // L358
+  double kappa = 0.0;
+  if (!(v == 0.0 && v1 == 0.0)) kappa = orc_wrap_pi(std::atan2(vy1, vx1) - (double)tr->yaw[i0]) / den;   // D4, D31, D32
+  *a_out = a; *k_out = kappa; *den_out = den;
+}
+
+void orc_expert_actions(const orc_traj* tr, int32_t t, int32_t n_steps, int32_t dynamics, double dt, float* action,
+                        uint8_t* valid, double* kden) {
+  const int B = tr->B, A = tr->A;
+  const int C = dynamics == ORC_DYN_BICYCLE ? 2 : 3;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b)
+    for (int s = 0; s < n_steps; ++s)
+      for (int a = 0; a < A; ++a) {
+        const size_t i0 = row(tr, b, t + s) + a, i1 = row(tr, b, t + s + 1) + a;
+        const size_t o = (((size_t)b * n_steps + s) * C) * A + a, ov = ((size_t)b * n_steps + s) * A + a;
+        const bool v = tr->valid[i0] != 0 && tr->valid[i1] != 0;
+        valid[ov] = (uint8_t)v;
+        for (int c = 0; c < C; ++c) action[o + (size_t)c * A] = 0.f;
+        if (kden) kden[ov] = 0.0;
+        if (!v) continue;
+        if (dynamics == ORC_DYN_BICYCLE) {
+          double acc, kap, den;
+          inverse_bicycle(tr, i0, i1, dt, &acc, &kap, &den);
+          action[o] = (float)acc; action[o + A] = (float)kap;
+          if (kden) kden[ov] = den;
+        } else {
+          const double th = tr->yaw[i0], cs = std::cos(th), sn = std::sin(th);
+          const double Dx = (double)tr->x[i1] - (double)tr->x[i0], Dy = (double)tr->y[i1] - (double)tr->y[i0];   // L335
+          action[o] = (float)(cs * Dx + sn * Dy);                   // body frame (D2)
+          action[o + A] = (float)(-sn * Dx + cs * Dy);
+          action[o + 2 * (size_t)A] = (float)((double)tr->yaw[i1] - th);
+        }
+      }
+}
+
+// -------------------------------------------------------------------------------------
+// O10 kinematic infeasibility: Eq. 3 on rows t+s-1 -> t+s, s = 0..n_steps-1;
+// flag = |a| > max_accel or |kappa| > max_curvature (6 m/s^2, 0.3 1/m), strictly.
+// Outputs [B][n_steps][A]; valid = both rows valid, otherwise 0 / flag 0.
+// -------------------------------------------------------------------------------------
+void orc_kinematic(const orc_traj* tr, int32_t t, int32_t n_steps, double dt, double max_accel, double max_curvature,
+                   float* accel, float* curvature, double* kden, uint8_t* flag, uint8_t* valid) {
+  const int B = tr->B, A = tr->A;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b)
+    for (int s = 0; s < n_steps; ++s)
+      for (int a = 0; a < A; ++a) {
+        const size_t i0 = row(tr, b, t + s - 1) + a, i1 = row(tr, b, t + s) + a;
+        const size_t o = ((size_t)b * n_steps + s) * A + a;
+        const bool v = tr->valid[i0] != 0 && tr->valid[i1] != 0;
+        double acc = 0.0, kap = 0.0, den = 0.0;
+        if (v) inverse_bicycle(tr, i0, i1, dt, &acc, &kap, &den);
+        accel[o] = (float)acc; curvature[o] = (float)kap;
+        if (kden) kden[o] = den;
+        flag[o] = (uint8_t)(v && (std::fabs(acc) > max_accel || std::fabs(kap) > max_curvature));
+        valid[o] = (uint8_t)v;
+      }
 }
 
 int32_t orc_num_threads() {
