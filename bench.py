@@ -144,7 +144,8 @@ def run_reference(args):
 
 def run_supplementary(args):
     """Supplementary lines for the other hot-path rows: config 3 observation (a6, a7), config 2
-    single DeltaLocal step + metrics (a2-a5), config 4 overlap-dense stress (a3, a4).  N=1 only."""
+    single DeltaLocal step + metrics (a2-a5), config 4 overlap-dense stress (a3, a4), RolloutExpert
+    on config 5 (expert actor + kinematic metric).  N=1 only."""
     import torch
     import oracle
     import wm_scenarios as ws
@@ -206,6 +207,61 @@ def run_supplementary(args):
                              "note": "top-k: one CTA per ego selects inside a square of point-grid cells; instruction-issue bound, see DESIGN.md"},
                 "cpu_baseline": {"value": sb * A / dt, "unit": "ego-observations/s", "cores": oracle.num_threads(), "kind": "oracle",
                                  "sample": "first %d of %d scenarios, %.1f s wall" % (sb, B, dt), "index_sets_equal": same},
+                "e2e": None, "gpu_launches": int(launches), "clocks": None}
+    elif args.workload == "expert":
+        # RolloutExpert (Table 2): expert actions from the log by inverse kinematics, the
+        # 80-step rollout with them, then the kinematic-infeasibility metric of the simulated rows (L104)
+        cfg = ws.make_config(5, B=args.B, n_steps=N_STEPS)
+        log, rg = cfg["log"], cfg["roadgraph"]
+        B, T, A = log["x"].shape
+        h = wm.wm_create()
+        log_d, rg_d = wm.to_device(log), wm.to_device(rg)
+        wm.wm_prepare(h, rg_d)
+        sim_d = wm.empty_traj_like(log_d)
+        out_d = wm.alloc_rollout_out(B, N_STEPS, A)
+        act = torch.empty((B, N_STEPS, 2, A), device="cuda"); av = torch.empty((B, N_STEPS, A), dtype=torch.uint8, device="cuda")
+        kacc = torch.empty((B, N_STEPS, A), device="cuda"); kcur = torch.empty((B, N_STEPS, A), device="cuda")
+        kfl = torch.empty((B, N_STEPS, A), dtype=torch.uint8, device="cuda")
+
+        def fn():
+            wm.wm_expert_actions(h, log_d, 10, N_STEPS, act, av)
+            t0 = wm.wm_reset(h, log_d, sim_d)
+            wm.wm_rollout(h, log_d, sim_d, t0, N_STEPS, act, av, out_d)
+            wm.wm_metrics_kinematic(h, sim_d, t0 + 1, N_STEPS, kacc, kcur, kfl)
+        l0 = wm.wm_kernel_launches(h)
+        ms = timed(fn, K, W)
+        launches = (wm.wm_kernel_launches(h) - l0) * K // (K + W)
+        ms_e = timed(lambda: wm.wm_expert_actions(h, log_d, 10, N_STEPS, act, av), K, W)
+        ms_k = timed(lambda: wm.wm_metrics_kinematic(h, sim_d, 11, N_STEPS, kacc, kcur, kfl), K, W)
+        n_as = float(B) * A * N_STEPS
+        inv_bytes = n_as * (13 + 9) + n_as * (13 + 9)            # per agent-step: one new row of (yaw, vx, vy, valid) in, 9 B out; twice
+        sb = min(64, B)
+        sub = lambda d: {q: np.ascontiguousarray(v[:sb]) for q, v in d.items()}
+        t0c = time.perf_counter()
+        e = oracle.expert_actions(sub(log), 10, N_STEPS, oracle.DYN_BICYCLE)
+        sim_o = oracle.reset(sub(log))
+        oo = oracle.rollout(sub(log), sim_o, sub(rg), 10, N_STEPS, oracle.DYN_BICYCLE, e["action"], e["valid"])
+        ko = oracle.kinematic(sim_o, 11, N_STEPS)
+        dt = time.perf_counter() - t0c
+        # flag agreement, teacher-forced: the oracle's metric on the GPU's own rows, outside the tolerance band
+        kt = oracle.kinematic({q: v[:sb].cpu().numpy() for q, v in sim_d.items()}, 11, N_STEPS)
+        tol_k = 1e-5 * np.abs(kt["curvature"]) + 4e-6 / np.maximum(kt["kden"], 1e-12) + 1e-6
+        band = (np.abs(np.abs(kt["accel"]) - 6.0) <= 1e-3) | (np.abs(np.abs(kt["curvature"]) - 0.3) <= tol_k)
+        clean = (kt["valid"] == 1) & ~band
+        line = {"metric": "agent-steps/s, RolloutExpert (expert actions by inverse kinematics + 80-step rollout + kinematic infeasibility), config 5",
+                "value": n_as / (ms * 1e-3), "unit": "agent-steps/s", "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "config5 RolloutExpert: B=%d A=%d R=%d T=%d" % (B, A, rg["x"].shape[1], T), "ms_expert_actions": ms_e,
+                           "ms_kinematic_metric": ms_k, "ms_reset_plus_rollout": ms - ms_e - ms_k, "l2": "working set 6 GB exceeds L2",
+                           "mean_ade_m": float(out_d["ade"].mean().item()), "kinematic_flag_rate": float(kfl.float().mean().item()),
+                           "paper_context": "Table 2 L153: RolloutExpert 73.3 ms at BS 1 on a V100 (all six metrics, WOMD)"},
+                "roofline": {"bound": "hbm", "achieved": inv_bytes / ((ms_e + ms_k) * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": inv_bytes / ((ms_e + ms_k) * 1e-3) / 1e9 / hbm_peak, "traffic": None, "kernel": "k_inverse<false> + k_inverse<true>",
+                             "algorithmic_bytes": inv_bytes, "note": "the rollout kernel itself: see the default workload"},
+                "cpu_baseline": {"value": sb * A * N_STEPS / dt, "unit": "agent-steps/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                 "sample": "first %d of %d scenarios, %.1f s wall" % (sb, B, dt),
+                                 "kinematic_flags_equal_outside_band": bool(np.array_equal(kt["flag"][clean], kfl[:sb].cpu().numpy()[clean])),
+                                 "transitions_in_band": int(((kt["valid"] == 1) & band).sum()), "transitions": int((kt["valid"] == 1).sum())},
                 "e2e": None, "gpu_launches": int(launches), "clocks": None}
     else:
         cid = 2 if args.workload == "step2" else 4
@@ -285,7 +341,7 @@ def main():
     ap.add_argument("--cpu-B", type=int, default=256, help="oracle sample for cpu_baseline (256 scenarios: ~15 s on 16 cores)")
     ap.add_argument("--ref-B", type=int, default=64, help="oracle sample per step of --impl reference (~4 s on 16 cores)")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4"],
+    ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4", "expert"],
                     help="rollout = the BASELINE metric (config 5, default); the others time the remaining "
                          "SURVEY 8(a) rows on configs 3, 2, 4 (supplementary lines, same JSON shape)")
     ap.add_argument("--no-e2e", action="store_true")

@@ -178,6 +178,32 @@ int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t
                void* stream);
 
 /*
+ * Expert actor = inverse kinematics on the rows of a trajectory ("Expert"; L335 delta
+ * inverse; L352-L359 Eq. 3 bicycle inverse), for the dynamics model of the handle.  Step s =
+ * 0 .. n_steps-1 uses rows t+s and t+s+1 of `tr`:
+ *   bicycle: a = (v' - v)/dt, v = |(vx, vy)|; kappa = wrap(atan2(vy', vx') - yaw) / (v dt + a dt^2/2)
+ *            (heading atan2(vy', vx'): D4; difference wrapped into [-pi, pi): D32; kappa = 0 when
+ *            v and v' are both exactly 0: D31);
+ *   delta:   (dx, dy) = R(-yaw)(p' - p) in the body frame of row t+s (D2), dyaw = yaw' - yaw.
+ * action [B][n_steps][C][A] (the layout wm_rollout takes; n_steps = 1: what wm_step takes),
+ * action_valid [B][n_steps][A] = both rows valid; action = 0 where not valid.  Replaying the
+ * DeltaLocal expert of the log reproduces the log (Table 3: Log ADE 0.00).
+ * Requires t >= 0, t + n_steps < T.
+ */
+int wm_expert_actions(wm_handle* h, const wm_traj* tr, int32_t t, int32_t n_steps, float* action,
+                      uint8_t* action_valid, void* stream);
+
+/*
+ * Kinematic-infeasibility metric, L104: Eq. 3 on the transitions INTO rows t .. t+n_steps-1 (row
+ * t+s-1 -> t+s), whatever the dynamics model of the handle; flag = |a| > max_accel or |kappa| >
+ * max_curvature of the config (6 m/s^2, 0.3 1/m), strictly.  accel, curvature (may be NULL), flag
+ * [B][n_steps][A]; a transition with an invalid end gives 0 / 0 / flag 0.  Requires t >= 1,
+ * t + n_steps <= T.  (L198: actions of the bicycle model inside the limits are never flagged.)
+ */
+int wm_metrics_kinematic(wm_handle* h, const wm_traj* sim, int32_t t, int32_t n_steps, float* accel,
+                         float* curvature, uint8_t* flag, void* stream);
+
+/*
  * Rollout, L200: for s = 0 .. n_steps-1: wm_step at t0+s, then overlap, offroad and log
  * divergence on row t0+s+1 (D11), written to row s of the per-step outputs; aggregates over
  * the n_steps rows at the end.  The whole sequence is one CUDA graph, captured on the first

@@ -23,7 +23,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
+           "wm_expert_actions", "wm_metrics_kinematic", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
 
 
 class wm_traj(C.Structure):
@@ -174,6 +174,18 @@ def wm_log_divergence(h, log, sim, t, dist, valid, stream=None):
     ls, ss = traj_struct(log), traj_struct(sim)
     _check(load().wm_log_divergence(h, C.byref(ls), C.byref(ss), C.c_int32(t), _ptr(dist, torch.float32),
                                     _ptr(valid, torch.uint8), _stream(stream)), "wm_log_divergence")
+
+
+def wm_expert_actions(h, tr, t, n_steps, action, action_valid, stream=None):
+    ts = traj_struct(tr)
+    _check(load().wm_expert_actions(h, C.byref(ts), C.c_int32(t), C.c_int32(n_steps), _ptr(action, torch.float32),
+                                    _ptr(action_valid, torch.uint8), _stream(stream)), "wm_expert_actions")
+
+
+def wm_metrics_kinematic(h, sim, t, n_steps, accel, curvature, flag, stream=None):
+    ss = traj_struct(sim)
+    _check(load().wm_metrics_kinematic(h, C.byref(ss), C.c_int32(t), C.c_int32(n_steps), _ptr(accel, torch.float32),
+                                       _ptr(curvature, torch.float32), _ptr(flag, torch.uint8), _stream(stream)), "wm_metrics_kinematic")
 
 
 def wm_observe(h, sim, rg, t, hist=None, hist_valid=None, rg_index=None, rg_feat=None, rg_type=None, stream=None):

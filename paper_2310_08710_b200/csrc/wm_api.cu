@@ -163,6 +163,23 @@ extern "C" int wm_log_divergence(wm_handle* h, const wm_traj* log, const wm_traj
   return WM_OK;
 }
 
+extern "C" int wm_expert_actions(wm_handle* h, const wm_traj* tr, int32_t t, int32_t n_steps, float* action,
+                                 uint8_t* action_valid, void* stream) {
+  if (!h || !traj_ok(tr) || !action || !action_valid) return WM_ERR_ARG;
+  if (n_steps < 1 || t < 0 || t + n_steps >= tr->T) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_expert(h, *tr, t, n_steps, action, action_valid, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_metrics_kinematic(wm_handle* h, const wm_traj* sim, int32_t t, int32_t n_steps, float* accel,
+                                    float* curvature, uint8_t* flag, void* stream) {
+  if (!h || !traj_ok(sim) || !flag) return WM_ERR_ARG;
+  if (n_steps < 1 || t < 1 || t + n_steps > sim->T) return WM_ERR_ARG;
+  if (!(h->cfg.max_accel > 0.f) || !(h->cfg.max_curvature > 0.f)) return WM_ERR_UNSUPPORTED;   // the metric needs its limits
+  WM_CUDA(wm_launch_kinematic(h, *sim, t, n_steps, accel, curvature, flag, (cudaStream_t)stream));
+  return WM_OK;
+}
+
 extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t t, float* hist,
                           uint8_t* hist_valid, int32_t* rg_index, float* rg_feat, int32_t* rg_type, void* stream) {
   if (!h || !traj_ok(sim)) return WM_ERR_ARG;

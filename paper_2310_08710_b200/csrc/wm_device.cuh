@@ -38,6 +38,22 @@ __device__ __forceinline__ void wm_dyn_step(const WmDynCfg& k, float x, float y,
   }
 }
 
+// Bicycle inverse, Eq. 3 (L352-L359), readings D4 / D31 / D32: acceleration and steering
+// curvature of the transition (th, vx, vy) -> (vx1, vy1).  Expert actor (L204) and kinematic
+// infeasibility metric (L104) share it.
+__device__ __forceinline__ void wm_inverse_bicycle(float dt, float th, float vx, float vy, float vx1, float vy1, float& acc,
+                                                   float& kappa) {
+  const float v = sqrtf(fmaf(vx, vx, vy * vy)), v1 = sqrtf(fmaf(vx1, vx1, vy1 * vy1));
+  acc = (v1 - v) / dt;                                       // L354
+  kappa = 0.f;
+  if (!(v == 0.f && v1 == 0.f)) {                            // D31
+    const float den = fmaf(v, dt, 0.5f * acc * dt * dt);     // L358
+    float d = atan2f(vy1, vx1) - th;                         // D4
+    d -= 6.28318530717958647692f * floorf((d + 3.14159265358979323846f) * 0.15915494309189533577f);   // D32: into [-pi, pi)
+    kappa = d / den;
+  }
+}
+
 // a5: displacement error, L106
 __device__ __forceinline__ float wm_logdiv(float x, float y, float lx, float ly) {
   const float ex = x - lx, ey = y - ly;

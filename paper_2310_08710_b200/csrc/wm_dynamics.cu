@@ -157,3 +157,86 @@ cudaError_t wm_launch_aggregate(wm_handle* h, int B, int A, int n_steps, const w
   h->launches++;
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------
+// Expert actor (L204; L335, Eq. 3) and kinematic-infeasibility metric (L104): one thread per
+// (scenario, step, agent); two state rows in, one action / metric row out.  HBM bound.
+// ---------------------------------------------------------------------------------------
+struct InvParams {
+  wm_traj tr;
+  int t, n_steps, dynamics;
+  float dt, max_accel, max_curvature;
+  float* action; uint8_t* valid;                // expert: [B][n][C][A], [B][n][A]
+  float* accel; float* curvature; uint8_t* flag;   // metric: [B][n][A]
+};
+
+constexpr int INV_CHUNK = 8;      // consecutive steps per thread: every state row is loaded once
+
+template <bool METRIC>
+__global__ void __launch_bounds__(256) k_inverse(InvParams p) {
+  const int A = p.tr.A, nchunk = (p.n_steps + INV_CHUNK - 1) / INV_CHUNK;
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= (int64_t)p.tr.B * nchunk * A) return;
+  const int a = (int)(i % A), ch = (int)((i / A) % nchunk), b = (int)(i / ((int64_t)A * nchunk));
+  const int s0 = ch * INV_CHUNK, s1 = min(s0 + INV_CHUNK, p.n_steps);
+  const bool delta = !METRIC && p.dynamics != WM_DYN_INVERTIBLE_BICYCLE;
+  const int C = p.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  int64_t r = ((int64_t)b * p.tr.T + (METRIC ? p.t + s0 - 1 : p.t + s0)) * A + a;      // first row of the chunk
+  // loads are unconditional (independent of `valid`, so they pipeline); an invalid slot's values
+  // never reach an output (D10): every use below is behind v
+  const float* pa = delta ? p.tr.x : p.tr.vel_x;
+  const float* pb = delta ? p.tr.y : p.tr.vel_y;
+  bool v0 = p.tr.valid[r] != 0;
+  float th = p.tr.yaw[r], vx = pa[r], vy = pb[r];
+  float x = vx, y = vy;
+#pragma unroll
+  for (int s = s0; s < s0 + INV_CHUNK; ++s) {
+    if (s >= s1) break;
+    r += A;
+    const bool v1 = p.tr.valid[r] != 0;
+    const float th1 = p.tr.yaw[r], vx1 = pa[r], vy1 = pb[r];
+    const float x1 = vx1, y1 = vy1;
+    const bool v = v0 && v1;
+    const int64_t o = ((int64_t)b * p.n_steps + s) * A + a;
+    if (METRIC) {
+      float acc = 0.f, kap = 0.f;
+      if (v) wm_inverse_bicycle(p.dt, th, vx, vy, vx1, vy1, acc, kap);
+      if (p.accel) p.accel[o] = acc;
+      if (p.curvature) p.curvature[o] = kap;
+      p.flag[o] = (uint8_t)(v && (fabsf(acc) > p.max_accel || fabsf(kap) > p.max_curvature));
+    } else {
+      float* act = p.action + (((int64_t)b * p.n_steps + s) * C) * A + a;
+      float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+      if (v) {
+        if (!delta) wm_inverse_bicycle(p.dt, th, vx, vy, vx1, vy1, a0, a1);
+        else {                                                 // L335 in the body frame (D2)
+          float sn, cs;
+          sincosf(th, &sn, &cs);
+          const float Dx = x1 - x, Dy = y1 - y;
+          a0 = fmaf(cs, Dx, sn * Dy); a1 = fmaf(cs, Dy, -sn * Dx); a2 = th1 - th;
+        }
+      }
+      act[0] = a0; act[A] = a1;
+      if (C == 3) act[2 * (int64_t)A] = a2;
+      p.valid[o] = (uint8_t)v;
+    }
+    v0 = v1; th = th1; vx = vx1; vy = vy1; x = x1; y = y1;
+  }
+}
+
+cudaError_t wm_launch_expert(wm_handle* h, const wm_traj& tr, int t, int n_steps, float* action, uint8_t* valid, cudaStream_t s) {
+  InvParams p{tr, t, n_steps, h->cfg.dynamics, h->cfg.dt, h->cfg.max_accel, h->cfg.max_curvature, action, valid, nullptr, nullptr, nullptr};
+  const int64_t n = (int64_t)tr.B * ((n_steps + INV_CHUNK - 1) / INV_CHUNK) * tr.A;
+  k_inverse<false><<<(unsigned)((n + 255) / 256), 256, 0, s>>>(p);
+  h->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t wm_launch_kinematic(wm_handle* h, const wm_traj& tr, int t, int n_steps, float* accel, float* curvature,
+                                uint8_t* flag, cudaStream_t s) {
+  InvParams p{tr, t, n_steps, h->cfg.dynamics, h->cfg.dt, h->cfg.max_accel, h->cfg.max_curvature, nullptr, nullptr, accel, curvature, flag};
+  const int64_t n = (int64_t)tr.B * ((n_steps + INV_CHUNK - 1) / INV_CHUNK) * tr.A;
+  k_inverse<true><<<(unsigned)((n + 255) / 256), 256, 0, s>>>(p);
+  h->launches++;
+  return cudaGetLastError();
+}

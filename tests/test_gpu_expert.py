@@ -1,0 +1,143 @@
+"""-m gpu parity tests of the expert actor (wm_expert_actions; L204, L335, Eq. 3) and the
+kinematic-infeasibility metric (wm_metrics_kinematic; L104) against the oracle.
+
+Tolerances: acceleration abs 1e-3 m/s^2 (float32 speeds, ulp(15 m/s)/dt = 1e-5, two square
+roots); curvature |d kappa| <= 1e-5 |kappa| + 4e-6 / den + 1e-6 (a float32 heading difference of up to
+~2 ulp(yaw) divided by the distance travelled den); delta actions abs 2e-5; flags bit-exact outside the
+band where |a| or |kappa| is within its tolerance of the limit (counted)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2310_08710_b200 as wm
+import wm_scenarios as ws
+from gpu_util import dev, host
+
+pytestmark = pytest.mark.gpu
+
+A_TOL = 1e-3
+
+
+def k_tol(kappa, den):
+    return 1e-5 * np.abs(kappa) + 4e-6 / np.maximum(den, 1e-12) + 1e-6
+
+
+def _gpu_expert(h, tr_d, t, n, C):
+    B, T, A = tr_d["x"].shape
+    act = torch.full((B, n, C, A), 7.0, device="cuda"); av = torch.full((B, n, A), 9, dtype=torch.uint8, device="cuda")
+    wm.wm_expert_actions(h, tr_d, t, n, act, av)
+    torch.cuda.synchronize()
+    return act, av
+
+
+@pytest.mark.parametrize("cid,B", [(1, None), (5, 6)])
+def test_expert_actions_match_oracle(cid, B):
+    cfg = ws.make_config(cid, n_steps=80) if B is None else ws.make_config(cid, B=B, n_steps=80)
+    log = cfg["log"]
+    log_d = dev(log)
+    for dyn, odyn, C in ((wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE, 2), (wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL, 3)):
+        h = wm.wm_create(dynamics=dyn)
+        act, av = _gpu_expert(h, log_d, 10, 80, C)
+        e = oracle.expert_actions(log, 10, 80, odyn)
+        assert np.array_equal(av.cpu().numpy(), e["valid"])
+        g = act.cpu().numpy().astype(np.float64); r = e["action"].astype(np.float64)
+        v = e["valid"] == 1
+        assert np.all(g[~np.broadcast_to(v[:, :, None, :], g.shape)] == 0)          # D10
+        if C == 2:
+            assert np.abs(g[:, :, 0] - r[:, :, 0])[v].max() <= A_TOL
+            dk = np.abs(g[:, :, 1] - r[:, :, 1])
+            assert np.all(dk[v] <= k_tol(r[:, :, 1], e["kden"])[v]), float((dk - k_tol(r[:, :, 1], e["kden"]))[v].max())
+            assert v.sum() > 1000 and np.abs(r[:, :, 1][v]).max() > 0.01
+        else:
+            assert np.abs(g - r)[np.broadcast_to(v[:, :, None, :], g.shape)].max() <= 2e-5
+        wm.wm_destroy(h)
+
+
+def test_kinematic_metric_matches_oracle_on_a_rollout():
+    """Rows of a GPU rollout with actions beyond the limits for some agents (clipping off), so that
+    both branches of the flag occur."""
+    n = 40
+    cfg = ws.make_config(5, B=8, n_steps=n)
+    log, rg = cfg["log"], cfg["roadgraph"]
+    B, T, A = log["x"].shape
+    acts = cfg["actions"].copy()
+    acts[:, :, 0, ::5] *= 2.6            # |a| up to 7.8
+    acts[:, :, 1, 1::7] *= 4.0           # |kappa| up to 0.4
+    h = wm.wm_create(max_accel=0.0, max_curvature=0.0)          # no clipping in the step (D7)
+    log_d, rg_d = dev(log), dev(rg)
+    sim_d = wm.empty_traj_like(log_d)
+    wm.wm_prepare(h, rg_d)
+    t0 = wm.wm_reset(h, log_d, sim_d)
+    out = wm.alloc_rollout_out(B, n, A)
+    wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(cfg["action_valid"]).cuda(), out)
+    hk = wm.wm_create()                                          # the metric's limits: 6, 0.3
+    acc = torch.full((B, n, A), 7.0, device="cuda"); cur = torch.full((B, n, A), 7.0, device="cuda")
+    fl = torch.full((B, n, A), 9, dtype=torch.uint8, device="cuda")
+    wm.wm_metrics_kinematic(hk, sim_d, t0 + 1, n, acc, cur, fl)
+    torch.cuda.synchronize()
+    sim = host(sim_d)
+    k = oracle.kinematic(sim, t0 + 1, n)
+    v = k["valid"] == 1
+    ga, gk, gf = acc.cpu().numpy().astype(np.float64), cur.cpu().numpy().astype(np.float64), fl.cpu().numpy()
+    assert np.all(ga[~v] == 0) and np.all(gk[~v] == 0) and np.all(gf[~v] == 0)
+    ra, rk = k["accel"].astype(np.float64), k["curvature"].astype(np.float64)
+    kt = k_tol(rk, k["kden"])
+    assert np.abs(ga - ra)[v].max() <= A_TOL
+    assert np.all(np.abs(gk - rk)[v] <= kt[v])
+    band = (np.abs(np.abs(ra) - 6.0) <= A_TOL) | (np.abs(np.abs(rk) - 0.3) <= kt)
+    clean = v & ~band
+    assert np.array_equal(gf[clean], k["flag"][clean])
+    n_flag = int(k["flag"][clean].sum())
+    print("kinematic: %d transitions, %d in the band, %d flagged" % (int(v.sum()), int((v & band).sum()), n_flag))
+    assert n_flag > 100 and n_flag < clean.sum() // 2
+    wm.wm_destroy(h); wm.wm_destroy(hk)
+
+
+def test_expert_rollouts():
+    """RolloutExpert (L200): expert actions of the log, then the rollout.  DeltaLocal reproduces the
+    log (Table 3: Log ADE 0.00); the bicycle expert follows the oracle's expert rollout and, by
+    construction (L198), stays kinematically feasible wherever the log is."""
+    n = 80
+    cfg = ws.make_config(5, B=8, n_steps=n)
+    log, rg = cfg["log"], cfg["roadgraph"]
+    B, T, A = log["x"].shape
+    log_d, rg_d = dev(log), dev(rg)
+    for dyn, odyn, C in ((wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL, 3), (wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE, 2)):
+        h = wm.wm_create(dynamics=dyn)
+        wm.wm_prepare(h, rg_d)
+        sim_d = wm.empty_traj_like(log_d)
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        act, av = _gpu_expert(h, log_d, t0, n, C)
+        out = wm.alloc_rollout_out(B, n, A)
+        wm.wm_rollout(h, log_d, sim_d, t0, n, act, av, out)
+        torch.cuda.synchronize()
+        ade = out["ade"].cpu().numpy()
+        e = oracle.expert_actions(log, t0, n, odyn)
+        sim_o = oracle.reset(log)
+        oo = oracle.rollout(log, sim_o, rg, t0, n, odyn, e["action"], e["valid"])
+        sim = host(sim_d)
+        assert np.array_equal(sim["valid"], sim_o["valid"])
+        v = sim_o["valid"][:, t0 + n] == 1
+        if dyn == wm.WM_DYN_DELTA_LOCAL:
+            assert round(float(ade.max()), 2) == 0.0 and ade.max() < 5e-3
+        err = np.hypot(sim["x"][:, t0 + n][v].astype(np.float64) - sim_o["x"][:, t0 + n][v], sim["y"][:, t0 + n][v].astype(np.float64) - sim_o["y"][:, t0 + n][v])
+        assert err.max() < 2e-3, float(err.max())
+        assert np.abs(ade - oo["ade"]).max() < 2e-3
+        wm.wm_destroy(h)
+
+
+def test_argument_checks():
+    cfg = ws.make_config(1, n_steps=4)
+    log_d = dev(cfg["log"])
+    B, T, A = log_d["x"].shape
+    h = wm.wm_create()
+    act = torch.zeros((B, 1, 2, A), device="cuda"); av = torch.zeros((B, 1, A), dtype=torch.uint8, device="cuda")
+    fl = torch.zeros((B, 1, A), dtype=torch.uint8, device="cuda")
+    for bad in (lambda: wm.wm_expert_actions(h, log_d, T - 1, 1, act, av), lambda: wm.wm_expert_actions(h, log_d, -1, 1, act, av),
+                lambda: wm.wm_metrics_kinematic(h, log_d, 0, 1, None, None, fl), lambda: wm.wm_metrics_kinematic(h, log_d, T, 1, None, None, fl)):
+        with pytest.raises(RuntimeError):
+            bad()
+    wm.wm_metrics_kinematic(h, log_d, T - 1, 1, None, None, fl)          # NULL accel / curvature are allowed
+    torch.cuda.synchronize()
+    wm.wm_destroy(h)
