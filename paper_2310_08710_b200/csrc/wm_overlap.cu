@@ -13,7 +13,7 @@ struct OverlapParams {
   uint8_t* flag; int64_t flag_stride_b;
 };
 
-__global__ void __launch_bounds__(256) k_overlap(OverlapParams p) {
+__global__ void __launch_bounds__(1024) k_overlap(OverlapParams p) {
   extern __shared__ float sm[];
   const int A = p.A, nb = p.W, Ap = nb * 32;
   float* sx = sm;            float* sy = sx + Ap;
@@ -88,7 +88,10 @@ cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t*
   p.pair_bits = pair_bits; p.flag = flag; p.flag_stride_b = flag_stride_b;
   const int Ap = p.W * 32;
   const size_t smem = (size_t)Ap * 8 * 4 + (size_t)p.W * 4;
-  k_overlap<<<sim.B, 256, smem, s>>>(p);
+  // one warp per 32 x 32 tile of the upper triangle, up to 32 warps per scenario (A = 512: 136 tiles)
+  const int ntile = p.W * (p.W + 1) / 2;
+  const int nt = ntile >= 32 ? 1024 : (ntile > 8 ? 512 : 256);
+  k_overlap<<<sim.B, nt, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
 }
