@@ -17,6 +17,7 @@ _LIB = os.path.join(_HERE, "libwm_oracle.so")
 
 DYN_BICYCLE = 0
 DYN_DELTA_LOCAL = 1
+DYN_DELTA_GLOBAL = 2
 BAND = 1e-4  # ambiguity band in metres (BASELINE.json north_star)
 
 TRAJ_F = ("x", "y", "yaw", "vel_x", "vel_y", "length", "width")

@@ -40,7 +40,7 @@ struct orc_roadgraph {       // [B][R] each
   uint8_t* valid;
 };
 
-enum { ORC_DYN_BICYCLE = 0, ORC_DYN_DELTA_LOCAL = 1 };
+enum { ORC_DYN_BICYCLE = 0, ORC_DYN_DELTA_LOCAL = 1, ORC_DYN_DELTA_GLOBAL = 2 };
 enum { ORC_TYPE_ROAD_EDGE = 2 };
 
 static inline size_t row(const orc_traj* tr, int b, int t) {
@@ -52,6 +52,7 @@ static inline size_t row(const orc_traj* tr, int b, int t) {
 //   InvertibleBicycle: PAPER.md L339-L350 (Appendix A.1, Eq. 2), literal: the position uses
 //     the velocity components, the acceleration term uses the yaw.
 //   DeltaLocal: PAPER.md L324-L333 (Eq. 1) after rotating the body-frame delta by yaw (D2).
+//   DeltaGlobal: Eq. 1 literally, the delta is in the world frame.
 //   Action clipping to +-max_accel / +-max_curvature when the limit is > 0 (D7; limits
 //     6 m/s^2, 0.3 1/m from L104).
 //   use_dyn = action_valid && sim.valid[t]; otherwise row t+1 <- log row t+1 (D8, L164).
@@ -97,7 +98,8 @@ void orc_step(const orc_traj* log, orc_traj* sim, int32_t t, int32_t dynamics, d
         vyn = vn * std::sin(thn);                                    // L349
       } else {
         const double dx = act[0 * A + a], dy = act[1 * A + a], dyaw = act[2 * A + a];
-        const double c = std::cos(th), s = std::sin(th);
+        // DeltaGlobal: Eq. 1 literally (world-frame delta); DeltaLocal: the body-frame delta rotated by yaw (D2)
+        const double c = dynamics == ORC_DYN_DELTA_GLOBAL ? 1.0 : std::cos(th), s = dynamics == ORC_DYN_DELTA_GLOBAL ? 0.0 : std::sin(th);
         xn = x + c * dx - s * dy;                                    // Eq. 1, world delta
         yn = y + s * dx + c * dy;                                    // L326
         thn = th + dyaw;                                             // L328
@@ -512,9 +514,10 @@ void orc_expert_actions(const orc_traj* tr, int32_t t, int32_t n_steps, int32_t 
           action[o] = (float)acc; action[o + A] = (float)kap;
           if (kden) kden[ov] = den;
         } else {
-          const double th = tr->yaw[i0], cs = std::cos(th), sn = std::sin(th);
+          const double th = tr->yaw[i0];
+          const double cs = dynamics == ORC_DYN_DELTA_GLOBAL ? 1.0 : std::cos(th), sn = dynamics == ORC_DYN_DELTA_GLOBAL ? 0.0 : std::sin(th);
           const double Dx = (double)tr->x[i1] - (double)tr->x[i0], Dy = (double)tr->y[i1] - (double)tr->y[i0];   // L335
-          action[o] = (float)(cs * Dx + sn * Dy);                   // body frame (D2)
+          action[o] = (float)(cs * Dx + sn * Dy);                   // body frame (D2); DeltaGlobal: (Dx, Dy) itself
           action[o + A] = (float)(-sn * Dx + cs * Dy);
           action[o + 2 * (size_t)A] = (float)((double)tr->yaw[i1] - th);
         }

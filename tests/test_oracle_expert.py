@@ -127,3 +127,32 @@ def test_rigid_invariance_of_the_bicycle_inverse():
     k1, k2 = oracle.kinematic(tr, 1), oracle.kinematic(tr2, 1)
     assert np.abs(k1["accel"] - k2["accel"]).max() < 1e-3
     assert np.all(np.abs(k1["curvature"] - k2["curvature"]) < 4e-6 / k1["kden"] + 1e-5)
+
+
+def test_delta_global_is_eq1_literally():
+    """Eq. 1 (L324-L333): x' = x + dx, y' = y + dy, yaw' = yaw + dyaw, v' = (p' - p)/dt, whatever
+    the yaw; its inverse (L335) is the plain difference."""
+    rng = np.random.default_rng(3)
+    A = 32
+    log = mk_traj(1, 2, A, valid=1); sim = mk_traj(1, 2, A, valid=1)
+    st = rng.uniform(-30, 30, (A, 3))
+    for a in range(A):
+        set_agent(sim, 0, 0, a, st[a, 0], st[a, 1], st[a, 2] * 0.2, 1.0, 2.0)
+    act = np.zeros((1, 3, A), np.float32)
+    act[0, 0] = rng.uniform(-0.5, 0.5, A); act[0, 1] = rng.uniform(-0.5, 0.5, A); act[0, 2] = rng.uniform(-0.1, 0.1, A)
+    x0, y0, th0 = sim["x"][0, 0].astype(np.float64), sim["y"][0, 0].astype(np.float64), sim["yaw"][0, 0].astype(np.float64)
+    oracle.step(log, sim, 0, oracle.DYN_DELTA_GLOBAL, act, np.ones((1, A), np.uint8))
+    assert np.allclose(sim["x"][0, 1], x0 + act[0, 0], atol=4e-6) and np.allclose(sim["y"][0, 1], y0 + act[0, 1], atol=4e-6)
+    assert np.allclose(sim["yaw"][0, 1], th0 + act[0, 2], atol=1e-6)
+    assert np.allclose(sim["vel_x"][0, 1], (sim["x"][0, 1].astype(np.float64) - x0) / DT, atol=1e-5)
+    assert np.allclose(sim["vel_y"][0, 1], (sim["y"][0, 1].astype(np.float64) - y0) / DT, atol=1e-5)
+    e = oracle.expert_actions(sim, 0, 1, oracle.DYN_DELTA_GLOBAL)["action"][0, 0]
+    assert np.allclose(e, act[0], atol=4e-6)
+    # and with yaw = 0 the local and the global model coincide (D2)
+    sim0 = mk_traj(1, 2, A, valid=1); sim1 = mk_traj(1, 2, A, valid=1)
+    for a in range(A):
+        set_agent(sim0, 0, 0, a, st[a, 0], st[a, 1], 0.0, 1.0, 2.0); set_agent(sim1, 0, 0, a, st[a, 0], st[a, 1], 0.0, 1.0, 2.0)
+    oracle.step(log, sim0, 0, oracle.DYN_DELTA_GLOBAL, act, np.ones((1, A), np.uint8))
+    oracle.step(log, sim1, 0, oracle.DYN_DELTA_LOCAL, act, np.ones((1, A), np.uint8))
+    for k in ("x", "y", "yaw", "vel_x", "vel_y"):
+        assert np.array_equal(sim0[k], sim1[k]), k
