@@ -42,7 +42,7 @@ typedef enum {
   WM_ERR_STATE = -4         /* e.g. metrics_offroad before wm_prepare */
 } wm_status;
 
-enum { WM_DYN_INVERTIBLE_BICYCLE = 0, WM_DYN_DELTA_LOCAL = 1 };
+enum { WM_DYN_INVERTIBLE_BICYCLE = 0, WM_DYN_DELTA_LOCAL = 1, WM_DYN_DELTA_GLOBAL = 2 };   /* DELTA_GLOBAL: Eq. 1 literally (world-frame delta) */
 enum { WM_TYPE_LANE = 1, WM_TYPE_ROAD_EDGE = 2 };
 
 /* Dynamic state, PAPER.md L82 / L322: s = (x, y, yaw, v_x, v_y) + box dims + validity,

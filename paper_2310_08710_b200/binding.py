@@ -12,7 +12,7 @@ import torch
 from . import _build
 
 WM_OK, WM_ERR_ARG, WM_ERR_CUDA, WM_ERR_UNSUPPORTED, WM_ERR_STATE = 0, -1, -2, -3, -4
-WM_DYN_INVERTIBLE_BICYCLE, WM_DYN_DELTA_LOCAL = 0, 1
+WM_DYN_INVERTIBLE_BICYCLE, WM_DYN_DELTA_LOCAL, WM_DYN_DELTA_GLOBAL = 0, 1, 2
 WM_TYPE_LANE, WM_TYPE_ROAD_EDGE = 1, 2
 WM_OFFROAD_CULLED, WM_OFFROAD_BRUTE_FORCE = 0, 1
 WM_ROLLOUT_FUSED, WM_ROLLOUT_STEPWISE = 0, 1

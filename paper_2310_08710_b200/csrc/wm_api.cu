@@ -28,7 +28,7 @@ static bool same_shape(const wm_traj* a, const wm_traj* b) { return a->B == b->B
 
 extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (!out || !cfg) return WM_ERR_ARG;
-  if (cfg->dynamics != WM_DYN_INVERTIBLE_BICYCLE && cfg->dynamics != WM_DYN_DELTA_LOCAL) return WM_ERR_ARG;
+  if (cfg->dynamics != WM_DYN_INVERTIBLE_BICYCLE && cfg->dynamics != WM_DYN_DELTA_LOCAL && cfg->dynamics != WM_DYN_DELTA_GLOBAL) return WM_ERR_ARG;
   if (!(cfg->dt > 0.f) || cfg->history < 1 || cfg->topk < 0) return WM_ERR_ARG;
   if (cfg->offroad_mode != WM_OFFROAD_CULLED && cfg->offroad_mode != WM_OFFROAD_BRUTE_FORCE) return WM_ERR_ARG;
   if (cfg->rollout_mode != WM_ROLLOUT_FUSED && cfg->rollout_mode != WM_ROLLOUT_STEPWISE) return WM_ERR_ARG;

@@ -29,8 +29,13 @@ __device__ __forceinline__ void wm_dyn_step(const WmDynCfg& k, float x, float y,
   } else {
     const float dx = a0, dy = a1, dyaw = a2;
     // explicit roundings: the compiler must not contract these differently in different kernels (P14)
-    xn = __fadd_rn(x, __fmaf_rn(cs, dx, -__fmul_rn(sn, dy)));     // Eq. 1 on the rotated delta (D2)
-    yn = __fadd_rn(y, __fmaf_rn(sn, dx, __fmul_rn(cs, dy)));
+    if (k.dynamics == WM_DYN_DELTA_GLOBAL) {                        // Eq. 1 literally: world-frame delta
+      xn = __fadd_rn(x, dx);
+      yn = __fadd_rn(y, dy);
+    } else {
+      xn = __fadd_rn(x, __fmaf_rn(cs, dx, -__fmul_rn(sn, dy)));   // Eq. 1 on the rotated delta (D2)
+      yn = __fadd_rn(y, __fmaf_rn(sn, dx, __fmul_rn(cs, dy)));
+    }
     thn = __fadd_rn(th, dyaw);
     vxn = __fdiv_rn(__fsub_rn(xn, x), dt);           // Eq. 1: on the stored float32 x' (D28)
     vyn = __fdiv_rn(__fsub_rn(yn, y), dt);

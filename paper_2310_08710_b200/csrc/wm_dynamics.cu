@@ -210,8 +210,8 @@ __global__ void __launch_bounds__(256) k_inverse(InvParams p) {
       if (v) {
         if (!delta) wm_inverse_bicycle(p.dt, th, vx, vy, vx1, vy1, a0, a1);
         else {                                                 // L335 in the body frame (D2)
-          float sn, cs;
-          sincosf(th, &sn, &cs);
+          float sn = 0.f, cs = 1.f;                            // DeltaGlobal: the plain difference
+          if (p.dynamics == WM_DYN_DELTA_LOCAL) sincosf(th, &sn, &cs);
           const float Dx = x1 - x, Dy = y1 - y;
           a0 = fmaf(cs, Dx, sn * Dy); a1 = fmaf(cs, Dy, -sn * Dx); a2 = th1 - th;
         }

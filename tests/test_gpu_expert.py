@@ -36,7 +36,8 @@ def test_expert_actions_match_oracle(cid, B):
     cfg = ws.make_config(cid, n_steps=80) if B is None else ws.make_config(cid, B=B, n_steps=80)
     log = cfg["log"]
     log_d = dev(log)
-    for dyn, odyn, C in ((wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE, 2), (wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL, 3)):
+    for dyn, odyn, C in ((wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE, 2), (wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL, 3),
+                         (wm.WM_DYN_DELTA_GLOBAL, oracle.DYN_DELTA_GLOBAL, 3)):
         h = wm.wm_create(dynamics=dyn)
         act, av = _gpu_expert(h, log_d, 10, 80, C)
         e = oracle.expert_actions(log, 10, 80, odyn)
@@ -103,7 +104,8 @@ def test_expert_rollouts():
     log, rg = cfg["log"], cfg["roadgraph"]
     B, T, A = log["x"].shape
     log_d, rg_d = dev(log), dev(rg)
-    for dyn, odyn, C in ((wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL, 3), (wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE, 2)):
+    for dyn, odyn, C in ((wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL, 3), (wm.WM_DYN_DELTA_GLOBAL, oracle.DYN_DELTA_GLOBAL, 3),
+                         (wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE, 2)):
         h = wm.wm_create(dynamics=dyn)
         wm.wm_prepare(h, rg_d)
         sim_d = wm.empty_traj_like(log_d)
@@ -119,7 +121,7 @@ def test_expert_rollouts():
         sim = host(sim_d)
         assert np.array_equal(sim["valid"], sim_o["valid"])
         v = sim_o["valid"][:, t0 + n] == 1
-        if dyn == wm.WM_DYN_DELTA_LOCAL:
+        if dyn != wm.WM_DYN_INVERTIBLE_BICYCLE:
             assert round(float(ade.max()), 2) == 0.0 and ade.max() < 5e-3
         err = np.hypot(sim["x"][:, t0 + n][v].astype(np.float64) - sim_o["x"][:, t0 + n][v], sim["y"][:, t0 + n][v].astype(np.float64) - sim_o["y"][:, t0 + n][v])
         assert err.max() < 2e-3, float(err.max())

@@ -13,7 +13,8 @@ from gpu_util import (dev, host, row_of, assert_state_close, gpu_offroad, compar
 pytestmark = pytest.mark.gpu
 
 DYN = {"bicycle": (wm.WM_DYN_INVERTIBLE_BICYCLE, oracle.DYN_BICYCLE),
-       "delta_local": (wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL)}
+       "delta_local": (wm.WM_DYN_DELTA_LOCAL, oracle.DYN_DELTA_LOCAL),
+       "delta_global": (wm.WM_DYN_DELTA_GLOBAL, oracle.DYN_DELTA_GLOBAL)}
 
 
 @pytest.fixture(scope="module")
@@ -54,7 +55,7 @@ def test_reset_matches_oracle(cfg1):
 
 
 # ---------------------------------------------------------------- dynamics
-@pytest.mark.parametrize("cfgid,dyn", [(1, "bicycle"), (2, "delta_local"), (5, "bicycle")])
+@pytest.mark.parametrize("cfgid,dyn", [(1, "bicycle"), (2, "delta_local"), (2, "delta_global"), (5, "bicycle")])
 def test_single_step_matches_oracle(cfgid, dyn):
     cfg = ws.make_config(cfgid, B=None if cfgid == 1 else 24, n_steps=2 if cfgid == 5 else None)
     h, log_d, rg_d, sim_d, _ = _setup(cfg, dyn)
@@ -255,7 +256,7 @@ def test_rollout_graph_replay_is_deterministic_and_matches_eager(cfg1, mode):
     wm.wm_destroy(h)
 
 
-@pytest.mark.parametrize("cfgid,dyn,n", [(5, "bicycle", 80), (2, "delta_local", 1), (1, "bicycle", 80), (4, "bicycle", 3)])
+@pytest.mark.parametrize("cfgid,dyn,n", [(5, "bicycle", 80), (2, "delta_local", 1), (2, "delta_global", 1), (1, "bicycle", 80), (4, "bicycle", 3)])
 def test_rollout_fused_equals_stepwise_bitwise(cfgid, dyn, n):
     """P14: the fused kernel and the stepwise graph run the same device arithmetic."""
     cfg = ws.make_config(cfgid, B=5, n_steps=n) if cfgid in (2, 5) else ws.make_config(cfgid, B=3 if cfgid == 4 else None)
