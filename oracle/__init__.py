@@ -200,3 +200,21 @@ def kinematic(tr, t, n_steps=1, dt=0.1, max_accel=6.0, max_curvature=0.3):
     lib().orc_kinematic(C.byref(ts), C.c_int32(t), C.c_int32(n_steps), C.c_double(dt), C.c_double(max_accel),
                         C.c_double(max_curvature), _p(acc), _p(cur), _p(den), _p(flag), _p(val))
     return dict(accel=acc, curvature=cur, kden=den, flag=flag, valid=val)
+
+
+class _Paths(C.Structure):
+    _fields_ = [("B", C.c_int32), ("A", C.c_int32), ("P", C.c_int32), ("x", C.c_void_p), ("y", C.c_void_p),
+                ("arc_len", C.c_void_p), ("valid", C.c_void_p)]
+
+
+def route_progress(log, sim, t, paths):
+    """O11 (L96). paths: dict x, y, arc_len float32 [B][A][P], valid uint8 [B][A][P]."""
+    ls, (B, T, A) = _traj(log); ss, _ = _traj(sim)
+    P = paths["x"].shape[2]
+    for k in ("x", "y", "arc_len"):
+        _check(paths[k], np.float32, (B, A, P))
+    _check(paths["valid"], np.uint8, (B, A, P))
+    ps = _Paths(B, A, P, _p(paths["x"]), _p(paths["y"]), _p(paths["arc_len"]), _p(paths["valid"]))
+    ratio = np.empty((B, A), np.float32); val = np.empty((B, A), np.uint8); cl = np.empty((B, 3, A), np.int32)
+    lib().orc_route_progress(C.byref(ls), C.byref(ss), C.c_int32(t), C.byref(ps), _p(ratio), _p(val), _p(cl))
+    return dict(ratio=ratio, valid=val, closest=cl)

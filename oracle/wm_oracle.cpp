@@ -548,6 +548,62 @@ void orc_kinematic(const orc_traj* tr, int32_t t, int32_t n_steps, double dt, do
       }
 }
 
+// -------------------------------------------------------------------------------------
+// O11 route progress ratio: "associates the vehicle's position to the closest
+// point x(t) in an on-route path ... distance along the path from the start of the path to
+// x(t), d_x(t) ... ratio = (d_x(t) - d_p) / (d_q - d_p), where d_p and d_q are the distances along
+// the path to the initial and final positions of the vehicle's logged trajectory ... could be
+// greater than 1".  One on-route path per agent: points [B][A][P] with their arc length (an
+// input, as in the paper's path structure) and validity.
+//   D33: closest POINT (not segment) among the valid path points, ties -> lower index; the
+//        comparison key is the float32 value fma(dy, dy, dx*dx) (the kernel's precision, as for
+//        the top-k: a floating-point value that decides an index);
+//   D34: initial / final logged position = first / last VALID logged row of the agent;
+//   D35: valid = sim valid at t, some valid path point, some valid logged row, d_q != d_p;
+//        otherwise ratio 0, valid 0.
+// closest (may be NULL): [B][3][A] indices of the closest points to (sim, log first, log last).
+// -------------------------------------------------------------------------------------
+struct orc_paths { int32_t B, A, P; float *x, *y, *arc_len; uint8_t* valid; };
+
+static int closest_path_point(const orc_paths* pa, int b, int a, float qx, float qy) {
+  const size_t o = ((size_t)b * pa->A + a) * pa->P;
+  int best = -1;
+  float bk = 0.f;
+  for (int i = 0; i < pa->P; ++i) {
+    if (!pa->valid[o + i]) continue;
+    const float dx = pa->x[o + i] - qx, dy = pa->y[o + i] - qy;        // float32 on purpose (D33)
+    const float key = std::fmaf(dy, dy, dx * dx);
+    if (best < 0 || key < bk) { best = i; bk = key; }                   // strict '<': ties -> lower index
+  }
+  return best;
+}
+
+void orc_route_progress(const orc_traj* log, const orc_traj* sim, int32_t t, const orc_paths* pa, float* ratio,
+                        uint8_t* valid, int32_t* closest) {
+  const int B = sim->B, A = sim->A, T = sim->T;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b)
+    for (int a = 0; a < A; ++a) {
+      const size_t o = (size_t)b * A + a;
+      ratio[o] = 0.f; valid[o] = 0;
+      if (closest) for (int c = 0; c < 3; ++c) closest[((size_t)b * 3 + c) * A + a] = -1;
+      int tf = -1, tl = -1;                                              // D34
+      for (int k = 0; k < T; ++k) if (log->valid[row(log, b, k) + a]) { if (tf < 0) tf = k; tl = k; }
+      const size_t rs = row(sim, b, t) + a;
+      if (!sim->valid[rs] || tf < 0) continue;
+      const int ix = closest_path_point(pa, b, a, sim->x[rs], sim->y[rs]);
+      if (ix < 0) continue;
+      const int ip = closest_path_point(pa, b, a, log->x[row(log, b, tf) + a], log->y[row(log, b, tf) + a]);
+      const int iq = closest_path_point(pa, b, a, log->x[row(log, b, tl) + a], log->y[row(log, b, tl) + a]);
+      if (closest) { closest[((size_t)b * 3 + 0) * A + a] = ix; closest[((size_t)b * 3 + 1) * A + a] = ip; closest[((size_t)b * 3 + 2) * A + a] = iq; }
+      const size_t po = ((size_t)b * pa->A + a) * pa->P;
+      const double dxp = pa->arc_len[po + ix], dp = pa->arc_len[po + ip], dq = pa->arc_len[po + iq];
+      if (dq == dp) continue;                                            // D35
+      ratio[o] = (float)((dxp - dp) / (dq - dp));                        // L96
+      valid[o] = 1;
+    }
+}
+
 int32_t orc_num_threads() {
 #ifdef _OPENMP
   return omp_get_max_threads();

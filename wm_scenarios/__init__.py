@@ -13,6 +13,7 @@ scenario ``b`` is identical whatever batch it is generated in (rank shards, pari
 from .rng import uniform, randint, MASTER_SEED
 from .configs import (
     make_config,
+    make_paths,
     make_street_scenarios,
     make_config1,
     make_config4,
@@ -22,6 +23,6 @@ from .configs import (
 )
 
 __all__ = [
-    "uniform", "randint", "MASTER_SEED", "make_config", "make_street_scenarios",
+    "uniform", "randint", "MASTER_SEED", "make_config", "make_paths", "make_street_scenarios",
     "make_config1", "make_config4", "CONFIG_SHAPES", "TYPE_LANE", "TYPE_ROAD_EDGE",
 ]

@@ -369,3 +369,32 @@ def make_config(cfg, B=None, b_ids=None, seed=None, R=None, A=None, T=None, n_st
         act, av = bicycle_actions(seed, b, shp["A"], ns, valid_t0)
         out.update(actions=act, action_valid=av, dynamics="bicycle", n_steps=ns)
     return out
+
+
+def make_paths(log, extend=16, spacing=1.0):
+    """One synthetic on-route path per agent (stand-in for the paper's roadgraph paths, L84): the
+    agent's valid logged positions in time order, then `extend` more points straight ahead of the
+    last logged heading at `spacing` metres.  arc_len = cumulative chord length from the first
+    point (float64 sum, one rounding to float32).  Returns x, y, arc_len [B][A][P], valid [B][A][P],
+    P = T + extend.  Input construction only: nothing here belongs to a metric."""
+    B, T, A = log["x"].shape
+    P = T + extend
+    out = dict(x=np.zeros((B, A, P), np.float32), y=np.zeros((B, A, P), np.float32),
+               arc_len=np.zeros((B, A, P), np.float32), valid=np.zeros((B, A, P), np.uint8))
+    v = np.transpose(log["valid"], (0, 2, 1)) == 1                         # [B][A][T]
+    x = np.transpose(log["x"], (0, 2, 1)).astype(np.float64); y = np.transpose(log["y"], (0, 2, 1)).astype(np.float64)
+    yaw = np.transpose(log["yaw"], (0, 2, 1)).astype(np.float64)
+    for b in range(B):
+        for a in range(A):
+            idx = np.nonzero(v[b, a])[0]
+            if len(idx) == 0:
+                continue
+            px = list(x[b, a, idx]); py = list(y[b, a, idx])
+            th = yaw[b, a, idx[-1]]
+            for e in range(1, extend + 1):
+                px.append(px[len(idx) - 1] + e * spacing * np.cos(th)); py.append(py[len(idx) - 1] + e * spacing * np.sin(th))
+            px = np.array(px); py = np.array(py)
+            arc = np.concatenate([[0.0], np.cumsum(np.hypot(np.diff(px), np.diff(py)))])
+            n = len(px)
+            out["x"][b, a, :n] = px; out["y"][b, a, :n] = py; out["arc_len"][b, a, :n] = arc; out["valid"][b, a, :n] = 1
+    return out
