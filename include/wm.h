@@ -203,6 +203,25 @@ int wm_expert_actions(wm_handle* h, const wm_traj* tr, int32_t t, int32_t n_step
 int wm_metrics_kinematic(wm_handle* h, const wm_traj* sim, int32_t t, int32_t n_steps, float* accel,
                          float* curvature, uint8_t* flag, void* stream);
 
+/* One on-route path per agent (L84, L96): points [B][A][P] with the distance along the path from
+ * its start (arc_len, an input) and validity.  DEVICE pointers, caller-owned. */
+typedef struct {
+  int32_t B, A, P;
+  const float *x, *y, *arc_len;
+  const uint8_t* valid;
+} wm_paths;
+
+/*
+ * Route-progress ratio, L96: for every agent, x(t) = the valid path point closest to the simulated
+ * position at row t (closest POINT, ties -> lower index; float32 key fma(dy, dy, dx*dx), D33);
+ * ratio = (arc_len[x(t)] - d_p) / (d_q - d_p), d_p / d_q = arc length of the path points closest
+ * to the agent's first / last VALID logged position (D34); it may exceed 1 or be negative.
+ * ratio [B][A], valid [B][A] = sim valid at t, a valid path point, a valid logged row and
+ * d_q != d_p (D35); ratio = 0 where not valid.  Requires 0 <= t < T and paths of the same B, A.
+ */
+int wm_metrics_route_progress(wm_handle* h, const wm_traj* log, const wm_traj* sim, int32_t t,
+                              const wm_paths* paths, float* ratio, uint8_t* valid, void* stream);
+
 /*
  * Rollout, L200: for s = 0 .. n_steps-1: wm_step at t0+s, then overlap, offroad and log
  * divergence on row t0+s+1 (D11), written to row s of the per-step outputs; aggregates over

@@ -23,7 +23,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_expert_actions", "wm_metrics_kinematic", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
+           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
 
 
 class wm_traj(C.Structure):
@@ -186,6 +186,21 @@ def wm_metrics_kinematic(h, sim, t, n_steps, accel, curvature, flag, stream=None
     ss = traj_struct(sim)
     _check(load().wm_metrics_kinematic(h, C.byref(ss), C.c_int32(t), C.c_int32(n_steps), _ptr(accel, torch.float32),
                                        _ptr(curvature, torch.float32), _ptr(flag, torch.uint8), _stream(stream)), "wm_metrics_kinematic")
+
+
+class wm_paths(C.Structure):
+    _fields_ = [("B", C.c_int32), ("A", C.c_int32), ("P", C.c_int32), ("x", C.c_void_p), ("y", C.c_void_p),
+                ("arc_len", C.c_void_p), ("valid", C.c_void_p)]
+
+
+def wm_metrics_route_progress(h, log, sim, t, paths, ratio, valid, stream=None):
+    """paths: dict of device tensors x, y, arc_len float32 [B][A][P], valid uint8 [B][A][P]."""
+    ls, ss = traj_struct(log), traj_struct(sim)
+    B, A, P = paths["x"].shape
+    ps = wm_paths(B, A, P, _ptr(paths["x"], torch.float32), _ptr(paths["y"], torch.float32), _ptr(paths["arc_len"], torch.float32),
+                  _ptr(paths["valid"], torch.uint8))
+    _check(load().wm_metrics_route_progress(h, C.byref(ls), C.byref(ss), C.c_int32(t), C.byref(ps), _ptr(ratio, torch.float32),
+                                            _ptr(valid, torch.uint8), _stream(stream)), "wm_metrics_route_progress")
 
 
 def wm_observe(h, sim, rg, t, hist=None, hist_valid=None, rg_index=None, rg_feat=None, rg_type=None, stream=None):

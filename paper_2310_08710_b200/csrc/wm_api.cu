@@ -180,6 +180,15 @@ extern "C" int wm_metrics_kinematic(wm_handle* h, const wm_traj* sim, int32_t t,
   return WM_OK;
 }
 
+extern "C" int wm_metrics_route_progress(wm_handle* h, const wm_traj* log, const wm_traj* sim, int32_t t, const wm_paths* paths,
+                                         float* ratio, uint8_t* valid, void* stream) {
+  if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !paths || !ratio || !valid) return WM_ERR_ARG;
+  if (t < 0 || t >= sim->T) return WM_ERR_ARG;
+  if (paths->B != sim->B || paths->A != sim->A || paths->P < 1 || !paths->x || !paths->y || !paths->arc_len || !paths->valid) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_route_progress(h, *log, *sim, t, *paths, ratio, valid, (cudaStream_t)stream));
+  return WM_OK;
+}
+
 extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t t, float* hist,
                           uint8_t* hist_valid, int32_t* rg_index, float* rg_feat, int32_t* rg_type, void* stream) {
   if (!h || !traj_ok(sim)) return WM_ERR_ARG;

@@ -142,6 +142,8 @@ cudaError_t wm_launch_logdiv(wm_handle* h, const wm_traj& log, const wm_traj& si
 cudaError_t wm_launch_expert(wm_handle* h, const wm_traj& tr, int t, int n_steps, float* action, uint8_t* valid, cudaStream_t s);
 cudaError_t wm_launch_kinematic(wm_handle* h, const wm_traj& tr, int t, int n_steps, float* accel, float* curvature,
                                 uint8_t* flag, cudaStream_t s);
+cudaError_t wm_launch_route_progress(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t, const wm_paths& pa, float* ratio,
+                                     uint8_t* valid, cudaStream_t s);
 cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t* pair_bits,
                               uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
 cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,

@@ -143,3 +143,39 @@ def test_argument_checks():
     wm.wm_metrics_kinematic(h, log_d, T - 1, 1, None, None, fl)          # NULL accel / curvature are allowed
     torch.cuda.synchronize()
     wm.wm_destroy(h)
+
+
+def test_route_progress_matches_oracle():
+    """wm_metrics_route_progress (L96) on the rows of a GPU rollout, synthetic per-agent paths; the
+    closest-point decision is taken in float32 on both sides (D33), so validity and the ratio's
+    numerator / denominator indices agree exactly and the ratio to float32 rounding."""
+    n = 80
+    for cid, B in ((5, 6), (1, None)):
+        cfg = ws.make_config(cid, n_steps=n) if B is None else ws.make_config(cid, B=B, n_steps=n)
+        log, rg = cfg["log"], cfg["roadgraph"]
+        Bn, T, A = log["x"].shape
+        paths = ws.make_paths(log)
+        paths["valid"][:, ::7, 5] = 0                          # holes in some paths
+        h = wm.wm_create()
+        log_d, rg_d = dev(log), dev(rg)
+        sim_d = wm.empty_traj_like(log_d)
+        wm.wm_prepare(h, rg_d)
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        out = wm.alloc_rollout_out(Bn, n, A)
+        wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(cfg["actions"]).cuda(), torch.from_numpy(cfg["action_valid"]).cuda(), out)
+        paths_d = {k: torch.from_numpy(v).cuda() for k, v in paths.items()}
+        sim = None
+        for t in (t0, t0 + 37, t0 + n):
+            ratio = torch.full((Bn, A), 7.0, device="cuda"); val = torch.full((Bn, A), 9, dtype=torch.uint8, device="cuda")
+            wm.wm_metrics_route_progress(h, log_d, sim_d, t, paths_d, ratio, val)
+            torch.cuda.synchronize()
+            sim = host(sim_d) if sim is None else sim
+            r = oracle.route_progress(log, sim, t, paths)
+            assert np.array_equal(val.cpu().numpy(), r["valid"])
+            g = ratio.cpu().numpy().astype(np.float64)
+            assert np.all(g[r["valid"] == 0] == 0)
+            v = r["valid"] == 1
+            assert np.all(np.abs(g - r["ratio"])[v] <= 1e-5 * np.maximum(1.0, np.abs(r["ratio"][v])))
+            assert v.sum() > 0.5 * (sim["valid"][:, t] == 1).sum()
+        # the reset state sits on its own logged position: progress of agents logged from step 0 at t0 = progress of the log
+        wm.wm_destroy(h)

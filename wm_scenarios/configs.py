@@ -379,22 +379,21 @@ def make_paths(log, extend=16, spacing=1.0):
     P = T + extend.  Input construction only: nothing here belongs to a metric."""
     B, T, A = log["x"].shape
     P = T + extend
-    out = dict(x=np.zeros((B, A, P), np.float32), y=np.zeros((B, A, P), np.float32),
-               arc_len=np.zeros((B, A, P), np.float32), valid=np.zeros((B, A, P), np.uint8))
     v = np.transpose(log["valid"], (0, 2, 1)) == 1                         # [B][A][T]
     x = np.transpose(log["x"], (0, 2, 1)).astype(np.float64); y = np.transpose(log["y"], (0, 2, 1)).astype(np.float64)
     yaw = np.transpose(log["yaw"], (0, 2, 1)).astype(np.float64)
-    for b in range(B):
-        for a in range(A):
-            idx = np.nonzero(v[b, a])[0]
-            if len(idx) == 0:
-                continue
-            px = list(x[b, a, idx]); py = list(y[b, a, idx])
-            th = yaw[b, a, idx[-1]]
-            for e in range(1, extend + 1):
-                px.append(px[len(idx) - 1] + e * spacing * np.cos(th)); py.append(py[len(idx) - 1] + e * spacing * np.sin(th))
-            px = np.array(px); py = np.array(py)
-            arc = np.concatenate([[0.0], np.cumsum(np.hypot(np.diff(px), np.diff(py)))])
-            n = len(px)
-            out["x"][b, a, :n] = px; out["y"][b, a, :n] = py; out["arc_len"][b, a, :n] = arc; out["valid"][b, a, :n] = 1
-    return out
+    order = np.argsort(~v, axis=2, kind="stable")                          # valid rows first, in time order
+    n = v.sum(axis=2)                                                      # [B][A] number of logged points
+    gx = np.take_along_axis(x, order, 2); gy = np.take_along_axis(y, order, 2); gth = np.take_along_axis(yaw, order, 2)
+    last = np.maximum(n - 1, 0)[..., None]
+    lx = np.take_along_axis(gx, last, 2); ly = np.take_along_axis(gy, last, 2); lth = np.take_along_axis(gth, last, 2)
+    j = np.arange(P)[None, None, :]
+    e = np.maximum(j - (n[..., None] - 1), 0) * spacing                    # metres beyond the last logged point
+    jj = np.minimum(j, T - 1)
+    px = np.where(j < n[..., None], np.take_along_axis(gx, np.broadcast_to(jj, (B, A, P)), 2), lx + e * np.cos(lth))
+    py = np.where(j < n[..., None], np.take_along_axis(gy, np.broadcast_to(jj, (B, A, P)), 2), ly + e * np.sin(lth))
+    ok = (j < n[..., None] + extend) & (n[..., None] > 0)
+    px = np.where(ok, px, 0.0); py = np.where(ok, py, 0.0)
+    seg = np.hypot(np.diff(px, axis=2), np.diff(py, axis=2)) * ok[..., 1:]
+    arc = np.concatenate([np.zeros((B, A, 1)), np.cumsum(seg, axis=2)], axis=2) * ok
+    return dict(x=px.astype(np.float32), y=py.astype(np.float32), arc_len=arc.astype(np.float32), valid=ok.astype(np.uint8))
