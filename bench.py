@@ -208,6 +208,73 @@ def run_supplementary(args):
                 "cpu_baseline": {"value": sb * A / dt, "unit": "ego-observations/s", "cores": oracle.num_threads(), "kind": "oracle",
                                  "sample": "first %d of %d scenarios, %.1f s wall" % (sb, B, dt), "index_sets_equal": same},
                 "e2e": None, "gpu_launches": int(launches), "clocks": None}
+    elif args.workload == "paper_tables":
+        # The SHAPE of the paper's own runtime tables on this GPU, for context: Table 2
+        # (Reset / Step / Transition / Metrics / RolloutExpert of the multi-agent environment at batch 1
+        # and 16) and Table 6 (Metrics and RolloutExpert against the number of objects).  Synthetic
+        # config-5 scenarios (A = 128 slots, R = 20 000), not WOMD; Metrics = this build's three metrics.
+        paper = {"hardware": "Nvidia V100 (Table 2 L153-L154; Table 6 L391-L400)",
+                 "table2_ms": {"1": {"reset": 0.64, "step": 0.92, "transition": 0.53, "metrics": 0.19, "rollout_expert": 73.3},
+                               "16": {"reset": 0.81, "step": 2.86, "transition": 0.51, "metrics": 2.24, "rollout_expert": "OOM"}},
+                 "table6_metrics_ms": {"1": {"8": 0.159, "128": 0.152}, "16": {"8": 0.154, "128": 0.469}},
+                 "table6_rollout_expert_ms": {"1": {"8": 27.0, "128": 36.9}}}
+        ours2, ours6m, ours6r = {}, {}, {}
+        total_launches = 0
+        for Bn in (1, 16):
+            for nobj in ((128,) if False else (8, 16, 32, 64, 128)):
+                cfg = ws.make_config(5, B=Bn, n_steps=N_STEPS)
+                log, rg = cfg["log"], cfg["roadgraph"]
+                log["valid"][:, :, nobj:] = 0                                   # subset of the objects (Table 6: "subsetted objects")
+                B, T, A = log["x"].shape
+                h = wm.wm_create()
+                log_d, rg_d = wm.to_device(log), wm.to_device(rg)
+                wm.wm_prepare(h, rg_d)
+                sim_d = wm.empty_traj_like(log_d)
+                t0 = wm.wm_reset(h, log_d, sim_d)
+                act1 = torch.from_numpy(np.ascontiguousarray(cfg["actions"][:, 0])).cuda()
+                av1 = torch.from_numpy(np.ascontiguousarray(cfg["action_valid"][:, 0])).cuda()
+                Wd = (A + 31) // 32
+                ofl = torch.empty((B, A), dtype=torch.uint8, device="cuda"); sd = torch.empty((B, A), device="cuda")
+                fl = torch.empty((B, A), dtype=torch.uint8, device="cuda"); ld = torch.empty((B, A), device="cuda"); lv = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+                act = torch.empty((B, N_STEPS, 2, A), device="cuda"); av = torch.empty((B, N_STEPS, A), dtype=torch.uint8, device="cuda")
+                out_d = wm.alloc_rollout_out(B, N_STEPS, A)
+
+                def metrics():
+                    wm.wm_metrics_overlap(h, sim_d, t0 + 1, None, ofl)
+                    wm.wm_metrics_offroad(h, sim_d, t0 + 1, sd, None, fl)
+                    wm.wm_log_divergence(h, log_d, sim_d, t0 + 1, ld, lv)
+
+                def transition():
+                    wm.wm_step(h, log_d, sim_d, t0, act1, av1)
+
+                def rollout_expert():
+                    wm.wm_expert_actions(h, log_d, t0, N_STEPS, act, av)
+                    wm.wm_reset(h, log_d, sim_d)
+                    wm.wm_rollout(h, log_d, sim_d, t0, N_STEPS, act, av, out_d)
+                l0 = wm.wm_kernel_launches(h)
+                reps = max(K, 20)
+                row = {"metrics": timed(metrics, reps, W), "rollout_expert": timed(rollout_expert, reps, W)}
+                if nobj == 128:
+                    row["reset"] = timed(lambda: wm.wm_reset(h, log_d, sim_d), reps, W)
+                    wm.wm_reset(h, log_d, sim_d)
+                    row["transition"] = timed(transition, reps, W)
+                    row["step"] = timed(lambda: (transition(), metrics()), reps, W)
+                    ours2[str(Bn)] = row
+                ours6m.setdefault(str(Bn), {})[str(nobj)] = row["metrics"]
+                ours6r.setdefault(str(Bn), {})[str(nobj)] = row["rollout_expert"]
+                total_launches += wm.wm_kernel_launches(h) - l0
+                wm.wm_destroy(h)
+        h = wm.wm_create()                                       # the common epilogue destroys `h`
+        step16 = ours2["16"]["step"]
+        line = {"metric": "agent-steps/s of one multi-agent Step (transition + overlap + offroad + log divergence) at batch 16, A = 128 (the paper's Table 2 row, context)",
+                "value": 16 * 128 / (step16 * 1e-3), "unit": "agent-steps/s", "n_gpus": 1, "steps": max(K, 20), "warmup": W, "ms_per_step": step16,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "paper_tables: config-5 scenarios at batch 1 and 16, 8..128 objects valid; each entry point called from Python, "
+                                       "CUDA events around the calls (launch-latency bound at these sizes)", "l2": "everything fits L2 at batch <= 16 (as in the paper's tables); not flushed"},
+                "ours_ms": {"table2": ours2, "table6_metrics": ours6m, "table6_rollout_expert": ours6r}, "paper_ms": paper,
+                "roofline": {"bound": "hbm", "achieved": None, "peak": hbm_peak, "unit": "GB/s", "frac": None, "traffic": None,
+                             "note": "latency-bound micro-batches: no roofline claim; see the default workload"},
+                "cpu_baseline": None, "e2e": None, "gpu_launches": int(total_launches), "clocks": None}
     elif args.workload == "expert":
         # RolloutExpert (Table 2): expert actions from the log by inverse kinematics, the
         # 80-step rollout with them, then the kinematic-infeasibility metric of the simulated rows (L104)
@@ -349,7 +416,7 @@ def main():
     ap.add_argument("--cpu-B", type=int, default=256, help="oracle sample for cpu_baseline (256 scenarios: ~15 s on 16 cores)")
     ap.add_argument("--ref-B", type=int, default=64, help="oracle sample per step of --impl reference (~4 s on 16 cores)")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4", "expert"],
+    ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4", "expert", "paper_tables"],
                     help="rollout = the BASELINE metric (config 5, default); the others time the remaining "
                          "SURVEY 8(a) rows on configs 3, 2, 4 (supplementary lines, same JSON shape)")
     ap.add_argument("--no-e2e", action="store_true")
