@@ -14,7 +14,9 @@
 // query is then: one 8-byte header load, a walk over ~7 candidate records, no bounding tests.
 // Cells with too many runs, and points outside both grids, take a warp search over all 32-record
 // chunks with bounding-box culling, which is exact as well.  Per-pair arithmetic is the same as in
-// the brute-force kernel (wm_offroad.cu), so both modes return the same distances bit for bit.
+// the brute-force kernel (wm_offroad.cu): both modes return the same bits whenever they pick the
+// same segment; at a polyline vertex, where rules P / N keep only the neighbour that wins in exact
+// arithmetic, the float32 distances of the two neighbours can differ by an ulp, and so can the modes.
 #pragma once
 #include <float.h>
 
