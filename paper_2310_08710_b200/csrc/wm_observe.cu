@@ -216,7 +216,7 @@ struct TkShared {
   uint2 col[TK_CAP];
   int scan[TK_THREADS / 32];
   uint32_t lo, hi, T;            // undecided key range [lo, hi); exact threshold
-  int shift, c_less, in_bin, n_col, quota, m, count, again;
+  int shift, c_less, in_bin, n_col, quota, m, count, again, n_tie;
 };
 
 // exclusive prefix sum of v over the CTA; total in `total`
@@ -314,6 +314,7 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
     if (lane == 0) { S.m = m; S.count = c; }
   }
   for (int i = tid; i < 2 * Wd; i += TK_THREADS) s_bits[i] = 0u;
+  if (tid == 0) S.n_tie = 0;
   __syncthreads();
 
   // one pass over the points of the current square: f(key, sorted position)
@@ -401,41 +402,61 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
   // ---- 4. mark the selected points over the roadgraph indices ----
   const uint32_t T = S.T;
   for_square([&](uint32_t key, int s) {
-    if (key <= T) { const int idx = __ldg(pidx + s); atomicOr((key < T ? bm : tb) + (idx >> 5), 1u << (idx & 31)); }
+    if (key <= T) {
+      const int idx = __ldg(pidx + s);
+      atomicOr((key < T ? bm : tb) + (idx >> 5), 1u << (idx & 31));
+      if (key == T) atomicAdd(&S.n_tie, 1);
+    }
   });
   __syncthreads();
-  // Words are dealt round-robin (word r * 128 + tid in round r): the selected points cluster in index
-  // ranges (polylines near the ego), and this spreads a cluster over all threads.
-  const int rounds = (Wd + TK_THREADS - 1) / TK_THREADS;
-  {                                                       // the first `quota` ties in index order
-    int c = 0, total;
-    for (int w = tid; w < Wd; w += TK_THREADS) c += __popc(tb[w]);
-    tk_block_scan(c, S.scan, total);
-    const int quota = S.quota;
-    if (total <= quota) { for (int w = tid; w < Wd; w += TK_THREADS) bm[w] |= tb[w]; }
-    else {
-      int base = 0;
-      for (int r = 0; r < rounds; ++r) {
-        const int w = r * TK_THREADS + tid;
-        uint32_t t = w < Wd ? tb[w] : 0u;
-        const int n = __popc(t);
-        int tot_r;
-        const int left = quota - (base + tk_block_scan(n, S.scan, tot_r));
-        if (left < n) { for (int drop = n - max(left, 0); drop > 0; --drop) t &= ~(0x80000000u >> __clz(t)); }   // keep the lowest bits
-        if (w < Wd) bm[w] |= t;
-        base += tot_r;
-      }
+  // The first `quota` ties in index order join the selection.  Nearly always every tie is taken
+  // (n_tie == quota); otherwise the tie words are trimmed in index order, word r * 128 + tid in round r.
+  const int quota = S.quota, n_tie = S.n_tie;
+  const bool trim = n_tie > quota;
+  if (trim) {
+    const int rounds = (Wd + TK_THREADS - 1) / TK_THREADS;
+    int base = 0;
+    for (int r = 0; r < rounds; ++r) {
+      const int w = r * TK_THREADS + tid;
+      uint32_t t = w < Wd ? tb[w] : 0u;
+      const int n = __popc(t);
+      int tot_r;
+      const int left = quota - (base + tk_block_scan(n, S.scan, tot_r));
+      if (left < n) { for (int drop = n - max(left, 0); drop > 0; --drop) t &= ~(0x80000000u >> __clz(t)); }   // keep the lowest bits
+      if (w < Wd) bm[w] |= t;
+      base += tot_r;
     }
+    __syncthreads();
   }
   // ---- 5. the set bits in ascending index order -> list, then features with coalesced stores ----
-  int n_out = 0;
-  for (int r = 0; r < rounds; ++r) {
-    const int w = r * TK_THREADS + tid;
-    uint32_t bits = w < Wd ? bm[w] : 0u;
-    int tot_r;
-    int pos = n_out + tk_block_scan(__popc(bits), S.scan, tot_r);
+  // Each warp owns a contiguous quarter of the words, its lanes interleaved over them (the selected
+  // points cluster in index ranges - polylines near the ego - and this spreads a cluster over the
+  // lanes); positions come from one exchange of the warp totals and shuffle scans, no block barrier.
+  const int Q = (Wd + TK_THREADS / 32 - 1) / (TK_THREADS / 32), wb = warp * Q, we = min(wb + Q, Wd);
+  {
+    int c = 0;
+    for (int w = wb + lane; w < we; w += 32) {
+      uint32_t v = bm[w];
+      if (!trim) { v |= tb[w]; bm[w] = v; }
+      c += __popc(v);
+    }
+    c = __reduce_add_sync(0xffffffffu, c);
+    if (lane == 0) S.scan[warp] = c;
+  }
+  __syncthreads();
+  int run = 0, n_out = 0;
+#pragma unroll
+  for (int w = 0; w < TK_THREADS / 32; ++w) { const int t = S.scan[w]; if (w < warp) run += t; n_out += t; }
+  for (int w0 = wb; w0 < we; w0 += 32) {
+    const int w = w0 + lane;
+    uint32_t bits = w < we ? bm[w] : 0u;
+    const int n = __popc(bits);
+    int inc = n;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += u; }
+    int pos = run + inc - n;
     while (bits) { if (pos < k) list[pos] = w * 32 + __ffs(bits) - 1; ++pos; bits &= bits - 1; }
-    n_out += tot_r;
+    run += __shfl_sync(0xffffffffu, inc, 31);
   }
   __syncthreads();
   n_out = min(n_out, k);
