@@ -294,17 +294,19 @@ def test_rollout_fused_equals_stepwise_bitwise(cfgid, dyn, n):
     assert res[0][1]["offroad"].sum() > 0
 
 
-def test_rollout_host_matches_device_rollout(cfg1):
+@pytest.mark.parametrize("mode", ["fused", "stepwise"])
+def test_rollout_host_matches_device_rollout(cfg1, mode):
     log, rg = cfg1["log"], cfg1["roadgraph"]
     B, T, A = log["x"].shape
     n = 30
-    h, log_d, rg_d, sim_d, _ = _setup(cfg1)
+    kw = {} if mode == "fused" else {"rollout_mode": wm.WM_ROLLOUT_STEPWISE}
+    h, log_d, rg_d, sim_d, _ = _setup(cfg1, **kw)
     t0 = wm.wm_reset(h, log_d, sim_d)
     acts = np.ascontiguousarray(cfg1["actions"][:, :n]); av = np.ascontiguousarray(cfg1["action_valid"][:, :n])
     out_d = wm.alloc_rollout_out(B, n, A)
     wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out_d)
     torch.cuda.synchronize()
-    h2 = wm.wm_create()
+    h2 = wm.wm_create(**kw)
     pin = lambda d: {k: torch.from_numpy(v).pin_memory() for k, v in d.items()}
     out_h = wm.alloc_rollout_out(B, n, A, device="cpu", pin=True)
     sim_h = {k: torch.zeros_like(v).pin_memory() for k, v in pin(log).items()}
