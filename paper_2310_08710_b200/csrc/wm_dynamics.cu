@@ -242,63 +242,72 @@ cudaError_t wm_launch_kinematic(wm_handle* h, const wm_traj& tr, int t, int n_st
 }
 
 // ---------------------------------------------------------------------------------------
-// Route-progress ratio, PAPER.md L96 (readings D33-D35).  One warp per (scenario, agent): three
-// closest-point searches over the agent's P path points (the simulated position and the first / last
-// valid logged position), lanes over points, (key, index) argmin by shuffles with the lower index
+// Route-progress ratio, PAPER.md L96 (readings D33-D35).  One warp per agent: three closest-point
+// searches over the agent's P path points (the simulated position and the first / last valid logged
+// position) in one pass, lanes over points, (key, index) argmin by shuffles with the lower index
 // winning ties.  Reads 9 B per path point once per agent: HBM bound.
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_route_progress(wm_traj log, wm_traj sim, int t, wm_paths pa, float* ratio, uint8_t* valid) {
-  const int lane = threadIdx.x & 31;
-  const int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-  const int A = sim.A, T = sim.T;
-  if (w >= (int64_t)sim.B * A) return;
-  const int b = (int)(w / A), a = (int)(w % A);
-  // first / last valid logged row (D34): lanes over rows
-  int tf = 0x7fffffff, tl = -1;
-  for (int k = lane; k < T; k += 32)
-    if (log.valid[((int64_t)b * T + k) * A + a] != 0) { tf = min(tf, k); tl = max(tl, k); }
-  tf = __reduce_min_sync(0xffffffffu, tf); tl = __reduce_max_sync(0xffffffffu, tl);
-  const int64_t rs = ((int64_t)b * T + t) * A + a;
-  const bool sv = sim.valid[rs] != 0 && tl >= 0;
-  float qx[3] = {0.f, 0.f, 0.f}, qy[3] = {0.f, 0.f, 0.f};
-  if (sv) {
-    const int64_t r0 = ((int64_t)b * T + tf) * A + a, r1 = ((int64_t)b * T + tl) * A + a;
-    qx[0] = sim.x[rs]; qy[0] = sim.y[rs]; qx[1] = log.x[r0]; qy[1] = log.y[r0]; qx[2] = log.x[r1]; qy[2] = log.y[r1];
+  // one CTA per (scenario, 32 consecutive agents): the first / last valid logged row of the 32 agents
+  // from coalesced 32-byte pieces of the valid plane (lane = agent, warps over rows), then 4 agents per warp
+  __shared__ int s_tf[32], s_tl[32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int A = sim.A, T = sim.T, b = blockIdx.y, a0 = blockIdx.x * 32;
+  if (threadIdx.x < 32) { s_tf[threadIdx.x] = 0x7fffffff; s_tl[threadIdx.x] = -1; }
+  __syncthreads();
+  {
+    int tf = 0x7fffffff, tl = -1;                            // D34
+    if (a0 + lane < A)
+      for (int k = warp; k < T; k += 8)
+        if (log.valid[((int64_t)b * T + k) * A + a0 + lane] != 0) { tf = min(tf, k); tl = max(tl, k); }
+    if (tl >= 0) { atomicMin(&s_tf[lane], tf); atomicMax(&s_tl[lane], tl); }
   }
-  const int64_t po = ((int64_t)b * pa.A + a) * pa.P;
-  unsigned long long best[3] = {~0ull, ~0ull, ~0ull};       // (key bits << 32) | index: keys are >= +0, so the bits order as floats
-  if (sv)
-    for (int i = lane; i < pa.P; i += 32) {
-      if (pa.valid[po + i] == 0) continue;
-      const float px = pa.x[po + i], py = pa.y[po + i];
+  __syncthreads();
+  for (int q = 0; q < 4; ++q) {
+    const int ai = warp * 4 + q, a = a0 + ai;
+    if (a >= A) break;                                       // warp-uniform
+    const int tf = s_tf[ai], tl = s_tl[ai];
+    const int64_t rs = ((int64_t)b * T + t) * A + a;
+    const bool sv = sim.valid[rs] != 0 && tl >= 0;
+    float qx[3] = {0.f, 0.f, 0.f}, qy[3] = {0.f, 0.f, 0.f};
+    if (sv) {
+      const int64_t r0 = ((int64_t)b * T + tf) * A + a, r1 = ((int64_t)b * T + tl) * A + a;
+      qx[0] = sim.x[rs]; qy[0] = sim.y[rs]; qx[1] = log.x[r0]; qy[1] = log.y[r0]; qx[2] = log.x[r1]; qy[2] = log.y[r1];
+    }
+    const int64_t po = ((int64_t)b * pa.A + a) * pa.P;
+    unsigned long long best[3] = {~0ull, ~0ull, ~0ull};     // (key bits << 32) | index: keys are >= +0, so the bits order as floats
+    if (sv)
+      for (int i = lane; i < pa.P; i += 32) {
+        if (pa.valid[po + i] == 0) continue;
+        const float px = pa.x[po + i], py = pa.y[po + i];
 #pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        const float dx = __fsub_rn(px, qx[c]), dy = __fsub_rn(py, qy[c]);
-        const unsigned long long kv = ((unsigned long long)__float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx))) << 32) | (unsigned)i;
-        best[c] = min(best[c], kv);                          // NaN coordinates of a valid point would order last-ish; inputs are finite where valid
+        for (int c = 0; c < 3; ++c) {
+          const float dx = __fsub_rn(px, qx[c]), dy = __fsub_rn(py, qy[c]);
+          const unsigned long long kv = ((unsigned long long)__float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx))) << 32) | (unsigned)i;
+          best[c] = min(best[c], kv);                        // ties -> lower index (D33)
+        }
       }
-    }
 #pragma unroll
-  for (int c = 0; c < 3; ++c)
+    for (int c = 0; c < 3; ++c)
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) best[c] = min(best[c], __shfl_xor_sync(0xffffffffu, best[c], d));
-  if (lane == 0) {
-    float r = 0.f;
-    uint8_t v = 0;
-    if (sv && best[0] != ~0ull) {
-      const float dx = pa.arc_len[po + (int)(best[0] & 0xffffffffu)], dp = pa.arc_len[po + (int)(best[1] & 0xffffffffu)],
-                  dq = pa.arc_len[po + (int)(best[2] & 0xffffffffu)];
-      if (dq != dp) { r = (dx - dp) / (dq - dp); v = 1; }     // D35
+      for (int d = 16; d > 0; d >>= 1) best[c] = min(best[c], __shfl_xor_sync(0xffffffffu, best[c], d));
+    if (lane == 0) {
+      float r = 0.f;
+      uint8_t v = 0;
+      if (sv && best[0] != ~0ull) {
+        const float dx = pa.arc_len[po + (int)(best[0] & 0xffffffffu)], dp = pa.arc_len[po + (int)(best[1] & 0xffffffffu)],
+                    dq = pa.arc_len[po + (int)(best[2] & 0xffffffffu)];
+        if (dq != dp) { r = (dx - dp) / (dq - dp); v = 1; }   // D35
+      }
+      ratio[(int64_t)b * A + a] = r;
+      valid[(int64_t)b * A + a] = v;
     }
-    ratio[(int64_t)b * A + a] = r;
-    valid[(int64_t)b * A + a] = v;
   }
 }
 
 cudaError_t wm_launch_route_progress(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t, const wm_paths& pa, float* ratio,
                                      uint8_t* valid, cudaStream_t s) {
-  const int64_t warps = (int64_t)sim.B * sim.A;
-  k_route_progress<<<(unsigned)((warps + 7) / 8), 256, 0, s>>>(log, sim, t, pa, ratio, valid);
+  k_route_progress<<<dim3((sim.A + 31) / 32, sim.B), 256, 0, s>>>(log, sim, t, pa, ratio, valid);
   h->launches++;
   return cudaGetLastError();
 }
