@@ -40,14 +40,14 @@
 #define FUSED_NT 256
 #endif
 #ifndef FUSED_MINB
-#define FUSED_MINB 4
+#define FUSED_MINB 5
 #endif
 constexpr int FUSED_S = 8;                 // steps per block: 8, 4, 2 or 1 (fewer when A is large: shared memory)
 constexpr float FUSED_HASH_H = 24.f;       // hash cell side, metres
 constexpr float FUSED_EXT_MAX = 11.7f;     // half extent limit of hashed agents (< FUSED_HASH_H / 2, with margin)
 constexpr uint32_t FUSED_EMPTY = 0xffffu;
 constexpr int FUSED_PAD = 4;                // slot rows are Ap + 4 long: the 8 steps of an agent fall into 8 different banks
-constexpr int FUSED_PL = 96;                // pair list entries per warp (overlap narrow phase)
+constexpr int FUSED_PL = 48;                // pair list entries per warp (overlap narrow phase)
 
 struct FusedParams {
   wm_traj log, sim;
@@ -69,7 +69,7 @@ __host__ __device__ inline size_t fused_persist_bytes(int Ap) {
 __host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)(Ap + FUSED_PAD) * (7 * 4 + 2); }
 static inline int fused_pick_S(int A) {
   const int Ap = (A + 31) / 32 * 32;
-  const size_t budget = 54 * 1024;                        // 4 CTAs per SM when it fits
+  const size_t budget = 45400;                           // 5 CTAs per SM when it fits (48 registers, FUSED_MINB)                       // 4 CTAs per SM when it fits
   const size_t per = fused_persist_bytes(Ap), slot = fused_slot_bytes(Ap);
   const int fit = per + slot >= budget ? 1 : (int)((budget - per) / slot);
   int S = FUSED_S;
