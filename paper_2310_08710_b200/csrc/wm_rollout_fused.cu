@@ -69,7 +69,7 @@ __host__ __device__ inline size_t fused_persist_bytes(int Ap) {
 __host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)(Ap + FUSED_PAD) * (7 * 4 + 2); }
 static inline int fused_pick_S(int A) {
   const int Ap = (A + 31) / 32 * 32;
-  const size_t budget = 45400;                           // 5 CTAs per SM when it fits (48 registers, FUSED_MINB)                       // 4 CTAs per SM when it fits
+  const size_t budget = 45400;                            // 5 CTAs per SM when it fits (48 registers, FUSED_MINB)
   const size_t per = fused_persist_bytes(Ap), slot = fused_slot_bytes(Ap);
   const int fit = per + slot >= budget ? 1 : (int)((budget - per) / slot);
   int S = FUSED_S;
