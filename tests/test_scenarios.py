@@ -59,3 +59,27 @@ def test_config4_lot():
     assert c["log"]["x"].shape == (2, 1, 512) and c["roadgraph"]["x"].shape == (2, 5000)
     assert (c["roadgraph"]["type"] == ws.TYPE_ROAD_EDGE).all() and (c["log"]["valid"] == 1).all()
     assert c["log"]["x"].min() > -1 and c["log"]["x"].max() < 49 and c["log"]["y"].max() < 193
+
+
+def test_make_paths_structure():
+    """Synthetic on-route paths: logged positions in time order, then a straight extension; arc length
+    non-decreasing from 0; agents never logged have no path; deterministic."""
+    cfg = ws.make_config(1, n_steps=2)
+    log = cfg["log"]
+    B, T, A = log["x"].shape
+    pa = ws.make_paths(log, extend=16)
+    pb = ws.make_paths(log, extend=16)
+    for k in pa:
+        assert np.array_equal(pa[k], pb[k]) and pa[k].shape == (B, A, T + 16)
+    n_logged = (log["valid"] == 1).sum(axis=1)                      # [B][A]
+    n_path = (pa["valid"] == 1).sum(axis=2)
+    assert np.array_equal(n_path, np.where(n_logged > 0, n_logged + 16, 0))
+    v = pa["valid"] == 1
+    assert np.all(v[:, :, :-1] >= v[:, :, 1:])                      # valid points form a prefix
+    d = np.diff(pa["arc_len"].astype(np.float64), axis=2)
+    assert np.all(d[v[:, :, 1:]] >= 0) and np.all(pa["arc_len"][:, :, 0] == 0)
+    assert np.isfinite(pa["x"]).all() and np.isfinite(pa["y"]).all()
+    # the first point is the first valid logged position
+    b, a = np.argwhere(n_logged > 0)[0]
+    t0 = int(np.argmax(log["valid"][b, :, a] == 1))
+    assert pa["x"][b, a, 0] == log["x"][b, t0, a] and pa["y"][b, a, 0] == log["y"][b, t0, a]
