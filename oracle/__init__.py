@@ -218,3 +218,22 @@ def route_progress(log, sim, t, paths):
     ratio = np.empty((B, A), np.float32); val = np.empty((B, A), np.uint8); cl = np.empty((B, 3, A), np.int32)
     lib().orc_route_progress(C.byref(ls), C.byref(ss), C.c_int32(t), C.byref(ps), _p(ratio), _p(val), _p(cl))
     return dict(ratio=ratio, valid=val, closest=cl)
+
+
+def _paths(paths, B, A):
+    P = paths["x"].shape[2]
+    for k in ("x", "y", "arc_len"):
+        _check(paths[k], np.float32, (B, A, P))
+    _check(paths["valid"], np.uint8, (B, A, P))
+    return _Paths(B, A, P, _p(paths["x"]), _p(paths["y"]), _p(paths["arc_len"]), _p(paths["valid"]))
+
+
+def offroute(sim, t, on_route, off_route, max_dist, margin):
+    """O12 (L98; thresholds are arguments, D36). off_route may be None."""
+    ss, (B, T, A) = _traj(sim)
+    on = _paths(on_route, B, A)
+    off = _paths(off_route, B, A) if off_route is not None else None
+    d = np.empty((B, A), np.float32); f = np.empty((B, A), np.uint8)
+    lib().orc_offroute(C.byref(ss), C.c_int32(t), C.byref(on), C.byref(off) if off is not None else None,
+                       C.c_float(max_dist), C.c_float(margin), _p(d), _p(f))
+    return dict(dist_on=d, flag=f)

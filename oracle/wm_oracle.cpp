@@ -604,6 +604,43 @@ void orc_route_progress(const orc_traj* log, const orc_traj* sim, int32_t t, con
     }
 }
 
+// -------------------------------------------------------------------------------------
+// O12 off-route metric: "If the vehicle is sufficiently closer to an off-route path
+// than on-route path or it is far enough away from an on-route path, it is considered off-route."
+// The two thresholds are not in the paper: they are arguments (D36).  d_on / d_off = distance from
+// the agent's position at row t to the closest valid point of its on-route / off-route path
+// (closest POINT, float32 key and float32 square root as in D33; +inf without an off-route point);
+//   flag = d_on > max_dist  ||  d_off + margin < d_on
+// for agents valid at t that have an on-route path point; otherwise flag 0, dist 0.
+// off may be NULL (no off-route paths).  dist_on [B][A] (float32), flag [B][A].
+// -------------------------------------------------------------------------------------
+static float closest_path_dist(const orc_paths* pa, int b, int a, float qx, float qy, bool* found) {
+  const int i = closest_path_point(pa, b, a, qx, qy);
+  *found = i >= 0;
+  if (i < 0) return INFINITY;
+  const size_t o = ((size_t)b * pa->A + a) * pa->P + i;
+  const float dx = pa->x[o] - qx, dy = pa->y[o] - qy;                  // float32 on purpose (D33 / D36)
+  return std::sqrt(std::fmaf(dy, dy, dx * dx));
+}
+
+void orc_offroute(const orc_traj* sim, int32_t t, const orc_paths* on, const orc_paths* off, float max_dist, float margin,
+                  float* dist_on, uint8_t* flag) {
+  const int B = sim->B, A = sim->A;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b)
+    for (int a = 0; a < A; ++a) {
+      const size_t o = (size_t)b * A + a, rs = row(sim, b, t) + a;
+      dist_on[o] = 0.f; flag[o] = 0;
+      if (!sim->valid[rs]) continue;
+      bool f_on = false, f_off = false;
+      const float d_on = closest_path_dist(on, b, a, sim->x[rs], sim->y[rs], &f_on);
+      if (!f_on) continue;
+      const float d_off = off ? closest_path_dist(off, b, a, sim->x[rs], sim->y[rs], &f_off) : INFINITY;
+      dist_on[o] = d_on;
+      flag[o] = (uint8_t)(d_on > max_dist || d_off + margin < d_on);   // L98
+    }
+}
+
 int32_t orc_num_threads() {
 #ifdef _OPENMP
   return omp_get_max_threads();

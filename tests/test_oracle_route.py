@@ -81,3 +81,26 @@ def test_log_playback_progress_runs_from_0_to_1_on_generated_paths():
     assert np.all(r0["ratio"][sel] == 0) and np.all(r1["ratio"][sel] == 1)   # the log's own first / last position (L96)
     assert np.all((rm["ratio"][sel] > 0) & (rm["ratio"][sel] <= 1))          # = 1 for agents that have braked to a stop by then
     assert (rm["ratio"][sel] < 1).sum() > sel.sum() // 2
+
+
+def test_offroute_hand_cases():
+    """O12 (L98), thresholds as arguments (D36): max_dist = 5 m, margin = 1 m.  On-route path along +x
+    (y = 0), off-route path parallel at y = 4."""
+    pts = [(10.0, 1.0), (10.0, 2.4), (10.0, 2.6), (10.0, -5.5), (10.0, -4.5), (10.3, 0.0)]
+    A = len(pts)
+    sim = mk_traj(1, 1, A)
+    for a, (x, y) in enumerate(pts):
+        set_agent(sim, 0, 0, a, x, y)
+    on = straight_path(1, A, 41)
+    off = straight_path(1, A, 41); off["y"][:] = 4.0
+    r = oracle.offroute(sim, 0, on, off, 5.0, 1.0)
+    # (10,1): d_on 1, d_off 3 -> on route.  (10,2.4): 2.4 vs 1.6 + 1 = 2.6 -> on.  (10,2.6): 2.6 vs 1.4 + 1 = 2.4 -> OFF.
+    # (10,-5.5): d_on 5.5 > 5 -> OFF.  (10,-4.5): 4.5 -> on.  (10.3, 0): nearest point (10, 0): d_on 0.3 -> on.
+    assert r["flag"][0].tolist() == [0, 0, 1, 1, 0, 0]
+    assert np.allclose(r["dist_on"][0], [1.0, 2.4, 2.6, 5.5, 4.5, 0.3], atol=1e-6)
+    # without off-route paths only the distance rule is left
+    assert oracle.offroute(sim, 0, on, None, 5.0, 1.0)["flag"][0].tolist() == [0, 0, 0, 1, 0, 0]
+    # invalid agents and agents without an on-route path are never flagged
+    sim["valid"][0, 0, 3] = 0; on["valid"][0, 2, :] = 0
+    r = oracle.offroute(sim, 0, on, off, 5.0, 1.0)
+    assert r["flag"][0].tolist() == [0, 0, 0, 0, 0, 0] and r["dist_on"][0, 3] == 0 and r["dist_on"][0, 2] == 0
