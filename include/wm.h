@@ -223,6 +223,19 @@ int wm_metrics_route_progress(wm_handle* h, const wm_traj* log, const wm_traj* s
                               const wm_paths* paths, float* ratio, uint8_t* valid, void* stream);
 
 /*
+ * Off-route metric, L98: "sufficiently closer to an off-route path than on-route path or ... far
+ * enough away from an on-route path".  The paper gives no thresholds: they are arguments (D36).
+ * d_on / d_off = distance from the agent's position at row t to the closest valid point of its
+ * on-route / off-route path (float32 key and square root; +inf without an off-route point);
+ *   flag = d_on > max_dist || d_off + margin < d_on
+ * for agents valid at t with an on-route path point, else flag 0 and dist_on 0.  off_route may be
+ * NULL.  dist_on [B][A] (may be NULL), flag [B][A].
+ */
+int wm_metrics_offroute(wm_handle* h, const wm_traj* sim, int32_t t, const wm_paths* on_route,
+                        const wm_paths* off_route, float max_dist, float margin, float* dist_on,
+                        uint8_t* flag, void* stream);
+
+/*
  * Rollout, L200: for s = 0 .. n_steps-1: wm_step at t0+s, then overlap, offroad and log
  * divergence on row t0+s+1 (D11), written to row s of the per-step outputs; aggregates over
  * the n_steps rows at the end.  The whole sequence is one CUDA graph, captured on the first

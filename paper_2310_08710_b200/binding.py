@@ -23,7 +23,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
+           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
 
 
 class wm_traj(C.Structure):
@@ -193,12 +193,24 @@ class wm_paths(C.Structure):
                 ("arc_len", C.c_void_p), ("valid", C.c_void_p)]
 
 
-def wm_metrics_route_progress(h, log, sim, t, paths, ratio, valid, stream=None):
+def paths_struct(paths):
     """paths: dict of device tensors x, y, arc_len float32 [B][A][P], valid uint8 [B][A][P]."""
-    ls, ss = traj_struct(log), traj_struct(sim)
     B, A, P = paths["x"].shape
-    ps = wm_paths(B, A, P, _ptr(paths["x"], torch.float32), _ptr(paths["y"], torch.float32), _ptr(paths["arc_len"], torch.float32),
-                  _ptr(paths["valid"], torch.uint8))
+    return wm_paths(B, A, P, _ptr(paths["x"], torch.float32), _ptr(paths["y"], torch.float32), _ptr(paths["arc_len"], torch.float32),
+                    _ptr(paths["valid"], torch.uint8))
+
+
+def wm_metrics_offroute(h, sim, t, on_route, off_route, max_dist, margin, dist_on, flag, stream=None):
+    ss, on = traj_struct(sim), paths_struct(on_route)
+    off = paths_struct(off_route) if off_route is not None else None
+    _check(load().wm_metrics_offroute(h, C.byref(ss), C.c_int32(t), C.byref(on), C.byref(off) if off is not None else None,
+                                      C.c_float(max_dist), C.c_float(margin), _ptr(dist_on, torch.float32), _ptr(flag, torch.uint8),
+                                      _stream(stream)), "wm_metrics_offroute")
+
+
+def wm_metrics_route_progress(h, log, sim, t, paths, ratio, valid, stream=None):
+    ls, ss = traj_struct(log), traj_struct(sim)
+    ps = paths_struct(paths)
     _check(load().wm_metrics_route_progress(h, C.byref(ls), C.byref(ss), C.c_int32(t), C.byref(ps), _ptr(ratio, torch.float32),
                                             _ptr(valid, torch.uint8), _stream(stream)), "wm_metrics_route_progress")
 

@@ -189,6 +189,18 @@ extern "C" int wm_metrics_route_progress(wm_handle* h, const wm_traj* log, const
   return WM_OK;
 }
 
+static bool paths_ok(const wm_paths* p, const wm_traj* sim) {
+  return p && p->B == sim->B && p->A == sim->A && p->P >= 1 && p->x && p->y && p->arc_len && p->valid;
+}
+
+extern "C" int wm_metrics_offroute(wm_handle* h, const wm_traj* sim, int32_t t, const wm_paths* on_route, const wm_paths* off_route,
+                                   float max_dist, float margin, float* dist_on, uint8_t* flag, void* stream) {
+  if (!h || !traj_ok(sim) || !paths_ok(on_route, sim) || (off_route && !paths_ok(off_route, sim)) || !flag) return WM_ERR_ARG;
+  if (t < 0 || t >= sim->T || !(max_dist >= 0.f) || !(margin >= 0.f)) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_offroute(h, *sim, t, *on_route, off_route, max_dist, margin, dist_on, flag, (cudaStream_t)stream));
+  return WM_OK;
+}
+
 extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t t, float* hist,
                           uint8_t* hist_valid, int32_t* rg_index, float* rg_feat, int32_t* rg_type, void* stream) {
   if (!h || !traj_ok(sim)) return WM_ERR_ARG;

@@ -311,3 +311,56 @@ cudaError_t wm_launch_route_progress(wm_handle* h, const wm_traj& log, const wm_
   h->launches++;
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------
+// Off-route metric, PAPER.md L98 (reading D36: thresholds are arguments).  One warp per agent, lanes
+// over the points of its on-route and off-route path; float32 keys, min by shuffles.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_offroute(wm_traj sim, int t, wm_paths on, wm_paths off, int has_off, float max_dist,
+                                                  float margin, float* dist_on, uint8_t* flag) {
+  const int lane = threadIdx.x & 31;
+  const int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int A = sim.A;
+  if (w >= (int64_t)sim.B * A) return;
+  const int b = (int)(w / A), a = (int)(w % A);
+  const int64_t rs = ((int64_t)b * sim.T + t) * A + a;
+  const bool sv = sim.valid[rs] != 0;
+  const float qx = sv ? sim.x[rs] : 0.f, qy = sv ? sim.y[rs] : 0.f;
+  uint32_t k_on = 0xffffffffu, k_off = 0xffffffffu;          // float bits of the smallest key (keys are >= +0)
+  if (sv) {
+    const int64_t po = ((int64_t)b * on.A + a) * on.P;
+    for (int i = lane; i < on.P; i += 32)
+      if (on.valid[po + i] != 0) {
+        const float dx = __fsub_rn(on.x[po + i], qx), dy = __fsub_rn(on.y[po + i], qy);
+        k_on = min(k_on, __float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
+      }
+    if (has_off) {
+      const int64_t pf = ((int64_t)b * off.A + a) * off.P;
+      for (int i = lane; i < off.P; i += 32)
+        if (off.valid[pf + i] != 0) {
+          const float dx = __fsub_rn(off.x[pf + i], qx), dy = __fsub_rn(off.y[pf + i], qy);
+          k_off = min(k_off, __float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
+        }
+    }
+  }
+  k_on = __reduce_min_sync(0xffffffffu, k_on); k_off = __reduce_min_sync(0xffffffffu, k_off);
+  if (lane == 0) {
+    float d = 0.f;
+    uint8_t f = 0;
+    if (sv && k_on != 0xffffffffu) {
+      d = __fsqrt_rn(__uint_as_float(k_on));
+      const float d_off = k_off != 0xffffffffu ? __fsqrt_rn(__uint_as_float(k_off)) : __int_as_float(0x7f800000);
+      f = (uint8_t)(d > max_dist || __fadd_rn(d_off, margin) < d);    // L98
+    }
+    if (dist_on) dist_on[(int64_t)b * A + a] = d;
+    flag[(int64_t)b * A + a] = f;
+  }
+}
+
+cudaError_t wm_launch_offroute(wm_handle* h, const wm_traj& sim, int t, const wm_paths& on, const wm_paths* off, float max_dist,
+                               float margin, float* dist_on, uint8_t* flag, cudaStream_t s) {
+  const int64_t warps = (int64_t)sim.B * sim.A;
+  k_offroute<<<(unsigned)((warps + 7) / 8), 256, 0, s>>>(sim, t, on, off ? *off : on, off != nullptr, max_dist, margin, dist_on, flag);
+  h->launches++;
+  return cudaGetLastError();
+}

@@ -179,3 +179,35 @@ def test_route_progress_matches_oracle():
             assert v.sum() > 0.5 * (sim["valid"][:, t] == 1).sum()
         # the reset state sits on its own logged position: progress of agents logged from step 0 at t0 = progress of the log
         wm.wm_destroy(h)
+
+
+def test_offroute_matches_oracle_bit_for_bit():
+    """wm_metrics_offroute (L98, thresholds as arguments): both sides take the closest-point decision, the
+    square root and the two comparisons in float32, so distances and flags agree exactly."""
+    n = 80
+    cfg = ws.make_config(5, B=6, n_steps=n)
+    log, rg = cfg["log"], cfg["roadgraph"]
+    B, T, A = log["x"].shape
+    on = ws.make_paths(log)
+    off = {k: np.ascontiguousarray(np.roll(v, 1, axis=1)) for k, v in on.items()}     # another agent's path as the off-route one
+    on["valid"][:, ::9, :] = 0                                    # agents without an on-route path
+    h = wm.wm_create()
+    log_d, rg_d = dev(log), dev(rg)
+    sim_d = wm.empty_traj_like(log_d)
+    wm.wm_prepare(h, rg_d)
+    t0 = wm.wm_reset(h, log_d, sim_d)
+    out = wm.alloc_rollout_out(B, n, A)
+    wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(cfg["actions"]).cuda(), torch.from_numpy(cfg["action_valid"]).cuda(), out)
+    on_d = {k: torch.from_numpy(v).cuda() for k, v in on.items()}
+    off_d = {k: torch.from_numpy(v).cuda() for k, v in off.items()}
+    sim = host(sim_d)
+    total = 0
+    for t, offp, offd in ((t0 + n, off, off_d), (t0 + 40, None, None)):
+        d = torch.full((B, A), 7.0, device="cuda"); f = torch.full((B, A), 9, dtype=torch.uint8, device="cuda")
+        wm.wm_metrics_offroute(h, sim_d, t, on_d, offd, 5.0, 1.0, d, f)
+        torch.cuda.synchronize()
+        r = oracle.offroute(sim, t, on, offp, 5.0, 1.0)
+        assert np.array_equal(d.cpu().numpy(), r["dist_on"]) and np.array_equal(f.cpu().numpy(), r["flag"])
+        total += int(r["flag"].sum())
+        assert 0 < r["flag"].sum() < (sim["valid"][:, t] == 1).sum()
+    wm.wm_destroy(h)
