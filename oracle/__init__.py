@@ -237,3 +237,22 @@ def offroute(sim, t, on_route, off_route, max_dist, margin):
     lib().orc_offroute(C.byref(ss), C.c_int32(t), C.byref(on), C.byref(off) if off is not None else None,
                        C.c_float(max_dist), C.c_float(margin), _p(d), _p(f))
     return dict(dist_on=d, flag=f)
+
+
+class _Idm(C.Structure):
+    _fields_ = [(k, C.c_float) for k in ("v0", "T", "s0", "a_max", "b", "delta", "b_max")]
+
+
+IDM_DEFAULTS = dict(v0=30.0, T=1.5, s0=2.0, a_max=1.0, b=1.5, delta=4.0, b_max=4.0)   # D37: declared, not from the paper
+
+
+def idm_step(sim, t, paths, idm_valid, dt=0.1, **params):
+    """O13: in place, writes row t+1 of the IDM-controlled agents (L110-L112; readings D37-D41)."""
+    ss, (B, T, A) = _traj(sim)
+    pa = _paths(paths, B, A)
+    _check(idm_valid, np.uint8, (B, A))
+    prm = dict(IDM_DEFAULTS); prm.update(params)
+    ps = _Idm(*[prm[k] for k in ("v0", "T", "s0", "a_max", "b", "delta", "b_max")])
+    acc = np.empty((B, A), np.float32); lead = np.empty((B, A), np.int32)
+    lib().orc_idm_step(C.byref(ss), C.c_int32(t), C.byref(pa), _p(idm_valid), C.byref(ps), C.c_double(dt), _p(acc), _p(lead))
+    return dict(accel=acc, lead=lead)

@@ -641,6 +641,115 @@ void orc_offroute(const orc_traj* sim, int32_t t, const orc_paths* on, const orc
     }
 }
 
+// -------------------------------------------------------------------------------------
+// O13 IDM reactive sim agent (Fig. 2b): "follows the logged path ... but uses IDM
+// to adjust the speed profile to avoid collisions and accelerate on free roads"; IDM = the
+// intelligent driver model of ref. [51] (Treiber, Hennecke, Helbing 2000):
+//     a = a_max [ 1 - (v / v0)^delta - (s* / s)^2 ],   s* = s0 + max(0, v T + v dv / (2 sqrt(a_max b)))
+// with s the bumper-to-bumper gap to the lead object and dv = v - v_lead (no lead: last term 0).
+// The paper gives no constants and no lead-finding rule; readings D37-D41:
+//   D37 the constants are arguments (orc_idm_params; defaults declared in the Python wrapper);
+//   D38 the path is the agent's on-route path (orc_paths), a polyline over index-consecutive valid
+//       points; a position's path coordinate sigma is the arc length of its projection on the
+//       nearest path segment (ties -> lower segment index);
+//   D39 lead object: among the other agents valid at t, those whose projection on THIS agent's
+//       path lies ahead (sigma_j > sigma_i) within a lateral distance of (W_i + W_j)/2; gap =
+//       sigma_j - sigma_i - (L_i + L_j)/2; the smallest gap wins, ties -> lower agent index; lead
+//       speed = |v_j|.  Projections and these decisions are taken in float32, operation for
+//       operation as the kernel does (a floating-point value that decides an index);
+//   D40 a is clamped to [-b_max, a_max], the gap to >= 0.1 m; v' = max(0, v + a dt); the agent
+//       advances ds = (v + v') dt / 2 along its path: it lands on the first segment at or after its
+//       own whose end lies beyond sigma_i + ds (linear interpolation), yaw' = that segment's
+//       direction; past the end of the path it stays on the last point with its yaw;
+//       velocity = v' (cos yaw', sin yaw'); length, width kept; valid' = 1;
+//   D41 only agents with idm_valid != 0 that are valid at t and have a path segment are written
+//       (row t+1); every other slot of row t+1 is left as it is (the caller's step fills it).
+// -------------------------------------------------------------------------------------
+struct orc_idm_params { float v0, T, s0, a_max, b, delta, b_max; };
+
+struct PathProj { int k; float u, d2, sigma; };
+
+// float32 projection of (qx, qy) on the segments (k, k+1) of agent a's path (D38)
+static PathProj project_on_path(const orc_paths* pa, int b, int a, float qx, float qy) {
+  const size_t o = ((size_t)b * pa->A + a) * pa->P;
+  PathProj best{-1, 0.f, INFINITY, 0.f};
+  for (int k = 0; k + 1 < pa->P; ++k) {
+    if (!pa->valid[o + k] || !pa->valid[o + k + 1]) continue;
+    const float ex = pa->x[o + k + 1] - pa->x[o + k], ey = pa->y[o + k + 1] - pa->y[o + k];
+    const float wx = qx - pa->x[o + k], wy = qy - pa->y[o + k];
+    const float ee = std::fmaf(ey, ey, ex * ex), dot = std::fmaf(wy, ey, wx * ex);
+    float u = 0.f;
+    if (ee > 0.f) u = std::fmin(std::fmax(dot / ee, 0.f), 1.f);
+    const float rx = std::fmaf(-u, ex, wx), ry = std::fmaf(-u, ey, wy);
+    const float d2 = std::fmaf(ry, ry, rx * rx);
+    if (d2 < best.d2) { best.k = k; best.u = u; best.d2 = d2; }
+  }
+  if (best.k >= 0) best.sigma = std::fmaf(best.u, pa->arc_len[o + best.k + 1] - pa->arc_len[o + best.k], pa->arc_len[o + best.k]);
+  return best;
+}
+
+void orc_idm_step(orc_traj* sim, int32_t t, const orc_paths* pa, const uint8_t* idm_valid, const orc_idm_params* prm, double dt,
+                  float* accel_out, int32_t* lead_out) {
+  const int B = sim->B, A = sim->A, P = pa->P;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b)
+    for (int i = 0; i < A; ++i) {
+      const size_t o = (size_t)b * A + i, r0 = row(sim, b, t) + i, r1 = row(sim, b, t + 1) + i;
+      if (accel_out) accel_out[o] = 0.f;
+      if (lead_out) lead_out[o] = -1;
+      if (!idm_valid[o] || !sim->valid[r0]) continue;
+      const PathProj self = project_on_path(pa, b, i, sim->x[r0], sim->y[r0]);
+      if (self.k < 0) continue;                                                            // D41
+      const size_t po = ((size_t)b * pa->A + i) * P;
+      // ---- lead object (D39), float32 decisions ----
+      int lead = -1;
+      float gap = INFINITY;
+      for (int j = 0; j < A; ++j) {
+        const size_t rj = row(sim, b, t) + j;
+        if (j == i || !sim->valid[rj]) continue;
+        const PathProj pj = project_on_path(pa, b, i, sim->x[rj], sim->y[rj]);
+        const float lat_max = 0.5f * (sim->width[r0] + sim->width[rj]);
+        if (!(pj.sigma > self.sigma) || pj.d2 > lat_max * lat_max) continue;
+        const float g = (pj.sigma - self.sigma) - 0.5f * (sim->length[r0] + sim->length[rj]);
+        if (g < gap) { gap = g; lead = j; }
+      }
+      // ---- IDM acceleration (ref. [51]) ----
+      const double vx = sim->vel_x[r0], vy = sim->vel_y[r0], v = std::sqrt(vx * vx + vy * vy);
+      double acc = 1.0 - std::pow(v / prm->v0, (double)prm->delta);
+      if (lead >= 0) {
+        const size_t rl = row(sim, b, t) + lead;
+        const double vl = std::sqrt((double)sim->vel_x[rl] * sim->vel_x[rl] + (double)sim->vel_y[rl] * sim->vel_y[rl]);
+        const double sstar = prm->s0 + std::max(0.0, v * prm->T + v * (v - vl) / (2.0 * std::sqrt((double)prm->a_max * prm->b)));
+        const double sgap = std::max((double)gap, 0.1);
+        acc -= (sstar / sgap) * (sstar / sgap);
+      }
+      acc *= prm->a_max;
+      acc = std::min(std::max(acc, -(double)prm->b_max), (double)prm->a_max);              // D40
+      const double v1 = std::max(0.0, v + acc * dt);
+      const double target = (double)self.sigma + 0.5 * (v + v1) * dt;
+      // ---- advance along the path (D40) ----
+      int ks = -1;
+      for (int k = self.k; k + 1 < P; ++k)
+        if (pa->valid[po + k] && pa->valid[po + k + 1] && (double)pa->arc_len[po + k + 1] > target) { ks = k; break; }
+      double xn, yn, yawn;
+      if (ks >= 0) {
+        const double ex = (double)pa->x[po + ks + 1] - pa->x[po + ks], ey = (double)pa->y[po + ks + 1] - pa->y[po + ks];
+        const double len = (double)pa->arc_len[po + ks + 1] - pa->arc_len[po + ks];
+        const double u = std::min(std::max((target - pa->arc_len[po + ks]) / len, 0.0), 1.0);
+        xn = pa->x[po + ks] + u * ex; yn = pa->y[po + ks] + u * ey; yawn = std::atan2(ey, ex);
+      } else {                                                                             // past the end: the last path point
+        int kl = self.k + 1;
+        for (int k = self.k + 1; k < P; ++k) if (pa->valid[po + k] && pa->valid[po + k - 1]) kl = k; else break;
+        xn = pa->x[po + kl]; yn = pa->y[po + kl]; yawn = sim->yaw[r0];
+      }
+      sim->x[r1] = (float)xn; sim->y[r1] = (float)yn; sim->yaw[r1] = (float)yawn;
+      sim->vel_x[r1] = (float)(v1 * std::cos(yawn)); sim->vel_y[r1] = (float)(v1 * std::sin(yawn));
+      sim->length[r1] = sim->length[r0]; sim->width[r1] = sim->width[r0]; sim->valid[r1] = 1;
+      if (accel_out) accel_out[o] = (float)acc;
+      if (lead_out) lead_out[o] = lead;
+    }
+}
+
 int32_t orc_num_threads() {
 #ifdef _OPENMP
   return omp_get_max_threads();
