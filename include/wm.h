@@ -235,6 +235,31 @@ int wm_metrics_offroute(wm_handle* h, const wm_traj* sim, int32_t t, const wm_pa
                         const wm_paths* off_route, float max_dist, float margin, float* dist_on,
                         uint8_t* flag, void* stream);
 
+/* Constants of the intelligent driver model (ref. [51] of the paper: Treiber, Hennecke, Helbing 2000).
+ * The paper gives none (D37); typical values: v0 = 30 m/s desired speed, T = 1.5 s time headway,
+ * s0 = 2 m minimum gap, a_max = 1 m/s^2, b = 1.5 m/s^2 comfortable deceleration, delta = 4,
+ * b_max = 4 m/s^2 hardest braking. */
+typedef struct { float v0, T, s0, a_max, b, delta, b_max; } wm_idm_params;
+
+/*
+ * IDM reactive sim agent, L110-L112: the agent "follows the logged path" (its `paths` polyline) with
+ * the speed profile of the intelligent driver model,
+ *   a = a_max [1 - (v/v0)^delta - (s_star/s)^2],  s_star = s0 + max(0, v T + v (v - v_lead) / (2 sqrt(a_max b))),
+ * s = bumper-to-bumper gap along the path to the lead object (no lead: last term 0).  Readings
+ * D38-D41: path coordinate = arc length of the projection on the nearest path segment;
+ * lead = the valid other agent whose projection on this agent's path is ahead, within (W_i + W_j)/2
+ * of the path, with the smallest gap sigma_j - sigma_i - (L_i + L_j)/2 (ties -> lower index), lead
+ * speed |v_j|; a clamped to [-b_max, a_max], gap to >= 0.1 m; v' = max(0, v + a dt); the agent advances
+ * (v + v') dt / 2 along the path (stops on its last point), yaw' = direction of the path piece it
+ * lands on, velocity v' (cos yaw', sin yaw').
+ * Writes row t+1 of `sim` ONLY for agents with idm_valid != 0 that are valid at row t and have a
+ * path segment (valid' = 1, box kept); every other slot of row t+1 is left untouched - call wm_step
+ * first (dynamics / log playback for everybody), then this.  Reads row t only.
+ * accel [B][A] (may be NULL): the IDM acceleration; lead [B][A] (may be NULL): lead agent or -1.
+ */
+int wm_idm_step(wm_handle* h, wm_traj* sim, int32_t t, const wm_paths* paths, const uint8_t* idm_valid,
+                const wm_idm_params* params, float* accel, int32_t* lead, void* stream);
+
 /*
  * Rollout, L200: for s = 0 .. n_steps-1: wm_step at t0+s, then overlap, offroad and log
  * divergence on row t0+s+1 (D11), written to row s of the per-step outputs; aggregates over

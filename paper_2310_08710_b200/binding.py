@@ -23,7 +23,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
+           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_idm_step", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
 
 
 class wm_traj(C.Structure):
@@ -206,6 +206,21 @@ def wm_metrics_offroute(h, sim, t, on_route, off_route, max_dist, margin, dist_o
     _check(load().wm_metrics_offroute(h, C.byref(ss), C.c_int32(t), C.byref(on), C.byref(off) if off is not None else None,
                                       C.c_float(max_dist), C.c_float(margin), _ptr(dist_on, torch.float32), _ptr(flag, torch.uint8),
                                       _stream(stream)), "wm_metrics_offroute")
+
+
+class wm_idm_params(C.Structure):
+    _fields_ = [(k, C.c_float) for k in ("v0", "T", "s0", "a_max", "b", "delta", "b_max")]
+
+
+IDM_DEFAULTS = dict(v0=30.0, T=1.5, s0=2.0, a_max=1.0, b=1.5, delta=4.0, b_max=4.0)   # D37: declared, not from the paper
+
+
+def wm_idm_step(h, sim, t, paths, idm_valid, accel=None, lead=None, stream=None, **params):
+    ss, ps = traj_struct(sim), paths_struct(paths)
+    prm = dict(IDM_DEFAULTS); prm.update(params)
+    q = wm_idm_params(*[prm[k] for k in ("v0", "T", "s0", "a_max", "b", "delta", "b_max")])
+    _check(load().wm_idm_step(h, C.byref(ss), C.c_int32(t), C.byref(ps), _ptr(idm_valid, torch.uint8), C.byref(q),
+                              _ptr(accel, torch.float32), _ptr(lead, torch.int32), _stream(stream)), "wm_idm_step")
 
 
 def wm_metrics_route_progress(h, log, sim, t, paths, ratio, valid, stream=None):

@@ -201,6 +201,17 @@ extern "C" int wm_metrics_offroute(wm_handle* h, const wm_traj* sim, int32_t t, 
   return WM_OK;
 }
 
+extern "C" int wm_idm_step(wm_handle* h, wm_traj* sim, int32_t t, const wm_paths* paths, const uint8_t* idm_valid,
+                           const wm_idm_params* params, float* accel, int32_t* lead, void* stream) {
+  if (!h || !traj_ok(sim) || !paths_ok(paths, sim) || !idm_valid || !params) return WM_ERR_ARG;
+  if (t < 0 || t + 1 >= sim->T) return WM_ERR_ARG;
+  if (!(params->v0 > 0.f) || !(params->a_max > 0.f) || !(params->b > 0.f) || !(params->b_max > 0.f) || !(params->T >= 0.f) ||
+      !(params->s0 >= 0.f) || !(params->delta > 0.f)) return WM_ERR_ARG;
+  if (paths->P > 1900) return WM_ERR_UNSUPPORTED;
+  WM_CUDA(wm_launch_idm_step(h, *sim, t, *paths, idm_valid, *params, accel, lead, (cudaStream_t)stream));
+  return WM_OK;
+}
+
 extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t t, float* hist,
                           uint8_t* hist_valid, int32_t* rg_index, float* rg_feat, int32_t* rg_type, void* stream) {
   if (!h || !traj_ok(sim)) return WM_ERR_ARG;

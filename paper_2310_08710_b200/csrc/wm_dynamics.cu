@@ -364,3 +364,146 @@ cudaError_t wm_launch_offroute(wm_handle* h, const wm_traj& sim, int t, const wm
   h->launches++;
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------
+// IDM reactive sim agent, PAPER.md L110-L112 + ref. [51]; readings D37-D41.  One warp per
+// (scenario, agent): its path is staged in shared memory, every other agent is projected on it with
+// lanes over the path segments (agents outside the path's bounding box + their lateral reach are
+// skipped: they cannot be within it of any segment).  Projections and the lead decision are float32,
+// operation for operation as DESIGN.md (D38, D39) lays them down.
+// ---------------------------------------------------------------------------------------
+struct IdmParams {
+  wm_traj sim; int t; wm_paths pa; const uint8_t* idm_valid; wm_idm_params prm; float dt;
+  float* accel; int32_t* lead;
+};
+
+struct IdmProj { int k; float u, d2, sigma; };
+
+// all lanes get the same result; sp: the warp's staged path, [0,P) x, [P,2P) y, [2P,3P) arc, then P valid bytes
+__device__ __forceinline__ IdmProj idm_project(const float* sp, const uint8_t* sv, int P, float qx, float qy) {
+  const int lane = threadIdx.x & 31;
+  unsigned long long best = ~0ull;
+  for (int k = lane; k + 1 < P; k += 32) {
+    if (sv[k] == 0 || sv[k + 1] == 0) continue;
+    const float ex = __fsub_rn(sp[k + 1], sp[k]), ey = __fsub_rn(sp[P + k + 1], sp[P + k]);
+    const float wx = __fsub_rn(qx, sp[k]), wy = __fsub_rn(qy, sp[P + k]);
+    const float ee = __fmaf_rn(ey, ey, __fmul_rn(ex, ex)), dot = __fmaf_rn(wy, ey, __fmul_rn(wx, ex));
+    float u = 0.f;
+    if (ee > 0.f) u = fminf(fmaxf(__fdiv_rn(dot, ee), 0.f), 1.f);
+    const float rx = __fmaf_rn(-u, ex, wx), ry = __fmaf_rn(-u, ey, wy);
+    const float d2 = __fmaf_rn(ry, ry, __fmul_rn(rx, rx));
+    best = min(best, ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)k);     // ties -> lower segment (D38)
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, d));
+  IdmProj r{-1, 0.f, __int_as_float(0x7f800000), 0.f};
+  if (best != ~0ull) {
+    const int k = (int)(best & 0xffffffffu);
+    r.k = k; r.d2 = __uint_as_float((uint32_t)(best >> 32));
+    const float ex = __fsub_rn(sp[k + 1], sp[k]), ey = __fsub_rn(sp[P + k + 1], sp[P + k]);
+    const float wx = __fsub_rn(qx, sp[k]), wy = __fsub_rn(qy, sp[P + k]);
+    const float ee = __fmaf_rn(ey, ey, __fmul_rn(ex, ex)), dot = __fmaf_rn(wy, ey, __fmul_rn(wx, ex));
+    if (ee > 0.f) r.u = fminf(fmaxf(__fdiv_rn(dot, ee), 0.f), 1.f);
+    r.sigma = __fmaf_rn(r.u, __fsub_rn(sp[2 * P + k + 1], sp[2 * P + k]), sp[2 * P + k]);
+  }
+  return r;
+}
+
+__global__ void __launch_bounds__(256) k_idm_step(IdmParams p) {
+  extern __shared__ __align__(16) float s_path[];            // per warp: 3 P floats + P bytes (padded to 4)
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int A = p.sim.A, T = p.sim.T, P = p.pa.P;
+  const int64_t w = blockIdx.x * (int64_t)(blockDim.x >> 5) + warp;
+  if (w >= (int64_t)p.sim.B * A) return;
+  const int b = (int)(w / A), i = (int)(w % A);
+  const int64_t o = (int64_t)b * A + i, r0 = ((int64_t)b * T + p.t) * A + i, r1 = r0 + A;
+  if (lane == 0) { if (p.accel) p.accel[o] = 0.f; if (p.lead) p.lead[o] = -1; }
+  if (p.idm_valid[o] == 0 || p.sim.valid[r0] == 0) return;     // warp-uniform
+  const int stride = 3 * P + ((P + 3) >> 2);
+  float* sp = s_path + (size_t)warp * stride;
+  uint8_t* sv = (uint8_t*)(sp + 3 * P);
+  const int64_t po = ((int64_t)b * p.pa.A + i) * P;
+  float bx0 = 3.0e38f, by0 = 3.0e38f, bx1 = -3.0e38f, by1 = -3.0e38f;
+  for (int k = lane; k < P; k += 32) {
+    const uint8_t v = p.pa.valid[po + k];
+    const float x = p.pa.x[po + k], y = p.pa.y[po + k];
+    sp[k] = x; sp[P + k] = y; sp[2 * P + k] = p.pa.arc_len[po + k]; sv[k] = v;
+    if (v) { bx0 = fminf(bx0, x); bx1 = fmaxf(bx1, x); by0 = fminf(by0, y); by1 = fmaxf(by1, y); }
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    bx0 = fminf(bx0, __shfl_xor_sync(0xffffffffu, bx0, d)); by0 = fminf(by0, __shfl_xor_sync(0xffffffffu, by0, d));
+    bx1 = fmaxf(bx1, __shfl_xor_sync(0xffffffffu, bx1, d)); by1 = fmaxf(by1, __shfl_xor_sync(0xffffffffu, by1, d));
+  }
+  __syncwarp();
+  const float xi = p.sim.x[r0], yi = p.sim.y[r0], Li = p.sim.length[r0], Wi = p.sim.width[r0];
+  const IdmProj self = idm_project(sp, sv, P, xi, yi);
+  if (self.k < 0) return;                                      // D41: no path segment
+  // ---- lead object (D39) ----
+  int lead = -1;
+  float gap = __int_as_float(0x7f800000);
+  const int64_t rb = ((int64_t)b * T + p.t) * A;
+  for (int j = 0; j < A; ++j) {
+    if (j == i || p.sim.valid[rb + j] == 0) continue;
+    const float xj = p.sim.x[rb + j], yj = p.sim.y[rb + j];
+    const float lat_max = __fmul_rn(0.5f, __fadd_rn(Wi, p.sim.width[rb + j]));
+    const float reach = fmaf(lat_max, 1.001f, 1e-3f);         // outside the inflated box: farther than lat_max from every segment
+    if (xj < bx0 - reach || xj > bx1 + reach || yj < by0 - reach || yj > by1 + reach) continue;
+    const IdmProj pj = idm_project(sp, sv, P, xj, yj);
+    if (!(pj.sigma > self.sigma) || pj.d2 > __fmul_rn(lat_max, lat_max)) continue;
+    const float g = __fsub_rn(__fsub_rn(pj.sigma, self.sigma), __fmul_rn(0.5f, __fadd_rn(Li, p.sim.length[rb + j])));
+    if (g < gap) { gap = g; lead = j; }
+  }
+  if (lane != 0) return;
+  // ---- IDM acceleration (ref. [51]) and the move along the path (D40) ----
+  const wm_idm_params& q = p.prm;
+  const float vx = p.sim.vel_x[r0], vy = p.sim.vel_y[r0], v = sqrtf(fmaf(vx, vx, vy * vy));
+  float acc = 1.f - powf(v / q.v0, q.delta);
+  if (lead >= 0) {
+    const float lx = p.sim.vel_x[rb + lead], ly = p.sim.vel_y[rb + lead], vl = sqrtf(fmaf(lx, lx, ly * ly));
+    const float sstar = q.s0 + fmaxf(0.f, fmaf(v, q.T, v * (v - vl) / (2.f * sqrtf(q.a_max * q.b))));
+    const float sg = sstar / fmaxf(gap, 0.1f);
+    acc -= sg * sg;
+  }
+  acc = fminf(fmaxf(acc * q.a_max, -q.b_max), q.a_max);
+  const float v1 = fmaxf(0.f, fmaf(acc, p.dt, v));
+  const float target = fmaf(0.5f * (v + v1), p.dt, self.sigma);
+  int ks = -1;
+  for (int k = self.k; k + 1 < P; ++k)
+    if (sv[k] != 0 && sv[k + 1] != 0 && sp[2 * P + k + 1] > target) { ks = k; break; }
+  float xn, yn, yawn;
+  if (ks >= 0) {
+    const float ex = sp[ks + 1] - sp[ks], ey = sp[P + ks + 1] - sp[P + ks];
+    const float len = sp[2 * P + ks + 1] - sp[2 * P + ks];
+    const float u = fminf(fmaxf((target - sp[2 * P + ks]) / len, 0.f), 1.f);
+    xn = fmaf(u, ex, sp[ks]); yn = fmaf(u, ey, sp[P + ks]); yawn = atan2f(ey, ex);
+  } else {                                                     // past the end: the last path point, yaw kept
+    int kl = self.k + 1;
+    for (int k = self.k + 1; k < P; ++k) { if (sv[k] != 0 && sv[k - 1] != 0) kl = k; else break; }
+    xn = sp[kl]; yn = sp[P + kl]; yawn = p.sim.yaw[r0];
+  }
+  float sn, cs;
+  sincosf(yawn, &sn, &cs);
+  p.sim.x[r1] = xn; p.sim.y[r1] = yn; p.sim.yaw[r1] = yawn;
+  p.sim.vel_x[r1] = v1 * cs; p.sim.vel_y[r1] = v1 * sn;
+  p.sim.length[r1] = Li; p.sim.width[r1] = Wi; p.sim.valid[r1] = 1;
+  if (p.accel) p.accel[o] = acc;
+  if (p.lead) p.lead[o] = lead;
+}
+
+cudaError_t wm_launch_idm_step(wm_handle* h, const wm_traj& sim, int t, const wm_paths& pa, const uint8_t* idm_valid,
+                               const wm_idm_params& prm, float* accel, int32_t* lead, cudaStream_t s) {
+  IdmParams p{sim, t, pa, idm_valid, prm, h->cfg.dt, accel, lead};
+  const int64_t warps = (int64_t)sim.B * sim.A;
+  const size_t smem = 8 * (size_t)(3 * pa.P + ((pa.P + 3) >> 2)) * sizeof(float);
+  if (smem > 200 * 1024) return cudaErrorInvalidValue;         // P > ~1900 points per path
+  static size_t configured = 0;
+  if (smem > 40 * 1024 && smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_idm_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = smem;
+  }
+  k_idm_step<<<(unsigned)((warps + 7) / 8), 256, smem, s>>>(p);
+  h->launches++;
+  return cudaGetLastError();
+}

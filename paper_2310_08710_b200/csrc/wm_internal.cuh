@@ -146,6 +146,8 @@ cudaError_t wm_launch_route_progress(wm_handle* h, const wm_traj& log, const wm_
                                      uint8_t* valid, cudaStream_t s);
 cudaError_t wm_launch_offroute(wm_handle* h, const wm_traj& sim, int t, const wm_paths& on, const wm_paths* off, float max_dist,
                                float margin, float* dist_on, uint8_t* flag, cudaStream_t s);
+cudaError_t wm_launch_idm_step(wm_handle* h, const wm_traj& sim, int t, const wm_paths& pa, const uint8_t* idm_valid,
+                               const wm_idm_params& prm, float* accel, int32_t* lead, cudaStream_t s);
 cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t* pair_bits,
                               uint8_t* flag, int64_t flag_stride_b, cudaStream_t s);
 cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,

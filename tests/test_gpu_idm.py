@@ -1,0 +1,75 @@
+"""-m gpu parity of the IDM sim agent (wm_idm_step; L110-L112, ref. [51], readings D37-D41) with the oracle.
+
+Teacher-forced: at the checked steps the oracle starts from the GPU's own row t.  Path projections and
+the lead decision are float32 on both sides (same operations), so the lead index must agree exactly;
+the acceleration and the new state are float32 against double: accel 1e-4 + 1e-4 |a| (relative because
+(s*/s)^2 amplifies the float32 gap at small gaps), position 1e-4 m, speed 1e-3 m/s.  The segment an agent
+lands on is decided by comparing its target arc length with the path's knots: agents whose target is
+within 1e-4 m of a knot may land on either neighbour (same position, the yaw of the other piece) - they
+are counted and only their position is compared."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2310_08710_b200 as wm
+import wm_scenarios as ws
+from gpu_util import dev, host
+
+pytestmark = pytest.mark.gpu
+
+
+def test_idm_step_matches_oracle_teacher_forced():
+    cfg = ws.make_config(5, B=4, n_steps=1)
+    log = cfg["log"]
+    B, T, A = log["x"].shape
+    paths = ws.make_paths(log)
+    h = wm.wm_create()
+    log_d = dev(log)
+    sim_d = wm.empty_traj_like(log_d)
+    t0 = wm.wm_reset(h, log_d, sim_d)
+    paths_d = {k: torch.from_numpy(v).cuda() for k, v in paths.items()}
+    idm = np.ones((B, A), np.uint8); idm[:, ::6] = 0              # every sixth agent stays on log playback
+    idm_d = torch.from_numpy(idm).cuda()
+    act0 = torch.zeros((B, 2, A), device="cuda"); av0 = torch.zeros((B, A), dtype=torch.uint8, device="cuda")
+    acc = torch.full((B, A), 7.0, device="cuda"); lead = torch.full((B, A), 7, dtype=torch.int32, device="cuda")
+    n_lead = n_band = n_moved = 0
+    for s in range(40):
+        t = t0 + s
+        before = host(sim_d) if s in (0, 15, 39) else None
+        wm.wm_step(h, log_d, sim_d, t, act0, av0)                   # everybody: log playback (L164)
+        wm.wm_idm_step(h, sim_d, t, paths_d, idm_d, acc, lead)      # the IDM agents override their slots
+        if before is None:
+            continue
+        torch.cuda.synchronize()
+        got = host(sim_d)
+        ref = {k: v.copy() for k, v in before.items()}
+        oracle.step(log, ref, t, oracle.DYN_BICYCLE, np.zeros((B, 2, A), np.float32), np.zeros((B, A), np.uint8))
+        r = oracle.idm_step(ref, t, paths, idm)
+        g_lead, g_acc = lead.cpu().numpy(), acc.cpu().numpy().astype(np.float64)
+        assert np.array_equal(g_lead, r["lead"])
+        assert np.all(np.abs(g_acc - r["accel"]) <= 1e-4 + 1e-4 * np.abs(r["accel"]))
+        assert np.array_equal(got["valid"][:, t + 1], ref["valid"][:, t + 1])
+        moved = (idm == 1) & (before["valid"][:, t] == 1) & ((paths["valid"].sum(axis=2) >= 2))
+        v = ref["valid"][:, t + 1] == 1
+        dpos = np.hypot(got["x"][:, t + 1].astype(np.float64) - ref["x"][:, t + 1], got["y"][:, t + 1].astype(np.float64) - ref["y"][:, t + 1])
+        assert dpos[v].max() <= 1e-4, float(dpos[v].max())
+        # knot band: target arc length within 1e-4 of a path knot
+        sp = np.hypot(before["vel_x"][:, t].astype(np.float64), before["vel_y"][:, t].astype(np.float64))
+        dyaw = np.abs(np.angle(np.exp(1j * (got["yaw"][:, t + 1].astype(np.float64) - ref["yaw"][:, t + 1]))))
+        dvel = np.hypot(got["vel_x"][:, t + 1].astype(np.float64) - ref["vel_x"][:, t + 1], got["vel_y"][:, t + 1].astype(np.float64) - ref["vel_y"][:, t + 1])
+        band = v & moved & (dyaw > 1e-4)
+        # a band member must really sit on a knot: its position coincides with a path point to 2e-4 m
+        for b, a in np.argwhere(band):
+            d = np.hypot(paths["x"][b, a].astype(np.float64) - got["x"][b, t + 1, a], paths["y"][b, a].astype(np.float64) - got["y"][b, t + 1, a])
+            assert d[paths["valid"][b, a] == 1].min() < 2e-4
+        ok = v & ~band
+        assert dyaw[ok].max() <= 1e-4 and dvel[ok].max() <= 1e-3
+        # slots that are not IDM-controlled are the log playback, bit for bit
+        nb = v & ~moved
+        for k in ("x", "y", "yaw", "vel_x", "vel_y"):
+            assert np.array_equal(got[k][:, t + 1][nb], ref[k][:, t + 1][nb])
+        n_lead += int((r["lead"] >= 0).sum()); n_band += int(band.sum()); n_moved += int((moved & v).sum())
+    print("idm: %d agent-steps checked, %d with a lead object, %d in the knot band" % (n_moved, n_lead, n_band))
+    assert n_lead > 50 and n_band < n_moved // 20
+    wm.wm_destroy(h)
