@@ -275,6 +275,55 @@ def run_supplementary(args):
                 "roofline": {"bound": "hbm", "achieved": None, "peak": hbm_peak, "unit": "GB/s", "frac": None, "traffic": None,
                              "note": "latency-bound micro-batches: no roofline claim; see the default workload"},
                 "cpu_baseline": None, "e2e": None, "gpu_launches": int(total_launches), "clocks": None}
+    elif args.workload == "idm":
+        # IDM reactive sim agents (L110-L112): every valid agent follows its logged path with the IDM speed
+        # profile, closed loop: per step wm_step (log playback for everybody) + wm_idm_step + overlap metric
+        cfg = ws.make_config(5, B=args.B, n_steps=1)
+        log = cfg["log"]
+        B, T, A = log["x"].shape
+        h = wm.wm_create()
+        log_d = wm.to_device(log)
+        sim_d = wm.empty_traj_like(log_d)
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        paths = ws.make_paths(log)
+        paths_d = {q: torch.from_numpy(v).cuda() for q, v in paths.items()}
+        idm_d = torch.ones((B, A), dtype=torch.uint8, device="cuda")
+        act0 = torch.zeros((B, 2, A), device="cuda"); av0 = torch.zeros((B, A), dtype=torch.uint8, device="cuda")
+        acc = torch.empty((B, A), device="cuda"); lead = torch.empty((B, A), dtype=torch.int32, device="cuda")
+        ofl = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+        n_sim = 20
+
+        def fn():
+            for s_ in range(n_sim):
+                wm.wm_step(h, log_d, sim_d, t0 + s_, act0, av0)
+                wm.wm_idm_step(h, sim_d, t0 + s_, paths_d, idm_d, acc, lead)
+                wm.wm_metrics_overlap(h, sim_d, t0 + s_ + 1, None, ofl)
+        l0 = wm.wm_kernel_launches(h)
+        ms = timed(fn, K, W)
+        launches = (wm.wm_kernel_launches(h) - l0) * K // (K + W)
+        ms_i = timed(lambda: wm.wm_idm_step(h, sim_d, t0 + 5, paths_d, idm_d, acc, lead), K, W)
+        P = paths["x"].shape[2]
+        idm_bytes = float(B) * A * (P * 13 + 29 + 29 + 8) + float(B) * A * 29
+        sb = min(16, B)
+        sub = lambda d: {q: np.ascontiguousarray(v[:sb]) for q, v in d.items()}
+        sim_o = {q: v[:sb].cpu().numpy().copy() for q, v in sim_d.items()}
+        t0c = time.perf_counter()
+        ro = oracle.idm_step(sim_o, t0 + 5, sub(paths), np.ones((sb, A), np.uint8))
+        dt = time.perf_counter() - t0c
+        wm.wm_idm_step(h, sim_d, t0 + 5, paths_d, idm_d, acc, lead); torch.cuda.synchronize()
+        line = {"metric": "agent-steps/s, closed loop with IDM sim agents (log playback + wm_idm_step + overlap), config 5", "value": float(B) * A * n_sim / (ms * 1e-3),
+                "unit": "agent-steps/s", "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "config5 IDM: B=%d A=%d T=%d, %d closed-loop steps per bench step, paths of %d points" % (B, A, T, n_sim, P),
+                           "ms_idm_step": ms_i, "l2": "paths 2.8 GB exceed L2", "collision_rate_after_%d_steps" % n_sim: float(ofl.float().mean().item()),
+                           "agents_with_lead": float((lead >= 0).float().mean().item())},
+                "roofline": {"bound": "hbm", "achieved": idm_bytes / (ms_i * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": idm_bytes / (ms_i * 1e-3) / 1e9 / hbm_peak, "traffic": None, "kernel": "k_idm_step", "algorithmic_bytes": idm_bytes,
+                             "note": "A x A x P projections per scenario-step, culled by the path's bounding box: ALU / shared-memory bound, not HBM bound"},
+                "cpu_baseline": {"value": sb * A / dt, "unit": "agent-steps/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                 "sample": "one idm_step of the first %d of %d scenarios, %.2f s wall" % (sb, B, dt),
+                                 "lead_indices_equal": bool(np.array_equal(ro["lead"], lead[:sb].cpu().numpy()))},
+                "e2e": None, "gpu_launches": int(launches), "clocks": None}
     elif args.workload == "expert":
         # RolloutExpert (Table 2): expert actions from the log by inverse kinematics, the
         # 80-step rollout with them, then the kinematic-infeasibility metric of the simulated rows (L104)
@@ -416,7 +465,7 @@ def main():
     ap.add_argument("--cpu-B", type=int, default=256, help="oracle sample for cpu_baseline (256 scenarios: ~15 s on 16 cores)")
     ap.add_argument("--ref-B", type=int, default=64, help="oracle sample per step of --impl reference (~4 s on 16 cores)")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4", "expert", "paper_tables"],
+    ap.add_argument("--workload", default="rollout", choices=["rollout", "observe", "step2", "stress4", "expert", "idm", "paper_tables"],
                     help="rollout = the BASELINE metric (config 5, default); the others time the remaining "
                          "SURVEY 8(a) rows on configs 3, 2, 4 (supplementary lines, same JSON shape)")
     ap.add_argument("--no-e2e", action="store_true")
