@@ -443,16 +443,27 @@ __global__ void __launch_bounds__(256) k_idm_step(IdmParams p) {
   int lead = -1;
   float gap = __int_as_float(0x7f800000);
   const int64_t rb = ((int64_t)b * T + p.t) * A;
-  for (int j = 0; j < A; ++j) {
-    if (j == i || p.sim.valid[rb + j] == 0) continue;
-    const float xj = p.sim.x[rb + j], yj = p.sim.y[rb + j];
-    const float lat_max = __fmul_rn(0.5f, __fadd_rn(Wi, p.sim.width[rb + j]));
-    const float reach = fmaf(lat_max, 1.001f, 1e-3f);         // outside the inflated box: farther than lat_max from every segment
-    if (xj < bx0 - reach || xj > bx1 + reach || yj < by0 - reach || yj > by1 + reach) continue;
-    const IdmProj pj = idm_project(sp, sv, P, xj, yj);
-    if (!(pj.sigma > self.sigma) || pj.d2 > __fmul_rn(lat_max, lat_max)) continue;
-    const float g = __fsub_rn(__fsub_rn(pj.sigma, self.sigma), __fmul_rn(0.5f, __fadd_rn(Li, p.sim.length[rb + j])));
-    if (g < gap) { gap = g; lead = j; }
+  for (int jb = 0; jb < A; jb += 32) {                        // lanes over the other agents: who can matter at all?
+    const int jl = jb + lane;
+    bool pass = jl < A && jl != i && p.sim.valid[rb + jl] != 0;
+    float xl = 0.f, yl = 0.f, wl = 0.f, ll = 0.f;
+    if (pass) {
+      xl = p.sim.x[rb + jl]; yl = p.sim.y[rb + jl]; wl = p.sim.width[rb + jl]; ll = p.sim.length[rb + jl];
+      const float reach = fmaf(__fmul_rn(0.5f, __fadd_rn(Wi, wl)), 1.001f, 1e-3f);   // outside the inflated box: farther than lat_max from every segment
+      pass = !(xl < bx0 - reach || xl > bx1 + reach || yl < by0 - reach || yl > by1 + reach);
+    }
+    uint32_t todo = __ballot_sync(0xffffffffu, pass);
+    while (todo) {                                             // ascending j: ties -> lower index (D39)
+      const int src = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const float xj = __shfl_sync(0xffffffffu, xl, src), yj = __shfl_sync(0xffffffffu, yl, src);
+      const float wj = __shfl_sync(0xffffffffu, wl, src), lj = __shfl_sync(0xffffffffu, ll, src);
+      const float lat_max = __fmul_rn(0.5f, __fadd_rn(Wi, wj));
+      const IdmProj pj = idm_project(sp, sv, P, xj, yj);
+      if (!(pj.sigma > self.sigma) || pj.d2 > __fmul_rn(lat_max, lat_max)) continue;
+      const float g = __fsub_rn(__fsub_rn(pj.sigma, self.sigma), __fmul_rn(0.5f, __fadd_rn(Li, lj)));
+      if (g < gap) { gap = g; lead = jb + src; }
+    }
   }
   if (lane != 0) return;
   // ---- IDM acceleration (ref. [51]) and the move along the path (D40) ----
