@@ -241,7 +241,8 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
       const float ox = (kk & 1) ? bx : ax, oy = (kk & 1) ? by : ay;
       offx = (kk & 2) ? -ox : ox; offy = (kk & 2) ? -oy : oy;
     };
-    // the cell header of a task's corner is requested one task ahead: its miss overlaps the walk
+    // the cell header of the NEXT task's corner is requested at the end of a task, ahead of the shared
+    // counter's round trip (measured: requesting it a whole task ahead costs registers and is slower)
     auto header = [&](int task) {
       if (task < nb || task >= n_task) return make_uint2(0u, 0u);
       int q; bool v; float cx, cy, hl, hw, offx, offy;
@@ -257,7 +258,6 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     uint2 hd = header(task);
     while (task < n_task) {
       const int task_next = grab();
-      const uint2 hd_next = header(task_next);
       if (task >= nb) {
         // ---- the 4 corners of one agent (8 / S agents) at every step of the block (a4) ----
         int q; bool v; float cx, cy, hl, hw, offx, offy;
@@ -343,7 +343,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
           if (s < Sb) narrow((int)(pr >> 16), (int)(pr & 0xffffu), s);
         }
       }
-      task = task_next; hd = hd_next;
+      task = task_next; hd = header(task);
     }
     __syncthreads();
     // ================= phase C: metric rows of the block (D18, D19, D10) =================
