@@ -79,13 +79,13 @@ static inline int fused_pick_S(int A) {
 
 struct FusedIn { float a0, a1, a2, lx, ly; uint8_t av, lv; };
 
-__device__ __forceinline__ FusedIn fused_load_in(const FusedParams& p, int64_t sb, int64_t ab, int k, int a, int A) {
+__device__ __forceinline__ FusedIn fused_load_in(const FusedParams& p, int64_t sb, int64_t ab, int k, int a, int A, int C) {
   FusedIn r;
   const int64_t o = sb + (int64_t)(p.t0 + k + 1) * A + a;
   const int64_t ak = ab + k;
   r.av = p.av[ak * A + a];
-  const float* act = p.actions + ak * p.C * A + a;
-  r.a0 = act[0]; r.a1 = act[A]; r.a2 = p.C > 2 ? act[2 * (int64_t)A] : 0.f;
+  const float* act = p.actions + ak * C * A + a;
+  r.a0 = act[0]; r.a1 = act[A]; r.a2 = C > 2 ? act[2 * (int64_t)A] : 0.f;
   r.lx = p.log.x[o]; r.ly = p.log.y[o]; r.lv = p.log.valid[o];
   return r;
 }
@@ -99,11 +99,14 @@ __device__ __forceinline__ uint32_t fused_bucket(int ix, int iy, uint32_t mask) 
 
 // AP_C / S_C > 0: padded agent count and steps per block known at compile time (the shared-memory
 // carve-up then folds into immediate offsets); 0: taken from the arguments.
-template <int AP_C, int S_C>
+template <int AP_C, int S_C, int DYN_C>
 __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int A = p.sim.A, nb = AP_C ? AP_C / 32 : (A + 31) / 32, Ap = nb * 32, Aps = Ap + FUSED_PAD, S = S_C ? S_C : p.S;
   const int NBK = fused_nbk(Ap);
+  WmDynCfg dyn = p.dyn;                              // DYN_C >= 0: the dynamics model is a compile-time constant
+  if (DYN_C >= 0) dyn.dynamics = DYN_C;
+  const int C = DYN_C >= 0 ? (DYN_C == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3) : p.C;
   // ---- persistent per-agent state ----
   double* s_sum = (double*)smem_raw;                 // [Ap] sum of valid log divergences (D21)
   float4* s_bb = (float4*)(s_sum + Ap);              // [Ap] bounding box over the block, inflated: x0, y0, x1, y1
@@ -174,17 +177,17 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
       double sum = s_sum[a];
       int cnt = s_cnt[a];
       float bx0 = 3.0e38f, by0 = 3.0e38f, bx1 = -3.0e38f, by1 = -3.0e38f, br = 0.f;
-      FusedIn in = fused_load_in(p, sb, ab, k0, a, A);
+      FusedIn in = fused_load_in(p, sb, ab, k0, a, A, C);
 #pragma unroll 1                          // measured: the unrolled chain (8 x sincosf, row IO) costs 6 % through its code size
       for (int s = 0; s < Sb; ++s) {
         const int k = k0 + s;
         const FusedIn cur = in;
-        if (s + 1 < Sb) in = fused_load_in(p, sb, ab, k + 1, a, A);     // prefetch: nothing below depends on it
+        if (s + 1 < Sb) in = fused_load_in(p, sb, ab, k + 1, a, A, C);     // prefetch: nothing below depends on it
         const int64_t o = sb + (int64_t)(p.t0 + k + 1) * A + a;
         const bool use_dyn = cur.av != 0 && v;                          // D8
         float xn, yn, thn, vxn, vyn, s1 = 0.f, c1 = 1.f;
         if (use_dyn) {
-          wm_dyn_step(p.dyn, x, y, th, vx, vy, sn, cs, cur.a0, cur.a1, cur.a2, xn, yn, thn, vxn, vyn, s1, c1);
+          wm_dyn_step(dyn, x, y, th, vx, vy, sn, cs, cur.a0, cur.a1, cur.a2, xn, yn, thn, vxn, vyn, s1, c1);
           v = true;                                                     // D9: keeps its box
         } else {                                                        // log playback, L164
           xn = cur.lx; yn = cur.ly; thn = p.log.yaw[o]; vxn = p.log.vel_x[o]; vyn = p.log.vel_y[o];
@@ -405,14 +408,15 @@ cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_t
   const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused<0, 0, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)(fused_persist_bytes(1024) + fused_slot_bytes(1024)));
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  if (Ap == 128 && p.S == 8) k_rollout_fused<128, 8><<<sim.B, FUSED_NT, smem, s>>>(p);
-  else if (Ap == 32 && p.S == 8) k_rollout_fused<32, 8><<<sim.B, FUSED_NT, smem, s>>>(p);
-  else k_rollout_fused<0, 0><<<sim.B, FUSED_NT, smem, s>>>(p);
+  if (Ap == 128 && p.S == 8 && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE) k_rollout_fused<128, 8, WM_DYN_INVERTIBLE_BICYCLE><<<sim.B, FUSED_NT, smem, s>>>(p);
+  else if (Ap == 128 && p.S == 8) k_rollout_fused<128, 8, -1><<<sim.B, FUSED_NT, smem, s>>>(p);
+  else if (Ap == 32 && p.S == 8) k_rollout_fused<32, 8, -1><<<sim.B, FUSED_NT, smem, s>>>(p);
+  else k_rollout_fused<0, 0, -1><<<sim.B, FUSED_NT, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
 }
