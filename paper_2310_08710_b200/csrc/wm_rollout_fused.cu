@@ -99,7 +99,7 @@ __device__ __forceinline__ uint32_t fused_bucket(int ix, int iy, uint32_t mask) 
 
 // AP_C / S_C > 0: padded agent count and steps per block known at compile time (the shared-memory
 // carve-up then folds into immediate offsets); 0: taken from the arguments.
-template <int AP_C, int S_C, int DYN_C>
+template <int AP_C, int S_C, int DYN_C, bool STATS>
 __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int A = p.sim.A, nb = AP_C ? AP_C / 32 : (A + 31) / 32, Ap = nb * 32, Aps = Ap + FUSED_PAD, S = S_C ? S_C : p.S;
@@ -377,7 +377,7 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     if (p.out.any_offroad) p.out.any_offroad[o] = s_anyoff[a];
     if (p.out.ade) p.out.ade[o] = s_cnt[a] ? (float)(s_sum[a] / s_cnt[a]) : 0.f;
   }
-  if (p.stats) {
+  if (STATS && p.stats) {
     const unsigned ne = __reduce_add_sync(0xffffffffu, (unsigned)n_eval), ns = __reduce_add_sync(0xffffffffu, (unsigned)n_slow);
     const unsigned nc = __reduce_add_sync(0xffffffffu, (unsigned)n_corner);
     if (lane == 0 && nc) {
@@ -408,15 +408,16 @@ cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_t
   const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused<0, 0, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused<0, 0, -1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)(fused_persist_bytes(1024) + fused_slot_bytes(1024)));
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  if (Ap == 128 && p.S == 8 && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE) k_rollout_fused<128, 8, WM_DYN_INVERTIBLE_BICYCLE><<<sim.B, FUSED_NT, smem, s>>>(p);
-  else if (Ap == 128 && p.S == 8) k_rollout_fused<128, 8, -1><<<sim.B, FUSED_NT, smem, s>>>(p);
-  else if (Ap == 32 && p.S == 8) k_rollout_fused<32, 8, -1><<<sim.B, FUSED_NT, smem, s>>>(p);
-  else k_rollout_fused<0, 0, -1><<<sim.B, FUSED_NT, smem, s>>>(p);
+  if (Ap == 128 && p.S == 8 && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE && !p.stats)
+    k_rollout_fused<128, 8, WM_DYN_INVERTIBLE_BICYCLE, false><<<sim.B, FUSED_NT, smem, s>>>(p);     // the pair counters compiled out
+  else if (Ap == 128 && p.S == 8) k_rollout_fused<128, 8, -1, true><<<sim.B, FUSED_NT, smem, s>>>(p);
+  else if (Ap == 32 && p.S == 8) k_rollout_fused<32, 8, -1, true><<<sim.B, FUSED_NT, smem, s>>>(p);
+  else k_rollout_fused<0, 0, -1, true><<<sim.B, FUSED_NT, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
 }
