@@ -7,28 +7,34 @@
 // a0 reset(scenario), PAPER.md L122 / L78.
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_reset(wm_traj log, wm_traj sim, int history) {
-  const int64_t n = (int64_t)sim.B * sim.T * sim.A;
-  const int64_t TA = (int64_t)sim.T * sim.A;
-  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    const int t = (int)((i % TA) / sim.A);
-    const bool c = t < history;
-    sim.x[i] = c ? log.x[i] : 0.f;
-    sim.y[i] = c ? log.y[i] : 0.f;
-    sim.yaw[i] = c ? log.yaw[i] : 0.f;
-    sim.vel_x[i] = c ? log.vel_x[i] : 0.f;
-    sim.vel_y[i] = c ? log.vel_y[i] : 0.f;
-    sim.length[i] = c ? log.length[i] : 0.f;
-    sim.width[i] = c ? log.width[i] : 0.f;
-    sim.valid[i] = c ? log.valid[i] : (uint8_t)0;
+  // one CTA per (scenario, chunk of 1024 row elements): no per-element division; rows [0, history) are
+  // copied, the rest cleared.  HBM-write bound (the whole simulated trajectory is written once).
+  const int64_t TA = (int64_t)sim.T * sim.A, HA = (int64_t)history * sim.A;
+  const int64_t base = (int64_t)blockIdx.y * TA;
+  for (int64_t e = (int64_t)blockIdx.x * 1024 + threadIdx.x; e < TA; e += (int64_t)gridDim.x * 1024) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int64_t r = e + q * 256;
+      if (r >= TA) break;
+      const int64_t i = base + r;
+      const bool c = r < HA;
+      sim.x[i] = c ? log.x[i] : 0.f;
+      sim.y[i] = c ? log.y[i] : 0.f;
+      sim.yaw[i] = c ? log.yaw[i] : 0.f;
+      sim.vel_x[i] = c ? log.vel_x[i] : 0.f;
+      sim.vel_y[i] = c ? log.vel_y[i] : 0.f;
+      sim.length[i] = c ? log.length[i] : 0.f;
+      sim.width[i] = c ? log.width[i] : 0.f;
+      sim.valid[i] = c ? log.valid[i] : (uint8_t)0;
+    }
   }
 }
 
 cudaError_t wm_launch_reset(wm_handle* h, const wm_traj& log, const wm_traj& sim, int history, cudaStream_t s) {
-  const int64_t n = (int64_t)sim.B * sim.T * sim.A;
-  int grid = (int)((n + 255) / 256);
-  const int cap = h->num_sms * 32;
-  if (grid > cap) grid = cap;
-  k_reset<<<grid, 256, 0, s>>>(log, sim, history);
+  const int64_t TA = (int64_t)sim.T * sim.A;
+  int gx = (int)((TA + 1023) / 1024);
+  if (gx > 64) gx = 64;
+  k_reset<<<dim3(gx, sim.B), 256, 0, s>>>(log, sim, history);
   h->launches++;
   return cudaGetLastError();
 }
