@@ -196,11 +196,11 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
           v = cur.lv != 0;
           if (v) sincosf(thn, &s1, &c1);
         }
-        __stcs(p.sim.x + o, xn); __stcs(p.sim.y + o, yn); __stcs(p.sim.yaw + o, thn); __stcs(p.sim.vel_x + o, vxn); __stcs(p.sim.vel_y + o, vyn);
-        __stcs(p.sim.length + o, ln); __stcs(p.sim.width + o, wd); __stcs(p.sim.valid + o, (uint8_t)v);
+        p.sim.x[o] = xn; p.sim.y[o] = yn; p.sim.yaw[o] = thn; p.sim.vel_x[o] = vxn; p.sim.vel_y[o] = vyn;
+        p.sim.length[o] = ln; p.sim.width[o] = wd; p.sim.valid[o] = (uint8_t)v;
         const bool ldv = v && cur.lv != 0;                              // a5, L106
         const float d = ldv ? wm_logdiv(xn, yn, cur.lx, cur.ly) : 0.f;
-        if (p.out.log_div) __stcs(p.out.log_div + (ab + k) * A + a, d);
+        if (p.out.log_div) p.out.log_div[(ab + k) * A + a] = d;
         if (ldv) { sum += (double)d; cnt += 1; }
         x = xn; y = yn; th = thn; vx = vxn; vy = vyn; sn = s1; cs = c1;
         // what the metrics of this step need; invalid slots: finite zeros (D10)
@@ -360,9 +360,9 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         const bool v = pvalid[q] != 0;
         const float m = v ? psd[q] : 0.f;
         const uint8_t fo = pov[q], ff = (uint8_t)(v && m > 0.f);
-        if (p.out.overlap) __stcs(p.out.overlap + o, fo);
-        if (p.out.offroad_dist) __stcs(p.out.offroad_dist + o, m);
-        if (p.out.offroad) __stcs(p.out.offroad + o, ff);
+        if (p.out.overlap) p.out.overlap[o] = fo;
+        if (p.out.offroad_dist) p.out.offroad_dist[o] = m;
+        if (p.out.offroad) p.out.offroad[o] = ff;
         aov |= fo; aoff |= ff;
       }
       s_anyov[a] = aov; s_anyoff[a] = aoff;
