@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(1024) k_overlap(OverlapParams p) {
   float* srad = shw + Ap;                     // circumradius
   uint32_t* svalid = (uint32_t*)(srad + Ap);  // [nb] ballot words
   uint32_t* sany = svalid + nb;               // [Ap] any-overlap per agent
-  const int b = blockIdx.x;
+  const int b = blockIdx.y;
   const int64_t ro = (int64_t)b * p.row.stride_b;
   for (int a = threadIdx.x; a < Ap; a += blockDim.x) {
     const bool v = a < A && p.row.valid[ro + a] != 0;
@@ -41,7 +41,9 @@ __global__ void __launch_bounds__(1024) k_overlap(OverlapParams p) {
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
   const int ntile = nb * (nb + 1) / 2;
-  for (int tile = warp; tile < ntile; tile += nw) {
+  // gridDim.x > 1 (large A): the CTAs of a scenario split the tiles, nw consecutive ones each
+  const int tile_lo = gridDim.x > 1 ? blockIdx.x * nw : 0, tile_hi = gridDim.x > 1 ? min(ntile, tile_lo + nw) : ntile;
+  for (int tile = tile_lo + warp; tile < tile_hi; tile += nw) {
     // unrank (I <= J) from the linear upper-triangle index
     int I = 0, rem = tile;
     while (rem >= nb - I) { rem -= nb - I; ++I; }
@@ -77,7 +79,13 @@ __global__ void __launch_bounds__(1024) k_overlap(OverlapParams p) {
     if (colword) atomicOr(&sany[j_mine], 1u);
   }
   __syncthreads();
-  for (int a = threadIdx.x; a < A; a += blockDim.x) p.flag[(int64_t)b * p.flag_stride_b + a] = (uint8_t)(sany[a] != 0);
+  if (gridDim.x == 1) {
+    for (int a = threadIdx.x; a < A; a += blockDim.x) p.flag[(int64_t)b * p.flag_stride_b + a] = (uint8_t)(sany[a] != 0);
+  } else {                                       // flags were zeroed by the launcher: OR this CTA's part in, byte a of a 4-byte word
+    uint8_t* row = p.flag + (int64_t)b * p.flag_stride_b;
+    for (int a = threadIdx.x; a < A; a += blockDim.x)
+      if (sany[a] != 0) atomicOr((unsigned int*)(row + (a & ~3)), 1u << (8 * (a & 3)));
+  }
 }
 
 cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t* pair_bits,
@@ -91,7 +99,16 @@ cudaError_t wm_launch_overlap(wm_handle* h, const wm_traj& sim, int t, uint32_t*
   // one warp per 32 x 32 tile of the upper triangle, up to 32 warps per scenario (A = 512: 136 tiles)
   const int ntile = p.W * (p.W + 1) / 2;
   const int nt = ntile >= 32 ? 1024 : (ntile > 8 ? 512 : 256);
-  k_overlap<<<sim.B, nt, smem, s>>>(p);
+  // More than 32 tiles (A > 224) and few scenarios: several CTAs per scenario, flags combined by atomic OR
+  // on 4-byte words of the (zeroed) flag rows - needs 4-byte aligned rows.
+  int split = 1;
+  if (ntile > 32 && sim.B < 4 * h->num_sms && ((uintptr_t)flag & 3u) == 0 && flag_stride_b % 4 == 0 && sim.A % 4 == 0) split = (ntile + 31) / 32;
+  if (split > 1) {
+    cudaError_t e = flag_stride_b == sim.A ? cudaMemsetAsync(flag, 0, (size_t)sim.B * sim.A, s)
+                                           : cudaMemset2DAsync(flag, (size_t)flag_stride_b, 0, (size_t)sim.A, (size_t)sim.B, s);
+    if (e != cudaSuccess) return e;
+  }
+  k_overlap<<<dim3(split, sim.B), nt, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
 }
