@@ -10,8 +10,8 @@
  *  - Every function returns int: WM_OK (0) or a negative wm_status.  Nothing throws, aborts
  *    or prints.  After WM_ERR_CUDA, wm_last_cuda_error() returns the cudaError_t.
  *  - Unless a function says HOST, every data pointer is a DEVICE pointer owned by the
- *    caller; the library owns only what hangs off wm_handle (prepared road-edge segments,
- *    prepared roadgraph points, scratch, the instantiated CUDA graph, staging buffers).
+ *    caller; the library owns only what hangs off wm_handle (prepared road-edge segments and
+ *    search grids, bucketed roadgraph points, scratch, the instantiated CUDA graph, staging buffers).
  *  - Work is enqueued on the caller's stream (`void* stream` = cudaStream_t; NULL = the
  *    legacy default stream) and NOT synchronised, unless a function says it synchronises.
  *  - Functions are pure in the paper's sense (L120): outputs depend only on the arguments,
@@ -72,15 +72,19 @@ typedef struct {
   int32_t rollout_mode; /* WM_ROLLOUT_*: how wm_rollout runs the n_steps */
 } wm_config;
 
-/* Both modes return the same values (the nearest segment is found exactly in both).
- * CULLED (default): segments are stored in spatial order with one bounding circle per group of
- *   64; a group is evaluated only if its lower bound can beat the current best of the agent.
+/* Both modes find the nearest segment exactly and use the same per-pair arithmetic; they return the
+ * same bits whenever they pick the same segment (at a polyline vertex the two neighbours' float32
+ * distances can differ by an ulp).
+ * CULLED (default): wm_prepare lays two nested grids over the segments; every cell lists, as runs of
+ *   consecutive segments, the only segments that can be nearest to a point inside it; a query walks
+ *   the list of its corner's cell (about 7 segments).  Crowded cells and points outside the grids
+ *   fall back to a bounding-box search over all segments, exact as well.
  * BRUTE_FORCE: every corner-segment pair is evaluated (the FP32-roofline reference kernel). */
 enum { WM_OFFROAD_CULLED = 0, WM_OFFROAD_BRUTE_FORCE = 1 };
 
-/* Both modes return bit-identical rows (same device arithmetic), both as one CUDA graph (L200).
- * FUSED (default): one kernel, one CTA per scenario, state resident in shared memory for all
- *   n_steps; needs WM_OFFROAD_CULLED (with BRUTE_FORCE the stepwise graph is used).
+/* Both modes return bit-identical rows (same device arithmetic), both replayed as one CUDA graph (L200).
+ * FUSED (default): ONE kernel launch for all n_steps, one CTA per scenario, state resident in shared
+ *   memory; needs WM_OFFROAD_CULLED (with BRUTE_FORCE the stepwise graph is used).
  * STEPWISE: n_steps x {k_step, k_overlap, k_offroad} + k_aggregate, the kernels of the single-step
  *   entry points. */
 enum { WM_ROLLOUT_FUSED = 0, WM_ROLLOUT_STEPWISE = 1 };
@@ -108,7 +112,8 @@ const char* wm_version(void);
  *  - road-edge segments for the offroad metric (L100; D14-D17): consecutive entries
  *    (i, i+1) with both valid, both WM_TYPE_ROAD_EDGE and equal id form a segment; an
  *    isolated valid road-edge point is a zero-length segment signed by its stored dir;
- *  - a packed copy of the roadgraph points for the top-k observation (L82).
+ *    and the nested grids of candidate lists over them (WM_OFFROAD_CULLED);
+ *  - the valid roadgraph points bucketed into a uniform grid for the top-k observation (L82).
  * Keeps pointers to nothing in `rg` (everything needed is copied); `rg` must match the B of
  * later calls.  SYNCHRONISES the stream (it sizes its buffers from a device-side count).
  * `n_segments_max` (HOST, may be NULL) receives max_b S_e(b).
