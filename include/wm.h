@@ -282,6 +282,10 @@ int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t0, int32
  * and the actions, runs wm_prepare, wm_reset and wm_rollout from t0 = history-1, downloads the
  * metric rows and aggregates into the HOST buffers of `out`, and, when sim_host is not NULL,
  * the simulated trajectory.  Device staging buffers are owned by the handle and reused.
+ * Scenarios are independent (L82), so the work is pipelined over up to 16 chunks of scenarios on
+ * the caller's stream (uploads) and three streams of the handle (prepare, rollout, downloads): the
+ * device work hides under the PCIe upload.  The uploads are enqueued on `stream`; it is
+ * synchronised once early (the record count of the road edges fixes the buffer sizes).
  * SYNCHRONISES before returning.  All pointers inside the structs are HOST pointers.
  */
 int wm_rollout_host(wm_handle* h, const wm_traj* log_host, const wm_roadgraph* rg_host,
