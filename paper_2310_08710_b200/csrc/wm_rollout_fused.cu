@@ -248,9 +248,10 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
     };
     // the cell header of the NEXT task's corner is requested at the end of a task, ahead of the shared
     // counter's round trip (measured: requesting it a whole task ahead costs registers and is slower)
+    // ... together with the task's corner set-up, which the walk then finds in registers
+    int q = 0; bool v = false; float cx = 0.f, cy = 0.f, hl = 0.f, hw = 0.f, offx = 0.f, offy = 0.f;
     auto header = [&](int task) {
       if (task < nb || task >= n_task) return make_uint2(0u, 0u);
-      int q; bool v; float cx, cy, hl, hw, offx, offy;
       corner(task, q, v, cx, cy, hl, hw, offx, offy);
       return wm_grid_header(gv, v, cx, cy, offx, offy);
     };
@@ -265,8 +266,6 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
       const int task_next = grab();
       if (task >= nb) {
         // ---- the 4 corners of one agent (8 / S agents) at every step of the block (a4) ----
-        int q; bool v; float cx, cy, hl, hw, offx, offy;
-        corner(task, q, v, cx, cy, hl, hw, offx, offy);
         if (__any_sync(0xffffffffu, v)) {                               // psd of invalid slots is never read
         float best; int bs;
         const bool slow = wm_grid_fast_hd(gv, hd, cx, cy, offx, offy, best, bs, n_eval);
