@@ -291,18 +291,21 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
   }
   uint8_t* ld_valid_rows = sc;
 
-  uint64_t key[24];
+  // cache key of the captured graph: every pointer and shape in a slot of its own
+  uint64_t key[WM_GRAPH_KEY_WORDS];
   memset(key, 0, sizeof(key));
-  int n = 0;
-  const void* ptrs[] = {log->x, log->y, log->yaw, log->vel_x, log->vel_y, log->length, log->width, log->valid,
-                        sim->x, sim->y, sim->yaw, sim->vel_x, sim->vel_y, sim->length, sim->width, sim->valid,
-                        actions, action_valid, o.overlap, o.offroad, o.offroad_dist};
-  for (const void* p : ptrs) key[n++] = (uint64_t)(uintptr_t)p;
-  key[n++] = (uint64_t)(uintptr_t)o.log_div ^ ((uint64_t)(uintptr_t)o.any_overlap << 1) ^ ((uint64_t)(uintptr_t)o.any_offroad << 2) ^
-             ((uint64_t)(uintptr_t)o.ade << 3);
-  key[n++] = ((uint64_t)sim->B << 40) ^ ((uint64_t)sim->A << 20) ^ (uint64_t)sim->T;
-  key[n++] = ((uint64_t)(uint32_t)t0 << 32) ^ (uint64_t)(uint32_t)n_steps ^ ((uint64_t)h->cfg.dynamics << 62);
-  key[n++] = (uint64_t)(uintptr_t)h->segrec ^ ((uint64_t)(uintptr_t)h->cells << 1);
+  const uint64_t words[] = {
+      (uint64_t)(uintptr_t)log->x, (uint64_t)(uintptr_t)log->y, (uint64_t)(uintptr_t)log->yaw, (uint64_t)(uintptr_t)log->vel_x,
+      (uint64_t)(uintptr_t)log->vel_y, (uint64_t)(uintptr_t)log->length, (uint64_t)(uintptr_t)log->width, (uint64_t)(uintptr_t)log->valid,
+      (uint64_t)(uintptr_t)sim->x, (uint64_t)(uintptr_t)sim->y, (uint64_t)(uintptr_t)sim->yaw, (uint64_t)(uintptr_t)sim->vel_x,
+      (uint64_t)(uintptr_t)sim->vel_y, (uint64_t)(uintptr_t)sim->length, (uint64_t)(uintptr_t)sim->width, (uint64_t)(uintptr_t)sim->valid,
+      (uint64_t)(uintptr_t)actions, (uint64_t)(uintptr_t)action_valid,
+      (uint64_t)(uintptr_t)o.overlap, (uint64_t)(uintptr_t)o.offroad, (uint64_t)(uintptr_t)o.offroad_dist, (uint64_t)(uintptr_t)o.log_div,
+      (uint64_t)(uintptr_t)o.any_overlap, (uint64_t)(uintptr_t)o.any_offroad, (uint64_t)(uintptr_t)o.ade,
+      (uint64_t)sim->B, (uint64_t)sim->A, (uint64_t)sim->T, (uint64_t)(uint32_t)t0, (uint64_t)(uint32_t)n_steps,
+      (uint64_t)h->cfg.dynamics, (uint64_t)(uintptr_t)h->segrec, (uint64_t)(uintptr_t)h->cells, (uint64_t)h->stats_on};
+  static_assert(sizeof(words) / sizeof(words[0]) <= WM_GRAPH_KEY_WORDS, "graph key too small for its contents");
+  memcpy(key, words, sizeof(words));
 
   if (!h->graph_exec || memcmp(key, h->graph_key, sizeof(key)) != 0) {
     wm_drop_graph(h);
@@ -463,3 +466,18 @@ extern "C" int wm_rollout_host(wm_handle* h, const wm_traj* lh, const wm_roadgra
   WM_CUDA(cudaStreamSynchronize(s));
   return WM_OK;
 }
+
+#ifdef WM_DEBUG_EXPORT
+// development builds only (never in libwm_b200.so): copy one scenario's search structures to the host
+extern "C" int wm_debug_copy_grid(wm_handle* h, int32_t b, void* cells_host, void* pool_host, void* grid_host, void* segrec_host, int32_t* seg_cap) {
+  if (!h || !h->cells) return WM_ERR_STATE;
+  cudaDeviceSynchronize();
+  const int64_t cap = (int64_t)h->seg_tiles * WM_TILE_SEGS;
+  WM_CUDA(cudaMemcpy(cells_host, h->cells + (int64_t)b * WM_GRID_CELLS, sizeof(uint2) * WM_GRID_CELLS, cudaMemcpyDeviceToHost));
+  WM_CUDA(cudaMemcpy(pool_host, h->pool + (int64_t)b * WM_POOL_CAP, sizeof(uint32_t) * WM_POOL_CAP, cudaMemcpyDeviceToHost));
+  WM_CUDA(cudaMemcpy(grid_host, h->gridp + b, sizeof(WmGrid), cudaMemcpyDeviceToHost));
+  if (segrec_host) WM_CUDA(cudaMemcpy(segrec_host, h->segrec + (int64_t)b * cap * 2, sizeof(float4) * 2 * cap, cudaMemcpyDeviceToHost));
+  if (seg_cap) *seg_cap = (int32_t)cap;
+  return WM_OK;
+}
+#endif

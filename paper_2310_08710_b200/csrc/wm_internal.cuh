@@ -56,6 +56,7 @@ constexpr int WM_PT_NG = 64;
 constexpr int WM_PT_CELLS = WM_PT_NG * WM_PT_NG;
 struct WmPtGrid { float x0, y0, inv_h, h; int nx, ny, nvalid, pad; };
 
+constexpr int WM_GRAPH_KEY_WORDS = 40;     // cache key of the captured rollout graph (wm_api.cu)
 constexpr int WM_HOST_CHUNKS = 16;          // scenario chunks of the pipelined host path
 
 struct wm_handle {
@@ -89,7 +90,7 @@ struct wm_handle {
   cudaGraph_t graph;
   cudaGraphExec_t graph_exec;
   int64_t graph_kernels;
-  uint64_t graph_key[24];
+  uint64_t graph_key[WM_GRAPH_KEY_WORDS];
   // scratch for rollouts / host staging
   void* scratch; size_t scratch_bytes;
   void* stage[16]; size_t stage_bytes[16];
