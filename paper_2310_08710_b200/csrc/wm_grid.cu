@@ -19,7 +19,7 @@
 // ======================================================================================
 // grid construction (wm_prepare)
 // ======================================================================================
-constexpr int BUILD_MAXRUN = 16;          // runs per cell before the cell falls back to the full search
+constexpr int BUILD_MAXRUN = WM_GRID_MAXRUN;   // runs per cell before the cell falls back to the full search
 constexpr int BUILD_MAXCAND = 256;        // candidates per cell before it falls back
 
 __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const float4* chunks, int seg_cap, float h_min,
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
       g.obase = 4 * ((g.nx + 1) >> 1) * ((g.ny + 1) >> 1);
     }
     gridp[b] = g;
-    pool_cnt[b] = 1;                                             // offset 0 is reserved (a header's {run, 0} means one run)
+    pool_cnt[b] = 0;
   }
 }
 
@@ -170,18 +170,17 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
     // (no list) sends the warp down the chunk-wise path.
     uint2 ph = make_uint2(0u, 0u);
     if (in) ph = cells_b[g.obase + wm_cell_index(g.icx0 + (ix >> 2), g.icy0 + (iy >> 2), g.onx)];
-    if (!__any_sync(0xffffffffu, ph.x == 0xffffffffu)) {
-      auto walk = [&](auto&& f) {
-        uint32_t r = ph.x, r1 = ph.y;
+    if (!__any_sync(0xffffffffu, (ph.x & ph.y) == 0xffffffffu)) {
+      auto walk = [&](auto&& f) {                       // the parent's pair runs (wm_internal.cuh), record by record
+        uint32_t r = ph.x & 0x1fffffu, r1 = ((ph.x >> 21) | (ph.y << 11)) & 0x1fffffu, r2 = ph.y >> 10;
         const uint32_t* pl = pool_b;
         int np = 0;
-        if (r1 != 0u && (r1 & 255u) == 0u) { pl += (r1 >> 8) & 0xfffffu; np = (int)(r1 >> 28); r1 = 0u; }
+        if (r2 & 0x200000u) { pl += r2 & 0x1fffffu; np = (int)pl[0]; r2 = pl[1]; pl += 2; --np; }
         while (r != 0u) {
-          const int s0 = (int)(r >> 8), s1 = s0 + (int)(r & 255u);
+          const int s0 = 2 * (int)(r >> 5), s1 = min(s0 + 2 * (int)(r & 31u), n);
           for (int sx = s0; sx < s1; ++sx) f(sx);
-          if (r1 != 0u) { r = r1; r1 = 0u; }
-          else if (np > 0) { r = *pl++; --np; }
-          else r = 0u;
+          r = r1; r1 = r2; r2 = 0u;
+          if (np > 0) { r2 = *pl++; --np; }
         }
       };
       walk([&](int sx) { dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * sx), __ldg(rec + 2 * sx + 1), cx, cy)); });
@@ -278,30 +277,58 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   }
   flush_run();
   if (!in) return;
-  uint2 hd = make_uint2(0xffffffffu, 0u);                      // fall back to the full search
-  if (nr <= 2 && ncand <= BUILD_MAXCAND) {
-    hd.x = nr > 0 ? s_runs[warp][0][lane] : 0u;                 // nr >= 1 whenever n > 0
-    hd.y = nr > 1 ? s_runs[warp][1][lane] : 0u;
-  } else if (nr <= BUILD_MAXRUN && ncand <= BUILD_MAXCAND) {
-    const int off = atomicAdd(&pool_cnt[b], nr - 1);            // the (nr - 1) runs after the first
-    if (off + nr - 1 <= WM_POOL_CAP) {
-      uint32_t* pr = pool_b + off;
-      for (int i = 1; i < nr; ++i) pr[i - 1] = s_runs[warp][i][lane];
-      hd.x = s_runs[warp][0][lane]; hd.y = ((uint32_t)(nr - 1) << 28) | ((uint32_t)off << 8);
+  // query header (wm_internal.cuh): the record runs as runs of pair records (runs that meet in a pair
+  // merge, runs of more than 31 pairs split), three in the header or two + the rest in the pool
+  uint2 hd = make_uint2(0xffffffffu, 0xffffffffu);              // fall back to the full search
+  if (n <= 0) hd = make_uint2(0u, 0u);
+  else if (nr <= BUILD_MAXRUN && ncand <= BUILD_MAXCAND) {
+    // in place: s_runs[i] <- (first pair << 12 | pairs), nm merged runs, nq runs after splitting
+    int nm = 0, nq = 0;
+    {
+      int ps = -1, pe = -2;
+      for (int i = 0; i < nr; ++i) {
+        const uint32_t r = s_runs[warp][i][lane];
+        const int f = (int)(r >> 8), c = (int)(r & 255u);
+        const int a = f >> 1, z = (f + c - 1) >> 1;
+        if (a <= pe + 1) pe = max(pe, z);
+        else {
+          if (pe >= ps && ps >= 0) { s_runs[warp][nm][lane] = ((uint32_t)ps << 12) | (uint32_t)(pe - ps + 1); ++nm; nq += (pe - ps + 31) / 31; }
+          ps = a; pe = z;
+        }
+      }
+      if (pe >= ps && ps >= 0) { s_runs[warp][nm][lane] = ((uint32_t)ps << 12) | (uint32_t)(pe - ps + 1); ++nm; nq += (pe - ps + 31) / 31; }
+    }
+    if (nq <= BUILD_MAXRUN) {
+      uint32_t f0 = 0u, f1 = 0u, f2 = 0u;
+      uint32_t* pw = nullptr;
+      bool ok = true;
+      if (nq > 3) {
+        const int off = atomicAdd(&pool_cnt[b], nq - 1);        // count word + (nq - 2) runs
+        if (off + nq - 1 <= WM_POOL_CAP && off < (1 << 21)) { pw = pool_b + off; pw[0] = (uint32_t)(nq - 2); f2 = 0x200000u | (uint32_t)off; }
+        else ok = false;
+      }
+      int k = 0;
+      for (int i = 0; i < nm && ok; ++i) {
+        const uint32_t r = s_runs[warp][i][lane];
+        int first = (int)(r >> 12), left = (int)(r & 4095u);
+        while (left > 0) {
+          const int m = min(left, 31);
+          const uint32_t w = ((uint32_t)first << 5) | (uint32_t)m;
+          if (k == 0) f0 = w; else if (k == 1) f1 = w; else if (pw) pw[k - 1] = w; else f2 = w;
+          ++k; first += m; left -= m;
+        }
+      }
+      if (ok) { hd.x = f0 | (f1 << 21); hd.y = (f1 >> 11) | (f2 << 10); }
     }
   }
   cells_b[(FINE ? 0 : g.obase) + wm_cell_index(ix, iy, gnx)] = hd;
 }
 
 cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
-  // inner cell side (lower bound), metres of outer / inner grid beyond the segments' bounding box; the
-  // cell sides grow when the boxes do not fit WM_GRID_NG_OUT / WM_GRID_NG_IN cells
-  static float h_min = 0.f, margin = 0.f, margin_in = 0.f;
-  if (h_min <= 0.f) {
-    const char* e = getenv("WM_GRID_CELL"); h_min = e ? (float)atof(e) : 2.0f; if (!(h_min >= 0.25f && h_min <= 64.f)) h_min = 2.0f;
-    e = getenv("WM_GRID_MARGIN"); margin = e ? (float)atof(e) : 120.f; if (!(margin >= 1.f && margin <= 4096.f)) margin = 120.f;
-    e = getenv("WM_GRID_MARGIN_IN"); margin_in = e ? (float)atof(e) : 32.f; if (!(margin_in >= 0.5f && margin_in <= margin)) margin_in = fminf(32.f, margin);
-  }
+  // inner cell side (lower bound), metres of outer / inner grid beyond the segments' bounding box (an agent at
+  // 15 m/s leaves the map by up to 120 m in 8 s); the cell sides grow when the boxes do not fit
+  // WM_GRID_NG_OUT / WM_GRID_NG_IN cells
+  const float h_min = 2.0f, margin = 120.f, margin_in = 32.f;
   const int seg_cap = h->seg_tiles * WM_TILE_SEGS;
   const float4* segrec = h->segrec + (int64_t)b0 * seg_cap * 2;
   const float4* chunks = h->chunks + (int64_t)b0 * (seg_cap / WM_CHUNK);

@@ -10,8 +10,8 @@
 //     dist(c, s) <= dmin(c) + 2 rho        (triangle inequality, twice)
 // where dmin(c) is the distance from c to its own nearest segment.  The cell keeps those segments
 // (minus the ones a neighbour on the same polyline always beats, wm_grid.cu), as runs of
-// consecutive record indices: polyline pieces are contiguous, so a road cell holds 1-3 runs.  A
-// query is then: one 8-byte header load, a walk over ~7 candidate records, no bounding tests.
+// consecutive pair records: polyline pieces are contiguous, so a road cell holds 1-3 runs.  A
+// query is then: one 8-byte header load, a walk over ~4 pair records, no bounding tests.
 // Cells with too many runs, and points outside both grids, take a warp search over all 32-record
 // chunks with bounding-box culling, which is exact as well.  Per-pair arithmetic is the same as in
 // the brute-force kernel (wm_offroad.cu): both modes return the same bits whenever they pick the
@@ -78,40 +78,44 @@ __device__ __forceinline__ void wm_pair_d2(const float4 P, const float4 NE, cons
   upk2(fma2(ry, ry, mul2(rx, rx)), d_e, d_o);
 }
 
+// Cell header (8 bytes, wm_internal.cuh): up to three runs of PAIR records, 21 bits each
+// (first pair << 5 | pairs, pairs <= 31), in bits 0-20, 21-41, 42-62.  Bit 63 set: the third field is
+// an offset into the pool instead, pool[offset] = n further runs, pool[offset + 1 ...] = the runs.
+// All ones = too many candidates: search all chunks.  Zero = nothing to walk.
+//
 // Walk of a cell's candidate runs as ONE flat loop (a warp runs max-over-lanes of the total
-// count, not the sum of per-run maxima), one pair record = 2 records per iteration (measured
-// against two pair records per iteration in the fused rollout at 40 warps per SM: 1.3 % faster,
-// less padding and less code).  A run that starts or ends inside a pair record evaluates the
-// pair's other record too: evaluating a real segment that is not a candidate cannot change the
-// result (it is no nearer than the winner, and on an exact tie the winner has the lower index:
-// D17; indices are visited in ascending order with strict '<').  Padding records sit at 1e18.
-// Up to 4 runs sit in registers, refilled from the pool.
-__device__ __forceinline__ void wm_grid_walk(const float4* __restrict__ pr, uint32_t r0, uint32_t r1, uint32_t r2,
-                                             uint32_t r3, const uint32_t* __restrict__ pool, int n_pool, float cx,
-                                             float cy, float offx, float offy, float& best, int& bs, int& n_eval) {
+// count, not the sum of per-run maxima), one pair record = 2 records per iteration.  A run counts
+// whole pair records: evaluating a real segment that is not a candidate cannot change the result
+// (it is no nearer than the winner, and on an exact tie the winner has the lower index: D17;
+// indices are visited in ascending order with strict '<').  Padding records sit at 1e18.
+// The current run is one word, (pair << 5 | pairs left): an iteration adds 31 to it; the next two
+// runs wait in registers, further ones come from the pool.
+__device__ __forceinline__ void wm_grid_walk(const float4* __restrict__ pr, uint32_t cur, uint32_t nx1, uint32_t nx2,
+                                             const uint32_t* __restrict__ pool, float cx, float cy, float offx, float offy,
+                                             float& best, int& bs, int& n_eval) {
   const wm_u64 cx2 = pk2(cx, cx), cy2 = pk2(cy, cy), ox2 = pk2(offx, offx), oy2 = pk2(offy, offy);
-  int p = 0, pe = -1;
+  int n_pool = 0;
+  if (nx2 & 0x200000u) {                                            // the third field points into the pool
+    pool += nx2 & 0x1fffffu;
+    n_pool = (int)__ldg(pool);
+    nx2 = __ldg(pool + 1);
+    pool += 2; n_pool -= 1;
+  }
   for (;;) {
-    if (p > pe) {
-      if (r0 == 0u) {
-        if (n_pool <= 0) break;
-        r0 = __ldg(pool);
-        r1 = n_pool > 1 ? __ldg(pool + 1) : 0u;
-        r2 = n_pool > 2 ? __ldg(pool + 2) : 0u;
-        r3 = n_pool > 3 ? __ldg(pool + 3) : 0u;
-        pool += 4; n_pool -= 4;
-      }
-      const int first = (int)(r0 >> 8), cnt = (int)(r0 & 255u);
-      p = first >> 1; pe = (first + cnt - 1) >> 1;
-      n_eval += cnt;
-      r0 = r1; r1 = r2; r2 = r3; r3 = 0u;
+    if ((cur & 31u) == 0u) {                                        // run finished: the next one
+      if (nx1 == 0u) break;
+      cur = nx1; nx1 = nx2; nx2 = 0u;
+      if (n_pool > 0) { nx2 = __ldg(pool); ++pool; --n_pool; }
     }
-    const float4 a0 = __ldg(pr + 3 * p), a1 = __ldg(pr + 3 * p + 1), a2 = __ldg(pr + 3 * p + 2);
+    const uint32_t p = cur >> 5;
+    const float4* a = pr + (size_t)p * 3u;
+    const float4 a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2);
     float d0, d1;
     wm_pair_d2(a0, a1, a2, cx2, cy2, ox2, oy2, d0, d1);
-    if (d0 < best) { best = d0; bs = 2 * p; }       // ascending index, strict '<': exact ties -> lower index (D17)
-    if (d1 < best) { best = d1; bs = 2 * p + 1; }
-    p += 1;
+    if (d0 < best) { best = d0; bs = (int)(2u * p); }               // ascending index, strict '<': exact ties -> lower index (D17)
+    if (d1 < best) { best = d1; bs = (int)(2u * p + 1u); }
+    cur += 31u;                                                     // pair + 1, pairs left - 1
+    n_eval += 2;
   }
 }
 
@@ -227,13 +231,14 @@ __device__ __forceinline__ void wm_grid_search_warp4(const WmGridView& v, float 
 }
 
 // ---- query API (D15-D17, D19, D20) -------------------------------------------------------
-// wm_grid_fast:   per thread; walks the candidate list of the corner's cell.  Returns true when
-//                 the corner needs the warp search instead (outside the grid, crowded cell).
+// wm_grid_header: per thread; the header of the corner's cell: 0 = nothing to walk (inactive lane,
+//                 no segments), all ones = the corner needs the warp search (outside both grids,
+//                 crowded cell).
+// wm_grid_fast_hd: per thread; walks the candidate list.  Returns true when the corner needs the
+//                 warp search instead.
 // wm_grid_search_warp: above.
 // wm_grid_finish: per thread; sign from the oriented winning segment and the signed distance.
 // wm_grid_corner_sd: the three combined for a warp of corners (k_offroad_grid).
-// header of the corner's cell, as the walk wants it: {0, 0} nothing to walk (inactive lane, no
-// segments), {~0, 0} the corner needs the warp search (outside the grid, crowded cell)
 __device__ __forceinline__ uint2 wm_grid_header(const WmGridView& v, bool active, float cx, float cy, float offx, float offy) {
   uint2 hd = make_uint2(0u, 0u);
   if (active && v.g.nseg > 0) {
@@ -245,7 +250,7 @@ __device__ __forceinline__ uint2 wm_grid_header(const WmGridView& v, bool active
       const float gx = (qx - v.g.ox0) * v.g.oinv_h, gy = (qy - v.g.oy0) * v.g.oinv_h;
       const int jx = (int)floorf(gx), jy = (int)floorf(gy);
       if (gx >= 0.f && gy >= 0.f && jx < v.g.onx && jy < v.g.ony) hd = __ldg(v.cells + v.g.obase + wm_cell_index(jx, jy, v.g.onx));
-      else hd = make_uint2(0xffffffffu, 0u);
+      else hd = make_uint2(0xffffffffu, 0xffffffffu);
     }
   }
   return hd;
@@ -255,23 +260,12 @@ __device__ __forceinline__ bool wm_grid_fast_hd(const WmGridView& v, uint2 hd, f
                                                 float& best, int& bs, int& n_eval) {
   best = __int_as_float(0x7f800000);
   bs = 0;
-  uint32_t r0 = hd.x, r1 = hd.y;
-  const uint32_t* pool = v.pool;
-  int n_pool = 0;
-  const bool slow = r0 == 0xffffffffu;
-  if (slow) { r0 = 0u; r1 = 0u; }
-  else if (r1 != 0u && (r1 & 255u) == 0u) {                       // further runs in the pool
-    pool += (r1 >> 8) & 0xfffffu;
-    n_pool = (int)(r1 >> 28);
-    r1 = 0u;
-  }
-  wm_grid_walk(v.pair, r0, r1, 0u, 0u, pool, n_pool, cx, cy, offx, offy, best, bs, n_eval);   // no-op without runs
+  const bool slow = (hd.x & hd.y) == 0xffffffffu;
+  if (slow) { hd.x = 0u; hd.y = 0u; }
+  // the three 21-bit fields; bit 21 of the third = "pool offset"
+  const uint32_t r0 = hd.x & 0x1fffffu, r1 = ((hd.x >> 21) | (hd.y << 11)) & 0x1fffffu, r2 = hd.y >> 10;
+  wm_grid_walk(v.pair, r0, r1, r2, v.pool, cx, cy, offx, offy, best, bs, n_eval);            // no-op without runs
   return slow;
-}
-
-__device__ __forceinline__ bool wm_grid_fast(const WmGridView& v, bool active, float cx, float cy, float offx, float offy,
-                                             float& best, int& bs, int& n_eval) {
-  return wm_grid_fast_hd(v, wm_grid_header(v, active, cx, cy, offx, offy), cx, cy, offx, offy, best, bs, n_eval);
 }
 
 __device__ __forceinline__ float wm_grid_finish(const WmGridView& v, float cx, float cy, float offx, float offy, float best,
@@ -299,7 +293,7 @@ __device__ __forceinline__ float wm_grid_corner_sd(const WmGridView& v, bool act
   const int lane = threadIdx.x & 31;
   float best;
   int bs;
-  const bool slow = wm_grid_fast(v, active, cx, cy, offx, offy, best, bs, n_eval);
+  const bool slow = wm_grid_fast_hd(v, wm_grid_header(v, active, cx, cy, offx, offy), cx, cy, offx, offy, best, bs, n_eval);
   fell_back = slow;
   uint32_t todo = __ballot_sync(0xffffffffu, slow);
   while (todo) {

@@ -25,16 +25,18 @@ constexpr int WM_TILE_BYTES = WM_TILE_F4 * 16;   // 12288
 constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding segments
 
 // Exact grid search (wm_grid.cuh): road-edge segments in ascending source order as 32-byte
-// records, bounding boxes per chunk of WM_CHUNK records, and TWO nested grids of square cells per
-// scenario: a fine inner grid (<= WM_GRID_NG_IN^2 cells, side >= 2 m) over the segments' bounding
-// box plus a small margin, where nearly all queries land, and a coarse outer grid
-// (<= WM_GRID_NG_OUT^2 cells, side >= 4 x the inner side) over the wide margin that agents reach
-// when they drive off the map.  The inner grid is aligned with the outer one: an outer cell under
-// it is the PARENT of 4 x 4 inner cells, and wm_prepare builds an inner cell's candidates from its
-// parent's list instead of from all segments (wm_grid.cu).  A cell has an 8-byte header {a, b} of runs, run = (first record << 8) | count:
-//   {run, 0}                one run             {run, run}     two runs
-//   {run, n << 28 | pool offset << 8} more: n further runs at pool[offset] (offset >= 1, n <= 15)
-//   {~0, 0}                 too many candidates: search all chunks
+// records (and two by two as 48-byte PAIR records), bounding boxes per chunk of WM_CHUNK records,
+// and TWO nested grids of square cells per scenario: a fine inner grid (<= WM_GRID_NG_IN^2 cells,
+// side >= 2 m) over the segments' bounding box plus a small margin, where nearly all queries land,
+// and a coarse outer grid (<= WM_GRID_NG_OUT^2 cells, side >= 4 x the inner side) over the wide
+// margin that agents reach when they drive off the map.  The inner grid is aligned with the outer
+// one: an outer cell under it is the PARENT of 4 x 4 inner cells, and wm_prepare builds an inner cell's
+// candidates from its parent's list instead of from all segments (wm_grid.cu).  A cell has an 8-byte header of up to three runs of pair records, 21 bits
+// each (first pair << 5 | pairs, 1 <= pairs <= 31) in bits 0-20, 21-41, 42-62:
+//   bit 63 clear            1-3 runs (unused fields zero); zero = nothing to walk
+//   bit 63 set              two runs, and bits 42-62 = offset into the pool: pool[offset] = n further
+//                           runs (n <= WM_GRID_MAXRUN - 2), pool[offset + 1 ...] = those runs
+//   all ones                too many candidates: search all chunks
 // Headers are stored in tiles of 2 x 2 cells (one 32-byte sector = 4 m x 4 m at the default
 // inner cell side), tile-row-major: the four corners of a box and its next steps share sectors.
 // The outer grid's headers follow the inner grid's at cell offset WmGrid::obase.
@@ -42,12 +44,13 @@ constexpr int WM_CHUNK = 32;
 constexpr int WM_GRID_NG_IN = 160;
 constexpr int WM_GRID_NG_OUT = 64;
 constexpr int WM_GRID_CELLS = WM_GRID_NG_IN * WM_GRID_NG_IN + WM_GRID_NG_OUT * WM_GRID_NG_OUT;
-constexpr int WM_POOL_CAP = 2 * WM_GRID_CELLS;   // words of overflow runs per scenario
+constexpr int WM_POOL_CAP = WM_GRID_CELLS;       // words of overflow runs per scenario
+constexpr int WM_GRID_MAXRUN = 16;               // runs per cell before the cell falls back to the full search
+constexpr int WM_MAX_RECORDS = 131072;           // pair indices are 16 bits
 struct WmGrid {
   float x0, y0, inv_h, h; int nx, ny, nseg, obase;        // inner grid; obase = first outer header
   float ox0, oy0, oinv_h, oh; int onx, ony, icx0, icy0;   // outer grid; the inner grid starts at its cell (icx0, icy0)
 };
-
 // Prepared roadgraph points for the top-k observation (wm_observe.cu): the valid points of a
 // scenario bucketed into a uniform grid of at most WM_PT_NG x WM_PT_NG cells (side >= 4 m) over
 // their bounding box, stored cell by cell in row-major cell order: (x, y), original index, and the

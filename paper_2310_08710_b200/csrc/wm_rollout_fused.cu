@@ -1,17 +1,23 @@
-// a8 closed-loop rollout ("Rollout ... faster than running Step 80 times"), fused:
-// ONE kernel runs all n_steps of a scenario — dynamics (a1/a2), log divergence (a5), pairwise
-// overlap (a3), offroad (a4) and the aggregates — one CTA per scenario, the scenario's state
-// resident in shared memory.
+// a8 closed-loop rollout ("Rollout ... faster than running Step 80 times"), fused
+// into TWO kernels that run back to back in one CUDA graph:
 //
-// The successor state depends on the state and the action only, never on a metric.  So the steps
-// are taken in blocks of up to FUSED_S: the agent threads first run the dynamics of the whole
-// block (one serial chain per agent, next step's inputs prefetched), leaving what the metrics need
-// (centre, sin/cos, half extents) in per-step slots of shared memory; then the metric work of all
-// steps of the block is one pool of independent warp tasks, handed out through a shared counter:
+//   k_rollout_dyn      one thread per (scenario, agent): the serial chain of n_steps successor states
+//                      (a1/a2, shared arithmetic with k_step: wm_device.cuh), log playback (D8), sim rows
+//                      -> HBM, log divergence (a5) and ADE.  The successor state depends on the state and
+//                      the action only, never on a metric, so the whole trajectory is laid down first.
+//                      HBM bound: ~51 B per agent-step.
+//   k_rollout_metrics  one CTA per (scenario, block of S steps), scheduled scenario-major: overlap (a3)
+//                      and offroad (a4) of the block's rows and the any-flags.  Every (scenario, block)
+//                      is independent, so nothing in this kernel is serial; consecutive CTAs belong to
+//                      the same scenario, so only ~B/10 scenarios are in flight at a time and their
+//                      search data (cell headers, pair records) stays in L2 instead of being re-fetched
+//                      from HBM (the single-kernel version of round 1 kept 740 scenarios in flight:
+//                      L2 hit rate 29 %, DRAM traffic 1.96 x the compulsory bytes).
 //
-//   phase A  one thread per agent : S successor states (shared arithmetic with k_step:
-//            wm_device.cuh), sim rows -> HBM, log divergence, per-step slots; the agent's bounding
-//            box over the block goes into a spatial hash
+//   metrics kernel, per CTA:
+//   phase A  all threads          : rows of the block -> per-step slots in shared memory (centre, sin/cos,
+//                                   half extents); then one thread per agent: its bounding box over the
+//                                   block into a spatial hash (warps 0-3, while the others start phase B)
 //   phase B  warp tasks, any warp : (agent, S steps) -> its 4 S box corners, one per lane: candidate
 //                                   walk of the corner's grid cell (wm_grid.cuh).  The lanes of a task
 //                                   follow one agent through consecutive steps, so they walk the
@@ -21,33 +27,29 @@
 //                                   3 x 3 hash cells around its agent and lists the pairs whose
 //                                   block bounding boxes meet; then one lane per (pair, step) runs
 //                                   the circle and separating-axis tests
-//   phase C  one thread per agent : metric rows of the block -> HBM, any-flags
+//   phase C  all threads          : metric rows of the block -> HBM, any-flags
 //
 // Overlap broad phase, once per block: an agent is hashed by the 24 m cell of the centre of its
-// bounding box over the block (linked lists in shared memory, entries tagged with the block number
-// so nothing is ever cleared).  Two agents whose boxes (inflated by the circumradius) have half
-// extents <= 11.7 m can only overlap from adjacent cells; larger ones go to a list that every agent
-// checks, and check every agent themselves.  A pair is always evaluated with the lower agent index
-// in the i role, like k_overlap, so flags equal the stepwise kernels' bit for bit.
+// bounding box over the block (linked lists in shared memory).  Two agents whose boxes (inflated by
+// the circumradius) have half extents <= 11.7 m can only overlap from adjacent cells; larger ones go
+// to a list that every agent checks, and check every agent themselves.  A pair is always evaluated
+// with the lower agent index in the i role, like k_overlap, so flags equal the stepwise kernels' bit
+// for bit.
 //
-// Bound: instruction issue and the latency of the candidate walk's dependent loads; compulsory HBM
-// traffic is ~77 B per agent-step.  Results are bit-identical to the stepwise graph
-// (WM_ROLLOUT_STEPWISE), which runs the same device functions kernel by kernel.
+// Results are bit-identical to the stepwise graph (WM_ROLLOUT_STEPWISE), which runs the same device
+// functions kernel by kernel.
 #include "wm_device.cuh"
 #include "wm_grid.cuh"
 
-#ifndef FUSED_NT
-#define FUSED_NT 256
-#endif
-#ifndef FUSED_MINB
-#define FUSED_MINB 5
-#endif
-constexpr int FUSED_S = 8;                 // steps per block: 8, 4, 2 or 1 (fewer when A is large: shared memory)
-constexpr float FUSED_HASH_H = 24.f;       // hash cell side, metres
-constexpr float FUSED_EXT_MAX = 11.7f;     // half extent limit of hashed agents (< FUSED_HASH_H / 2, with margin)
+constexpr int FUSED_NT = 256;               // threads per CTA of the metrics kernel
+constexpr int FUSED_MINB = 5;               // CTAs per SM it is compiled for (48 registers)
+constexpr int FUSED_S = 8;                  // steps per block: 8, 4, 2 or 1 (fewer when A is large: shared memory)
+constexpr float FUSED_HASH_H = 24.f;        // hash cell side, metres
+constexpr float FUSED_EXT_MAX = 11.7f;      // half extent limit of hashed agents (< FUSED_HASH_H / 2, with margin)
 constexpr uint32_t FUSED_EMPTY = 0xffffu;
 constexpr int FUSED_PAD = 4;                // slot rows are Ap + 4 long: the 8 steps of an agent fall into 8 different banks
 constexpr int FUSED_PL = 48;                // pair list entries per warp (overlap narrow phase)
+constexpr int DYN_NT = 128;                 // threads per CTA of the dynamics kernel
 
 struct FusedParams {
   wm_traj log, sim;
@@ -61,10 +63,10 @@ struct FusedParams {
   unsigned long long* stats;
 };
 
-// shared-memory carve-up: persistent per-agent state, then S per-step slots
+// shared-memory carve-up of the metrics kernel: per-agent block state, then S per-step slots
 __host__ __device__ inline int fused_nbk(int Ap) { int n = 64; while (n < 2 * Ap) n <<= 1; return n; }
 __host__ __device__ inline size_t fused_persist_bytes(int Ap) {
-  return (size_t)Ap * (8 + 9 * 4 + 4 + 4 + 16 + 4 + 2 + 2) + (size_t)fused_nbk(Ap) * 4 + 64 + (FUSED_NT / 32) * (FUSED_PL + 1) * 4;
+  return (size_t)Ap * (16 + 4 + 2 + 2 + 1) + (size_t)fused_nbk(Ap) * 4 + 64 + (FUSED_NT / 32) * (FUSED_PL + 1) * 4 + 16;
 }
 __host__ __device__ inline size_t fused_slot_bytes(int Ap) { return (size_t)(Ap + FUSED_PAD) * (7 * 4 + 2); }
 static inline int fused_pick_S(int A) {
@@ -83,12 +85,69 @@ __device__ __forceinline__ FusedIn fused_load_in(const FusedParams& p, int64_t s
   FusedIn r;
   const int64_t o = sb + (int64_t)(p.t0 + k + 1) * A + a;
   const int64_t ak = ab + k;
-  // streamed once: evict-first loads, so that they do not push the search data out of L1 / L2
+  // streamed once: evict-first loads
   r.av = __ldcs(p.av + ak * A + a);
   const float* act = p.actions + ak * C * A + a;
   r.a0 = __ldcs(act); r.a1 = __ldcs(act + A); r.a2 = C > 2 ? __ldcs(act + 2 * (int64_t)A) : 0.f;
   r.lx = __ldcs(p.log.x + o); r.ly = __ldcs(p.log.y + o); r.lv = __ldcs(p.log.valid + o);
   return r;
+}
+
+// ======================================================================================
+// k_rollout_dyn: the trajectory (a1 / a2, D8, D9), log divergence (a5), ADE (D21)
+// ======================================================================================
+// DYN_C >= 0: the dynamics model is a compile-time constant
+template <int DYN_C>
+__global__ void __launch_bounds__(DYN_NT) k_rollout_dyn(FusedParams p) {
+  const int A = p.sim.A, nba = (A + DYN_NT - 1) / DYN_NT;
+  const int b = blockIdx.x / nba, a = (blockIdx.x % nba) * DYN_NT + threadIdx.x;
+  if (a >= A) return;
+  WmDynCfg dyn = p.dyn;
+  if (DYN_C >= 0) dyn.dynamics = DYN_C;
+  const int C = DYN_C >= 0 ? (DYN_C == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3) : p.C;
+  const int64_t TA = (int64_t)p.sim.T * A;
+  const int64_t sb = (int64_t)b * TA;                // scenario offset in the trajectories
+  const int64_t ab = (int64_t)b * p.n_steps;         // scenario offset in the action / metric rows, in rows
+  const int64_t o0 = sb + (int64_t)p.t0 * A + a;
+  bool v = p.sim.valid[o0] != 0;
+  float x = 0.f, y = 0.f, th = 0.f, vx = 0.f, vy = 0.f, ln = 0.f, wd = 0.f, sn = 0.f, cs = 1.f;
+  if (v) {
+    x = p.sim.x[o0]; y = p.sim.y[o0]; th = p.sim.yaw[o0]; vx = p.sim.vel_x[o0]; vy = p.sim.vel_y[o0];
+    ln = p.sim.length[o0]; wd = p.sim.width[o0];
+    sincosf(th, &sn, &cs);
+  }
+  double sum = 0.0;                                   // sum of valid log divergences (D21)
+  int cnt = 0;
+  FusedIn in = fused_load_in(p, sb, ab, 0, a, A, C);
+#pragma unroll 1
+  for (int k = 0; k < p.n_steps; ++k) {
+    const FusedIn cur = in;
+    if (k + 1 < p.n_steps) in = fused_load_in(p, sb, ab, k + 1, a, A, C);     // prefetch: nothing below depends on it
+    const int64_t o = sb + (int64_t)(p.t0 + k + 1) * A + a;
+    const bool use_dyn = cur.av != 0 && v;                          // D8
+    float xn, yn, thn, vxn, vyn, s1 = 0.f, c1 = 1.f;
+    if (use_dyn) {
+      wm_dyn_step(dyn, x, y, th, vx, vy, sn, cs, cur.a0, cur.a1, cur.a2, xn, yn, thn, vxn, vyn, s1, c1);
+      v = true;                                                     // D9: keeps its box
+    } else {                                                        // log playback, L164
+      xn = cur.lx; yn = cur.ly; thn = p.log.yaw[o]; vxn = p.log.vel_x[o]; vyn = p.log.vel_y[o];
+      ln = p.log.length[o]; wd = p.log.width[o];
+      v = cur.lv != 0;
+      if (v) sincosf(thn, &s1, &c1);
+    }
+    __stcs(p.sim.x + o, xn); __stcs(p.sim.y + o, yn); __stcs(p.sim.yaw + o, thn);
+    __stcs(p.sim.vel_x + o, vxn); __stcs(p.sim.vel_y + o, vyn);
+    __stcs(p.sim.length + o, ln); __stcs(p.sim.width + o, wd); __stcs(p.sim.valid + o, (uint8_t)v);
+    const bool ldv = v && cur.lv != 0;                              // a5, L106
+    const float d = ldv ? wm_logdiv(xn, yn, cur.lx, cur.ly) : 0.f;
+    if (p.out.log_div) __stcs(p.out.log_div + (ab + k) * A + a, d);
+    if (ldv) { sum += (double)d; cnt += 1; }
+    x = xn; y = yn; th = thn; vx = vxn; vy = vyn; sn = s1; cs = c1;
+  }
+  const int64_t oa = (int64_t)b * A + a;
+  if (p.out.ade) p.out.ade[oa] = cnt ? (float)(sum / cnt) : 0.f;
+  if (p.out.any_overlap) p.out.any_overlap[oa] = 0;                 // the metrics kernel sets the flags that are 1
+  if (p.out.any_offroad) p.out.any_offroad[oa] = 0;
 }
 
 __device__ __forceinline__ int fused_cell(float v) {
@@ -98,33 +157,26 @@ __device__ __forceinline__ uint32_t fused_bucket(int ix, int iy, uint32_t mask) 
   return (((uint32_t)ix * 73856093u) ^ ((uint32_t)iy * 19349663u)) & mask;
 }
 
+// ======================================================================================
+// k_rollout_metrics: overlap (a3) and offroad (a4) of one block of steps of one scenario
+// ======================================================================================
 // AP_C / S_C > 0: padded agent count and steps per block known at compile time (the shared-memory
 // carve-up then folds into immediate offsets); 0: taken from the arguments.
-template <int AP_C, int S_C, int DYN_C, bool STATS>
-__global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedParams p) {
+template <int AP_C, int S_C, bool STATS>
+__global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_metrics(FusedParams p, int nblk) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int A = p.sim.A, nb = AP_C ? AP_C / 32 : (A + 31) / 32, Ap = nb * 32, Aps = Ap + FUSED_PAD, S = S_C ? S_C : p.S;
   const int NBK = fused_nbk(Ap);
-  WmDynCfg dyn = p.dyn;                              // DYN_C >= 0: the dynamics model is a compile-time constant
-  if (DYN_C >= 0) dyn.dynamics = DYN_C;
-  const int C = DYN_C >= 0 ? (DYN_C == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3) : p.C;
-  // ---- persistent per-agent state ----
-  double* s_sum = (double*)smem_raw;                 // [Ap] sum of valid log divergences (D21)
-  float4* s_bb = (float4*)(s_sum + Ap);              // [Ap] bounding box over the block, inflated: x0, y0, x1, y1
-  float* sx = (float*)(s_bb + Ap);
-  float* sy = sx + Ap;    float* syaw = sy + Ap;   float* svx = syaw + Ap;  float* svy = svx + Ap;
-  float* slen = svy + Ap; float* swid = slen + Ap; float* sc = swid + Ap;   float* ss = sc + Ap;
-  float* s_br = ss + Ap;                             // [Ap] largest circumradius over the block, inflated
-  int* s_cnt = (int*)(s_br + Ap);                    // [Ap] count of valid log divergences
-  uint32_t* heads = (uint32_t*)(s_cnt + Ap);         // [NBK] (block tag << 16) | agent
-  int* s_nover = (int*)(heads + NBK);                // [2] oversize counts, by block parity (+ padding to 64 B)
+  // ---- per-agent state of the block ----
+  float4* s_bb = (float4*)smem_raw;                  // [Ap] bounding box over the block, inflated: x0, y0, x1, y1
+  float* s_br = (float*)(s_bb + Ap);                 // [Ap] largest circumradius over the block, inflated
+  uint32_t* heads = (uint32_t*)(s_br + Ap);          // [NBK] first agent of the bucket, FUSED_EMPTY if none
+  int* s_nover = (int*)(heads + NBK);                // oversize count (+ padding to 64 B)
   uint32_t* s_pl = (uint32_t*)(s_nover + 16);        // [warps][FUSED_PL + 1] pairs whose block boxes meet: count, (lo << 16) | hi
-  uint16_t* nxt = (uint16_t*)(s_pl + (FUSED_NT / 32) * (FUSED_PL + 1));      // [Ap] next agent of the same bucket
+  int* s_task = (int*)(s_pl + (FUSED_NT / 32) * (FUSED_PL + 1));            // corner task counter (+ padding to 16 B)
+  uint16_t* nxt = (uint16_t*)(s_task + 4);           // [Ap] next agent of the same bucket
   uint16_t* over = nxt + Ap;                         // [Ap] agents too large for the hash
-  uint8_t* s_valid = (uint8_t*)(over + Ap);          // [Ap]
-  uint8_t* s_anyov = s_valid + Ap;                   // [Ap]
-  uint8_t* s_anyoff = s_anyov + Ap;                  // [Ap]
-  uint8_t* s_bvalid = s_anyoff + Ap;                 // [Ap] valid at some step of the block
+  uint8_t* s_bvalid = (uint8_t*)(over + Ap);         // [Ap] valid at some step of the block
   // ---- per-step slots ----
   float* px = (float*)(smem_raw + fused_persist_bytes(Ap));      // [S][Aps] each
   float* py = px + S * Aps;  float* pc = py + S * Aps;  float* ps = pc + S * Aps;
@@ -133,89 +185,46 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
   uint8_t* pvalid = (uint8_t*)(psd + S * Aps);       // [S][Aps]
   uint8_t* pov = pvalid + S * Aps;                   // [S][Aps] overlap flag (a3)
 
-  __shared__ int s_task;
-  const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+  const int b = blockIdx.x / nblk, k0 = (blockIdx.x % nblk) * S, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int Sb = min(S, p.n_steps - k0);
   const int64_t TA = (int64_t)p.sim.T * A;
-  const int64_t sb = (int64_t)b * TA;                // scenario offset in the trajectories
-  const int64_t ab = (int64_t)b * p.n_steps;         // scenario offset in the action / metric rows, in rows
+  const int64_t sb = (int64_t)b * TA + (int64_t)(p.t0 + 1 + k0) * A;      // first row of the block
+  const int64_t ab = (int64_t)b * p.n_steps + k0;    // first metric row of the block
   const WmGridView gv = wm_grid_view(p.segrec, p.segpair, p.segfin, p.chunks, p.cells, p.pool, p.gridp, p.seg_cap, WM_POOL_CAP, b);
 
-  // ---- prologue: row t0 of the simulated trajectory -> shared memory ----
-  for (int a = tid; a < Ap; a += FUSED_NT) {
-    const int64_t o = sb + (int64_t)p.t0 * A + a;
-    const bool v = a < A && p.sim.valid[o] != 0;
-    float x = 0.f, y = 0.f, th = 0.f, vx = 0.f, vy = 0.f, ln = 0.f, wd = 0.f, sn = 0.f, cs = 1.f;
-    if (v) {
-      x = p.sim.x[o]; y = p.sim.y[o]; th = p.sim.yaw[o]; vx = p.sim.vel_x[o]; vy = p.sim.vel_y[o];
-      ln = p.sim.length[o]; wd = p.sim.width[o];
-      sincosf(th, &sn, &cs);
-    }
-    sx[a] = x; sy[a] = y; syaw[a] = th; svx[a] = vx; svy[a] = vy; slen[a] = ln; swid[a] = wd;
-    sc[a] = cs; ss[a] = sn; s_valid[a] = v;
-    s_sum[a] = 0.0; s_cnt[a] = 0; s_anyov[a] = 0; s_anyoff[a] = 0;
-  }
-  for (int i = tid; i < NBK; i += FUSED_NT) heads[i] = 0u;              // tag 0 = no block
-  if (tid < 2) s_nover[tid] = 0;
-  __syncthreads();
-
-  // lanes of a corner task: 4 corners x S steps x (8 / S) agents
-  const int kk = lane & 3, ls = (lane >> 2) & (S - 1), la = (lane >> 2) / S, apt = 8 / S;
-  int n_eval = 0, n_slow = 0, n_corner = 0;
-  for (int k0 = 0, blk = 1; k0 < p.n_steps; k0 += S, ++blk) {
-    const int Sb = min(S, p.n_steps - k0);
-    const uint32_t tag = (uint32_t)(blk & 0xffff) << 16;
-    int* nover = s_nover + (blk & 1);
-    // ================= phase A: one thread per agent, Sb steps =================
-    if (tid == 0) { s_task = 0; s_nover[(blk + 1) & 1] = 0; }           // both last read before the previous barrier
-    for (int a = tid; a < Ap; a += FUSED_NT) {
-      if (a >= A) {
-        for (int s = 0; s < Sb; ++s) { pvalid[s * Aps + a] = 0; pov[s * Aps + a] = 0; psd[s * Aps + a] = 0.f; }
-        s_bvalid[a] = 0;
-        continue;
+  // ================= phase A: rows of the block -> slots =================
+  for (int e = tid; e < S * Ap; e += FUSED_NT) {
+    const int s = AP_C ? e / AP_C : e / Ap, a = e - s * Ap, q = s * Aps + a;
+    bool v = false;
+    float x = 0.f, y = 0.f, hl = 0.f, hw = 0.f, sn = 0.f, cs = 1.f;       // invalid slots: finite zeros (D10)
+    if (s < Sb && a < A) {
+      const int64_t o = sb + (int64_t)s * A + a;
+      v = __ldcs(p.sim.valid + o) != 0;
+      if (v) {
+        x = __ldcs(p.sim.x + o); y = __ldcs(p.sim.y + o);
+        hl = 0.5f * __ldcs(p.sim.length + o); hw = 0.5f * __ldcs(p.sim.width + o);
+        sincosf(__ldcs(p.sim.yaw + o), &sn, &cs);
       }
-      float x = sx[a], y = sy[a], th = syaw[a], vx = svx[a], vy = svy[a], ln = slen[a], wd = swid[a], cs = sc[a], sn = ss[a];
-      bool v = s_valid[a] != 0;
-      double sum = s_sum[a];
-      int cnt = s_cnt[a];
+    }
+    px[q] = x; py[q] = y; pc[q] = cs; ps[q] = sn; phl[q] = hl; phw[q] = hw; psd[q] = 0.f;
+    pvalid[q] = (uint8_t)v; pov[q] = 0;
+  }
+  for (int i = tid; i < NBK; i += FUSED_NT) heads[i] = FUSED_EMPTY;
+  if (tid == 0) { *s_task = 0; *s_nover = 0; }
+  __syncthreads();
+  // overlap broad phase of the block, one thread per agent (the first nb warps; the others go on to the
+  // corner tasks): the agent's boxes all lie inside [bx0 - br, bx1 + br] x [..]
+  if (warp < nb || nb > FUSED_NT / 32) {
+    for (int a = tid; a < Ap; a += FUSED_NT) {
       float bx0 = 3.0e38f, by0 = 3.0e38f, bx1 = -3.0e38f, by1 = -3.0e38f, br = 0.f;
-      FusedIn in = fused_load_in(p, sb, ab, k0, a, A, C);
-#pragma unroll 1                          // measured: the unrolled chain (8 x sincosf, row IO) costs 6 % through its code size
       for (int s = 0; s < Sb; ++s) {
-        const int k = k0 + s;
-        const FusedIn cur = in;
-        if (s + 1 < Sb) in = fused_load_in(p, sb, ab, k + 1, a, A, C);     // prefetch: nothing below depends on it
-        const int64_t o = sb + (int64_t)(p.t0 + k + 1) * A + a;
-        const bool use_dyn = cur.av != 0 && v;                          // D8
-        float xn, yn, thn, vxn, vyn, s1 = 0.f, c1 = 1.f;
-        if (use_dyn) {
-          wm_dyn_step(dyn, x, y, th, vx, vy, sn, cs, cur.a0, cur.a1, cur.a2, xn, yn, thn, vxn, vyn, s1, c1);
-          v = true;                                                     // D9: keeps its box
-        } else {                                                        // log playback, L164
-          xn = cur.lx; yn = cur.ly; thn = p.log.yaw[o]; vxn = p.log.vel_x[o]; vyn = p.log.vel_y[o];
-          ln = p.log.length[o]; wd = p.log.width[o];
-          v = cur.lv != 0;
-          if (v) sincosf(thn, &s1, &c1);
-        }
-        p.sim.x[o] = xn; p.sim.y[o] = yn; p.sim.yaw[o] = thn; p.sim.vel_x[o] = vxn; p.sim.vel_y[o] = vyn;
-        p.sim.length[o] = ln; p.sim.width[o] = wd; p.sim.valid[o] = (uint8_t)v;
-        const bool ldv = v && cur.lv != 0;                              // a5, L106
-        const float d = ldv ? wm_logdiv(xn, yn, cur.lx, cur.ly) : 0.f;
-        if (p.out.log_div) p.out.log_div[(ab + k) * A + a] = d;
-        if (ldv) { sum += (double)d; cnt += 1; }
-        x = xn; y = yn; th = thn; vx = vxn; vy = vyn; sn = s1; cs = c1;
-        // what the metrics of this step need; invalid slots: finite zeros (D10)
         const int q = s * Aps + a;
-        const float hl = v ? 0.5f * ln : 0.f, hw = v ? 0.5f * wd : 0.f;
-        px[q] = v ? xn : 0.f; py[q] = v ? yn : 0.f; pc[q] = v ? c1 : 1.f; ps[q] = v ? s1 : 0.f;
-        phl[q] = hl; phw[q] = hw; pvalid[q] = (uint8_t)v; pov[q] = 0;
-        if (v) {
+        if (pvalid[q] != 0) {
+          const float xn = px[q], yn = py[q], hl = phl[q], hw = phw[q];
           bx0 = fminf(bx0, xn); bx1 = fmaxf(bx1, xn); by0 = fminf(by0, yn); by1 = fmaxf(by1, yn);
           br = fmaxf(br, sqrtf(fmaf(hl, hl, hw * hw)));
         }
       }
-      sx[a] = x; sy[a] = y; syaw[a] = th; svx[a] = vx; svy[a] = vy; slen[a] = ln; swid[a] = wd; sc[a] = cs; ss[a] = sn;
-      s_valid[a] = v; s_sum[a] = sum; s_cnt[a] = cnt;
-      // overlap broad phase of the block: the agent's boxes all lie inside [bx0 - br, bx1 + br] x [..]
       const bool bv = bx0 <= bx1;
       s_bvalid[a] = (uint8_t)bv;
       if (bv) {
@@ -225,157 +234,151 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_fused(FusedPar
         const float ext = 0.5f * fmaxf(bx1 - bx0, by1 - by0) + br;
         if (ext <= FUSED_EXT_MAX) {
           const uint32_t bk = fused_bucket(fused_cell(0.5f * (bx0 + bx1)), fused_cell(0.5f * (by0 + by1)), (uint32_t)NBK - 1u);
-          const uint32_t old = atomicExch(&heads[bk], tag | (uint32_t)a);
-          nxt[a] = (uint16_t)((old & 0xffff0000u) == tag ? (old & 0xffffu) : FUSED_EMPTY);
+          nxt[a] = (uint16_t)atomicExch(&heads[bk], (uint32_t)a);
         } else {
-          over[atomicAdd(nover, 1)] = (uint16_t)a;
+          over[atomicAdd(s_nover, 1)] = (uint16_t)a;
         }
       }
     }
-    __syncthreads();
-    // ================= phase B: warp tasks =================
-    const int n_ctask = Ap / apt, n_task = n_ctask + nb;             // the nb overlap tasks first: they are the long ones
-    // a corner task's lane: agent slot q, validity, centre, half extents, corner offset
-    auto corner = [&](int task, int& q, bool& v, float& cx, float& cy, float& hl, float& hw, float& offx, float& offy) {
-      const int a = (task - nb) * apt + la;
-      q = ls * Aps + a;
-      v = ls < Sb && pvalid[q] != 0;
-      cx = px[q]; cy = py[q]; hl = phl[q]; hw = phw[q];
-      float ax, ay, bx, by;
-      wm_box_offsets_h(ps[q], pc[q], hl, hw, ax, ay, bx, by);
-      const float ox = (kk & 1) ? bx : ax, oy = (kk & 1) ? by : ay;
-      offx = (kk & 2) ? -ox : ox; offy = (kk & 2) ? -oy : oy;
-    };
-    // the cell header of the NEXT task's corner is requested at the end of a task, ahead of the shared
-    // counter's round trip (measured: requesting it a whole task ahead costs registers and is slower)
-    // ... together with the task's corner set-up, which the walk then finds in registers
-    int q = 0; bool v = false; float cx = 0.f, cy = 0.f, hl = 0.f, hw = 0.f, offx = 0.f, offy = 0.f;
-    auto header = [&](int task) {
-      if (task < nb || task >= n_task) return make_uint2(0u, 0u);
-      corner(task, q, v, cx, cy, hl, hw, offx, offy);
-      return wm_grid_header(gv, v, cx, cy, offx, offy);
-    };
-    auto grab = [&]() {
-      int t = 0;
-      if (lane == 0) t = atomicAdd(&s_task, 1);
-      return __shfl_sync(0xffffffffu, t, 0);
-    };
-    int task = grab();
-    uint2 hd = header(task);
-    while (task < n_task) {
-      const int task_next = grab();
-      if (task >= nb) {
-        // ---- the 4 corners of one agent (8 / S agents) at every step of the block (a4) ----
-        if (__any_sync(0xffffffffu, v)) {                               // psd of invalid slots is never read
-        float best; int bs;
-        const bool slow = wm_grid_fast_hd(gv, hd, cx, cy, offx, offy, best, bs, n_eval);
-        n_slow += slow; n_corner += v;
-        uint32_t todo = __ballot_sync(0xffffffffu, slow);
-        while (todo) {                                  // boxes with corners off the grid / in a crowded cell
-          const int g4 = (__ffs(todo) - 1) & ~3;
-          const uint32_t gm = (todo >> g4) & 15u;
-          todo &= ~(15u << g4);
-          const float acx = __shfl_sync(0xffffffffu, cx, g4), acy = __shfl_sync(0xffffffffu, cy, g4);
-          const float fax = __shfl_sync(0xffffffffu, offx, g4), fay = __shfl_sync(0xffffffffu, offy, g4);
-          const float fbx = __shfl_sync(0xffffffffu, offx, g4 + 1), fby = __shfl_sync(0xffffffffu, offy, g4 + 1);
-          const float ahl = __shfl_sync(0xffffffffu, hl, g4), ahw = __shfl_sync(0xffffffffu, hw, g4);
-          const float o4x[4] = {fax, fbx, -fax, -fbx}, o4y[4] = {fay, fby, -fay, -fby};
-          float b4[4]; int i4[4], ne = 0;
-          wm_grid_search_warp4(gv, acx, acy, o4x, o4y, sqrtf(fmaf(ahl, ahl, ahw * ahw)), b4, i4, ne);
-          if ((lane & ~3) == g4 && ((gm >> kk) & 1u)) {
-            best = kk == 0 ? b4[0] : kk == 1 ? b4[1] : kk == 2 ? b4[2] : b4[3];
-            bs = kk == 0 ? i4[0] : kk == 1 ? i4[1] : kk == 2 ? i4[2] : i4[3];
-          }
-          if (lane == 0) n_eval += ne;
-        }
-        float m = v ? wm_grid_finish(gv, cx, cy, offx, offy, best, bs) : 0.f;
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));               // D18: max over the 4 corners
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-        if (kk == 0 && v) psd[q] = m;
-        }
-      } else {
-        // ---- overlap flags of 32 agents at every step of the block (a3) ----
-        // broad phase, one lane per agent i: the pairs (i, j > i) whose block boxes meet go to the
-        // warp's list; narrow phase, one lane per (pair, step): the pair test of k_overlap
-        const int i = task * 32 + lane;
-        uint32_t* pl = s_pl + (tid >> 5) * (FUSED_PL + 1);
-        auto narrow = [&](int lo, int hi, int s) {       // lo < hi: the lower index takes the i role of k_overlap
-          const int ql = s * Aps + lo, qh = s * Aps + hi;
-          if (pvalid[ql] == 0 || pvalid[qh] == 0) return;
-          const float dx = px[qh] - px[ql], dy = py[qh] - py[ql];
-          const float hll = phl[ql], hwl = phw[ql], hlh = phl[qh], hwh = phw[qh];
-          if (wm_circles_touch(dx, dy, sqrtf(fmaf(hlh, hlh, hwh * hwh)) + sqrtf(fmaf(hll, hll, hwl * hwl))) &&
-              wm_sat_overlap(dx, dy, pc[ql], ps[ql], hll, hwl, pc[qh], ps[qh], hlh, hwh)) { pov[ql] = 1; pov[qh] = 1; }
-        };
-        if (lane == 0) pl[0] = 0;
-        __syncwarp();
-        if (s_bvalid[i] != 0) {                         // per lane: no warp-level operation inside
-          const float4 bi = s_bb[i];
-          auto test = [&](int j) {
-            if (j <= i) return;
-            const float4 bj = s_bb[j];
-            if (bi.x > bj.z || bj.x > bi.z || bi.y > bj.w || bj.y > bi.w) return;     // boxes of the block apart
-            const uint32_t slot = atomicAdd(&pl[0], 1u);
-            if (slot < (uint32_t)FUSED_PL) pl[1 + slot] = ((uint32_t)i << 16) | (uint32_t)j;
-            else for (int s = 0; s < Sb; ++s) narrow(i, j, s);                        // list full: in place
-          };
-          if (0.5f * fmaxf(bi.z - bi.x, bi.w - bi.y) <= FUSED_EXT_MAX) {
-            const int ix = fused_cell(0.5f * (bi.x + bi.z)), iy = fused_cell(0.5f * (bi.y + bi.w));
-            uint32_t j = FUSED_EMPTY;
-            for (int probe = 0; ;) {                    // one flat loop over the 9 cells and their lists
-              if (j == FUSED_EMPTY) {
-                if (probe == 9) break;
-                const uint32_t hd = heads[fused_bucket(ix + probe % 3 - 1, iy + probe / 3 - 1, (uint32_t)NBK - 1u)];
-                j = (hd & 0xffff0000u) == tag ? (hd & 0xffffu) : FUSED_EMPTY;
-                ++probe;
-                continue;
-              }
-              test((int)j);
-              j = nxt[j];
-            }
-            const int no = *nover;
-            for (int e = 0; e < no; ++e) test((int)over[e]);
-          } else {
-            for (int j = i + 1; j < A; ++j) if (s_bvalid[j] != 0) test(j);
-          }
-        }
-        __syncwarp();
-        const int np = (int)min(pl[0], (uint32_t)FUSED_PL);
-        for (int it = lane; it < np * S; it += 32) {
-          const uint32_t pr = pl[1 + it / S];
-          const int s = it & (S - 1);
-          if (s < Sb) narrow((int)(pr >> 16), (int)(pr & 0xffffu), s);
-        }
-      }
-      task = task_next; hd = header(task);
-    }
-    __syncthreads();
-    // ================= phase C: metric rows of the block (D18, D19, D10) =================
-    for (int a = tid; a < A; a += FUSED_NT) {
-      uint8_t aov = s_anyov[a], aoff = s_anyoff[a];
-      for (int s = 0; s < Sb; ++s) {
-        const int q = s * Aps + a;
-        const int64_t o = (ab + k0 + s) * A + a;
-        const bool v = pvalid[q] != 0;
-        const float m = v ? psd[q] : 0.f;
-        const uint8_t fo = pov[q], ff = (uint8_t)(v && m > 0.f);
-        if (p.out.overlap) p.out.overlap[o] = fo;
-        if (p.out.offroad_dist) p.out.offroad_dist[o] = m;
-        if (p.out.offroad) p.out.offroad[o] = ff;
-        aov |= fo; aoff |= ff;
-      }
-      s_anyov[a] = aov; s_anyoff[a] = aoff;
-    }
-    // no barrier: phase A of the next block is run by the same threads for the same agents, and the
-    // hash entries are tagged with the block number
+    // the warps that built the hash meet at a named barrier of their own
+    const int nhw = min(nb, FUSED_NT / 32);
+    asm volatile("bar.sync 1, %0;" ::"r"(nhw * 32) : "memory");
   }
-
-  // ---- epilogue: aggregates (D21) ----
-  for (int a = tid; a < A; a += FUSED_NT) {
-    const int64_t o = (int64_t)b * A + a;
-    if (p.out.any_overlap) p.out.any_overlap[o] = s_anyov[a];
-    if (p.out.any_offroad) p.out.any_offroad[o] = s_anyoff[a];
-    if (p.out.ade) p.out.ade[o] = s_cnt[a] ? (float)(s_sum[a] / s_cnt[a]) : 0.f;
+  // ================= phase B: warp tasks =================
+  // lanes of a corner task: 4 corners x S steps x (8 / S) agents
+  const int kk = lane & 3, ls = (lane >> 2) & (S - 1), la = (lane >> 2) / S, apt = 8 / S;
+  int n_eval = 0, n_slow = 0, n_corner = 0;
+  const int n_ctask = Ap / apt;
+  // ---- overlap flags of 32 agents at every step of the block (a3): the warps that built the hash ----
+  // broad phase, one lane per agent i: the pairs (i, j > i) whose block boxes meet go to the
+  // warp's list; narrow phase, one lane per (pair, step): the pair test of k_overlap
+  if (warp < nb || nb > FUSED_NT / 32) {
+    for (int task = warp; task < nb; task += FUSED_NT / 32) {
+      const int i = task * 32 + lane;
+      uint32_t* pl = s_pl + warp * (FUSED_PL + 1);
+      auto narrow = [&](int lo, int hi, int s) {       // lo < hi: the lower index takes the i role of k_overlap
+        const int ql = s * Aps + lo, qh = s * Aps + hi;
+        if (pvalid[ql] == 0 || pvalid[qh] == 0) return;
+        const float dx = px[qh] - px[ql], dy = py[qh] - py[ql];
+        const float hll = phl[ql], hwl = phw[ql], hlh = phl[qh], hwh = phw[qh];
+        if (wm_circles_touch(dx, dy, sqrtf(fmaf(hlh, hlh, hwh * hwh)) + sqrtf(fmaf(hll, hll, hwl * hwl))) &&
+            wm_sat_overlap(dx, dy, pc[ql], ps[ql], hll, hwl, pc[qh], ps[qh], hlh, hwh)) { pov[ql] = 1; pov[qh] = 1; }
+      };
+      __syncwarp();
+      if (lane == 0) pl[0] = 0;
+      __syncwarp();
+      if (s_bvalid[i] != 0) {                         // per lane: no warp-level operation inside
+        const float4 bi = s_bb[i];
+        auto test = [&](int j) {
+          if (j <= i) return;
+          const float4 bj = s_bb[j];
+          if (bi.x > bj.z || bj.x > bi.z || bi.y > bj.w || bj.y > bi.w) return;     // boxes of the block apart
+          const uint32_t slot = atomicAdd(&pl[0], 1u);
+          if (slot < (uint32_t)FUSED_PL) pl[1 + slot] = ((uint32_t)i << 16) | (uint32_t)j;
+          else for (int s = 0; s < Sb; ++s) narrow(i, j, s);                        // list full: in place
+        };
+        if (0.5f * fmaxf(bi.z - bi.x, bi.w - bi.y) <= FUSED_EXT_MAX) {
+          const int ix = fused_cell(0.5f * (bi.x + bi.z)), iy = fused_cell(0.5f * (bi.y + bi.w));
+          uint32_t j = FUSED_EMPTY;
+          for (int probe = 0; ;) {                    // one flat loop over the 9 cells and their lists
+            if (j == FUSED_EMPTY) {
+              if (probe == 9) break;
+              j = heads[fused_bucket(ix + probe % 3 - 1, iy + probe / 3 - 1, (uint32_t)NBK - 1u)];
+              ++probe;
+              continue;
+            }
+            test((int)j);
+            j = nxt[j];
+          }
+          const int no = *s_nover;
+          for (int e = 0; e < no; ++e) test((int)over[e]);
+        } else {
+          for (int j = i + 1; j < A; ++j) if (s_bvalid[j] != 0) test(j);
+        }
+      }
+      __syncwarp();
+      const int np = (int)min(pl[0], (uint32_t)FUSED_PL);
+      for (int it = lane; it < np * S; it += 32) {
+        const uint32_t pr = pl[1 + it / S];
+        const int s = it & (S - 1);
+        if (s < Sb) narrow((int)(pr >> 16), (int)(pr & 0xffffu), s);
+      }
+    }
+  }
+  // ---- the 4 corners of one agent (8 / S agents) at every step of the block (a4) ----
+  // a corner task's lane: agent slot q, validity, centre, half extents, corner offset
+  auto corner = [&](int task, int& q, bool& v, float& cx, float& cy, float& hl, float& hw, float& offx, float& offy) {
+    const int a = task * apt + la;
+    q = ls * Aps + a;
+    v = ls < Sb && pvalid[q] != 0;
+    cx = px[q]; cy = py[q]; hl = phl[q]; hw = phw[q];
+    float ax, ay, bx, by;
+    wm_box_offsets_h(ps[q], pc[q], hl, hw, ax, ay, bx, by);
+    const float ox = (kk & 1) ? bx : ax, oy = (kk & 1) ? by : ay;
+    offx = (kk & 2) ? -ox : ox; offy = (kk & 2) ? -oy : oy;
+  };
+  // the cell header of the NEXT task's corner is requested at the end of a task, ahead of the shared
+  // counter's round trip, together with the task's corner set-up, which the walk then finds in registers
+  int q = 0; bool v = false; float cx = 0.f, cy = 0.f, hl = 0.f, hw = 0.f, offx = 0.f, offy = 0.f;
+  auto header = [&](int task) {
+    if (task >= n_ctask) return make_uint2(0u, 0u);
+    corner(task, q, v, cx, cy, hl, hw, offx, offy);
+    return wm_grid_header(gv, v, cx, cy, offx, offy);
+  };
+  auto grab = [&]() {
+    int t = 0;
+    if (lane == 0) t = atomicAdd(s_task, 1);
+    return __shfl_sync(0xffffffffu, t, 0);
+  };
+  int task = grab();
+  uint2 hd = header(task);
+  while (task < n_ctask) {
+    const int task_next = grab();
+    if (__any_sync(0xffffffffu, v)) {                               // psd of invalid slots is never read
+      float best; int bs;
+      const bool slow = wm_grid_fast_hd(gv, hd, cx, cy, offx, offy, best, bs, n_eval);
+      n_slow += slow; n_corner += v;
+      uint32_t todo = __ballot_sync(0xffffffffu, slow);
+      while (todo) {                                  // boxes with corners off the grid / in a crowded cell
+        const int g4 = (__ffs(todo) - 1) & ~3;
+        const uint32_t gm = (todo >> g4) & 15u;
+        todo &= ~(15u << g4);
+        const float acx = __shfl_sync(0xffffffffu, cx, g4), acy = __shfl_sync(0xffffffffu, cy, g4);
+        const float fax = __shfl_sync(0xffffffffu, offx, g4), fay = __shfl_sync(0xffffffffu, offy, g4);
+        const float fbx = __shfl_sync(0xffffffffu, offx, g4 + 1), fby = __shfl_sync(0xffffffffu, offy, g4 + 1);
+        const float ahl = __shfl_sync(0xffffffffu, hl, g4), ahw = __shfl_sync(0xffffffffu, hw, g4);
+        const float o4x[4] = {fax, fbx, -fax, -fbx}, o4y[4] = {fay, fby, -fay, -fby};
+        float b4[4]; int i4[4], ne = 0;
+        wm_grid_search_warp4(gv, acx, acy, o4x, o4y, sqrtf(fmaf(ahl, ahl, ahw * ahw)), b4, i4, ne);
+        if ((lane & ~3) == g4 && ((gm >> kk) & 1u)) {
+          best = kk == 0 ? b4[0] : kk == 1 ? b4[1] : kk == 2 ? b4[2] : b4[3];
+          bs = kk == 0 ? i4[0] : kk == 1 ? i4[1] : kk == 2 ? i4[2] : i4[3];
+        }
+        if (lane == 0) n_eval += ne;
+      }
+      float m = v ? wm_grid_finish(gv, cx, cy, offx, offy, best, bs) : 0.f;
+      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));               // D18: max over the 4 corners
+      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+      if (kk == 0 && v) psd[q] = m;
+    }
+    task = task_next; hd = header(task);
+  }
+  __syncthreads();
+  // ================= phase C: metric rows of the block (D18, D19, D10) =================
+  for (int e = tid; e < Sb * Ap; e += FUSED_NT) {
+    const int s = AP_C ? e / AP_C : e / Ap, a = e - s * Ap;
+    if (a >= A) continue;
+    const int q = s * Aps + a;
+    const int64_t o = (ab + s) * A + a;
+    const bool vv = pvalid[q] != 0;
+    const float m = vv ? psd[q] : 0.f;
+    const uint8_t fo = pov[q], ff = (uint8_t)(vv && m > 0.f);
+    if (p.out.overlap) __stcs(p.out.overlap + o, fo);
+    if (p.out.offroad_dist) __stcs(p.out.offroad_dist + o, m);
+    if (p.out.offroad) __stcs(p.out.offroad + o, ff);
+    // aggregates: k_rollout_dyn cleared them; every writer stores the same 1
+    if (fo && p.out.any_overlap) p.out.any_overlap[(int64_t)b * A + a] = 1;
+    if (ff && p.out.any_offroad) p.out.any_offroad[(int64_t)b * A + a] = 1;
   }
   if (STATS && p.stats) {
     const unsigned ne = __reduce_add_sync(0xffffffffu, (unsigned)n_eval), ns = __reduce_add_sync(0xffffffffu, (unsigned)n_slow);
@@ -404,20 +407,29 @@ cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_t
   p.chunks = h->chunks + b0 * (cap / WM_CHUNK); p.cells = h->cells + (int64_t)b0 * WM_GRID_CELLS;
   p.pool = h->pool + (int64_t)b0 * WM_POOL_CAP; p.gridp = h->gridp + b0;
   p.stats = h->stats_on ? h->cull_stats : nullptr;
+  // ---- the trajectory ----
+  const int nba = (sim.A + DYN_NT - 1) / DYN_NT;
+  const int64_t n_dyn = (int64_t)sim.B * nba;
+  if (h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE) k_rollout_dyn<WM_DYN_INVERTIBLE_BICYCLE><<<(unsigned)n_dyn, DYN_NT, 0, s>>>(p);
+  else k_rollout_dyn<-1><<<(unsigned)n_dyn, DYN_NT, 0, s>>>(p);
+  h->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  // ---- its metrics ----
   const int Ap = (sim.A + 31) / 32 * 32;
   const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_rollout_fused<0, 0, -1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)(fused_persist_bytes(1024) + fused_slot_bytes(1024)));
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  if (Ap == 128 && p.S == 8 && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE && !p.stats)
-    k_rollout_fused<128, 8, WM_DYN_INVERTIBLE_BICYCLE, false><<<sim.B, FUSED_NT, smem, s>>>(p);     // the pair counters compiled out
-  else if (Ap == 128 && p.S == 8) k_rollout_fused<128, 8, -1, true><<<sim.B, FUSED_NT, smem, s>>>(p);
-  else if (Ap == 32 && p.S == 8) k_rollout_fused<32, 8, -1, true><<<sim.B, FUSED_NT, smem, s>>>(p);
-  else k_rollout_fused<0, 0, -1, true><<<sim.B, FUSED_NT, smem, s>>>(p);
+  const int nblk = (n_steps + p.S - 1) / p.S;
+  const int64_t n_cta = (int64_t)sim.B * nblk;
+  if (n_cta > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+  // the opt-in above 48 KB is a per-device attribute: set it at every launch (cheap), so that a second
+  // handle on another device gets it too
+  e = cudaFuncSetAttribute(k_rollout_metrics<0, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)(fused_persist_bytes(1024) + fused_slot_bytes(1024)));
+  if (e != cudaSuccess) return e;
+  if (Ap == 128 && p.S == 8 && !p.stats) k_rollout_metrics<128, 8, false><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);     // the pair counters compiled out
+  else if (Ap == 128 && p.S == 8) k_rollout_metrics<128, 8, true><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);
+  else if (Ap == 32 && p.S == 8) k_rollout_metrics<32, 8, true><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);
+  else k_rollout_metrics<0, 0, true><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);
   h->launches++;
   return cudaGetLastError();
 }

@@ -251,7 +251,7 @@ def test_rollout_graph_replay_is_deterministic_and_matches_eager(cfg1, mode):
     got_e = host(sim_e)
     for k in got_e:
         assert np.array_equal(got_e[k], outs[0][0][k], equal_nan=True)
-    per_rollout = 1 if mode == "fused" else 3 * n + 1            # kernel nodes of the graph (+ 1 reset each)
+    per_rollout = 2 if mode == "fused" else 3 * n + 1            # kernel nodes of the graph: dynamics + metrics, or 3 per step + aggregates (+ 1 reset each)
     assert wm.wm_kernel_launches(h) - l_start == 3 * (per_rollout + 1) + 1 + 4 * n
     wm.wm_destroy(h)
 
