@@ -402,14 +402,28 @@ __global__ void __launch_bounds__(128) k_offroad_grid(GridParams p) {
 
 cudaError_t wm_launch_offroad_grid(wm_handle* h, const wm_traj& sim, int t, float* sd, int64_t sd_stride_b,
                                    float* corner, uint8_t* flag, int64_t flag_stride_b, cudaStream_t s) {
-  GridParams p;
-  p.row = wm_make_row(sim, t);
-  p.A = sim.A;
-  p.segrec = h->segrec; p.segpair = h->segpair; p.segfin = h->segfin; p.chunks = h->chunks; p.cells = h->cells; p.pool = h->pool; p.gridp = h->gridp;
-  p.seg_cap = h->seg_tiles * WM_TILE_SEGS;
-  p.sd = sd; p.sd_stride_b = sd_stride_b; p.corner = corner; p.flag = flag; p.flag_stride_b = flag_stride_b;
-  p.stats = h->stats_on ? h->cull_stats : nullptr;
-  k_offroad_grid<<<dim3((sim.A + 31) / 32, sim.B), 128, 0, s>>>(p);
-  h->launches++;
-  return cudaGetLastError();
+  const int64_t cap = (int64_t)h->seg_tiles * WM_TILE_SEGS;
+  int64_t nbmax = cap > 0 ? (int64_t)0xffffffffLL / (cap * 24) : sim.B;     // pair records of a launch span < 4 GB (wm_grid.cuh)
+  if (nbmax < 1) nbmax = 1;
+  if (nbmax > 65535) nbmax = 65535;                                         // gridDim.y
+  for (int64_t c0 = 0; c0 < sim.B; c0 += nbmax) {
+    const int nb = (int)(sim.B - c0 < nbmax ? sim.B - c0 : nbmax);
+    GridParams p;
+    p.row = wm_make_row(sim, t);
+    const int64_t ro = c0 * p.row.stride_b;
+    p.row.x += ro; p.row.y += ro; p.row.yaw += ro; p.row.vel_x += ro; p.row.vel_y += ro; p.row.length += ro; p.row.width += ro; p.row.valid += ro;
+    p.A = sim.A;
+    p.segrec = h->segrec + c0 * cap * 2; p.segpair = h->segpair + c0 * (cap / 2) * 3; p.segfin = h->segfin + c0 * cap;
+    p.chunks = h->chunks + c0 * (cap / WM_CHUNK); p.cells = h->cells + c0 * WM_GRID_CELLS; p.pool = h->pool + c0 * WM_POOL_CAP;
+    p.gridp = h->gridp + c0;
+    p.seg_cap = (int)cap;
+    p.sd = sd + c0 * sd_stride_b; p.sd_stride_b = sd_stride_b; p.corner = corner ? corner + c0 * 4 * sim.A : nullptr;
+    p.flag = flag + c0 * flag_stride_b; p.flag_stride_b = flag_stride_b;
+    p.stats = h->stats_on ? h->cull_stats : nullptr;
+    k_offroad_grid<<<dim3((sim.A + 31) / 32, nb), 128, 0, s>>>(p);
+    h->launches++;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }

@@ -34,6 +34,8 @@ struct WmGridView {          // one scenario's prepared search structures
   const float4* rec;         // [nseg][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}
   const float4* fin;         // [nseg] {p0x, p0y, sx, sy}
   const float4* pair;        // [ceil(nseg/2)][3] records 2p (e) and 2p+1 (o): {p0x_e,p0x_o,p0y_e,p0y_o} {-ex_e,-ex_o,-ey_e,-ey_o} {gx_e,gx_o,gy_e,gy_o}
+  const char* pair0;         // pair records of scenario 0 of the launch; this scenario's start at byte pair_off (< 2^32: the launchers see to it)
+  uint32_t pair_off;
   const float4* chunks;      // [ceil(nseg/32)] bounding boxes {x0,y0,x1,y1}
   const uint2* cells;        // headers, 2 x 2 tiles (wm_cell_index)
   const uint32_t* pool;      // overflow runs
@@ -46,6 +48,8 @@ __device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const f
   WmGridView v;
   v.rec = segrec + (int64_t)b * seg_cap * 2;
   v.pair = segpair + (int64_t)b * (seg_cap / 2) * 3;
+  v.pair0 = (const char*)segpair;
+  v.pair_off = (uint32_t)b * (uint32_t)(seg_cap / 2) * 48u;
   v.fin = segfin + (int64_t)b * seg_cap;
   v.chunks = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
   v.cells = cells + (int64_t)b * WM_GRID_CELLS;
@@ -90,33 +94,41 @@ __device__ __forceinline__ void wm_pair_d2(const float4 P, const float4 NE, cons
 // indices are visited in ascending order with strict '<').  Padding records sit at 1e18.
 // The current run is one word, (pair << 5 | pairs left): an iteration adds 31 to it; the next two
 // runs wait in registers, further ones come from the pool.
-__device__ __forceinline__ void wm_grid_walk(const float4* __restrict__ pr, uint32_t cur, uint32_t nx1, uint32_t nx2,
+// The winner comes back as `bso` = byte offset of its pair record from the scenario's first (a multiple
+// of 48) + 1 for the odd record of the pair; wm_bso_of / wm_rec_of convert.  Inside the walk offsets
+// count from the first pair record of the LAUNCH (32 bits: one uniform base + a 32-bit lane offset).
+__device__ __forceinline__ uint32_t wm_bso_of(int rec) { return (uint32_t)(rec >> 1) * 48u + (uint32_t)(rec & 1); }
+__device__ __forceinline__ int wm_rec_of(uint32_t bso) { return (int)(2u * ((bso & ~1u) / 48u) + (bso & 1u)); }
+
+__device__ __forceinline__ void wm_grid_walk(const char* __restrict__ base, uint32_t off0, uint32_t r0, uint32_t r1, uint32_t r2,
                                              const uint32_t* __restrict__ pool, float cx, float cy, float offx, float offy,
-                                             float& best, int& bs, int& n_eval) {
+                                             float& best, uint32_t& bso, int& n_eval) {
   const wm_u64 cx2 = pk2(cx, cx), cy2 = pk2(cy, cy), ox2 = pk2(offx, offx), oy2 = pk2(offy, offy);
   int n_pool = 0;
-  if (nx2 & 0x200000u) {                                            // the third field points into the pool
-    pool += nx2 & 0x1fffffu;
+  if (r2 & 0x200000u) {                                             // the third field points into the pool
+    pool += r2 & 0x1fffffu;
     n_pool = (int)__ldg(pool);
-    nx2 = __ldg(pool + 1);
+    r2 = __ldg(pool + 1);
     pool += 2; n_pool -= 1;
   }
+  uint32_t off = off0 + (r0 >> 5) * 48u, cnt = r0 & 31u;            // the open run: byte offset of its next pair record, pairs left
   for (;;) {
-    if ((cur & 31u) == 0u) {                                        // run finished: the next one
-      if (nx1 == 0u) break;
-      cur = nx1; nx1 = nx2; nx2 = 0u;
-      if (n_pool > 0) { nx2 = __ldg(pool); ++pool; --n_pool; }
+    if (cnt == 0u) {                                                // run finished: the next one
+      if (r1 == 0u) break;
+      off = off0 + (r1 >> 5) * 48u; cnt = r1 & 31u;
+      r1 = r2; r2 = 0u;
+      if (n_pool > 0) { r2 = __ldg(pool); ++pool; --n_pool; }
     }
-    const uint32_t p = cur >> 5;
-    const float4* a = pr + (size_t)p * 3u;
+    const float4* a = (const float4*)(base + off);
     const float4 a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2);
     float d0, d1;
     wm_pair_d2(a0, a1, a2, cx2, cy2, ox2, oy2, d0, d1);
-    if (d0 < best) { best = d0; bs = (int)(2u * p); }               // ascending index, strict '<': exact ties -> lower index (D17)
-    if (d1 < best) { best = d1; bs = (int)(2u * p + 1u); }
-    cur += 31u;                                                     // pair + 1, pairs left - 1
+    if (d0 < best) { best = d0; bso = off; }                        // ascending index, strict '<': exact ties -> lower index (D17)
+    if (d1 < best) { best = d1; bso = off + 1u; }
+    off += 48u; --cnt;
     n_eval += 2;
   }
+  bso -= off0;
 }
 
 // Exact search over all chunks with bounding-box culling, by a whole warp for ONE corner (points
@@ -257,28 +269,30 @@ __device__ __forceinline__ uint2 wm_grid_header(const WmGridView& v, bool active
 }
 
 __device__ __forceinline__ bool wm_grid_fast_hd(const WmGridView& v, uint2 hd, float cx, float cy, float offx, float offy,
-                                                float& best, int& bs, int& n_eval) {
+                                                float& best, uint32_t& bso, int& n_eval) {
   best = __int_as_float(0x7f800000);
-  bs = 0;
+  bso = 0u;
   const bool slow = (hd.x & hd.y) == 0xffffffffu;
   if (slow) { hd.x = 0u; hd.y = 0u; }
   // the three 21-bit fields; bit 21 of the third = "pool offset"
   const uint32_t r0 = hd.x & 0x1fffffu, r1 = ((hd.x >> 21) | (hd.y << 11)) & 0x1fffffu, r2 = hd.y >> 10;
-  wm_grid_walk(v.pair, r0, r1, r2, v.pool, cx, cy, offx, offy, best, bs, n_eval);            // no-op without runs
+  bso = v.pair_off;
+  wm_grid_walk(v.pair0, v.pair_off, r0, r1, r2, v.pool, cx, cy, offx, offy, best, bso, n_eval);   // no-op without runs
   return slow;
 }
 
 __device__ __forceinline__ float wm_grid_finish(const WmGridView& v, float cx, float cy, float offx, float offy, float best,
-                                                int bs) {
+                                                uint32_t bso) {
   if (v.g.nseg <= 0) return -FLT_MAX;                                      // D20
   // e x (q - p0) > 0 is the left side of the oriented segment = on-road (D16).  p0 and e come from
   // the winner's pair record, which the walk has just pulled into L1 (no third dependent miss);
   // only a zero-length segment needs its stored direction from the finish record (D16 / D29).
-  const float4 P = __ldg(v.pair + 3 * (bs >> 1)), NE = __ldg(v.pair + 3 * (bs >> 1) + 1);
-  const bool odd = (bs & 1) != 0;
+  const float4* a = (const float4*)((const char*)v.pair + (bso & ~1u));
+  const float4 P = __ldg(a), NE = __ldg(a + 1);
+  const bool odd = (bso & 1u) != 0u;
   const float p0x = odd ? P.y : P.x, p0y = odd ? P.w : P.z;
   float sx = -(odd ? NE.y : NE.x), sy = -(odd ? NE.w : NE.z);
-  if (sx == 0.f && sy == 0.f) { const float4 f = __ldg(v.fin + bs); sx = f.z; sy = f.w; }
+  if (sx == 0.f && sy == 0.f) { const float4 f = __ldg(v.fin + wm_rec_of(bso)); sx = f.z; sy = f.w; }
   const float wx = __fadd_rn(__fsub_rn(cx, p0x), offx), wy = __fadd_rn(__fsub_rn(cy, p0y), offy);
   const float side = __fmaf_rn(sx, wy, -__fmul_rn(sy, wx));
   const float d = sqrtf(best);
@@ -292,8 +306,8 @@ __device__ __forceinline__ float wm_grid_corner_sd(const WmGridView& v, bool act
                                                    float offy, int& n_eval, bool& fell_back) {
   const int lane = threadIdx.x & 31;
   float best;
-  int bs;
-  const bool slow = wm_grid_fast_hd(v, wm_grid_header(v, active, cx, cy, offx, offy), cx, cy, offx, offy, best, bs, n_eval);
+  uint32_t bso;
+  const bool slow = wm_grid_fast_hd(v, wm_grid_header(v, active, cx, cy, offx, offy), cx, cy, offx, offy, best, bso, n_eval);
   fell_back = slow;
   uint32_t todo = __ballot_sync(0xffffffffu, slow);
   while (todo) {
@@ -303,8 +317,8 @@ __device__ __forceinline__ float wm_grid_corner_sd(const WmGridView& v, bool act
     wm_grid_search_warp(v, __shfl_sync(0xffffffffu, cx, l), __shfl_sync(0xffffffffu, cy, l),
                         __shfl_sync(0xffffffffu, offx, l), __shfl_sync(0xffffffffu, offy, l), b2, s2, ne);
     ne = __shfl_sync(0xffffffffu, ne, 0);
-    if (lane == l) { best = b2; bs = s2; n_eval += ne; }
+    if (lane == l) { best = b2; bso = wm_bso_of(s2); n_eval += ne; }
   }
   if (!active) return 0.f;
-  return wm_grid_finish(v, cx, cy, offx, offy, best, bs);
+  return wm_grid_finish(v, cx, cy, offx, offy, best, bso);
 }

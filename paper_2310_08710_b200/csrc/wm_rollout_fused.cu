@@ -325,18 +325,17 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_metrics(FusedP
     corner(task, q, v, cx, cy, hl, hw, offx, offy);
     return wm_grid_header(gv, v, cx, cy, offx, offy);
   };
-  auto grab = [&]() {
-    int t = 0;
-    if (lane == 0) t = atomicAdd(s_task, 1);
-    return __shfl_sync(0xffffffffu, t, 0);
-  };
-  int task = grab();
+  // the shared counter is bumped by lane 0 at the START of a task and its answer is only read at the end:
+  // the atomic's round trip hides under the walk
+  int tn = 0;
+  if (lane == 0) tn = atomicAdd(s_task, 1);
+  int task = __shfl_sync(0xffffffffu, tn, 0);
   uint2 hd = header(task);
   while (task < n_ctask) {
-    const int task_next = grab();
+    if (lane == 0) tn = atomicAdd(s_task, 1);
     if (__any_sync(0xffffffffu, v)) {                               // psd of invalid slots is never read
-      float best; int bs;
-      const bool slow = wm_grid_fast_hd(gv, hd, cx, cy, offx, offy, best, bs, n_eval);
+      float best; uint32_t bso;
+      const bool slow = wm_grid_fast_hd(gv, hd, cx, cy, offx, offy, best, bso, n_eval);
       n_slow += slow; n_corner += v;
       uint32_t todo = __ballot_sync(0xffffffffu, slow);
       while (todo) {                                  // boxes with corners off the grid / in a crowded cell
@@ -352,16 +351,16 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_metrics(FusedP
         wm_grid_search_warp4(gv, acx, acy, o4x, o4y, sqrtf(fmaf(ahl, ahl, ahw * ahw)), b4, i4, ne);
         if ((lane & ~3) == g4 && ((gm >> kk) & 1u)) {
           best = kk == 0 ? b4[0] : kk == 1 ? b4[1] : kk == 2 ? b4[2] : b4[3];
-          bs = kk == 0 ? i4[0] : kk == 1 ? i4[1] : kk == 2 ? i4[2] : i4[3];
+          bso = wm_bso_of(kk == 0 ? i4[0] : kk == 1 ? i4[1] : kk == 2 ? i4[2] : i4[3]);
         }
         if (lane == 0) n_eval += ne;
       }
-      float m = v ? wm_grid_finish(gv, cx, cy, offx, offy, best, bs) : 0.f;
+      float m = v ? wm_grid_finish(gv, cx, cy, offx, offy, best, bso) : 0.f;
       m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));               // D18: max over the 4 corners
       m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
       if (kk == 0 && v) psd[q] = m;
     }
-    task = task_next; hd = header(task);
+    task = __shfl_sync(0xffffffffu, tn, 0); hd = header(task);
   }
   __syncthreads();
   // ================= phase C: metric rows of the block (D18, D19, D10) =================
@@ -392,9 +391,48 @@ __global__ void __launch_bounds__(FUSED_NT, FUSED_MINB) k_rollout_metrics(FusedP
   }
 }
 
+// scenarios per launch such that the pair records of a launch span less than 4 GB (32-bit offsets in the walk)
+static inline int fused_launch_batch(int64_t seg_cap) {
+  const int64_t per = seg_cap * 24;                   // bytes of pair records per scenario
+  int64_t n = per > 0 ? (int64_t)0xffffffffLL / per : 1 << 30;
+  if (n < 1) n = 1;
+  return (int)(n > (1 << 30) ? (1 << 30) : n);
+}
+
+static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
+                                     const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
+                                     int b0, cudaStream_t s);
+
 cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
                                     const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
                                     int b0, cudaStream_t s) {
+  const int nbmax = fused_launch_batch((int64_t)h->seg_tiles * WM_TILE_SEGS);
+  if (sim.B <= nbmax) return fused_launch_part(h, log, sim, t0, n_steps, actions, action_valid, out, b0, s);
+  const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  for (int c0 = 0; c0 < sim.B; c0 += nbmax) {          // very large batches: scenario ranges, one launch pair each
+    const int nb = sim.B - c0 < nbmax ? sim.B - c0 : nbmax;
+    const int64_t oT = (int64_t)c0 * sim.T * sim.A, oW = (int64_t)c0 * n_steps * sim.A, oA = (int64_t)c0 * sim.A;
+    wm_traj cl = log, cs = sim;
+    cl.B = nb; cs.B = nb;
+    cl.x += oT; cl.y += oT; cl.yaw += oT; cl.vel_x += oT; cl.vel_y += oT; cl.length += oT; cl.width += oT; cl.valid += oT;
+    cs.x += oT; cs.y += oT; cs.yaw += oT; cs.vel_x += oT; cs.vel_y += oT; cs.length += oT; cs.width += oT; cs.valid += oT;
+    wm_rollout_out co = out;
+    if (co.overlap) co.overlap += oW;
+    if (co.offroad) co.offroad += oW;
+    if (co.offroad_dist) co.offroad_dist += oW;
+    if (co.log_div) co.log_div += oW;
+    if (co.any_overlap) co.any_overlap += oA;
+    if (co.any_offroad) co.any_offroad += oA;
+    if (co.ade) co.ade += oA;
+    const cudaError_t e = fused_launch_part(h, cl, cs, t0, n_steps, actions + oW * C, action_valid + oW, co, b0 + c0, s);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
+                                     const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
+                                     int b0, cudaStream_t s) {
   FusedParams p;
   p.log = log; p.sim = sim; p.t0 = t0; p.n_steps = n_steps;
   p.C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
