@@ -153,11 +153,12 @@ def observe_history(sim, t, H=11):
     return dict(hist=hist, hist_valid=hv)
 
 
-def observe_topk(sim, rg, t, k):
+def observe_topk(sim, rg, t, k, order=0):
+    """order 0: ascending roadgraph index (D24); 1: ascending (distance key, index) (D44)."""
     ss, (B, T, A) = _traj(sim); rs, _ = _rg(rg)
     idx = np.empty((B, A, k), np.int32); feat = np.empty((B, A, 4, k), np.float32)
     typ = np.empty((B, A, k), np.int32); kth = np.empty((B, A), np.float32)
-    lib().orc_observe_topk(C.byref(ss), C.byref(rs), C.c_int32(t), C.c_int32(k), _p(idx), _p(feat),
+    lib().orc_observe_topk(C.byref(ss), C.byref(rs), C.c_int32(t), C.c_int32(k), C.c_int32(order), _p(idx), _p(feat),
                            _p(typ), _p(kth))
     return dict(rg_index=idx, rg_feat=feat, rg_type=typ, kth_key=kth)
 
@@ -256,3 +257,51 @@ def idm_step(sim, t, paths, idm_valid, dt=0.1, **params):
     acc = np.empty((B, A), np.float32); lead = np.empty((B, A), np.int32)
     lib().orc_idm_step(C.byref(ss), C.c_int32(t), C.byref(pa), _p(idm_valid), C.byref(ps), C.c_double(dt), _p(acc), _p(lead))
     return dict(accel=acc, lead=lead)
+
+
+def rollout_vjp(sim, t0, n_steps, dynamics, actions, action_valid, g_rows, dt=0.1, max_accel=6.0, max_curvature=0.3):
+    """O14: reverse-mode derivative of the rollout's dynamics (L252).  g_rows [B][n_steps][5][A] float32 = cotangents
+    of rows t0+1..t0+n_steps (x, y, yaw, vel_x, vel_y).  Returns g_actions [B][n_steps][C][A], g_state0 [B][5][A]."""
+    ss, (B, T, A) = _traj(sim)
+    Cn = 2 if dynamics == DYN_BICYCLE else 3
+    _check(actions, np.float32, (B, n_steps, Cn, A)); _check(action_valid, np.uint8, (B, n_steps, A))
+    _check(g_rows, np.float32, (B, n_steps, 5, A))
+    ga = np.empty((B, n_steps, Cn, A), np.float32); g0 = np.empty((B, 5, A), np.float32)
+    lib().orc_rollout_vjp(C.byref(ss), C.c_int32(t0), C.c_int32(n_steps), C.c_int32(dynamics), C.c_double(dt), C.c_double(max_accel),
+                          C.c_double(max_curvature), _p(actions), _p(action_valid), _p(g_rows), _p(ga), _p(g0))
+    return dict(g_actions=ga, g_state0=g0)
+
+
+class _Grid(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3), ("lo", C.c_float * 3), ("hi", C.c_float * 3)]
+
+
+def _grid(n, lo, hi):
+    g = _Grid()
+    for c in range(3):
+        g.n[c] = int(n[c]) if c < len(n) else 1
+        g.lo[c] = float(lo[c]) if c < len(lo) else 0.0
+        g.hi[c] = float(hi[c]) if c < len(hi) else 0.0
+    return g
+
+
+def discretize_actions(action, n, lo, hi, valid=None):
+    """O15 (L204, D42): action [..., C, A] float32 -> joint bin index [..., A] int32 and the de-quantised action."""
+    Cn, A = action.shape[-2:]
+    N = int(np.prod(action.shape[:-2], dtype=np.int64))
+    act = np.ascontiguousarray(action, np.float32)
+    idx = np.empty(action.shape[:-2] + (A,), np.int32); deq = np.empty_like(act)
+    v = None if valid is None else np.ascontiguousarray(valid, np.uint8)
+    g = _grid(n, lo, hi)
+    lib().orc_discretize_actions(C.byref(g), C.c_int32(Cn), C.c_int64(N), C.c_int32(A), _p(act), _p(v), _p(idx), _p(deq))
+    return dict(index=idx, action=deq)
+
+
+def actions_from_index(index, Cn, n, lo, hi):
+    A = index.shape[-1]
+    N = int(np.prod(index.shape[:-1], dtype=np.int64))
+    idx = np.ascontiguousarray(index, np.int32)
+    act = np.empty(index.shape[:-1] + (Cn, A), np.float32)
+    g = _grid(n, lo, hi)
+    lib().orc_actions_from_index(C.byref(g), C.c_int32(Cn), C.c_int64(N), C.c_int32(A), _p(idx), _p(act))
+    return act

@@ -366,7 +366,8 @@ void orc_observe_history(const orc_traj* sim, int32_t t, int32_t H, float* hist,
 // -------------------------------------------------------------------------------------
 // O7 observation, roadgraph part ("sub-samples the roadgraph via distance";
 // D23-D25): for each ego valid at t, the k valid roadgraph points nearest the ego centre,
-// ties -> lower index, emitted in ascending index order, padded with -1.
+// ties -> lower index, emitted in ascending index order (order = 0, D24) or by ascending
+// (distance key, index) — the sorted-by-distance variant of SURVEY 8(f)(4), D44 (order = 1) —, padded with -1.
 // The integer decision (which points) is taken in float32, the kernel's precision:
 //   key = fma(dy, dy, dx*dx) with dx = fl(px-ex), dy = fl(py-ey), round-to-nearest
 // (DESIGN.md R-topk).  Features are computed in double: p' = R(-yaw_e)(p-p_e),
@@ -374,7 +375,7 @@ void orc_observe_history(const orc_traj* sim, int32_t t, int32_t H, float* hist,
 // (NaN if fewer than k valid points) for the band report.
 // rg_index [B][E][k], rg_feat [B][E][4][k] (x,y,dir_x,dir_y), rg_type [B][E][k].
 // -------------------------------------------------------------------------------------
-void orc_observe_topk(const orc_traj* sim, const orc_roadgraph* rg, int32_t t, int32_t k,
+void orc_observe_topk(const orc_traj* sim, const orc_roadgraph* rg, int32_t t, int32_t k, int32_t order,
                       int32_t* rg_index, float* rg_feat, int32_t* rg_type, float* kth_key) {
   const int B = sim->B, A = sim->A, R = rg->R;
 #pragma omp parallel for schedule(dynamic, 1)
@@ -401,7 +402,7 @@ void orc_observe_topk(const orc_traj* sim, const orc_roadgraph* rg, int32_t t, i
       const int n = std::min<int>(k, (int)keys.size());
       sel.clear();
       for (int j = 0; j < n; ++j) sel.push_back(keys[j].second);
-      std::sort(sel.begin(), sel.end());        // ascending index (D24)
+      if (order == 0) std::sort(sel.begin(), sel.end());        // ascending index (D24); order 1: by (distance key, index), D44
       if (kth_key && (int)keys.size() >= k && k > 0) kth_key[(size_t)b * A + e] = keys[k - 1].first;
       const double ex = exf, ey = eyf, eth = sim->yaw[rt + e];
       const double c = std::cos(eth), s = std::sin(eth);
@@ -747,6 +748,139 @@ void orc_idm_step(orc_traj* sim, int32_t t, const orc_paths* pa, const uint8_t* 
       sim->length[r1] = sim->length[r0]; sim->width[r1] = sim->width[r0]; sim->valid[r1] = 1;
       if (accel_out) accel_out[o] = (float)acc;
       if (lead_out) lead_out[o] = lead;
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O14 backward pass of the dynamics ("the entire simulation can be assembled within a
+// single ... computation graph" / differentiable simulation): the vector-Jacobian
+// product of O1 / O2, chained in reverse over the rows of a rollout.  Plain reverse-mode
+// differentiation of Eq. 2 (L339-L350) and Eq. 1 (L324-L333) written out term by term, in double,
+// evaluated on the STORED float32 rows (state at row t0+k, actions of step k).  Readings (DESIGN D43):
+//   * a playback slot (use_dyn = action_valid && sim.valid[t0+k] false, D8) takes its successor from
+//     the log: zero gradient to the state and to the action;
+//   * clipping (D7): d clip(a)/da = 1 for |a| <= limit, 0 beyond it;
+//   * v = sqrt(vx^2 + vy^2): dv/dvx = vx / v, and 0 at v = 0;
+//   * Eq. 1's v' = (x' - x)/dt differentiates as written (the float32 rounding of x', D28, is the
+//     identity for the derivative): for the delta models v' does not depend on x.
+// g_rows [B][n_steps][5][A]: cotangents of the loss w.r.t. (x, y, yaw, vel_x, vel_y) of rows
+// t0+1 .. t0+n_steps.  Outputs: g_actions [B][n_steps][C][A], g_state0 [B][5][A] (w.r.t. row t0).
+// -------------------------------------------------------------------------------------
+void orc_rollout_vjp(const orc_traj* sim, int32_t t0, int32_t n_steps, int32_t dynamics, double dt, double max_accel,
+                     double max_curvature, const float* actions, const uint8_t* action_valid, const float* g_rows,
+                     float* g_actions, float* g_state0) {
+  const int B = sim->B, A = sim->A;
+  const int C = dynamics == ORC_DYN_BICYCLE ? 2 : 3;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < B; ++b)
+    for (int a = 0; a < A; ++a) {
+      double gx = 0, gy = 0, gth = 0, gvx = 0, gvy = 0;            // cotangent of row t0+k+1, carried backwards
+      for (int k = n_steps - 1; k >= 0; --k) {
+        const size_t gr = (((size_t)b * n_steps + k) * 5) * A + a;
+        gx += g_rows[gr]; gy += g_rows[gr + A]; gth += g_rows[gr + 2 * (size_t)A];
+        gvx += g_rows[gr + 3 * (size_t)A]; gvy += g_rows[gr + 4 * (size_t)A];
+        const size_t r0 = row(sim, b, t0 + k) + a;
+        const size_t oa = (((size_t)b * n_steps + k) * C) * A + a;
+        const bool use_dyn = action_valid[((size_t)b * n_steps + k) * A + a] != 0 && sim->valid[r0] != 0;
+        for (int c = 0; c < C; ++c) g_actions[oa + (size_t)c * A] = 0.f;
+        if (!use_dyn) { gx = gy = gth = gvx = gvy = 0; continue; }  // the successor came from the log
+        const double th = sim->yaw[r0], vx = sim->vel_x[r0], vy = sim->vel_y[r0];
+        double nx_, ny_, nth, nvx, nvy;                             // cotangent of row t0+k
+        if (dynamics == ORC_DYN_BICYCLE) {
+          double acc = actions[oa], kappa = actions[oa + A];
+          double da = 1.0, dk = 1.0;
+          if (max_accel > 0) { if (std::fabs(acc) > max_accel) da = 0.0; acc = std::min(std::max(acc, -max_accel), max_accel); }
+          if (max_curvature > 0) { if (std::fabs(kappa) > max_curvature) dk = 0.0; kappa = std::min(std::max(kappa, -max_curvature), max_curvature); }
+          const double v = std::sqrt(vx * vx + vy * vy);
+          const double thn = th + kappa * (v * dt + 0.5 * acc * dt * dt);   // L343
+          const double vn = v + acc * dt;                                    // L345
+          const double c0 = std::cos(th), s0 = std::sin(th), c1 = std::cos(thn), s1 = std::sin(thn);
+          // vx' = vn cos(thn), vy' = vn sin(thn)                           (L347, L349)
+          const double gvn = gvx * c1 + gvy * s1;
+          const double gthn = gth + vn * (-gvx * s1 + gvy * c1);
+          // thn = th + kappa (v dt + a dt^2/2)
+          const double gv = gvn + gthn * kappa * dt;
+          const double gk = gthn * (v * dt + 0.5 * acc * dt * dt);
+          // x' = x + vx dt + a cos(th) dt^2/2, y' = y + vy dt + a sin(th) dt^2/2   (L339, L341)
+          const double ga = gvn * dt + gthn * kappa * 0.5 * dt * dt + 0.5 * dt * dt * (gx * c0 + gy * s0);
+          nth = gthn + 0.5 * acc * dt * dt * (-gx * s0 + gy * c0);
+          nx_ = gx; ny_ = gy;
+          const double ux = v > 0 ? vx / v : 0.0, uy = v > 0 ? vy / v : 0.0;
+          nvx = gx * dt + gv * ux; nvy = gy * dt + gv * uy;
+          g_actions[oa] = (float)(ga * da); g_actions[oa + A] = (float)(gk * dk);
+        } else {
+          const double dx = actions[oa], dy = actions[oa + A];
+          const bool glob = dynamics == ORC_DYN_DELTA_GLOBAL;
+          const double c = glob ? 1.0 : std::cos(th), s = glob ? 0.0 : std::sin(th);
+          // x' = x + c dx - s dy, y' = y + s dx + c dy, th' = th + dyaw, vx' = (x' - x)/dt, vy' = (y' - y)/dt
+          const double hx = gx + gvx / dt, hy = gy + gvy / dt;      // cotangents of the world-frame delta
+          g_actions[oa] = (float)(hx * c + hy * s);
+          g_actions[oa + A] = (float)(-hx * s + hy * c);
+          g_actions[oa + 2 * (size_t)A] = (float)gth;
+          nx_ = gx; ny_ = gy;
+          nth = gth + (glob ? 0.0 : hx * (-s * dx - c * dy) + hy * (c * dx - s * dy));
+          nvx = 0.0; nvy = 0.0;
+        }
+        gx = nx_; gy = ny_; gth = nth; gvx = nvx; gvy = nvy;
+      }
+      const size_t o = ((size_t)b * 5) * A + a;
+      g_state0[o] = (float)gx; g_state0[o + A] = (float)gy; g_state0[o + 2 * (size_t)A] = (float)gth;
+      g_state0[o + 3 * (size_t)A] = (float)gvx; g_state0[o + 4 * (size_t)A] = (float)gvy;
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O15 discretised action spaces ("For discrete action spaces, the inverse is computed by
+// discretizing the continuous inverse"; the Bicycle-Discrete / Delta-Discrete spaces of L373).  The
+// paper prints no grids, so they are arguments (DESIGN D42): channel c has n[c] >= 1 values
+// lo[c] + i (hi[c] - lo[c]) / (n[c] - 1), i = 0 .. n[c]-1 (n = 1: the single value lo).  A continuous
+// value maps to the NEAREST grid value, ties to the even bin, beyond the range to the end bin.  The
+// bin decision is taken in float32 (the kernel's precision: a floating-point value that decides an
+// integer): i = clamp(rint((v - lo) * inv_step), 0, n-1) with inv_step = (n-1)/(hi-lo) rounded to
+// float32 and every operation rounded to float32.  The joint index is row-major over the channels,
+// index = (i_0 n_1 + i_1) n_2 + i_2.  The de-quantised value is lo + i step in double, rounded once.
+// action [N][C][A] -> index [N][A] (N = B n_steps rows), dequant [N][C][A] (may be NULL).
+// -------------------------------------------------------------------------------------
+struct orc_action_grid { int32_t n[3]; float lo[3], hi[3]; };
+
+void orc_discretize_actions(const orc_action_grid* g, int32_t C, int64_t N, int32_t A, const float* action, const uint8_t* valid,
+                            int32_t* index, float* dequant) {
+  for (int64_t r = 0; r < N; ++r)
+    for (int a = 0; a < A; ++a) {
+      int32_t idx = 0;
+      const bool v = valid == nullptr || valid[r * A + a] != 0;
+      for (int c = 0; c < C; ++c) {
+        const size_t o = ((size_t)r * C + c) * A + a;
+        int i = 0;
+        if (v && g->n[c] > 1) {
+          const float inv_step = (float)(g->n[c] - 1) / (g->hi[c] - g->lo[c]);
+          const float q = std::nearbyintf((action[o] - g->lo[c]) * inv_step);        // round half to even, float32
+          i = q <= 0.f ? 0 : q >= (float)(g->n[c] - 1) ? g->n[c] - 1 : (int)q;       // NaN -> bin 0
+          if (!(q == q)) i = 0;
+        }
+        idx = idx * g->n[c] + i;
+        if (dequant) {
+          const double step = g->n[c] > 1 ? ((double)g->hi[c] - (double)g->lo[c]) / (double)(g->n[c] - 1) : 0.0;
+          dequant[o] = v ? (float)((double)g->lo[c] + (double)i * step) : 0.f;
+        }
+      }
+      index[r * A + a] = v ? idx : -1;
+    }
+}
+
+// joint index -> continuous action (the de-quantised grid value; index < 0 -> 0)
+void orc_actions_from_index(const orc_action_grid* g, int32_t C, int64_t N, int32_t A, const int32_t* index, float* action) {
+  for (int64_t r = 0; r < N; ++r)
+    for (int a = 0; a < A; ++a) {
+      int32_t idx = index[r * A + a];
+      for (int c = C - 1; c >= 0; --c) {
+        const size_t o = ((size_t)r * C + c) * A + a;
+        if (idx < 0) { action[o] = 0.f; continue; }
+        const int i = idx % g->n[c];
+        idx /= g->n[c];
+        const double step = g->n[c] > 1 ? ((double)g->hi[c] - (double)g->lo[c]) / (double)(g->n[c] - 1) : 0.0;
+        action[o] = (float)((double)g->lo[c] + (double)i * step);
+      }
     }
 }
 
