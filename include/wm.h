@@ -70,6 +70,7 @@ typedef struct {
   int32_t topk;         /* 1000 nearest roadgraph points per ego (D23) */
   int32_t offroad_mode; /* WM_OFFROAD_*: how wm_metrics_offroad / wm_rollout search the segments */
   int32_t rollout_mode; /* WM_ROLLOUT_*: how wm_rollout runs the n_steps */
+  int32_t topk_order;   /* WM_TOPK_*: order of the k selected roadgraph points in wm_observe's outputs */
 } wm_config;
 
 /* Both modes find the nearest segment exactly and use the same per-pair arithmetic; they return the
@@ -88,6 +89,11 @@ enum { WM_OFFROAD_CULLED = 0, WM_OFFROAD_BRUTE_FORCE = 1 };
  * STEPWISE: n_steps x {k_step, k_overlap, k_offroad} + k_aggregate, the kernels of the single-step
  *   entry points. */
 enum { WM_ROLLOUT_FUSED = 0, WM_ROLLOUT_STEPWISE = 1 };
+
+/* Order of the top-k outputs of wm_observe (the selected SET is the same).  BY_INDEX (default, D24): ascending
+ * roadgraph index.  BY_DISTANCE (D44): ascending distance to the ego centre (the float32 selection key),
+ * ties -> lower index: "sub-samples the roadgraph via distance" (L82) as a nearest-first list. */
+enum { WM_TOPK_BY_INDEX = 0, WM_TOPK_BY_DISTANCE = 1 };
 
 typedef struct wm_handle wm_handle; /* opaque */
 
@@ -173,7 +179,8 @@ int wm_log_divergence(wm_handle* h, const wm_traj* log, const wm_traj* sim, int3
  *    yaw' = wrap(yaw - yaw_e) in [-pi, pi), v' = R(-yaw_e) v, length, width (D22);
  *  - rg_index [B][A_ego][k], rg_feat [B][A_ego][4][k] (x', y', dir_x', dir_y'), rg_type
  *    [B][A_ego][k]: the k = topk valid roadgraph points nearest the ego centre, ties to the
- *    lower index, emitted in ascending index order, padded with -1 / 0 (D23-D25).  The
+ *    lower index, emitted in ascending index order (or nearest first: wm_config.topk_order), padded
+ *    with -1 / 0 (D23-D25).  The
  *    selection key is the float32 value fma(dy, dy, dx*dx), dx = px - ex, dy = py - ey.
  * Either group of outputs may be skipped by passing NULL for all of its pointers.
  * The top-k part needs wm_prepare (WM_ERR_STATE otherwise). Requires t >= history-1.
@@ -207,6 +214,45 @@ int wm_expert_actions(wm_handle* h, const wm_traj* tr, int32_t t, int32_t n_step
  */
 int wm_metrics_kinematic(wm_handle* h, const wm_traj* sim, int32_t t, int32_t n_steps, float* accel,
                          float* curvature, uint8_t* flag, void* stream);
+
+/*
+ * Discretised action spaces (L204: "For discrete action spaces, the inverse is computed by discretizing
+ * the continuous inverse"; the Bicycle-Discrete / Delta-Discrete spaces of L373).  The paper prints no
+ * grids, so they are arguments (D42): channel c has n[c] >= 1 values lo[c] + i (hi[c] - lo[c]) / (n[c] - 1),
+ * i = 0 .. n[c]-1.  A continuous value maps to the nearest grid value (ties -> the even bin, values
+ * beyond the range -> the end bin); the bin is decided in float32: rint((v - lo) * fl((n-1)/(hi-lo))).
+ * The joint index is row-major over the C channels: (i_0 n_1 + i_1) n_2 + i_2.  Channels beyond C are ignored.
+ */
+typedef struct { int32_t n[3]; float lo[3], hi[3]; } wm_action_grid;
+
+/* action [N][C][A] (N rows, e.g. B*n_steps; C = 2 or 3 as for the handle's dynamics) -> index [N][A]
+ * (-1 where valid == 0; valid [N][A] may be NULL = all valid) and dequant [N][C][A], the grid values
+ * (0 where not valid; may be NULL; may alias `action`). */
+int wm_discretize_actions(wm_handle* h, const wm_action_grid* grid, int64_t N, int32_t A, const float* action,
+                          const uint8_t* valid, int32_t* index, float* dequant, void* stream);
+/* index [N][A] -> action [N][C][A]: the grid values (index < 0 -> 0), ready for wm_step / wm_rollout. */
+int wm_actions_from_index(wm_handle* h, const wm_action_grid* grid, int64_t N, int32_t A, const int32_t* index,
+                          float* action, void* stream);
+/* Discrete expert (L204): wm_expert_actions followed by wm_discretize_actions in place.  action
+ * [B][n_steps][C][A] receives the de-quantised expert action, index [B][n_steps][A] its joint bin. */
+int wm_expert_actions_discrete(wm_handle* h, const wm_traj* tr, int32_t t, int32_t n_steps, const wm_action_grid* grid,
+                               int32_t* index, float* action, uint8_t* action_valid, void* stream);
+
+/*
+ * Backward pass of the dynamics for differentiable rollouts (L252: "the entire simulation can be assembled
+ * within a single ... computation graph"; Eq. 2, Eq. 1): the vector-Jacobian product of
+ * the n_steps transitions that produced rows t0+1 .. t0+n_steps of `sim` from row t0 with `actions`.
+ * g_rows [B][n_steps][5][A]: cotangents of a loss w.r.t. (x, y, yaw, vel_x, vel_y) of those rows.
+ * g_actions [B][n_steps][C][A]: its gradient w.r.t. the actions; g_state0 [B][5][A] (may be NULL): w.r.t.
+ * row t0.  A log-playback slot (D8) passes no gradient to its action or to earlier rows; an action
+ * beyond the clip limits (D7) has zero gradient; dv/dv_x = 0 at v = 0 (D43).  Reads the stored rows:
+ * call it after wm_rollout / wm_step with the same actions.  wm_step_vjp is the n_steps = 1 case
+ * (g_next [B][5][A], g_action [B][C][A]).
+ */
+int wm_rollout_vjp(wm_handle* h, const wm_traj* sim, int32_t t0, int32_t n_steps, const float* actions,
+                   const uint8_t* action_valid, const float* g_rows, float* g_actions, float* g_state0, void* stream);
+int wm_step_vjp(wm_handle* h, const wm_traj* sim, int32_t t, const float* action, const uint8_t* action_valid,
+                const float* g_next, float* g_state, float* g_action, void* stream);
 
 /* One on-route path per agent (L84, L96): points [B][A][P] with the distance along the path from
  * its start (arc_len, an input) and validity.  DEVICE pointers, caller-owned. */

@@ -9,7 +9,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libwm_b200.so")
-SOURCES = ["wm_api.cu", "wm_dynamics.cu", "wm_overlap.cu", "wm_offroad.cu", "wm_grid.cu", "wm_rollout_fused.cu", "wm_observe.cu"]
+SOURCES = ["wm_api.cu", "wm_dynamics.cu", "wm_overlap.cu", "wm_offroad.cu", "wm_grid.cu", "wm_rollout_fused.cu", "wm_observe.cu", "wm_variants.cu"]
 HEADERS = [os.path.join(CSRC, "wm_internal.cuh"), os.path.join(CSRC, "wm_grid.cuh"), os.path.join(CSRC, "wm_device.cuh"), os.path.join(_HERE, "..", "include", "wm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]

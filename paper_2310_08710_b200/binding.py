@@ -16,6 +16,7 @@ WM_DYN_INVERTIBLE_BICYCLE, WM_DYN_DELTA_LOCAL, WM_DYN_DELTA_GLOBAL = 0, 1, 2
 WM_TYPE_LANE, WM_TYPE_ROAD_EDGE = 1, 2
 WM_OFFROAD_CULLED, WM_OFFROAD_BRUTE_FORCE = 0, 1
 WM_ROLLOUT_FUSED, WM_ROLLOUT_STEPWISE = 0, 1
+WM_TOPK_BY_INDEX, WM_TOPK_BY_DISTANCE = 0, 1
 _ERR = {-1: "WM_ERR_ARG", -2: "WM_ERR_CUDA", -3: "WM_ERR_UNSUPPORTED", -4: "WM_ERR_STATE"}
 
 TRAJ_F = ("x", "y", "yaw", "vel_x", "vel_y", "length", "width")
@@ -23,7 +24,8 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_idm_step", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable")
+           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_idm_step", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable",
+           "wm_discretize_actions", "wm_actions_from_index", "wm_expert_actions_discrete", "wm_rollout_vjp", "wm_step_vjp")
 
 
 class wm_traj(C.Structure):
@@ -39,7 +41,7 @@ class wm_roadgraph(C.Structure):
 class wm_config(C.Structure):
     _fields_ = [("dynamics", C.c_int32), ("dt", C.c_float), ("max_accel", C.c_float),
                 ("max_curvature", C.c_float), ("history", C.c_int32), ("topk", C.c_int32),
-                ("offroad_mode", C.c_int32), ("rollout_mode", C.c_int32)]
+                ("offroad_mode", C.c_int32), ("rollout_mode", C.c_int32), ("topk_order", C.c_int32)]
 
 
 class wm_rollout_out(C.Structure):
@@ -126,9 +128,9 @@ def wm_version():
 
 
 def wm_create(dynamics=WM_DYN_INVERTIBLE_BICYCLE, dt=0.1, max_accel=6.0, max_curvature=0.3, history=11, topk=1000,
-              offroad_mode=WM_OFFROAD_CULLED, rollout_mode=WM_ROLLOUT_FUSED):
+              offroad_mode=WM_OFFROAD_CULLED, rollout_mode=WM_ROLLOUT_FUSED, topk_order=WM_TOPK_BY_INDEX):
     h = C.c_void_p()
-    cfg = wm_config(dynamics, dt, max_accel, max_curvature, history, topk, offroad_mode, rollout_mode)
+    cfg = wm_config(dynamics, dt, max_accel, max_curvature, history, topk, offroad_mode, rollout_mode, topk_order)
     _check(load().wm_create(C.byref(h), C.byref(cfg)), "wm_create")
     return h
 
@@ -191,6 +193,56 @@ def wm_metrics_kinematic(h, sim, t, n_steps, accel, curvature, flag, stream=None
 class wm_paths(C.Structure):
     _fields_ = [("B", C.c_int32), ("A", C.c_int32), ("P", C.c_int32), ("x", C.c_void_p), ("y", C.c_void_p),
                 ("arc_len", C.c_void_p), ("valid", C.c_void_p)]
+
+
+class wm_action_grid(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3), ("lo", C.c_float * 3), ("hi", C.c_float * 3)]
+
+
+def action_grid(n, lo, hi):
+    g = wm_action_grid()
+    for c in range(3):
+        g.n[c] = int(n[c]) if c < len(n) else 1
+        g.lo[c] = float(lo[c]) if c < len(lo) else 0.0
+        g.hi[c] = float(hi[c]) if c < len(hi) else 0.0
+    return g
+
+
+def wm_discretize_actions(h, grid, action, index, dequant=None, valid=None, stream=None):
+    """action [..., C, A] -> index [..., A] int32, dequant like action (may be the same tensor)."""
+    A = action.shape[-1]
+    N = index.numel() // A
+    _check(load().wm_discretize_actions(h, C.byref(grid), C.c_int64(N), C.c_int32(A), _ptr(action, torch.float32),
+                                        _ptr(valid, torch.uint8), _ptr(index, torch.int32), _ptr(dequant, torch.float32),
+                                        _stream(stream)), "wm_discretize_actions")
+
+
+def wm_actions_from_index(h, grid, index, action, stream=None):
+    A = index.shape[-1]
+    N = index.numel() // A
+    _check(load().wm_actions_from_index(h, C.byref(grid), C.c_int64(N), C.c_int32(A), _ptr(index, torch.int32),
+                                        _ptr(action, torch.float32), _stream(stream)), "wm_actions_from_index")
+
+
+def wm_expert_actions_discrete(h, tr, t, n_steps, grid, index, action, action_valid, stream=None):
+    ts = traj_struct(tr)
+    _check(load().wm_expert_actions_discrete(h, C.byref(ts), C.c_int32(t), C.c_int32(n_steps), C.byref(grid), _ptr(index, torch.int32),
+                                             _ptr(action, torch.float32), _ptr(action_valid, torch.uint8), _stream(stream)),
+           "wm_expert_actions_discrete")
+
+
+def wm_rollout_vjp(h, sim, t0, n_steps, actions, action_valid, g_rows, g_actions, g_state0=None, stream=None):
+    ss = traj_struct(sim)
+    _check(load().wm_rollout_vjp(h, C.byref(ss), C.c_int32(t0), C.c_int32(n_steps), _ptr(actions, torch.float32),
+                                 _ptr(action_valid, torch.uint8), _ptr(g_rows, torch.float32), _ptr(g_actions, torch.float32),
+                                 _ptr(g_state0, torch.float32), _stream(stream)), "wm_rollout_vjp")
+
+
+def wm_step_vjp(h, sim, t, action, action_valid, g_next, g_state, g_action, stream=None):
+    ss = traj_struct(sim)
+    _check(load().wm_step_vjp(h, C.byref(ss), C.c_int32(t), _ptr(action, torch.float32), _ptr(action_valid, torch.uint8),
+                              _ptr(g_next, torch.float32), _ptr(g_state, torch.float32), _ptr(g_action, torch.float32),
+                              _stream(stream)), "wm_step_vjp")
 
 
 def paths_struct(paths):

@@ -32,6 +32,7 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (!(cfg->dt > 0.f) || cfg->history < 1 || cfg->topk < 0) return WM_ERR_ARG;
   if (cfg->offroad_mode != WM_OFFROAD_CULLED && cfg->offroad_mode != WM_OFFROAD_BRUTE_FORCE) return WM_ERR_ARG;
   if (cfg->rollout_mode != WM_ROLLOUT_FUSED && cfg->rollout_mode != WM_ROLLOUT_STEPWISE) return WM_ERR_ARG;
+  if (cfg->topk_order != WM_TOPK_BY_INDEX && cfg->topk_order != WM_TOPK_BY_DISTANCE) return WM_ERR_ARG;
   wm_handle* h = (wm_handle*)calloc(1, sizeof(wm_handle));
   if (!h) return WM_ERR_ARG;
   h->cfg = *cfg;
@@ -178,6 +179,56 @@ extern "C" int wm_metrics_kinematic(wm_handle* h, const wm_traj* sim, int32_t t,
   if (!(h->cfg.max_accel > 0.f) || !(h->cfg.max_curvature > 0.f)) return WM_ERR_UNSUPPORTED;   // the metric needs its limits
   WM_CUDA(wm_launch_kinematic(h, *sim, t, n_steps, accel, curvature, flag, (cudaStream_t)stream));
   return WM_OK;
+}
+
+static bool grid_ok(const wm_action_grid* g, int C) {
+  if (!g) return false;
+  int64_t total = 1;
+  for (int c = 0; c < C; ++c) {
+    if (g->n[c] < 1 || (g->n[c] > 1 && !(g->hi[c] > g->lo[c]))) return false;
+    total *= g->n[c];
+    if (total > 0x7fffffffLL) return false;
+  }
+  return true;
+}
+
+extern "C" int wm_discretize_actions(wm_handle* h, const wm_action_grid* grid, int64_t N, int32_t A, const float* action,
+                                     const uint8_t* valid, int32_t* index, float* dequant, void* stream) {
+  const int C = h && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  if (!h || !grid_ok(grid, C) || N < 1 || A < 1 || !action || !index) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_discretize(h, *grid, C, N, A, action, valid, index, dequant, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_actions_from_index(wm_handle* h, const wm_action_grid* grid, int64_t N, int32_t A, const int32_t* index,
+                                     float* action, void* stream) {
+  const int C = h && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  if (!h || !grid_ok(grid, C) || N < 1 || A < 1 || !action || !index) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_from_index(h, *grid, C, N, A, index, action, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_expert_actions_discrete(wm_handle* h, const wm_traj* tr, int32_t t, int32_t n_steps, const wm_action_grid* grid,
+                                          int32_t* index, float* action, uint8_t* action_valid, void* stream) {
+  const int C = h && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
+  if (!h || !traj_ok(tr) || !grid_ok(grid, C) || !action || !action_valid || !index) return WM_ERR_ARG;
+  if (n_steps < 1 || t < 0 || t + n_steps >= tr->T) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_expert(h, *tr, t, n_steps, action, action_valid, (cudaStream_t)stream));
+  WM_CUDA(wm_launch_discretize(h, *grid, C, (int64_t)tr->B * n_steps, tr->A, action, action_valid, index, action, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_rollout_vjp(wm_handle* h, const wm_traj* sim, int32_t t0, int32_t n_steps, const float* actions,
+                              const uint8_t* action_valid, const float* g_rows, float* g_actions, float* g_state0, void* stream) {
+  if (!h || !traj_ok(sim) || !actions || !action_valid || !g_rows || !g_actions) return WM_ERR_ARG;
+  if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
+  WM_CUDA(wm_launch_rollout_vjp(h, *sim, t0, n_steps, actions, action_valid, g_rows, g_actions, g_state0, (cudaStream_t)stream));
+  return WM_OK;
+}
+
+extern "C" int wm_step_vjp(wm_handle* h, const wm_traj* sim, int32_t t, const float* action, const uint8_t* action_valid,
+                           const float* g_next, float* g_state, float* g_action, void* stream) {
+  return wm_rollout_vjp(h, sim, t, 1, action, action_valid, g_next, g_action, g_state, stream);
 }
 
 extern "C" int wm_metrics_route_progress(wm_handle* h, const wm_traj* log, const wm_traj* sim, int32_t t, const wm_paths* paths,

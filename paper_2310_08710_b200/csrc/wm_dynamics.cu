@@ -514,11 +514,9 @@ cudaError_t wm_launch_idm_step(wm_handle* h, const wm_traj& sim, int t, const wm
   const int64_t warps = (int64_t)sim.B * sim.A;
   const size_t smem = 8 * (size_t)(3 * pa.P + ((pa.P + 3) >> 2)) * sizeof(float);
   if (smem > 200 * 1024) return cudaErrorInvalidValue;         // P > ~1900 points per path
-  static size_t configured = 0;
-  if (smem > 40 * 1024 && smem > configured) {
+  if (smem > 40 * 1024) {                          // per-device attribute: set whenever a launch needs it (cheap)
     cudaError_t e = cudaFuncSetAttribute(k_idm_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = smem;
   }
   k_idm_step<<<(unsigned)((warps + 7) / 8), 256, smem, s>>>(p);
   h->launches++;

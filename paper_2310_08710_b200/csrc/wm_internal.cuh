@@ -146,6 +146,12 @@ cudaError_t wm_launch_logdiv(wm_handle* h, const wm_traj& log, const wm_traj& si
 cudaError_t wm_launch_expert(wm_handle* h, const wm_traj& tr, int t, int n_steps, float* action, uint8_t* valid, cudaStream_t s);
 cudaError_t wm_launch_kinematic(wm_handle* h, const wm_traj& tr, int t, int n_steps, float* accel, float* curvature,
                                 uint8_t* flag, cudaStream_t s);
+cudaError_t wm_launch_rollout_vjp(wm_handle* h, const wm_traj& sim, int t0, int n_steps, const float* actions, const uint8_t* av,
+                                  const float* g_rows, float* g_actions, float* g_state0, cudaStream_t s);
+cudaError_t wm_launch_discretize(wm_handle* h, const wm_action_grid& g, int C, int64_t N, int A, const float* action,
+                                 const uint8_t* valid, int32_t* index, float* dequant, cudaStream_t s);
+cudaError_t wm_launch_from_index(wm_handle* h, const wm_action_grid& g, int C, int64_t N, int A, const int32_t* index, float* action,
+                                 cudaStream_t s);
 cudaError_t wm_launch_route_progress(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t, const wm_paths& pa, float* ratio,
                                      uint8_t* valid, cudaStream_t s);
 cudaError_t wm_launch_offroute(wm_handle* h, const wm_traj& sim, int t, const wm_paths& on, const wm_paths* off, float max_dist,

@@ -82,11 +82,9 @@ __global__ void __launch_bounds__(256) k_observe_hist(wm_traj sim, int t, int H,
 cudaError_t wm_launch_observe_hist(wm_handle* h, const wm_traj& sim, int t, float* hist, uint8_t* hist_valid, cudaStream_t s) {
   const int H = h->cfg.history;
   const size_t smem = (size_t)H * 7 * sim.A * 4 + (size_t)H * sim.A;
-  static size_t configured = 0;
-  if (smem > 48 * 1024 && smem > configured) {
+  if (smem > 48 * 1024) {                          // per-device attribute: set whenever a launch needs it (cheap)
     cudaError_t e = cudaFuncSetAttribute(k_observe_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = smem;
   }
   dim3 grid((sim.A + HIST_EGOS - 1) / HIST_EGOS, sim.B);
   k_observe_hist<<<grid, 256, smem, s>>>(sim, t, H, hist, hist_valid);
@@ -201,7 +199,7 @@ constexpr int TK_BASE = 119 << 3;            // level-0 bins start at d2 = 2^-8,
 
 struct TopkParams {
   wm_row row;
-  int A, R, k;
+  int A, R, k, by_distance;
   const float2* pt_xy; const int32_t* pt_idx; const int32_t* pt_start; const WmPtGrid* pt_grid;
   const float *x, *y, *dir_x, *dir_y; const int32_t* type;
   int32_t* rg_index; float* rg_feat; int32_t* rg_type;
@@ -462,6 +460,35 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
   n_out = min(n_out, k);
   const float *gx = p.x + (int64_t)b * R, *gy = p.y + (int64_t)b * R, *gdx = p.dir_x + (int64_t)b * R, *gdy = p.dir_y + (int64_t)b * R;
   const int32_t* gt = p.type + (int64_t)b * R;
+  if (p.by_distance) {
+    // WM_TOPK_BY_DISTANCE (D44): the selected points by ascending (key, index) - a bitonic sort of
+    // (key bits << 32 | index) in shared memory, padded to a power of two with all-ones
+    unsigned long long* sk = (unsigned long long*)(s_bits + ((2 * Wd + k + 1) & ~1));
+    int P = 1;
+    while (P < n_out) P <<= 1;
+    for (int j = tid; j < P; j += TK_THREADS) {
+      unsigned long long kv = ~0ull;
+      if (j < n_out) {
+        const int idx = list[j];
+        const float dx = __fsub_rn(__ldg(gx + idx), ex), dy = __fsub_rn(__ldg(gy + idx), ey);
+        kv = ((unsigned long long)__float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx))) << 32) | (unsigned)idx;
+      }
+      sk[j] = kv;
+    }
+    __syncthreads();
+    for (int len = 2; len <= P; len <<= 1)
+      for (int st = len >> 1; st > 0; st >>= 1) {
+        for (int i = tid; i < (P >> 1); i += TK_THREADS) {
+          const int lo = ((i & ~(st - 1)) << 1) | (i & (st - 1)), hi = lo | st;
+          const bool up = (lo & len) == 0;
+          const unsigned long long a = sk[lo], c = sk[hi];
+          if ((a > c) == up) { sk[lo] = c; sk[hi] = a; }
+        }
+        __syncthreads();
+      }
+    for (int j = tid; j < n_out; j += TK_THREADS) list[j] = (int)(unsigned)(sk[j] & 0xffffffffull);
+    __syncthreads();
+  }
   for (int j = tid; j < n_out; j += TK_THREADS) {
     const int idx = list[j];
     const float dx = __fsub_rn(__ldg(gx + idx), ex), dy = __fsub_rn(__ldg(gy + idx), ey);
@@ -480,17 +507,20 @@ cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_ro
                                    int32_t* rg_index, float* rg_feat, int32_t* rg_type, cudaStream_t s) {
   TopkParams p;
   p.row = wm_make_row(sim, t);
-  p.A = sim.A; p.R = rg.R; p.k = h->cfg.topk;
+  p.A = sim.A; p.R = rg.R; p.k = h->cfg.topk; p.by_distance = h->cfg.topk_order == WM_TOPK_BY_DISTANCE;
   p.pt_xy = h->pt_xy; p.pt_idx = h->pt_idx; p.pt_start = h->pt_start; p.pt_grid = h->pt_grid;
   p.x = rg.x; p.y = rg.y; p.dir_x = rg.dir_x; p.dir_y = rg.dir_y; p.type = rg.type;
   p.rg_index = rg_index; p.rg_feat = rg_feat; p.rg_type = rg_type;
-  const size_t smem = (2 * (size_t)((rg.R + 31) / 32) + (size_t)h->cfg.topk) * sizeof(uint32_t);
+  size_t smem = (2 * (size_t)((rg.R + 31) / 32) + (size_t)h->cfg.topk) * sizeof(uint32_t);
+  if (p.by_distance) {                                        // + the sort keys: 8 B x the power of two >= k
+    size_t P = 1;
+    while (P < (size_t)h->cfg.topk) P <<= 1;
+    smem = ((smem + 7) & ~(size_t)7) + P * sizeof(unsigned long long);
+  }
   if (smem > 200 * 1024) return cudaErrorInvalidValue;       // R > 819 200 points per scenario
-  static size_t configured = 0;
-  if (smem > 40 * 1024 && smem > configured) {
+  if (smem > 40 * 1024) {                                     // per-device attribute: set whenever a launch needs it (cheap)
     cudaError_t e = cudaFuncSetAttribute(k_observe_topk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = smem;
   }
   k_observe_topk<<<dim3(sim.A, sim.B), TK_THREADS, smem, s>>>(p);
   h->launches++;

@@ -519,13 +519,9 @@ cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd
   const size_t fixed = off_fixed_bytes(sim.A);
   // Two 256-thread CTAs per SM (each <= 113 KB of shared memory) so that one CTA's set-up,
   // flushes and re-scan overlap the other's main loop; one 512-thread CTA per SM when the
-  // per-agent arrays leave too little room (large A).  WM_OFFROAD_CTA=512|256 forces a variant.
-  static int forced = -1;
-  if (forced < 0) { const char* e = getenv("WM_OFFROAD_CTA"); forced = e ? atoi(e) : 0; }
+  // per-agent arrays leave too little room (large A).
   const size_t sm_total = 227 * 1024, per_cta2 = (sm_total - 2048) / 2;
-  bool two = fixed + 2 * 2 * (size_t)WM_TILE_BYTES <= per_cta2;
-  if (forced == 512) two = false;
-  if (forced == 256 && fixed + 2 * (size_t)WM_TILE_BYTES <= per_cta2) two = true;
+  const bool two = fixed + 2 * 2 * (size_t)WM_TILE_BYTES <= per_cta2;
   const size_t max_smem = two ? per_cta2 : sm_total;
   int tpb = (int)((max_smem - fixed) / (2 * (size_t)WM_TILE_BYTES));
   const int need = (h->seg_tiles + 1) / 2;        // two buffers hold the whole scenario if they can
@@ -533,12 +529,10 @@ cudaError_t wm_launch_offroad(wm_handle* h, const wm_traj& sim, int t, float* sd
   if (tpb < 1) tpb = 1;
   p.tiles_per_buf = tpb;
   const size_t smem = fixed + 2 * (size_t)tpb * WM_TILE_BYTES;
-  static bool configured = false;
-  if (!configured) {
+  {                                                // per-device attributes: set at every launch (cheap)
     cudaError_t e = cudaFuncSetAttribute(k_offroad<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_total);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_offroad<256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)per_cta2);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   if (two) k_offroad<256, 2><<<sim.B, 256, smem, s>>>(p);
   else k_offroad<512, 1><<<sim.B, 512, smem, s>>>(p);
