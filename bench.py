@@ -42,14 +42,55 @@ FLOP_PER_PAIR = 13.0           # w(2) t(3) c(4) d2(3) min(1)
 METRIC = "agent-steps/sec for step+overlap+offroad (B=4096,A=128); % of roofline"
 
 
-def profiled_traffic(kernel):
-    """dram__bytes_read+write per launch of `kernel` from the latest committed ncu summary."""
+def source_hash():
+    """sha256 over the CUDA sources of the library: ties a profiled number to the code it was taken from."""
     import glob
-    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_%s_traffic_bytes.txt" % kernel)))
+    import hashlib
+    hsh = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2310_08710_b200", "csrc", "*.cu*"))):
+        hsh.update(open(f, "rb").read())
+    return hsh.hexdigest()
+
+
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+
+
+def profiled_traffic(kernel):
+    """dram__bytes_read + write per launch of `kernel` from the committed ncu pass (profiles/r02_traffic.json,
+    written by `bench.py --write-traffic <ncu csv>`).  A number taken from other sources than the ones
+    that are being timed is not reported: (None, why)."""
     try:
-        return float(open(files[-1]).read().split()[0]) if files else None
+        d = json.load(open(TRAFFIC_FILE))
     except Exception:
-        return None
+        return None, "no profiles/r02_traffic.json"
+    if d.get("source_sha256") != source_hash():
+        return None, "profiles/r02_traffic.json was taken from other kernel sources (sha256 differs): re-run the ncu pass"
+    v = d.get("kernels", {}).get(kernel)
+    return (float(v), "profiles/r02_traffic.json (%s)" % d.get("command", "ncu")) if v is not None else (None, "kernel not in profiles/r02_traffic.json")
+
+
+def write_traffic(csv_path):
+    """Parse `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum --csv` output into profiles/r02_traffic.json."""
+    import csv
+    rows = list(csv.reader(open(csv_path)))
+    i = [k for k, r in enumerate(rows) if r and r[0] == "ID"][0]
+    hdr = rows[i]
+    kn, mn, mv, mu = hdr.index("Kernel Name"), hdr.index("Metric Name"), hdr.index("Metric Value"), hdr.index("Metric Unit")
+    acc = {}
+    for r in rows[i + 1:]:
+        if len(r) <= mv or not r[mn].startswith("dram__bytes"):
+            continue
+        name = r[kn].split("(")[0].split("<")[0].replace("void ", "").strip()
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(r[mu], 1.0)
+        a = acc.setdefault(name, {})
+        a.setdefault(r[0], 0.0)
+        a[r[0]] += float(r[mv].replace(",", "")) * scale
+    kernels = {k: float(np.mean(list(v.values()))) for k, v in acc.items()}
+    out = {"source_sha256": source_hash(), "kernels": kernels, "unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
+           "command": "ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum --clock-control none --csv; bench.py --write-traffic"}
+    json.dump(out, open(TRAFFIC_FILE, "w"), indent=1)
+    print(json.dumps(out))
+    return 0
 
 
 def measured_peaks():
@@ -454,6 +495,122 @@ def run_supplementary(args):
     return 0
 
 
+def other_configs(wm, ws, torch, hbm_peak, log5_d, sim5_d, stream):
+    """The remaining SURVEY 8(a)/(f) rows in the default line: configs 3, 2, 4 (BASELINE.json configs[2], [1], [3]),
+    the expert actor / kinematic metric and the IDM step on config-5 scenarios.  Device-resident, CUDA events per
+    repetition on the launching stream, L2 flushed (a 256 MB write) before every repetition, 3 warm-ups + 5 timed."""
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn, reps=5, warm=3):
+        for _ in range(warm):
+            fn()
+        tot = 0.0
+        for _ in range(reps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); fn(); b.record(stream)
+            torch.cuda.synchronize()
+            tot += a.elapsed_time(b)
+        return tot / reps
+
+    def rl(nbytes, ms):
+        return {"ms": ms, "algorithmic_bytes": float(nbytes), "hbm_frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak}
+    out = {"protocol": "L2 flushed (256 MB write) before every repetition; CUDA events on the launching stream; 3 warm-ups + 5 timed"}
+    # ---- config 3: observation (a6, a7) ----
+    cfg = ws.make_config(3)
+    log, rg = cfg["log"], cfg["roadgraph"]
+    B, T, A = log["x"].shape
+    R = rg["x"].shape[1]
+    k, H, t = 1000, 11, 10
+    h = wm.wm_create(topk=k)
+    log_d, rg_d = wm.to_device(log), wm.to_device(rg)
+    wm.wm_prepare(h, rg_d)
+    hist = torch.empty((B, A, H, 7, A), device="cuda"); hv = torch.empty((B, A, H, A), dtype=torch.uint8, device="cuda")
+    idx = torch.empty((B, A, k), dtype=torch.int32, device="cuda"); feat = torch.empty((B, A, 4, k), device="cuda")
+    typ = torch.empty((B, A, k), dtype=torch.int32, device="cuda")
+    l0 = wm.wm_kernel_launches(h)
+    ms_h = timed(lambda: wm.wm_observe(h, log_d, rg_d, t, hist, hv, None, None, None))
+    ms_k = timed(lambda: wm.wm_observe(h, log_d, rg_d, t, None, None, idx, feat, typ))
+    b_h = hist.numel() * 4 + hv.numel() + B * H * A * 29
+    b_k = idx.numel() * 4 + feat.numel() * 4 + typ.numel() * 4 + B * R * 8
+    out["config3_observe"] = {"workload": "B=%d A=%d R=%d H=%d k=%d, every valid agent an ego" % (B, A, R, H, k),
+                              "k_observe_hist": rl(b_h, ms_h), "k_observe_topk": rl(b_k, ms_k), "ms": ms_h + ms_k,
+                              "ego_observations_per_s": B * A / ((ms_h + ms_k) * 1e-3)}
+    launches = wm.wm_kernel_launches(h) - l0
+    wm.wm_destroy(h)
+    del hist, hv, idx, feat, typ, log_d, rg_d
+    # ---- config 2: one DeltaLocal step + overlap + offroad + log divergence (a2-a5) ----
+    for cid in (2, 4):
+        cfg = ws.make_config(cid)
+        log, rg = cfg["log"], cfg["roadgraph"]
+        B, T, A = log["x"].shape
+        h = wm.wm_create(dynamics=wm.WM_DYN_DELTA_LOCAL)
+        log_d, rg_d = wm.to_device(log), wm.to_device(rg)
+        wm.wm_prepare(h, rg_d)
+        sim_d = wm.empty_traj_like(log_d)
+        Wd = (A + 31) // 32
+        bits = torch.empty((B, A, Wd), dtype=torch.int32, device="cuda"); ofl = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+        sd = torch.empty((B, A), device="cuda"); fl = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+        ld = torch.empty((B, A), device="cuda"); lv = torch.empty((B, A), dtype=torch.uint8, device="cuda")
+        l0 = wm.wm_kernel_launches(h)
+        if cid == 2:
+            t = wm.wm_reset(h, log_d, sim_d)
+            act = torch.from_numpy(np.ascontiguousarray(cfg["actions"][:, 0])).cuda()
+            av = torch.from_numpy(np.ascontiguousarray(cfg["action_valid"][:, 0])).cuda()
+            ms_st = timed(lambda: wm.wm_step(h, log_d, sim_d, t, act, av))
+            ms_ov = timed(lambda: wm.wm_metrics_overlap(h, sim_d, t + 1, bits, ofl))
+            ms_of = timed(lambda: wm.wm_metrics_offroad(h, sim_d, t + 1, sd, None, fl))
+            ms_ld = timed(lambda: wm.wm_log_divergence(h, log_d, sim_d, t + 1, ld, lv))
+            n = float(B) * A
+            out["config2_step"] = {"workload": "B=%d A=%d R=%d, DeltaLocal step + overlap matrix + offroad + log divergence" % (B, A, rg["x"].shape[1]),
+                                   "k_step": rl(n * (29 + 13 + 29 + 29), ms_st), "k_overlap": rl(n * (29 + 4 * Wd + 1), ms_ov),
+                                   "k_offroad_grid": rl(n * (29 + 5), ms_of), "k_logdiv": rl(n * (18 + 5), ms_ld),
+                                   "ms": ms_st + ms_ov + ms_of + ms_ld, "agent_steps_per_s": n / ((ms_st + ms_ov + ms_of + ms_ld) * 1e-3),
+                                   "note": "%d agents per call: launch / latency bound, the HBM fractions are not roofline claims" % int(n)}
+        else:
+            ms_ov = timed(lambda: wm.wm_metrics_overlap(h, log_d, 0, bits, ofl))
+            ms_of = timed(lambda: wm.wm_metrics_offroad(h, log_d, 0, sd, None, fl))
+            n = float(B) * A
+            out["config4_stress"] = {"workload": "B=%d A=%d R=%d, overlap matrix + offroad of the crowded lot" % (B, A, rg["x"].shape[1]),
+                                     "k_overlap": rl(n * (29 + 4 * Wd + 1), ms_ov), "k_offroad_grid": rl(n * (29 + 5), ms_of),
+                                     "ms": ms_ov + ms_of, "pair_tests_per_s": B * A * (A - 1) / 2 / (ms_ov * 1e-3),
+                                     "note": "%d agents per call: launch / latency bound, the HBM fractions are not roofline claims" % int(n)}
+        launches += wm.wm_kernel_launches(h) - l0
+        wm.wm_destroy(h)
+        del log_d, rg_d, sim_d
+    # ---- expert actor + kinematic metric (NEXT(1)) and the backward pass (NEXT(4)) on the config-5 batch ----
+    B, T, A = log5_d["x"].shape
+    h = wm.wm_create()
+    act = torch.empty((B, N_STEPS, 2, A), device="cuda"); av = torch.empty((B, N_STEPS, A), dtype=torch.uint8, device="cuda")
+    kacc = torch.empty((B, N_STEPS, A), device="cuda"); kcur = torch.empty((B, N_STEPS, A), device="cuda")
+    kfl = torch.empty((B, N_STEPS, A), dtype=torch.uint8, device="cuda")
+    l0 = wm.wm_kernel_launches(h)
+    ms_e = timed(lambda: wm.wm_expert_actions(h, log5_d, 10, N_STEPS, act, av))
+    ms_m = timed(lambda: wm.wm_metrics_kinematic(h, sim5_d, 11, N_STEPS, kacc, kcur, kfl))
+    n_as = float(B) * A * N_STEPS
+    g_rows = torch.ones((B, N_STEPS, 5, A), device="cuda"); g_act = torch.empty((B, N_STEPS, 2, A), device="cuda")
+    ms_v = timed(lambda: wm.wm_rollout_vjp(h, sim5_d, 10, N_STEPS, act, av, g_rows, g_act, None))
+    out["config5_expert"] = {"workload": "B=%d A=%d, 80 transitions per agent" % (B, A), "k_inverse_expert": rl(n_as * 22, ms_e),
+                             "k_inverse_kinematic": rl(n_as * 22, ms_m), "k_rollout_vjp": rl(n_as * (13 + 9 + 20 + 8), ms_v)}
+    del g_rows, g_act, kacc, kcur, kfl
+    # ---- IDM sim agent step (NEXT(2)) on the first 1024 config-5 scenarios ----
+    Bi = min(1024, B)
+    logi = {q: v[:Bi].contiguous() for q, v in log5_d.items()}
+    simi = wm.empty_traj_like(logi)
+    t0 = wm.wm_reset(h, logi, simi)
+    paths = ws.make_paths({q: v.cpu().numpy() for q, v in logi.items()})
+    paths_d = {q: torch.from_numpy(v).cuda() for q, v in paths.items()}
+    idm_d = torch.ones((Bi, A), dtype=torch.uint8, device="cuda")
+    acc = torch.empty((Bi, A), device="cuda"); lead = torch.empty((Bi, A), dtype=torch.int32, device="cuda")
+    ms_i = timed(lambda: wm.wm_idm_step(h, simi, t0, paths_d, idm_d, acc, lead))
+    P = paths["x"].shape[2]
+    out["config5_idm"] = {"workload": "B=%d A=%d, paths of %d points, every valid agent IDM-controlled" % (Bi, A, P),
+                          "k_idm_step": rl(float(Bi) * A * (P * 13 + 29 + 29 + 8), ms_i), "agent_steps_per_s": Bi * A / (ms_i * 1e-3)}
+    launches += wm.wm_kernel_launches(h) - l0
+    wm.wm_destroy(h)
+    return out, int(launches)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -469,8 +626,11 @@ def main():
                     help="rollout = the BASELINE metric (config 5, default); the others time the remaining "
                          "SURVEY 8(a) rows on configs 3, 2, 4 (supplementary lines, same JSON shape)")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (single-step grid kernel, brute-force kernel)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (single-step grid kernel, brute-force kernel, other configs)")
+    ap.add_argument("--write-traffic", default=None, metavar="NCU_CSV", help="parse an ncu dram__bytes csv into profiles/r02_traffic.json and exit")
     args = ap.parse_args()
+    if args.write_traffic:
+        return write_traffic(args.write_traffic)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     args.steps_ref = max(1, min(args.steps, 3)); args.warmup_ref = max(1, min(args.warmup, 1))
     if args.impl == "reference":
@@ -545,7 +705,7 @@ def main():
         torch.cuda.synchronize()
         return ka.elapsed_time(kb) / N_STEPS
 
-    # dominant kernel of the timed region: k_rollout_fused (one launch = the whole 80-step rollout)
+    # the rollout's two kernels (one graph; the whole 80-step rollout = one launch of each), timed one by one
     def time_rollout():
         wm.wm_rollout(h, log_d, sim_d, 10, N_STEPS, acts_d, av_d, out_d)
         torch.cuda.synchronize()
@@ -558,6 +718,27 @@ def main():
         return ka.elapsed_time(kb) / 5
 
     kf_ms = time_rollout()
+    kt = np.array([wm.wm_rollout_kernel_times(h, log_d, sim_d, 10, N_STEPS, acts_d, av_d, out_d) for _ in range(6)][1:])
+    dyn_ms, met_ms = float(kt[:, 0].mean()), float(kt[:, 1].mean())
+    # wm_prepare (the static precompute a NEW batch of scenarios needs before its first rollout), and reset alone
+    def time_prepare(reps=3):
+        wm.wm_prepare(h, rg_d)
+        torch.cuda.synchronize()
+        ka, kb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ka.record(stream)
+        for _ in range(reps):
+            wm.wm_prepare(h, rg_d)
+        kb.record(stream)
+        torch.cuda.synchronize()
+        return ka.elapsed_time(kb) / reps
+    prepare_ms = sharding.max_over_ranks(time_prepare(), dev)
+    ka, kb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ka.record(stream)
+    for _ in range(5):
+        wm.wm_reset(h, log_d, sim_d)
+    kb.record(stream)
+    torch.cuda.synchronize()
+    reset_ms = ka.elapsed_time(kb) / 5
     # pair counters of the search, from one more rollout with the kernel's counters switched on
     wm.wm_offroad_stats_enable(h, True); wm.wm_offroad_stats(h)
     wm.wm_rollout(h, log_d, sim_d, 10, N_STEPS, acts_d, av_d, out_d)
@@ -573,26 +754,50 @@ def main():
     hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"
     fp32_peak = props.multi_processor_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12              # TFLOP/s
     peak_src = "SMs(%d)*128*2*%.0f MHz (nominal, B200_PROFILING.md unit counts/clocks)" % (props.multi_processor_count, sm_max_mhz)
-    # compulsory bytes of one rollout launch: per agent-step the action (C*4) and its mask (1),
-    # log row t+1 in (29), sim row t+1 out (29), metric rows out (1+1+4+4); per agent row t0 in (29) and
-    # the aggregates out (1+1+4).  The search structures (cells, records) are not compulsory IO.
+    # FP32 peak as a register-resident FMA loop reaches it in THIS run: scalar FFMA and packed FFMA2
+    fp32_measured = {}
+    for packed, name in ((0, "ffma"), (1, "ffma2")):
+        best = 0.0
+        for _ in range(3):
+            ms_f, flop = wm.wm_selftest_ffma(h, packed, props.multi_processor_count * 8, 4096)
+            best = max(best, flop / (ms_f * 1e-3) / 1e12)
+        fp32_measured[name] = best
+    fp32_peak_measured = max(fp32_measured.values())
+    # Compulsory bytes of the rollout: per agent-step the action (C*4) and its mask (1), log row
+    # t+1 in (29), sim row t+1 out (29), metric rows out (1+1+4+4); per agent row t0 in (29) and the
+    # aggregates out (1+1+4).  NOT compulsory, hence not counted: the search structures (cells, records) and
+    # the metrics kernel's re-read of the simulated rows (21 B per agent-step: x, y, yaw, length, width, valid).
     C_ACT = 2
-    fused_bytes = float(B) * N_STEPS * A * (C_ACT * 4 + 1 + 29 + 29 + 10) + float(B) * A * (29 + 6)
+    n_as = float(B) * N_STEPS * A
+    fused_bytes = n_as * (C_ACT * 4 + 1 + 29 + 29 + 10) + float(B) * A * (29 + 6)
+    dyn_bytes = n_as * (C_ACT * 4 + 1 + 9 + 29 + 4) + float(B) * A * (29 + 6)      # k_rollout_dyn: action, mask, log x/y/valid in; sim row, log divergence out
+    met_bytes = n_as * (21 + 6)                                                    # k_rollout_metrics: x, y, yaw, length, width, valid in; 2 flags + distance out
     fused_flops = pairs_eval * N_STEPS * FLOP_PER_PAIR
-    roofline = {"bound": "hbm", "achieved": fused_bytes / (kf_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": fused_bytes / (kf_ms * 1e-3) / 1e9 / hbm_peak, "traffic": profiled_traffic("k_rollout_fused"),
-                "kernel": "k_rollout_fused", "kernel_ms": kf_ms, "algorithmic_bytes_per_launch": fused_bytes,
-                "peak_source": hbm_src, "kernel_share_of_step": kf_ms / ms_step,
+    roll_ms = dyn_ms + met_ms
+    tr_dyn, src_dyn = profiled_traffic("k_rollout_dyn")
+    tr_met, src_met = profiled_traffic("k_rollout_metrics")
+    roofline = {"bound": "hbm", "achieved": fused_bytes / (roll_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": fused_bytes / (roll_ms * 1e-3) / 1e9 / hbm_peak,
+                "traffic": (tr_dyn + tr_met) if (tr_dyn is not None and tr_met is not None) else None, "traffic_source": src_met,
+                "kernel": "k_rollout_dyn + k_rollout_metrics (the rollout graph: one launch of each per 80-step rollout)",
+                "kernel_ms": roll_ms, "graph_replay_ms": kf_ms, "algorithmic_bytes_per_launch": fused_bytes,
+                "peak_source": hbm_src, "kernel_share_of_step": roll_ms / ms_step,
                 "hbm_time_ms_at_peak": fused_bytes / (hbm_peak * 1e9) * 1e3,
+                "kernels": {
+                    "k_rollout_metrics": {"ms": met_ms, "share_of_step": met_ms / ms_step, "algorithmic_bytes_per_launch": met_bytes,
+                                          "hbm_frac": met_bytes / (met_ms * 1e-3) / 1e9 / hbm_peak, "traffic": tr_met,
+                                          "bound_observed": "instruction issue (ncu: profiles/r02_k_rollout_metrics_ncu.md), not HBM and not the FP32 pipe",
+                                          "alu_frac_on_evaluated_pairs": fused_flops / (met_ms * 1e-3) / 1e12 / fp32_peak},
+                    "k_rollout_dyn": {"ms": dyn_ms, "share_of_step": dyn_ms / ms_step, "algorithmic_bytes_per_launch": dyn_bytes,
+                                      "hbm_frac": dyn_bytes / (dyn_ms * 1e-3) / 1e9 / hbm_peak, "traffic": tr_dyn}},
                 "fp32_time_ms_at_peak_on_evaluated_pairs": fused_flops / (fp32_peak * 1e12) * 1e3,
                 "pairs_bruteforce_per_step": pairs_per_launch, "pairs_evaluated_per_step": pairs_eval,
                 "evaluated_fraction": pairs_eval / pairs_per_launch, "pairs_per_corner": ev_pairs / max(n_corner, 1),
                 "slow_path_corner_fraction": n_slow / max(n_corner, 1),
-                "alu_frac_on_evaluated_pairs": fused_flops / (kf_ms * 1e-3) / 1e12 / fp32_peak,
-                "alu_frac_bruteforce_equivalent": pairs_per_launch * N_STEPS * FLOP_PER_PAIR / (kf_ms * 1e-3) / 1e12 / fp32_peak,
-                "note": "exact culling (SURVEY 8(d)) leaves under 0.1 % of the pairs, so the slower roof of the kernel is its "
-                        "compulsory HBM IO; the FP32 fractions on evaluated pairs and on the brute-force count are beside it. "
-                        "ncu: the kernel is bound by gather latency and instruction issue, not by HBM bandwidth (profiles/)"}
+                "alu_frac_bruteforce_equivalent": pairs_per_launch * N_STEPS * FLOP_PER_PAIR / (roll_ms * 1e-3) / 1e12 / fp32_peak,
+                "note": "achieved = compulsory HBM bytes of the rollout / (k_rollout_dyn + k_rollout_metrics) CUDA-event time. The exact culling "
+                        "(SURVEY 8(d)) leaves under 0.1 % of the corner-segment pairs, so the slower roof is the compulsory IO; the dominant "
+                        "kernel k_rollout_metrics is bound by instruction issue (gathers through the cell lists), see DESIGN.md 7"}
     hbm_bytes = float(n_seg.sum()) * 24.0 + B * A * 29.0 + B * A * 5.0    # brute force: segments once + one state row + outputs
     rl_ms = max(pairs_per_launch * FLOP_PER_PAIR / (fp32_peak * 1e12), hbm_bytes / (hbm_peak * 1e9)) * 1e3
     step_roofline = {"definition": "north_star: slower of algorithmic bytes/HBM peak and brute-force FP32 flops/FP32 peak, per simulated step",
@@ -610,10 +815,15 @@ def main():
         wm.wm_destroy(hb)
         bf_achieved = pairs_per_launch * FLOP_PER_PAIR / (kb_ms * 1e-3) / 1e12
         roofline_bf = {"bound": "alu", "achieved": bf_achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                       "frac": bf_achieved / fp32_peak, "traffic": profiled_traffic("k_offroad_brute"),
+                       "frac": bf_achieved / fp32_peak, "traffic": profiled_traffic("k_offroad")[0],
                        "kernel": "k_offroad (offroad_mode=WM_OFFROAD_BRUTE_FORCE)", "kernel_ms": kb_ms,
-                       "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR, "peak_source": peak_src}
+                       "pairs_per_launch": pairs_per_launch, "flop_per_pair": FLOP_PER_PAIR, "peak_source": peak_src,
+                       "peak_measured": fp32_peak_measured, "frac_of_measured_peak": bf_achieved / fp32_peak_measured,
+                       "peak_measured_source": "wm_selftest_ffma in this run: register-resident FFMA %.1f / FFMA2 %.1f TFLOP/s" % (fp32_measured["ffma"], fp32_measured["ffma2"])}
     clocks = sampler.stop() if rank == 0 else None
+    others = None
+    if rank == 0 and world == 1 and not args.no_extras:
+        others, _ = other_configs(wm, ws, torch, hbm_peak, log_d, sim_d, stream)
 
     # ---- e2e: the same job from pinned host buffers through the C-ABI ----
     e2e = None
@@ -654,9 +864,33 @@ def main():
                            np.ascontiguousarray(cfg["actions"][:sb]), np.ascontiguousarray(cfg["action_valid"][:sb]))
         dt = time.perf_counter() - t0
         agree = float((o["offroad"] == out_d["offroad"][:sb].cpu().numpy()).mean())
+        # parity on the same sample, teacher-forced (P16): the oracle's metrics on the GPU's OWN rows at 9 of the 80
+        # steps, flags compared outside the 1e-4 m ambiguity band (P15), band members counted
+        got = {k: v[:sb].cpu().numpy() for k, v in sim_d.items()}
+        g_off = out_d["offroad"][:sb].cpu().numpy(); g_sd = out_d["offroad_dist"][:sb].cpu().numpy(); g_ov = out_d["overlap"][:sb].cpu().numpy()
+        flags_equal, amb_corners, n_corners, amb_pairs, dist_ok, checked = True, 0, 0, 0, True, []
+        for s_ in list(range(0, N_STEPS, 10)) + [N_STEPS - 1]:
+            tt = cfg["t0"] + s_ + 1
+            off = oracle.offroad(got, tt, rgs)
+            v_ = got["valid"][:, tt] == 1
+            amb = off["ambig"] == 1
+            clean = v_ & ~amb.any(axis=1)
+            flags_equal &= bool(np.array_equal(g_off[:, s_][clean], off["flag"][clean]))
+            ref = off["signed_dist"].astype(np.float64)[clean]
+            dist_ok &= bool(np.all(np.abs(g_sd[:, s_][clean].astype(np.float64) - ref) <= 1e-5 * np.abs(ref) + 3e-6))
+            amb_corners += int((amb & v_[:, None, :]).sum()); n_corners += 4 * int(v_.sum())
+            ovl = oracle.overlap(got, tt)
+            band = np.abs(ovl["gap"]) < 1e-4
+            cl = ~band.any(axis=2)
+            flags_equal &= bool(np.array_equal(g_ov[:, s_][cl], ovl["flag"][cl]))
+            amb_pairs += int(band.sum())
+            checked.append(s_)
         cpu = {"value": sb * A * N_STEPS / dt, "unit": "agent-steps/s", "cores": oracle.num_threads(), "kind": "oracle",
                "sample": "first %d of %d scenarios x %d steps, oracle.rollout, %.1f s wall" % (sb, B, N_STEPS, dt),
-               "offroad_flag_agreement_free_running": agree}
+               "offroad_flag_agreement_free_running": agree,
+               "parity_teacher_forced": {"scenarios": sb, "steps_checked": checked, "flags_equal_outside_band": flags_equal,
+                                         "distances_within_tolerance": dist_ok, "tolerance": "rel 1e-5 + 3e-6 m",
+                                         "ambiguous_corners": amb_corners, "corners": n_corners, "ambiguous_overlap_pairs": amb_pairs}}
 
     if rank == 0:
         line = {
@@ -667,7 +901,13 @@ def main():
                        "B_per_gpu": B, "A": A, "R": R, "T": T, "n_steps": N_STEPS, "S_e_max": int(seg_max),
                        "S_e_mean": float(n_seg.mean()), "l2": "inputs exceed L2 (segments %.2f GB + state per step)" % (n_seg.sum() * 24 / 1e9),
                        "parallelism": "scenario shards, no collective", "valid_agent_steps_per_s": valid_value,
-                       "ms_per_sim_step": ms_step / N_STEPS},
+                       "ms_per_sim_step": ms_step / N_STEPS,
+                       "value_counts": "agent SLOTS (valid or not, SURVEY 8(d)); valid_agent_steps_per_s counts the valid ones"},
+            # wm_prepare = the static precompute a NEW batch of scenarios needs before its first rollout (outside `value`:
+            # `value` assumes prepared scenarios, e.g. re-rolled in training); value_incl_prepare = one prepare per rollout
+            "prepare_ms": prepare_ms, "reset_ms": reset_ms,
+            "value_incl_prepare": agent_steps / ((prepare_ms + ms_step) * 1e-3),
+            "other_configs": others,
             "roofline": roofline, "roofline_offroad_grid": roofline_grid, "roofline_bruteforce": roofline_bf, "step_roofline": step_roofline,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }

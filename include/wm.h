@@ -352,6 +352,17 @@ int64_t wm_kernel_launches(const wm_handle* h);
 int wm_offroad_stats(wm_handle* h, int64_t* out_host, void* stream);
 int wm_offroad_stats_enable(wm_handle* h, int32_t on);
 
+/* Diagnostics for the bench (HOST outputs; both synchronise the stream).
+ * wm_rollout_kernel_times: runs the fused rollout's two kernels once, eagerly, with CUDA events around
+ * each: ms_host[0] = k_rollout_dyn, ms_host[1] = k_rollout_metrics (a graph replay cannot be timed node
+ * by node).  Same arguments and results as wm_rollout; WM_ERR_UNSUPPORTED outside the fused mode.
+ * wm_selftest_ffma: duration of a register-resident FFMA (packed = 0) / FFMA2 (packed = 1) loop on `ctas`
+ * CTAs of 256 threads, `iters` x 32 FMAs per thread, and the flop it executed: the measured FP32 peak. */
+int wm_rollout_kernel_times(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t0, int32_t n_steps,
+                            const float* actions, const uint8_t* action_valid, const wm_rollout_out* out,
+                            float* ms_host, void* stream);
+int wm_selftest_ffma(wm_handle* h, int32_t packed, int32_t ctas, int32_t iters, float* ms_host, double* flop_host, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
            "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_idm_step", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable",
-           "wm_discretize_actions", "wm_actions_from_index", "wm_expert_actions_discrete", "wm_rollout_vjp", "wm_step_vjp")
+           "wm_discretize_actions", "wm_actions_from_index", "wm_expert_actions_discrete", "wm_rollout_vjp", "wm_step_vjp", "wm_rollout_kernel_times", "wm_selftest_ffma")
 
 
 class wm_traj(C.Structure):
@@ -296,6 +296,23 @@ def wm_rollout(h, log, sim, t0, n_steps, actions, action_valid, out, stream=None
     _check(load().wm_rollout(h, C.byref(ls), C.byref(ss), C.c_int32(t0), C.c_int32(n_steps),
                              _ptr(actions, torch.float32), _ptr(action_valid, torch.uint8), C.byref(os_),
                              _stream(stream)), "wm_rollout")
+
+
+def wm_rollout_kernel_times(h, log, sim, t0, n_steps, actions, action_valid, out, stream=None):
+    """(ms of k_rollout_dyn, ms of k_rollout_metrics) of one eager run of the fused rollout."""
+    ls, ss, os_ = traj_struct(log), traj_struct(sim), rollout_out_struct(out)
+    ms = (C.c_float * 2)()
+    _check(load().wm_rollout_kernel_times(h, C.byref(ls), C.byref(ss), C.c_int32(t0), C.c_int32(n_steps), _ptr(actions, torch.float32),
+                                          _ptr(action_valid, torch.uint8), C.byref(os_), ms, _stream(stream)), "wm_rollout_kernel_times")
+    return float(ms[0]), float(ms[1])
+
+
+def wm_selftest_ffma(h, packed, ctas, iters, stream=None):
+    """(ms, flop) of a register-resident FFMA / FFMA2 loop: the FP32 peak as measured on this GPU."""
+    ms = C.c_float(0); fl = C.c_double(0)
+    _check(load().wm_selftest_ffma(h, C.c_int32(int(packed)), C.c_int32(ctas), C.c_int32(iters), C.byref(ms), C.byref(fl), _stream(stream)),
+           "wm_selftest_ffma")
+    return float(ms.value), float(fl.value)
 
 
 def wm_rollout_host(h, log_host, rg_host, n_steps, actions_host, action_valid_host, out_host, sim_host=None, stream=None):

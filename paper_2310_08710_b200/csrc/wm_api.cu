@@ -384,6 +384,46 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
   return WM_OK;
 }
 
+// Diagnostics for the bench: the two kernels of the fused rollout launched eagerly with CUDA events
+// between them (a graph replay cannot be timed node by node).  Synchronises.
+extern "C" int wm_rollout_kernel_times(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t0, int32_t n_steps,
+                                       const float* actions, const uint8_t* action_valid, const wm_rollout_out* out,
+                                       float* ms_host, void* stream) {
+  if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !actions || !action_valid || !out || !ms_host) return WM_ERR_ARG;
+  if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
+  if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
+  if (h->cfg.rollout_mode != WM_ROLLOUT_FUSED || h->cfg.offroad_mode != WM_OFFROAD_CULLED) return WM_ERR_UNSUPPORTED;
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaEvent_t ev[3];
+  for (int i = 0; i < 3; ++i) WM_CUDA(cudaEventCreate(&ev[i]));
+  cudaError_t e = wm_launch_rollout_fused_timed(h, *log, *sim, t0, n_steps, actions, action_valid, *out, ev, s);
+  if (e == cudaSuccess) e = cudaEventSynchronize(ev[2]);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms_host[0], ev[0], ev[1]);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms_host[1], ev[1], ev[2]);
+  for (int i = 0; i < 3; ++i) cudaEventDestroy(ev[i]);
+  WM_CUDA(e);
+  return WM_OK;
+}
+
+// Diagnostics for the bench: duration of a register-resident FFMA (packed = 0) or FFMA2 (packed = 1) loop.
+// flop = ctas * 256 * iters * 32 * (packed ? 4 : 2).  Synchronises.
+extern "C" int wm_selftest_ffma(wm_handle* h, int32_t packed, int32_t ctas, int32_t iters, float* ms_host, double* flop_host, void* stream) {
+  if (!h || !ms_host || ctas < 1 || iters < 1) return WM_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaEvent_t a, b;
+  WM_CUDA(cudaEventCreate(&a)); WM_CUDA(cudaEventCreate(&b));
+  cudaError_t e = wm_launch_ffma_peak(h, packed, ctas, iters, (float*)h->cull_stats, s);      // warm-up
+  if (e == cudaSuccess) e = cudaEventRecord(a, s);
+  if (e == cudaSuccess) e = wm_launch_ffma_peak(h, packed, ctas, iters, (float*)h->cull_stats, s);
+  if (e == cudaSuccess) e = cudaEventRecord(b, s);
+  if (e == cudaSuccess) e = cudaEventSynchronize(b);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(ms_host, a, b);
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  WM_CUDA(e);
+  if (flop_host) *flop_host = (double)ctas * 256.0 * (double)iters * 32.0 * (packed ? 4.0 : 2.0);
+  return WM_OK;
+}
+
 // ---------------------------------------------------------------------------------------
 // the same job from host memory
 // ---------------------------------------------------------------------------------------

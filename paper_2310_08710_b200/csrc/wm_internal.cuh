@@ -152,6 +152,7 @@ cudaError_t wm_launch_discretize(wm_handle* h, const wm_action_grid& g, int C, i
                                  const uint8_t* valid, int32_t* index, float* dequant, cudaStream_t s);
 cudaError_t wm_launch_from_index(wm_handle* h, const wm_action_grid& g, int C, int64_t N, int A, const int32_t* index, float* action,
                                  cudaStream_t s);
+cudaError_t wm_launch_ffma_peak(wm_handle* h, int packed, int ctas, int iters, float* sink, cudaStream_t s);
 cudaError_t wm_launch_route_progress(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t, const wm_paths& pa, float* ratio,
                                      uint8_t* valid, cudaStream_t s);
 cudaError_t wm_launch_offroute(wm_handle* h, const wm_traj& sim, int t, const wm_paths& on, const wm_paths* off, float max_dist,
@@ -171,6 +172,10 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s);  
 cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
                                     const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
                                     int b0, cudaStream_t s);
+// the same two launches with events: ev[0] before the dynamics kernel, ev[1] between, ev[2] after the metrics kernel
+cudaError_t wm_launch_rollout_fused_timed(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
+                                          const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
+                                          cudaEvent_t* ev, cudaStream_t s);
 int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);
 int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);   // needs type, id, valid; syncs s
 int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaStream_t s);            // scenarios [b0, b0 + nb), no sync

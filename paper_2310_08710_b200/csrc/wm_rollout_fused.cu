@@ -401,7 +401,14 @@ static inline int fused_launch_batch(int64_t seg_cap) {
 
 static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
                                      const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
-                                     int b0, cudaStream_t s);
+                                     int b0, cudaStream_t s, cudaEvent_t* ev = nullptr);
+
+cudaError_t wm_launch_rollout_fused_timed(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
+                                          const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
+                                          cudaEvent_t* ev, cudaStream_t s) {
+  if (sim.B > fused_launch_batch((int64_t)h->seg_tiles * WM_TILE_SEGS)) return cudaErrorInvalidValue;   // one launch pair only
+  return fused_launch_part(h, log, sim, t0, n_steps, actions, action_valid, out, 0, s, ev);
+}
 
 cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
                                     const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
@@ -432,7 +439,7 @@ cudaError_t wm_launch_rollout_fused(wm_handle* h, const wm_traj& log, const wm_t
 
 static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_traj& sim, int t0, int n_steps,
                                      const float* actions, const uint8_t* action_valid, const wm_rollout_out& out,
-                                     int b0, cudaStream_t s) {
+                                     int b0, cudaStream_t s, cudaEvent_t* ev) {
   FusedParams p;
   p.log = log; p.sim = sim; p.t0 = t0; p.n_steps = n_steps;
   p.C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
@@ -448,11 +455,13 @@ static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_
   // ---- the trajectory ----
   const int nba = (sim.A + DYN_NT - 1) / DYN_NT;
   const int64_t n_dyn = (int64_t)sim.B * nba;
+  if (ev) cudaEventRecord(ev[0], s);
   if (h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE) k_rollout_dyn<WM_DYN_INVERTIBLE_BICYCLE><<<(unsigned)n_dyn, DYN_NT, 0, s>>>(p);
   else k_rollout_dyn<-1><<<(unsigned)n_dyn, DYN_NT, 0, s>>>(p);
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  if (ev) cudaEventRecord(ev[1], s);
   // ---- its metrics ----
   const int Ap = (sim.A + 31) / 32 * 32;
   const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
@@ -469,5 +478,6 @@ static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_
   else if (Ap == 32 && p.S == 8) k_rollout_metrics<32, 8, true><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);
   else k_rollout_metrics<0, 0, true><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);
   h->launches++;
+  if (ev) cudaEventRecord(ev[2], s);
   return cudaGetLastError();
 }

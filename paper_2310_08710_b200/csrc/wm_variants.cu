@@ -171,3 +171,51 @@ cudaError_t wm_launch_from_index(wm_handle* h, const wm_action_grid& g, int C, i
   h->launches++;
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------
+// wm_selftest_ffma: the FP32 peak of this GPU as a register-resident FMA loop can reach it (the
+// denominator SURVEY 8(d) asks to MEASURE in the same run as the brute-force offroad kernel):
+// 8 independent accumulator chains per thread, scalar FFMA or packed FFMA2, no memory traffic.
+// ---------------------------------------------------------------------------------------
+template <bool PACKED>
+__global__ void __launch_bounds__(256) k_ffma_peak(int iters, float seed, float* sink) {
+  float a = seed + (float)threadIdx.x * 1e-6f, b = 0.999f;
+  if (PACKED) {
+    wm_u64 acc[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[j] = pk2(a + (float)j, a - (float)j);
+    const wm_u64 m = pk2(b, b), c = pk2(1e-3f, -1e-3f);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[j] = fma2(acc[j], m, c);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { float lo, hi; upk2(acc[j], lo, hi); s += lo + hi; }
+    if (s == 12345.678f) sink[0] = s;                      // never true: keeps the loop alive
+  } else {
+    float acc[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[j] = a + (float)j;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[j] = fmaf(acc[j], b, 1e-3f);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) s += acc[j];
+    if (s == 12345.678f) sink[0] = s;
+  }
+}
+
+// flops of one launch = CTAs * 256 threads * iters * 32 FMA (* 2 lanes when packed) * 2
+cudaError_t wm_launch_ffma_peak(wm_handle* h, int packed, int ctas, int iters, float* sink, cudaStream_t s) {
+  if (packed) k_ffma_peak<true><<<ctas, 256, 0, s>>>(iters, 1.0f, sink);
+  else k_ffma_peak<false><<<ctas, 256, 0, s>>>(iters, 1.0f, sink);
+  h->launches++;
+  return cudaGetLastError();
+}
