@@ -558,17 +558,3 @@ extern "C" int wm_rollout_host(wm_handle* h, const wm_traj* lh, const wm_roadgra
   return WM_OK;
 }
 
-#ifdef WM_DEBUG_EXPORT
-// development builds only (never in libwm_b200.so): copy one scenario's search structures to the host
-extern "C" int wm_debug_copy_grid(wm_handle* h, int32_t b, void* cells_host, void* pool_host, void* grid_host, void* segrec_host, int32_t* seg_cap) {
-  if (!h || !h->cells) return WM_ERR_STATE;
-  cudaDeviceSynchronize();
-  const int64_t cap = (int64_t)h->seg_tiles * WM_TILE_SEGS;
-  WM_CUDA(cudaMemcpy(cells_host, h->cells + (int64_t)b * WM_GRID_CELLS, sizeof(uint2) * WM_GRID_CELLS, cudaMemcpyDeviceToHost));
-  WM_CUDA(cudaMemcpy(pool_host, h->pool + (int64_t)b * WM_POOL_CAP, sizeof(uint32_t) * WM_POOL_CAP, cudaMemcpyDeviceToHost));
-  WM_CUDA(cudaMemcpy(grid_host, h->gridp + b, sizeof(WmGrid), cudaMemcpyDeviceToHost));
-  if (segrec_host) WM_CUDA(cudaMemcpy(segrec_host, h->segrec + (int64_t)b * cap * 2, sizeof(float4) * 2 * cap, cudaMemcpyDeviceToHost));
-  if (seg_cap) *seg_cap = (int32_t)cap;
-  return WM_OK;
-}
-#endif

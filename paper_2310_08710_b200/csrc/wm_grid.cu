@@ -80,39 +80,18 @@ __device__ __forceinline__ float centre_d2(const float4 r0, const float4 r1, flo
   const float rx = fmaf(-t, r0.z, wx), ry = fmaf(-t, r0.w, wy);
   return fmaf(ry, ry, rx * rx);
 }
-
-// rules P and N below; (cx, cy) cell centre, hh half side of the inflated cell
-__device__ __forceinline__ bool slab_drop(const float4* __restrict__ rec, const int32_t* __restrict__ src, int s, int n,
-                                          const float4 q0, const float4 q1, float cx, float cy, float hh) {
-  const float ex = q0.z, ey = q0.w;
-  if (ex == 0.f && ey == 0.f) return false;                       // isolated point: no slab
-  const float ae = fabsf(ex) + fabsf(ey);
-  const float eps = 2e-3f * ae;                                     // 2 mm along e: far above float32 rounding
-  const int is = __ldg(src + s);
-  const float wx = cx - q0.x, wy = cy - q0.y;
-  const float pc = fmaf(wx, ex, wy * ey);                           // (c - p0).e
-  if (s > 0 && __ldg(src + s - 1) + 1 == is) {                      // rule P (s-1 is a real segment then)
-    const float4 m1 = __ldg(rec + 2 * (s - 1) + 1);
-    if ((m1.x != 0.f || m1.y != 0.f) && pc + hh * ae < -eps) return true;
-  }
-  if (s + 1 < n && __ldg(src + s + 1) == is + 1) {                  // rule N
-    const float4 n0 = __ldg(rec + 2 * (s + 1));
-    const float fx = n0.z, fy = n0.w, af = fabsf(fx) + fabsf(fy);
-    if (af > 0.f) {
-      const float vx = cx - n0.x, vy = cy - n0.y;                   // c - p1, p1 = p0(s+1) as stored
-      const bool beyond = fmaf(vx, ex, vy * ey) - hh * ae > eps;
-      const bool inside_next = fmaf(vx, fx, vy * fy) - hh * af > 2e-3f * af;
-      if (beyond && inside_next) return true;
-    }
-  }
-  return false;
+// The same for the two records of a pair record (P, NE, G: wm_grid.cuh), packed; w = c - p0 comes back too.
+__device__ __forceinline__ void centre_pair_d2(const float4 P, const float4 NE, const float4 G, wm_u64 cx2, wm_u64 cy2,
+                                               wm_u64& wx, wm_u64& wy, float& d_e, float& d_o) {
+  wx = sub2(cx2, pk2(P.x, P.y)); wy = sub2(cy2, pk2(P.z, P.w));
+  const wm_u64 m = mul2(wx, pk2(G.x, G.y));
+  float wy_e, wy_o, m_e, m_o;
+  upk2(wy, wy_e, wy_o); upk2(m, m_e, m_o);
+  const wm_u64 t = pk2(__saturatef(fmaf(wy_e, G.z, m_e)), __saturatef(fmaf(wy_o, G.w, m_o)));
+  const wm_u64 rx = fma2(t, pk2(NE.x, NE.y), wx), ry = fma2(t, pk2(NE.z, NE.w), wy);
+  upk2(fma2(ry, ry, mul2(rx, rx)), d_e, d_o);
 }
 
-// One warp per block of 8 x 4 cells, one lane per cell.  Outer cells (and inner cells under a
-// crowded parent): chunks that cannot hold a candidate of any cell of the block are dropped with one
-// box-box test per chunk (lanes over chunks); the survivors are walked twice with lanes over cells:
-// dmin(c), then the candidate runs.  Inner cells: both passes walk the parent's runs.
-//
 // A record that passes the distance test is still dropped when it can never be the REPORTED
 // nearest segment of any point of the cell (exact in real arithmetic, tested on the four corners
 // of the inflated cell because the conditions are linear in q):
@@ -121,9 +100,36 @@ __device__ __forceinline__ bool slab_drop(const float4* __restrict__ rec, const 
 //   N  the whole cell projects beyond p1 of s AND onto the interior side of s+1, which starts in
 //      that same stored point: then d(q, s+1) < |q - p1| = d(q, s).
 // Along a polyline this leaves the few segments whose perpendicular slab meets the cell (about
-// h/spacing + 2) instead of everything within dmin + 2 rho.
+// h/spacing + 2) instead of everything within dmin + 2 rho.  Whether a rule can apply to a record, the
+// next record's edge vector f and |ex| + |ey| come precomputed per pair record (seglk, k_fill_segments), so
+// the test is a dozen packed operations on w = c - p0 with no further loads and no branches:
+//   P   w.e + hh ae < -eps                          <=>  w.(-e) > kk aP          kk = hh + 2 mm, eps = 2 mm ae
+//   N   (w - e).e - hh ae > eps  and  (w - e).f - hh af > 2 mm af     (w - e = c - p1 up to an ulp of the coordinates)
+// aP / aN are +inf when the rule cannot apply.  Returns the keep flags of the even and the odd record.
+__device__ __forceinline__ void slab_keep(const float4 NE, const float4 L0, const float4 L1, wm_u64 wx, wm_u64 wy, float kk,
+                                          bool& keep_e, bool& keep_o) {
+  const wm_u64 nex = pk2(NE.x, NE.y), ney = pk2(NE.z, NE.w);
+  float pn_e, pn_o, vn_e, vn_o, vf_e, vf_o;
+  upk2(fma2(wy, ney, mul2(wx, nex)), pn_e, pn_o);                        // w.(-e)
+  const wm_u64 vx = add2(wx, nex), vy = add2(wy, ney);                   // c - p1
+  upk2(fma2(vy, ney, mul2(vx, nex)), vn_e, vn_o);                        // (c - p1).(-e)
+  upk2(fma2(vy, pk2(L0.z, L0.w), mul2(vx, pk2(L0.x, L0.y))), vf_e, vf_o);   // (c - p1).f
+  const float af_e = fabsf(L0.x) + fabsf(L0.z), af_o = fabsf(L0.y) + fabsf(L0.w);
+  const bool drop_e = pn_e > kk * L1.x || (-vn_e > kk * L1.z && vf_e > kk * af_e);
+  const bool drop_o = pn_o > kk * L1.y || (-vn_o > kk * L1.w && vf_o > kk * af_o);
+  keep_e = !drop_e; keep_o = !drop_o;
+}
+
+// One warp per block of 8 x 4 cells, one lane per cell.  Outer cells (and inner cells under a
+// crowded parent): chunks that cannot hold a candidate of any cell of the block are dropped with one
+// box-box test per chunk (lanes over chunks); the survivors are walked twice with lanes over cells:
+// dmin(c), then the candidates.  Inner cells: both passes walk the parent's runs.
+//
+// Both passes take the records two by two (pair records, packed arithmetic).  Pass 2 marks the pair
+// records that hold a candidate in a bit mask over the run (or chunk) being walked; the set stretches
+// of the mask are the cell's runs, already in the header's format (first pair << 5 | pairs).
 template <bool FINE>
-__global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* chunks, const int32_t* seg_src,
+__global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* segpair, const float4* seglk, const float4* chunks,
                                                      int seg_cap, const WmGrid* gridp, uint2* cells, uint32_t* pool,
                                                      int32_t* pool_cnt) {
   __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
@@ -138,28 +144,56 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   const int bx = wg % nbx, by = wg / nbx;
   const int ix = bx * 8 + (lane & 7), iy = by * 4 + (lane >> 3);
   const float4* rec = segrec + (int64_t)b * seg_cap * 2;
+  const float4* pair = segpair + (int64_t)b * (seg_cap / 2) * 3;
+  const float4* lk = seglk + (int64_t)b * (seg_cap / 2) * 2;
   const float4* ch = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
-  const int32_t* src = seg_src + (int64_t)b * seg_cap;
   uint2* cells_b = cells + (int64_t)b * WM_GRID_CELLS;
   uint32_t* pool_b = pool + (int64_t)b * WM_POOL_CAP;
   const int n = g.nseg, nch = (n + WM_CHUNK - 1) / WM_CHUNK;
   const float cx = gx0 + ((float)ix + 0.5f) * h, cy = gy0 + ((float)iy + 0.5f) * h;
+  const wm_u64 cx2 = pk2(cx, cx), cy2 = pk2(cy, cy);
   // cell box inflated by delta (float32 rounding of the query's cell index), half diagonal rho
   const float delta = 1e-3f + 1e-4f * h;
   const float hh = 0.5f * h + delta;
+  const float kk = hh + 2e-3f;                                    // rules P / N: half side + 2 mm along the edge
   const float rho = 1.41421362f * hh;
   const bool in = ix < gnx && iy < gny;
   const float INF = __int_as_float(0x7f800000);
 
   float dmin2 = INF;
-  int nr = 0, ncand = 0, rs = 0, rl = 0;
-  auto flush_run = [&]() { if (rl > 0) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = ((uint32_t)rs << 8) | (uint32_t)rl; ++nr; } };
-  auto candidate = [&](int sx, const float4 q0, const float4 q1, float d2, float thr2) {
-    if (in && d2 <= thr2 && !slab_drop(rec, src, sx, n, q0, q1, cx, cy, hh)) {
-      ++ncand;
-      if (rl > 0 && sx == rs + rl && rl < 255) ++rl;
-      else { flush_run(); rs = sx; rl = 1; }
+  int nr = 0, npair = 0;
+  uint32_t open_run = 0u;                                         // the last run, not yet stored: first pair << 5 | pairs
+  // the set stretches of `m` (bit j = pair record first + j holds a candidate) join the cell's runs
+  auto add_mask = [&](uint32_t m, int first) {
+    while (m) {
+      const int a = __ffs(m) - 1;
+      const uint32_t t = ~(m >> a);
+      const int len = t ? __ffs(t) - 1 : 32 - a;
+      m = len + a >= 32 ? 0u : (m & (0xffffffffu << (a + len)));
+      npair += len;
+      int f0 = first + a, left = len;
+      // continue the open run when it ends where this stretch begins
+      if (open_run && (int)(open_run >> 5) + (int)(open_run & 31u) == f0 && (open_run & 31u) < 31u) {
+        const int take = min(left, 31 - (int)(open_run & 31u));
+        open_run += (uint32_t)take; f0 += take; left -= take;
+      }
+      while (left > 0) {
+        if (open_run) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = open_run; ++nr; }
+        const int take = min(left, 31);
+        open_run = ((uint32_t)f0 << 5) | (uint32_t)take; f0 += take; left -= take;
+      }
     }
+  };
+  // pass 2 on one pair record: does it hold a candidate of this cell?
+  auto pair_hit = [&](int pid, float thr2) -> bool {
+    const float4 P = __ldg(pair + 3 * pid), NE = __ldg(pair + 3 * pid + 1), G = __ldg(pair + 3 * pid + 2);
+    const float4 L0 = __ldg(lk + 2 * pid), L1 = __ldg(lk + 2 * pid + 1);
+    wm_u64 wx, wy;
+    float de, dq;
+    bool ke, ko;
+    centre_pair_d2(P, NE, G, cx2, cy2, wx, wy, de, dq);
+    slab_keep(NE, L0, L1, wx, wy, kk, ke, ko);
+    return (de <= thr2 && ke) || (dq <= thr2 && ko);              // padding records (1e18) never pass
   };
   bool done = false;
   if (FINE) {
@@ -171,25 +205,33 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
     uint2 ph = make_uint2(0u, 0u);
     if (in) ph = cells_b[g.obase + wm_cell_index(g.icx0 + (ix >> 2), g.icy0 + (iy >> 2), g.onx)];
     if (!__any_sync(0xffffffffu, (ph.x & ph.y) == 0xffffffffu)) {
-      auto walk = [&](auto&& f) {                       // the parent's pair runs (wm_internal.cuh), record by record
+      auto walk_runs = [&](auto&& f) {                  // the parent's pair runs (wm_internal.cuh): f(first pair, pairs)
         uint32_t r = ph.x & 0x1fffffu, r1 = ((ph.x >> 21) | (ph.y << 11)) & 0x1fffffu, r2 = ph.y >> 10;
         const uint32_t* pl = pool_b;
         int np = 0;
         if (r2 & 0x200000u) { pl += r2 & 0x1fffffu; np = (int)pl[0]; r2 = pl[1]; pl += 2; --np; }
         while (r != 0u) {
-          const int s0 = 2 * (int)(r >> 5), s1 = min(s0 + 2 * (int)(r & 31u), n);
-          for (int sx = s0; sx < s1; ++sx) f(sx);
+          f((int)(r >> 5), (int)(r & 31u));
           r = r1; r1 = r2; r2 = 0u;
           if (np > 0) { r2 = *pl++; --np; }
         }
       };
-      walk([&](int sx) { dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * sx), __ldg(rec + 2 * sx + 1), cx, cy)); });
+      walk_runs([&](int first, int cnt) {
+        for (int q = 0; q < cnt; ++q) {
+          const int pid = first + q;
+          wm_u64 wx, wy;
+          float de, dq;
+          centre_pair_d2(__ldg(pair + 3 * pid), __ldg(pair + 3 * pid + 1), __ldg(pair + 3 * pid + 2), cx2, cy2, wx, wy, de, dq);
+          dmin2 = fminf(dmin2, fminf(de, dq));
+        }
+      });
       const float dmin = sqrtf(dmin2);
       const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
       const float thr2 = thr * thr;
-      walk([&](int sx) {
-        const float4 q0 = __ldg(rec + 2 * sx), q1 = __ldg(rec + 2 * sx + 1);
-        candidate(sx, q0, q1, centre_d2(q0, q1, cx, cy), thr2);
+      walk_runs([&](int first, int cnt) {
+        uint32_t m = 0u;
+        for (int q = 0; q < cnt; ++q) m |= (uint32_t)pair_hit(first + q, thr2) << q;
+        if (in) add_mask(m, first);
       });
       done = true;
     }
@@ -234,6 +276,7 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
     return __ballot_sync(0xffffffffu, sv);
   };
   const int nround = (nch + 31) >> 5;
+  constexpr int CP = WM_CHUNK / 2;                                  // pair records per chunk
 
   {
     // pass 1: dmin(c).  The block's nearest chunk first (a tight start); a chunk is evaluated only
@@ -241,9 +284,14 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
     auto pass1_chunk = [&](int c) {
       const float lb2 = wm_chunk_lb2(__ldg(ch + c), cx, cy);
       if (!__any_sync(0xffffffffu, lb2 < dmin2)) return;
-      const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
 #pragma unroll 4
-      for (int sx = s0; sx < s1; ++sx) dmin2 = fminf(dmin2, centre_d2(__ldg(rec + 2 * sx), __ldg(rec + 2 * sx + 1), cx, cy));
+      for (int q = 0; q < CP; ++q) {
+        const int pid = c * CP + q;
+        wm_u64 wx, wy;
+        float de, dq;
+        centre_pair_d2(__ldg(pair + 3 * pid), __ldg(pair + 3 * pid + 1), __ldg(pair + 3 * pid + 2), cx2, cy2, wx, wy, de, dq);
+        dmin2 = fminf(dmin2, fminf(de, dq));
+      }
     };
     if (nch > 0) pass1_chunk(cmin);
     for (int r = 0; r < nround; ++r) {
@@ -254,7 +302,7 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
         if (c != cmin) pass1_chunk(c);
       }
     }
-    // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack), as runs of consecutive records; chunks whose box is beyond the threshold for every cell of the block are skipped
+    // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack); chunks whose box is beyond the threshold for every cell of the block are skipped
     const float dmin = sqrtf(dmin2);
     const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
     const float thr2 = thr * thr;
@@ -265,61 +313,32 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
         const int c = r * 32 + __ffs(mask) - 1;
         mask &= mask - 1;
         if (!__any_sync(0xffffffffu, wm_chunk_lb2(__ldg(ch + c), cx, cy) <= thr2c)) continue;
-        const int s0 = c * WM_CHUNK, s1 = min(s0 + WM_CHUNK, n);
+        uint32_t m = 0u;
 #pragma unroll 2
-        for (int sx = s0; sx < s1; ++sx) {
-          const float4 q0 = __ldg(rec + 2 * sx), q1 = __ldg(rec + 2 * sx + 1);
-          candidate(sx, q0, q1, centre_d2(q0, q1, cx, cy), thr2);
-        }
+        for (int q = 0; q < CP; ++q) m |= (uint32_t)pair_hit(c * CP + q, thr2) << q;
+        if (in) add_mask(m, c * CP);
       }
     }
   }
   }
-  flush_run();
+  if (open_run) { if (nr < BUILD_MAXRUN) s_runs[warp][nr][lane] = open_run; ++nr; }
   if (!in) return;
-  // query header (wm_internal.cuh): the record runs as runs of pair records (runs that meet in a pair
-  // merge, runs of more than 31 pairs split), three in the header or two + the rest in the pool
+  // query header (wm_internal.cuh): three runs in the header, or two + the rest in the pool
   uint2 hd = make_uint2(0xffffffffu, 0xffffffffu);              // fall back to the full search
   if (n <= 0) hd = make_uint2(0u, 0u);
-  else if (nr <= BUILD_MAXRUN && ncand <= BUILD_MAXCAND) {
-    // in place: s_runs[i] <- (first pair << 12 | pairs), nm merged runs, nq runs after splitting
-    int nm = 0, nq = 0;
-    {
-      int ps = -1, pe = -2;
-      for (int i = 0; i < nr; ++i) {
-        const uint32_t r = s_runs[warp][i][lane];
-        const int f = (int)(r >> 8), c = (int)(r & 255u);
-        const int a = f >> 1, z = (f + c - 1) >> 1;
-        if (a <= pe + 1) pe = max(pe, z);
-        else {
-          if (pe >= ps && ps >= 0) { s_runs[warp][nm][lane] = ((uint32_t)ps << 12) | (uint32_t)(pe - ps + 1); ++nm; nq += (pe - ps + 31) / 31; }
-          ps = a; pe = z;
-        }
-      }
-      if (pe >= ps && ps >= 0) { s_runs[warp][nm][lane] = ((uint32_t)ps << 12) | (uint32_t)(pe - ps + 1); ++nm; nq += (pe - ps + 31) / 31; }
+  else if (nr <= BUILD_MAXRUN && 2 * npair <= BUILD_MAXCAND) {
+    uint32_t f0 = nr > 0 ? s_runs[warp][0][lane] : 0u, f1 = nr > 1 ? s_runs[warp][1][lane] : 0u, f2 = nr > 2 ? s_runs[warp][2][lane] : 0u;
+    bool ok = true;
+    if (nr > 3) {
+      const int off = atomicAdd(&pool_cnt[b], nr - 1);        // count word + (nr - 2) runs
+      if (off + nr - 1 <= WM_POOL_CAP && off < (1 << 21)) {
+        uint32_t* pw = pool_b + off;
+        pw[0] = (uint32_t)(nr - 2);
+        for (int i = 2; i < nr; ++i) pw[i - 1] = s_runs[warp][i][lane];
+        f2 = 0x200000u | (uint32_t)off;
+      } else ok = false;
     }
-    if (nq <= BUILD_MAXRUN) {
-      uint32_t f0 = 0u, f1 = 0u, f2 = 0u;
-      uint32_t* pw = nullptr;
-      bool ok = true;
-      if (nq > 3) {
-        const int off = atomicAdd(&pool_cnt[b], nq - 1);        // count word + (nq - 2) runs
-        if (off + nq - 1 <= WM_POOL_CAP && off < (1 << 21)) { pw = pool_b + off; pw[0] = (uint32_t)(nq - 2); f2 = 0x200000u | (uint32_t)off; }
-        else ok = false;
-      }
-      int k = 0;
-      for (int i = 0; i < nm && ok; ++i) {
-        const uint32_t r = s_runs[warp][i][lane];
-        int first = (int)(r >> 12), left = (int)(r & 4095u);
-        while (left > 0) {
-          const int m = min(left, 31);
-          const uint32_t w = ((uint32_t)first << 5) | (uint32_t)m;
-          if (k == 0) f0 = w; else if (k == 1) f1 = w; else if (pw) pw[k - 1] = w; else f2 = w;
-          ++k; first += m; left -= m;
-        }
-      }
-      if (ok) { hd.x = f0 | (f1 << 21); hd.y = (f1 >> 11) | (f2 << 10); }
-    }
+    if (ok) { hd.x = f0 | (f1 << 21); hd.y = (f1 >> 11) | (f2 << 10); }
   }
   cells_b[(FINE ? 0 : g.obase) + wm_cell_index(ix, iy, gnx)] = hd;
 }
@@ -336,15 +355,16 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const int32_t* src = h->seg_src + (int64_t)b0 * seg_cap;
+  const float4* segpair = h->segpair + (int64_t)b0 * (seg_cap / 2) * 3;
+  const float4* seglk = h->seglk + (int64_t)b0 * (seg_cap / 2) * 2;
   uint2* cells = h->cells + (int64_t)b0 * WM_GRID_CELLS;
   uint32_t* pool = h->pool + (int64_t)b0 * WM_POOL_CAP;
   // the outer grid first: its cells are the parents the inner cells build from
-  k_build_cells<false><<<dim3((WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4) / 8, B), 256, 0, s>>>(segrec, chunks, src, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  k_build_cells<false><<<dim3((WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  k_build_cells<true><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / 8, B), 256, 0, s>>>(segrec, chunks, src, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  k_build_cells<true><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   return cudaGetLastError();
 }

@@ -104,7 +104,7 @@ __device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir
 // One warp per group of 64 stored segments: writes the tile records (brute-force layout), the
 // 32-byte records of the grid search and their pair form, and the bounding box of each chunk of 32.
 __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, const int32_t* n_seg, float4* edges,
-                                                       float2* sign_dir, int32_t* seg_src, float4* segrec, float4* segpair, float4* segfin, float4* chunks) {
+                                                       float2* sign_dir, int32_t* seg_src, float4* segrec, float4* segpair, float4* seglk, float4* segfin, float4* chunks) {
   const int b = blockIdx.y, lane = threadIdx.x & 31;
   const int grp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int ngrp = seg_tiles * (WM_TILE_SEGS / 64);
@@ -117,6 +117,8 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
   float x0 = 3.0e38f, y0 = 3.0e38f, x1 = -3.0e38f, y1 = -3.0e38f;
   float ax[2], ay[2], bx[2], by[2];
   float pp[2][6];                                 // p0x, p0y, -ex, -ey, gx, gy of the lane's two segments
+  float lk[2][4];                                 // fx, fy, aP, aN (wm_internal.cuh: seglk)
+  const float PINF = __int_as_float(0x7f800000);
   bool real[2];
 #pragma unroll
   for (int hf = 0; hf < 2; ++hf) {
@@ -138,6 +140,20 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
       rec[1] = make_float4(gx, gy, sx, sy);
       segfin[(int64_t)b * cap + s] = make_float4(p0x, p0y, sx, sy);
       pp[hf][0] = p0x; pp[hf][1] = p0y; pp[hf][2] = -ex; pp[hf][3] = -ey; pp[hf][4] = gx; pp[hf][5] = gy;
+      // neighbour rules of the cell build (wm_grid.cu): P needs the previous record to be the real segment
+      // that ends in p0, N the next record to be the real segment that starts in p1
+      lk[hf][0] = 0.f; lk[hf][1] = 0.f; lk[hf][2] = PINF; lk[hf][3] = PINF;
+      if (ee > 0.f) {
+        const float ae = fabsf(ex) + fabsf(ey);
+        if (i > 0 && rg_starts(g, o, i - 1)) {
+          const float qx = p0x - g.x[o + i - 1], qy = p0y - g.y[o + i - 1];
+          if (fmaf(qx, qx, qy * qy) > 0.f) lk[hf][2] = ae;
+        }
+        if (rg_starts(g, o, i + 1)) {
+          const float fx = g.x[o + i + 2] - g.x[o + i + 1], fy = g.y[o + i + 2] - g.y[o + i + 1];
+          if (fmaf(fx, fx, fy * fy) > 0.f) { lk[hf][0] = fx; lk[hf][1] = fy; lk[hf][3] = ae; }
+        }
+      }
       ax[hf] = p0x; ay[hf] = p0y; bx[hf] = p0x + ex; by[hf] = p0y + ey;
       x0 = fminf(x0, fminf(ax[hf], bx[hf])); x1 = fmaxf(x1, fmaxf(ax[hf], bx[hf]));
       y0 = fminf(y0, fminf(ay[hf], by[hf])); y1 = fmaxf(y1, fmaxf(ay[hf], by[hf]));
@@ -149,6 +165,7 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
       segfin[(int64_t)b * cap + s] = make_float4(WM_FAR, WM_FAR, 1.f, 0.f);
       src[s] = -1;
       pp[hf][0] = WM_FAR; pp[hf][1] = WM_FAR; pp[hf][2] = 0.f; pp[hf][3] = 0.f; pp[hf][4] = 0.f; pp[hf][5] = 0.f;
+      lk[hf][0] = 0.f; lk[hf][1] = 0.f; lk[hf][2] = PINF; lk[hf][3] = PINF;
     }
   }
   {                                               // the lane's two records as one pair record
@@ -156,6 +173,9 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
     pr[0] = make_float4(pp[0][0], pp[1][0], pp[0][1], pp[1][1]);
     pr[1] = make_float4(pp[0][2], pp[1][2], pp[0][3], pp[1][3]);
     pr[2] = make_float4(pp[0][4], pp[1][4], pp[0][5], pp[1][5]);
+    float4* pl = seglk + ((int64_t)b * (cap / 2) + grp * 32 + lane) * 2;
+    pl[0] = make_float4(lk[0][0], lk[1][0], lk[0][1], lk[1][1]);
+    pl[1] = make_float4(lk[0][2], lk[1][2], lk[0][3], lk[1][3]);
   }
 #pragma unroll
   for (int d = 8; d > 0; d >>= 1) {             // 16 lanes = one chunk of 32 records
@@ -172,9 +192,9 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
 
 void wm_prepare_free(wm_handle* h) {
   cudaFree(h->n_seg); cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->pt_xy); cudaFree(h->pt_idx); cudaFree(h->pt_start); cudaFree(h->pt_grid);
-  cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->segfin); cudaFree(h->chunks); cudaFree(h->gridp); cudaFree(h->cells); cudaFree(h->pool); cudaFree(h->pool_cnt);
+  cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->seglk); cudaFree(h->segfin); cudaFree(h->chunks); cudaFree(h->gridp); cudaFree(h->cells); cudaFree(h->pool); cudaFree(h->pool_cnt);
   h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pt_xy = nullptr; h->pt_idx = nullptr; h->pt_start = nullptr; h->pt_grid = nullptr;
-  h->segrec = nullptr; h->segpair = nullptr; h->segfin = nullptr; h->chunks = nullptr; h->gridp = nullptr; h->cells = nullptr; h->pool = nullptr; h->pool_cnt = nullptr;
+  h->segrec = nullptr; h->segpair = nullptr; h->seglk = nullptr; h->segfin = nullptr; h->chunks = nullptr; h->gridp = nullptr; h->cells = nullptr; h->pool = nullptr; h->pool_cnt = nullptr;
   h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0;
 }
 
@@ -210,13 +230,14 @@ int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_m
   if (e == cudaSuccess) for (int b = 0; b < B; ++b) mx = host[b] > mx ? host[b] : mx;
   free(host);
   WM_CUDA(e);
+  if (mx > WM_MAX_RECORDS) return WM_ERR_UNSUPPORTED;      // pair indices of the cell lists are 16 bits
   h->seg_max = mx;
   int tiles = (mx + WM_TILE_SEGS - 1) / WM_TILE_SEGS;
   if (tiles < 1) tiles = 1;
   if (tiles > h->seg_tiles || !h->edges) {       // grow only: seg_tiles is the row stride of `edges`
     wm_drop_graph(h);
-    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->segfin); cudaFree(h->chunks);
-    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->segrec = nullptr; h->segpair = nullptr; h->segfin = nullptr; h->chunks = nullptr;
+    cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->seglk); cudaFree(h->segfin); cudaFree(h->chunks);
+    h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->segrec = nullptr; h->segpair = nullptr; h->seglk = nullptr; h->segfin = nullptr; h->chunks = nullptr;
     h->seg_tiles = tiles;
     const size_t cap = (size_t)tiles * WM_TILE_SEGS;
     WM_CUDA(cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES));
@@ -224,6 +245,7 @@ int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_m
     WM_CUDA(cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t)));
     WM_CUDA(cudaMalloc(&h->segrec, (size_t)B * cap * 2 * sizeof(float4)));
     WM_CUDA(cudaMalloc(&h->segpair, (size_t)B * (cap / 2) * 3 * sizeof(float4)));
+    WM_CUDA(cudaMalloc(&h->seglk, (size_t)B * (cap / 2) * 2 * sizeof(float4)));
     WM_CUDA(cudaMalloc(&h->segfin, (size_t)B * cap * sizeof(float4)));
     WM_CUDA(cudaMalloc(&h->chunks, (size_t)B * (cap / WM_CHUNK) * sizeof(float4)));
   }
@@ -247,7 +269,7 @@ int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaS
     const int ngrp = tiles * (WM_TILE_SEGS / 64);
     k_fill_segments<<<dim3((ngrp + 7) / 8, nb), 256, 0, s>>>(g, tiles, h->n_seg + b0, h->edges + (int64_t)b0 * tiles * WM_TILE_F4,
                                                              h->sign_dir + b0 * cap, seg_src, h->segrec + b0 * cap * 2,
-                                                             h->segpair + b0 * (cap / 2) * 3, h->segfin + b0 * cap,
+                                                             h->segpair + b0 * (cap / 2) * 3, h->seglk + b0 * (cap / 2) * 2, h->segfin + b0 * cap,
                                                              h->chunks + b0 * (cap / WM_CHUNK));
   }
   h->launches++;
