@@ -2,11 +2,12 @@
 // See wm_grid.cuh for the structure and the argument why no nearest segment can be missed.
 //
 //   k_grid_params        per scenario: bounding box of the segments -> the outer grid (box + wide margin,
-//                        coarse cells) and, aligned with it, the inner grid (box + small margin, each
-//                        outer cell under it split into 4 x 4)
-//   k_build_cells<false> per outer cell: dmin(c), then the runs of records with dist(c, s) <= dmin + 2 rho,
+//                        coarse cells) and, aligned with it, the mid grid (the outer cells under box + small
+//                        margin split 2 x 2) and the inner grid (the mid cells split 2 x 2)
+//   k_build_cells<0>     per outer cell: dmin(c), then the runs of records with dist(c, s) <= dmin + 2 rho,
 //                        from the chunks whose boxes can matter (one warp per 8 x 4 cells)
-//   k_build_cells<true>  per inner cell: the same two passes over its PARENT's list only
+//   k_build_cells<1>     per mid cell: the same two passes over its PARENT's list only
+//   k_build_cells<2>     per inner cell: likewise, over its mid parent's list
 //   k_offroad_grid       one thread per box corner, 4 lanes per agent: header load, candidate walk,
 //                        sign of the winner; max over the corners by shuffles
 //
@@ -21,6 +22,7 @@
 // ======================================================================================
 constexpr int BUILD_MAXRUN = WM_GRID_MAXRUN;   // runs per cell before the cell falls back to the full search
 constexpr int BUILD_MAXCAND = 256;        // candidates per cell before it falls back
+constexpr int BUILD_AHEAD = 8;            // scenarios between a CTA and the one whose records it prefetches into L2
 
 __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const float4* chunks, int seg_cap, float h_min,
                                                      float margin_in, float margin, WmGrid* gridp, int32_t* pool_cnt) {
@@ -45,7 +47,7 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
       x0 = fminf(x0, s_red[0][w]); y0 = fminf(y0, s_red[1][w]); x1 = fmaxf(x1, s_red[2][w]); y1 = fmaxf(y1, s_red[3][w]);
     }
     WmGrid g;
-    g.nseg = n; g.icx0 = 0; g.icy0 = 0;
+    g.nseg = n; g.icx0 = 0; g.icy0 = 0; g.mbase = 0; g.pad0 = 0; g.pad1 = 0; g.pad2 = 0;
     if (n <= 0) {
       g.x0 = 0.f; g.y0 = 0.f; g.h = h_min; g.inv_h = 1.f / h_min; g.nx = 0; g.ny = 0; g.obase = 0;
       g.ox0 = 0.f; g.oy0 = 0.f; g.oh = 4.f * h_min; g.oinv_h = 1.f / g.oh; g.onx = 0; g.ony = 0;
@@ -67,6 +69,7 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
       g.x0 = g.ox0 + (float)cx0 * oh; g.y0 = g.oy0 + (float)cy0 * oh;
       g.nx = 4 * (cx1 - cx0); g.ny = 4 * (cy1 - cy0);
       g.obase = 4 * ((g.nx + 1) >> 1) * ((g.ny + 1) >> 1);
+      g.mbase = g.obase + 4 * ((g.onx + 1) >> 1) * ((g.ony + 1) >> 1);
     }
     gridp[b] = g;
     pool_cnt[b] = 0;
@@ -128,17 +131,32 @@ __device__ __forceinline__ void slab_keep(const float4 NE, const float4 L0, cons
 // Both passes take the records two by two (pair records, packed arithmetic).  Pass 2 marks the pair
 // records that hold a candidate in a bit mask over the run (or chunk) being walked; the set stretches
 // of the mask are the cell's runs, already in the header's format (first pair << 5 | pairs).
-template <bool FINE>
-__global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const float4* segpair, const float4* seglk, const float4* chunks,
+// LEVEL 0: outer cells, 1: mid cells, 2: inner cells
+template <int LEVEL>
+__global__ void __launch_bounds__(256, 4) k_build_cells(const float4* segrec, const float4* segpair, const float4* seglk, const float4* chunks,
                                                      int seg_cap, const WmGrid* gridp, uint2* cells, uint32_t* pool,
                                                      int32_t* pool_cnt) {
   __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
   const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const WmGrid g = gridp[b];
-  // the warp's block of 8 x 4 cells of the outer (FINE = false) or the inner grid
+  // A scenario's records are read by its own CTAs only, all at about the same time: every first touch
+  // would be a DRAM miss in a dependent chain.  Each CTA asks L2 for its share of the pair and link records of
+  // the scenario BUILD_AHEAD places further on (bulk prefetch: no registers, no waiting).
+  if (threadIdx.x == 0 && b + BUILD_AHEAD < (int)gridDim.y) {
+    const int bn = b + BUILD_AHEAD;
+    const uint32_t np = (uint32_t)((gridp[bn].nseg + 1) >> 1), per = (np + gridDim.x - 1) / gridDim.x;
+    const uint32_t p0 = min(np, per * blockIdx.x), p1 = min(np, p0 + per);
+    if (p1 > p0) {
+      l2_prefetch(segpair + ((int64_t)bn * (seg_cap / 2) + p0) * 3, (p1 - p0) * 48u);
+      l2_prefetch(seglk + ((int64_t)bn * (seg_cap / 2) + p0) * 2, (p1 - p0) * 32u);
+    }
+  }
+  // the warp's block of 8 x 4 cells of its level
+  constexpr bool FINE = LEVEL > 0;
   const int wg = blockIdx.x * 8 + warp;
-  const int gnx = FINE ? g.nx : g.onx, gny = FINE ? g.ny : g.ony;
-  const float gx0 = FINE ? g.x0 : g.ox0, gy0 = FINE ? g.y0 : g.oy0, h = FINE ? g.h : g.oh;
+  const int gnx = LEVEL == 0 ? g.onx : LEVEL == 1 ? (g.nx >> 1) : g.nx, gny = LEVEL == 0 ? g.ony : LEVEL == 1 ? (g.ny >> 1) : g.ny;
+  const float gx0 = FINE ? g.x0 : g.ox0, gy0 = FINE ? g.y0 : g.oy0, h = LEVEL == 0 ? g.oh : LEVEL == 1 ? 2.f * g.h : g.h;
+  const int cbase = LEVEL == 0 ? g.obase : LEVEL == 1 ? g.mbase : 0;
   const int nbx = (gnx + 7) >> 3, nby = (gny + 3) >> 2;
   if (wg >= nbx * nby) return;                                  // warp-uniform
   const int bx = wg % nbx, by = wg / nbx;
@@ -197,13 +215,14 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   };
   bool done = false;
   if (FINE) {
-    // Inner cell: its inflated box lies inside its parent's (the outer cell above it, 4 x 4 inner
-    // cells), so every segment that is the reported nearest one of a point of this cell is in the
+    // Mid / inner cell: its inflated box lies inside its parent's (the cell above it, 2 x 2 children),
+    // so every segment that is the reported nearest one of a point of this cell is in the
     // parent's list, and so is the nearest segment of the cell centre: both passes walk the
     // parent's runs (a few dozen records) instead of the surviving chunks.  A crowded parent
     // (no list) sends the warp down the chunk-wise path.
     uint2 ph = make_uint2(0u, 0u);
-    if (in) ph = cells_b[g.obase + wm_cell_index(g.icx0 + (ix >> 2), g.icy0 + (iy >> 2), g.onx)];
+    if (in) ph = LEVEL == 1 ? cells_b[g.obase + wm_cell_index(g.icx0 + (ix >> 1), g.icy0 + (iy >> 1), g.onx)]
+                            : cells_b[g.mbase + wm_cell_index(ix >> 1, iy >> 1, g.nx >> 1)];
     if (!__any_sync(0xffffffffu, (ph.x & ph.y) == 0xffffffffu)) {
       auto walk_runs = [&](auto&& f) {                  // the parent's pair runs (wm_internal.cuh): f(first pair, pairs)
         uint32_t r = ph.x & 0x1fffffu, r1 = ((ph.x >> 21) | (ph.y << 11)) & 0x1fffffu, r2 = ph.y >> 10;
@@ -217,12 +236,17 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
         }
       };
       walk_runs([&](int first, int cnt) {
+        // the next pair record is requested before this one is evaluated
+        const float4* a = pair + 3 * first;
+        float4 P = __ldg(a), NE = __ldg(a + 1), G = __ldg(a + 2);
         for (int q = 0; q < cnt; ++q) {
-          const int pid = first + q;
+          const float4* an = a + (q + 1 < cnt ? 3 : 0);
+          const float4 Pn = __ldg(an), NEn = __ldg(an + 1), Gn = __ldg(an + 2);
           wm_u64 wx, wy;
           float de, dq;
-          centre_pair_d2(__ldg(pair + 3 * pid), __ldg(pair + 3 * pid + 1), __ldg(pair + 3 * pid + 2), cx2, cy2, wx, wy, de, dq);
+          centre_pair_d2(P, NE, G, cx2, cy2, wx, wy, de, dq);
           dmin2 = fminf(dmin2, fminf(de, dq));
+          a = an; P = Pn; NE = NEn; G = Gn;
         }
       });
       const float dmin = sqrtf(dmin2);
@@ -279,20 +303,52 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
   constexpr int CP = WM_CHUNK / 2;                                  // pair records per chunk
 
   {
-    // pass 1: dmin(c).  The block's nearest chunk first (a tight start); a chunk is evaluated only
-    // if its box can still improve some cell of the block.
+    // Both passes run chunk by chunk with the roles turned: the lanes hold the chunk's 16 pair records
+    // (twice: lanes 0-15 and 16-31), and only the cells whose own bound reaches the chunk's box are taken,
+    // two at a time, one per half warp.  A cell far from a chunk that its block neighbours need costs nothing.
+    const int half = lane >> 4, q = lane & 15;
+    auto cell_centre = [&](int i, float& x, float& y) { x = __shfl_sync(0xffffffffu, cx, i); y = __shfl_sync(0xffffffffu, cy, i); };
+    auto half_min = [&](float v) {                          // min over the 16 lanes of a half warp
+#pragma unroll
+      for (int d = 8; d > 0; d >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, d));
+      return v;
+    };
+    // pass 1: dmin(c).  The block's nearest chunk first (a tight start); a cell takes a chunk only if
+    // the chunk's box can still improve it.
     auto pass1_chunk = [&](int c) {
-      const float lb2 = wm_chunk_lb2(__ldg(ch + c), cx, cy);
-      if (!__any_sync(0xffffffffu, lb2 < dmin2)) return;
-#pragma unroll 4
-      for (int q = 0; q < CP; ++q) {
-        const int pid = c * CP + q;
+      uint32_t need = __ballot_sync(0xffffffffu, in && wm_chunk_lb2(__ldg(ch + c), cx, cy) < dmin2);
+      if (!need) return;
+      const int pid = c * CP + q;
+      const float4 P = __ldg(pair + 3 * pid), NE = __ldg(pair + 3 * pid + 1), G = __ldg(pair + 3 * pid + 2);
+      while (need) {
+        const int i0 = __ffs(need) - 1;
+        need &= need - 1;
+        const int i1 = need ? __ffs(need) - 1 : i0;
+        need &= need - 1;                                           // 0 & (0 - 1) = 0
+        float x, y;
+        cell_centre(half ? i1 : i0, x, y);
         wm_u64 wx, wy;
         float de, dq;
-        centre_pair_d2(__ldg(pair + 3 * pid), __ldg(pair + 3 * pid + 1), __ldg(pair + 3 * pid + 2), cx2, cy2, wx, wy, de, dq);
-        dmin2 = fminf(dmin2, fminf(de, dq));
+        centre_pair_d2(P, NE, G, pk2(x, x), pk2(y, y), wx, wy, de, dq);
+        const float mb = half_min(fminf(de, dq));
+        const float m0 = __shfl_sync(0xffffffffu, mb, 0), m1 = __shfl_sync(0xffffffffu, mb, 16);
+        if (lane == i0) dmin2 = fminf(dmin2, m0);
+        if (lane == i1) dmin2 = fminf(dmin2, m1);
       }
     };
+    // a bound for every cell first: its distance to the first and the middle point of every surviving chunk
+    // (lanes over cells, 2 loads per chunk); the chunks that can still improve a cell are then few
+    for (int r = 0; r < nround; ++r) {
+      uint32_t mask = survivors(r);
+      while (mask) {
+        const int c = r * 32 + __ffs(mask) - 1;
+        mask &= mask - 1;
+        const float4 Pa = __ldg(pair + 3 * (c * CP)), Pb = __ldg(pair + 3 * (c * CP + CP / 2));      // p0 of records 32 c and 32 c + 16 (1e18 if padding)
+        const float ax = cx - Pa.x, ay = cy - Pa.z, bx2 = cx - Pb.x, by2 = cy - Pb.z;
+        dmin2 = fminf(dmin2, fminf(fmaf(ax, ax, ay * ay), fmaf(bx2, bx2, by2 * by2)));
+      }
+    }
+    dmin2 = dmin2 * 1.00001f + 1e-6f;                       // the bound is a point distance in other roundings than centre_pair_d2's
     if (nch > 0) pass1_chunk(cmin);
     for (int r = 0; r < nround; ++r) {
       uint32_t mask = survivors(r);
@@ -302,7 +358,7 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
         if (c != cmin) pass1_chunk(c);
       }
     }
-    // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack); chunks whose box is beyond the threshold for every cell of the block are skipped
+    // pass 2: candidates dist(c, s) <= dmin + 2 rho (+ slack)
     const float dmin = sqrtf(dmin2);
     const float thr = dmin + 2.f * rho + (1e-3f + 1e-4f * dmin);
     const float thr2 = thr * thr;
@@ -312,11 +368,31 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
       while (mask) {
         const int c = r * 32 + __ffs(mask) - 1;
         mask &= mask - 1;
-        if (!__any_sync(0xffffffffu, wm_chunk_lb2(__ldg(ch + c), cx, cy) <= thr2c)) continue;
-        uint32_t m = 0u;
-#pragma unroll 2
-        for (int q = 0; q < CP; ++q) m |= (uint32_t)pair_hit(c * CP + q, thr2) << q;
-        if (in) add_mask(m, c * CP);
+        uint32_t need = __ballot_sync(0xffffffffu, wm_chunk_lb2(__ldg(ch + c), cx, cy) <= thr2c);
+        if (!need) continue;
+        const int pid = c * CP + q;
+        const float4 P = __ldg(pair + 3 * pid), NE = __ldg(pair + 3 * pid + 1), G = __ldg(pair + 3 * pid + 2);
+        const float4 L0 = __ldg(lk + 2 * pid), L1 = __ldg(lk + 2 * pid + 1);
+        uint32_t mine = 0u;
+        while (need) {
+          const int i0 = __ffs(need) - 1;
+          need &= need - 1;
+          const int i1 = need ? __ffs(need) - 1 : i0;
+          need &= need - 1;
+          const int i = half ? i1 : i0;
+          float x, y;
+          cell_centre(i, x, y);
+          const float t2 = __shfl_sync(0xffffffffu, thr2, i);
+          wm_u64 wx, wy;
+          float de, dq;
+          bool ke, ko;
+          centre_pair_d2(P, NE, G, pk2(x, x), pk2(y, y), wx, wy, de, dq);
+          slab_keep(NE, L0, L1, wx, wy, kk, ke, ko);
+          const uint32_t bal = __ballot_sync(0xffffffffu, (de <= t2 && ke) || (dq <= t2 && ko));
+          if (lane == i0) mine = bal & 0xffffu;                     // bit j = pair record c * 16 + j holds a candidate of cell i0
+          if (lane == i1 && i1 != i0) mine = bal >> 16;
+        }
+        if (mine) add_mask(mine, c * CP);
       }
     }
   }
@@ -340,7 +416,7 @@ __global__ void __launch_bounds__(256) k_build_cells(const float4* segrec, const
     }
     if (ok) { hd.x = f0 | (f1 << 21); hd.y = (f1 >> 11) | (f2 << 10); }
   }
-  cells_b[(FINE ? 0 : g.obase) + wm_cell_index(ix, iy, gnx)] = hd;
+  cells_b[cbase + wm_cell_index(ix, iy, gnx)] = hd;
 }
 
 cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
@@ -360,11 +436,15 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
   uint2* cells = h->cells + (int64_t)b0 * WM_GRID_CELLS;
   uint32_t* pool = h->pool + (int64_t)b0 * WM_POOL_CAP;
   // the outer grid first: its cells are the parents the inner cells build from
-  k_build_cells<false><<<dim3((WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  k_build_cells<0><<<dim3((WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  k_build_cells<true><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  k_build_cells<1><<<dim3((WM_GRID_NG_IN / 16) * (WM_GRID_NG_IN / 8) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  h->launches++;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_build_cells<2><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   return cudaGetLastError();
 }

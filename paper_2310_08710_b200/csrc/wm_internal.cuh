@@ -30,8 +30,9 @@ constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding seg
 // side >= 2 m) over the segments' bounding box plus a small margin, where nearly all queries land,
 // and a coarse outer grid (<= WM_GRID_NG_OUT^2 cells, side >= 4 x the inner side) over the wide
 // margin that agents reach when they drive off the map.  The inner grid is aligned with the outer
-// one: an outer cell under it is the PARENT of 4 x 4 inner cells, and wm_prepare builds an inner cell's
-// candidates from its parent's list instead of from all segments (wm_grid.cu).  A cell has an 8-byte header of up to three runs of pair records, 21 bits
+// one: an outer cell under it splits into 2 x 2 MID cells (a level that only wm_prepare uses) and each of
+// those into 2 x 2 inner cells; a mid / inner cell takes its candidates from its PARENT's list instead of
+// from all segments (wm_grid.cu).  A cell has an 8-byte header of up to three runs of pair records, 21 bits
 // each (first pair << 5 | pairs, 1 <= pairs <= 31) in bits 0-20, 21-41, 42-62:
 //   bit 63 clear            1-3 runs (unused fields zero); zero = nothing to walk
 //   bit 63 set              two runs, and bits 42-62 = offset into the pool: pool[offset] = n further
@@ -39,17 +40,18 @@ constexpr float WM_FAR = 1.0e18f;          // sentinel coordinate of padding seg
 //   all ones                too many candidates: search all chunks
 // Headers are stored in tiles of 2 x 2 cells (one 32-byte sector = 4 m x 4 m at the default
 // inner cell side), tile-row-major: the four corners of a box and its next steps share sectors.
-// The outer grid's headers follow the inner grid's at cell offset WmGrid::obase.
+// The outer grid's headers follow the inner grid's at cell offset WmGrid::obase, the mid grid's at mbase.
 constexpr int WM_CHUNK = 32;
 constexpr int WM_GRID_NG_IN = 160;
 constexpr int WM_GRID_NG_OUT = 64;
-constexpr int WM_GRID_CELLS = WM_GRID_NG_IN * WM_GRID_NG_IN + WM_GRID_NG_OUT * WM_GRID_NG_OUT;
+constexpr int WM_GRID_CELLS = WM_GRID_NG_IN * WM_GRID_NG_IN + WM_GRID_NG_OUT * WM_GRID_NG_OUT + (WM_GRID_NG_IN / 2) * (WM_GRID_NG_IN / 2);
 constexpr int WM_POOL_CAP = WM_GRID_CELLS;       // words of overflow runs per scenario
 constexpr int WM_GRID_MAXRUN = 16;               // runs per cell before the cell falls back to the full search
 constexpr int WM_MAX_RECORDS = 131072;           // pair indices are 16 bits
 struct WmGrid {
   float x0, y0, inv_h, h; int nx, ny, nseg, obase;        // inner grid; obase = first outer header
   float ox0, oy0, oinv_h, oh; int onx, ony, icx0, icy0;   // outer grid; the inner grid starts at its cell (icx0, icy0)
+  int mbase, pad0, pad1, pad2;                            // mid grid (build only): (nx / 2) x (ny / 2) cells of side 2 h at (x0, y0); first header
 };
 // Prepared roadgraph points for the top-k observation (wm_observe.cu): the valid points of a
 // scenario bucketed into a uniform grid of at most WM_PT_NG x WM_PT_NG cells (side >= 4 m) over
@@ -244,5 +246,9 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
                "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// bulk prefetch of [p, p + bytes) into L2 (bytes % 16 == 0, p 16-byte aligned); fire and forget
+__device__ __forceinline__ void l2_prefetch(const void* p, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 #endif
