@@ -7,19 +7,24 @@
 //
 // k_observe_topk: exact top-k on the float32 key d2 = fma(dy,dy,dx*dx) (the bit pattern of a
 // non-negative float is order preserving; DESIGN.md R-topk).  wm_prepare buckets the valid points of
-// a scenario into a uniform grid (k_point_grid).  One 128-thread CTA per ego:
+// a scenario into a uniform grid (k_point_grid).  One 128-thread CTA per ego (9 CTAs per SM; 256 threads
+// were measured slower: the phases are short and a barrier then waits on more warps):
 //   0. the square of cells around the ego's cell that holds ~1.6 k points (cell counts only);
-//   1. histogram of the keys' top bits over the points of that square (shared-memory atomics)
-//      -> bin of the k-th key (repeated on the bin's sub-range only if the bin is too large);
-//   2. collect the (key, index) pairs of that bin (<= 512) -> bitwise descent gives the exact k-th
-//      key T and the number of ties to take;
+//   1. ONE pass over the points of that square: keys -> shared memory (squares of up to 3072 points; the
+//      later passes read them there), histogram of their top bits (1024 bins: exponent + 5 mantissa bits,
+//      shared-memory atomics) -> bin of the k-th key (a 256-bin pass on the bin's sub-range only if it
+//      holds more than 512 keys);
+//   2. collect the keys of that bin (<= 512) -> 8-bit descents give the exact k-th key T, the number of
+//      keys equal to it and the number of those to take;
 //   3. every point outside a square of m rings is farther than m h, so if sqrt(T) < m h the k
 //      nearest points of the square are the k nearest of the scenario; otherwise the square grows
 //      to hold the disc of radius sqrt(T) and 1-2 run again (T of a subset is never too small);
-//   4. mark key < T in a bitmap over the roadgraph indices, key == T in a second one; the first
-//      `quota` tie bits in index order join (ties -> lower index, D23);
-//   5. emit the set bits in ascending index order (block scan of popcounts) with ego-frame features.
-// It reads ~2.3 k of the scenario's 30 k points per ego instead of all of them three times.
+//   4. mark key < T (and == T when every tie is taken, the usual case) in a bitmap over the roadgraph
+//      indices and append the index to an unordered list (warp-aggregated); otherwise the ties go to a
+//      bitmap of their own and the first `quota` of them in index order join (ties -> lower index, D23);
+//   5. ascending index order without walking the bitmap: prefix sums of the words' popcounts, then every
+//      listed index finds its rank with one popc and is stored at that place; ego-frame features follow.
+// It reads ~2.3 k of the scenario's 30 k points per ego once instead of all of them three times.
 #include "wm_internal.cuh"
 
 // ======================================================================================
@@ -193,9 +198,11 @@ cudaError_t wm_launch_point_grid(wm_handle* h, const wm_roadgraph& rg, int b0, i
 }
 
 constexpr int TK_THREADS = 128;              // one CTA per ego
-constexpr int TK_BINS = 256;
-constexpr int TK_CAP = 512;                  // boundary (key, index) pairs
-constexpr int TK_BASE = 119 << 3;            // level-0 bins start at d2 = 2^-8, 3 mantissa bits per bin
+constexpr int TK_BINS = 1024;                // level-0 bins: exponent + 5 mantissa bits
+constexpr int TK_SH0 = 18;
+constexpr int TK_CAP = 512;                  // boundary (key, position) pairs
+constexpr int TK_BASE = 119 << 5;            // level-0 bins start at d2 = 2^-8
+constexpr int TK_KEYS = 2560;                // keys of the square kept in shared memory (larger squares recompute them)
 
 struct TopkParams {
   wm_row row;
@@ -205,16 +212,16 @@ struct TopkParams {
   int32_t* rg_index; float* rg_feat; int32_t* rg_type;
 };
 
-__device__ __forceinline__ int tk_bin0(uint32_t key) { return min(max((int)(key >> 20) - TK_BASE, 0), TK_BINS - 1); }
-__device__ __forceinline__ uint32_t tk_bin0_lo(int bin) { return bin <= 0 ? 0u : (uint32_t)(bin + TK_BASE) << 20; }
-__device__ __forceinline__ uint32_t tk_bin0_hi(int bin) { return bin >= TK_BINS - 1 ? 0xffffffffu : (uint32_t)(bin + TK_BASE + 1) << 20; }
+__device__ __forceinline__ int tk_bin0(uint32_t key) { return min(max((int)(key >> TK_SH0) - TK_BASE, 0), TK_BINS - 1); }
+__device__ __forceinline__ uint32_t tk_bin0_lo(int bin) { return bin <= 0 ? 0u : (uint32_t)(bin + TK_BASE) << TK_SH0; }
+__device__ __forceinline__ uint32_t tk_bin0_hi(int bin) { return bin >= TK_BINS - 1 ? 0xffffffffu : (uint32_t)(bin + TK_BASE + 1) << TK_SH0; }
 
 struct TkShared {
-  uint32_t hist[TK_BINS];
-  uint2 col[TK_CAP];
   int scan[TK_THREADS / 32];
   uint32_t lo, hi, T;            // undecided key range [lo, hi); exact threshold
-  int shift, c_less, in_bin, n_col, quota, m, count, again, n_tie;
+  int shift, c_less, in_bin, n_col, quota, m, count, again, n_tie, n_sel, n_rows;
+  int row_s0[WM_PT_NG];          // the square's rows of cells: first sorted point of the row,
+  int row_base[WM_PT_NG + 1];    //   and its position in the square's own numbering (prefix counts)
 };
 
 // exclusive prefix sum of v over the CTA; total in `total`
@@ -232,40 +239,50 @@ __device__ __forceinline__ int tk_block_scan(int v, int* s_scan, int& total) {
   return base + inc - v;
 }
 
-// warp 0, after a histogram pass: the bin that holds rank `need` (1-based) of the current range
-__device__ __forceinline__ void tk_locate(TkShared& S, int need, bool level0) {
+// warp 0, after a histogram pass over `nbins` bins: the bin that holds rank `need` (1-based) of the current range
+template <int NBINS>
+__device__ __forceinline__ void tk_locate(TkShared& S, const uint32_t* hist, int need, bool level0) {
   const int lane = threadIdx.x & 31;
-  constexpr int PER = TK_BINS / 32;
-  int tot[PER], mine = 0;
+  constexpr int per = NBINS >> 5;
+  int mine = 0;
+  {
+    const uint4* h4 = (const uint4*)(hist + lane * per);
 #pragma unroll
-  for (int q = 0; q < PER; ++q) { tot[q] = (int)S.hist[lane * PER + q]; mine += tot[q]; }
+    for (int q = 0; q < per / 4; ++q) { const uint4 v = h4[q]; mine += (int)(v.x + v.y + v.z + v.w); }
+  }
   int inc = mine;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += u; }
   const uint32_t has = __ballot_sync(0xffffffffu, inc >= need);
   const int L = has ? __ffs(has) - 1 : 31;
-  int ex = inc - mine, bq = PER - 1, cq = 0, found = 0;
-#pragma unroll
-  for (int q = 0; q < PER; ++q) if (!found) { if (ex + tot[q] >= need) { bq = q; cq = tot[q]; found = 1; } else ex += tot[q]; }
-  const int bin = __shfl_sync(0xffffffffu, lane * PER + bq, L);
-  const int below = __shfl_sync(0xffffffffu, ex, L);
-  const int cnt = __shfl_sync(0xffffffffu, cq, L);
-  if (lane == 0) {
+  if (lane == L) {
+    int ex = inc - mine, bin = lane * per + per - 1, cnt = 0;
+    for (int q = 0; q < per; ++q) {
+      const int t = (int)hist[lane * per + q];
+      if (ex + t >= need || q == per - 1) { bin = lane * per + q; cnt = t; break; }
+      ex += t;
+    }
     if (level0) { S.lo = tk_bin0_lo(bin); S.hi = tk_bin0_hi(bin); }
     else { const uint32_t base = S.lo; S.lo = base + ((uint32_t)bin << S.shift); S.hi = min(S.hi, base + ((uint32_t)(bin + 1) << S.shift)); }
-    S.c_less += below;
+    S.c_less += ex;
     S.in_bin = cnt;
   }
 }
 
 __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
-  extern __shared__ __align__(16) uint32_t s_bits[];     // [2][Wd]: key < T; key == T (ties); then [k] indices
+  extern __shared__ __align__(16) uint32_t s_dyn[];
   __shared__ TkShared S;
   const int b = blockIdx.y, ego = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int A = p.A, k = p.k, R = p.R, Wd = (R + 31) >> 5;
-  uint32_t* bm = s_bits;
-  uint32_t* tb = s_bits + Wd;
-  int* list = (int*)(s_bits + 2 * Wd);                    // [k] selected indices, ascending
+  const int Wd4 = (Wd + 3) & ~3;                          // 16-byte aligned pieces
+  uint32_t* bm = s_dyn;                                   // [Wd] key < T (and the ties that join)
+  uint32_t* tb = bm + Wd4;                                // [Wd] key == T (only when some ties stay out); later:
+  uint32_t* pre = tb;                                     //   [Wd] set bits of bm before word w
+  uint32_t* keys = tb + Wd4;                              // [max(TK_KEYS, k)] keys of the square, in its order; later:
+  int* list = (int*)keys;                                 //   [k] the selected indices, ascending
+  uint32_t* const hist = keys + ((max(TK_KEYS, k) + 3) & ~3);   // [TK_BINS] histogram, [TK_CAP] keys of the k-th key's bin; later:
+  uint32_t* const col = hist + TK_BINS;
+  int* sel = (int*)hist;                                  //   [k] the selected indices as they were found
   const int64_t ro = (int64_t)b * p.row.stride_b;
   const int64_t oi = ((int64_t)b * A + ego) * k;          // rg_index / rg_type row
   float* feat = p.rg_feat + ((int64_t)b * A + ego) * 4 * k;
@@ -296,82 +313,109 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
     for (int j = j0 + lane; j <= j1; j += 32) c += __ldg(start + j * g.nx + i1 + 1) - __ldg(start + j * g.nx + i0);
     return __reduce_add_sync(0xffffffffu, c);
   };
+  // the rows of the square of m rings in shared memory: a pass then runs over the square's points as one
+  // flat range instead of row by row (warp 0)
+  auto set_rows = [&](int m) {
+    const int i0 = max(ci - m, 0), i1 = min(ci + m, g.nx - 1), j0 = max(cj - m, 0), j1 = min(cj + m, g.ny - 1);
+    const int nr = j1 - j0 + 1;                           // <= WM_PT_NG = 64
+    int run = 0;
+#pragma unroll
+    for (int r0 = 0; r0 < WM_PT_NG; r0 += 32) {
+      const int r = r0 + lane;
+      int s0 = 0, c = 0;
+      if (r < nr) { s0 = __ldg(start + (j0 + r) * g.nx + i0); c = __ldg(start + (j0 + r) * g.nx + i1 + 1) - s0; }
+      int inc = c;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += u; }
+      S.row_s0[r] = s0; S.row_base[r] = run + inc - c;
+      run += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) { S.row_base[WM_PT_NG] = run; S.m = m; S.count = run; S.n_rows = nr; }
+  };
   if (warp == 0) {                                        // 0. the first square: ~1.6 k points
     const int want = min(g.nvalid, kk + (kk * 60) / 100);
     // lanes over m = 0..31 (independent loads), then one m at a time
+    // m = 0..15 first, two lanes per m (the rows of a square split in halves: independent loads)
     int c = 0;
     {
-      const int m = lane;
+      const int m = lane >> 1;
       const int i0 = max(ci - m, 0), i1 = min(ci + m, g.nx - 1), j0 = max(cj - m, 0), j1 = min(cj + m, g.ny - 1);
-      for (int j = j0; j <= j1; ++j) c += __ldg(start + j * g.nx + i1 + 1) - __ldg(start + j * g.nx + i0);
+      for (int j = j0 + (lane & 1); j <= j1; j += 2) c += __ldg(start + j * g.nx + i1 + 1) - __ldg(start + j * g.nx + i0);
+      c += __shfl_xor_sync(0xffffffffu, c, 1);
     }
     const uint32_t ok = __ballot_sync(0xffffffffu, c >= want);
-    int m = ok ? __ffs(ok) - 1 : 32;
-    c = __shfl_sync(0xffffffffu, c, m & 31);
+    int m = ok ? (__ffs(ok) - 1) >> 1 : 16;
     if (!ok) for (;; ++m) { c = square_count(m); if (c >= want || m >= WM_PT_NG) break; }
-    if (lane == 0) { S.m = m; S.count = c; }
+    set_rows(m);
   }
-  for (int i = tid; i < 2 * Wd; i += TK_THREADS) s_bits[i] = 0u;
-  if (tid == 0) S.n_tie = 0;
+  for (int i = tid; i < 2 * Wd4; i += TK_THREADS) s_dyn[i] = 0u;
+  if (tid == 0) { S.n_tie = 0; S.n_sel = 0; }
   __syncthreads();
 
-  // one pass over the points of the current square: f(key, sorted position)
-  auto for_square = [&](auto&& f) {
-    const int m = S.m;
-    const int i0 = max(ci - m, 0), i1 = min(ci + m, g.nx - 1), j0 = max(cj - m, 0), j1 = min(cj + m, g.ny - 1);
-    for (int j = j0; j <= j1; ++j) {
-      const int s0 = __ldg(start + j * g.nx + i0), s1 = __ldg(start + j * g.nx + i1 + 1);
-      for (int s = s0 + tid; s < s1; s += TK_THREADS) {
-        const float2 pt = __ldg(pxy + s);
-        const float dx = __fsub_rn(pt.x, ex), dy = __fsub_rn(pt.y, ey);
-        f(__float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx))), s);
+  // One pass over the points of the current square, numbered 0 .. count - 1 row after row: f(key, position).
+  // The first pass of a square (fill) computes the keys, a warp per row of cells, and keeps them in shared
+  // memory when the square fits; the later ones read them there as one flat range.
+  bool cached = false;
+  auto key_at = [&](int s) {
+    const float2 pt = __ldg(pxy + s);
+    const float dx = __fsub_rn(pt.x, ex), dy = __fsub_rn(pt.y, ey);
+    return __float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+  };
+  auto for_square = [&](bool fill, auto&& f) {
+    if (cached && !fill) { const int count = S.count; for (int j = tid; j < count; j += TK_THREADS) f(keys[j], j); return; }
+    const int nr = S.n_rows;
+    for (int r = warp; r < nr; r += TK_THREADS / 32) {
+      const int s0 = S.row_s0[r], base = S.row_base[r], cnt = S.row_base[r + 1] - base;
+      for (int i = lane; i < cnt; i += 32) {
+        const uint32_t key = key_at(s0 + i);
+        if (cached) keys[base + i] = key;
+        f(key, base + i);
       }
     }
   };
 
   for (;;) {
     // ---- 1. level-0 histogram, bin of the kk-th key ----
-    for (int i = tid; i < TK_BINS; i += TK_THREADS) S.hist[i] = 0u;
+    for (int i = tid; i < TK_BINS; i += TK_THREADS) hist[i] = 0u;
     if (tid == 0) { S.lo = 0u; S.hi = 0xffffffffu; S.c_less = 0; S.n_col = 0; S.shift = 0; }
+    cached = S.count <= TK_KEYS;
     __syncthreads();
-    for_square([&](uint32_t key, int) { atomicAdd(&S.hist[tk_bin0(key)], 1u); });
+    for_square(true, [&](uint32_t key, int) { atomicAdd(&hist[tk_bin0(key)], 1u); });
     __syncthreads();
-    if (warp == 0) tk_locate(S, kk, true);
+    if (warp == 0) tk_locate<TK_BINS>(S, hist, kk, true);
     __syncthreads();
     // ---- refine while the bin is too large for the collect buffer ----
     while (S.in_bin > TK_CAP && S.hi - S.lo > 1u) {
       const uint32_t lo = S.lo, hi = S.hi;
       const int shift = max(0, 32 - __clz(hi - lo - 1u) - 8);           // (span - 1) >> shift < 256
       __syncthreads();
-      for (int i = tid; i < TK_BINS; i += TK_THREADS) S.hist[i] = 0u;
+      for (int i = tid; i < 256; i += TK_THREADS) hist[i] = 0u;
       if (tid == 0) S.shift = shift;
       __syncthreads();
-      for_square([&](uint32_t key, int) { if (key >= lo && key < hi) atomicAdd(&S.hist[(key - lo) >> shift], 1u); });
+      for_square(false, [&](uint32_t key, int) { if (key >= lo && key < hi) atomicAdd(&hist[(key - lo) >> shift], 1u); });
       __syncthreads();
-      if (warp == 0) tk_locate(S, kk - S.c_less, false);
+      if (warp == 0) tk_locate<256>(S, hist, kk - S.c_less, false);
       __syncthreads();
     }
-    // ---- 2. collect the bin, then narrow [lo, hi) to one key value on the collected pairs ----
+    // ---- 2. collect the bin, then narrow [lo, hi) to one key value on the collected keys ----
     {
       const uint32_t lo = S.lo, hi = S.hi;
-      if (S.in_bin <= TK_CAP && hi - lo > 1u) for_square([&](uint32_t key, int s) {
-        if (key >= lo && key < hi) { const int q = atomicAdd(&S.n_col, 1); if (q < TK_CAP) S.col[q] = make_uint2(key, (uint32_t)s); }
+      if (S.in_bin <= TK_CAP && hi - lo > 1u) for_square(false, [&](uint32_t key, int s) {
+        if (key >= lo && key < hi) { const int q = atomicAdd(&S.n_col, 1); if (q < TK_CAP) col[q] = key; }
       });
       __syncthreads();
     }
-    while (S.hi - S.lo > 1u) {                            // in_bin <= TK_CAP here: all of the range is in col
-      const uint32_t lo = S.lo, hi = S.hi;
-      const int shift = max(0, 32 - __clz(hi - lo - 1u) - 8), n_col = min(S.n_col, TK_CAP);
-      __syncthreads();
-      for (int i = tid; i < TK_BINS; i += TK_THREADS) S.hist[i] = 0u;
-      if (tid == 0) S.shift = shift;
-      __syncthreads();
+    {                                                     // in_bin <= TK_CAP here: all of the range is in col
+      // the kk-th key by counting: the collected key with c smaller and e equal ones, c < need <= c + e
+      const bool open_range = S.hi - S.lo > 1u;
+      const int n_col = open_range ? min(S.n_col, TK_CAP) : 0, need = kk - S.c_less;
+      __syncthreads();                                    // everyone has read the range before a winner rewrites it
       for (int i = tid; i < n_col; i += TK_THREADS) {
-        const uint32_t key = S.col[i].x;
-        if (key >= lo && key < hi) atomicAdd(&S.hist[(key - lo) >> shift], 1u);
+        const uint32_t mine = col[i];
+        int c = 0, e = 0;
+        for (int j = 0; j < n_col; ++j) { const uint32_t o = col[j]; c += o < mine; e += o == mine; }
+        if (c < need && need <= c + e) { S.lo = mine; S.hi = mine + 1u; S.c_less = kk - need + c; S.in_bin = e; }   // every writer stores the same values
       }
-      __syncthreads();
-      if (warp == 0) tk_locate(S, kk - S.c_less, false);
       __syncthreads();
     }
     if (warp == 0) {
@@ -386,84 +430,93 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
       if (!all && !(dT < reach)) {
         int m2 = max(m + 1, (int)ceilf((dT + tol) * g.inv_h) + 1);
         m2 = min(m2, WM_PT_NG);
-        const int c = square_count(m2);
-        if (lane == 0) { S.m = m2; S.count = c; }
+        set_rows(m2);
         again = 1;
       }
-      if (lane == 0) { S.T = T; S.quota = r; S.again = again; }   // r = ties (key == T) to take, in index order
+      if (lane == 0) { S.T = T; S.quota = r; S.again = again; S.n_tie = S.in_bin; }   // r = ties (key == T) to take, in index order; in_bin = all ties
     }
     __syncthreads();
     if (!S.again) break;
     __syncthreads();
   }
 
-  // ---- 4. mark the selected points over the roadgraph indices ----
+  // ---- 4. mark the selected points over the roadgraph indices and list them as they come ----
+  // Nearly always every tie is taken (n_tie == quota); otherwise the ties go to a bitmap of their own, are
+  // trimmed in index order and join afterwards.
   const uint32_t T = S.T;
-  for_square([&](uint32_t key, int s) {
-    if (key <= T) {
-      const int idx = __ldg(pidx + s);
-      atomicOr((key < T ? bm : tb) + (idx >> 5), 1u << (idx & 31));
-      if (key == T) atomicAdd(&S.n_tie, 1);
+  const int quota = S.quota;
+  const bool trim = S.n_tie > quota;
+  {
+    const int nr = S.n_rows;
+    for (int r = warp; r < nr; r += TK_THREADS / 32) {        // a warp per row of cells; appends are warp-aggregated
+      const int s0 = S.row_s0[r], base = S.row_base[r], cnt = S.row_base[r + 1] - base;
+      for (int ib = 0; ib < cnt; ib += 32) {
+        const int i = ib + lane;
+        bool take = false, tie = false;
+        if (i < cnt) {
+          const uint32_t key = cached ? keys[base + i] : key_at(s0 + i);
+          take = key < T || (key == T && !trim);
+          tie = key == T && trim;
+        }
+        const uint32_t bal = __ballot_sync(0xffffffffu, take);
+        if (take || tie) {
+          const int idx = __ldg(pidx + s0 + i);
+          atomicOr((take ? bm : tb) + (idx >> 5), 1u << (idx & 31));
+          if (take) {
+            int q0 = 0;
+            const int leader = __ffs(bal) - 1;
+            if (lane == leader) q0 = atomicAdd(&S.n_sel, __popc(bal));
+            q0 = __shfl_sync(bal, q0, leader);
+            const int q = q0 + __popc(bal & ((1u << lane) - 1u));
+            if (q < k) sel[q] = idx;
+          }
+        }
+      }
     }
-  });
+  }
   __syncthreads();
-  // The first `quota` ties in index order join the selection.  Nearly always every tie is taken
-  // (n_tie == quota); otherwise the tie words are trimmed in index order, word r * 128 + tid in round r.
-  const int quota = S.quota, n_tie = S.n_tie;
-  const bool trim = n_tie > quota;
   if (trim) {
+    // the first `quota` ties in index order join: word r * TK_THREADS + tid in round r
     const int rounds = (Wd + TK_THREADS - 1) / TK_THREADS;
-    int base = 0;
+    int basec = 0;
     for (int r = 0; r < rounds; ++r) {
       const int w = r * TK_THREADS + tid;
       uint32_t t = w < Wd ? tb[w] : 0u;
       const int n = __popc(t);
       int tot_r;
-      const int left = quota - (base + tk_block_scan(n, S.scan, tot_r));
+      const int left = quota - (basec + tk_block_scan(n, S.scan, tot_r));
       if (left < n) { for (int drop = n - max(left, 0); drop > 0; --drop) t &= ~(0x80000000u >> __clz(t)); }   // keep the lowest bits
-      if (w < Wd) bm[w] |= t;
-      base += tot_r;
+      if (w < Wd) {
+        bm[w] |= t;
+        while (t) { const int q = atomicAdd(&S.n_sel, 1); if (q < k) sel[q] = w * 32 + __ffs(t) - 1; t &= t - 1; }
+      }
+      basec += tot_r;
     }
     __syncthreads();
   }
-  // ---- 5. the set bits in ascending index order -> list, then features with coalesced stores ----
-  // Each warp owns a contiguous quarter of the words, its lanes interleaved over them (the selected
-  // points cluster in index ranges - polylines near the ego - and this spreads a cluster over the
-  // lanes); positions come from one exchange of the warp totals and shuffle scans, no block barrier.
-  const int Q = (Wd + TK_THREADS / 32 - 1) / (TK_THREADS / 32), wb = warp * Q, we = min(wb + Q, Wd);
+  // ---- 5. rank of every selected index = set bits of bm below it: word prefix sums, then one popc each ----
   {
+    const int PW = (Wd + TK_THREADS - 1) / TK_THREADS;      // consecutive words per thread
     int c = 0;
-    for (int w = wb + lane; w < we; w += 32) {
-      uint32_t v = bm[w];
-      if (!trim) { v |= tb[w]; bm[w] = v; }
-      c += __popc(v);
-    }
-    c = __reduce_add_sync(0xffffffffu, c);
-    if (lane == 0) S.scan[warp] = c;
+    for (int q = 0; q < PW; ++q) { const int w = tid * PW + q; if (w < Wd) c += __popc(bm[w]); }
+    int tot;
+    int run = tk_block_scan(c, S.scan, tot);
+    for (int q = 0; q < PW; ++q) { const int w = tid * PW + q; if (w < Wd) { pre[w] = (uint32_t)run; run += __popc(bm[w]); } }
+  }
+  __syncthreads();                                          // keys are dead from here on: list takes their place
+  const int n_out = min(S.n_sel, k);
+  for (int i = tid; i < n_out; i += TK_THREADS) {
+    const int idx = sel[i], w = idx >> 5;
+    const int pos = (int)pre[w] + __popc(bm[w] & ((1u << (idx & 31)) - 1u));
+    if (pos < k) list[pos] = idx;
   }
   __syncthreads();
-  int run = 0, n_out = 0;
-#pragma unroll
-  for (int w = 0; w < TK_THREADS / 32; ++w) { const int t = S.scan[w]; if (w < warp) run += t; n_out += t; }
-  for (int w0 = wb; w0 < we; w0 += 32) {
-    const int w = w0 + lane;
-    uint32_t bits = w < we ? bm[w] : 0u;
-    const int n = __popc(bits);
-    int inc = n;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += u; }
-    int pos = run + inc - n;
-    while (bits) { if (pos < k) list[pos] = w * 32 + __ffs(bits) - 1; ++pos; bits &= bits - 1; }
-    run += __shfl_sync(0xffffffffu, inc, 31);
-  }
-  __syncthreads();
-  n_out = min(n_out, k);
   const float *gx = p.x + (int64_t)b * R, *gy = p.y + (int64_t)b * R, *gdx = p.dir_x + (int64_t)b * R, *gdy = p.dir_y + (int64_t)b * R;
   const int32_t* gt = p.type + (int64_t)b * R;
   if (p.by_distance) {
     // WM_TOPK_BY_DISTANCE (D44): the selected points by ascending (key, index) - a bitonic sort of
     // (key bits << 32 | index) in shared memory, padded to a power of two with all-ones
-    unsigned long long* sk = (unsigned long long*)(s_bits + ((2 * Wd + k + 1) & ~1));
+    unsigned long long* sk = (unsigned long long*)(hist + ((max(TK_BINS + TK_CAP, k) + 1) & ~1));
     int P = 1;
     while (P < n_out) P <<= 1;
     for (int j = tid; j < P; j += TK_THREADS) {
@@ -511,14 +564,16 @@ cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_ro
   p.pt_xy = h->pt_xy; p.pt_idx = h->pt_idx; p.pt_start = h->pt_start; p.pt_grid = h->pt_grid;
   p.x = rg.x; p.y = rg.y; p.dir_x = rg.dir_x; p.dir_y = rg.dir_y; p.type = rg.type;
   p.rg_index = rg_index; p.rg_feat = rg_feat; p.rg_type = rg_type;
-  size_t smem = (2 * (size_t)((rg.R + 31) / 32) + (size_t)h->cfg.topk) * sizeof(uint32_t);
+  const size_t kq = (size_t)h->cfg.topk;
+  const size_t hcq = (size_t)(TK_BINS + TK_CAP), wd4 = ((size_t)((rg.R + 31) / 32) + 3) & ~(size_t)3;
+  size_t smem = (2 * wd4 + (((kq > (size_t)TK_KEYS ? kq : (size_t)TK_KEYS) + 3) & ~(size_t)3) + (((kq > hcq ? kq : hcq) + 1) & ~(size_t)1)) * sizeof(uint32_t);
   if (p.by_distance) {                                        // + the sort keys: 8 B x the power of two >= k
     size_t P = 1;
     while (P < (size_t)h->cfg.topk) P <<= 1;
-    smem = ((smem + 7) & ~(size_t)7) + P * sizeof(unsigned long long);
+    smem += P * sizeof(unsigned long long);
   }
-  if (smem > 200 * 1024) return cudaErrorInvalidValue;       // R > 819 200 points per scenario
-  if (smem > 40 * 1024) {                                     // per-device attribute: set whenever a launch needs it (cheap)
+  if (smem > 200 * 1024) return cudaErrorInvalidValue;       // R > ~500 000 points per scenario
+  if (smem > 24 * 1024) {                                     // per-device attribute: set whenever a launch needs it (cheap)
     cudaError_t e = cudaFuncSetAttribute(k_observe_topk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
