@@ -319,6 +319,20 @@ __device__ __forceinline__ float seg_d2(float wx, float wy, float ex, float ey, 
   return fmaf(ry, ry, rx * rx);
 }
 
+// exact ties across lanes (rare): the lowest stored position, among the lane's 16 segments of a tile, whose
+// distance^2 has the bits m; kept out of line so that it costs the scan no registers
+__device__ __noinline__ uint32_t tie_position(const float4* tp, int lane, float cx, float cy, float ox, float oy, float sgn, uint32_t m) {
+  uint32_t pos = 0xffffffffu;
+  for (int it = 7; it >= 0; --it) {
+    const float4 P = __ldg(&tp[(it * 3 + 0) * 32]), E = __ldg(&tp[(it * 3 + 1) * 32]), Gv = __ldg(&tp[(it * 3 + 2) * 32]);
+    const float d1 = seg_d2(fmaf(sgn, ox, cx - P.y), fmaf(sgn, oy, cy - P.w), E.y, E.w, Gv.y, Gv.w);
+    const float d0 = seg_d2(fmaf(sgn, ox, cx - P.x), fmaf(sgn, oy, cy - P.z), E.x, E.z, Gv.x, Gv.z);
+    if (__float_as_uint(d1) == m) pos = (uint32_t)(it * 64 + 2 * lane + 1);
+    if (__float_as_uint(d0) == m) pos = (uint32_t)(it * 64 + 2 * lane);
+  }
+  return pos;
+}
+
 template <int OFF_THREADS, int OFF_MINB>
 __global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams p) {
   constexpr int OFF_WARPS = OFF_THREADS / 32;
@@ -412,7 +426,24 @@ __global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams
         const int ci = cur_u * OFF_NA + (k >> 2);
         const uint32_t bits = __float_as_uint(best[k]);
         const uint32_t m = __reduce_min_sync(0xffffffffu, bits);
-        const uint32_t cand = bits == m ? (uint32_t)brun[k] * 32u + (uint32_t)lane : 0xffffffffu;
+        uint32_t cand = bits == m ? (uint32_t)brun[k] * 32u + (uint32_t)lane : 0xffffffffu;
+        const uint32_t tied = __ballot_sync(0xffffffffu, bits == m);
+        if (__popc(tied) > 1) {
+          // Several lanes hold the minimum (an exact tie, e.g. two segments that meet in the nearest
+          // vertex): a lane's segments of a tile are interleaved with the other lanes' (lane l holds
+          // stored segments it * 64 + 2 l, + 1), so the lowest lane is not the lowest segment.  The tied
+          // lanes of the lowest tile find their lowest tied stored segment; that one decides (D17).
+          const uint32_t tmin = __reduce_min_sync(0xffffffffu, bits == m ? (uint32_t)brun[k] : 0xffffffffu);
+          uint32_t pos = 0xffffffffu;                     // stored position inside the tile
+          if (bits == m && (uint32_t)brun[k] == tmin) {
+            const int n = k >> 2, kc = k & 3;
+            pos = tie_position(edges_b + (int64_t)tmin * WM_TILE_F4 + lane, lane, cx[n], cy[n], (kc & 1) ? bx[n] : ax[n],
+                               (kc & 1) ? by[n] : ay[n], (kc & 2) ? -1.f : 1.f, m);
+          }
+          const uint32_t pmin = __reduce_min_sync(0xffffffffu, pos);
+          cand = (pos == pmin && pos != 0xffffffffu) ? tmin * 32u + (uint32_t)lane : 0xffffffffu;
+          if (pmin == 0xffffffffu) cand = bits == m ? (uint32_t)brun[k] * 32u + (uint32_t)lane : 0xffffffffu;   // cannot happen: the rescan repeats the scan's arithmetic
+        }
         const uint32_t r = __reduce_min_sync(0xffffffffu, cand);
         if (lane == 0 && ci < nvalid) atomicMin(&s_key[ci * 4 + (k & 3)], ((wm_u64)m << 32) | r);
       }

@@ -111,3 +111,27 @@ def test_topk_egos_far_off_the_map_and_sparse_points():
     assert np.array_equal(typ.cpu().numpy(), o["rg_type"])
     assert np.allclose(feat.cpu().numpy(), o["rg_feat"], rtol=1e-5, atol=2e-3)     # ego-frame coordinates up to 6 km in float32
     wm.wm_destroy(h)
+
+
+@pytest.mark.parametrize("mode", ["culled", "brute"])
+def test_exact_tie_between_stored_segments_63_and_64(mode):
+    """D17 (ties -> lower index) where the brute-force scan keeps its segments interleaved over the lanes: stored
+    segments 63 and 64 of a tile sit in lanes 31 and 0.  A polyline runs east along y = 0 to the vertex (64, 0) and
+    turns back by 135 degrees; the box corner (66, 1) is nearest to that vertex on BOTH segments (d2 = 5 exactly, all
+    coordinates are small integers), left of segment 63 and right of segment 64: the lower index, 63, must give
+    the sign (negative = on-road).  The oracle marks the corner ambiguous, so the generic comparisons skip it."""
+    from util import mk_roadgraph
+    pts = [(float(i), 0.0) for i in range(65)] + [(59.0, 5.0)]
+    rg = mk_roadgraph([np.array(pts)], B=1, R=128)
+    tr = mk_traj(1, 1, 32)
+    set_agent(tr, 0, 0, 0, 65.0, 0.0, 0.0, 0, 0, 2.0, 2.0)
+    orc = oracle.offroad(tr, 0, rg)
+    k = 0                                                         # D30: corner 0 = front-left = (66, 1)
+    assert orc["win_seg"][0, k, 0] == 63 and orc["ambig"][0, k, 0] == 1
+    assert orc["corner_dist"][0, k, 0] == -np.float32(np.sqrt(np.float32(5.0)))
+    h = wm.wm_create(offroad_mode=wm.WM_OFFROAD_CULLED if mode == "culled" else wm.WM_OFFROAD_BRUTE_FORCE)
+    tr_d, rg_d = dev(tr), dev(rg)
+    wm.wm_prepare(h, rg_d)
+    sd, cd, fl = gpu_offroad(h, tr_d, 0)
+    assert cd[0, k, 0] == orc["corner_dist"][0, k, 0], (cd[0, :, 0], orc["corner_dist"][0, :, 0])
+    wm.wm_destroy(h)
