@@ -71,8 +71,24 @@ def test_observe_config3_sample():
     orc = _check_topk(cfg["log"], cfg["roadgraph"], 10, 1000, idx, feat, typ)
     v = cfg["log"]["valid"][:, 10] == 1
     assert (idx[v] >= 0).all() and (idx[~v] == -1).all()
-    # report how many points sit within 1e-4 m of the k-th distance (band of the north_star)
-    print("top-k cfg3: egos=%d, all index sets bit-equal to the float32-keyed oracle" % int(v.sum()))
+    # P15 in double, as north_star words it: the GPU's set holds every point nearer than d_k - 1e-4 m and
+    # nothing farther than d_k + 1e-4 m; the points inside that band are counted and reported
+    rg, log, k = cfg["roadgraph"], cfg["log"], 1000
+    n_band = n_band_in = 0
+    for b in range(idx.shape[0]):
+        pv = rg["valid"][b] == 1
+        px, py = rg["x"][b].astype(np.float64), rg["y"][b].astype(np.float64)
+        for a in np.nonzero(v[b])[0]:
+            d = np.hypot(px - float(log["x"][b, 10, a]), py - float(log["y"][b, 10, a]))
+            d[~pv] = np.inf
+            dk = np.sort(d)[k - 1]
+            chosen = np.zeros(px.shape[0], bool)
+            chosen[idx[b, a][idx[b, a] >= 0]] = True
+            assert chosen[d < dk - 1e-4].all() and not chosen[d > dk + 1e-4].any()
+            band = np.abs(d - dk) <= 1e-4
+            n_band += int(band.sum()); n_band_in += int((band & chosen).sum())
+    print("top-k cfg3: egos=%d, index sets bit-equal to the float32-keyed oracle; double-precision band |d - d_k| <= 1e-4 m: "
+          "%d points, %d of them selected" % (int(v.sum()), n_band, n_band_in))
 
 
 def test_topk_fewer_valid_points_than_k_and_trailing_invalid():
