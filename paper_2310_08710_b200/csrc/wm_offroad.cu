@@ -86,11 +86,11 @@ __global__ void __launch_bounds__(1024) k_order_segments(RgView g, int cap, int3
   }
 }
 
-// position of stored segment s inside its tile: it = (s%512)/64, lane = (s%64)/2, half = s&1
+// position of stored segment s inside its tile: lane = (s%512)/16, it = (s%16)/2, half = s&1 (wm_internal.cuh)
 __device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir, int s, float p0x, float p0y,
                                               float ex, float ey, float gx, float gy, float sx, float sy) {
   const int tau = s / WM_TILE_SEGS, r = s % WM_TILE_SEGS;
-  const int it = r >> 6, lane = (r >> 1) & 31, half = r & 1;
+  const int it = (r & 15) >> 1, lane = r >> 4, half = r & 1;
   float* t = tile_base + (int64_t)tau * (WM_TILE_F4 * 4);
   float* q0 = t + ((it * 3 + 0) * 32 + lane) * 4;
   float* q1 = t + ((it * 3 + 1) * 32 + lane) * 4;
@@ -319,20 +319,6 @@ __device__ __forceinline__ float seg_d2(float wx, float wy, float ex, float ey, 
   return fmaf(ry, ry, rx * rx);
 }
 
-// exact ties across lanes (rare): the lowest stored position, among the lane's 16 segments of a tile, whose
-// distance^2 has the bits m; kept out of line so that it costs the scan no registers
-__device__ __noinline__ uint32_t tie_position(const float4* tp, int lane, float cx, float cy, float ox, float oy, float sgn, uint32_t m) {
-  uint32_t pos = 0xffffffffu;
-  for (int it = 7; it >= 0; --it) {
-    const float4 P = __ldg(&tp[(it * 3 + 0) * 32]), E = __ldg(&tp[(it * 3 + 1) * 32]), Gv = __ldg(&tp[(it * 3 + 2) * 32]);
-    const float d1 = seg_d2(fmaf(sgn, ox, cx - P.y), fmaf(sgn, oy, cy - P.w), E.y, E.w, Gv.y, Gv.w);
-    const float d0 = seg_d2(fmaf(sgn, ox, cx - P.x), fmaf(sgn, oy, cy - P.z), E.x, E.z, Gv.x, Gv.z);
-    if (__float_as_uint(d1) == m) pos = (uint32_t)(it * 64 + 2 * lane + 1);
-    if (__float_as_uint(d0) == m) pos = (uint32_t)(it * 64 + 2 * lane);
-  }
-  return pos;
-}
-
 template <int OFF_THREADS, int OFF_MINB>
 __global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams p) {
   constexpr int OFF_WARPS = OFF_THREADS / 32;
@@ -426,24 +412,9 @@ __global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams
         const int ci = cur_u * OFF_NA + (k >> 2);
         const uint32_t bits = __float_as_uint(best[k]);
         const uint32_t m = __reduce_min_sync(0xffffffffu, bits);
-        uint32_t cand = bits == m ? (uint32_t)brun[k] * 32u + (uint32_t)lane : 0xffffffffu;
-        const uint32_t tied = __ballot_sync(0xffffffffu, bits == m);
-        if (__popc(tied) > 1) {
-          // Several lanes hold the minimum (an exact tie, e.g. two segments that meet in the nearest
-          // vertex): a lane's segments of a tile are interleaved with the other lanes' (lane l holds
-          // stored segments it * 64 + 2 l, + 1), so the lowest lane is not the lowest segment.  The tied
-          // lanes of the lowest tile find their lowest tied stored segment; that one decides (D17).
-          const uint32_t tmin = __reduce_min_sync(0xffffffffu, bits == m ? (uint32_t)brun[k] : 0xffffffffu);
-          uint32_t pos = 0xffffffffu;                     // stored position inside the tile
-          if (bits == m && (uint32_t)brun[k] == tmin) {
-            const int n = k >> 2, kc = k & 3;
-            pos = tie_position(edges_b + (int64_t)tmin * WM_TILE_F4 + lane, lane, cx[n], cy[n], (kc & 1) ? bx[n] : ax[n],
-                               (kc & 1) ? by[n] : ay[n], (kc & 2) ? -1.f : 1.f, m);
-          }
-          const uint32_t pmin = __reduce_min_sync(0xffffffffu, pos);
-          cand = (pos == pmin && pos != 0xffffffffu) ? tmin * 32u + (uint32_t)lane : 0xffffffffu;
-          if (pmin == 0xffffffffu) cand = bits == m ? (uint32_t)brun[k] * 32u + (uint32_t)lane : 0xffffffffu;   // cannot happen: the rescan repeats the scan's arithmetic
-        }
+        // a lane holds 16 CONSECUTIVE stored segments of a tile, so (tile, lane) order is index order: exact
+        // ties between lanes go to the lower index (D17)
+        const uint32_t cand = bits == m ? (uint32_t)brun[k] * 32u + (uint32_t)lane : 0xffffffffu;
         const uint32_t r = __reduce_min_sync(0xffffffffu, cand);
         if (lane == 0 && ci < nvalid) atomicMin(&s_key[ci * 4 + (k & 3)], ((wm_u64)m << 32) | r);
       }
@@ -526,23 +497,23 @@ __global__ void __launch_bounds__(OFF_THREADS, OFF_MINB) k_offroad(OffroadParams
       const float sgn = (k & 2) ? -1.f : 1.f;
       const float qx = s_ag[0 * Ap + ci], qy = s_ag[1 * Ap + ci];
       const float4* tp = edges_b + (int64_t)tau * WM_TILE_F4 + ln;
-      // the lane's 16 stored segments of this tile sit at it*64 + lane*2 + {0,1}; exact ties
+      // the lane's 16 stored segments of this tile sit at lane*16 + it*2 + {0,1}; exact ties
       // inside the run go to the lower source point index (D17)
-      const int32_t* srcp = p.seg_src + (int64_t)b * p.seg_tiles * WM_TILE_SEGS + tau * WM_TILE_SEGS + ln * 2;
+      const int32_t* srcp = p.seg_src + (int64_t)b * p.seg_tiles * WM_TILE_SEGS + tau * WM_TILE_SEGS + ln * WM_RUN;
       float bd2 = __int_as_float(0x7f800000), bwx = 0.f, bwy = 0.f;
       int bs = 0, bsrc = 0x7fffffff;
 #pragma unroll
       for (int it = 0; it < 8; ++it) {
         const float4 P = __ldg(&tp[(it * 3 + 0) * 32]), E = __ldg(&tp[(it * 3 + 1) * 32]), Gv = __ldg(&tp[(it * 3 + 2) * 32]);
-        const int2 sr = __ldg((const int2*)(srcp + it * 64));
+        const int2 sr = __ldg((const int2*)(srcp + it * 2));
         const float w0x = fmaf(sgn, offx, qx - P.x), w0y = fmaf(sgn, offy, qy - P.z);
         const float w1x = fmaf(sgn, offx, qx - P.y), w1y = fmaf(sgn, offy, qy - P.w);
         const float d0 = seg_d2(w0x, w0y, E.x, E.z, Gv.x, Gv.z);
         const float d1 = seg_d2(w1x, w1y, E.y, E.w, Gv.y, Gv.w);
-        if (sr.x >= 0 && (d0 < bd2 || (d0 == bd2 && sr.x < bsrc))) { bd2 = d0; bwx = w0x; bwy = w0y; bs = it * 64; bsrc = sr.x; }
-        if (sr.y >= 0 && (d1 < bd2 || (d1 == bd2 && sr.y < bsrc))) { bd2 = d1; bwx = w1x; bwy = w1y; bs = it * 64 + 1; bsrc = sr.y; }
+        if (sr.x >= 0 && (d0 < bd2 || (d0 == bd2 && sr.x < bsrc))) { bd2 = d0; bwx = w0x; bwy = w0y; bs = it * 2; bsrc = sr.x; }
+        if (sr.y >= 0 && (d1 < bd2 || (d1 == bd2 && sr.y < bsrc))) { bd2 = d1; bwx = w1x; bwy = w1y; bs = it * 2 + 1; bsrc = sr.y; }
       }
-      const int s = tau * WM_TILE_SEGS + ln * 2 + bs;
+      const int s = tau * WM_TILE_SEGS + ln * WM_RUN + bs;
       const float2 sdir = __ldg(&p.sign_dir[(int64_t)b * p.seg_tiles * WM_TILE_SEGS + s]);
       const float side = fmaf(sdir.x, bwy, -sdir.y * bwx);                 // e x (q - p0), D16
       const float d = sqrtf(bd2);

@@ -98,7 +98,7 @@ __device__ __forceinline__ FusedIn fused_load_in(const FusedParams& p, int64_t s
 // ======================================================================================
 // DYN_C >= 0: the dynamics model is a compile-time constant
 template <int DYN_C>
-__global__ void __launch_bounds__(DYN_NT) k_rollout_dyn(FusedParams p) {
+__global__ void __launch_bounds__(DYN_NT, 16) k_rollout_dyn(FusedParams p) {
   const int A = p.sim.A, nba = (A + DYN_NT - 1) / DYN_NT;
   const int b = blockIdx.x / nba, a = (blockIdx.x % nba) * DYN_NT + threadIdx.x;
   if (a >= A) return;
