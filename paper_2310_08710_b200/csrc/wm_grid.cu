@@ -126,7 +126,7 @@ __device__ __forceinline__ void slab_keep(const float4 NE, const float4 L0, cons
 // One warp per block of 8 x 4 cells, one lane per cell.  Outer cells (and inner cells under a
 // crowded parent): chunks that cannot hold a candidate of any cell of the block are dropped with one
 // box-box test per chunk (lanes over chunks); the survivors are walked twice with lanes over cells:
-// dmin(c), then the candidates.  Inner cells: both passes walk the parent's runs.
+// dmin(c), then the candidates.  Mid and inner cells: both passes walk the parent's runs.
 //
 // Both passes take the records two by two (pair records, packed arithmetic).  Pass 2 marks the pair
 // records that hold a candidate in a bit mask over the run (or chunk) being walked; the set stretches
@@ -213,17 +213,19 @@ __global__ void __launch_bounds__(256, 4) k_build_cells(const float4* segrec, co
     slab_keep(NE, L0, L1, wx, wy, kk, ke, ko);
     return (de <= thr2 && ke) || (dq <= thr2 && ko);              // padding records (1e18) never pass
   };
-  bool done = false;
-  if (FINE) {
+  bool crowded = false;                                           // under a crowded parent: crowded as well
+  if constexpr (FINE) {
     // Mid / inner cell: its inflated box lies inside its parent's (the cell above it, 2 x 2 children),
     // so every segment that is the reported nearest one of a point of this cell is in the
     // parent's list, and so is the nearest segment of the cell centre: both passes walk the
-    // parent's runs (a few dozen records) instead of the surviving chunks.  A crowded parent
-    // (no list) sends the warp down the chunk-wise path.
+    // parent's runs (a few dozen records) instead of the surviving chunks.  The children of a crowded
+    // parent (no list: its queries search all chunks) are crowded too.
     uint2 ph = make_uint2(0u, 0u);
     if (in) ph = LEVEL == 1 ? cells_b[g.obase + wm_cell_index(g.icx0 + (ix >> 1), g.icy0 + (iy >> 1), g.onx)]
                             : cells_b[g.mbase + wm_cell_index(ix >> 1, iy >> 1, g.nx >> 1)];
-    if (!__any_sync(0xffffffffu, (ph.x & ph.y) == 0xffffffffu)) {
+    crowded = (ph.x & ph.y) == 0xffffffffu;
+    if (crowded) ph = make_uint2(0u, 0u);
+    {
       auto walk_runs = [&](auto&& f) {                  // the parent's pair runs (wm_internal.cuh): f(first pair, pairs)
         uint32_t r = ph.x & 0x1fffffu, r1 = ((ph.x >> 21) | (ph.y << 11)) & 0x1fffffu, r2 = ph.y >> 10;
         const uint32_t* pl = pool_b;
@@ -236,17 +238,12 @@ __global__ void __launch_bounds__(256, 4) k_build_cells(const float4* segrec, co
         }
       };
       walk_runs([&](int first, int cnt) {
-        // the next pair record is requested before this one is evaluated
-        const float4* a = pair + 3 * first;
-        float4 P = __ldg(a), NE = __ldg(a + 1), G = __ldg(a + 2);
         for (int q = 0; q < cnt; ++q) {
-          const float4* an = a + (q + 1 < cnt ? 3 : 0);
-          const float4 Pn = __ldg(an), NEn = __ldg(an + 1), Gn = __ldg(an + 2);
+          const int pid = first + q;
           wm_u64 wx, wy;
           float de, dq;
-          centre_pair_d2(P, NE, G, cx2, cy2, wx, wy, de, dq);
+          centre_pair_d2(__ldg(pair + 3 * pid), __ldg(pair + 3 * pid + 1), __ldg(pair + 3 * pid + 2), cx2, cy2, wx, wy, de, dq);
           dmin2 = fminf(dmin2, fminf(de, dq));
-          a = an; P = Pn; NE = NEn; G = Gn;
         }
       });
       const float dmin = sqrtf(dmin2);
@@ -257,10 +254,8 @@ __global__ void __launch_bounds__(256, 4) k_build_cells(const float4* segrec, co
         for (int q = 0; q < cnt; ++q) m |= (uint32_t)pair_hit(first + q, thr2) << q;
         if (in) add_mask(m, first);
       });
-      done = true;
     }
-  }
-  if (!done) {
+  } else {
   // block box
   const float X0 = gx0 + (float)(bx * 8) * h - delta, X1 = gx0 + (float)(bx * 8 + 8) * h + delta;
   const float Y0 = gy0 + (float)(by * 4) * h - delta, Y1 = gy0 + (float)(by * 4 + 4) * h + delta;
@@ -402,7 +397,7 @@ __global__ void __launch_bounds__(256, 4) k_build_cells(const float4* segrec, co
   // query header (wm_internal.cuh): three runs in the header, or two + the rest in the pool
   uint2 hd = make_uint2(0xffffffffu, 0xffffffffu);              // fall back to the full search
   if (n <= 0) hd = make_uint2(0u, 0u);
-  else if (nr <= BUILD_MAXRUN && 2 * npair <= BUILD_MAXCAND) {
+  else if (!crowded && nr <= BUILD_MAXRUN && 2 * npair <= BUILD_MAXCAND) {
     uint32_t f0 = nr > 0 ? s_runs[warp][0][lane] : 0u, f1 = nr > 1 ? s_runs[warp][1][lane] : 0u, f2 = nr > 2 ? s_runs[warp][2][lane] : 0u;
     bool ok = true;
     if (nr > 3) {
