@@ -15,11 +15,12 @@ value     device-resident: inputs in HBM when the timed region starts, CUDA even
 e2e       the same job through wm_rollout_host with pinned HOST buffers: scenario + action
           upload, wm_prepare, reset, rollout, metric download all inside the timed region
           (pipelined over scenario chunks: its floor is the PCIe time of the 3.8 GB upload).
-roofline  dominant kernel k_rollout_fused (the whole rollout is one launch of it).  The exact grid
-          search leaves < 0.1 % of the corner-segment pairs, so the slower roof of the kernel is its
+roofline  the rollout graph = k_rollout_dyn + k_rollout_metrics (one launch of each per 80-step rollout).  The
+          exact grid search leaves ~0.1 % of the corner-segment pairs, so the slower roof of the graph is its
           compulsory HBM IO (actions + log row in, sim row + metric rows out, per agent-step):
-          achieved = those bytes / CUDA-event duration of the launch, against the measured HBM peak;
-          the FP32 fractions on evaluated pairs and on the brute-force pair count are beside it.
+          achieved = those bytes / CUDA-event duration of the two launches, against the measured HBM peak;
+          roofline.kernels has each kernel's own time, bytes and fraction; the FP32 fractions on evaluated
+          pairs and on the brute-force pair count are beside it.
 roofline_bruteforce  the brute-force kernel k_offroad: 13 flop per corner-segment pair (SURVEY
           §8(d)) / its CUDA-event duration, against the FP32 peak SMs*128*2*max clock.
 cpu_baseline  the oracle (oracle/, as it stands) on the host cores, bounded sample.

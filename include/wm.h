@@ -76,9 +76,9 @@ typedef struct {
 /* Both modes find the nearest segment exactly and use the same per-pair arithmetic; they return the
  * same bits whenever they pick the same segment (at a polyline vertex the two neighbours' float32
  * distances can differ by an ulp).
- * CULLED (default): wm_prepare lays two nested grids over the segments; every cell lists, as runs of
- *   consecutive segments, the only segments that can be nearest to a point inside it; a query walks
- *   the list of its corner's cell (about 7 segments).  Crowded cells and points outside the grids
+ * CULLED (default): wm_prepare lays nested grids over the segments (2 m cells near the map, 8 m cells in the
+ *   wide margin around it); every cell lists, as runs of consecutive segments, the only segments that can
+ *   be nearest to a point inside it; a query walks the list of its corner's cell (about 8 segments).  Crowded cells and points outside the grids
  *   fall back to a bounding-box search over all segments, exact as well.
  * BRUTE_FORCE: every corner-segment pair is evaluated (the FP32-roofline reference kernel). */
 enum { WM_OFFROAD_CULLED = 0, WM_OFFROAD_BRUTE_FORCE = 1 };

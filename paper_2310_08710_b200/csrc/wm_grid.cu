@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const
                                                 fmaxf(Wi, Hi) * (1.0001f / (WM_GRID_NG_IN / 4 - 1))));
       g.ox0 = x0 - margin; g.oy0 = y0 - margin; g.oh = oh; g.oinv_h = 1.f / oh;
       g.onx = min(WM_GRID_NG_OUT, (int)ceilf(W / oh)); g.ony = min(WM_GRID_NG_OUT, (int)ceilf(H / oh));
-      // inner: the outer cells that meet the bounding box + margin_in, each split 4 x 4
+      // inner: the outer cells that meet the bounding box + margin_in, each split 4 x 4 (2 x 2 mid cells of 2 x 2)
       const int cx0 = max(0, (int)floorf((x0 - margin_in - g.ox0) / oh)), cy0 = max(0, (int)floorf((y0 - margin_in - g.oy0) / oh));
       int cx1 = min(g.onx, (int)ceilf((x1 + margin_in - g.ox0) / oh)), cy1 = min(g.ony, (int)ceilf((y1 + margin_in - g.oy0) / oh));
       cx1 = min(cx1, cx0 + WM_GRID_NG_IN / 4); cy1 = min(cy1, cy0 + WM_GRID_NG_IN / 4);
