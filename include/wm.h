@@ -38,7 +38,7 @@ typedef enum {
   WM_OK = 0,
   WM_ERR_ARG = -1,          /* null / misaligned pointer, bad shape, t out of range */
   WM_ERR_CUDA = -2,         /* a CUDA call failed; see wm_last_cuda_error() */
-  WM_ERR_UNSUPPORTED = -3,  /* e.g. A > 1024, topk > R */
+  WM_ERR_UNSUPPORTED = -3,  /* e.g. A > 1024, B > 65535 scenarios per call, topk > R, more than 131 072 road-edge segments in a scenario */
   WM_ERR_STATE = -4         /* e.g. metrics_offroad before wm_prepare */
 } wm_status;
 

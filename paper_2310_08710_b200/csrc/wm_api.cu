@@ -106,6 +106,7 @@ extern "C" int64_t wm_kernel_launches(const wm_handle* h) { return h ? h->launch
 
 extern "C" int wm_prepare(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, void* stream) {
   if (!h || !rg_ok(rg)) return WM_ERR_ARG;
+  if (rg->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   return wm_prepare_impl(h, rg, n_segments_max, (cudaStream_t)stream);
 }
 
@@ -120,7 +121,7 @@ extern "C" int wm_segment_counts(wm_handle* h, int32_t* n_seg_host, int32_t B, v
 extern "C" int wm_reset(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t* t, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim)) return WM_ERR_ARG;
   if (h->cfg.history > sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   WM_CUDA(wm_launch_reset(h, *log, *sim, h->cfg.history, (cudaStream_t)stream));
   if (t) *t = h->cfg.history - 1;
   return WM_OK;
@@ -130,7 +131,7 @@ extern "C" int wm_step(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t
                        const uint8_t* action_valid, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !action || !action_valid) return WM_ERR_ARG;
   if (t < 0 || t + 1 >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   WM_CUDA(wm_launch_step(h, *log, *sim, t, action, (int64_t)C * sim->A, action_valid, sim->A, nullptr, nullptr, 0,
                          (cudaStream_t)stream));
@@ -141,7 +142,7 @@ extern "C" int wm_metrics_overlap(wm_handle* h, const wm_traj* sim, int32_t t, u
                                   uint8_t* agent_flag, void* stream) {
   if (!h || !traj_ok(sim) || !agent_flag) return WM_ERR_ARG;
   if (t < 0 || t >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   WM_CUDA(wm_launch_overlap(h, *sim, t, pair_bits, agent_flag, sim->A, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -150,7 +151,7 @@ extern "C" int wm_metrics_offroad(wm_handle* h, const wm_traj* sim, int32_t t, f
                                   float* corner_dist, uint8_t* agent_flag, void* stream) {
   if (!h || !traj_ok(sim) || !signed_dist || !agent_flag) return WM_ERR_ARG;
   if (t < 0 || t >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
   WM_CUDA(wm_launch_offroad(h, *sim, t, signed_dist, sim->A, corner_dist, agent_flag, sim->A, (cudaStream_t)stream));
   return WM_OK;
@@ -270,7 +271,7 @@ extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* 
   if (want_hist && !(hist && hist_valid)) return WM_ERR_ARG;
   if (want_topk && !(rg_index && rg_feat && rg_type && rg_ok(rg))) return WM_ERR_ARG;
   if (t < h->cfg.history - 1 || t >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   if (want_hist) WM_CUDA(wm_launch_observe_hist(h, *sim, t, hist, hist_valid, (cudaStream_t)stream));
   if (want_topk) {
     if (h->cfg.topk < 1 || h->cfg.topk > rg->R) return WM_ERR_UNSUPPORTED;
@@ -315,7 +316,7 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
                           const float* actions, const uint8_t* action_valid, const wm_rollout_out* out, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !actions || !action_valid || !out) return WM_ERR_ARG;
   if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024) return WM_ERR_UNSUPPORTED;
+  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
   const bool fused = h->cfg.rollout_mode == WM_ROLLOUT_FUSED && h->cfg.offroad_mode == WM_OFFROAD_CULLED &&
                      n_steps < 60000;                  // its hash entries carry a 16-bit block number
@@ -446,7 +447,7 @@ extern "C" int wm_rollout_host(wm_handle* h, const wm_traj* lh, const wm_roadgra
   const int B = lh->B, A = lh->A, T = lh->T, R = gh->R;
   const int t0 = h->cfg.history - 1;
   if (n_steps < 1 || t0 + n_steps >= T) return WM_ERR_ARG;
-  if (A > 1024) return WM_ERR_UNSUPPORTED;
+  if (A > 1024 || B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
   cudaStream_t s = (cudaStream_t)stream;
   const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   const size_t nTA = (size_t)B * T * A, nR = (size_t)B * R, rows = (size_t)B * n_steps * A, nBA = (size_t)B * A;

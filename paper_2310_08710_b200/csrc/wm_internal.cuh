@@ -61,6 +61,7 @@ constexpr int WM_PT_NG = 64;
 constexpr int WM_PT_CELLS = WM_PT_NG * WM_PT_NG;
 struct WmPtGrid { float x0, y0, inv_h, h; int nx, ny, nvalid, pad; };
 
+constexpr int WM_MAX_B = 65535;            // scenarios per call: several launchers put the scenario in gridDim.y
 constexpr int WM_GRAPH_KEY_WORDS = 40;     // cache key of the captured rollout graph (wm_api.cu)
 constexpr int WM_HOST_CHUNKS = 16;          // scenario chunks of the pipelined host path
 

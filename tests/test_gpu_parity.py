@@ -351,3 +351,58 @@ def test_rollout_host_pipelined_chunks_match_device_rollout():
         assert np.array_equal(v, sim_h[k].numpy(), equal_nan=True), k
     assert out_h["offroad"].numpy().sum() > 0
     wm.wm_destroy(h); wm.wm_destroy(h2)
+
+
+@pytest.mark.parametrize("A", [160, 256, 300])
+def test_rollout_fused_equals_stepwise_bitwise_wide_scenarios(A):
+    """The corner-task lane mappings with 4 and 2 steps per block (A = 160: S = 4; A = 256, 300: S = 2), and the
+    broad-phase fallbacks of the overlap tasks: agents too fast / too long for the hash (block extent above 11.7 m:
+    the oversize list), and a dense cluster of more than 48 overlapping pairs per 32 agents (pair-list overflow).
+    Config 5 tiled to A agents; the extras are written into the logged rows and driven by playback."""
+    n = 10
+    base = ws.make_config(5, B=3, n_steps=n)
+    reps = (A + 127) // 128
+    tile = lambda v, ax: np.ascontiguousarray(np.concatenate([v] * reps, axis=ax).take(range(A), axis=ax))
+    log = {k: tile(v, 2) for k, v in base["log"].items()}
+    acts = tile(base["actions"][:, :n], 3); av = tile(base["action_valid"][:, :n], 2)
+    B, T, _ = log["x"].shape
+    rng = np.random.default_rng(A)
+    # (1) fast agents: 40 m/s along x from row 0 on (4 m per step, 16 - 32 m per block); (2) long boxes (30 m);
+    # (3) a cluster of 40 boxes within 3 m of one point, all overlapping each other.  All on playback.
+    fast = np.arange(0, 6); longb = np.arange(6, 10); clus = np.arange(10, 50)
+    for b in range(B):
+        for a in fast:
+            log["x"][b, :, a] = 50.0 + 4.0 * np.arange(T) + a; log["y"][b, :, a] = 60.0 + 3.0 * a
+            log["yaw"][b, :, a] = 0.0; log["vel_x"][b, :, a] = 40.0; log["vel_y"][b, :, a] = 0.0
+            log["length"][b, :, a] = 4.5; log["width"][b, :, a] = 2.0; log["valid"][b, :, a] = 1
+        for a in longb:
+            log["x"][b, :, a] = 100.0 + 0.5 * np.arange(T); log["y"][b, :, a] = 20.0 * (a - 5)
+            log["yaw"][b, :, a] = 0.3 * a; log["vel_x"][b, :, a] = 5.0; log["vel_y"][b, :, a] = 0.0
+            log["length"][b, :, a] = 30.0; log["width"][b, :, a] = 2.5; log["valid"][b, :, a] = 1
+        for a in clus:
+            c = rng.uniform(-1.5, 1.5, 2)
+            log["x"][b, :, a] = 120.0 + c[0] + 0.1 * np.arange(T); log["y"][b, :, a] = 120.0 + c[1]
+            log["yaw"][b, :, a] = rng.uniform(-3, 3); log["vel_x"][b, :, a] = 1.0; log["vel_y"][b, :, a] = 0.0
+            log["length"][b, :, a] = 4.5; log["width"][b, :, a] = 2.0; log["valid"][b, :, a] = 1
+    av[:, :, :50] = 0                                               # the extras follow their logged rows (D8)
+    cfg = {"log": log, "roadgraph": base["roadgraph"]}
+    res = []
+    for mode in (wm.WM_ROLLOUT_FUSED, wm.WM_ROLLOUT_STEPWISE):
+        h, log_d, rg_d, sim_d, _ = _setup(cfg, rollout_mode=mode)
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        out_d = wm.alloc_rollout_out(B, n, A)
+        wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out_d)
+        torch.cuda.synchronize()
+        res.append((host(sim_d), host(out_d)))
+        wm.wm_destroy(h)
+    for k in res[0][0]:
+        assert np.array_equal(res[0][0][k], res[1][0][k], equal_nan=True), k
+    for k in res[0][1]:
+        assert np.array_equal(res[0][1][k], res[1][1][k]), k
+    ov = res[0][1]["overlap"]
+    assert ov[:, :, 10:50].all()                                    # every box of the cluster overlaps another one
+    # and against the oracle at the last step (teacher-forced), outside the ambiguity band
+    got = res[0][0]
+    o = oracle.overlap(got, t0 + n, want_pair=False)
+    cl = ~(np.abs(o["gap"]) < 1e-4).any(axis=2)
+    assert np.array_equal(ov[:, n - 1][cl], o["flag"][cl])
