@@ -52,7 +52,7 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   }
   if (e == cudaSuccess) e = cudaMalloc(&h->cull_stats, 4 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMemset(h->cull_stats, 0, 4 * sizeof(unsigned long long));
-  if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; free(h); return WM_ERR_CUDA; }
+  if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; wm_destroy(h); return WM_ERR_CUDA; }   // frees what was created so far
   *out = h;
   return WM_OK;
 }
@@ -84,6 +84,9 @@ void wm_drop_graph(wm_handle* h) {
 
 extern "C" int wm_destroy(wm_handle* h) {
   if (!h) return WM_ERR_ARG;
+  int cur = -1;                                       // the handle's device, not whichever is current
+  cudaGetDevice(&cur);
+  if (cur != h->device) cudaSetDevice(h->device);
   cudaDeviceSynchronize();
   wm_drop_graph(h);
   wm_prepare_free(h);
@@ -98,6 +101,7 @@ extern "C" int wm_destroy(wm_handle* h) {
     if (h->ev_prep[i]) cudaEventDestroy(h->ev_prep[i]);
     if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
   }
+  if (cur >= 0 && cur != h->device) cudaSetDevice(cur);
   free(h);
   return WM_OK;
 }

@@ -240,14 +240,15 @@ int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_m
     h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->segrec = nullptr; h->segpair = nullptr; h->seglk = nullptr; h->segfin = nullptr; h->chunks = nullptr;
     h->seg_tiles = tiles;
     const size_t cap = (size_t)tiles * WM_TILE_SEGS;
-    WM_CUDA(cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES));
-    WM_CUDA(cudaMalloc(&h->sign_dir, (size_t)B * cap * sizeof(float2)));
-    WM_CUDA(cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t)));
-    WM_CUDA(cudaMalloc(&h->segrec, (size_t)B * cap * 2 * sizeof(float4)));
-    WM_CUDA(cudaMalloc(&h->segpair, (size_t)B * (cap / 2) * 3 * sizeof(float4)));
-    WM_CUDA(cudaMalloc(&h->seglk, (size_t)B * (cap / 2) * 2 * sizeof(float4)));
-    WM_CUDA(cudaMalloc(&h->segfin, (size_t)B * cap * sizeof(float4)));
-    WM_CUDA(cudaMalloc(&h->chunks, (size_t)B * (cap / WM_CHUNK) * sizeof(float4)));
+    cudaError_t ea = cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES);
+    if (ea == cudaSuccess) ea = cudaMalloc(&h->sign_dir, (size_t)B * cap * sizeof(float2));
+    if (ea == cudaSuccess) ea = cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t));
+    if (ea == cudaSuccess) ea = cudaMalloc(&h->segrec, (size_t)B * cap * 2 * sizeof(float4));
+    if (ea == cudaSuccess) ea = cudaMalloc(&h->segpair, (size_t)B * (cap / 2) * 3 * sizeof(float4));
+    if (ea == cudaSuccess) ea = cudaMalloc(&h->seglk, (size_t)B * (cap / 2) * 2 * sizeof(float4));
+    if (ea == cudaSuccess) ea = cudaMalloc(&h->segfin, (size_t)B * cap * sizeof(float4));
+    if (ea == cudaSuccess) ea = cudaMalloc(&h->chunks, (size_t)B * (cap / WM_CHUNK) * sizeof(float4));
+    if (ea != cudaSuccess) { wm_prepare_free(h); WM_CUDA(ea); }     // out of memory: back to the unprepared state
   }
   if (n_segments_max) *n_segments_max = mx;
   return WM_OK;
