@@ -150,6 +150,122 @@ __global__ void __launch_bounds__(DYN_NT, 16) k_rollout_dyn(FusedParams p) {
   if (p.out.any_offroad) p.out.any_offroad[oa] = 0;
 }
 
+// ======================================================================================
+// k_rollout_dyn_bulk: the same trajectory kernel with its input rows staged by bulk (TMA) copies
+// ======================================================================================
+// One CTA per scenario, one thread per agent.  The inputs of DYN_SS consecutive steps - actions, action masks and
+// the logged rows - are contiguous per array ([...][A] row-major), so thread 0 brings each of them into shared
+// memory with ONE 1-D bulk copy (cp.async.bulk -> mbarrier), two stages ahead, and the threads read them there with
+// 32-bit addresses and immediate offsets instead of ten global streams of 128-byte requests per warp with 64-bit
+// address arithmetic each (k_rollout_dyn is bound by instruction issue and load latency, profiles/r02_k_rollout_ncu.md).
+// The successor rows leave with plain streaming stores: staging them for bulk stores as well costs the shared
+// memory that keeps enough CTAs resident (measured: 0.62 ms with both directions staged, 0.51 ms with the inputs
+// only, 0.65 ms for k_rollout_dyn).  Needs A % 16 == 0 and 16-byte aligned arrays (bulk copies); other shapes take
+// k_rollout_dyn.  Same device arithmetic: bit-identical rows.
+constexpr int DYN_SS = 4;                   // steps per stage (2: 0.54 ms, 4: 0.51 ms, 6: 0.67 ms, 8: 0.87 ms)
+
+struct DynBulkSmem { int act, av, lx, ly, lyaw, lvx, lvy, llen, lwid, lv, in_bytes; };   // byte offsets inside a stage buffer
+__host__ __device__ inline DynBulkSmem dyn_bulk_layout(int A, int C) {
+  DynBulkSmem m;
+  const int row = A * 4 * DYN_SS, rowb = A * DYN_SS;
+  int o = 0;
+  m.act = o; o += C * row;
+  m.lx = o; o += row; m.ly = o; o += row; m.lyaw = o; o += row; m.lvx = o; o += row; m.lvy = o; o += row;
+  m.llen = o; o += row; m.lwid = o; o += row;
+  m.av = o; o += rowb; m.lv = o; o += rowb;
+  m.in_bytes = (o + 127) & ~127;
+  return m;
+}
+
+template <int DYN_C>
+__global__ void __launch_bounds__(1024) k_rollout_dyn_bulk(FusedParams p) {
+  extern __shared__ __align__(128) unsigned char dsm[];
+  __shared__ __align__(8) uint64_t bars[2];
+  const int A = p.sim.A, b = blockIdx.x, a = threadIdx.x;
+  WmDynCfg dyn = p.dyn;
+  if (DYN_C >= 0) dyn.dynamics = DYN_C;
+  const int C = DYN_C >= 0 ? (DYN_C == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3) : p.C;
+  const DynBulkSmem m = dyn_bulk_layout(A, C);
+  const int64_t TA = (int64_t)p.sim.T * A;
+  const int64_t sb = (int64_t)b * TA;                // scenario offset in the trajectories
+  const int64_t ab = (int64_t)b * p.n_steps;         // scenario offset in the action / metric rows, in rows
+  const int n_stage = (p.n_steps + DYN_SS - 1) / DYN_SS;
+  if (a == 0) { mbar_init(&bars[0], 1); mbar_init(&bars[1], 1); mbar_fence_init(); }
+  __syncthreads();
+  // producer (thread 0): the inputs of stage s -> buffer s & 1
+  auto load_stage = [&](int s) {
+    const int k0 = s * DYN_SS, ns = min(DYN_SS, p.n_steps - k0);
+    unsigned char* d = dsm + (s & 1) * m.in_bytes;
+    uint64_t* bar = &bars[s & 1];
+    const uint32_t rf = (uint32_t)(ns * A * 4), rb = (uint32_t)(ns * A);
+    mbar_expect_tx(bar, (uint32_t)(C + 7) * rf + 2u * rb);
+    const int64_t ro = sb + (int64_t)(p.t0 + 1 + k0) * A;          // first logged row of the stage
+    tma_load_1d(d + m.act, p.actions + (ab + k0) * C * A, (uint32_t)C * rf, bar);
+    tma_load_1d(d + m.lx, p.log.x + ro, rf, bar);       tma_load_1d(d + m.ly, p.log.y + ro, rf, bar);
+    tma_load_1d(d + m.lyaw, p.log.yaw + ro, rf, bar);   tma_load_1d(d + m.lvx, p.log.vel_x + ro, rf, bar);
+    tma_load_1d(d + m.lvy, p.log.vel_y + ro, rf, bar);  tma_load_1d(d + m.llen, p.log.length + ro, rf, bar);
+    tma_load_1d(d + m.lwid, p.log.width + ro, rf, bar);
+    tma_load_1d(d + m.av, p.av + (ab + k0) * A, rb, bar);
+    tma_load_1d(d + m.lv, p.log.valid + ro, rb, bar);
+  };
+  if (a == 0) { load_stage(0); if (n_stage > 1) load_stage(1); }
+  // the state at t0
+  bool v = false;
+  float x = 0.f, y = 0.f, th = 0.f, vx = 0.f, vy = 0.f, ln = 0.f, wd = 0.f, sn = 0.f, cs = 1.f;
+  if (a < A) {
+    const int64_t o0 = sb + (int64_t)p.t0 * A + a;
+    v = p.sim.valid[o0] != 0;
+    if (v) {
+      x = p.sim.x[o0]; y = p.sim.y[o0]; th = p.sim.yaw[o0]; vx = p.sim.vel_x[o0]; vy = p.sim.vel_y[o0];
+      ln = p.sim.length[o0]; wd = p.sim.width[o0];
+      sincosf(th, &sn, &cs);
+    }
+  }
+  double sum = 0.0;                                   // sum of valid log divergences (D21)
+  int cnt = 0;
+  for (int s = 0; s < n_stage; ++s) {
+    const int k0 = s * DYN_SS, ns = min(DYN_SS, p.n_steps - k0);
+    const unsigned char* in = dsm + (s & 1) * m.in_bytes;
+    mbar_wait(&bars[s & 1], (uint32_t)((s >> 1) & 1));
+    if (a < A) {
+      for (int j = 0; j < ns; ++j) {
+        const int r = j * A + a;
+        const float* act = (const float*)(in + m.act) + (size_t)j * C * A + a;
+        const uint8_t avk = in[m.av + r], lvk = in[m.lv + r];
+        const float lx = ((const float*)(in + m.lx))[r], ly = ((const float*)(in + m.ly))[r];
+        const bool use_dyn = avk != 0 && v;                          // D8
+        float xn, yn, thn, vxn, vyn, s1 = 0.f, c1 = 1.f;
+        if (use_dyn) {
+          wm_dyn_step(dyn, x, y, th, vx, vy, sn, cs, act[0], act[A], C > 2 ? act[2 * A] : 0.f, xn, yn, thn, vxn, vyn, s1, c1);
+          v = true;                                                  // D9: keeps its box
+        } else {                                                     // log playback, L164
+          xn = lx; yn = ly; thn = ((const float*)(in + m.lyaw))[r]; vxn = ((const float*)(in + m.lvx))[r];
+          vyn = ((const float*)(in + m.lvy))[r]; ln = ((const float*)(in + m.llen))[r]; wd = ((const float*)(in + m.lwid))[r];
+          v = lvk != 0;
+          if (v) sincosf(thn, &s1, &c1);
+        }
+        const bool ldv = v && lvk != 0;                              // a5, L106
+        const float d = ldv ? wm_logdiv(xn, yn, lx, ly) : 0.f;
+        const int64_t o = sb + (int64_t)(p.t0 + 1 + k0 + j) * A + a;
+        __stcs(p.sim.x + o, xn); __stcs(p.sim.y + o, yn); __stcs(p.sim.yaw + o, thn);
+        __stcs(p.sim.vel_x + o, vxn); __stcs(p.sim.vel_y + o, vyn);
+        __stcs(p.sim.length + o, ln); __stcs(p.sim.width + o, wd); __stcs(p.sim.valid + o, (uint8_t)v);
+        if (p.out.log_div) __stcs(p.out.log_div + (ab + k0 + j) * A + a, d);
+        if (ldv) { sum += (double)d; cnt += 1; }
+        x = xn; y = yn; th = thn; vx = vxn; vy = vyn; sn = s1; cs = c1;
+      }
+    }
+    __syncthreads();                                   // everyone has read the buffer: it takes stage s + 2
+    if (a == 0 && s + 2 < n_stage) load_stage(s + 2);
+  }
+  if (a < A) {
+    const int64_t oa = (int64_t)b * A + a;
+    if (p.out.ade) p.out.ade[oa] = cnt ? (float)(sum / cnt) : 0.f;
+    if (p.out.any_overlap) p.out.any_overlap[oa] = 0;                 // the metrics kernel sets the flags that are 1
+    if (p.out.any_offroad) p.out.any_offroad[oa] = 0;
+  }
+}
+
 __device__ __forceinline__ int fused_cell(float v) {
   return (int)floorf(fminf(fmaxf(v * (1.f / FUSED_HASH_H), -1.0e9f), 1.0e9f));
 }
@@ -455,11 +571,33 @@ static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_
   // ---- the trajectory ----
   const int nba = (sim.A + DYN_NT - 1) / DYN_NT;
   const int64_t n_dyn = (int64_t)sim.B * nba;
+  cudaError_t e = cudaSuccess;
   if (ev) cudaEventRecord(ev[0], s);
-  if (h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE) k_rollout_dyn<WM_DYN_INVERTIBLE_BICYCLE><<<(unsigned)n_dyn, DYN_NT, 0, s>>>(p);
+  // bulk-copy staging needs 16-byte aligned rows of every array
+  bool bulk = sim.A % 16 == 0 && sim.A <= 1024;
+  {
+    const void* ptrs[] = {log.x, log.y, log.yaw, log.vel_x, log.vel_y, log.length, log.width, log.valid, sim.x, sim.y, sim.yaw,
+                          sim.vel_x, sim.vel_y, sim.length, sim.width, sim.valid, actions, action_valid, out.log_div};
+    for (const void* q : ptrs) bulk = bulk && ((uintptr_t)q & 15u) == 0;
+  }
+  const DynBulkSmem bm = dyn_bulk_layout(sim.A, p.C);
+  const size_t dsmem = 2 * (size_t)bm.in_bytes;
+  bulk = bulk && dsmem <= 200 * 1024;
+  if (bulk) {
+    const unsigned nt = (unsigned)((sim.A + 31) / 32 * 32);
+    if (h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE) {
+      e = cudaFuncSetAttribute(k_rollout_dyn_bulk<WM_DYN_INVERTIBLE_BICYCLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem);
+      if (e != cudaSuccess) return e;
+      k_rollout_dyn_bulk<WM_DYN_INVERTIBLE_BICYCLE><<<(unsigned)sim.B, nt, dsmem, s>>>(p);
+    } else {
+      e = cudaFuncSetAttribute(k_rollout_dyn_bulk<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem);
+      if (e != cudaSuccess) return e;
+      k_rollout_dyn_bulk<-1><<<(unsigned)sim.B, nt, dsmem, s>>>(p);
+    }
+  } else if (h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE) k_rollout_dyn<WM_DYN_INVERTIBLE_BICYCLE><<<(unsigned)n_dyn, DYN_NT, 0, s>>>(p);
   else k_rollout_dyn<-1><<<(unsigned)n_dyn, DYN_NT, 0, s>>>(p);
   h->launches++;
-  cudaError_t e = cudaGetLastError();
+  e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (ev) cudaEventRecord(ev[1], s);
   // ---- its metrics ----
