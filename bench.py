@@ -15,7 +15,7 @@ value     device-resident: inputs in HBM when the timed region starts, CUDA even
 e2e       the same job through wm_rollout_host with pinned HOST buffers: scenario + action
           upload, wm_prepare, reset, rollout, metric download all inside the timed region
           (pipelined over scenario chunks: its floor is the PCIe time of the 3.8 GB upload).
-roofline  the rollout graph = k_rollout_dyn + k_rollout_metrics (one launch of each per 80-step rollout).  The
+roofline  the rollout graph = k_rollout_dyn(_bulk) + k_rollout_metrics (one launch of each per 80-step rollout).  The
           exact grid search leaves ~0.1 % of the corner-segment pairs, so the slower roof of the graph is its
           compulsory HBM IO (actions + log row in, sim row + metric rows out, per agent-step):
           achieved = those bytes / CUDA-event duration of the two launches, against the measured HBM peak;
@@ -775,19 +775,21 @@ def main():
     met_bytes = n_as * (21 + 6)                                                    # k_rollout_metrics: x, y, yaw, length, width, valid in; 2 flags + distance out
     fused_flops = pairs_eval * N_STEPS * FLOP_PER_PAIR
     roll_ms = dyn_ms + met_ms
-    tr_dyn, src_dyn = profiled_traffic("k_rollout_dyn")
+    tr_dyn, src_dyn = profiled_traffic("k_rollout_dyn_bulk")          # A % 16 == 0: the bulk-staged variant runs
+    if tr_dyn is None:
+        tr_dyn, src_dyn = profiled_traffic("k_rollout_dyn")
     tr_met, src_met = profiled_traffic("k_rollout_metrics")
     roofline = {"bound": "hbm", "achieved": fused_bytes / (roll_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": fused_bytes / (roll_ms * 1e-3) / 1e9 / hbm_peak,
                 "traffic": (tr_dyn + tr_met) if (tr_dyn is not None and tr_met is not None) else None, "traffic_source": src_met,
-                "kernel": "k_rollout_dyn + k_rollout_metrics (the rollout graph: one launch of each per 80-step rollout)",
+                "kernel": "k_rollout_dyn_bulk + k_rollout_metrics (the rollout graph: one launch of each per 80-step rollout)",
                 "kernel_ms": roll_ms, "graph_replay_ms": kf_ms, "algorithmic_bytes_per_launch": fused_bytes,
                 "peak_source": hbm_src, "kernel_share_of_step": roll_ms / ms_step,
                 "hbm_time_ms_at_peak": fused_bytes / (hbm_peak * 1e9) * 1e3,
                 "kernels": {
                     "k_rollout_metrics": {"ms": met_ms, "share_of_step": met_ms / ms_step, "algorithmic_bytes_per_launch": met_bytes,
                                           "hbm_frac": met_bytes / (met_ms * 1e-3) / 1e9 / hbm_peak, "traffic": tr_met,
-                                          "bound_observed": "instruction issue (ncu: profiles/r02_k_rollout_metrics_ncu.md), not HBM and not the FP32 pipe",
+                                          "bound_observed": "instruction issue (ncu: profiles/r02_k_rollout_ncu.md), not HBM and not the FP32 pipe",
                                           "alu_frac_on_evaluated_pairs": fused_flops / (met_ms * 1e-3) / 1e12 / fp32_peak},
                     "k_rollout_dyn": {"ms": dyn_ms, "share_of_step": dyn_ms / ms_step, "algorithmic_bytes_per_launch": dyn_bytes,
                                       "hbm_frac": dyn_bytes / (dyn_ms * 1e-3) / 1e9 / hbm_peak, "traffic": tr_dyn}},
