@@ -366,10 +366,21 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
     const int nr = S.n_rows;
     for (int r = warp; r < nr; r += TK_THREADS / 32) {
       const int s0 = S.row_s0[r], base = S.row_base[r], cnt = S.row_base[r + 1] - base;
-      for (int i = lane; i < cnt; i += 32) {
-        const uint32_t key = key_at(s0 + i);
-        if (cached) keys[base + i] = key;
-        f(key, base + i);
+      // four points of the row in flight per lane: the loads do not depend on one another
+      for (int i0 = lane; i0 < cnt; i0 += 128) {
+        float2 pt[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) pt[u] = __ldg(pxy + s0 + min(i0 + 32 * u, cnt - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int i = i0 + 32 * u;
+          if (i < cnt) {
+            const float dx = __fsub_rn(pt[u].x, ex), dy = __fsub_rn(pt[u].y, ey);
+            const uint32_t key = __float_as_uint(__fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            if (cached) keys[base + i] = key;
+            f(key, base + i);
+          }
+        }
       }
     }
   };
@@ -453,6 +464,7 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
       for (int ib = 0; ib < cnt; ib += 32) {
         const int i = ib + lane;
         bool take = false, tie = false;
+        const int idx = __ldg(pidx + s0 + min(i, cnt - 1));        // requested before the key decides: no dependent miss
         if (i < cnt) {
           const uint32_t key = cached ? keys[base + i] : key_at(s0 + i);
           take = key < T || (key == T && !trim);
@@ -460,7 +472,6 @@ __global__ void __launch_bounds__(TK_THREADS) k_observe_topk(TopkParams p) {
         }
         const uint32_t bal = __ballot_sync(0xffffffffu, take);
         if (take || tie) {
-          const int idx = __ldg(pidx + s0 + i);
           atomicOr((take ? bm : tb) + (idx >> 5), 1u << (idx & 31));
           if (take) {
             int q0 = 0;
