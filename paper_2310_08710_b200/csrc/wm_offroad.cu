@@ -45,7 +45,7 @@ __device__ __forceinline__ bool rg_record(const RgView& g, int64_t o, int i, boo
   return rg_is_edge(g, o, i) && !(i > 0 && rg_starts(g, o, i - 1));
 }
 
-__global__ void __launch_bounds__(256) k_count_segments(RgView g, int32_t* n_seg) {
+__global__ void __launch_bounds__(1024) k_count_segments(RgView g, int32_t* n_seg) {
   __shared__ int s_cnt;
   if (threadIdx.x == 0) s_cnt = 0;
   __syncthreads();
@@ -64,26 +64,28 @@ __global__ void __launch_bounds__(256) k_count_segments(RgView g, int32_t* n_seg
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(1024) k_order_segments(RgView g, int cap, int32_t* seg_src) {
   __shared__ int s_w[32];
-  __shared__ int s_base;
   const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t o = (int64_t)b * g.R;
   int32_t* out = seg_src + (int64_t)b * cap;
-  if (tid == 0) s_base = 0;
+  // a thread owns a contiguous stretch of points: count, one block scan, write (two barriers in all)
+  const int per = (g.R + 1023) / 1024, i0 = tid * per, i1 = min(g.R, i0 + per);
+  int c = 0;
+  bool sg;
+  for (int i = i0; i < i1; ++i) c += rg_record(g, o, i, &sg) ? 1 : 0;
+  int inc = c;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += u; }
+  if (lane == 31) s_w[warp] = inc;
   __syncthreads();
-  for (int base = 0; base < g.R; base += 1024) {
-    const int i = base + tid;
-    bool sg;
-    const bool rec = rg_record(g, o, i, &sg);
-    const uint32_t bal = __ballot_sync(0xffffffffu, rec);
-    if (lane == 0) s_w[warp] = __popc(bal);
-    __syncthreads();
-    int pre = s_base;
-    for (int w = 0; w < warp; ++w) pre += s_w[w];
-    if (rec) out[pre + __popc(bal & ((1u << lane) - 1u))] = i;
-    __syncthreads();
-    if (tid == 0) { int tot = 0; for (int w = 0; w < 32; ++w) tot += s_w[w]; s_base += tot; }
-    __syncthreads();
+  if (warp == 0) {
+    int v = s_w[lane], w = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int u = __shfl_up_sync(0xffffffffu, w, d); if (lane >= d) w += u; }
+    s_w[lane] = w - v;
   }
+  __syncthreads();
+  int pos = s_w[warp] + inc - c;
+  for (int i = i0; i < i1; ++i) if (rg_record(g, o, i, &sg)) out[pos++] = i;
 }
 
 // position of stored segment s inside its tile: lane = (s%512)/16, it = (s%16)/2, half = s&1 (wm_internal.cuh)
@@ -104,7 +106,7 @@ __device__ __forceinline__ void store_segment(float* tile_base, float2* sign_dir
 // One warp per group of 64 stored segments: writes the tile records (brute-force layout), the
 // 32-byte records of the grid search and their pair form, and the bounding box of each chunk of 32.
 __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, const int32_t* n_seg, float4* edges,
-                                                       float2* sign_dir, int32_t* seg_src, float4* segrec, float4* segpair, float4* seglk, float4* segfin, float4* chunks) {
+                                                       float2* sign_dir, int32_t* seg_src, float4* segrec, float4* segpair, float4* seglk, float4* segfin, float4* chunks, int tiles_on) {
   const int b = blockIdx.y, lane = threadIdx.x & 31;
   const int grp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int ngrp = seg_tiles * (WM_TILE_SEGS / 64);
@@ -134,7 +136,7 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
       float gx = 0.f, gy = 0.f, sx, sy;
       if (ee > 0.f) { gx = ex / ee; gy = ey / ee; sx = ex; sy = ey; }
       else { ex = 0.f; ey = 0.f; sx = g.dir_x[o + i]; sy = g.dir_y[o + i]; }     // D16 / D29
-      store_segment(tile_base, sd, s, p0x, p0y, ex, ey, gx, gy, sx, sy);
+      if (tiles_on) store_segment(tile_base, sd, s, p0x, p0y, ex, ey, gx, gy, sx, sy);     // the brute-force kernel's layout: only that mode reads it
       float4* rec = segrec + ((int64_t)b * cap + s) * 2;
       rec[0] = make_float4(p0x, p0y, ex, ey);
       rec[1] = make_float4(gx, gy, sx, sy);
@@ -158,7 +160,7 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
       x0 = fminf(x0, fminf(ax[hf], bx[hf])); x1 = fmaxf(x1, fmaxf(ax[hf], bx[hf]));
       y0 = fminf(y0, fminf(ay[hf], by[hf])); y1 = fmaxf(y1, fmaxf(ay[hf], by[hf]));
     } else {                                      // padding: far away, never wins against a real segment
-      store_segment(tile_base, sd, s, WM_FAR, WM_FAR, 0.f, 0.f, 0.f, 0.f, 1.f, 0.f);
+      if (tiles_on) store_segment(tile_base, sd, s, WM_FAR, WM_FAR, 0.f, 0.f, 0.f, 0.f, 1.f, 0.f);
       float4* rec = segrec + ((int64_t)b * cap + s) * 2;
       rec[0] = make_float4(WM_FAR, WM_FAR, 0.f, 0.f);
       rec[1] = make_float4(0.f, 0.f, 1.f, 0.f);
@@ -219,7 +221,7 @@ int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_m
     WM_CUDA(cudaMalloc(&h->pool_cnt, (size_t)B * sizeof(int32_t)));
     h->prep_B = B; h->prep_R = R;
   }
-  k_count_segments<<<B, 256, 0, s>>>(g, h->n_seg);
+  k_count_segments<<<B, 1024, 0, s>>>(g, h->n_seg);
   h->launches++;
   WM_CUDA(cudaGetLastError());
   int32_t* host = (int32_t*)malloc((size_t)B * sizeof(int32_t));
@@ -271,7 +273,7 @@ int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaS
     k_fill_segments<<<dim3((ngrp + 7) / 8, nb), 256, 0, s>>>(g, tiles, h->n_seg + b0, h->edges + (int64_t)b0 * tiles * WM_TILE_F4,
                                                              h->sign_dir + b0 * cap, seg_src, h->segrec + b0 * cap * 2,
                                                              h->segpair + b0 * (cap / 2) * 3, h->seglk + b0 * (cap / 2) * 2, h->segfin + b0 * cap,
-                                                             h->chunks + b0 * (cap / WM_CHUNK));
+                                                             h->chunks + b0 * (cap / WM_CHUNK), h->cfg.offroad_mode == WM_OFFROAD_BRUTE_FORCE);
   }
   h->launches++;
   WM_CUDA(cudaGetLastError());
