@@ -22,6 +22,7 @@
 // ======================================================================================
 constexpr int BUILD_MAXRUN = WM_GRID_MAXRUN;   // runs per cell before the cell falls back to the full search
 constexpr int BUILD_MAXCAND = 256;        // candidates per cell before it falls back
+constexpr int BUILD_WARPS = 4;            // warps per CTA of the build kernels (8: 0.6 ms slower, the warps of a CTA end at very different times)
 constexpr int BUILD_AHEAD = 8;            // scenarios between a CTA and the one whose records it prefetches into L2
 
 __global__ void __launch_bounds__(128) k_grid_params(const int32_t* n_seg, const float4* chunks, int seg_cap, float h_min,
@@ -133,10 +134,10 @@ __device__ __forceinline__ void slab_keep(const float4 NE, const float4 L0, cons
 // of the mask are the cell's runs, already in the header's format (first pair << 5 | pairs).
 // LEVEL 0: outer cells, 1: mid cells, 2: inner cells
 template <int LEVEL>
-__global__ void __launch_bounds__(256, 4) k_build_cells(const float4* segrec, const float4* segpair, const float4* seglk, const float4* chunks,
+__global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k_build_cells(const float4* segrec, const float4* segpair, const float4* seglk, const float4* chunks,
                                                      int seg_cap, const WmGrid* gridp, uint2* cells, uint32_t* pool,
                                                      int32_t* pool_cnt) {
-  __shared__ uint32_t s_runs[8][BUILD_MAXRUN][32];
+  __shared__ uint32_t s_runs[BUILD_WARPS][BUILD_MAXRUN][32];
   const int b = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const WmGrid g = gridp[b];
   // A scenario's records are read by its own CTAs only, all at about the same time: every first touch
@@ -153,7 +154,7 @@ __global__ void __launch_bounds__(256, 4) k_build_cells(const float4* segrec, co
   }
   // the warp's block of 8 x 4 cells of its level
   constexpr bool FINE = LEVEL > 0;
-  const int wg = blockIdx.x * 8 + warp;
+  const int wg = blockIdx.x * BUILD_WARPS + warp;
   const int gnx = LEVEL == 0 ? g.onx : LEVEL == 1 ? (g.nx >> 1) : g.nx, gny = LEVEL == 0 ? g.ony : LEVEL == 1 ? (g.ny >> 1) : g.ny;
   const float gx0 = FINE ? g.x0 : g.ox0, gy0 = FINE ? g.y0 : g.oy0, h = LEVEL == 0 ? g.oh : LEVEL == 1 ? 2.f * g.h : g.h;
   const int cbase = LEVEL == 0 ? g.obase : LEVEL == 1 ? g.mbase : 0;
@@ -431,15 +432,15 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
   uint2* cells = h->cells + (int64_t)b0 * WM_GRID_CELLS;
   uint32_t* pool = h->pool + (int64_t)b0 * WM_POOL_CAP;
   // the outer grid first: its cells are the parents the inner cells build from
-  k_build_cells<0><<<dim3((WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  k_build_cells<0><<<dim3((WM_GRID_NG_OUT / 8) * (WM_GRID_NG_OUT / 4) / BUILD_WARPS, B), 32 * BUILD_WARPS, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  k_build_cells<1><<<dim3((WM_GRID_NG_IN / 16) * (WM_GRID_NG_IN / 8) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  k_build_cells<1><<<dim3((WM_GRID_NG_IN / 16) * (WM_GRID_NG_IN / 8) / BUILD_WARPS, B), 32 * BUILD_WARPS, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  k_build_cells<2><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / 8, B), 256, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  k_build_cells<2><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / BUILD_WARPS, B), 32 * BUILD_WARPS, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
   h->launches++;
   return cudaGetLastError();
 }
