@@ -148,7 +148,8 @@ __global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k
     const uint32_t np = (uint32_t)((gridp[bn].nseg + 1) >> 1), per = (np + gridDim.x - 1) / gridDim.x;
     const uint32_t p0 = min(np, per * blockIdx.x), p1 = min(np, p0 + per);
     if (p1 > p0) {
-      l2_prefetch(segpair + ((int64_t)bn * (seg_cap / 2) + p0) * 3, (p1 - p0) * 48u);
+      const float4* pn = segpair + (int64_t)bn * (seg_cap / 2) * 3 + p0;
+      l2_prefetch(pn, (p1 - p0) * 16u); l2_prefetch(pn + seg_cap / 2, (p1 - p0) * 16u); l2_prefetch(pn + 2 * (seg_cap / 2), (p1 - p0) * 16u);
       l2_prefetch(seglk + ((int64_t)bn * (seg_cap / 2) + p0) * 2, (p1 - p0) * 32u);
     }
   }
@@ -163,7 +164,8 @@ __global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k
   const int bx = wg % nbx, by = wg / nbx;
   const int ix = bx * 8 + (lane & 7), iy = by * 4 + (lane >> 3);
   const float4* rec = segrec + (int64_t)b * seg_cap * 2;
-  const float4* pair = segpair + (int64_t)b * (seg_cap / 2) * 3;
+  const float4* pair = segpair + (int64_t)b * (seg_cap / 2) * 3;     // three planes of PS parts (wm_grid.cuh)
+  const int PS = seg_cap / 2;
   const float4* lk = seglk + (int64_t)b * (seg_cap / 2) * 2;
   const float4* ch = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
   uint2* cells_b = cells + (int64_t)b * WM_GRID_CELLS;
@@ -205,7 +207,7 @@ __global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k
   };
   // pass 2 on one pair record: does it hold a candidate of this cell?
   auto pair_hit = [&](int pid, float thr2) -> bool {
-    const float4 P = __ldg(pair + 3 * pid), NE = __ldg(pair + 3 * pid + 1), G = __ldg(pair + 3 * pid + 2);
+    const float4 P = __ldg(pair + pid), NE = __ldg(pair + PS + pid), G = __ldg(pair + 2 * PS + pid);
     const float4 L0 = __ldg(lk + 2 * pid), L1 = __ldg(lk + 2 * pid + 1);
     wm_u64 wx, wy;
     float de, dq;
@@ -243,7 +245,7 @@ __global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k
           const int pid = first + q;
           wm_u64 wx, wy;
           float de, dq;
-          centre_pair_d2(__ldg(pair + 3 * pid), __ldg(pair + 3 * pid + 1), __ldg(pair + 3 * pid + 2), cx2, cy2, wx, wy, de, dq);
+          centre_pair_d2(__ldg(pair + pid), __ldg(pair + PS + pid), __ldg(pair + 2 * PS + pid), cx2, cy2, wx, wy, de, dq);
           dmin2 = fminf(dmin2, fminf(de, dq));
         }
       });
@@ -315,7 +317,7 @@ __global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k
       uint32_t need = __ballot_sync(0xffffffffu, in && wm_chunk_lb2(__ldg(ch + c), cx, cy) < dmin2);
       if (!need) return;
       const int pid = c * CP + q;
-      const float4 P = __ldg(pair + 3 * pid), NE = __ldg(pair + 3 * pid + 1), G = __ldg(pair + 3 * pid + 2);
+      const float4 P = __ldg(pair + pid), NE = __ldg(pair + PS + pid), G = __ldg(pair + 2 * PS + pid);
       while (need) {
         const int i0 = __ffs(need) - 1;
         need &= need - 1;
@@ -339,7 +341,7 @@ __global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k
       while (mask) {
         const int c = r * 32 + __ffs(mask) - 1;
         mask &= mask - 1;
-        const float4 Pa = __ldg(pair + 3 * (c * CP)), Pb = __ldg(pair + 3 * (c * CP + CP / 2));      // p0 of records 32 c and 32 c + 16 (1e18 if padding)
+        const float4 Pa = __ldg(pair + c * CP), Pb = __ldg(pair + c * CP + CP / 2);      // p0 of records 32 c and 32 c + 16 (1e18 if padding)
         const float ax = cx - Pa.x, ay = cy - Pa.z, bx2 = cx - Pb.x, by2 = cy - Pb.z;
         dmin2 = fminf(dmin2, fminf(fmaf(ax, ax, ay * ay), fmaf(bx2, bx2, by2 * by2)));
       }
@@ -367,7 +369,7 @@ __global__ void __launch_bounds__(32 * BUILD_WARPS, 1024 / (32 * BUILD_WARPS)) k
         uint32_t need = __ballot_sync(0xffffffffu, wm_chunk_lb2(__ldg(ch + c), cx, cy) <= thr2c);
         if (!need) continue;
         const int pid = c * CP + q;
-        const float4 P = __ldg(pair + 3 * pid), NE = __ldg(pair + 3 * pid + 1), G = __ldg(pair + 3 * pid + 2);
+        const float4 P = __ldg(pair + pid), NE = __ldg(pair + PS + pid), G = __ldg(pair + 2 * PS + pid);
         const float4 L0 = __ldg(lk + 2 * pid), L1 = __ldg(lk + 2 * pid + 1);
         uint32_t mine = 0u;
         while (need) {

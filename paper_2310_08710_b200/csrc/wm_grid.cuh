@@ -33,9 +33,10 @@ __host__ __device__ __forceinline__ int wm_cell_index(int ix, int iy, int nx) {
 struct WmGridView {          // one scenario's prepared search structures
   const float4* rec;         // [nseg][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}
   const float4* fin;         // [nseg] {p0x, p0y, sx, sy}
-  const float4* pair;        // [ceil(nseg/2)][3] records 2p (e) and 2p+1 (o): {p0x_e,p0x_o,p0y_e,p0y_o} {-ex_e,-ex_o,-ey_e,-ey_o} {gx_e,gx_o,gy_e,gy_o}
+  const float4* pair;        // [3][seg_cap/2] three planes; pair record p = records 2p (e) and 2p+1 (o): {p0x_e,p0x_o,p0y_e,p0y_o} | {-ex_e,-ex_o,-ey_e,-ey_o} | {gx_e,gx_o,gy_e,gy_o}
   const char* pair0;         // pair records of scenario 0 of the launch; this scenario's start at byte pair_off (< 2^32: the launchers see to it)
   uint32_t pair_off;
+  uint32_t plane;            // bytes between the planes of a scenario = seg_cap / 2 * 16
   const float4* chunks;      // [ceil(nseg/32)] bounding boxes {x0,y0,x1,y1}
   const uint2* cells;        // headers, 2 x 2 tiles (wm_cell_index)
   const uint32_t* pool;      // overflow runs
@@ -50,6 +51,7 @@ __device__ __forceinline__ WmGridView wm_grid_view(const float4* segrec, const f
   v.pair = segpair + (int64_t)b * (seg_cap / 2) * 3;
   v.pair0 = (const char*)segpair;
   v.pair_off = (uint32_t)b * (uint32_t)(seg_cap / 2) * 48u;
+  v.plane = (uint32_t)(seg_cap / 2) * 16u;
   v.fin = segfin + (int64_t)b * seg_cap;
   v.chunks = chunks + (int64_t)b * (seg_cap / WM_CHUNK);
   v.cells = cells + (int64_t)b * WM_GRID_CELLS;
@@ -94,13 +96,17 @@ __device__ __forceinline__ void wm_pair_d2(const float4 P, const float4 NE, cons
 // indices are visited in ascending order with strict '<').  Padding records sit at 1e18.
 // The current run is one word, (pair << 5 | pairs left): an iteration adds 31 to it; the next two
 // runs wait in registers, further ones come from the pool.
-// The winner comes back as `bso` = byte offset of its pair record from the scenario's first (a multiple
-// of 48) + 1 for the odd record of the pair; wm_bso_of / wm_rec_of convert.  Inside the walk offsets
+// The three 16-byte parts of a pair record live in three PLANES of the scenario's block (all first parts, all
+// second parts, all third parts): the lanes of a warp walk neighbouring records, and eight neighbouring parts
+// share a 128-byte line where the 48-byte records of an array-of-structures share it between 2.7 (the walk's
+// loads are bound by the LSU's line wavefronts, profiles/r02_k_rollout_ncu.md).
+// The winner comes back as `bso` = byte offset of its first part from the scenario's first (a multiple
+// of 16) + 1 for the odd record of the pair; wm_bso_of / wm_rec_of convert.  Inside the walk offsets
 // count from the first pair record of the LAUNCH (32 bits: one uniform base + a 32-bit lane offset).
-__device__ __forceinline__ uint32_t wm_bso_of(int rec) { return (uint32_t)(rec >> 1) * 48u + (uint32_t)(rec & 1); }
-__device__ __forceinline__ int wm_rec_of(uint32_t bso) { return (int)(2u * ((bso & ~1u) / 48u) + (bso & 1u)); }
+__device__ __forceinline__ uint32_t wm_bso_of(int rec) { return (uint32_t)(rec >> 1) * 16u + (uint32_t)(rec & 1); }
+__device__ __forceinline__ int wm_rec_of(uint32_t bso) { return (int)(2u * (bso >> 4) + (bso & 1u)); }
 
-__device__ __forceinline__ void wm_grid_walk(const char* __restrict__ base, uint32_t off0, uint32_t r0, uint32_t r1, uint32_t r2,
+__device__ __forceinline__ void wm_grid_walk(const char* __restrict__ base, uint32_t off0, uint32_t plane, uint32_t r0, uint32_t r1, uint32_t r2,
                                              const uint32_t* __restrict__ pool, float cx, float cy, float offx, float offy,
                                              float& best, uint32_t& bso, int& n_eval) {
   const wm_u64 cx2 = pk2(cx, cx), cy2 = pk2(cy, cy), ox2 = pk2(offx, offx), oy2 = pk2(offy, offy);
@@ -111,21 +117,21 @@ __device__ __forceinline__ void wm_grid_walk(const char* __restrict__ base, uint
     r2 = __ldg(pool + 1);
     pool += 2; n_pool -= 1;
   }
-  uint32_t off = off0 + (r0 >> 5) * 48u, cnt = r0 & 31u;            // the open run: byte offset of its next pair record, pairs left
+  uint32_t off = off0 + (r0 >> 5) * 16u, cnt = r0 & 31u;            // the open run: byte offset of its next pair record, pairs left
   for (;;) {
     if (cnt == 0u) {                                                // run finished: the next one
       if (r1 == 0u) break;
-      off = off0 + (r1 >> 5) * 48u; cnt = r1 & 31u;
+      off = off0 + (r1 >> 5) * 16u; cnt = r1 & 31u;
       r1 = r2; r2 = 0u;
       if (n_pool > 0) { r2 = __ldg(pool); ++pool; --n_pool; }
     }
-    const float4* a = (const float4*)(base + off);
-    const float4 a0 = __ldg(a), a1 = __ldg(a + 1), a2 = __ldg(a + 2);
+    const char* a = base + off;
+    const float4 a0 = __ldg((const float4*)a), a1 = __ldg((const float4*)(a + plane)), a2 = __ldg((const float4*)(a + 2u * plane));
     float d0, d1;
     wm_pair_d2(a0, a1, a2, cx2, cy2, ox2, oy2, d0, d1);
     if (d0 < best) { best = d0; bso = off; }                        // ascending index, strict '<': exact ties -> lower index (D17)
     if (d1 < best) { best = d1; bso = off + 1u; }
-    off += 48u; --cnt;
+    off += 16u; --cnt;
     n_eval += 2;
   }
   bso -= off0;
@@ -277,7 +283,7 @@ __device__ __forceinline__ bool wm_grid_fast_hd(const WmGridView& v, uint2 hd, f
   // the three 21-bit fields; bit 21 of the third = "pool offset"
   const uint32_t r0 = hd.x & 0x1fffffu, r1 = ((hd.x >> 21) | (hd.y << 11)) & 0x1fffffu, r2 = hd.y >> 10;
   bso = v.pair_off;
-  wm_grid_walk(v.pair0, v.pair_off, r0, r1, r2, v.pool, cx, cy, offx, offy, best, bso, n_eval);   // no-op without runs
+  wm_grid_walk(v.pair0, v.pair_off, v.plane, r0, r1, r2, v.pool, cx, cy, offx, offy, best, bso, n_eval);   // no-op without runs
   return slow;
 }
 
@@ -287,8 +293,8 @@ __device__ __forceinline__ float wm_grid_finish(const WmGridView& v, float cx, f
   // e x (q - p0) > 0 is the left side of the oriented segment = on-road (D16).  p0 and e come from
   // the winner's pair record, which the walk has just pulled into L1 (no third dependent miss);
   // only a zero-length segment needs its stored direction from the finish record (D16 / D29).
-  const float4* a = (const float4*)((const char*)v.pair + (bso & ~1u));
-  const float4 P = __ldg(a), NE = __ldg(a + 1);
+  const char* a = (const char*)v.pair + (bso & ~1u);
+  const float4 P = __ldg((const float4*)a), NE = __ldg((const float4*)(a + v.plane));
   const bool odd = (bso & 1u) != 0u;
   const float p0x = odd ? P.y : P.x, p0y = odd ? P.w : P.z;
   float sx = -(odd ? NE.y : NE.x), sy = -(odd ? NE.w : NE.z);

@@ -80,7 +80,7 @@ struct wm_handle {
   int32_t* seg_src;         // [B][seg_tiles*512]  first-point index of each stored segment (-1: padding)
   float4* segrec;           // [B][seg_tiles*512][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}, ascending source order
   float4* segfin;           // [B][seg_tiles*512] {p0x, p0y, sx, sy}: what the sign of the winner needs
-  float4* segpair;          // [B][seg_tiles*256][3] the same records two by two, component-wise (wm_grid.cuh)
+  float4* segpair;          // [B][3][seg_tiles*256] the same records two by two, component-wise, in three planes (wm_grid.cuh)
   float4* seglk;            // [B][seg_tiles*256][2] per pair record, for the cell build only (wm_grid.cu): what the
                             //   neighbour rules P / N need - {fx, fx', fy, fy'} {aP, aP', aN, aN'}, f = e of the NEXT record
                             //   of the same polyline (0 if none), aP / aN = |ex| + |ey| when the rule can apply, +inf otherwise

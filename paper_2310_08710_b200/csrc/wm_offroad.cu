@@ -171,10 +171,10 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
     }
   }
   {                                               // the lane's two records as one pair record
-    float4* pr = segpair + ((int64_t)b * (cap / 2) + grp * 32 + lane) * 3;
+    float4* pr = segpair + (int64_t)b * (cap / 2) * 3 + grp * 32 + lane;       // three planes of cap / 2 parts (wm_grid.cuh)
     pr[0] = make_float4(pp[0][0], pp[1][0], pp[0][1], pp[1][1]);
-    pr[1] = make_float4(pp[0][2], pp[1][2], pp[0][3], pp[1][3]);
-    pr[2] = make_float4(pp[0][4], pp[1][4], pp[0][5], pp[1][5]);
+    pr[cap / 2] = make_float4(pp[0][2], pp[1][2], pp[0][3], pp[1][3]);
+    pr[2 * (cap / 2)] = make_float4(pp[0][4], pp[1][4], pp[0][5], pp[1][5]);
     float4* pl = seglk + ((int64_t)b * (cap / 2) + grp * 32 + lane) * 2;
     pl[0] = make_float4(lk[0][0], lk[1][0], lk[0][1], lk[1][1]);
     pl[1] = make_float4(lk[0][2], lk[1][2], lk[0][3], lk[1][3]);
