@@ -88,7 +88,7 @@ def write_traffic(csv_path):
         a[r[0]] += float(r[mv].replace(",", "")) * scale
     kernels = {k: float(np.mean(list(v.values()))) for k, v in acc.items()}
     out = {"source_sha256": source_hash(), "kernels": kernels, "unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
-           "command": "ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum --clock-control none --csv; bench.py --write-traffic"}
+           "command": "ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum --clock-control none -c 400 --csv --log-file <csv> python bench.py --steps 2 --warmup 1 --no-cpu --no-e2e --no-extras; python bench.py --write-traffic <csv>"}
     json.dump(out, open(TRAFFIC_FILE, "w"), indent=1)
     print(json.dumps(out))
     return 0
