@@ -406,3 +406,33 @@ def test_rollout_fused_equals_stepwise_bitwise_wide_scenarios(A):
     o = oracle.overlap(got, t0 + n, want_pair=False)
     cl = ~(np.abs(o["gap"]) < 1e-4).any(axis=2)
     assert np.array_equal(ov[:, n - 1][cl], o["flag"][cl])
+
+
+@pytest.mark.parametrize("dyn", ["delta_local", "delta_global"])
+def test_rollout_bulk_staged_dynamics_delta_models_ragged_stages(dyn):
+    """k_rollout_dyn_bulk (A % 16 == 0) with three action channels and a step count that is not a multiple of its
+    stage (11 steps = 2 full stages of 4 + one of 3): bitwise equal to the stepwise graph, which takes k_step."""
+    n = 11
+    cfg = ws.make_config(5, B=3, n_steps=n)
+    log = cfg["log"]
+    B, T, A = log["x"].shape
+    rng = np.random.default_rng(11)
+    acts = np.stack([rng.uniform(-0.5, 0.5, (B, n, A)), rng.uniform(-0.5, 0.5, (B, n, A)), rng.uniform(-0.1, 0.1, (B, n, A))], axis=2).astype(np.float32)
+    av = np.ascontiguousarray(cfg["action_valid"][:, :n])
+    res = []
+    for mode in (wm.WM_ROLLOUT_FUSED, wm.WM_ROLLOUT_STEPWISE):
+        h, log_d, rg_d, sim_d, _ = _setup(cfg, dynamics=dyn, rollout_mode=mode)
+        t0 = wm.wm_reset(h, log_d, sim_d)
+        out_d = wm.alloc_rollout_out(B, n, A)
+        wm.wm_rollout(h, log_d, sim_d, t0, n, torch.from_numpy(acts).cuda(), torch.from_numpy(av).cuda(), out_d)
+        torch.cuda.synchronize()
+        res.append((host(sim_d), host(out_d)))
+        wm.wm_destroy(h)
+    for k in res[0][0]:
+        assert np.array_equal(res[0][0][k], res[1][0][k], equal_nan=True), k
+    for k in res[0][1]:
+        assert np.array_equal(res[0][1][k], res[1][1][k]), k
+    # and the first step against the oracle
+    sim_o = oracle.reset(log)
+    oracle.step(log, sim_o, t0, DYN[dyn][1], np.ascontiguousarray(acts[:, 0]), np.ascontiguousarray(av[:, 0]))
+    assert_state_close(row_of(res[0][0], t0 + 1), row_of(sim_o, t0 + 1))
