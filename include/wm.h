@@ -39,7 +39,9 @@ typedef enum {
   WM_ERR_ARG = -1,          /* null / misaligned pointer, bad shape, t out of range */
   WM_ERR_CUDA = -2,         /* a CUDA call failed; see wm_last_cuda_error() */
   WM_ERR_UNSUPPORTED = -3,  /* e.g. A > 1024, B > 65535 scenarios per call, topk > R, more than 131 072 road-edge segments in a scenario */
-  WM_ERR_STATE = -4         /* e.g. metrics_offroad before wm_prepare */
+  WM_ERR_STATE = -4,        /* e.g. metrics_offroad before wm_prepare */
+  WM_ERR_TOO_LARGE = -5     /* the problem does not fit the fixed, built-in scratch of a no-allocation entry point
+                               (wm_observe_topk_static): use the regular entry point, which allocates what it needs */
 } wm_status;
 
 enum { WM_DYN_INVERTIBLE_BICYCLE = 0, WM_DYN_DELTA_LOCAL = 1, WM_DYN_DELTA_GLOBAL = 2 };   /* DELTA_GLOBAL: Eq. 1 literally (world-frame delta) */
@@ -188,6 +190,42 @@ int wm_log_divergence(wm_handle* h, const wm_traj* log, const wm_traj* sim, int3
 int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* rg, int32_t t, float* hist,
                uint8_t* hist_valid, int32_t* rg_index, float* rg_feat, int32_t* rg_type,
                void* stream);
+
+/*
+ * The top-k half of wm_observe (L82: "sub-samples the roadgraph via distance") for callers that are not
+ * allowed to allocate device memory at the point where they call the library.  Who that is:
+ *  - code running inside a training or serving job whose framework has already handed (nearly) all of the
+ *    GPU's memory to its own pooling allocator: a cudaMalloc issued by a library then fails, or eats into
+ *    the pool's head-room;
+ *  - planners and controllers with a memory budget fixed at start-up, where allocating later is forbidden;
+ *  - latency-critical loops: cudaMalloc and cudaFree stall the whole device while they run.
+ * The regular route cannot serve them: wm_create and wm_prepare call cudaMalloc (handle counters, the
+ * bucketed roadgraph points).  This function needs NO handle and calls no cudaMalloc, cudaFree, stream- or
+ * event-creating routine, nor anything else that allocates.  Its scratch memory - the roadgraph points of
+ * every scenario bucketed into a uniform grid - lives in an array that is part of the library image:
+ * about 13 MiB of every GPU that loads libwm_b200.so, held until the process exits, used or not.
+ *
+ * Same result as wm_prepare followed by wm_observe (hist = NULL) on a handle with this topk / topk_order,
+ * bit for bit: the same two kernels run (bucket the points, then select), both on `stream`, so the
+ * bucketing is redone on every call instead of once per episode.
+ *   sim, rg, t, rg_index [B][A][topk], rg_feat [B][A][4][topk], rg_type [B][A][topk]: as for wm_observe
+ *   (DEVICE pointers owned by the caller, same layouts; only x, y, yaw, valid of `sim` and x, y, dir_x,
+ *   dir_y, type, valid of `rg` are read); topk_order = WM_TOPK_BY_INDEX or WM_TOPK_BY_DISTANCE.
+ * Limits, fixed when the library is built: B <= WM_STATIC_MAX_B scenarios and B * R <= WM_STATIC_MAX_POINTS
+ * roadgraph points per call (e.g. 32 scenarios of 30 000 points).  Anything larger returns WM_ERR_TOO_LARGE
+ * and launches nothing; also A <= 1024 and 1 <= topk <= R (WM_ERR_UNSUPPORTED), as for wm_observe.
+ * Sharing: there is ONE array per GPU, shared by every call from every thread.  It keeps the last call's
+ * contents; nothing in it needs clearing, because the bucketing kernel rewrites every word the selection
+ * kernel reads.  Two calls whose kernels may run at the same time on one GPU (different streams without an
+ * event between them, or two host threads) RACE on it and return garbage: put all calls on one stream, or
+ * order them with events.  The outputs are yours as soon as the work on `stream` has completed.
+ * First call on each device: looks up the array's address on that device (cudaGetSymbolAddress, the device
+ * being current) and remembers it.  Make that first call during start-up, outside any stream capture.
+ */
+#define WM_STATIC_MAX_B 64
+#define WM_STATIC_MAX_POINTS (1 << 20)
+int wm_observe_topk_static(const wm_traj* sim, const wm_roadgraph* rg, int32_t t, int32_t topk, int32_t topk_order,
+                           int32_t* rg_index, float* rg_feat, int32_t* rg_type, void* stream);
 
 /*
  * Expert actor = inverse kinematics on the rows of a trajectory ("Expert"; L335 delta

@@ -11,13 +11,14 @@ import torch
 
 from . import _build
 
-WM_OK, WM_ERR_ARG, WM_ERR_CUDA, WM_ERR_UNSUPPORTED, WM_ERR_STATE = 0, -1, -2, -3, -4
+WM_OK, WM_ERR_ARG, WM_ERR_CUDA, WM_ERR_UNSUPPORTED, WM_ERR_STATE, WM_ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5
+WM_STATIC_MAX_B, WM_STATIC_MAX_POINTS = 64, 1 << 20
 WM_DYN_INVERTIBLE_BICYCLE, WM_DYN_DELTA_LOCAL, WM_DYN_DELTA_GLOBAL = 0, 1, 2
 WM_TYPE_LANE, WM_TYPE_ROAD_EDGE = 1, 2
 WM_OFFROAD_CULLED, WM_OFFROAD_BRUTE_FORCE = 0, 1
 WM_ROLLOUT_FUSED, WM_ROLLOUT_STEPWISE = 0, 1
 WM_TOPK_BY_INDEX, WM_TOPK_BY_DISTANCE = 0, 1
-_ERR = {-1: "WM_ERR_ARG", -2: "WM_ERR_CUDA", -3: "WM_ERR_UNSUPPORTED", -4: "WM_ERR_STATE"}
+_ERR = {-1: "WM_ERR_ARG", -2: "WM_ERR_CUDA", -3: "WM_ERR_UNSUPPORTED", -4: "WM_ERR_STATE", -5: "WM_ERR_TOO_LARGE"}
 
 TRAJ_F = ("x", "y", "yaw", "vel_x", "vel_y", "length", "width")
 RG_F = ("x", "y", "dir_x", "dir_y")
@@ -25,7 +26,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
            "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_idm_step", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable",
-           "wm_discretize_actions", "wm_actions_from_index", "wm_expert_actions_discrete", "wm_rollout_vjp", "wm_step_vjp", "wm_rollout_kernel_times", "wm_selftest_ffma")
+           "wm_discretize_actions", "wm_actions_from_index", "wm_expert_actions_discrete", "wm_rollout_vjp", "wm_step_vjp", "wm_rollout_kernel_times", "wm_selftest_ffma", "wm_observe_topk_static")
 
 
 class wm_traj(C.Structure):
@@ -288,6 +289,17 @@ def wm_observe(h, sim, rg, t, hist=None, hist_valid=None, rg_index=None, rg_feat
     _check(load().wm_observe(h, C.byref(ss), C.byref(rs) if rs is not None else None, C.c_int32(t),
                              _ptr(hist, torch.float32), _ptr(hist_valid, torch.uint8), _ptr(rg_index, torch.int32),
                              _ptr(rg_feat, torch.float32), _ptr(rg_type, torch.int32), _stream(stream)), "wm_observe")
+
+
+def wm_observe_topk_static(sim, rg, t, topk, rg_index, rg_feat, rg_type, topk_order=WM_TOPK_BY_INDEX, stream=None):
+    """Top-k observation without a handle and without any device allocation (see include/wm.h): for callers
+    whose GPU memory is already spoken for (a framework's pooled allocator, a fixed start-up budget) or who
+    cannot afford cudaMalloc's device-wide stall.  B <= WM_STATIC_MAX_B and B * R <= WM_STATIC_MAX_POINTS,
+    else WmError(WM_ERR_TOO_LARGE).  All calls share one built-in scratch array per GPU: keep them on one stream."""
+    ss, rs = traj_struct(sim), roadgraph_struct(rg)
+    _check(load().wm_observe_topk_static(C.byref(ss), C.byref(rs), C.c_int32(t), C.c_int32(topk), C.c_int32(topk_order),
+                                         _ptr(rg_index, torch.int32), _ptr(rg_feat, torch.float32),
+                                         _ptr(rg_type, torch.int32), _stream(stream)), "wm_observe_topk_static")
 
 
 def wm_rollout(h, log, sim, t0, n_steps, actions, action_valid, out, stream=None):

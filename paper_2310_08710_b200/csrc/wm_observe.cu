@@ -25,6 +25,10 @@
 //   5. ascending index order without walking the bitmap: prefix sums of the words' popcounts, then every
 //      listed index finds its rank with one popc and is stored at that place; ego-frame features follow.
 // It reads ~2.3 k of the scenario's 30 k points per ego once instead of all of them three times.
+#include <string.h>
+
+#include <mutex>
+
 #include "wm_internal.cuh"
 
 // ======================================================================================
@@ -591,4 +595,83 @@ cudaError_t wm_launch_observe_topk(wm_handle* h, const wm_traj& sim, const wm_ro
   k_observe_topk<<<dim3(sim.A, sim.B), TK_THREADS, smem, s>>>(p);
   h->launches++;
   return cudaGetLastError();
+}
+
+// ======================================================================================
+// wm_observe_topk_static: the top-k observation for callers that must not allocate
+// ======================================================================================
+// The regular route (wm_create -> wm_prepare -> wm_observe) keeps the bucketed roadgraph points in
+// buffers it obtains with cudaMalloc.  Some users of this library cannot do that where they call it:
+//   - a simulator step running inside a training job whose framework allocator has already taken
+//     (nearly) all of the HBM for its own pool, so a raw cudaMalloc from a library fails or fragments it;
+//   - a control / planning loop with a fixed memory budget that forbids allocation after start-up;
+//   - a latency-sensitive loop that cannot afford cudaMalloc / cudaFree, which synchronise the device.
+// For them the bucketed points live in the file-scope array below, reserved in the library's image: every
+// GPU that loads libwm_b200.so holds its WM_STATIC_BYTES (about 13 MiB) from then until the process exits,
+// whether or not this entry point is ever called.  The entry point needs no wm_handle (creating one
+// allocates) and calls no cudaMalloc / cudaFree / stream or event creation: two kernel launches
+// (k_point_grid, k_observe_topk - the same kernels and arithmetic as wm_prepare + wm_observe) on the
+// caller's stream.
+//
+// Layout of the array (bytes): [pt_xy: MAX_POINTS float2][pt_idx: MAX_POINTS int32]
+//                              [pt_start: MAX_B x (WM_PT_CELLS + 1) int32][pt_grid: MAX_B WmPtGrid]
+// A call with B scenarios of R points uses the first B * R entries of pt_xy / pt_idx and the first B rows of
+// the other two.  Nothing in it has to start at zero: k_point_grid rewrites every word that k_observe_topk
+// reads for the same (B, R) (cell starts 0 .. ncell, the grid descriptor, the nvalid bucketed points), so
+// the previous call's contents are simply overwritten or left unread.
+//
+// In HOST code the name g_wm_static_obs is only a stand-in the runtime knows the symbol by, not a device
+// address; the address comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr size_t WM_ST_OFF_IDX = (size_t)WM_STATIC_MAX_POINTS * sizeof(float2);
+constexpr size_t WM_ST_OFF_START = WM_ST_OFF_IDX + (size_t)WM_STATIC_MAX_POINTS * sizeof(int32_t);
+constexpr size_t WM_ST_OFF_GRID = (WM_ST_OFF_START + (size_t)WM_STATIC_MAX_B * (WM_PT_CELLS + 1) * sizeof(int32_t) + 255) / 256 * 256;
+constexpr size_t WM_STATIC_BYTES = WM_ST_OFF_GRID + (size_t)WM_STATIC_MAX_B * sizeof(WmPtGrid);
+static_assert(WM_ST_OFF_IDX % 256 == 0 && WM_ST_OFF_START % 256 == 0, "pieces of the static scratch stay 256-byte aligned");
+
+static __device__ __align__(256) unsigned char g_wm_static_obs[WM_STATIC_BYTES];
+
+constexpr int WM_STATIC_MAX_DEVICES = 64;
+static std::mutex g_wm_static_mu;
+static unsigned char* g_wm_static_ptr[WM_STATIC_MAX_DEVICES];     // device address of the array on each device, once known
+
+// Set-up, once per device: the current device's address of the array.  Allocates nothing.
+static int wm_static_base(unsigned char** out) {
+  int dev = -1;
+  WM_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= WM_STATIC_MAX_DEVICES) return WM_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_wm_static_mu);
+  if (!g_wm_static_ptr[dev]) {
+    int major = 0;
+    WM_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return WM_ERR_UNSUPPORTED;                   // sm_100a kernels only; no fallback
+    unsigned char* ptr = nullptr;
+    WM_CUDA(cudaGetSymbolAddress((void**)&ptr, g_wm_static_obs));
+    if (!ptr) return WM_ERR_CUDA;
+    g_wm_static_ptr[dev] = ptr;
+  }
+  *out = g_wm_static_ptr[dev];
+  return WM_OK;
+}
+
+extern "C" int wm_observe_topk_static(const wm_traj* sim, const wm_roadgraph* rg, int32_t t, int32_t topk, int32_t topk_order,
+                                      int32_t* rg_index, float* rg_feat, int32_t* rg_type, void* stream) {
+  if (!sim || !rg || !rg_index || !rg_feat || !rg_type) return WM_ERR_ARG;
+  if (sim->B < 1 || sim->A < 1 || sim->T < 1 || rg->B != sim->B || rg->R < 1 || t < 0 || t >= sim->T) return WM_ERR_ARG;
+  if (!sim->x || !sim->y || !sim->yaw || !sim->valid || !rg->x || !rg->y || !rg->dir_x || !rg->dir_y || !rg->type || !rg->valid) return WM_ERR_ARG;
+  if (topk_order != WM_TOPK_BY_INDEX && topk_order != WM_TOPK_BY_DISTANCE) return WM_ERR_ARG;
+  if (sim->B > WM_STATIC_MAX_B || (int64_t)sim->B * rg->R > WM_STATIC_MAX_POINTS) return WM_ERR_TOO_LARGE;   // the array is what it is
+  if (sim->A > 1024 || topk < 1 || topk > rg->R) return WM_ERR_UNSUPPORTED;
+  unsigned char* base = nullptr;
+  const int rc = wm_static_base(&base);
+  if (rc != WM_OK) return rc;
+  // the launchers of the regular path read only these fields of a handle: a zeroed one on the stack
+  // pointing into the static array runs the very same launches
+  wm_handle tmp;
+  memset(&tmp, 0, sizeof(tmp));
+  tmp.cfg.topk = topk; tmp.cfg.topk_order = topk_order;
+  tmp.pt_xy = (float2*)base; tmp.pt_idx = (int32_t*)(base + WM_ST_OFF_IDX);
+  tmp.pt_start = (int32_t*)(base + WM_ST_OFF_START); tmp.pt_grid = (WmPtGrid*)(base + WM_ST_OFF_GRID);
+  WM_CUDA(wm_launch_point_grid(&tmp, *rg, 0, rg->B, (cudaStream_t)stream));
+  WM_CUDA(wm_launch_observe_topk(&tmp, *sim, *rg, t, rg_index, rg_feat, rg_type, (cudaStream_t)stream));
+  return WM_OK;
 }
