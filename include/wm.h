@@ -268,7 +268,9 @@ typedef struct { int32_t n[3]; float lo[3], hi[3]; } wm_action_grid;
  * (0 where not valid; may be NULL; may alias `action`). */
 int wm_discretize_actions(wm_handle* h, const wm_action_grid* grid, int64_t N, int32_t A, const float* action,
                           const uint8_t* valid, int32_t* index, float* dequant, void* stream);
-/* index [N][A] -> action [N][C][A]: the grid values (index < 0 -> 0), ready for wm_step / wm_rollout. */
+/* index [N][A] -> action [N][C][A]: the grid values, ready for wm_step / wm_rollout.  An index that names no
+ * bin of the grid - negative, or >= n[0] * .. * n[C-1] - decodes to the zero action (D45); it never wraps
+ * around into some other bin. */
 int wm_actions_from_index(wm_handle* h, const wm_action_grid* grid, int64_t N, int32_t A, const int32_t* index,
                           float* action, void* stream);
 /* Discrete expert (L204): wm_expert_actions followed by wm_discretize_actions in place.  action

@@ -868,11 +868,15 @@ void orc_discretize_actions(const orc_action_grid* g, int32_t C, int64_t N, int3
     }
 }
 
-// joint index -> continuous action (the de-quantised grid value; index < 0 -> 0)
+// joint index -> continuous action (the de-quantised grid value; index < 0 -> 0; D45: an index that is not
+// a bin of the grid, index >= n_0 n_1 .. n_{C-1}, is no action either -> 0)
 void orc_actions_from_index(const orc_action_grid* g, int32_t C, int64_t N, int32_t A, const int32_t* index, float* action) {
+  int64_t total = 1;
+  for (int c = 0; c < C; ++c) total *= g->n[c];
   for (int64_t r = 0; r < N; ++r)
     for (int a = 0; a < A; ++a) {
       int32_t idx = index[r * A + a];
+      if ((int64_t)idx >= total) idx = -1;
       for (int c = C - 1; c >= 0; --c) {
         const size_t o = ((size_t)r * C + c) * A + a;
         if (idx < 0) { action[o] = 0.f; continue; }

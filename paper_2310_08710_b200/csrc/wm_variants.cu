@@ -139,6 +139,9 @@ __global__ void __launch_bounds__(256) k_from_index(GridDev g, int C, int64_t N,
   const int64_t r = i / A;
   const int a = (int)(i - r * A);
   int idx = index[i];
+  int64_t total = 1;
+  for (int c = 0; c < C; ++c) total *= g.n[c];
+  if ((int64_t)idx >= total) idx = -1;                     // D45: not a bin of this grid -> no action, like index < 0
   for (int c = C - 1; c >= 0; --c) {
     const int64_t o = (r * C + c) * A + a;
     const int n = g.n[c];

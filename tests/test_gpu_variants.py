@@ -108,6 +108,15 @@ def test_discretize_and_decode_bit_exact(dyn):
     assert np.array_equal(idx.cpu().numpy(), ref["index"])
     assert np.array_equal(deq.cpu().numpy(), ref["action"])
     assert np.array_equal(back.cpu().numpy(), oracle.actions_from_index(ref["index"], C, n, lo, hi))
+    # D45: indices that are no bin of the grid (total, total + 1, INT_MAX, negative) decode to the zero action
+    total = int(np.prod(n[:C]))
+    odd = np.array([[total - 1, total, total + 1, 2**31 - 1, -1, -7, 0]], np.int32)
+    back2 = torch.full((1, C, odd.shape[1]), 9.0, device="cuda")
+    wm.wm_actions_from_index(h, grid, torch.from_numpy(odd).cuda(), back2)
+    torch.cuda.synchronize()
+    got = back2.cpu().numpy()
+    assert np.array_equal(got, oracle.actions_from_index(odd, C, n, lo, hi))
+    assert np.all(got[0, :, 1:6] == 0.0) and np.all(got[0, :, 6] == np.asarray(lo[:C], np.float32)) and np.all(got[0, :, 0] != 0.0)
     wm.wm_destroy(h)
 
 

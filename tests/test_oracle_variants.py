@@ -161,6 +161,14 @@ def test_discretize_invalid_and_single_bin():
     assert oracle.actions_from_index(r["index"], 2, [3, 1], [0.0, 4.0], [1.0, 4.0])[0, :, 1].tolist() == [0.0, 0.0]
 
 
+
+def test_index_outside_the_grid_decodes_to_the_zero_action():
+    """D45: 3 x 2 bins; indices -1, 6 (= total), 7 and INT_MAX are no bins and give 0, never a wrapped bin; 0 .. 5 by hand."""
+    idx = np.array([[0, 1, 2, 3, 4, 5, -1, 6, 7, 2**31 - 1]], np.int32)
+    back = oracle.actions_from_index(idx, 2, [3, 2], [0.0, 10.0], [1.0, 20.0])
+    assert back[0, 0].tolist() == [0.0, 0.0, 0.5, 0.5, 1.0, 1.0, 0.0, 0.0, 0.0, 0.0]
+    assert back[0, 1].tolist() == [10.0, 20.0, 10.0, 20.0, 10.0, 20.0, 0.0, 0.0, 0.0, 0.0]
+
 # ---------------------------------------------------------------------------------------
 # O7 with order = 1: sorted by distance
 # ---------------------------------------------------------------------------------------
