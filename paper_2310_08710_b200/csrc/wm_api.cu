@@ -26,6 +26,17 @@ static bool rg_ok(const wm_roadgraph* g) {
 }
 static bool same_shape(const wm_traj* a, const wm_traj* b) { return a->B == b->B && a->A == b->A && a->T == b->T; }
 
+// Launch-shape limits, checked by EVERY entry point that launches over scenarios and agents (wm.h "Limits"):
+// several kernels put the scenario in gridDim.y (<= 65 535) and hold a row of agents in one CTA (A <= 1024);
+// the others run a 1-D grid of 256-thread blocks over `elems` items (<= 2^31 - 1 blocks).  A shape beyond them
+// is refused here instead of coming back as a failed launch.
+static int shape_guard(int64_t B, int64_t A, int64_t elems) {
+  if (A > 1024 || B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
+  if (elems > (int64_t)0x7fffffff * 128) return WM_ERR_UNSUPPORTED;
+  return WM_OK;
+}
+#define WM_SHAPE(B, A, elems) do { const int rc__ = shape_guard((B), (A), (elems)); if (rc__ != WM_OK) return rc__; } while (0)
+
 extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
   if (!out || !cfg) return WM_ERR_ARG;
   if (cfg->dynamics != WM_DYN_INVERTIBLE_BICYCLE && cfg->dynamics != WM_DYN_DELTA_LOCAL && cfg->dynamics != WM_DYN_DELTA_GLOBAL) return WM_ERR_ARG;
@@ -125,7 +136,7 @@ extern "C" int wm_segment_counts(wm_handle* h, int32_t* n_seg_host, int32_t B, v
 extern "C" int wm_reset(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t* t, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim)) return WM_ERR_ARG;
   if (h->cfg.history > sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
   WM_CUDA(wm_launch_reset(h, *log, *sim, h->cfg.history, (cudaStream_t)stream));
   if (t) *t = h->cfg.history - 1;
   return WM_OK;
@@ -135,7 +146,7 @@ extern "C" int wm_step(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_t t
                        const uint8_t* action_valid, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !action || !action_valid) return WM_ERR_ARG;
   if (t < 0 || t + 1 >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
   const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   WM_CUDA(wm_launch_step(h, *log, *sim, t, action, (int64_t)C * sim->A, action_valid, sim->A, nullptr, nullptr, 0,
                          (cudaStream_t)stream));
@@ -146,7 +157,7 @@ extern "C" int wm_metrics_overlap(wm_handle* h, const wm_traj* sim, int32_t t, u
                                   uint8_t* agent_flag, void* stream) {
   if (!h || !traj_ok(sim) || !agent_flag) return WM_ERR_ARG;
   if (t < 0 || t >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
   WM_CUDA(wm_launch_overlap(h, *sim, t, pair_bits, agent_flag, sim->A, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -155,8 +166,8 @@ extern "C" int wm_metrics_offroad(wm_handle* h, const wm_traj* sim, int32_t t, f
                                   float* corner_dist, uint8_t* agent_flag, void* stream) {
   if (!h || !traj_ok(sim) || !signed_dist || !agent_flag) return WM_ERR_ARG;
   if (t < 0 || t >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
-  if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
+  if (!h->seg_ready || h->prep_B != sim->B) return WM_ERR_STATE;
   WM_CUDA(wm_launch_offroad(h, *sim, t, signed_dist, sim->A, corner_dist, agent_flag, sim->A, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -165,6 +176,7 @@ extern "C" int wm_log_divergence(wm_handle* h, const wm_traj* log, const wm_traj
                                  uint8_t* valid, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !dist) return WM_ERR_ARG;
   if (t < 0 || t >= sim->T) return WM_ERR_ARG;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
   WM_CUDA(wm_launch_logdiv(h, *log, *sim, t, dist, valid, sim->A, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -173,6 +185,7 @@ extern "C" int wm_expert_actions(wm_handle* h, const wm_traj* tr, int32_t t, int
                                  uint8_t* action_valid, void* stream) {
   if (!h || !traj_ok(tr) || !action || !action_valid) return WM_ERR_ARG;
   if (n_steps < 1 || t < 0 || t + n_steps >= tr->T) return WM_ERR_ARG;
+  WM_SHAPE(tr->B, tr->A, (int64_t)tr->B * n_steps * tr->A);
   WM_CUDA(wm_launch_expert(h, *tr, t, n_steps, action, action_valid, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -181,6 +194,7 @@ extern "C" int wm_metrics_kinematic(wm_handle* h, const wm_traj* sim, int32_t t,
                                     float* curvature, uint8_t* flag, void* stream) {
   if (!h || !traj_ok(sim) || !flag) return WM_ERR_ARG;
   if (n_steps < 1 || t < 1 || t + n_steps > sim->T) return WM_ERR_ARG;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * n_steps * sim->A);
   if (!(h->cfg.max_accel > 0.f) || !(h->cfg.max_curvature > 0.f)) return WM_ERR_UNSUPPORTED;   // the metric needs its limits
   WM_CUDA(wm_launch_kinematic(h, *sim, t, n_steps, accel, curvature, flag, (cudaStream_t)stream));
   return WM_OK;
@@ -201,6 +215,7 @@ extern "C" int wm_discretize_actions(wm_handle* h, const wm_action_grid* grid, i
                                      const uint8_t* valid, int32_t* index, float* dequant, void* stream) {
   const int C = h && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   if (!h || !grid_ok(grid, C) || N < 1 || A < 1 || !action || !index) return WM_ERR_ARG;
+  if (N > (int64_t)0x7fffffff * 128 / A) return WM_ERR_UNSUPPORTED;           // the 1-D grid over N * A items
   WM_CUDA(wm_launch_discretize(h, *grid, C, N, A, action, valid, index, dequant, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -209,6 +224,7 @@ extern "C" int wm_actions_from_index(wm_handle* h, const wm_action_grid* grid, i
                                      float* action, void* stream) {
   const int C = h && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   if (!h || !grid_ok(grid, C) || N < 1 || A < 1 || !action || !index) return WM_ERR_ARG;
+  if (N > (int64_t)0x7fffffff * 128 / A) return WM_ERR_UNSUPPORTED;           // the 1-D grid over N * A items
   WM_CUDA(wm_launch_from_index(h, *grid, C, N, A, index, action, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -218,6 +234,7 @@ extern "C" int wm_expert_actions_discrete(wm_handle* h, const wm_traj* tr, int32
   const int C = h && h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   if (!h || !traj_ok(tr) || !grid_ok(grid, C) || !action || !action_valid || !index) return WM_ERR_ARG;
   if (n_steps < 1 || t < 0 || t + n_steps >= tr->T) return WM_ERR_ARG;
+  WM_SHAPE(tr->B, tr->A, (int64_t)tr->B * n_steps * tr->A);
   WM_CUDA(wm_launch_expert(h, *tr, t, n_steps, action, action_valid, (cudaStream_t)stream));
   WM_CUDA(wm_launch_discretize(h, *grid, C, (int64_t)tr->B * n_steps, tr->A, action, action_valid, index, action, (cudaStream_t)stream));
   return WM_OK;
@@ -227,6 +244,7 @@ extern "C" int wm_rollout_vjp(wm_handle* h, const wm_traj* sim, int32_t t0, int3
                               const uint8_t* action_valid, const float* g_rows, float* g_actions, float* g_state0, void* stream) {
   if (!h || !traj_ok(sim) || !actions || !action_valid || !g_rows || !g_actions) return WM_ERR_ARG;
   if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
   WM_CUDA(wm_launch_rollout_vjp(h, *sim, t0, n_steps, actions, action_valid, g_rows, g_actions, g_state0, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -241,6 +259,7 @@ extern "C" int wm_metrics_route_progress(wm_handle* h, const wm_traj* log, const
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !paths || !ratio || !valid) return WM_ERR_ARG;
   if (t < 0 || t >= sim->T) return WM_ERR_ARG;
   if (paths->B != sim->B || paths->A != sim->A || paths->P < 1 || !paths->x || !paths->y || !paths->arc_len || !paths->valid) return WM_ERR_ARG;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);                            // the scenario is gridDim.y
   WM_CUDA(wm_launch_route_progress(h, *log, *sim, t, *paths, ratio, valid, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -253,6 +272,7 @@ extern "C" int wm_metrics_offroute(wm_handle* h, const wm_traj* sim, int32_t t, 
                                    float max_dist, float margin, float* dist_on, uint8_t* flag, void* stream) {
   if (!h || !traj_ok(sim) || !paths_ok(on_route, sim) || (off_route && !paths_ok(off_route, sim)) || !flag) return WM_ERR_ARG;
   if (t < 0 || t >= sim->T || !(max_dist >= 0.f) || !(margin >= 0.f)) return WM_ERR_ARG;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A * 32);                       // a warp per agent
   WM_CUDA(wm_launch_offroute(h, *sim, t, *on_route, off_route, max_dist, margin, dist_on, flag, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -264,6 +284,7 @@ extern "C" int wm_idm_step(wm_handle* h, wm_traj* sim, int32_t t, const wm_paths
   if (!(params->v0 > 0.f) || !(params->a_max > 0.f) || !(params->b > 0.f) || !(params->b_max > 0.f) || !(params->T >= 0.f) ||
       !(params->s0 >= 0.f) || !(params->delta > 0.f)) return WM_ERR_ARG;
   if (paths->P > 1900) return WM_ERR_UNSUPPORTED;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A * 32);                       // a warp per agent
   WM_CUDA(wm_launch_idm_step(h, *sim, t, *paths, idm_valid, *params, accel, lead, (cudaStream_t)stream));
   return WM_OK;
 }
@@ -275,7 +296,7 @@ extern "C" int wm_observe(wm_handle* h, const wm_traj* sim, const wm_roadgraph* 
   if (want_hist && !(hist && hist_valid)) return WM_ERR_ARG;
   if (want_topk && !(rg_index && rg_feat && rg_type && rg_ok(rg))) return WM_ERR_ARG;
   if (t < h->cfg.history - 1 || t >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
   if (want_hist) WM_CUDA(wm_launch_observe_hist(h, *sim, t, hist, hist_valid, (cudaStream_t)stream));
   if (want_topk) {
     if (h->cfg.topk < 1 || h->cfg.topk > rg->R) return WM_ERR_UNSUPPORTED;
@@ -320,8 +341,8 @@ extern "C" int wm_rollout(wm_handle* h, const wm_traj* log, wm_traj* sim, int32_
                           const float* actions, const uint8_t* action_valid, const wm_rollout_out* out, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !actions || !action_valid || !out) return WM_ERR_ARG;
   if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
-  if (sim->A > 1024 || sim->B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
-  if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
+  if (!h->seg_ready || h->prep_B != sim->B) return WM_ERR_STATE;
   const bool fused = h->cfg.rollout_mode == WM_ROLLOUT_FUSED && h->cfg.offroad_mode == WM_OFFROAD_CULLED &&
                      n_steps < 60000;                  // its hash entries carry a 16-bit block number
   const int64_t rows = fused ? 0 : (int64_t)sim->B * n_steps * sim->A;
@@ -396,16 +417,18 @@ extern "C" int wm_rollout_kernel_times(wm_handle* h, const wm_traj* log, wm_traj
                                        float* ms_host, void* stream) {
   if (!h || !traj_ok(log) || !traj_ok(sim) || !same_shape(log, sim) || !actions || !action_valid || !out || !ms_host) return WM_ERR_ARG;
   if (n_steps < 1 || t0 < 0 || t0 + n_steps >= sim->T) return WM_ERR_ARG;
-  if (!h->edges || h->prep_B != sim->B) return WM_ERR_STATE;
+  WM_SHAPE(sim->B, sim->A, (int64_t)sim->B * sim->A);
+  if (!h->seg_ready || h->prep_B != sim->B) return WM_ERR_STATE;
   if (h->cfg.rollout_mode != WM_ROLLOUT_FUSED || h->cfg.offroad_mode != WM_OFFROAD_CULLED) return WM_ERR_UNSUPPORTED;
   cudaStream_t s = (cudaStream_t)stream;
-  cudaEvent_t ev[3];
-  for (int i = 0; i < 3; ++i) WM_CUDA(cudaEventCreate(&ev[i]));
-  cudaError_t e = wm_launch_rollout_fused_timed(h, *log, *sim, t0, n_steps, actions, action_valid, *out, ev, s);
+  cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+  cudaError_t e = cudaSuccess;
+  for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaEventCreate(&ev[i]);
+  if (e == cudaSuccess) e = wm_launch_rollout_fused_timed(h, *log, *sim, t0, n_steps, actions, action_valid, *out, ev, s);
   if (e == cudaSuccess) e = cudaEventSynchronize(ev[2]);
   if (e == cudaSuccess) e = cudaEventElapsedTime(&ms_host[0], ev[0], ev[1]);
   if (e == cudaSuccess) e = cudaEventElapsedTime(&ms_host[1], ev[1], ev[2]);
-  for (int i = 0; i < 3; ++i) cudaEventDestroy(ev[i]);
+  for (int i = 0; i < 3; ++i) if (ev[i]) cudaEventDestroy(ev[i]);      // whatever was created, on every exit path
   WM_CUDA(e);
   return WM_OK;
 }
@@ -415,15 +438,17 @@ extern "C" int wm_rollout_kernel_times(wm_handle* h, const wm_traj* log, wm_traj
 extern "C" int wm_selftest_ffma(wm_handle* h, int32_t packed, int32_t ctas, int32_t iters, float* ms_host, double* flop_host, void* stream) {
   if (!h || !ms_host || ctas < 1 || iters < 1) return WM_ERR_ARG;
   cudaStream_t s = (cudaStream_t)stream;
-  cudaEvent_t a, b;
-  WM_CUDA(cudaEventCreate(&a)); WM_CUDA(cudaEventCreate(&b));
-  cudaError_t e = wm_launch_ffma_peak(h, packed, ctas, iters, (float*)h->cull_stats, s);      // warm-up
+  cudaEvent_t a = nullptr, b = nullptr;
+  cudaError_t e = cudaEventCreate(&a);
+  if (e == cudaSuccess) e = cudaEventCreate(&b);
+  if (e == cudaSuccess) e = wm_launch_ffma_peak(h, packed, ctas, iters, (float*)h->cull_stats, s);      // warm-up
   if (e == cudaSuccess) e = cudaEventRecord(a, s);
   if (e == cudaSuccess) e = wm_launch_ffma_peak(h, packed, ctas, iters, (float*)h->cull_stats, s);
   if (e == cudaSuccess) e = cudaEventRecord(b, s);
   if (e == cudaSuccess) e = cudaEventSynchronize(b);
   if (e == cudaSuccess) e = cudaEventElapsedTime(ms_host, a, b);
-  cudaEventDestroy(a); cudaEventDestroy(b);
+  if (a) cudaEventDestroy(a);
+  if (b) cudaEventDestroy(b);
   WM_CUDA(e);
   if (flop_host) *flop_host = (double)ctas * 256.0 * (double)iters * 32.0 * (packed ? 4.0 : 2.0);
   return WM_OK;
@@ -451,7 +476,7 @@ extern "C" int wm_rollout_host(wm_handle* h, const wm_traj* lh, const wm_roadgra
   const int B = lh->B, A = lh->A, T = lh->T, R = gh->R;
   const int t0 = h->cfg.history - 1;
   if (n_steps < 1 || t0 + n_steps >= T) return WM_ERR_ARG;
-  if (A > 1024 || B > WM_MAX_B) return WM_ERR_UNSUPPORTED;
+  WM_SHAPE(B, A, (int64_t)B * n_steps * A);
   cudaStream_t s = (cudaStream_t)stream;
   const int C = h->cfg.dynamics == WM_DYN_INVERTIBLE_BICYCLE ? 2 : 3;
   const size_t nTA = (size_t)B * T * A, nR = (size_t)B * R, rows = (size_t)B * n_steps * A, nBA = (size_t)B * A;

@@ -74,14 +74,16 @@ struct wm_handle {
   int32_t prep_B, prep_R;
   int32_t seg_tiles;        // tiles per scenario in `edges`
   int32_t seg_max;          // max_b n_seg[b]
+  int32_t seg_ready;        // the record arrays below are allocated for prep_B x seg_tiles: wm_prepare has run ("is prepared" marker)
   int32_t* n_seg;           // [B]
-  float4* edges;            // [B][seg_tiles][WM_TILE_F4]
-  float2* sign_dir;         // [B][seg_tiles*512]  sign direction (e, or stored dir if e == 0)
+  float4* edges;            // [B][seg_tiles][WM_TILE_F4]  WM_OFFROAD_BRUTE_FORCE only (NULL otherwise)
+  float2* sign_dir;         // [B][seg_tiles*512]  sign direction (e, or stored dir if e == 0); WM_OFFROAD_BRUTE_FORCE only
   int32_t* seg_src;         // [B][seg_tiles*512]  first-point index of each stored segment (-1: padding)
   float4* segrec;           // [B][seg_tiles*512][2] {p0x,p0y,ex,ey} {gx,gy,sx,sy}, ascending source order
   float4* segfin;           // [B][seg_tiles*512] {p0x, p0y, sx, sy}: what the sign of the winner needs
   float4* segpair;          // [B][3][seg_tiles*256] the same records two by two, component-wise, in three planes (wm_grid.cuh)
-  float4* seglk;            // [B][seg_tiles*256][2] per pair record, for the cell build only (wm_grid.cu): what the
+  float4* seglk;            // [B][seg_tiles*256][2] per pair record, for the cell build only (wm_grid.cu; kept between
+                            //   wm_prepare calls so that re-preparing a batch of the same size calls no cudaMalloc): what the
                             //   neighbour rules P / N need - {fx, fx', fy, fy'} {aP, aP', aN, aN'}, f = e of the NEXT record
                             //   of the same polyline (0 if none), aP / aN = |ex| + |ey| when the rule can apply, +inf otherwise
   float4* chunks;           // [B][seg_tiles*16]   bounding box of each chunk of 32 records

@@ -113,8 +113,8 @@ __global__ void __launch_bounds__(256) k_fill_segments(RgView g, int seg_tiles, 
   if (grp >= ngrp) return;
   const int64_t o = (int64_t)b * g.R;
   const int cap = seg_tiles * WM_TILE_SEGS, n = n_seg[b];
-  float* tile_base = (float*)(edges + (int64_t)b * seg_tiles * WM_TILE_F4);
-  float2* sd = sign_dir + (int64_t)b * cap;
+  float* tile_base = tiles_on ? (float*)(edges + (int64_t)b * seg_tiles * WM_TILE_F4) : nullptr;   // NULL outside the brute-force mode
+  float2* sd = tiles_on ? sign_dir + (int64_t)b * cap : nullptr;
   int32_t* src = seg_src + (int64_t)b * cap;
   float x0 = 3.0e38f, y0 = 3.0e38f, x1 = -3.0e38f, y1 = -3.0e38f;
   float ax[2], ay[2], bx[2], by[2];
@@ -197,7 +197,7 @@ void wm_prepare_free(wm_handle* h) {
   cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->seglk); cudaFree(h->segfin); cudaFree(h->chunks); cudaFree(h->gridp); cudaFree(h->cells); cudaFree(h->pool); cudaFree(h->pool_cnt);
   h->n_seg = nullptr; h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->pt_xy = nullptr; h->pt_idx = nullptr; h->pt_start = nullptr; h->pt_grid = nullptr;
   h->segrec = nullptr; h->segpair = nullptr; h->seglk = nullptr; h->segfin = nullptr; h->chunks = nullptr; h->gridp = nullptr; h->cells = nullptr; h->pool = nullptr; h->pool_cnt = nullptr;
-  h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0;
+  h->prep_B = 0; h->prep_R = 0; h->seg_tiles = 0; h->seg_max = 0; h->seg_ready = 0;
 }
 
 // Step 1 of wm_prepare: per-scenario record counts (needs type, id, valid only), the capacity they
@@ -236,14 +236,17 @@ int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_m
   h->seg_max = mx;
   int tiles = (mx + WM_TILE_SEGS - 1) / WM_TILE_SEGS;
   if (tiles < 1) tiles = 1;
-  if (tiles > h->seg_tiles || !h->edges) {       // grow only: seg_tiles is the row stride of `edges`
+  if (tiles > h->seg_tiles || !h->seg_ready) {   // grow only: seg_tiles is the row stride of the record arrays
     wm_drop_graph(h);
     cudaFree(h->edges); cudaFree(h->sign_dir); cudaFree(h->seg_src); cudaFree(h->segrec); cudaFree(h->segpair); cudaFree(h->seglk); cudaFree(h->segfin); cudaFree(h->chunks);
     h->edges = nullptr; h->sign_dir = nullptr; h->seg_src = nullptr; h->segrec = nullptr; h->segpair = nullptr; h->seglk = nullptr; h->segfin = nullptr; h->chunks = nullptr;
-    h->seg_tiles = tiles;
+    h->seg_tiles = tiles; h->seg_ready = 0;
     const size_t cap = (size_t)tiles * WM_TILE_SEGS;
-    cudaError_t ea = cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES);
-    if (ea == cudaSuccess) ea = cudaMalloc(&h->sign_dir, (size_t)B * cap * sizeof(float2));
+    cudaError_t ea = cudaSuccess;
+    if (h->cfg.offroad_mode == WM_OFFROAD_BRUTE_FORCE) {     // the tile layout and its sign directions: only k_offroad reads them
+      ea = cudaMalloc(&h->edges, (size_t)B * tiles * WM_TILE_BYTES);
+      if (ea == cudaSuccess) ea = cudaMalloc(&h->sign_dir, (size_t)B * cap * sizeof(float2));
+    }
     if (ea == cudaSuccess) ea = cudaMalloc(&h->seg_src, (size_t)B * cap * sizeof(int32_t));
     if (ea == cudaSuccess) ea = cudaMalloc(&h->segrec, (size_t)B * cap * 2 * sizeof(float4));
     if (ea == cudaSuccess) ea = cudaMalloc(&h->segpair, (size_t)B * (cap / 2) * 3 * sizeof(float4));
@@ -251,6 +254,7 @@ int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_m
     if (ea == cudaSuccess) ea = cudaMalloc(&h->segfin, (size_t)B * cap * sizeof(float4));
     if (ea == cudaSuccess) ea = cudaMalloc(&h->chunks, (size_t)B * (cap / WM_CHUNK) * sizeof(float4));
     if (ea != cudaSuccess) { wm_prepare_free(h); WM_CUDA(ea); }     // out of memory: back to the unprepared state
+    h->seg_ready = 1;
   }
   if (n_segments_max) *n_segments_max = mx;
   return WM_OK;
@@ -270,10 +274,11 @@ int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaS
   WM_CUDA(cudaGetLastError());
   {
     const int ngrp = tiles * (WM_TILE_SEGS / 64);
-    k_fill_segments<<<dim3((ngrp + 7) / 8, nb), 256, 0, s>>>(g, tiles, h->n_seg + b0, h->edges + (int64_t)b0 * tiles * WM_TILE_F4,
-                                                             h->sign_dir + b0 * cap, seg_src, h->segrec + b0 * cap * 2,
+    const bool brute = h->cfg.offroad_mode == WM_OFFROAD_BRUTE_FORCE;   // edges / sign_dir exist in that mode only
+    k_fill_segments<<<dim3((ngrp + 7) / 8, nb), 256, 0, s>>>(g, tiles, h->n_seg + b0, brute ? h->edges + (int64_t)b0 * tiles * WM_TILE_F4 : nullptr,
+                                                             brute ? h->sign_dir + b0 * cap : nullptr, seg_src, h->segrec + b0 * cap * 2,
                                                              h->segpair + b0 * (cap / 2) * 3, h->seglk + b0 * (cap / 2) * 2, h->segfin + b0 * cap,
-                                                             h->chunks + b0 * (cap / WM_CHUNK), h->cfg.offroad_mode == WM_OFFROAD_BRUTE_FORCE);
+                                                             h->chunks + b0 * (cap / WM_CHUNK), brute);
   }
   h->launches++;
   WM_CUDA(cudaGetLastError());

@@ -572,7 +572,7 @@ static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_
   const int nba = (sim.A + DYN_NT - 1) / DYN_NT;
   const int64_t n_dyn = (int64_t)sim.B * nba;
   cudaError_t e = cudaSuccess;
-  if (ev) cudaEventRecord(ev[0], s);
+  if (ev && (e = cudaEventRecord(ev[0], s)) != cudaSuccess) return e;
   // bulk-copy staging needs 16-byte aligned rows of every array
   bool bulk = sim.A % 16 == 0 && sim.A <= 1024;
   {
@@ -599,7 +599,7 @@ static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_
   h->launches++;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  if (ev) cudaEventRecord(ev[1], s);
+  if (ev && (e = cudaEventRecord(ev[1], s)) != cudaSuccess) return e;
   // ---- its metrics ----
   const int Ap = (sim.A + 31) / 32 * 32;
   const size_t smem = fused_persist_bytes(Ap) + (size_t)p.S * fused_slot_bytes(Ap);
@@ -616,6 +616,8 @@ static cudaError_t fused_launch_part(wm_handle* h, const wm_traj& log, const wm_
   else if (Ap == 32 && p.S == 8) k_rollout_metrics<32, 8, true><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);
   else k_rollout_metrics<0, 0, true><<<(unsigned)n_cta, FUSED_NT, smem, s>>>(p, nblk);
   h->launches++;
-  if (ev) cudaEventRecord(ev[2], s);
-  return cudaGetLastError();
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  if (ev) e = cudaEventRecord(ev[2], s);
+  return e;
 }

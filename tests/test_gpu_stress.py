@@ -135,3 +135,46 @@ def test_exact_tie_between_stored_segments_63_and_64(mode):
     sd, cd, fl = gpu_offroad(h, tr_d, 0)
     assert cd[0, k, 0] == orc["corner_dist"][0, k, 0], (cd[0, :, 0], orc["corner_dist"][0, :, 0])
     wm.wm_destroy(h)
+
+
+def test_oversize_shapes_are_refused_not_launched():
+    """wm.h "Limits": A <= 1024 agents, B <= 65 535 scenarios per call.  Every entry point that launches over
+    (scenario, agent) returns WM_ERR_UNSUPPORTED for a shape beyond them - not WM_ERR_CUDA from a launch the
+    hardware rejected - before touching its outputs."""
+    def traj(B, T, A):
+        tr = {k: torch.zeros((B, T, A), device="cuda") for k in wm.TRAJ_F}
+        tr["valid"] = torch.ones((B, T, A), dtype=torch.uint8, device="cuda")
+        return tr
+    def paths(B, A, P=2):
+        return dict(x=torch.zeros((B, A, P), device="cuda"), y=torch.zeros((B, A, P), device="cuda"),
+                    arc_len=torch.zeros((B, A, P), device="cuda"), valid=torch.ones((B, A, P), dtype=torch.uint8, device="cuda"))
+    h = wm.wm_create(history=1)
+    for B, A in ((1, 1025), (65536, 1)):
+        T, n = 3, 1
+        tr, sim = traj(B, T, A), traj(B, T, A)
+        f = lambda *s: torch.full(s, 7.0, device="cuda")
+        u = lambda *s: torch.full(s, 7, dtype=torch.uint8, device="cuda")
+        act, av = f(B, n, 2, A), u(B, n, A)
+        out = wm.alloc_rollout_out(B, n, A)
+        pa = paths(B, A)
+        calls = {
+            "wm_reset": lambda: wm.wm_reset(h, tr, sim),
+            "wm_step": lambda: wm.wm_step(h, tr, sim, 0, act[:, 0].contiguous(), av[:, 0].contiguous()),
+            "wm_metrics_overlap": lambda: wm.wm_metrics_overlap(h, sim, 0, None, u(B, A)),
+            "wm_log_divergence": lambda: wm.wm_log_divergence(h, tr, sim, 0, f(B, A), u(B, A)),
+            "wm_expert_actions": lambda: wm.wm_expert_actions(h, tr, 0, n, f(B, n, 2, A), u(B, n, A)),
+            "wm_metrics_kinematic": lambda: wm.wm_metrics_kinematic(h, sim, 1, n, f(B, n, A), f(B, n, A), u(B, n, A)),
+            "wm_rollout_vjp": lambda: wm.wm_rollout_vjp(h, sim, 0, n, act, av, f(B, n, 5, A), f(B, n, 2, A)),
+            "wm_metrics_route_progress": lambda: wm.wm_metrics_route_progress(h, tr, sim, 0, pa, f(B, A), u(B, A)),
+            "wm_metrics_offroute": lambda: wm.wm_metrics_offroute(h, sim, 0, pa, None, 5.0, 1.0, f(B, A), u(B, A)),
+            "wm_idm_step": lambda: wm.wm_idm_step(h, sim, 0, pa, u(B, A)),
+            "wm_observe": lambda: wm.wm_observe(h, sim, None, 0, f(B, A, 1, 7, A), u(B, A, 1, A)),
+            "wm_rollout": lambda: wm.wm_rollout(h, tr, sim, 0, n, act, av, out),
+            "wm_rollout_kernel_times": lambda: wm.wm_rollout_kernel_times(h, tr, sim, 0, n, act, av, out),
+        }
+        for name, call in calls.items():
+            with pytest.raises(wm.WmError, match="WM_ERR_UNSUPPORTED"):
+                call()
+        torch.cuda.synchronize()
+        assert float(out["ade"].abs().sum()) == 0.0
+    wm.wm_destroy(h)
