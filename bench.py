@@ -572,7 +572,9 @@ def other_configs(wm, ws, torch, hbm_peak, log5_d, sim5_d, stream):
             ms_ov = timed(lambda: wm.wm_metrics_overlap(h, log_d, 0, bits, ofl))
             ms_of = timed(lambda: wm.wm_metrics_offroad(h, log_d, 0, sd, None, fl))
             n = float(B) * A
+            gs = wm.wm_grid_stats(h)
             out["config4_stress"] = {"workload": "B=%d A=%d R=%d, overlap matrix + offroad of the crowded lot" % (B, A, rg["x"].shape[1]),
+                                     "grid_cells_without_list_frac": {k: v[2] for k, v in gs.items()},
                                      "k_overlap": rl(n * (29 + 4 * Wd + 1), ms_ov), "k_offroad_grid": rl(n * (29 + 5), ms_of),
                                      "ms": ms_ov + ms_of, "pair_tests_per_s": B * A * (A - 1) / 2 / (ms_ov * 1e-3),
                                      "note": "%d agents per call: launch / latency bound, the HBM fractions are not roofline claims" % int(n)}
@@ -733,6 +735,7 @@ def main():
         torch.cuda.synchronize()
         return ka.elapsed_time(kb) / reps
     prepare_ms = sharding.max_over_ranks(time_prepare(), dev)
+    grid_stats = wm.wm_grid_stats(h)          # cells per level and how many of them have no candidate list
     ka, kb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ka.record(stream)
     for _ in range(5):
@@ -896,6 +899,19 @@ def main():
                                          "ambiguous_corners": amb_corners, "corners": n_corners, "ambiguous_overlap_pairs": amb_pairs}}
 
     if rank == 0:
+        extra = {"prepare_ms": prepare_ms, "reset_ms": reset_ms, "value_incl_prepare": agent_steps / ((prepare_ms + ms_step) * 1e-3),
+                 "grid_cells_without_list_frac": {k: v[2] for k, v in grid_stats.items()}}
+        if roofline_bf:
+            extra["bruteforce_frac"] = roofline_bf.get("frac")
+        if others:
+            o3, o5 = others["config3_observe"], others["config5_expert"]
+            extra.update(ms_hist=o3["k_observe_hist"]["ms"], hist_hbm_frac=o3["k_observe_hist"]["hbm_frac"],
+                         ms_topk=o3["k_observe_topk"]["ms"], topk_hbm_frac=o3["k_observe_topk"]["hbm_frac"],
+                         ms_config2=others["config2_step"]["ms"], ms_config4=others["config4_stress"]["ms"],
+                         config4_cells_without_list_frac=others["config4_stress"]["grid_cells_without_list_frac"],
+                         ms_expert=o5["k_inverse_expert"]["ms"], ms_kinematic=o5["k_inverse_kinematic"]["ms"],
+                         ms_vjp=o5["k_rollout_vjp"]["ms"], ms_idm_step=others["config5_idm"]["k_idm_step"]["ms"],
+                         idm_workload=others["config5_idm"]["workload"])
         line = {
             "metric": METRIC, "value": value, "unit": "agent-steps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
@@ -905,7 +921,8 @@ def main():
                        "S_e_mean": float(n_seg.mean()), "l2": "inputs exceed L2 (segments %.2f GB + state per step)" % (n_seg.sum() * 24 / 1e9),
                        "parallelism": "scenario shards, no collective", "valid_agent_steps_per_s": valid_value,
                        "ms_per_sim_step": ms_step / N_STEPS,
-                       "value_counts": "agent SLOTS (valid or not, SURVEY 8(d)); valid_agent_steps_per_s counts the valid ones"},
+                       "value_counts": "agent SLOTS (valid or not, SURVEY 8(d)); valid_agent_steps_per_s counts the valid ones",
+                       **extra},
             # wm_prepare = the static precompute a NEW batch of scenarios needs before its first rollout (outside `value`:
             # `value` assumes prepared scenarios, e.g. re-rolled in training); value_incl_prepare = one prepare per rollout
             "prepare_ms": prepare_ms, "reset_ms": reset_ms,

@@ -390,6 +390,12 @@ int64_t wm_kernel_launches(const wm_handle* h);
  * Counting costs global atomics, so it is off until wm_offroad_stats_enable(h, 1); toggling it
  * drops a cached rollout graph.  All 0 in brute-force mode. */
 int wm_offroad_stats(wm_handle* h, int64_t* out_host, void* stream);
+/* wm_grid_stats: the prepared search grids (WM_OFFROAD_CULLED), summed over the scenarios of the last wm_prepare:
+ * out_host[6] int64 on the HOST = {inner cells, inner cells without a list, mid cells, mid cells without a list,
+ * outer cells, outer cells without a list}.  A cell "without a list" has too many candidate segments (or its
+ * parent had): queries landing in it take the exact search over all segments - slower, same result.  Dense
+ * roadgraphs (config 4: points 0.1 m apart) have many such cells.  Synchronises.  WM_ERR_STATE before wm_prepare. */
+int wm_grid_stats(wm_handle* h, int64_t* out_host, void* stream);
 int wm_offroad_stats_enable(wm_handle* h, int32_t on);
 
 /* Diagnostics for the bench (HOST outputs; both synchronise the stream).

@@ -25,7 +25,7 @@ RG_F = ("x", "y", "dir_x", "dir_y")
 
 EXPORTS = ("wm_create", "wm_destroy", "wm_last_cuda_error", "wm_version", "wm_prepare", "wm_reset",
            "wm_step", "wm_metrics_overlap", "wm_metrics_offroad", "wm_log_divergence", "wm_observe",
-           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_idm_step", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable",
+           "wm_expert_actions", "wm_metrics_kinematic", "wm_metrics_route_progress", "wm_metrics_offroute", "wm_idm_step", "wm_rollout", "wm_rollout_host", "wm_segment_counts", "wm_kernel_launches", "wm_offroad_stats", "wm_offroad_stats_enable", "wm_grid_stats",
            "wm_discretize_actions", "wm_actions_from_index", "wm_expert_actions_discrete", "wm_rollout_vjp", "wm_step_vjp", "wm_rollout_kernel_times", "wm_selftest_ffma", "wm_observe_topk_static")
 
 
@@ -353,6 +353,15 @@ def wm_offroad_stats(h, stream=None):
     buf = (C.c_int64 * 4)()
     _check(load().wm_offroad_stats(h, buf, _stream(stream)), "wm_offroad_stats")
     return tuple(int(v) for v in buf)
+
+
+def wm_grid_stats(h, stream=None):
+    """Cells of the prepared search grids and how many have no candidate list (their queries search all segments):
+    dict level -> (cells, cells without a list, share), levels inner / mid / outer, summed over the prepared scenarios."""
+    buf = (C.c_int64 * 6)()
+    _check(load().wm_grid_stats(h, buf, _stream(stream)), "wm_grid_stats")
+    v = [int(x) for x in buf]
+    return {k: (v[2 * i], v[2 * i + 1], v[2 * i + 1] / max(v[2 * i], 1)) for i, k in enumerate(("inner", "mid", "outer"))}
 
 
 def wm_offroad_stats_enable(h, on=True):

@@ -61,8 +61,8 @@ extern "C" int wm_create(wm_handle** out, const wm_config* cfg) {
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_prep[i], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming);
   }
-  if (e == cudaSuccess) e = cudaMalloc(&h->cull_stats, 4 * sizeof(unsigned long long));
-  if (e == cudaSuccess) e = cudaMemset(h->cull_stats, 0, 4 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&h->cull_stats, 16 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMemset(h->cull_stats, 0, 16 * sizeof(unsigned long long));
   if (e != cudaSuccess) { g_wm_last_cuda_error = (int)e; wm_destroy(h); return WM_ERR_CUDA; }   // frees what was created so far
   *out = h;
   return WM_OK;
@@ -76,6 +76,20 @@ extern "C" int wm_offroad_stats(wm_handle* h, int64_t* out_host, void* stream) {
   WM_CUDA(cudaMemsetAsync(h->cull_stats, 0, sizeof(v), s));
   WM_CUDA(cudaStreamSynchronize(s));
   for (int i = 0; i < 4; ++i) out_host[i] = (int64_t)v[i];
+  return WM_OK;
+}
+
+extern "C" int wm_grid_stats(wm_handle* h, int64_t* out_host, void* stream) {
+  if (!h || !out_host) return WM_ERR_ARG;
+  if (!h->seg_ready || !h->cells) return WM_ERR_STATE;
+  cudaStream_t s = (cudaStream_t)stream;
+  unsigned long long v[6];
+  unsigned long long* d = h->cull_stats + 8;
+  WM_CUDA(cudaMemsetAsync(d, 0, sizeof(v), s));
+  WM_CUDA(wm_launch_grid_cell_stats(h, d, s));
+  WM_CUDA(cudaMemcpyAsync(v, d, sizeof(v), cudaMemcpyDeviceToHost, s));
+  WM_CUDA(cudaStreamSynchronize(s));
+  for (int i = 0; i < 6; ++i) out_host[i] = (int64_t)v[i];
   return WM_OK;
 }
 

@@ -124,10 +124,12 @@ __device__ __forceinline__ void slab_keep(const float4 NE, const float4 L0, cons
   keep_e = !drop_e; keep_o = !drop_o;
 }
 
-// One warp per block of 8 x 4 cells, one lane per cell.  Outer cells (and inner cells under a
-// crowded parent): chunks that cannot hold a candidate of any cell of the block are dropped with one
-// box-box test per chunk (lanes over chunks); the survivors are walked twice with lanes over cells:
-// dmin(c), then the candidates.  Mid and inner cells: both passes walk the parent's runs.
+// One warp per block of 8 x 4 cells, one lane per cell.  Outer cells: chunks that cannot hold a candidate
+// of any cell of the block are dropped with one box-box test per chunk (lanes over chunks); the survivors
+// are walked twice: dmin(c), then the candidates.  Mid and inner cells: both passes walk the parent's runs;
+// there is no chunk pass at these levels, so a cell whose parent has no list (all-ones header: too many runs
+// or candidates, or the pool was full) gets the all-ones header too and its queries take the exact search
+// over all chunks.  wm_grid_stats counts such cells per level (the bench prints the shares).
 //
 // Both passes take the records two by two (pair records, packed arithmetic).  Pass 2 marks the pair
 // records that hold a candidate in a bit mask over the run (or chunk) being walked; the set stretches
@@ -443,6 +445,33 @@ cudaError_t wm_launch_build_grid(wm_handle* h, int b0, int B, cudaStream_t s) {
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   k_build_cells<2><<<dim3((WM_GRID_NG_IN / 8) * (WM_GRID_NG_IN / 4) / BUILD_WARPS, B), 32 * BUILD_WARPS, 0, s>>>(segrec, segpair, seglk, chunks, seg_cap, h->gridp + b0, cells, pool, h->pool_cnt + b0);
+  h->launches++;
+  return cudaGetLastError();
+}
+
+// Diagnostics (wm_grid_stats): how many cells of each level exist and how many of them carry the
+// "search all chunks" header.  One CTA per scenario; out[2 l] += cells, out[2 l + 1] += all-ones headers of
+// level l = 0 inner, 1 mid, 2 outer.
+__global__ void __launch_bounds__(256) k_grid_cell_stats(const WmGrid* gridp, const uint2* cells, unsigned long long* out) {
+  const int b = blockIdx.x;
+  const WmGrid g = gridp[b];
+  const uint2* cb = cells + (int64_t)b * WM_GRID_CELLS;
+  const int nx[3] = {g.nx, g.nx >> 1, g.onx}, ny[3] = {g.ny, g.ny >> 1, g.ony}, base[3] = {0, g.mbase, g.obase};
+  for (int l = 0; l < 3; ++l) {
+    int full = 0;
+    const int n = nx[l] * ny[l];
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const uint2 hd = cb[base[l] + wm_cell_index(i % nx[l], i / nx[l], nx[l])];
+      full += (hd.x & hd.y) == 0xffffffffu;
+    }
+    full = __reduce_add_sync(0xffffffffu, full);
+    if ((threadIdx.x & 31) == 0 && full) atomicAdd(&out[2 * l + 1], (unsigned long long)full);
+    if (threadIdx.x == 0) atomicAdd(&out[2 * l], (unsigned long long)n);
+  }
+}
+
+cudaError_t wm_launch_grid_cell_stats(wm_handle* h, unsigned long long* out, cudaStream_t s) {
+  k_grid_cell_stats<<<h->prep_B, 256, 0, s>>>(h->gridp, h->cells, out);
   h->launches++;
   return cudaGetLastError();
 }

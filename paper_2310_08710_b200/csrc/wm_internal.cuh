@@ -105,7 +105,8 @@ struct wm_handle {
   // scratch for rollouts / host staging
   void* scratch; size_t scratch_bytes;
   void* stage[16]; size_t stage_bytes[16];
-  unsigned long long* cull_stats;   // device [4]: pairs evaluated, brute-force pairs, slow-path corners, corners
+  unsigned long long* cull_stats;   // device [16]: [0..3] pairs evaluated, brute-force pairs, slow-path corners, corners;
+                                    //   [8..13] scratch of wm_grid_stats
   int stats_on;                     // counters are collected only when enabled (wm_offroad_stats_enable)
 };
 
@@ -187,6 +188,7 @@ cudaError_t wm_launch_rollout_fused_timed(wm_handle* h, const wm_traj& log, cons
 int wm_prepare_impl(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);
 int wm_prepare_count(wm_handle* h, const wm_roadgraph* rg, int32_t* n_segments_max, cudaStream_t s);   // needs type, id, valid; syncs s
 int wm_prepare_build(wm_handle* h, const wm_roadgraph* rg, int b0, int nb, cudaStream_t s);            // scenarios [b0, b0 + nb), no sync
+cudaError_t wm_launch_grid_cell_stats(wm_handle* h, unsigned long long* out6, cudaStream_t s);   // out6: device, zeroed by the caller
 void wm_prepare_free(wm_handle* h);
 void wm_drop_graph(wm_handle* h);
 cudaError_t wm_launch_observe_hist(wm_handle* h, const wm_traj& sim, int t, float* hist, uint8_t* hist_valid, cudaStream_t s);

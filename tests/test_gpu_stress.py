@@ -178,3 +178,26 @@ def test_oversize_shapes_are_refused_not_launched():
         torch.cuda.synchronize()
         assert float(out["ade"].abs().sum()) == 0.0
     wm.wm_destroy(h)
+
+
+def test_grid_stats_counts_cells_without_a_list():
+    """wm_grid_stats: cell counts follow the grid geometry (4 inner per mid cell); an ordinary street map leaves (almost)
+    no cell without a list, the 0.1 m-spaced boundary of config 4 leaves many - and the results stay exact there
+    (test_gpu_fullsize checks config 4 against the oracle)."""
+    import wm_scenarios as ws
+    h = wm.wm_create()
+    with pytest.raises(wm.WmError, match="STATE"):
+        wm.wm_grid_stats(h)
+    shares = {}
+    for cid, kw in ((1, {}), (4, {"B": 2})):
+        cfg = ws.make_config(cid, **kw)
+        wm.wm_prepare(h, dev(cfg["roadgraph"]))
+        st = wm.wm_grid_stats(h)
+        assert st == wm.wm_grid_stats(h)                           # the counters are cleared on every call
+        (ni, ci, _), (nm, cm, _), (no, co, _) = st["inner"], st["mid"], st["outer"]
+        assert ni > 0 and ni == 4 * nm and no > 0 and 0 <= ci <= ni and 0 <= cm <= nm and 0 <= co <= no
+        assert ci >= 4 * cm                                        # the children of a cell without a list have none either
+        shares[cid] = st["inner"][2]
+        print("config %d: cells without a candidate list: inner %.4f, mid %.4f, outer %.4f" % (cid, st["inner"][2], st["mid"][2], st["outer"][2]))
+    assert shares[1] < 0.01
+    wm.wm_destroy(h)
