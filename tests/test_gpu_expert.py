@@ -14,6 +14,8 @@ import paper_2310_08710_b200 as wm
 import wm_scenarios as ws
 from gpu_util import dev, host
 
+from defs_f64 import route_ratio_in_double
+
 pytestmark = pytest.mark.gpu
 
 A_TOL = 1e-3
@@ -177,6 +179,14 @@ def test_route_progress_matches_oracle():
             v = r["valid"] == 1
             assert np.all(np.abs(g - r["ratio"])[v] <= 1e-5 * np.maximum(1.0, np.abs(r["ratio"][v])))
             assert v.sum() > 0.5 * (sim["valid"][:, t] == 1).sum()
+            # the double-precision definition (D33 takes the decision in float32 on both sides above): wherever the
+            # closest points are decided by more than 1e-4 m the GPU's ratio is the definition's; the rest is counted
+            rd, decided = route_ratio_in_double(log, sim, t, paths)
+            chk = decided & v
+            assert np.all(np.abs(g - rd)[chk] <= 1e-5 * np.maximum(1.0, np.abs(rd[chk])))
+            print("route progress cfg%d t=%d: %d valid agents, %d decided by > 1e-4 m and equal to the float64 definition, %d in the band"
+                  % (cid, t, int(v.sum()), int(chk.sum()), int((v & ~decided).sum())))
+            assert chk.sum() > 0.5 * v.sum()
         # the reset state sits on its own logged position: progress of agents logged from step 0 at t0 = progress of the log
         wm.wm_destroy(h)
 

@@ -114,7 +114,10 @@ def test_offroad_matches_oracle(cfgid, B, mode):
     orc = oracle.offroad(cfg["log"], t, cfg["roadgraph"])
     st = compare_offroad(sd, cd, fl, orc, cfg["log"]["valid"][:, t])
     print("offroad cfg%d: %s flagged=%d" % (cfgid, st, int(fl.sum())))
-    assert st["ambiguous"] < 0.2 * st["corners"]
+    # corners inside the 1e-4 m ambiguity band are exempt from the flag / sign comparison, so their share must stay
+    # what it is observed to be (0 on these samples, ~2e-5 on the config-5 rollouts): 0.5 % at most
+    print("offroad cfg%d %s: %d of %d corners in the ambiguity band" % (cfgid, mode, st["ambiguous"], st["corners"]))
+    assert st["ambiguous"] <= 0.005 * st["corners"]
     assert 0 < fl.sum() < (cfg["log"]["valid"][:, t] == 1).sum()
     wm.wm_destroy(h)
 
@@ -210,6 +213,15 @@ def test_rollout_config1_full():
 def test_rollout_config5_sample():
     st = _rollout_parity(ws.make_config(5, B=6, n_steps=80), 80, check_every=8)
     print("rollout cfg5 sample:", st)
+
+
+def test_rollout_generic_kernels_A45_against_the_oracle():
+    """A = 45 (not a multiple of 16, not 32 / 128): the fused rollout runs the plain k_rollout_dyn (no bulk staging)
+    and the generic k_rollout_metrics<0, 0, ...>, with a ragged last block of steps (13 = 8 + 5).  Compared directly
+    with the oracle, every step, not only through the stepwise graph."""
+    st = _rollout_parity(ws.make_config(5, B=3, A=45, n_steps=13), 13)
+    print("rollout A=45, 13 steps:", st)
+    assert st["corners"] > 0 and st["ambiguous"] <= 0.005 * st["corners"]
 
 
 @pytest.mark.parametrize("mode", ["fused", "stepwise"])

@@ -120,3 +120,25 @@ def test_follows_a_curved_path_and_stops_at_its_end():
     assert np.all(np.abs(np.angle(np.exp(1j * (sim["yaw"][0, 1:50, 0] - (th + np.pi / 2))))) < np.deg2rad(0.5))   # tangent heading
     # 20 s at >= 8 m/s is more than the 62.8 m of path: it ends on the last point
     assert abs(sim["x"][0, 200, 0] - pa["x"][0, 0, -1]) < 1e-5 and abs(sim["y"][0, 200, 0] - pa["y"][0, 0, -1]) < 1e-5
+
+
+def test_lead_choice_equals_the_float64_definition_outside_the_band():
+    """The oracle takes the lead decision of D39 in float32, operation for operation as the kernel does.  Pin: a
+    float64 numpy restatement of the definition (tests/defs_f64.py) picks the same lead wherever every comparison
+    behind the choice is clear by more than 1e-4 m; that is nearly everywhere on the config-5 traffic."""
+    import wm_scenarios as ws
+    from defs_f64 import idm_lead_in_double
+    cfg = ws.make_config(5, B=3, n_steps=1)
+    log = cfg["log"]
+    B, T, A = log["x"].shape
+    paths = ws.make_paths(log)
+    idm = np.ones((B, A), np.uint8); idm[:, ::6] = 0
+    n_ctl = n_dec = n_lead = 0
+    for t in (10, 33):
+        sim = {k: v.copy() for k, v in log.items()}
+        r = oracle.idm_step(sim, t, paths, idm)
+        ld, dec = idm_lead_in_double(log, t, paths, idm)
+        ctl = (idm == 1) & (log["valid"][:, t] == 1)
+        assert np.array_equal(r["lead"][dec & ctl], ld[dec & ctl])
+        n_ctl += int(ctl.sum()); n_dec += int((dec & ctl).sum()); n_lead += int(((ld >= 0) & dec & ctl).sum())
+    assert n_dec > 0.9 * n_ctl and n_lead > 50

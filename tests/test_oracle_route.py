@@ -104,3 +104,21 @@ def test_offroute_hand_cases():
     sim["valid"][0, 0, 3] = 0; on["valid"][0, 2, :] = 0
     r = oracle.offroute(sim, 0, on, off, 5.0, 1.0)
     assert r["flag"][0].tolist() == [0, 0, 0, 0, 0, 0] and r["dist_on"][0, 3] == 0 and r["dist_on"][0, 2] == 0
+
+
+def test_route_progress_equals_the_float64_definition_outside_the_band():
+    """The oracle takes the closest-point decision of D33 on the kernel's float32 key.  Pin: a float64 numpy
+    restatement of L96 / D33-D35 (tests/defs_f64.py) gives the same ratio wherever the three closest points are
+    decided by more than 1e-4 m."""
+    import wm_scenarios as ws
+    from defs_f64 import route_ratio_in_double
+    cfg = ws.make_config(5, B=3, n_steps=1)
+    log = cfg["log"]
+    paths = ws.make_paths(log)
+    paths["valid"][:, ::7, 5] = 0
+    for t in (10, 47, 90):
+        r = oracle.route_progress(log, log, t, paths)
+        rd, dec = route_ratio_in_double(log, log, t, paths)
+        chk = dec & (r["valid"] == 1)
+        assert chk.sum() > 0.8 * (r["valid"] == 1).sum()
+        assert np.all(np.abs(r["ratio"] - rd)[chk] <= 1e-6 * np.maximum(1.0, np.abs(rd[chk])))
