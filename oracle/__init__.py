@@ -51,7 +51,8 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
+        # WM_ORACLE_LIB: another build of the SAME source (tests/test_sanitizers.py loads an ASan / UBSan build)
+        _lib = C.CDLL(os.environ.get("WM_ORACLE_LIB") or build())
         _lib.orc_count_segments.restype = C.c_int32
         _lib.orc_num_threads.restype = C.c_int32
     return _lib

@@ -15,26 +15,34 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 
 
-def _stale():
-    if not os.path.exists(LIB):
+# The same sources with the HOST code under AddressSanitizer + UndefinedBehaviorSanitizer (device code is unchanged):
+# tests/test_zy_host_sanitizer.py runs the C-ABI's host logic (argument checks, graph cache key, scratch carving,
+# host staging) under it on the GPU box.  Never loaded by default.
+LIB_SAN = os.path.join(_HERE, "libwm_b200_san.so")
+SAN_FLAGS = ["-Xcompiler", "-fsanitize=address", "-Xcompiler", "-fsanitize=undefined", "-Xcompiler", "-fno-omit-frame-pointer", "-g"]   # (nvcc splits -Xcompiler arguments at commas)
+
+
+def _stale(lib=LIB):
+    if not os.path.exists(lib):
         return True
-    m = os.path.getmtime(LIB)
+    m = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > m for d in deps)
 
 
-def build(force=False, verbose=False):
+def build(force=False, verbose=False, sanitize=False):
     """Compile every kernel for sm_100a into one shared library. Returns its path."""
-    if not force and not _stale():
-        return LIB
+    lib = LIB_SAN if sanitize else LIB
+    if not force and not _stale(lib):
+        return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [nvcc] + NVCC_FLAGS + (SAN_FLAGS if sanitize else []) + ["-o", lib] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if verbose or res.returncode != 0:
         print(res.stdout)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libwm_b200.so")
-    return LIB
+        raise RuntimeError("nvcc failed building %s" % os.path.basename(lib))
+    return lib
 
 
 if __name__ == "__main__":

@@ -61,7 +61,8 @@ def load():
     """dlopen libwm_b200.so (building it first if the sources are newer). Raises if absent."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        # WM_B200_LIB: another build of the SAME sources (the host-sanitizer test loads libwm_b200_san.so)
+        path = os.environ.get("WM_B200_LIB") or _build.build()
         if not os.path.exists(path):
             raise RuntimeError("libwm_b200.so is missing: the CUDA extension must be built (no fallback)")
         _lib = C.CDLL(path)
