@@ -86,8 +86,10 @@ typedef struct {
 enum { WM_OFFROAD_CULLED = 0, WM_OFFROAD_BRUTE_FORCE = 1 };
 
 /* Both modes return bit-identical rows (same device arithmetic), both replayed as one CUDA graph (L200).
- * FUSED (default): ONE kernel launch for all n_steps, one CTA per scenario, state resident in shared
- *   memory; needs WM_OFFROAD_CULLED (with BRUTE_FORCE the stepwise graph is used).
+ * FUSED (default): TWO kernel launches for all n_steps: k_rollout_dyn_bulk (k_rollout_dyn when A is not a multiple
+ *   of 16) lays down the whole trajectory with its log divergence and ADE, one CTA per scenario; k_rollout_metrics
+ *   then computes overlap and offroad of every row, one CTA per (scenario, block of 8 steps) with those rows in
+ *   shared memory; needs WM_OFFROAD_CULLED (with BRUTE_FORCE the stepwise graph is used).
  * STEPWISE: n_steps x {k_step, k_overlap, k_offroad} + k_aggregate, the kernels of the single-step
  *   entry points. */
 enum { WM_ROLLOUT_FUSED = 0, WM_ROLLOUT_STEPWISE = 1 };
