@@ -53,25 +53,25 @@ def source_hash():
     return hsh.hexdigest()
 
 
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json.txt")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r03_traffic.json.txt")
 
 
 def profiled_traffic(kernel):
-    """dram__bytes_read + write per launch of `kernel` from the committed ncu pass (profiles/r02_traffic.json.txt,
+    """dram__bytes_read + write per launch of `kernel` from the committed ncu pass (profiles/r03_traffic.json.txt,
     written by `bench.py --write-traffic <ncu csv>`).  A number taken from other sources than the ones
     that are being timed is not reported: (None, why)."""
     try:
         d = json.load(open(TRAFFIC_FILE))
     except Exception:
-        return None, "no profiles/r02_traffic.json.txt"
+        return None, "no profiles/r03_traffic.json.txt"
     if d.get("source_sha256") != source_hash():
-        return None, "profiles/r02_traffic.json.txt was taken from other kernel sources (sha256 differs): re-run the ncu pass"
+        return None, "profiles/r03_traffic.json.txt was taken from other kernel sources (sha256 differs): re-run the ncu pass"
     v = d.get("kernels", {}).get(kernel)
-    return (float(v), "profiles/r02_traffic.json.txt (%s)" % d.get("command", "ncu")) if v is not None else (None, "kernel not in profiles/r02_traffic.json.txt")
+    return (float(v), "profiles/r03_traffic.json.txt (%s)" % d.get("command", "ncu")) if v is not None else (None, "kernel not in profiles/r03_traffic.json.txt")
 
 
 def write_traffic(csv_path):
-    """Parse `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum --csv` output into profiles/r02_traffic.json.txt."""
+    """Parse `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum --csv` output into profiles/r03_traffic.json.txt."""
     import csv
     rows = list(csv.reader(open(csv_path)))
     i = [k for k, r in enumerate(rows) if r and r[0] == "ID"][0]
@@ -630,7 +630,7 @@ def main():
                          "SURVEY 8(a) rows on configs 3, 2, 4 (supplementary lines, same JSON shape)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (single-step grid kernel, brute-force kernel, other configs)")
-    ap.add_argument("--write-traffic", default=None, metavar="NCU_CSV", help="parse an ncu dram__bytes csv into profiles/r02_traffic.json.txt and exit")
+    ap.add_argument("--write-traffic", default=None, metavar="NCU_CSV", help="parse an ncu dram__bytes csv into profiles/r03_traffic.json.txt and exit")
     args = ap.parse_args()
     if args.write_traffic:
         return write_traffic(args.write_traffic)
@@ -792,7 +792,7 @@ def main():
                 "kernels": {
                     "k_rollout_metrics": {"ms": met_ms, "share_of_step": met_ms / ms_step, "algorithmic_bytes_per_launch": met_bytes,
                                           "hbm_frac": met_bytes / (met_ms * 1e-3) / 1e9 / hbm_peak, "traffic": tr_met,
-                                          "bound_observed": "instruction issue (ncu: profiles/r02_k_rollout_ncu.md), not HBM and not the FP32 pipe",
+                                          "bound_observed": "instruction issue 77.5 % and LSU data-pipe wavefronts 71.5 % (ncu: profiles/r03_k_rollout_ncu.md), not HBM and not the FP32 pipe",
                                           "alu_frac_on_evaluated_pairs": fused_flops / (met_ms * 1e-3) / 1e12 / fp32_peak},
                     "k_rollout_dyn": {"ms": dyn_ms, "share_of_step": dyn_ms / ms_step, "algorithmic_bytes_per_launch": dyn_bytes,
                                       "hbm_frac": dyn_bytes / (dyn_ms * 1e-3) / 1e9 / hbm_peak, "traffic": tr_dyn}},
